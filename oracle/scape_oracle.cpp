@@ -1,0 +1,203 @@
+// ORACLE — TEST INFRASTRUCTURE ONLY.
+//
+// Plain, slow, single-threaded CPU restatement of Algorithm 1 of SCAPE
+// (arXiv 2607.01678) for ONE rank's partition with R simulated
+// data-parallel replicas.  It exists so that tests can check the CUDA path against
+// something a reader can compare with the paper by eye.  Only tests/,
+// __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+// load it.  It shares no code with paper_2607_01678_b200/ (the product) and the
+// product never calls it.
+//
+// Parity pins (tests/test_oracle_pins.py, all `-m "not gpu"`):
+//   P1 top-k vs brute-force rank count      P2 packed + residual == m-tilde (bitwise)
+//   P3 sparsity 0 == dense AdamS (Eq. 2)    P4 Eq. 3 reconstruction identity
+//   P5 Eq. 4-6 off-mask behaviour           P6 telescoped error feedback (nothing lost)
+//   P7 one-step mask delay                  P8 R = 1
+//   P9 worked example tests/golden/p9_worked_example.json
+// Unpinned by the paper (decisions): S3 clip_grad omitted,
+// S4 no bias correction, S8 replica 0 owns the statistic, S9 flat (not per-layer) top-k.
+//
+// The algorithm is instantiated twice from the same template: T = float is the graded
+// arithmetic (operation order pinned below);
+// T = double exists only for the exact-arithmetic pins P3, P4, P6.
+//
+// Build: g++ -O2 -std=c++17 -ffp-contract=off -shared -fPIC   (see oracle/build.py)
+// -ffp-contract=off matters: every rounding below is written out, the compiler must not
+// fuse a*b+c on its own.
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <numeric>
+#include <vector>
+
+namespace {
+
+// Sort key of the selection statistic abs(m-tilde) (Alg. 1 l.11; §IV-B,
+// PAPER.md:182).  For finite IEEE numbers the unsigned bit pattern of |x| orders exactly
+// like |x|; -0 and +0 get the same key.
+template <class T> struct KeyOf;
+template <> struct KeyOf<float> {
+  using U = uint32_t;
+  static U key(float x) { float a = std::fabs(x); U u; std::memcpy(&u, &a, sizeof u); return u; }
+};
+template <> struct KeyOf<double> {
+  using U = uint64_t;
+  static U key(double x) { double a = std::fabs(x); U u; std::memcpy(&u, &a, sizeof u); return u; }
+};
+
+template <class T>
+struct Oracle {
+  using U = typename KeyOf<T>::U;
+
+  int64_t N = 0;
+  int R = 0;
+  int64_t k = 0;      // number selected per refresh: k = N - floor(sparsity * N)  (reading S6)
+  int64_t t = 0;      // steps taken
+  T beta1, beta2, eps, lr, wd;
+  T c1, c2;           // 1 - beta1, 1 - beta2, evaluated in T
+
+  std::vector<T> m;                 // m_{t-1}, zero off the previous mask (Eq. 4)
+  std::vector<std::vector<T>> e;    // e^r_{t-1}, one residual per replica (Alg. 1 l.2, :141)
+  std::vector<uint8_t> cur;         // M_{t-1}, the mask used by the coming step (l.1: all ones)
+
+  // What the last step produced (kept for inspection by tests).
+  std::vector<int32_t> idx;             // ascending indices of the mask the step used
+  std::vector<std::vector<T>> mt;       // m-tilde^r, all N entries (l.6)
+  std::vector<std::vector<T>> b;        // packed payload b^r[j] = m-tilde^r[idx[j]] (l.9)
+  std::vector<T> bbar;                  // mean payload (l.10)
+  std::vector<T> ghat, v, u;            // l.13, l.15, l.16 on the mask, by position j
+
+  Oracle(int64_t N_, int R_, double sparsity, double b1, double b2, double eps_, double lr_, double wd_)
+      : N(N_), R(R_) {
+    // Hyper-parameters are cast to T once; 1 - beta is evaluated in T.
+    beta1 = (T)b1; beta2 = (T)b2; eps = (T)eps_; lr = (T)lr_; wd = (T)wd_;
+    c1 = (T)1 - beta1;
+    c2 = (T)1 - beta2;
+    // Reading S6: k = N - floor(s*N) in IEEE double.
+    k = N - (int64_t)std::floor(sparsity * (double)N);
+    m.assign(N, (T)0);                                   // reading S5: m_0 = 0
+    e.assign(R, std::vector<T>(N, (T)0));                // l.2: e_0 = 0
+    cur.assign(N, 1);                                    // l.1: M_0 = 1
+  }
+
+  // refresh_mask (l.11): the k entries with the largest key; ties to the lower index (S7).
+  // Written as the definition: stable sort of all indices by key, descending; take k.
+  static std::vector<uint8_t> topk_mask(const T* x, int64_t n, int64_t kk) {
+    std::vector<int64_t> order(n);
+    std::iota(order.begin(), order.end(), (int64_t)0);
+    std::stable_sort(order.begin(), order.end(), [&](int64_t a, int64_t c) {
+      return KeyOf<T>::key(x[a]) > KeyOf<T>::key(x[c]);
+    });
+    std::vector<uint8_t> mask(n, 0);
+    for (int64_t j = 0; j < kk; ++j) mask[order[j]] = 1;
+    return mask;
+  }
+
+  void step(T* theta, const T* const* g) {
+    t += 1;                                              // l.3
+    // Indices of M_{t-1}, ascending.
+    idx.clear();
+    for (int64_t i = 0; i < N; ++i) if (cur[i]) idx.push_back((int32_t)i);
+    const int64_t K = (int64_t)idx.size();
+
+    // l.6: m-tilde^r = beta1 m_{t-1} + (1 - beta1) g^r + e^r_{t-1}
+    mt.assign(R, std::vector<T>(N));
+    for (int r = 0; r < R; ++r)
+      for (int64_t i = 0; i < N; ++i) {
+        T p = beta1 * m[i];
+        mt[r][i] = std::fma(c1, g[r][i], p) + e[r][i];
+      }
+
+    // l.4 + l.9: b^r <- 0; b^r[M_{t-1}] <- m-tilde^r[M_{t-1}]  (stored packed, by position j)
+    b.assign(R, std::vector<T>(K));
+    for (int r = 0; r < R; ++r)
+      for (int64_t j = 0; j < K; ++j) b[r][j] = mt[r][idx[j]];
+
+    // l.7-8: e^r[not M_{t-1}] <- m-tilde^r ; e^r[M_{t-1}] <- 0
+    for (int r = 0; r < R; ++r)
+      for (int64_t i = 0; i < N; ++i) e[r][i] = cur[i] ? (T)0 : mt[r][i];
+
+    // l.11: M_t <- refresh_mask(density, abs(m-tilde)) from the owner's (replica 0) statistic,
+    // over all N positions (readings S8, S11).  Used from the next step on (§IV-A, :178).
+    std::vector<uint8_t> next = topk_mask(mt[0].data(), N, k);
+
+    // l.10, l.12-17 on the mask.
+    std::vector<T> m_new(N, (T)0);                       // l.12 / Eq. 4: zero off the mask
+    bbar.assign(K, (T)0); ghat.assign(K, (T)0); v.assign(K, (T)0); u.assign(K, (T)0);
+    for (int64_t j = 0; j < K; ++j) {
+      const int64_t i = idx[j];
+      T s = b[0][j];                                     // l.10: sum over replicas, r ascending
+      for (int r = 1; r < R; ++r) s = s + b[r][j];
+      T bb = s / (T)R;
+      T p = beta1 * m[i];
+      T gh = (bb - p) / c1;                              // l.13 (Eq. 3, :188)
+      T vv = std::fma(c2, gh * gh, beta2 * (m[i] * m[i]));   // l.15
+      T uu = bb / (std::sqrt(vv) + eps);                 // l.16 with m_t = bbar (l.12)
+      T w = std::fma(wd, theta[i], uu);                  // l.17
+      theta[i] = std::fma(-lr, w, theta[i]);
+      m_new[i] = bb;                                     // l.12
+      bbar[j] = bb; ghat[j] = gh; v[j] = vv; u[j] = uu;
+    }
+    // Off the mask: u = 0 (Eq. 5, :202), so l.17 is pure weight decay (Eq. 6, :207-211).
+    for (int64_t i = 0; i < N; ++i) {
+      if (cur[i]) continue;
+      T uu = (T)0;
+      T w = std::fma(wd, theta[i], uu);
+      theta[i] = std::fma(-lr, w, theta[i]);
+    }
+    m.swap(m_new);
+    cur.swap(next);                                      // the delay: M_t is used at step t+1
+  }
+};
+
+template <class T> void copy_out(const std::vector<T>& v, T* dst) {
+  if (!v.empty()) std::memcpy(dst, v.data(), v.size() * sizeof(T));
+}
+
+}  // namespace
+
+#define ORACLE_API(SUF, T)                                                                          \
+  extern "C" void* oracle_create_##SUF(int64_t N, int R, double sparsity, double b1, double b2,     \
+                                       double eps, double lr, double wd) {                          \
+    if (N <= 0 || N >= (int64_t)1 << 31 || R < 1 || !(sparsity >= 0.0 && sparsity < 1.0))           \
+      return nullptr;                                                                               \
+    return new Oracle<T>(N, R, sparsity, b1, b2, eps, lr, wd);                                      \
+  }                                                                                                 \
+  extern "C" void oracle_destroy_##SUF(void* h) { delete (Oracle<T>*)h; }                           \
+  extern "C" void oracle_step_##SUF(void* h, T* theta, const T* const* grads) {                     \
+    ((Oracle<T>*)h)->step(theta, grads);                                                            \
+  }                                                                                                 \
+  extern "C" int64_t oracle_k_##SUF(void* h) { return ((Oracle<T>*)h)->k; }                         \
+  extern "C" int64_t oracle_t_##SUF(void* h) { return ((Oracle<T>*)h)->t; }                         \
+  extern "C" int64_t oracle_K_last_##SUF(void* h) { return (int64_t)((Oracle<T>*)h)->idx.size(); }  \
+  extern "C" void oracle_get_m_##SUF(void* h, T* dst) { copy_out(((Oracle<T>*)h)->m, dst); }        \
+  extern "C" void oracle_set_m_##SUF(void* h, const T* src) {                                       \
+    auto* o = (Oracle<T>*)h; std::memcpy(o->m.data(), src, o->N * sizeof(T));                       \
+  }                                                                                                 \
+  extern "C" void oracle_get_e_##SUF(void* h, int r, T* dst) { copy_out(((Oracle<T>*)h)->e[r], dst); } \
+  extern "C" void oracle_set_e_##SUF(void* h, int r, const T* src) {                                \
+    auto* o = (Oracle<T>*)h; std::memcpy(o->e[r].data(), src, o->N * sizeof(T));                    \
+  }                                                                                                 \
+  extern "C" void oracle_get_mask_##SUF(void* h, uint8_t* dst) {                                    \
+    copy_out(((Oracle<T>*)h)->cur, dst);                                                            \
+  }                                                                                                 \
+  extern "C" void oracle_set_mask_##SUF(void* h, const uint8_t* src) {                              \
+    auto* o = (Oracle<T>*)h; std::memcpy(o->cur.data(), src, o->N);                                 \
+  }                                                                                                 \
+  extern "C" void oracle_set_t_##SUF(void* h, int64_t t) { ((Oracle<T>*)h)->t = t; }                \
+  extern "C" void oracle_get_idx_##SUF(void* h, int32_t* dst) { copy_out(((Oracle<T>*)h)->idx, dst); } \
+  extern "C" void oracle_get_mt_##SUF(void* h, int r, T* dst) { copy_out(((Oracle<T>*)h)->mt[r], dst); } \
+  extern "C" void oracle_get_b_##SUF(void* h, int r, T* dst) { copy_out(((Oracle<T>*)h)->b[r], dst); } \
+  extern "C" void oracle_get_bbar_##SUF(void* h, T* dst) { copy_out(((Oracle<T>*)h)->bbar, dst); }  \
+  extern "C" void oracle_get_ghat_##SUF(void* h, T* dst) { copy_out(((Oracle<T>*)h)->ghat, dst); }  \
+  extern "C" void oracle_get_v_##SUF(void* h, T* dst) { copy_out(((Oracle<T>*)h)->v, dst); }        \
+  extern "C" void oracle_get_u_##SUF(void* h, T* dst) { copy_out(((Oracle<T>*)h)->u, dst); }        \
+  extern "C" void oracle_topk_##SUF(const T* x, int64_t n, int64_t kk, uint8_t* mask) {             \
+    auto mk = Oracle<T>::topk_mask(x, n, kk); std::memcpy(mask, mk.data(), (size_t)n);              \
+  }
+
+ORACLE_API(f32, float)
+ORACLE_API(f64, double)

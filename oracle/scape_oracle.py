@@ -1,0 +1,155 @@
+"""ctypes binding of the CPU oracle (TEST INFRASTRUCTURE ONLY — see scape_oracle.cpp).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+import this module.  It imports nothing from paper_2607_01678_b200.
+"""
+import ctypes
+
+import numpy as np
+
+from . import build as _build
+
+_LIB = None
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        _LIB = ctypes.CDLL(_build.build())
+    return _LIB
+
+
+class ScapeOracle:
+    """One rank's partition of Algorithm 1 with R simulated replicas.
+
+    dtype np.float32 is the graded arithmetic; np.float64 is the same source instantiated in
+    double for the exact-arithmetic pins.
+    """
+
+    def __init__(self, shard_numel, R, sparsity, beta1, beta2, eps, lr, wd, dtype=np.float32):
+        self.dtype = np.dtype(dtype)
+        self.suf = {"float32": "f32", "float64": "f64"}[self.dtype.name]
+        self.N, self.R = int(shard_numel), int(R)
+        L = _lib()
+        self._f = lambda name: getattr(L, f"oracle_{name}_{self.suf}")
+        cr = self._f("create")
+        cr.restype = ctypes.c_void_p
+        cr.argtypes = [ctypes.c_int64, ctypes.c_int] + [ctypes.c_double] * 6
+        self.h = cr(self.N, self.R, sparsity, beta1, beta2, eps, lr, wd)
+        if not self.h:
+            raise ValueError("oracle_create rejected the arguments")
+        for name in ("k", "t", "K_last"):
+            fn = self._f(name)
+            fn.restype = ctypes.c_int64
+            fn.argtypes = [ctypes.c_void_p]
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            d = self._f("destroy")
+            d.argtypes = [ctypes.c_void_p]
+            d(self.h)
+            self.h = None
+
+    # ---- scalars -------------------------------------------------------------------
+    @property
+    def k(self):
+        return int(self._f("k")(self.h))
+
+    @property
+    def t(self):
+        return int(self._f("t")(self.h))
+
+    @property
+    def K_last(self):
+        return int(self._f("K_last")(self.h))
+
+    def set_t(self, t):
+        fn = self._f("set_t")
+        fn.argtypes = [ctypes.c_void_p, ctypes.c_int64]
+        fn(self.h, int(t))
+
+    # ---- the step ------------------------------------------------------------------
+    def step(self, theta, grads):
+        """theta: contiguous array [N] of self.dtype, updated in place. grads: R arrays [N]."""
+        assert theta.dtype == self.dtype and theta.flags.c_contiguous and theta.size == self.N
+        gs = [np.ascontiguousarray(g, dtype=self.dtype) for g in grads]
+        assert len(gs) == self.R and all(g.size == self.N for g in gs)
+        arr = (ctypes.c_void_p * self.R)(*[g.ctypes.data for g in gs])
+        fn = self._f("step")
+        fn.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        fn(self.h, theta.ctypes.data, arr)
+
+    # ---- state / last-step outputs ---------------------------------------------------
+    def _get(self, name, n, dtype=None, r=None):
+        out = np.empty(n, dtype=dtype or self.dtype)
+        fn = self._f("get_" + name)
+        if r is None:
+            fn.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+            fn(self.h, out.ctypes.data)
+        else:
+            fn.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]
+            fn(self.h, int(r), out.ctypes.data)
+        return out
+
+    def _set(self, name, arr, dtype=None, r=None):
+        a = np.ascontiguousarray(arr, dtype=dtype or self.dtype)
+        assert a.size == self.N
+        fn = self._f("set_" + name)
+        if r is None:
+            fn.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+            fn(self.h, a.ctypes.data)
+        else:
+            fn.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]
+            fn(self.h, int(r), a.ctypes.data)
+
+    def m(self):
+        return self._get("m", self.N)
+
+    def set_m(self, a):
+        self._set("m", a)
+
+    def e(self, r):
+        return self._get("e", self.N, r=r)
+
+    def set_e(self, r, a):
+        self._set("e", a, r=r)
+
+    def mask(self):
+        """The mask the NEXT step will use (M_t after step t), as uint8 [N]."""
+        return self._get("mask", self.N, dtype=np.uint8)
+
+    def set_mask(self, a):
+        self._set("mask", a, dtype=np.uint8)
+
+    def idx(self):
+        """Ascending indices of the mask the LAST step used."""
+        return self._get("idx", self.K_last, dtype=np.int32)
+
+    def mt(self, r):
+        return self._get("mt", self.N, r=r)
+
+    def b(self, r):
+        return self._get("b", self.K_last, r=r)
+
+    def bbar(self):
+        return self._get("bbar", self.K_last)
+
+    def ghat(self):
+        return self._get("ghat", self.K_last)
+
+    def v(self):
+        return self._get("v", self.K_last)
+
+    def u(self):
+        return self._get("u", self.K_last)
+
+
+def topk_mask(x, k):
+    """refresh_mask on its own: uint8 mask of the k largest |x|, ties to the lower index."""
+    x = np.ascontiguousarray(x)
+    suf = {"float32": "f32", "float64": "f64"}[x.dtype.name]
+    fn = getattr(_lib(), f"oracle_topk_{suf}")
+    fn.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p]
+    out = np.zeros(x.size, dtype=np.uint8)
+    fn(x.ctypes.data, x.size, int(k), out.ctypes.data)
+    return out

@@ -1,0 +1,340 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (CPU only).
+
+Each test names the pin (P1..P9, SURVEY.md §8(c)-5 / DESIGN.md §Oracle pins) and the passage of
+PAPER.md it rests on.  None of the expected values comes from oracle/ or from the CUDA path:
+they are brute force, closed forms, invariants, independent numpy restatements of Eq. 2, or
+the hand-derived golden fixture.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from oracle.scape_oracle import ScapeOracle, topk_mask
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+HYP = dict(beta1=0.9, beta2=0.95, eps=1e-8, lr=1e-3, wd=0.1)
+
+
+def make_grads(rng, N, R, T, dtype=np.float32, rho=0.9):
+    """AR(1) signal + per-replica noise, as in BASELINE.json config 1."""
+    out, a = [], None
+    for _ in range(T):
+        xi = rng.standard_normal(N)
+        a = xi if a is None else rho * a + np.sqrt(1 - rho * rho) * xi
+        out.append([(1e-3 * (a + rng.standard_normal(N))).astype(dtype) for _ in range(R)])
+    return out
+
+
+def ulp32(x):
+    return np.spacing(np.abs(np.asarray(x, dtype=np.float32)))
+
+
+# ------------------------------------------------------------------------------------ P1
+def brute_force_topk(x, k):
+    """Definition (reading S7): rank_i = #{j : |x_j| > |x_i| or (|x_j| == |x_i| and j < i)};
+    selected iff rank_i < k.  O(n^2), written without any sort."""
+    a = np.abs(x)
+    n = len(x)
+    mask = np.zeros(n, dtype=np.uint8)
+    for i in range(n):
+        rank = 0
+        for j in range(n):
+            if a[j] > a[i] or (a[j] == a[i] and j < i):
+                rank += 1
+        mask[i] = 1 if rank < k else 0
+    return mask
+
+
+CRAFTED = {
+    "all_equal": np.full(17, 0.25, np.float32),
+    "pm_pairs": np.array([1, -1, 2, -2, 3, -3, 0.5, -0.5], np.float32),
+    "zeros": np.zeros(9, np.float32),
+    "signed_zeros": np.array([0.0, -0.0, 0.0, -0.0, 1.0], np.float32),
+    "dups_straddle": np.array([5, 3, 3, 3, 3, 1, 3, 0, 3], np.float32),
+    "denormals": np.array([1e-45, -3e-45, 2e-45, 0, 1e-38, -1e-45], np.float32),
+    "descending": np.arange(20, 0, -1).astype(np.float32),
+    "ascending": np.arange(1, 21).astype(np.float32),
+}
+
+
+@pytest.mark.parametrize("name", sorted(CRAFTED))
+def test_p1_topk_crafted_vs_brute_force(name):
+    x = CRAFTED[name]
+    for k in range(1, len(x) + 1):
+        got = topk_mask(x, k)
+        assert got.sum() == k
+        np.testing.assert_array_equal(got, brute_force_topk(x, k), err_msg=f"{name} k={k}")
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_p1_topk_random_vs_brute_force(seed):
+    rng = np.random.default_rng(seed)
+    n = int(rng.integers(2, 65))
+    # few distinct magnitudes -> many ties
+    x = (rng.integers(-4, 5, n) * 0.125).astype(np.float32)
+    y = rng.standard_normal(n).astype(np.float32)
+    for v in (x, y, y.astype(np.float64)):
+        for k in {1, max(1, n // 10), n // 2 + 1, n}:
+            np.testing.assert_array_equal(topk_mask(v, k), brute_force_topk(v, k))
+
+
+def test_exactly_k_selected_and_k_rule():
+    # Reading S6: k = N - floor(s N) in IEEE double.
+    for N, s in [(1 << 20, 0.9), (1000, 0.99), (1000, 0.999), (7, 0.5), (354501632 // 1000, 0.99)]:
+        o = ScapeOracle(N, 1, s, **HYP)
+        assert o.k == N - int(np.floor(s * N))
+    o = ScapeOracle(1 << 20, 2, 0.9, **HYP)
+    assert o.k == 104858
+    rng = np.random.default_rng(1)
+    N, R = 4096, 2
+    o = ScapeOracle(N, R, 0.9, **HYP)
+    th = rng.standard_normal(N).astype(np.float32)
+    for g in make_grads(rng, N, R, 4):
+        o.step(th, g)
+        mk = o.mask()
+        assert mk.sum() == o.k
+        idx = np.nonzero(mk)[0]
+        assert np.all(np.diff(idx) > 0) and idx[-1] < N
+
+
+def test_create_rejects_bad_arguments():
+    for bad in [dict(N=0), dict(N=1 << 31), dict(R=0), dict(s=1.0), dict(s=-0.1), dict(s=float("nan"))]:
+        args = dict(N=16, R=1, s=0.5)
+        args.update(bad)
+        with pytest.raises(ValueError):
+            ScapeOracle(args["N"], args["R"], args["s"], **HYP)
+
+
+# ------------------------------------------------------------------------------------ P2
+def test_p2_packed_plus_residual_is_mtilde_bitwise():
+    """'packed values plus residual equal the pre-mask quantity' (Alg. 1 l.7-9)."""
+    rng = np.random.default_rng(2)
+    N, R = 5000, 3
+    o = ScapeOracle(N, R, 0.9, **HYP)
+    th = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    for g in make_grads(rng, N, R, 5):
+        o.step(th, g)
+        idx = o.idx()
+        on = np.zeros(N, bool)
+        on[idx] = True
+        for r in range(R):
+            scat = np.zeros(N, np.float32)
+            scat[idx] = o.b(r)
+            e, mt = o.e(r), o.mt(r)
+            # one of the two terms is exactly zero at every position
+            assert np.all(e[on] == 0) and np.all(scat[~on] == 0)
+            total = scat + e
+            assert np.array_equal(total.view(np.uint32) & 0x7FFFFFFF, mt.view(np.uint32) & 0x7FFFFFFF)
+            nz = mt != 0
+            assert np.array_equal(total.view(np.uint32)[nz], mt.view(np.uint32)[nz])
+
+
+# ------------------------------------------------------------------------------------ P3
+def dense_adams_f64(theta, m, gbar, beta1, beta2, eps, lr, wd):
+    """Eq. 2, written independently of the oracle, no bias correction (S4)."""
+    m_new = beta1 * m + (1 - beta1) * gbar
+    v = beta2 * m * m + (1 - beta2) * gbar * gbar
+    theta_new = theta - lr * (m_new / (np.sqrt(v) + eps) + wd * theta)
+    return theta_new, m_new
+
+
+def test_p3_sparsity_zero_is_dense_adams_double():
+    rng = np.random.default_rng(3)
+    N, R, T = 3000, 4, 6
+    o = ScapeOracle(N, R, 0.0, dtype=np.float64, **HYP)
+    assert o.k == N
+    th = 0.02 * rng.standard_normal(N)
+    th_ref, m_ref = th.copy(), np.zeros(N)
+    for g in make_grads(rng, N, R, T, dtype=np.float64):
+        o.step(th, g)
+        gbar = sum(g) / R
+        th_ref, m_ref = dense_adams_f64(th_ref, m_ref, gbar, **HYP)
+        assert o.K_last == N and o.mask().all()
+        for r in range(R):
+            assert not o.e(r).any()
+        np.testing.assert_allclose(o.m(), m_ref, rtol=1e-12, atol=1e-300)
+        np.testing.assert_allclose(th, th_ref, rtol=1e-12, atol=1e-300)
+
+
+def test_p3_sparsity_zero_is_dense_adams_fp32_loose():
+    """fp32: l.13 re-derives g-bar through a cancellation, so not bitwise; 1e-5 on theta."""
+    rng = np.random.default_rng(4)
+    N, R, T = 3000, 2, 6
+    o = ScapeOracle(N, R, 0.0, **HYP)
+    th = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    th_ref, m_ref = th.astype(np.float64), np.zeros(N)
+    for g in make_grads(rng, N, R, T):
+        o.step(th, g)
+        gbar = sum(x.astype(np.float64) for x in g) / R
+        th_ref, m_ref = dense_adams_f64(th_ref, m_ref, gbar, **HYP)
+    np.testing.assert_allclose(th, th_ref, rtol=1e-5, atol=1e-9)
+    np.testing.assert_allclose(o.m(), m_ref, rtol=1e-5, atol=1e-9)   # |m| ~ 1e-3; near-zero entries cancel
+
+
+# ------------------------------------------------------------------------------------ P4
+def test_p4_eq3_reconstruction_identity_double():
+    """Eq. 3 with l.6: (b-bar - beta1 m)/(1-beta1) = g-bar + e-bar/(1-beta1) (S2)."""
+    rng = np.random.default_rng(5)
+    N, R, T = 2000, 3, 6
+    o = ScapeOracle(N, R, 0.9, dtype=np.float64, **HYP)
+    th = 0.02 * rng.standard_normal(N)
+    for g in make_grads(rng, N, R, T, dtype=np.float64):
+        e_prev = [o.e(r) for r in range(R)]
+        o.step(th, g)
+        idx = o.idx()
+        gbar = sum(g) / R
+        ebar = sum(e_prev) / R
+        want = gbar[idx] + ebar[idx] / (1 - HYP["beta1"])
+        np.testing.assert_allclose(o.ghat(), want, rtol=1e-9, atol=1e-15)
+    assert o.K_last == o.k      # after step 1 the mask has k entries
+
+
+# ------------------------------------------------------------------------------------ P5
+def test_p5_off_mask_eq4_5_6():
+    rng = np.random.default_rng(6)
+    N, R, T = 4000, 2, 8
+    o = ScapeOracle(N, R, 0.99, **HYP)
+    th = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    th0 = th.copy()
+    ever = np.zeros(N, bool)
+    decay = np.float32(1.0) - np.float32(HYP["lr"]) * np.float32(HYP["wd"])
+    for g in make_grads(rng, N, R, T):
+        before = th.copy()
+        o.step(th, g)
+        on = np.zeros(N, bool)
+        on[o.idx()] = True
+        ever |= on
+        assert not o.m()[~on].any()                                   # Eq. 4
+        want = before[~on] * decay                                   # Eq. 6
+        assert np.all(np.abs(th[~on] - want) <= 2 * ulp32(want))     # l.17 form vs Eq. 6: <= ~1 ulp
+    # the first step is dense (M_0 = 1), so "never selected" is judged from step 2 on
+    o2 = ScapeOracle(N, R, 0.99, **HYP)
+    th = th0.copy()
+    gs = make_grads(np.random.default_rng(7), N, R, T)
+    o2.step(th, gs[0])
+    th1 = th.copy()
+    never = np.ones(N, bool)
+    for g in gs[1:]:
+        o2.step(th, g)
+        never[o2.idx()] = False
+    want = th1[never].astype(np.float64) * (1 - HYP["lr"] * HYP["wd"]) ** (T - 1)
+    assert never.sum() > N // 2
+    assert np.all(np.abs(th[never] - want) <= (T + 1) * ulp32(want))
+
+
+# ------------------------------------------------------------------------------------ P6
+def test_p6_telescoped_error_feedback_double():
+    """(1-b1) sum_{t<=T} gbar_t = ebar_T + m_T + (1-b1) sum_{t<T} m_t  (DESIGN.md §Oracle pins)."""
+    rng = np.random.default_rng(8)
+    N, R, T = 1500, 3, 12
+    o = ScapeOracle(N, R, 0.95, dtype=np.float64, **HYP)
+    th = 0.02 * rng.standard_normal(N)
+    c1 = 1 - HYP["beta1"]
+    sum_g, sum_m_before = np.zeros(N), np.zeros(N)
+    for g in make_grads(rng, N, R, T, dtype=np.float64):
+        sum_m_before += o.m()          # adds m_{t-1}; m_0 = 0
+        o.step(th, g)
+        sum_g += sum(g) / R
+        ebar = sum(o.e(r) for r in range(R)) / R
+        lhs = c1 * sum_g
+        rhs = ebar + o.m() + c1 * sum_m_before
+        np.testing.assert_allclose(lhs, rhs, rtol=1e-10, atol=1e-14)
+
+
+# ------------------------------------------------------------------------------------ P7
+def test_p7_mask_is_used_one_step_late():
+    rng = np.random.default_rng(9)
+    N, R = 2048, 2
+    o = ScapeOracle(N, R, 0.9, **HYP)
+    th = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    prev_next = None
+    for t, g in enumerate(make_grads(rng, N, R, 5), 1):
+        o.step(th, g)
+        if t == 1:
+            np.testing.assert_array_equal(o.idx(), np.arange(N, dtype=np.int32))   # M_0 = 1
+        else:
+            np.testing.assert_array_equal(o.idx(), np.nonzero(prev_next)[0].astype(np.int32))
+        # the refreshed mask is the top-k of THIS step's |m-tilde^0| over all positions (l.11)
+        np.testing.assert_array_equal(o.mask(), brute_force_topk_fast(o.mt(0), o.k))
+        prev_next = o.mask()
+
+
+def brute_force_topk_fast(x, k):
+    """Same definition as brute_force_topk, via lexsort on (index, -|x|) — still independent of
+    the oracle's stable_sort; used where n is too large for the O(n^2) loop."""
+    order = np.lexsort((np.arange(len(x)), -np.abs(x.astype(np.float64))))
+    mask = np.zeros(len(x), np.uint8)
+    mask[order[:k]] = 1
+    return mask
+
+
+def test_brute_force_variants_agree():
+    rng = np.random.default_rng(10)
+    x = (rng.integers(-3, 4, 50) * 0.5).astype(np.float32)
+    for k in (1, 7, 25, 50):
+        np.testing.assert_array_equal(brute_force_topk(x, k), brute_force_topk_fast(x, k))
+
+
+# ------------------------------------------------------------------------------------ P8
+def test_p8_single_replica():
+    rng = np.random.default_rng(11)
+    N = 3000
+    o = ScapeOracle(N, 1, 0.9, **HYP)
+    od = ScapeOracle(N, 1, 0.9, dtype=np.float64, **HYP)
+    th = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    thd = th.astype(np.float64)
+    for g in make_grads(rng, N, 1, 5):
+        e_prev = od.e(0)
+        o.step(th, g)
+        od.step(thd, [g[0].astype(np.float64)])
+        assert np.array_equal(o.bbar().view(np.uint32), o.b(0).view(np.uint32))   # b-bar = b^0 bitwise
+        idx = od.idx()
+        want = g[0].astype(np.float64)[idx] + e_prev[idx] / (1 - HYP["beta1"])
+        np.testing.assert_allclose(od.ghat(), want, rtol=1e-9, atol=1e-15)
+
+
+# ------------------------------------------------------------------------------------ P9
+def test_p9_worked_example_golden():
+    with open(os.path.join(HERE, "golden", "p9_worked_example.json")) as f:
+        G = json.load(f)
+    o = ScapeOracle(G["N"], G["R"], G["sparsity"], G["beta1"], G["beta2"], G["eps"], G["lr"], G["wd"])
+    assert o.k == G["k"]
+    th = np.array(G["theta0"], np.float32)
+    sc = np.float32(G["grad_scale"])
+    for s in G["steps"]:
+        g = [np.array(s["g0"], np.float32) * sc, np.array(s["g1"], np.float32) * sc]
+        o.step(th, g)
+        np.testing.assert_array_equal(o.idx(), np.array(s["cur"], np.int32))
+        np.testing.assert_array_equal(np.nonzero(o.mask())[0], np.array(s["next"]))
+        # exact (dyadic) quantities
+        for r, key in ((0, "mt0"), (1, "mt1")):
+            np.testing.assert_array_equal(o.mt(r), np.array(s[key], np.float32))
+        for r, key in ((0, "b0"), (1, "b1")):
+            np.testing.assert_array_equal(o.b(r), np.array(s[key], np.float32))
+        for r, key in ((0, "e0_after"), (1, "e1_after")):
+            np.testing.assert_array_equal(o.e(r), np.array(s[key], np.float32))
+        np.testing.assert_array_equal(o.m(), np.array(s["m_after"], np.float32))
+        K = len(s["cur"])
+        take = (lambda a: np.array(a, np.float32)[np.array(s["cur"])]) if len(s["ghat"]) == G["N"] and K == G["N"] \
+            else (lambda a: np.array(a, np.float32))
+        np.testing.assert_array_equal(o.ghat(), take(s["ghat"]))
+        np.testing.assert_array_equal(o.v(), take(s["v"]))
+        # non-dyadic
+        np.testing.assert_allclose(o.u(), take(s["u"]), rtol=1e-6, atol=0)
+        np.testing.assert_allclose(th, np.array(s["theta_after"], np.float32), rtol=1e-6, atol=0)
+
+
+# ------------------------------------------------------------------------- f32 vs f64 sanity
+def test_f32_and_f64_instantiations_track_each_other():
+    rng = np.random.default_rng(12)
+    N, R = 2000, 2
+    o32 = ScapeOracle(N, R, 0.9, **HYP)
+    o64 = ScapeOracle(N, R, 0.9, dtype=np.float64, **HYP)
+    th32 = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    th64 = th32.astype(np.float64)
+    for g in make_grads(rng, N, R, 3):
+        o32.step(th32, g)
+        o64.step(th64, [x.astype(np.float64) for x in g])
+    np.testing.assert_allclose(th32, th64, rtol=2e-4, atol=1e-7)
