@@ -1,0 +1,128 @@
+/* scape.h — C-ABI of the SCAPE per-shard sparse optimizer step for NVIDIA B200 (sm_100a).
+ *
+ * What the library computes: one rank's partition of Algorithm 1 of "SCAPE: Accurate and
+ * Efficient LLM Training with Extreme Sparse Communication" (arXiv 2607.01678;
+ * PAPER.md:131-174), with the N data-parallel workers of the paper simulated as R gradient
+ * buffers resident in one GPU's HBM and the all-reduce of Alg. 1 l.10 replaced by
+ * an in-device sum over those R buffers.  Per step, in the paper's order:
+ *   l.6   m~^r = beta1 m + (1-beta1) g^r + e^r
+ *   l.7-8 e^r <- m~^r off the mask M_{t-1}, 0 on it
+ *   l.9   b^r <- m~^r on M_{t-1}, packed: fp32 values + int32 idx
+ *   l.10  b- = (1/R) sum_r b^r
+ *   l.11  M_t = top-k of |m~^0| over the whole partition, used from
+ *         step t+1 on (one-step delay)
+ *   l.12  m <- b- (zero off the mask, Eq. 4)
+ *   l.13  g^ = (b- - beta1 m_old)/(1-beta1)   (Eq. 3)
+ *   l.15-17 v = beta2 m_old^2 + (1-beta2) g^^2 ; u = m/(sqrt(v)+eps);
+ *         theta <- theta - lr (u + wd theta)   (AdamS, Eq. 2)
+ * clip_grad (l.14) and bias correction are NOT applied (readings S3, S4).
+ * Ties in the top-k go to the lower index; exactly k = N - floor(sparsity*N) entries are kept.
+ * The fp32 operation order is pinned.
+ *
+ * All pointers are plain pointers; "device" means memory of the CUDA device that was current
+ * when scape_create ran.  No call throws or aborts; failures return NULL / a negative code and
+ * leave a message retrievable with scape_last_error() (thread-local).  There is no CPU
+ * fallback: without a CUDA device scape_create fails.
+ */
+#ifndef SCAPE_H_
+#define SCAPE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct scape scape_t;
+
+/* error codes (negative) */
+#define SCAPE_OK       0
+#define SCAPE_EINVAL  (-1)   /* bad argument (NULL handle, misaligned pointer, bad selector/size) */
+#define SCAPE_ECUDA   (-2)   /* a CUDA runtime call or kernel launch failed                        */
+#define SCAPE_ENOMEM  (-3)   /* device or host allocation failed                                   */
+
+/* gradient element types for scape_set_grad_dtype */
+#define SCAPE_GRAD_F32   0
+#define SCAPE_GRAD_BF16  1
+
+/* selectors for scape_get / scape_set / scape_count.  "LAST" = what the last completed step
+ * used or produced; "NEXT" = what the coming step will use.                                      */
+#define SCAPE_MOMENT        0  /* m, dense [N] f32                                    get/set      */
+#define SCAPE_RESIDUAL      1  /* e^r, dense [N] f32 (argument r)                     get/set      */
+#define SCAPE_MASK_NEXT     2  /* M_t: bit i%32 of word i/32, [ceil(N/32)] u32        get/set      */
+#define SCAPE_MASK_LAST     3  /* M_{t-1} as used by the last step, same layout       get          */
+#define SCAPE_IDX_NEXT      4  /* ascending indices of MASK_NEXT, [count] i32         get          */
+#define SCAPE_IDX_LAST      5  /* ascending indices of MASK_LAST, [count] i32         get          */
+#define SCAPE_PACKED        6  /* b^r of the last step, [count_last] f32 (argument r) get          */
+#define SCAPE_PACKED_MEAN   7  /* b- of the last step, [count_last] f32               get          */
+
+/* Alg. 1 "Require" line + l.1-2: create the state of one partition.
+ *   shard_numel  N, number of fp32 parameters in the flattened shard, 0 < N < 2^31
+ *   R            number of simulated data-parallel replicas (the paper's N workers), 1..8
+ *   sparsity     s in [0,1); k = N - floor(s*N) (evaluated in double) entries are selected
+ *   beta1,beta2  in [0,1); eps >= 0; lr; wd : AdamS hyper-parameters, cast to fp32 once
+ * Allocates on the current CUDA device and OWNS: m [N] (zeros), e^r [R][N] (zeros, l.2), the
+ * current mask (all ones, l.1) and the next mask, index lists, packed buffers and select
+ * scratch.  Returns NULL on failure (invalid argument, no device, out of memory).             */
+scape_t* scape_create(int64_t shard_numel, int R, double sparsity, double beta1, double beta2,
+                      double eps, double lr, double wd);
+
+/* One pass of Alg. 1 l.4-17 over the partition.
+ *   param        device, N fp32, 16-byte aligned, caller-owned, updated IN PLACE (l.17)
+ *   grads        HOST array of R device pointers; grads[r] holds g^r: N elements of the type
+ *                set by scape_set_grad_dtype (fp32 default), 16-byte aligned, caller-owned,
+ *                never written
+ *   cuda_stream  a cudaStream_t (NULL = legacy default stream)
+ * All work is enqueued on cuda_stream; the call does not synchronise and allocates nothing,
+ * so it can be captured into a CUDA graph.  One step may be in flight per handle.  Advances the
+ * step counter.  Returns SCAPE_OK or a negative code; the state is unchanged on SCAPE_EINVAL. */
+int scape_step(scape_t* h, float* param, const void* const* grads, void* cuda_stream);
+
+/* Same step with HOST buffers (end-to-end path): copies param (N fp32) and the R gradient
+ * buffers host->device into handle-owned staging (allocated on first use), runs scape_step,
+ * copies param back device->host, and synchronises cuda_stream before returning.  Pinned host
+ * memory makes the copies asynchronous DMA; pageable memory works but is slower.
+ * Bytes moved per call: h2d = 4N + R*N*sizeof(grad element), d2h = 4N.                          */
+int scape_step_host(scape_t* h, float* param_host, const void* const* grads_host,
+                    void* cuda_stream);
+
+/* Synchronises the handle's device work and frees everything it owns.  NULL is a no-op.       */
+void scape_destroy(scape_t* h);
+
+/* k of reading S6; the number of completed steps t; kernels launched so far by this handle.   */
+int64_t scape_k(const scape_t* h);
+int64_t scape_step_count(const scape_t* h);
+int64_t scape_launch_count(const scape_t* h);
+
+/* Number of entries of SCAPE_MASK_NEXT / SCAPE_MASK_LAST (N while the mask is all ones, else
+ * k); `which` is one of those two selectors.  Negative code on error.                           */
+int64_t scape_count(const scape_t* h, int which);
+
+/* Element type of the gradient buffers passed to the following steps (S16: fp32 or bf16;
+ * bf16 is widened exactly to fp32 in registers).                                               */
+int scape_set_grad_dtype(scape_t* h, int dtype);
+
+/* Option: also materialise b^r on steps whose mask is all ones (step 1, or sparsity 0), where
+ * the packed buffer would be R*N floats.  Off by default: on such steps SCAPE_PACKED is then
+ * unavailable (SCAPE_EINVAL) and SCAPE_PACKED_MEAN equals SCAPE_MOMENT.  Allocates R*N floats
+ * when switched on.  For tests.                                                                */
+int scape_set_keep_dense_pack(scape_t* h, int on);
+
+/* State accessors (tests, checkpoint/resume, the "identical state each step" loader).  `buf`
+ * may be a host or a device pointer (unified addressing); `bytes` must equal the size of the
+ * selected object; `r` is the replica for SCAPE_RESIDUAL / SCAPE_PACKED and ignored otherwise.
+ * Both calls synchronise `cuda_stream` before returning.  Not part of the timed path.
+ * scape_set(SCAPE_MASK_NEXT) accepts any mask with at most max(k, count) ... precisely: with
+ * at most k set bits, or all N bits set; bits at positions >= N are ignored.                    */
+int scape_get(scape_t* h, int what, int r, void* buf, size_t bytes, void* cuda_stream);
+int scape_set(scape_t* h, int what, int r, const void* buf, size_t bytes, void* cuda_stream);
+int scape_set_step_count(scape_t* h, int64_t t);
+
+/* Message of the last failure on the calling thread ("" if none).  Never NULL.                 */
+const char* scape_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SCAPE_H_ */

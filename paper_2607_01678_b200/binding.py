@@ -1,0 +1,254 @@
+"""Thin ctypes binding of libscape.so (include/scape.h).  Argument marshalling only: every step
+of the path runs in the CUDA kernels.  There is no fallback: if the library is missing, cannot be
+loaded, or no CUDA device exists, the calls raise.
+
+The module-level functions carry the C names (scape_create, scape_step, ...) and take raw
+pointers (ints); `Scape` is a small convenience wrapper over torch tensors (torch is used for
+device memory and streams only).
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libscape.so")
+
+SCAPE_OK, SCAPE_EINVAL, SCAPE_ECUDA, SCAPE_ENOMEM = 0, -1, -2, -3
+SCAPE_GRAD_F32, SCAPE_GRAD_BF16 = 0, 1
+(SCAPE_MOMENT, SCAPE_RESIDUAL, SCAPE_MASK_NEXT, SCAPE_MASK_LAST, SCAPE_IDX_NEXT, SCAPE_IDX_LAST,
+ SCAPE_PACKED, SCAPE_PACKED_MEAN) = range(8)
+
+# every symbol include/scape.h declares: name -> (restype, argtypes)
+_VP, _I64, _I, _D, _SZ = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+SYMBOLS = {
+    "scape_create": (_VP, [_I64, _I, _D, _D, _D, _D, _D, _D]),
+    "scape_step": (_I, [_VP, _VP, _VP, _VP]),
+    "scape_step_host": (_I, [_VP, _VP, _VP, _VP]),
+    "scape_destroy": (None, [_VP]),
+    "scape_k": (_I64, [_VP]),
+    "scape_step_count": (_I64, [_VP]),
+    "scape_launch_count": (_I64, [_VP]),
+    "scape_count": (_I64, [_VP, _I]),
+    "scape_set_grad_dtype": (_I, [_VP, _I]),
+    "scape_set_keep_dense_pack": (_I, [_VP, _I]),
+    "scape_get": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
+    "scape_set": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
+    "scape_set_step_count": (_I, [_VP, _I64]),
+    "scape_last_error": (ctypes.c_char_p, []),
+}
+
+_LIB = None
+
+
+class ScapeError(RuntimeError):
+    pass
+
+
+def lib():
+    """Load libscape.so (once).  Raises if it has not been built — there is no fallback."""
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise ScapeError(f"{LIB_PATH} is missing: run `python -m paper_2607_01678_b200.build` "
+                             "(or __graft_entry__.build()); there is no CPU or PyTorch fallback")
+        L = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _LIB = L
+    return _LIB
+
+
+def scape_last_error() -> str:
+    return lib().scape_last_error().decode()
+
+
+def _check(rc, what):
+    if rc != SCAPE_OK:
+        raise ScapeError(f"{what} failed ({rc}): {scape_last_error()}")
+
+
+def scape_create(shard_numel, R, sparsity, beta1, beta2, eps, lr, wd):
+    h = lib().scape_create(int(shard_numel), int(R), float(sparsity), float(beta1), float(beta2),
+                           float(eps), float(lr), float(wd))
+    if not h:
+        raise ScapeError(f"scape_create failed: {scape_last_error()}")
+    return h
+
+
+def scape_step(h, param_ptr, grad_ptrs, stream=0):
+    arr = (ctypes.c_void_p * len(grad_ptrs))(*grad_ptrs)
+    _check(lib().scape_step(h, param_ptr, arr, stream), "scape_step")
+
+
+def scape_step_host(h, param_ptr, grad_ptrs, stream=0):
+    arr = (ctypes.c_void_p * len(grad_ptrs))(*grad_ptrs)
+    _check(lib().scape_step_host(h, param_ptr, arr, stream), "scape_step_host")
+
+
+def scape_destroy(h):
+    lib().scape_destroy(h)
+
+
+def scape_k(h):
+    return int(lib().scape_k(h))
+
+
+def scape_step_count(h):
+    return int(lib().scape_step_count(h))
+
+
+def scape_launch_count(h):
+    return int(lib().scape_launch_count(h))
+
+
+def scape_count(h, which):
+    n = int(lib().scape_count(h, which))
+    if n < 0:
+        raise ScapeError(f"scape_count failed ({n}): {scape_last_error()}")
+    return n
+
+
+def scape_set_grad_dtype(h, dtype):
+    _check(lib().scape_set_grad_dtype(h, dtype), "scape_set_grad_dtype")
+
+
+def scape_set_keep_dense_pack(h, on):
+    _check(lib().scape_set_keep_dense_pack(h, int(on)), "scape_set_keep_dense_pack")
+
+
+def scape_set_step_count(h, t):
+    _check(lib().scape_set_step_count(h, int(t)), "scape_set_step_count")
+
+
+def scape_get(h, what, r, buf_ptr, nbytes, stream=0):
+    _check(lib().scape_get(h, what, r, buf_ptr, nbytes, stream), "scape_get")
+
+
+def scape_set(h, what, r, buf_ptr, nbytes, stream=0):
+    _check(lib().scape_set(h, what, r, buf_ptr, nbytes, stream), "scape_set")
+
+
+class Scape:
+    """Convenience wrapper: one partition's SCAPE state on the current CUDA device.
+
+    step(param, grads) takes torch CUDA tensors (param fp32 [N]; grads: R tensors [N], all fp32 or
+    all bf16) and enqueues the step on torch's current stream.
+    """
+
+    def __init__(self, shard_numel, R, sparsity, beta1=0.9, beta2=0.95, eps=1e-8, lr=1e-3, wd=0.1):
+        self.N, self.R = int(shard_numel), int(R)
+        self.h = scape_create(shard_numel, R, sparsity, beta1, beta2, eps, lr, wd)
+        self._gdt = SCAPE_GRAD_F32
+
+    def close(self):
+        if getattr(self, "h", None):
+            scape_destroy(self.h)
+            self.h = None
+
+    __del__ = close
+
+    @property
+    def k(self):
+        return scape_k(self.h)
+
+    @property
+    def t(self):
+        return scape_step_count(self.h)
+
+    @property
+    def launches(self):
+        return scape_launch_count(self.h)
+
+    @staticmethod
+    def _stream():
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+
+    def _set_dtype_for(self, g0):
+        import torch
+        want = SCAPE_GRAD_BF16 if g0.dtype == torch.bfloat16 else SCAPE_GRAD_F32
+        if want == SCAPE_GRAD_F32 and g0.dtype != torch.float32:
+            raise TypeError("gradients must be float32 or bfloat16")
+        if want != self._gdt:
+            scape_set_grad_dtype(self.h, want)
+            self._gdt = want
+
+    def step(self, param, grads):
+        import torch
+        assert param.is_cuda and param.dtype == torch.float32 and param.is_contiguous() and param.numel() == self.N
+        assert len(grads) == self.R
+        for g in grads:
+            assert g.is_cuda and g.is_contiguous() and g.numel() == self.N and g.dtype == grads[0].dtype
+        self._set_dtype_for(grads[0])
+        scape_step(self.h, param.data_ptr(), [g.data_ptr() for g in grads], self._stream())
+
+    def step_host(self, param, grads):
+        """param / grads: CPU tensors (pinned for async DMA). Synchronises before returning."""
+        assert not param.is_cuda and param.is_contiguous() and param.numel() == self.N
+        self._set_dtype_for(grads[0])
+        scape_step_host(self.h, param.data_ptr(), [g.data_ptr() for g in grads], self._stream())
+
+    # ---- accessors (numpy in / out) -------------------------------------------------
+    def _get(self, what, n, dtype, r=0):
+        out = np.empty(n, dtype=dtype)
+        scape_get(self.h, what, r, out.ctypes.data, out.nbytes, self._stream())
+        return out
+
+    def _set(self, what, arr, dtype, r=0):
+        a = np.ascontiguousarray(arr, dtype=dtype)
+        scape_set(self.h, what, r, a.ctypes.data, a.nbytes, self._stream())
+
+    def moment(self):
+        return self._get(SCAPE_MOMENT, self.N, np.float32)
+
+    def set_moment(self, a):
+        self._set(SCAPE_MOMENT, a, np.float32)
+
+    def residual(self, r):
+        return self._get(SCAPE_RESIDUAL, self.N, np.float32, r)
+
+    def set_residual(self, r, a):
+        self._set(SCAPE_RESIDUAL, a, np.float32, r)
+
+    def _mask(self, what):
+        words = self._get(what, (self.N + 31) // 32, np.uint32)
+        return np.unpackbits(words.view(np.uint8), bitorder="little")[: self.N]
+
+    def mask_next(self):
+        return self._mask(SCAPE_MASK_NEXT)
+
+    def mask_last(self):
+        return self._mask(SCAPE_MASK_LAST)
+
+    def set_mask_next(self, mask_u8):
+        m = np.asarray(mask_u8, dtype=np.uint8)
+        assert m.size == self.N
+        pad = (-self.N) % 32
+        bits = np.packbits(np.concatenate([m, np.zeros(pad, np.uint8)]), bitorder="little")
+        self._set(SCAPE_MASK_NEXT, bits.view(np.uint32), np.uint32)
+
+    def count_next(self):
+        return scape_count(self.h, SCAPE_MASK_NEXT)
+
+    def count_last(self):
+        return scape_count(self.h, SCAPE_MASK_LAST)
+
+    def idx_next(self):
+        return self._get(SCAPE_IDX_NEXT, self.count_next(), np.int32)
+
+    def idx_last(self):
+        return self._get(SCAPE_IDX_LAST, self.count_last(), np.int32)
+
+    def packed(self, r):
+        return self._get(SCAPE_PACKED, self.count_last(), np.float32, r)
+
+    def packed_mean(self):
+        return self._get(SCAPE_PACKED_MEAN, self.count_last(), np.float32)
+
+    def keep_dense_pack(self, on=True):
+        scape_set_keep_dense_pack(self.h, on)
+
+    def set_step_count(self, t):
+        scape_set_step_count(self.h, t)

@@ -1,0 +1,513 @@
+// scape.cu — host side of libscape.so: the C-ABI of include/scape.h, the handle, and the
+// stream-ordered launch sequence of one SCAPE step (Algorithm 1, :131-174).
+// No CPU fallback exists: every stage runs in the kernels of scape_kernels.cuh.
+#include "../../include/scape.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "scape_kernels.cuh"
+
+using namespace scapek;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof g_err, fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define CU_TRY(expr)                                                                         \
+  do {                                                                                       \
+    cudaError_t _e = (expr);                                                                 \
+    if (_e != cudaSuccess) return fail(SCAPE_ECUDA, "%s: %s", #expr, cudaGetErrorString(_e)); \
+  } while (0)
+
+struct MaskSlot {
+  uint32_t* bits = nullptr;   // [n_words]
+  uint32_t* rank = nullptr;   // [n_chunks]
+  int32_t* idx = nullptr;     // [k]   (not materialised while all_ones)
+  int64_t count = 0;
+  bool all_ones = false;
+  bool valid = false;
+};
+
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+    if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+}  // namespace
+
+struct scape {
+  int64_t N = 0, Npad = 0, n_chunks = 0, n_words = 0, k = 0;
+  int R = 0, dev = 0, n_sm = 148, grad_dtype = SCAPE_GRAD_F32;
+  int64_t t = 0, launches = 0;
+  float b1, b2, eps, lr, wd, c1, c2;
+
+  float* m = nullptr;          // [Npad]
+  float* e = nullptr;          // [R][Npad]
+  MaskSlot slot[2];
+  int use = 0;                 // slot the coming step uses (SCAPE_MASK_NEXT); 1-use = SCAPE_MASK_LAST
+  float* packed = nullptr;     // [R][packed_stride]
+  int64_t packed_stride = 0;
+  float* packed_mean = nullptr;   // [packed_stride]
+  float* dense_pack = nullptr;    // optional [R][Npad]
+  bool last_dense = false;
+
+  SelState* sel = nullptr;
+  uint32_t* ghist = nullptr;      // [kBins]
+  uint32_t* block_sum = nullptr;  // [n_compact_blocks]
+  uint32_t* total = nullptr;      // [1]
+  int n_compact_blocks = 0;
+
+  // scape_step_host staging
+  float* st_param = nullptr;
+  void* st_grad[kMaxR] = {};
+  size_t st_grad_bytes = 0;
+};
+
+namespace {
+
+int grid_for(const scape* h, int64_t n_chunks, int warps_per_block, int blocks_per_sm) {
+  int64_t need = (n_chunks + warps_per_block - 1) / warps_per_block;
+  int64_t cap = (int64_t)h->n_sm * blocks_per_sm;
+  if (need < 1) need = 1;
+  return (int)(need < cap ? need : cap);
+}
+
+template <typename G, int R, bool DENSE>
+int launch_fused_t(scape* h, const StepParams& p, cudaStream_t st) {
+  static int bps = 0;   // resident blocks per SM of this instantiation
+  if (bps == 0) {
+    int v = 0;
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, scape_fused_step_kernel<G, R, DENSE>, 256, 0));
+    bps = v > 0 ? v : 1;
+  }
+  const int grid = grid_for(h, p.n_chunks, 8, bps);
+  scape_fused_step_kernel<G, R, DENSE><<<grid, 256, 0, st>>>(p);
+  h->launches++;
+  CU_TRY(cudaGetLastError());
+  return SCAPE_OK;
+}
+
+template <typename G, bool DENSE>
+int launch_fused_r(scape* h, const StepParams& p, cudaStream_t st) {
+  switch (h->R) {
+    case 1: return launch_fused_t<G, 1, DENSE>(h, p, st);
+    case 2: return launch_fused_t<G, 2, DENSE>(h, p, st);
+    case 3: return launch_fused_t<G, 3, DENSE>(h, p, st);
+    case 4: return launch_fused_t<G, 4, DENSE>(h, p, st);
+    case 5: return launch_fused_t<G, 5, DENSE>(h, p, st);
+    case 6: return launch_fused_t<G, 6, DENSE>(h, p, st);
+    case 7: return launch_fused_t<G, 7, DENSE>(h, p, st);
+    case 8: return launch_fused_t<G, 8, DENSE>(h, p, st);
+  }
+  return fail(SCAPE_EINVAL, "R out of range");
+}
+
+int launch_fused(scape* h, const StepParams& p, bool dense, cudaStream_t st) {
+  if (h->grad_dtype == SCAPE_GRAD_BF16)
+    return dense ? launch_fused_r<__nv_bfloat16, true>(h, p, st) : launch_fused_r<__nv_bfloat16, false>(h, p, st);
+  return dense ? launch_fused_r<float, true>(h, p, st) : launch_fused_r<float, false>(h, p, st);
+}
+
+// rank128 (+ idx when idx != nullptr) of slot.bits; leaves the bit count in *h->total
+int compact_mask(scape* h, MaskSlot& s, bool want_idx, cudaStream_t st) {
+  const int nb = h->n_compact_blocks;
+  mask_block_count_kernel<<<nb, 1024, 0, st>>>(s.bits, h->n_chunks, h->block_sum);
+  mask_scan_blocks_kernel<<<1, 1024, 0, st>>>(h->block_sum, nb, h->total);
+  mask_rank_idx_kernel<<<nb, 1024, 0, st>>>(s.bits, h->n_chunks, h->block_sum, s.rank, want_idx ? s.idx : nullptr,
+                                            h->packed_stride);
+  h->launches += 3;
+  CU_TRY(cudaGetLastError());
+  return SCAPE_OK;
+}
+
+// Stage 2 (Alg. 1 l.11): exact top-k of |m~^0| -> nxt.bits / rank / idx.
+int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, cudaStream_t st) {
+  KeySrc src;
+  src.e0 = h->e;
+  src.cur_bits = cur.all_ones ? nullptr : cur.bits;
+  src.cur_rank = cur.all_ones ? nullptr : cur.rank;
+  src.packed0 = h->packed;
+  src.N = h->N;
+  src.n_chunks = h->n_chunks;
+  const int grid = grid_for(h, h->n_chunks, 8, 6);
+  sel_init_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist, (long long)h->k);
+  h->launches++;
+  static const int shifts[kSelPasses] = {51, 38, 25, 12, 0};
+  static const int widths[kSelPasses] = {13, 13, 13, 13, 12};
+  for (int p = 0; p < kSelPasses; ++p) {
+    sel_hist_dense_kernel<<<grid, 256, 0, st>>>(src, h->sel, h->ghist, shifts[p], widths[p]);
+    sel_pick_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist, shifts[p], widths[p]);
+    h->launches += 2;
+  }
+  sel_write_mask_dense_kernel<<<grid, 256, 0, st>>>(src, h->sel, nxt.bits);
+  h->launches++;
+  CU_TRY(cudaGetLastError());
+  int rc = compact_mask(h, nxt, true, st);
+  if (rc) return rc;
+  nxt.count = h->k;
+  nxt.all_ones = false;
+  nxt.valid = true;
+  return SCAPE_OK;
+}
+
+bool finite_all(std::initializer_list<double> v) {
+  for (double x : v) if (!std::isfinite(x)) return false;
+  return true;
+}
+
+void free_all(scape* h) {
+  cudaFree(h->m); cudaFree(h->e);
+  for (auto& s : h->slot) { cudaFree(s.bits); cudaFree(s.rank); cudaFree(s.idx); }
+  cudaFree(h->packed); cudaFree(h->packed_mean); cudaFree(h->dense_pack);
+  cudaFree(h->sel); cudaFree(h->ghist); cudaFree(h->block_sum); cudaFree(h->total);
+  cudaFree(h->st_param);
+  for (auto& g : h->st_grad) cudaFree(g);
+}
+
+}  // namespace
+
+extern "C" const char* scape_last_error(void) { return g_err; }
+
+extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1, double beta2, double eps,
+                                 double lr, double wd) {
+  g_err[0] = 0;
+  if (!finite_all({sparsity, beta1, beta2, eps, lr, wd})) { fail(SCAPE_EINVAL, "non-finite argument"); return nullptr; }
+  if (N <= 0 || N >= ((int64_t)1 << 31)) { fail(SCAPE_EINVAL, "shard_numel must be in (0, 2^31)"); return nullptr; }
+  if (R < 1 || R > kMaxR) { fail(SCAPE_EINVAL, "R must be in [1, %d]", kMaxR); return nullptr; }
+  if (!(sparsity >= 0.0 && sparsity < 1.0)) { fail(SCAPE_EINVAL, "sparsity must be in [0, 1)"); return nullptr; }
+  if (!(beta1 >= 0.0 && beta1 < 1.0) || !(beta2 >= 0.0 && beta2 < 1.0)) { fail(SCAPE_EINVAL, "beta must be in [0, 1)"); return nullptr; }
+  if (eps < 0.0) { fail(SCAPE_EINVAL, "eps must be >= 0"); return nullptr; }
+
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { fail(SCAPE_ECUDA, "no CUDA device (there is no CPU fallback)"); cudaGetLastError(); return nullptr; }
+  scape* h = new (std::nothrow) scape();
+  if (!h) { fail(SCAPE_ENOMEM, "host allocation failed"); return nullptr; }
+  h->dev = dev;
+  cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev);
+  h->N = N; h->R = R;
+  h->Npad = (N + kChunk - 1) / kChunk * kChunk;
+  h->n_chunks = h->Npad / kChunk;
+  h->n_words = h->Npad / 32;
+  h->k = N - (int64_t)std::floor(sparsity * (double)N);          // reading S6
+  // hyper-parameters are cast to fp32 once; 1 - beta is evaluated in fp32
+  h->b1 = (float)beta1; h->b2 = (float)beta2; h->eps = (float)eps; h->lr = (float)lr; h->wd = (float)wd;
+  h->c1 = 1.0f - h->b1; h->c2 = 1.0f - h->b2;
+  h->n_compact_blocks = (int)((h->n_chunks + kCompactChunksPerBlock - 1) / kCompactChunksPerBlock);
+  const bool sparse = h->k < N;
+  h->packed_stride = sparse ? (h->k + 31) / 32 * 32 : 0;
+
+  bool ok = true;
+  auto alloc = [&](void** p, size_t bytes, bool zero) {
+    if (!ok) return;
+    if (cudaMalloc(p, bytes ? bytes : 16) != cudaSuccess) { ok = false; *p = nullptr; return; }
+    if (zero && cudaMemset(*p, 0, bytes ? bytes : 16) != cudaSuccess) ok = false;
+  };
+  alloc((void**)&h->m, sizeof(float) * h->Npad, true);                       // S5: m_0 = 0
+  alloc((void**)&h->e, sizeof(float) * h->Npad * R, true);                   // l.2: e_0 = 0
+  for (auto& s : h->slot) {
+    alloc((void**)&s.bits, sizeof(uint32_t) * h->n_words, true);
+    alloc((void**)&s.rank, sizeof(uint32_t) * h->n_chunks, true);
+    if (sparse) alloc((void**)&s.idx, sizeof(int32_t) * h->packed_stride, true);
+  }
+  if (sparse) {
+    alloc((void**)&h->packed, sizeof(float) * h->packed_stride * R, true);
+    alloc((void**)&h->packed_mean, sizeof(float) * h->packed_stride, true);
+  }
+  alloc((void**)&h->sel, sizeof(SelState), true);
+  alloc((void**)&h->ghist, sizeof(uint32_t) * kBins, true);
+  alloc((void**)&h->block_sum, sizeof(uint32_t) * (h->n_compact_blocks + 1), true);
+  alloc((void**)&h->total, sizeof(uint32_t), true);
+  if (!ok) {
+    fail(SCAPE_ENOMEM, "device allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
+    free_all(h); delete h; return nullptr;
+  }
+  h->slot[0].all_ones = true;                                                // l.1: M_0 = 1
+  h->slot[0].count = N;
+  h->slot[0].valid = true;
+  h->use = 0;
+  if (cudaDeviceSynchronize() != cudaSuccess) { fail(SCAPE_ECUDA, "create: sync failed"); free_all(h); delete h; return nullptr; }
+  return h;
+}
+
+extern "C" void scape_destroy(scape_t* h) {
+  if (!h) return;
+  DeviceGuard g(h->dev);
+  cudaDeviceSynchronize();
+  free_all(h);
+  delete h;
+}
+
+extern "C" int64_t scape_k(const scape_t* h) { return h ? h->k : SCAPE_EINVAL; }
+extern "C" int64_t scape_step_count(const scape_t* h) { return h ? h->t : SCAPE_EINVAL; }
+extern "C" int64_t scape_launch_count(const scape_t* h) { return h ? h->launches : SCAPE_EINVAL; }
+
+extern "C" int64_t scape_count(const scape_t* h, int which) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (which == SCAPE_MASK_NEXT) return h->slot[h->use].count;
+  if (which == SCAPE_MASK_LAST) {
+    if (!h->slot[1 - h->use].valid || h->t == 0) return fail(SCAPE_EINVAL, "no step has run yet");
+    return h->slot[1 - h->use].count;
+  }
+  return fail(SCAPE_EINVAL, "scape_count: bad selector %d", which);
+}
+
+extern "C" int scape_set_grad_dtype(scape_t* h, int dtype) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (dtype != SCAPE_GRAD_F32 && dtype != SCAPE_GRAD_BF16) return fail(SCAPE_EINVAL, "unknown grad dtype %d", dtype);
+  if (dtype != h->grad_dtype) {            // staging buffers are sized by dtype
+    for (auto& g : h->st_grad) { cudaFree(g); g = nullptr; }
+    h->st_grad_bytes = 0;
+  }
+  h->grad_dtype = dtype;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_set_keep_dense_pack(scape_t* h, int on) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  DeviceGuard g(h->dev);
+  if (on && !h->dense_pack) {
+    if (cudaMalloc((void**)&h->dense_pack, sizeof(float) * h->Npad * h->R) != cudaSuccess) {
+      h->dense_pack = nullptr; cudaGetLastError();
+      return fail(SCAPE_ENOMEM, "keep_dense_pack: allocation of R*N floats failed");
+    }
+  } else if (!on && h->dense_pack) {
+    cudaDeviceSynchronize();
+    cudaFree(h->dense_pack);
+    h->dense_pack = nullptr;
+  }
+  return SCAPE_OK;
+}
+
+extern "C" int scape_set_step_count(scape_t* h, int64_t t) {
+  if (!h || t < 0) return fail(SCAPE_EINVAL, "bad argument");
+  h->t = t;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, void* cuda_stream) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (!param || !grads) return fail(SCAPE_EINVAL, "NULL param/grads");
+  if ((uintptr_t)param & 15) return fail(SCAPE_EINVAL, "param must be 16-byte aligned");
+  for (int r = 0; r < h->R; ++r) {
+    if (!grads[r]) return fail(SCAPE_EINVAL, "grads[%d] is NULL", r);
+    if ((uintptr_t)grads[r] & 15) return fail(SCAPE_EINVAL, "grads[%d] must be 16-byte aligned", r);
+  }
+  DeviceGuard guard(h->dev);
+  if (!guard.ok) return fail(SCAPE_ECUDA, "cannot select the handle's device");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+
+  MaskSlot& cur = h->slot[h->use];
+  MaskSlot& nxt = h->slot[1 - h->use];
+  const bool need_select = h->k < h->N;
+
+  StepParams p{};
+  p.theta = param; p.m = h->m; p.e = h->e; p.e_stride = h->Npad;
+  for (int r = 0; r < h->R; ++r) p.g[r] = grads[r];
+  p.cur_bits = cur.bits; p.cur_rank = cur.rank;
+  p.packed = cur.all_ones ? h->dense_pack : h->packed;
+  p.packed_stride = cur.all_ones ? h->Npad : h->packed_stride;
+  p.packed_mean = h->packed_mean;
+  p.N = h->N; p.n_chunks = h->n_chunks;
+  p.b1 = h->b1; p.c1 = h->c1; p.b2 = h->b2; p.c2 = h->c2; p.eps = h->eps; p.wd = h->wd; p.neg_lr = -h->lr;
+  p.R_f = (float)h->R; p.inv_R = 1.0f / (float)h->R;
+  p.r_pow2 = (h->R & (h->R - 1)) == 0;      // x / 2^n == x * 2^-n bit for bit
+  p.stash = cur.all_ones && need_select;
+
+  int rc = launch_fused(h, p, cur.all_ones, st);
+  if (rc) return rc;
+
+  if (need_select) {
+    rc = run_select(h, cur, nxt, st);
+    if (rc) return rc;
+    if (cur.all_ones) CU_TRY(cudaMemsetAsync(h->e, 0, sizeof(float) * h->Npad, st));   // l.8 for e^0 after the stash
+  } else {
+    nxt.all_ones = true; nxt.count = h->N; nxt.valid = true;                            // k = N: M_t = 1
+  }
+  h->last_dense = cur.all_ones;
+  h->use = 1 - h->use;
+  h->t += 1;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_step_host(scape_t* h, float* param_host, const void* const* grads_host, void* cuda_stream) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (!param_host || !grads_host) return fail(SCAPE_EINVAL, "NULL param/grads");
+  DeviceGuard guard(h->dev);
+  if (!guard.ok) return fail(SCAPE_ECUDA, "cannot select the handle's device");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t gb = (size_t)h->N * (h->grad_dtype == SCAPE_GRAD_BF16 ? 2 : 4);
+  if (!h->st_param) {
+    if (cudaMalloc((void**)&h->st_param, sizeof(float) * h->N) != cudaSuccess) { h->st_param = nullptr; cudaGetLastError(); return fail(SCAPE_ENOMEM, "staging allocation failed"); }
+  }
+  if (h->st_grad_bytes != gb) {
+    for (int r = 0; r < h->R; ++r) {
+      cudaFree(h->st_grad[r]); h->st_grad[r] = nullptr;
+      if (cudaMalloc(&h->st_grad[r], gb) != cudaSuccess) { h->st_grad[r] = nullptr; h->st_grad_bytes = 0; cudaGetLastError(); return fail(SCAPE_ENOMEM, "staging allocation failed"); }
+    }
+    h->st_grad_bytes = gb;
+  }
+  for (int r = 0; r < h->R; ++r) {
+    if (!grads_host[r]) return fail(SCAPE_EINVAL, "grads[%d] is NULL", r);
+    CU_TRY(cudaMemcpyAsync(h->st_grad[r], grads_host[r], gb, cudaMemcpyHostToDevice, st));
+  }
+  CU_TRY(cudaMemcpyAsync(h->st_param, param_host, sizeof(float) * h->N, cudaMemcpyHostToDevice, st));
+  int rc = scape_step(h, h->st_param, (const void* const*)h->st_grad, cuda_stream);
+  if (rc) return rc;
+  CU_TRY(cudaMemcpyAsync(param_host, h->st_param, sizeof(float) * h->N, cudaMemcpyDeviceToHost, st));
+  CU_TRY(cudaStreamSynchronize(st));
+  return SCAPE_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// accessors
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+int materialise_all_ones(scape* h, MaskSlot& s, cudaStream_t st) {
+  mask_all_ones_kernel<<<256, 256, 0, st>>>(s.bits, h->n_words, h->N);
+  h->launches++;
+  CU_TRY(cudaGetLastError());
+  return SCAPE_OK;
+}
+
+int get_idx(scape* h, MaskSlot& s, void* buf, size_t bytes, cudaStream_t st) {
+  if (bytes != sizeof(int32_t) * (size_t)s.count) return fail(SCAPE_EINVAL, "idx: expected %zu bytes", sizeof(int32_t) * (size_t)s.count);
+  if (!s.all_ones) {
+    CU_TRY(cudaMemcpyAsync(buf, s.idx, bytes, cudaMemcpyDefault, st));
+    return SCAPE_OK;
+  }
+  int32_t* tmp = nullptr;
+  CU_TRY(cudaMalloc((void**)&tmp, bytes));
+  iota_i32_kernel<<<256, 256, 0, st>>>(tmp, h->N);
+  h->launches++;
+  cudaError_t e1 = cudaMemcpyAsync(buf, tmp, bytes, cudaMemcpyDefault, st);
+  cudaError_t e2 = cudaStreamSynchronize(st);
+  cudaFree(tmp);
+  if (e1 != cudaSuccess || e2 != cudaSuccess) return fail(SCAPE_ECUDA, "idx copy failed");
+  return SCAPE_OK;
+}
+
+}  // namespace
+
+extern "C" int scape_get(scape_t* h, int what, int r, void* buf, size_t bytes, void* cuda_stream) {
+  if (!h || !buf) return fail(SCAPE_EINVAL, "NULL argument");
+  DeviceGuard guard(h->dev);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t nbytes = sizeof(float) * (size_t)h->N;
+  MaskSlot& nx = h->slot[h->use];
+  MaskSlot& la = h->slot[1 - h->use];
+  int rc = SCAPE_OK;
+  switch (what) {
+    case SCAPE_MOMENT:
+      if (bytes != nbytes) return fail(SCAPE_EINVAL, "moment: expected %zu bytes", nbytes);
+      CU_TRY(cudaMemcpyAsync(buf, h->m, bytes, cudaMemcpyDefault, st));
+      break;
+    case SCAPE_RESIDUAL:
+      if (r < 0 || r >= h->R) return fail(SCAPE_EINVAL, "residual: replica %d out of range", r);
+      if (bytes != nbytes) return fail(SCAPE_EINVAL, "residual: expected %zu bytes", nbytes);
+      CU_TRY(cudaMemcpyAsync(buf, h->e + (size_t)r * h->Npad, bytes, cudaMemcpyDefault, st));
+      break;
+    case SCAPE_MASK_NEXT:
+    case SCAPE_MASK_LAST: {
+      MaskSlot& s = what == SCAPE_MASK_NEXT ? nx : la;
+      if (what == SCAPE_MASK_LAST && (h->t == 0 || !s.valid)) return fail(SCAPE_EINVAL, "no step has run yet");
+      const size_t mb = sizeof(uint32_t) * (size_t)((h->N + 31) / 32);
+      if (bytes != mb) return fail(SCAPE_EINVAL, "mask: expected %zu bytes", mb);
+      if (s.all_ones && (rc = materialise_all_ones(h, s, st))) return rc;
+      CU_TRY(cudaMemcpyAsync(buf, s.bits, bytes, cudaMemcpyDefault, st));
+      break;
+    }
+    case SCAPE_IDX_NEXT:
+      if ((rc = get_idx(h, nx, buf, bytes, st))) return rc;
+      break;
+    case SCAPE_IDX_LAST:
+      if (h->t == 0 || !la.valid) return fail(SCAPE_EINVAL, "no step has run yet");
+      if ((rc = get_idx(h, la, buf, bytes, st))) return rc;
+      break;
+    case SCAPE_PACKED: {
+      if (h->t == 0 || !la.valid) return fail(SCAPE_EINVAL, "no step has run yet");
+      if (r < 0 || r >= h->R) return fail(SCAPE_EINVAL, "packed: replica %d out of range", r);
+      if (bytes != sizeof(float) * (size_t)la.count) return fail(SCAPE_EINVAL, "packed: expected %zu bytes", sizeof(float) * (size_t)la.count);
+      if (h->last_dense) {
+        if (!h->dense_pack) return fail(SCAPE_EINVAL, "packed: the last step's mask was all ones and keep_dense_pack is off");
+        CU_TRY(cudaMemcpyAsync(buf, h->dense_pack + (size_t)r * h->Npad, bytes, cudaMemcpyDefault, st));
+      } else {
+        CU_TRY(cudaMemcpyAsync(buf, h->packed + (size_t)r * h->packed_stride, bytes, cudaMemcpyDefault, st));
+      }
+      break;
+    }
+    case SCAPE_PACKED_MEAN:
+      if (h->t == 0 || !la.valid) return fail(SCAPE_EINVAL, "no step has run yet");
+      if (bytes != sizeof(float) * (size_t)la.count) return fail(SCAPE_EINVAL, "packed_mean: expected %zu bytes", sizeof(float) * (size_t)la.count);
+      CU_TRY(cudaMemcpyAsync(buf, h->last_dense ? h->m : h->packed_mean, bytes, cudaMemcpyDefault, st));
+      break;
+    default:
+      return fail(SCAPE_EINVAL, "scape_get: bad selector %d", what);
+  }
+  CU_TRY(cudaStreamSynchronize(st));
+  return SCAPE_OK;
+}
+
+extern "C" int scape_set(scape_t* h, int what, int r, const void* buf, size_t bytes, void* cuda_stream) {
+  if (!h || !buf) return fail(SCAPE_EINVAL, "NULL argument");
+  DeviceGuard guard(h->dev);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t nbytes = sizeof(float) * (size_t)h->N;
+  switch (what) {
+    case SCAPE_MOMENT:
+      if (bytes != nbytes) return fail(SCAPE_EINVAL, "moment: expected %zu bytes", nbytes);
+      CU_TRY(cudaMemcpyAsync(h->m, buf, bytes, cudaMemcpyDefault, st));
+      break;
+    case SCAPE_RESIDUAL:
+      if (r < 0 || r >= h->R) return fail(SCAPE_EINVAL, "residual: replica %d out of range", r);
+      if (bytes != nbytes) return fail(SCAPE_EINVAL, "residual: expected %zu bytes", nbytes);
+      CU_TRY(cudaMemcpyAsync(h->e + (size_t)r * h->Npad, buf, bytes, cudaMemcpyDefault, st));
+      break;
+    case SCAPE_MASK_NEXT: {
+      MaskSlot& s = h->slot[h->use];
+      const size_t mb = sizeof(uint32_t) * (size_t)((h->N + 31) / 32);
+      if (bytes != mb) return fail(SCAPE_EINVAL, "mask: expected %zu bytes", mb);
+      CU_TRY(cudaMemsetAsync(s.bits, 0, sizeof(uint32_t) * h->n_words, st));
+      CU_TRY(cudaMemcpyAsync(s.bits, buf, bytes, cudaMemcpyDefault, st));
+      mask_clear_tail_kernel<<<1, 256, 0, st>>>(s.bits, h->n_words, h->N);
+      h->launches++;
+      // count first (rank only), then decide whether an index list fits
+      int rc = compact_mask(h, s, false, st);
+      if (rc) return rc;
+      uint32_t total = 0;
+      CU_TRY(cudaMemcpyAsync(&total, h->total, sizeof total, cudaMemcpyDeviceToHost, st));
+      CU_TRY(cudaStreamSynchronize(st));
+      if ((int64_t)total == h->N) {
+        s.all_ones = true; s.count = h->N; s.valid = true;
+      } else if ((int64_t)total <= h->k && h->k < h->N) {
+        s.all_ones = false; s.count = total; s.valid = true;
+        if ((rc = compact_mask(h, s, true, st))) return rc;
+      } else {
+        s.all_ones = true; s.count = h->N; s.valid = true;   // fall back to a defined state
+        return fail(SCAPE_EINVAL, "mask: %u bits set, at most k = %lld (or all N) allowed", total, (long long)h->k);
+      }
+      break;
+    }
+    default:
+      return fail(SCAPE_EINVAL, "scape_set: selector %d is not settable", what);
+  }
+  CU_TRY(cudaStreamSynchronize(st));
+  return SCAPE_OK;
+}

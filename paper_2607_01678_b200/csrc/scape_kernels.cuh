@@ -1,0 +1,434 @@
+// scape_kernels.cuh — sm_100a kernels of the SCAPE step (Algorithm 1, :131-174).
+//
+// Data layout: the shard is cut into CHUNKS of 128 consecutive
+// parameters; one warp handles one chunk per loop trip, lane l owning elements 4l..4l+3
+// (one 128-bit access per fp32 array, one 64-bit access per bf16 array).  A mask is stored as
+// bits (word i/32, bit i%32 => one uint4 per chunk) plus `rank128[c]`, the number of set bits
+// before chunk c, so the packed position of a selected element is rank128[c] + popc(bits
+// before it inside the chunk): the pack of Alg. 1 l.9 needs no atomics and keeps ascending
+// index order.
+//
+// Every fp32 operation of the method is written with a _rn intrinsic so that nvcc cannot
+// contract or reorder it; the order is the one pinned in DESIGN.md and followed by the oracle.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace scapek {
+
+constexpr int kChunk = 128;          // parameters per warp trip
+constexpr int kMaxR = 8;
+constexpr int kDigitBits = 13;       // radix-select digit width
+constexpr int kBins = 1 << kDigitBits;
+constexpr int kSelPasses = 5;        // 64-bit composite key = 13+13+13+13+12 bits
+
+struct StepParams {
+  float* theta;                 // [N] caller-owned
+  float* m;                     // [Npad]
+  float* e;                     // [R][e_stride]
+  int64_t e_stride;
+  const void* g[kMaxR];         // R caller-owned gradient buffers
+  const uint32_t* cur_bits;     // [Npad/32]   (unused when DENSE)
+  const uint32_t* cur_rank;     // [Npad/128]
+  float* packed;                // [R][packed_stride] or nullptr (DENSE without keep_dense_pack)
+  int64_t packed_stride;
+  float* packed_mean;           // [k]          (unused when DENSE)
+  int64_t N;
+  int64_t n_chunks;             // ceil(N/128)
+  float b1, c1, b2, c2, eps, wd, neg_lr;
+  float R_f, inv_R;
+  int r_pow2;
+  int stash;                    // DENSE only: leave m~^0 in e^0 (keys for the select), not 0
+};
+
+// ------------------------------------------------------------------------------------------
+// 128-bit streaming accesses.  ld.global.cs / st.global.cs = evict-first: every dense array is
+// touched exactly once per step, so nothing here should displace the small resident arrays
+// (mask bits, rank128, packed buffers) from L2.
+// ------------------------------------------------------------------------------------------
+template <bool GUARD>
+__device__ __forceinline__ void load4_f32(const float* __restrict__ p, int64_t i0, int64_t N, float (&v)[4]) {
+  if (!GUARD) {
+    const float4 t = __ldcs(reinterpret_cast<const float4*>(p + i0));
+    v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+  } else {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) v[q] = (i0 + q < N) ? __ldcs(p + i0 + q) : 0.0f;
+  }
+}
+
+template <bool GUARD>
+__device__ __forceinline__ void store4_f32(float* __restrict__ p, int64_t i0, int64_t N, const float (&v)[4]) {
+  if (!GUARD) {
+    __stcs(reinterpret_cast<float4*>(p + i0), make_float4(v[0], v[1], v[2], v[3]));
+  } else {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) if (i0 + q < N) __stcs(p + i0 + q, v[q]);
+  }
+}
+
+// Gradient loads: fp32, or bf16 widened exactly (S16) by placing the 16 bits in the high half.
+template <typename G, bool GUARD>
+__device__ __forceinline__ void load4_grad(const void* __restrict__ base, int64_t i0, int64_t N, float (&v)[4]) {
+  if constexpr (sizeof(G) == 4) {
+    load4_f32<GUARD>(reinterpret_cast<const float*>(base), i0, N, v);
+  } else {
+    const uint16_t* p = reinterpret_cast<const uint16_t*>(base);
+    if (!GUARD) {
+      const uint2 t = __ldcs(reinterpret_cast<const uint2*>(p + i0));
+      v[0] = __uint_as_float(t.x << 16); v[1] = __uint_as_float(t.x & 0xFFFF0000u);
+      v[2] = __uint_as_float(t.y << 16); v[3] = __uint_as_float(t.y & 0xFFFF0000u);
+    } else {
+#pragma unroll
+      for (int q = 0; q < 4; ++q)
+        v[q] = (i0 + q < N) ? __uint_as_float(((uint32_t)__ldcs(p + i0 + q)) << 16) : 0.0f;
+    }
+  }
+}
+
+// Position of this lane's 4 mask bits inside the chunk's uint4, and the packed rank before them.
+__device__ __forceinline__ void lane_mask_bits(const uint32_t* __restrict__ bits, const uint32_t* __restrict__ rank,
+                                               int64_t c, int lane, uint32_t& mybits, uint32_t& jbase) {
+  const uint4 mw = __ldg(reinterpret_cast<const uint4*>(bits) + c);
+  const uint32_t r0 = __ldg(rank + c);
+  const int ws = lane >> 3, sh = (lane & 7) << 2;
+  const uint32_t p0 = __popc(mw.x), p1 = p0 + __popc(mw.y), p2 = p1 + __popc(mw.z);
+  const uint32_t w = ws == 0 ? mw.x : ws == 1 ? mw.y : ws == 2 ? mw.z : mw.w;
+  const uint32_t before = ws == 0 ? 0u : ws == 1 ? p0 : ws == 2 ? p1 : p2;
+  mybits = (w >> sh) & 0xFu;
+  jbase = r0 + before + __popc(w & ((1u << sh) - 1u));
+}
+
+// ------------------------------------------------------------------------------------------
+// Stages 1, 3, 4, 5, 6 fused: one streaming pass (Alg. 1 l.6-10, l.12-17).
+// ------------------------------------------------------------------------------------------
+template <typename G, int R, bool DENSE, bool GUARD>
+__device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int lane) {
+  const int64_t i0 = (c << 7) + ((int64_t)lane << 2);
+  uint32_t mybits = 0xFu, jbase = 0;
+  if (!DENSE) lane_mask_bits(p.cur_bits, p.cur_rank, c, lane, mybits, jbase);
+
+  float th[4], mo[4], gg[R][4], ee[R][4];
+  load4_f32<GUARD>(p.theta, i0, p.N, th);
+  load4_f32<false>(p.m, i0, p.N, mo);                       // own arrays are padded to Npad
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    load4_grad<G, GUARD>(p.g[r], i0, p.N, gg[r]);
+    load4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
+  }
+
+  float mn[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const bool on = DENSE || ((mybits >> q) & 1u);
+    const float pq = __fmul_rn(p.b1, mo[q]);                // beta1 * m_{t-1}, reused by l.6 and l.13
+    const int64_t j = DENSE ? (i0 + q) : (int64_t)(jbase + __popc(mybits & ((1u << q) - 1u)));
+    float s = 0.0f;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      const float mt = __fadd_rn(__fmaf_rn(p.c1, gg[r][q], pq), ee[r][q]);   // l.6
+      ee[r][q] = on ? ((DENSE && r == 0 && p.stash) ? mt : 0.0f) : mt;       // l.7-8
+      if (on) {
+        if (!DENSE || p.packed != nullptr) {
+          if (!GUARD || i0 + q < p.N) p.packed[r * p.packed_stride + j] = mt;   // l.9
+        }
+        s = (r == 0) ? mt : __fadd_rn(s, mt);                                // l.10, r ascending
+      }
+    }
+    float u = 0.0f;                                                          // Eq. 5: u = 0 off the mask
+    mn[q] = 0.0f;                                                            // Eq. 4: m = 0 off the mask
+    if (on) {
+      const float bb = p.r_pow2 ? __fmul_rn(s, p.inv_R) : __fdiv_rn(s, p.R_f);    // l.10
+      const float gh = __fdiv_rn(__fsub_rn(bb, pq), p.c1);                          // l.13 (Eq. 3)
+      const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), __fmul_rn(p.b2, __fmul_rn(mo[q], mo[q])));  // l.15
+      u = __fdiv_rn(bb, __fadd_rn(__fsqrt_rn(v), p.eps));                           // l.16
+      mn[q] = bb;                                                                   // l.12
+      if (!DENSE) p.packed_mean[j] = bb;
+    }
+    const float w = __fmaf_rn(p.wd, th[q], u);                                      // l.17
+    th[q] = __fmaf_rn(p.neg_lr, w, th[q]);
+  }
+
+  store4_f32<GUARD>(p.theta, i0, p.N, th);
+  store4_f32<false>(p.m, i0, p.N, mn);
+#pragma unroll
+  for (int r = 0; r < R; ++r) store4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
+}
+
+template <typename G, int R, bool DENSE>
+__global__ void __launch_bounds__(256) scape_fused_step_kernel(const __grid_constant__ StepParams p) {
+  const int lane = threadIdx.x & 31;
+  const int64_t wpb = blockDim.x >> 5;
+  const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
+  const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  const int64_t full = p.N >> 7;
+  for (int64_t c = warp; c < full; c += nwarps) fused_chunk<G, R, DENSE, false>(p, c, lane);
+  if (full < p.n_chunks && warp == full % nwarps) fused_chunk<G, R, DENSE, true>(p, full, lane);
+}
+
+// ------------------------------------------------------------------------------------------
+// Stage 2: exact top-k by radix select on the composite 64-bit key
+//     K64(i) = bits(|m~^0[i]|) << 32 | (0xFFFFFFFF - i)
+// Larger K64 = larger magnitude, ties to the LOWER index (reading S7); all keys are distinct,
+// so "the k largest" is unique and selected(i) <=> K64(i) >= T64, T64 the k-th largest.
+// The statistic is not stored on its own: off the current mask |m~^0| is exactly the new e^0,
+// on it it is b^0 (conservation, pin P2), so the passes re-read those.
+// ------------------------------------------------------------------------------------------
+struct KeySrc {
+  const float* e0;            // [Npad]
+  const uint32_t* cur_bits;   // mask the step used (nullptr => treat every position as "off":
+  const uint32_t* cur_rank;   //   all-ones step with m~^0 stashed in e^0)
+  const float* packed0;       // b^0
+  int64_t N;
+  int64_t n_chunks;
+};
+
+struct SelState {
+  unsigned long long prefix;  // digits fixed so far
+  unsigned long long himask;  // mask of those digits
+  long long rank;             // rank (1-based from the top) still sought inside the prefix class
+  int pad[2];
+};
+
+__device__ __forceinline__ unsigned long long make_k64(float x, int64_t i) {
+  return ((unsigned long long)(__float_as_uint(x) & 0x7FFFFFFFu) << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)i);
+}
+
+// keys of this lane's 4 elements of chunk c (valid[q] false past N)
+__device__ __forceinline__ void chunk_keys(const KeySrc& s, int64_t c, int lane, unsigned long long (&k64)[4], bool (&valid)[4]) {
+  const int64_t i0 = (c << 7) + ((int64_t)lane << 2);
+  const float4 ev = __ldcs(reinterpret_cast<const float4*>(s.e0 + i0));
+  float x[4] = {ev.x, ev.y, ev.z, ev.w};
+  if (s.cur_bits != nullptr) {
+    uint32_t mybits, jbase;
+    lane_mask_bits(s.cur_bits, s.cur_rank, c, lane, mybits, jbase);
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+      if ((mybits >> q) & 1u) x[q] = __ldg(s.packed0 + jbase + __popc(mybits & ((1u << q) - 1u)));
+  }
+#pragma unroll
+  for (int q = 0; q < 4; ++q) { valid[q] = i0 + q < s.N; k64[q] = make_k64(x[q], i0 + q); }
+}
+
+__global__ void sel_init_kernel(SelState* st, uint32_t* ghist, long long k) {
+  for (int b = threadIdx.x; b < kBins; b += blockDim.x) ghist[b] = 0;
+  if (threadIdx.x == 0) { st->prefix = 0; st->himask = 0; st->rank = k; }
+}
+
+// Histogram of digit (K64 >> shift) & (kBins-1) over the keys whose higher digits equal prefix.
+__global__ void __launch_bounds__(256) sel_hist_dense_kernel(const __grid_constant__ KeySrc s, const SelState* __restrict__ st,
+                                                            uint32_t* __restrict__ ghist, int shift, int bits) {
+  __shared__ uint32_t h[kBins];
+  for (int b = threadIdx.x; b < kBins; b += blockDim.x) h[b] = 0;
+  __syncthreads();
+  const unsigned long long prefix = st->prefix, himask = st->himask;
+  const uint32_t dmask = (1u << bits) - 1u;
+  const int lane = threadIdx.x & 31;
+  const int64_t wpb = blockDim.x >> 5;
+  const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
+  const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  for (int64_t c = warp; c < s.n_chunks; c += nwarps) {
+    unsigned long long k64[4]; bool valid[4];
+    chunk_keys(s, c, lane, k64, valid);
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+      if (valid[q] && (k64[q] & himask) == prefix) atomicAdd(&h[(uint32_t)(k64[q] >> shift) & dmask], 1u);
+  }
+  __syncthreads();
+  for (int b = threadIdx.x; b < kBins; b += blockDim.x) if (h[b]) atomicAdd(&ghist[b], h[b]);
+}
+
+// One block: find the digit d whose class holds the sought rank; fix it; clear the histogram.
+__global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* ghist, int shift, int bits) {
+  constexpr int PER = kBins / 1024;                 // bins per thread
+  __shared__ long long warp_tot[32];
+  const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
+  // thread t owns bins [kBins - PER*(t+1), kBins - PER*t): thread 0 owns the TOP bins
+  const int top = kBins - PER * t;
+  uint32_t hv[PER];
+  long long local = 0;
+#pragma unroll
+  for (int q = 0; q < PER; ++q) { hv[q] = ghist[top - 1 - q]; local += hv[q]; }
+  // inclusive prefix sum over threads (from the top bins downwards)
+  long long incl = local;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { long long v = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += v; }
+  if (lane == 31) warp_tot[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    long long v = warp_tot[lane], iv = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { long long x = __shfl_up_sync(0xFFFFFFFFu, iv, o); if (lane >= o) iv += x; }
+    warp_tot[lane] = iv - v;                        // exclusive
+  }
+  __syncthreads();
+  const long long above = warp_tot[wid] + incl - local;   // keys in bins above this thread's bins
+  const long long rank = st->rank;
+  __syncthreads();
+  if (above < rank && rank <= above + local) {
+    long long cum = above;
+#pragma unroll
+    for (int q = 0; q < PER; ++q) {
+      if (cum < rank && rank <= cum + hv[q]) {
+        const unsigned long long d = (unsigned long long)(top - 1 - q);
+        st->prefix |= d << shift;
+        st->himask |= ((1ull << bits) - 1ull) << shift;
+        st->rank = rank - cum;
+      }
+      cum += hv[q];
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < PER; ++q) ghist[top - 1 - q] = 0;
+}
+
+// next mask bits: selected(i) <=> K64(i) >= T64 (= st->prefix once every digit is fixed).
+__global__ void __launch_bounds__(256) sel_write_mask_dense_kernel(const __grid_constant__ KeySrc s, const SelState* __restrict__ st,
+                                                                  uint32_t* __restrict__ next_bits) {
+  const unsigned long long T64 = st->prefix;
+  const int lane = threadIdx.x & 31;
+  const int64_t wpb = blockDim.x >> 5;
+  const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
+  const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  for (int64_t c = warp; c < s.n_chunks; c += nwarps) {
+    unsigned long long k64[4]; bool valid[4];
+    chunk_keys(s, c, lane, k64, valid);
+    uint32_t nib = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) nib |= (valid[q] && k64[q] >= T64) ? (1u << q) : 0u;
+    uint32_t w = nib << ((lane & 7) << 2);
+    w |= __shfl_xor_sync(0xFFFFFFFFu, w, 1);
+    w |= __shfl_xor_sync(0xFFFFFFFFu, w, 2);
+    w |= __shfl_xor_sync(0xFFFFFFFFu, w, 4);
+    if ((lane & 7) == 0) next_bits[(c << 2) + (lane >> 3)] = w;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// Ordered compaction of a bit mask: rank128[c] and the ascending index list (the int32 half of
+// the sparse buffer).  Three small kernels over N/8 bytes.
+// ------------------------------------------------------------------------------------------
+constexpr int kCompactChunksPerBlock = 1024;   // one thread per chunk
+
+__global__ void __launch_bounds__(1024) mask_block_count_kernel(const uint32_t* __restrict__ bits, int64_t n_chunks,
+                                                               uint32_t* __restrict__ block_sum) {
+  __shared__ uint32_t ws[32];
+  const int64_t c = (int64_t)blockIdx.x * kCompactChunksPerBlock + threadIdx.x;
+  uint32_t n = 0;
+  if (c < n_chunks) {
+    const uint4 w = __ldg(reinterpret_cast<const uint4*>(bits) + c);
+    n = __popc(w.x) + __popc(w.y) + __popc(w.z) + __popc(w.w);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) n += __shfl_xor_sync(0xFFFFFFFFu, n, o);
+  if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = n;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    uint32_t v = ws[threadIdx.x];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+    if (threadIdx.x == 0) block_sum[blockIdx.x] = v;
+  }
+}
+
+// exclusive scan of block_sum[0..nb) in place, one block; total -> *total_out
+__global__ void __launch_bounds__(1024) mask_scan_blocks_kernel(uint32_t* __restrict__ block_sum, int nb, uint32_t* total_out) {
+  __shared__ uint32_t ws[32];
+  __shared__ uint32_t carry;
+  if (threadIdx.x == 0) carry = 0;
+  __syncthreads();
+  for (int base = 0; base < nb; base += 1024) {
+    const int i = base + threadIdx.x;
+    const uint32_t v = i < nb ? block_sum[i] : 0u;
+    uint32_t incl = v;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += x; }
+    if (lane == 31) ws[wid] = incl;
+    __syncthreads();
+    if (wid == 0) {
+      uint32_t x = ws[lane], ix = x;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xFFFFFFFFu, ix, o); if (lane >= o) ix += y; }
+      ws[lane] = ix - x;
+    }
+    __syncthreads();
+    const uint32_t excl = carry + ws[wid] + incl - v;
+    if (i < nb) block_sum[i] = excl;
+    __syncthreads();
+    if (threadIdx.x == 1023) carry = excl + v;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0 && total_out) *total_out = carry;
+}
+
+__global__ void __launch_bounds__(1024) mask_rank_idx_kernel(const uint32_t* __restrict__ bits, int64_t n_chunks,
+                                                            const uint32_t* __restrict__ block_off,
+                                                            uint32_t* __restrict__ rank128, int32_t* __restrict__ idx, int64_t idx_cap) {
+  __shared__ uint32_t ws[32];
+  const int64_t c = (int64_t)blockIdx.x * kCompactChunksPerBlock + threadIdx.x;
+  uint4 w = make_uint4(0, 0, 0, 0);
+  if (c < n_chunks) w = __ldg(reinterpret_cast<const uint4*>(bits) + c);
+  const uint32_t n = __popc(w.x) + __popc(w.y) + __popc(w.z) + __popc(w.w);
+  uint32_t incl = n;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += x; }
+  if (lane == 31) ws[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    uint32_t x = ws[lane], ix = x;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xFFFFFFFFu, ix, o); if (lane >= o) ix += y; }
+    ws[lane] = ix - x;
+  }
+  __syncthreads();
+  if (c >= n_chunks) return;
+  uint32_t j = block_off[blockIdx.x] + ws[wid] + incl - n;
+  rank128[c] = j;
+  if (idx == nullptr) return;
+  const uint32_t words[4] = {w.x, w.y, w.z, w.w};
+  const int64_t base = c << 7;
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    uint32_t x = words[q];
+    while (x) {
+      const int b = __ffs(x) - 1;
+      x &= x - 1;
+      if ((int64_t)j < idx_cap) idx[j] = (int32_t)(base + (q << 5) + b);
+      ++j;
+    }
+  }
+}
+
+// scatter / gather helpers for the dense <-> packed views used by the accessors
+__global__ void fill_u32_kernel(uint32_t* p, int64_t n, uint32_t v) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) p[i] = v;
+}
+
+__global__ void iota_i32_kernel(int32_t* p, int64_t n) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) p[i] = (int32_t)i;
+}
+
+// all-ones mask over [0,N), zero padding bits up to n_words*32
+__global__ void mask_all_ones_kernel(uint32_t* bits, int64_t n_words, int64_t N) {
+  for (int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; w < n_words; w += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t lo = w << 5;
+    uint32_t v = 0;
+    if (lo + 32 <= N) v = 0xFFFFFFFFu;
+    else if (lo < N) v = (1u << (uint32_t)(N - lo)) - 1u;
+    bits[w] = v;
+  }
+}
+
+// clear bits at positions >= N (after a user-supplied mask was copied in)
+__global__ void mask_clear_tail_kernel(uint32_t* bits, int64_t n_words, int64_t N) {
+  for (int64_t w = (N >> 5) + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; w < n_words; w += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t lo = w << 5;
+    if (lo >= N) bits[w] = 0;
+    else bits[w] &= (1u << (uint32_t)(N - lo)) - 1u;
+  }
+}
+
+}  // namespace scapek

@@ -1,0 +1,295 @@
+"""Parity of the CUDA path (through the C-ABI) against the CPU oracle — `-m gpu`.
+
+Bar (BASELINE.json north_star): from identical state each step, masks / indices / counts
+bit-exact (ties to the lower index) and fp32 theta, m, e within max relative error 1e-6; after
+100 chained steps theta within 1e-4 relative and masks agreeing on >= 99.99 % of entries.
+With the pinned operation order the expectation is 0 ulp, which the tests also report.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle.scape_oracle import ScapeOracle  # noqa: E402
+from paper_2607_01678_b200 import synth  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+HYP = dict(beta1=0.9, beta2=0.95, eps=1e-8, lr=1e-3, wd=0.1)
+REL_TOL = 1e-6          # north_star: per-step max relative error on fp32 state
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2607_01678_b200 import binding
+    binding.lib()       # raises if libscape.so is missing: no fallback
+    return binding
+
+
+def max_rel(a, b):
+    a = np.asarray(a, np.float64)
+    b = np.asarray(b, np.float64)
+    den = np.maximum(np.abs(a), np.abs(b))
+    with np.errstate(invalid="ignore", divide="ignore"):
+        r = np.where(den > 0, np.abs(a - b) / den, 0.0)
+    return float(r.max()) if r.size else 0.0
+
+
+def assert_close(a, b, what, tol=REL_TOL):
+    assert a.shape == b.shape, what
+    r = max_rel(a, b)
+    assert r <= tol, f"{what}: max rel err {r:.3e} > {tol}"
+
+
+def to_np32(g):
+    return g.detach().to(torch.float32).cpu().numpy()
+
+
+def load_state(gpu, ora, R):
+    """Copy the oracle's state (m, e^r, mask the coming step uses, t) into the CUDA handle."""
+    gpu.set_moment(ora.m())
+    for r in range(R):
+        gpu.set_residual(r, ora.e(r))
+    gpu.set_mask_next(ora.mask())
+    gpu.set_step_count(ora.t)
+
+
+def compare_step(gpu, ora, th_gpu, th_ora, R, tag, exact=True):
+    """Everything one step produces, GPU vs oracle."""
+    K = ora.K_last
+    assert gpu.count_last() == K, tag
+    np.testing.assert_array_equal(gpu.idx_last(), ora.idx(), err_msg=f"{tag} idx_last")
+    mk_g, mk_o = gpu.mask_next(), ora.mask()
+    np.testing.assert_array_equal(mk_g, mk_o, err_msg=f"{tag} mask_next")
+    assert gpu.count_next() == int(mk_o.sum()), tag
+    np.testing.assert_array_equal(gpu.idx_next(), np.nonzero(mk_o)[0].astype(np.int32), err_msg=f"{tag} idx_next")
+    th = th_gpu.cpu().numpy()
+    assert_close(th, th_ora, f"{tag} theta")
+    assert_close(gpu.moment(), ora.m(), f"{tag} m")
+    for r in range(R):
+        assert_close(gpu.residual(r), ora.e(r), f"{tag} e[{r}]")
+        assert_close(gpu.packed(r), ora.b(r), f"{tag} b[{r}]")
+    assert_close(gpu.packed_mean(), ora.bbar(), f"{tag} bbar")
+    if exact:   # the pinned operation order makes the two sides agree to the bit
+        assert np.array_equal(th.view(np.uint32), th_ora.view(np.uint32)), f"{tag} theta not bit-exact"
+        assert np.array_equal(gpu.moment().view(np.uint32), ora.m().view(np.uint32)), f"{tag} m not bit-exact"
+        for r in range(R):
+            assert np.array_equal(gpu.residual(r).view(np.uint32), ora.e(r).view(np.uint32)), f"{tag} e[{r}] not bit-exact"
+
+
+def run_reload_parity(B, w, steps, seed=0, hyp=HYP):
+    """Per-step parity 'when both start from identical state each step'."""
+    N, R = w.numel, w.R
+    gs = synth.GradStream(w, device="cuda", seed=seed)
+    th0 = gs.theta0()
+    gpu = B.Scape(N, R, w.sparsity, **hyp)
+    gpu.keep_dense_pack(True)
+    ora = ScapeOracle(N, R, w.sparsity, **hyp)
+    assert gpu.k == ora.k
+    th_ora = th0.cpu().numpy().copy()
+    for t in range(1, steps + 1):
+        grads = gs.next()
+        load_state(gpu, ora, R)
+        th_gpu = torch.from_numpy(th_ora.copy()).cuda()
+        gpu.step(th_gpu, grads)
+        ora.step(th_ora, [to_np32(g) for g in grads])
+        torch.cuda.synchronize()
+        compare_step(gpu, ora, th_gpu, th_ora, R, f"{w.name} step {t}")
+    gpu.close()
+
+
+# ------------------------------------------------------------------------------------------
+def test_config1_pr1_per_step_parity(B):
+    """BASELINE.json configs[0]: N = 2^20, R = 2, s = 0.9, 10 steps, seed 0."""
+    run_reload_parity(B, synth.workload("pr1"), steps=10, seed=0)
+
+
+def test_config1_pr1_chained_parity_is_exact(B):
+    """Same config, no reload: the GPU carries its own state for 10 steps."""
+    w = synth.workload("pr1")
+    N, R = w.numel, w.R
+    gs = synth.GradStream(w, device="cuda", seed=0)
+    th_gpu = gs.theta0()
+    th_ora = th_gpu.cpu().numpy().copy()
+    gpu = B.Scape(N, R, w.sparsity, **HYP)
+    gpu.keep_dense_pack(True)
+    ora = ScapeOracle(N, R, w.sparsity, **HYP)
+    for t in range(1, 11):
+        grads = gs.next()
+        gpu.step(th_gpu, grads)
+        ora.step(th_ora, [to_np32(g) for g in grads])
+        compare_step(gpu, ora, th_gpu, th_ora, R, f"chained step {t}")
+    gpu.close()
+
+
+def test_chained_100_steps(B):
+    """north_star: after 100 chained steps theta within 1e-4 relative, masks agree >= 99.99 %."""
+    w = synth.Workload("chain100", [("flat", 300_000 + 77)], R=3, sparsity=0.99, dist="t4", rho=0.9,
+                       grad_dtype="f32", steps=100, per_tensor_scale=False, const_scale=1e-3)
+    N, R = w.numel, w.R
+    gs = synth.GradStream(w, device="cuda", seed=5)
+    th_gpu = gs.theta0()
+    th_ora = th_gpu.cpu().numpy().copy()
+    gpu = B.Scape(N, R, w.sparsity, **HYP)
+    ora = ScapeOracle(N, R, w.sparsity, **HYP)
+    for _ in range(100):
+        grads = gs.next()
+        gpu.step(th_gpu, grads)
+        ora.step(th_ora, [to_np32(g) for g in grads])
+    agree = float((gpu.mask_next() == ora.mask()).mean())
+    assert agree >= 0.9999, agree
+    assert_close(th_gpu.cpu().numpy(), th_ora, "theta after 100 chained steps", tol=1e-4)
+    assert_close(gpu.moment(), ora.m(), "m after 100 chained steps", tol=1e-4)
+    gpu.close()
+
+
+@pytest.mark.parametrize("N,R,s,gdt", [
+    (1, 1, 0.0, "f32"), (3, 2, 0.5, "f32"), (127, 1, 0.9, "f32"), (128, 2, 0.9, "bf16"),
+    (129, 3, 0.99, "f32"), (1000, 4, 0.999, "bf16"), (4099, 5, 0.9, "f32"), (128 * 37 + 5, 8, 0.99, "bf16"),
+    (131072 + 1, 2, 0.5, "f32"), (200_003, 7, 0.9, "f32"), (150_000, 6, 0.0, "bf16"), (40_000, 4, 0.25, "f32"),
+])
+def test_ragged_sizes_replica_counts_and_dtypes(B, N, R, s, gdt):
+    w = synth.Workload(f"ragged{N}", [("a", N // 2), ("b", N - N // 2)], R=R, sparsity=s, dist="t3", rho=0.9,
+                       grad_dtype=gdt, steps=4)
+    run_reload_parity(B, w, steps=4, seed=N)
+
+
+@pytest.mark.parametrize("name,div", [("gpt345m", 256), ("llama500m", 256), ("llama1p8b", 512)])
+def test_scaled_model_shaped_shards(B, name, div):
+    """Configs 2-4 with every tensor `div` times smaller (same structure, scales, distributions)."""
+    w = synth.workload(name, div=div)
+    run_reload_parity(B, w, steps=3, seed=1)
+
+
+def test_crafted_ties_and_zeros(B):
+    """Quantised gradients: many exactly equal |m~| straddle the threshold; zero regions."""
+    rng = np.random.default_rng(0)
+    N, R, s = 10_000 + 13, 2, 0.9
+    gpu = B.Scape(N, R, s, **HYP)
+    gpu.keep_dense_pack(True)
+    ora = ScapeOracle(N, R, s, **HYP)
+    th_ora = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    th_gpu = torch.from_numpy(th_ora.copy()).cuda()
+    for t in range(1, 7):
+        base = (rng.integers(-3, 4, N) * 0.25).astype(np.float32)     # 7 distinct values
+        base[: N // 3] = 0.0                                          # a zero region
+        if t == 4:
+            base[:] = 0.5                                             # every key equal
+        if t == 5:
+            base[:] = 0.0                                             # all-zero gradients
+        grads = [torch.from_numpy(base.copy()).cuda() for _ in range(R)]
+        gpu.step(th_gpu, grads)
+        ora.step(th_ora, [base.copy() for _ in range(R)])
+        compare_step(gpu, ora, th_gpu, th_ora, R, f"ties step {t}")
+    gpu.close()
+
+
+def test_p9_worked_example_on_gpu(B):
+    with open(os.path.join(HERE, "golden", "p9_worked_example.json")) as f:
+        G = json.load(f)
+    gpu = B.Scape(G["N"], G["R"], G["sparsity"], G["beta1"], G["beta2"], G["eps"], G["lr"], G["wd"])
+    gpu.keep_dense_pack(True)
+    assert gpu.k == G["k"]
+    th = torch.tensor(G["theta0"], dtype=torch.float32, device="cuda")
+    for s in G["steps"]:
+        g = [torch.tensor(s[k], dtype=torch.float32, device="cuda") * G["grad_scale"] for k in ("g0", "g1")]
+        gpu.step(th, g)
+        np.testing.assert_array_equal(gpu.idx_last(), np.array(s["cur"], np.int32))
+        np.testing.assert_array_equal(np.nonzero(gpu.mask_next())[0], np.array(s["next"]))
+        np.testing.assert_array_equal(gpu.packed(0), np.array(s["b0"], np.float32))
+        np.testing.assert_array_equal(gpu.packed(1), np.array(s["b1"], np.float32))
+        np.testing.assert_array_equal(gpu.residual(0), np.array(s["e0_after"], np.float32))
+        np.testing.assert_array_equal(gpu.residual(1), np.array(s["e1_after"], np.float32))
+        np.testing.assert_array_equal(gpu.moment(), np.array(s["m_after"], np.float32))
+        np.testing.assert_allclose(th.cpu().numpy(), np.array(s["theta_after"], np.float32), rtol=1e-6, atol=0)
+    gpu.close()
+
+
+def test_sparsity_zero_stays_dense(B):
+    w = synth.Workload("dense", [("flat", 50_000 + 3)], R=2, sparsity=0.0, dist="gauss", rho=0.5,
+                       grad_dtype="f32", steps=3, per_tensor_scale=False)
+    run_reload_parity(B, w, steps=3)
+
+
+def test_api_errors(B):
+    import ctypes
+    L = B.lib()
+    assert not L.scape_create(0, 1, 0.5, 0.9, 0.95, 1e-8, 1e-3, 0.1)
+    assert "shard_numel" in B.scape_last_error()
+    assert not L.scape_create(1 << 31, 1, 0.5, 0.9, 0.95, 1e-8, 1e-3, 0.1)
+    assert not L.scape_create(16, 0, 0.5, 0.9, 0.95, 1e-8, 1e-3, 0.1)
+    assert not L.scape_create(16, 9, 0.5, 0.9, 0.95, 1e-8, 1e-3, 0.1)
+    assert not L.scape_create(16, 1, 1.0, 0.9, 0.95, 1e-8, 1e-3, 0.1)
+    assert not L.scape_create(16, 1, 0.5, 1.0, 0.95, 1e-8, 1e-3, 0.1)
+    assert not L.scape_create(16, 1, 0.5, 0.9, 0.95, -1.0, 1e-3, 0.1)
+    assert not L.scape_create(16, 1, float("nan"), 0.9, 0.95, 1e-8, 1e-3, 0.1)
+    g = B.Scape(1024, 2, 0.9)
+    th = torch.zeros(1024 + 4, device="cuda")
+    gr = [torch.zeros(1024, device="cuda") for _ in range(2)]
+    arr = (ctypes.c_void_p * 2)(*[x.data_ptr() for x in gr])
+    assert L.scape_step(g.h, th.data_ptr() + 4, arr, None) == B.SCAPE_EINVAL      # misaligned param
+    assert "aligned" in B.scape_last_error()
+    assert L.scape_step(None, th.data_ptr(), arr, None) == B.SCAPE_EINVAL
+    assert L.scape_step(g.h, None, arr, None) == B.SCAPE_EINVAL
+    assert g.t == 0                                                              # state unchanged
+    with pytest.raises(B.ScapeError):
+        g.packed(0)                                                              # no step has run yet
+    with pytest.raises(B.ScapeError):
+        B.scape_set_grad_dtype(g.h, 7)
+    L.scape_destroy(None)                                                        # NULL is a no-op
+    g.close()
+
+
+def test_step_host_matches_device_step(B):
+    w = synth.Workload("host", [("flat", 70_001)], R=2, sparsity=0.9, dist="gauss", rho=0.9,
+                       grad_dtype="bf16", steps=3, per_tensor_scale=False)
+    gs = synth.GradStream(w, device="cuda", seed=3)
+    th_d = gs.theta0()
+    th_h = th_d.cpu().pin_memory()
+    a, b = B.Scape(w.numel, w.R, w.sparsity), B.Scape(w.numel, w.R, w.sparsity)
+    for _ in range(3):
+        grads = gs.next()
+        a.step(th_d, grads)
+        b.step_host(th_h, [g.cpu().pin_memory() for g in grads])
+        torch.cuda.synchronize()
+        assert torch.equal(th_d.cpu(), th_h)
+        np.testing.assert_array_equal(a.mask_next(), b.mask_next())
+    a.close()
+    b.close()
+
+
+def test_cuda_graph_capture_of_a_step(B):
+    """scape_step allocates nothing and never synchronises, so it can be captured."""
+    w = synth.Workload("graph", [("flat", 100_000)], R=2, sparsity=0.9, dist="gauss", rho=0.9,
+                       grad_dtype="f32", steps=4, per_tensor_scale=False)
+    gs = synth.GradStream(w, device="cuda", seed=4)
+    th = gs.theta0()
+    th2 = th.clone()
+    ref, cap = B.Scape(w.numel, w.R, w.sparsity), B.Scape(w.numel, w.R, w.sparsity)
+    grads = gs.next()
+    for sc, p in ((ref, th), (cap, th2)):       # step 1 (dense) and 2 eagerly on both
+        sc.step(p, grads)
+        sc.step(p, grads)
+    # steps 3 and 4 use different internal buffers (mask double buffer): capture both
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(graph, stream=s):
+            cap.step(th2, grads)
+            cap.step(th2, grads)
+    torch.cuda.current_stream().wait_stream(s)
+    graph.replay()
+    ref.step(th, grads)
+    ref.step(th, grads)
+    torch.cuda.synchronize()
+    assert torch.equal(th, th2)
+    np.testing.assert_array_equal(ref.mask_next(), cap.mask_next())
+    ref.close()
+    cap.close()
