@@ -1,0 +1,360 @@
+#!/usr/bin/env python
+"""bench.py — SCAPE step throughput on B200 (BASELINE.json `metric`): params/s, step ms and
+achieved HBM GB/s against the measured peak.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload llama1p8b] [--impl reference]
+
+A "step" is one pass of the whole hot path (scape_step: stages 1-6 of the north star) over one
+seeded synthetic gradient set of the workload's shape.  The default workload is the Llama-1.8B-
+shaped shard (R = 4 bf16 gradient buffers, 99 % sparsity), the configuration the headline bar
+is quoted on; it fits one GPU.  Inputs (~50 GB) are far larger than L2, so no flush is needed
+between steps.  The path does not shard across GPUs ("replicas only"):
+with --gpus N each rank runs an independent replica of the same workload, no collective on the
+data path; `value` = params all ranks processed / max-over-ranks device time ("weak").
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle instead (a deliberately
+plain program: the ratio against it is not the headline; parity and roofline.frac are).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "scape_step_params_per_s"
+UNIT = "params/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="llama1p8b",
+                    help="pr1 | gpt345m | llama500m | llama1p8b | llama1p8b_literal | sweep:<log2n>:<sparsity>:<R>")
+    ap.add_argument("--div", type=int, default=1, help="shrink every tensor by this factor")
+    ap.add_argument("--sparsity", type=float, default=None)
+    ap.add_argument("--sets", type=int, default=4, help="distinct consecutive gradient sets kept resident and cycled")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-div", type=int, default=64, help="oracle sample: every tensor this many times smaller")
+    ap.add_argument("--cpu-steps", type=int, default=3)
+    ap.add_argument("--seed", type=int, default=0)
+    return ap.parse_args()
+
+
+def get_workload(args):
+    from paper_2607_01678_b200 import synth
+    if args.workload.startswith("sweep:"):
+        _, l2, s, r = args.workload.split(":")
+        return synth.sweep_point(int(l2), float(s), int(r))
+    return synth.workload(args.workload, div=args.div, sparsity=args.sparsity)
+
+
+# ---------------------------------------------------------------------------------------------
+# algorithmic bytes
+# ---------------------------------------------------------------------------------------------
+def grad_bytes(w):
+    return 2 if w.grad_dtype == "bf16" else 4
+
+
+def bytes_per_param_fused(w, k, N):
+    """Fused streaming kernel, steady state: reads theta, m, g^r, e^r, mask bits, rank128; writes
+    theta, m, e^r, b^r, b-bar."""
+    G, R, d = grad_bytes(w), w.R, k / N
+    return (G + 8) * R + 16 + 4 * d * (R + 1) + 1 / 8 + 4 / 128
+
+
+def bytes_per_param_step(w, k, N):
+    """Whole step, the method's own traffic with dense m (SURVEY.md §8(d) B_dense)."""
+    G, R, d = grad_bytes(w), w.R, k / N
+    return (G + 8) * R + 16 + 8 * d + 4 * d * R + 1 / 4
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def recorded_traffic(workload_name):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed
+    `ncu --set full` capture (profiles/traffic.json), or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(workload_name, {}).get("fused_dram_bytes_per_launch")
+    except Exception:
+        return None
+
+
+# ---------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md recipe)
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100", "-i", str(self.index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        os.unlink(self.f.name)
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ---------------------------------------------------------------------------------------------
+# the CPU oracle as a timed baseline (bounded sample)
+# ---------------------------------------------------------------------------------------------
+def time_oracle(args, steps, warmup, div):
+    """Runs oracle/ as it stands, single-threaded, on the same workload with every tensor `div`
+    times smaller.  Returns (params_per_s, ms_per_step, sample description, N_sample)."""
+    import numpy as np
+    import torch
+    from oracle.scape_oracle import ScapeOracle
+    from paper_2607_01678_b200 import synth
+    wl = args.workload
+    if wl.startswith("sweep:"):
+        w = get_workload(args)
+    else:
+        w = synth.workload(wl, div=max(div, args.div), sparsity=args.sparsity)
+    gs = synth.GradStream(w, device="cpu", seed=args.seed)
+    th = gs.theta0().numpy().copy()
+    ora = ScapeOracle(w.numel, w.R, w.sparsity, **w.hyper)
+    # the first step of Alg. 1 is dense (M_0 = 1); it is always part of the warm-up
+    total = 0.0
+    for i in range(1 + warmup + steps):
+        grads = [g.to(torch.float32).numpy() for g in gs.next()]
+        t0 = time.perf_counter()
+        ora.step(th, grads)
+        dt = time.perf_counter() - t0
+        if i >= 1 + warmup:
+            total += dt
+    ms = 1e3 * total / steps
+    desc = (f"{w.name}: N={w.numel} (every tensor /{max(div, args.div)}), R={w.R}, sparsity={w.sparsity}, "
+            f"{steps} steady-state steps after {1 + warmup} warm-up (incl. the dense first step); "
+            f"oracle/scape_oracle.cpp -O2 -ffp-contract=off, 1 thread")
+    return w.numel * steps / total, ms, desc, w.numel
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = get_workload(args)
+    pps, ms, desc, n = time_oracle(args, steps=max(1, args.steps), warmup=max(0, args.warmup), div=args.cpu_div)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": pps, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic (seeded)",
+        "config": {"workload": w.name, "R": w.R, "sparsity": w.sparsity, "grad_dtype": w.grad_dtype,
+                   "sample": desc},
+        "cpu_baseline": {"value": pps, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
+                         "host_cores": os.cpu_count()},
+        "e2e": {"value": pps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2607_01678_b200 import binding, synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    binding.lib()
+
+    w = get_workload(args)
+    N, R = w.numel, w.R
+    K, W = args.steps, max(args.warmup, 3)
+    dev = torch.device("cuda", local)
+
+    # ---- inputs resident in HBM before the timed region --------------------------------
+    gs = synth.GradStream(w, device=dev, seed=args.seed + rank)
+    theta = gs.theta0()
+    n_sets = max(1, min(args.sets, K + W + 1))
+    ring = [gs.next() for _ in range(n_sets)]
+    del gs
+    torch.cuda.empty_cache()
+
+    sc = binding.Scape(N, R, w.sparsity, **w.hyper)
+    k = sc.k
+    # the first step of Alg. 1 is dense (M_0 = 1): always warm-up, reported separately
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); sc.step(theta, ring[0]); e1.record(); torch.cuda.synchronize()
+    first_step_ms = e0.elapsed_time(e1)
+    for i in range(W):
+        sc.step(theta, ring[(1 + i) % n_sets])
+    torch.cuda.synchronize()
+
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()
+    sc.profile(True)
+    launches0 = sc.launches
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for i in range(K):
+        sc.step(theta, ring[(1 + W + i) % n_sets])
+    t1.record()
+    torch.cuda.synchronize()
+    elapsed_ms = t0.elapsed_time(t1)
+    fused_ms, select_ms, psteps = sc.profile_read()
+    sc.profile(False)
+    gpu_launches = sc.launches - launches0
+    clk = clocks.stop() if rank == 0 else None
+    if world > 1:
+        tt = torch.tensor([elapsed_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        elapsed_ms = float(tt.item())
+        dist.barrier()
+    assert bool(torch.isfinite(theta).all()), "theta is not finite after the timed steps"
+    mask_count = sc.count_next()
+    assert mask_count == k, (mask_count, k)
+
+    ms_per_step = elapsed_ms / K
+    value = world * N * K / (elapsed_ms * 1e-3)
+
+    # ---- roofline of the dominant kernel -------------------------------------------------
+    peak, peak_src = measured_peak()
+    fused_avg_ms = fused_ms / max(1, psteps)
+    fb = bytes_per_param_fused(w, k, N) * N
+    achieved = fb / (fused_avg_ms * 1e-3) / 1e9
+    sb = bytes_per_param_step(w, k, N) * N
+    roofline = {
+        "bound": "hbm", "kernel": "scape_fused_step_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+        "frac": achieved / peak, "traffic": recorded_traffic(w.name),
+        "peak_source": peak_src, "algorithmic_bytes_per_launch": fb, "kernel_ms": fused_avg_ms,
+        "kernel_share_of_step": fused_avg_ms / ms_per_step,
+        "select_ms": select_ms / max(1, psteps),
+        "step_algorithmic_bytes": sb, "step_gbs": sb / (ms_per_step * 1e-3) / 1e9,
+        "step_frac_of_peak": sb / (ms_per_step * 1e-3) / 1e9 / peak,
+        "step_frac_of_8TBs_nominal": sb / (ms_per_step * 1e-3) / 1e9 / 8000.0,
+    }
+
+    sc.close()
+    del ring, sc
+    torch.cuda.empty_cache()
+
+    # ---- end to end through the C-ABI with HOST buffers ---------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        gs = synth.GradStream(w, device=dev, seed=args.seed + rank)
+        th_h = gs.theta0().cpu().pin_memory()
+        g_h = [g.cpu().pin_memory() for g in gs.next()]
+        del gs
+        torch.cuda.empty_cache()
+        sh = binding.Scape(N, R, w.sparsity, **w.hyper)
+        for _ in range(2):                       # dense first step + one sparse step: warm-up
+            sh.step_host(th_h, g_h)
+        n_e2e = max(1, args.e2e_steps)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(n_e2e):
+            sh.step_host(th_h, g_h)
+        b.record()
+        torch.cuda.synchronize()
+        e2e_ms = a.elapsed_time(b)
+        if world > 1:
+            tt = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            e2e_ms = float(tt.item())
+        gbytes = N * grad_bytes(w) * R
+        e2e = {"value": world * N * n_e2e / (e2e_ms * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": 4 * N + gbytes, "d2h_bytes_per_step": 4 * N,
+               "steps": n_e2e, "ms_per_step": e2e_ms / n_e2e,
+               "api": "scape_step_host (pinned host param + R gradient buffers in, param out)"}
+        sh.close()
+        del sh, th_h, g_h
+
+    # ---- the oracle on the host cores, bounded sample (rank 0, N = 1 only) --------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        pps, cms, desc, _ = time_oracle(args, steps=args.cpu_steps, warmup=1, div=args.cpu_div)
+        cpu = {"value": pps, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
+               "ms_per_step_on_sample": cms, "host_cores": os.cpu_count()}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic (seeded; shapes and distributions of BASELINE.json configs)",
+            "config": {"workload": w.name, "shard_numel": N, "R": R, "sparsity": w.sparsity, "k": k,
+                       "grad_dtype": w.grad_dtype, "dist": w.dist, "ar1_rho": w.rho, "hyper": w.hyper,
+                       "gradient_sets_cycled": n_sets, "l2": "inputs (tens of GB) exceed the 126 MB L2; no flush needed",
+                       "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU",
+                       "first_dense_step_ms": first_step_ms},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": gpu_launches, "clocks": clk,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -113,11 +113,26 @@ int scape_set_keep_dense_pack(scape_t* h, int on);
  * may be a host or a device pointer (unified addressing); `bytes` must equal the size of the
  * selected object; `r` is the replica for SCAPE_RESIDUAL / SCAPE_PACKED and ignored otherwise.
  * Both calls synchronise `cuda_stream` before returning.  Not part of the timed path.
- * scape_set(SCAPE_MASK_NEXT) accepts any mask with at most max(k, count) ... precisely: with
- * at most k set bits, or all N bits set; bits at positions >= N are ignored.                    */
+ * scape_set(SCAPE_MASK_NEXT) accepts a mask with at most k set bits, or with all N bits set;
+ * bits at positions >= N are ignored.                                                          */
 int scape_get(scape_t* h, int what, int r, void* buf, size_t bytes, void* cuda_stream);
 int scape_set(scape_t* h, int what, int r, const void* buf, size_t bytes, void* cuda_stream);
 int scape_set_step_count(scape_t* h, int64_t t);
+
+/* How often the stage-2 select could use the candidate list gathered by the fused pass (the
+ * threshold predicted from the previous step bracketed the true one: `fast`) and how often it
+ * fell back to radix passes over the whole partition (`general`; always the case on all-ones
+ * steps).  Both routes are exact.  Synchronises cuda_stream.                                     */
+int scape_select_stats(scape_t* h, int64_t* fast, int64_t* general, void* cuda_stream);
+
+/* Optional timing, for bench.py's roofline: while switched on, every scape_step also records
+ * three CUDA events on its stream (before the fused streaming kernel of stages 1,3-6, after it,
+ * and after the stage-2 select), at most 64 steps between reads without a host wait.
+ * scape_profile(h, on) resets the totals.  scape_profile_read waits for the recorded events and
+ * returns the summed milliseconds of the fused kernel and of the select stage and the number of
+ * steps they cover (any pointer may be NULL).                                                   */
+int scape_profile(scape_t* h, int on);
+int scape_profile_read(scape_t* h, double* fused_ms, double* select_ms, int64_t* steps);
 
 /* Message of the last failure on the calling thread ("" if none).  Never NULL.                 */
 const char* scape_last_error(void);

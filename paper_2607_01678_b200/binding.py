@@ -35,6 +35,9 @@ SYMBOLS = {
     "scape_get": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
     "scape_set": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
     "scape_set_step_count": (_I, [_VP, _I64]),
+    "scape_select_stats": (_I, [_VP, _VP, _VP, _VP]),
+    "scape_profile": (_I, [_VP, _I]),
+    "scape_profile_read": (_I, [_VP, _VP, _VP, _VP]),
     "scape_last_error": (ctypes.c_char_p, []),
 }
 
@@ -128,6 +131,24 @@ def scape_get(h, what, r, buf_ptr, nbytes, stream=0):
 
 def scape_set(h, what, r, buf_ptr, nbytes, stream=0):
     _check(lib().scape_set(h, what, r, buf_ptr, nbytes, stream), "scape_set")
+
+
+def scape_select_stats(h, stream=0):
+    """-> (steps whose select used the fused candidate list, steps that took the general path)"""
+    a, b = ctypes.c_int64(), ctypes.c_int64()
+    _check(lib().scape_select_stats(h, ctypes.byref(a), ctypes.byref(b), stream), "scape_select_stats")
+    return a.value, b.value
+
+
+def scape_profile(h, on):
+    _check(lib().scape_profile(h, int(on)), "scape_profile")
+
+
+def scape_profile_read(h):
+    """-> (fused_ms_total, select_ms_total, steps)"""
+    a, b, n = ctypes.c_double(), ctypes.c_double(), ctypes.c_int64()
+    _check(lib().scape_profile_read(h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(n)), "scape_profile_read")
+    return a.value, b.value, n.value
 
 
 class Scape:
@@ -252,3 +273,12 @@ class Scape:
 
     def set_step_count(self, t):
         scape_set_step_count(self.h, t)
+
+    def select_stats(self):
+        return scape_select_stats(self.h, self._stream())
+
+    def profile(self, on=True):
+        scape_profile(self.h, on)
+
+    def profile_read(self):
+        return scape_profile_read(self.h)

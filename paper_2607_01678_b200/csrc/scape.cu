@@ -69,10 +69,26 @@ struct scape {
   bool last_dense = false;
 
   SelState* sel = nullptr;
+  unsigned long long* cand = nullptr;   // [cand_cap] candidate composite keys of the fused select
+  int64_t cand_cap = 0;
+  uint32_t* seg_count = nullptr;  // [max_seg]
+  uint32_t* seg_above = nullptr;  // [max_seg]
+  int max_seg = 0;
   uint32_t* ghist = nullptr;      // [kBins]
   uint32_t* block_sum = nullptr;  // [n_compact_blocks]
   uint32_t* total = nullptr;      // [1]
   int n_compact_blocks = 0;
+  int n_seg = 0;                  // segments (= warps) of the last fused launch
+  uint32_t seg_cap = 0;
+
+  // optional per-step CUDA-event timing of the fused kernel and of the select stage
+  bool prof_on = false;
+  static constexpr int kProfRing = 64;
+  cudaEvent_t prof_ev[kProfRing][3] = {};
+  bool prof_have_events = false;
+  int prof_pending = 0;              // steps recorded since the last drain
+  double prof_fused_ms = 0.0, prof_select_ms = 0.0;
+  int64_t prof_steps = 0;
 
   // scape_step_host staging
   float* st_param = nullptr;
@@ -90,14 +106,20 @@ int grid_for(const scape* h, int64_t n_chunks, int warps_per_block, int blocks_p
 }
 
 template <typename G, int R, bool DENSE>
-int launch_fused_t(scape* h, const StepParams& p, cudaStream_t st) {
+int launch_fused_t(scape* h, StepParams& p, cudaStream_t st) {
   static int bps = 0;   // resident blocks per SM of this instantiation
   if (bps == 0) {
     int v = 0;
     CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, scape_fused_step_kernel<G, R, DENSE>, 256, 0));
-    bps = v > 0 ? v : 1;
+    bps = v > 0 ? (v > 8 ? 8 : v) : 1;
   }
   const int grid = grid_for(h, p.n_chunks, 8, bps);
+  // one candidate segment per warp of this launch
+  h->n_seg = grid * 8;
+  int64_t cap = (h->cand_cap / h->n_seg) & ~(int64_t)15;
+  if (cap > 0x7FFFFFF0) cap = 0x7FFFFFF0;
+  h->seg_cap = (uint32_t)cap;
+  p.seg_cap = h->seg_cap;
   scape_fused_step_kernel<G, R, DENSE><<<grid, 256, 0, st>>>(p);
   h->launches++;
   CU_TRY(cudaGetLastError());
@@ -105,7 +127,7 @@ int launch_fused_t(scape* h, const StepParams& p, cudaStream_t st) {
 }
 
 template <typename G, bool DENSE>
-int launch_fused_r(scape* h, const StepParams& p, cudaStream_t st) {
+int launch_fused_r(scape* h, StepParams& p, cudaStream_t st) {
   switch (h->R) {
     case 1: return launch_fused_t<G, 1, DENSE>(h, p, st);
     case 2: return launch_fused_t<G, 2, DENSE>(h, p, st);
@@ -119,7 +141,7 @@ int launch_fused_r(scape* h, const StepParams& p, cudaStream_t st) {
   return fail(SCAPE_EINVAL, "R out of range");
 }
 
-int launch_fused(scape* h, const StepParams& p, bool dense, cudaStream_t st) {
+int launch_fused(scape* h, StepParams& p, bool dense, cudaStream_t st) {
   if (h->grad_dtype == SCAPE_GRAD_BF16)
     return dense ? launch_fused_r<__nv_bfloat16, true>(h, p, st) : launch_fused_r<__nv_bfloat16, false>(h, p, st);
   return dense ? launch_fused_r<float, true>(h, p, st) : launch_fused_r<float, false>(h, p, st);
@@ -137,8 +159,10 @@ int compact_mask(scape* h, MaskSlot& s, bool want_idx, cudaStream_t st) {
   return SCAPE_OK;
 }
 
-// Stage 2 (Alg. 1 l.11): exact top-k of |m~^0| -> nxt.bits / rank / idx.
-int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, cudaStream_t st) {
+// Stage 2 (Alg. 1 l.11): exact top-k of |m~^0| -> nxt.bits / rank / idx.  When the fused pass ran
+// with a predicted bracket (sparse step) the radix select works on its candidate list if the
+// bracket held; otherwise (or on all-ones steps: force_general) on every key of the partition.
+int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st) {
   KeySrc src;
   src.e0 = h->e;
   src.cur_bits = cur.all_ones ? nullptr : cur.bits;
@@ -146,17 +170,20 @@ int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, cudaStream_t st) {
   src.packed0 = h->packed;
   src.N = h->N;
   src.n_chunks = h->n_chunks;
+  CandList cl;
+  cl.cand = h->cand; cl.seg_count = h->seg_count; cl.seg_above = h->seg_above;
+  cl.seg_cap = h->seg_cap; cl.n_seg = force_general ? 0 : h->n_seg;
   const int grid = grid_for(h, h->n_chunks, 8, 6);
-  sel_init_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist, (long long)h->k);
+  sel_decide_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist, cl, (long long)h->k, force_general ? 1 : 0);
   h->launches++;
   static const int shifts[kSelPasses] = {51, 38, 25, 12, 0};
   static const int widths[kSelPasses] = {13, 13, 13, 13, 12};
   for (int p = 0; p < kSelPasses; ++p) {
-    sel_hist_dense_kernel<<<grid, 256, 0, st>>>(src, h->sel, h->ghist, shifts[p], widths[p]);
-    sel_pick_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist, shifts[p], widths[p]);
+    sel_hist_kernel<<<grid, 256, 0, st>>>(src, cl, h->sel, h->ghist, shifts[p], widths[p]);
+    sel_pick_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist, shifts[p], widths[p], p == kSelPasses - 1);
     h->launches += 2;
   }
-  sel_write_mask_dense_kernel<<<grid, 256, 0, st>>>(src, h->sel, nxt.bits);
+  sel_finish_kernel<<<grid, 256, 0, st>>>(src, cl, h->sel, nxt.bits);
   h->launches++;
   CU_TRY(cudaGetLastError());
   int rc = compact_mask(h, nxt, true, st);
@@ -164,6 +191,19 @@ int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, cudaStream_t st) {
   nxt.count = h->k;
   nxt.all_ones = false;
   nxt.valid = true;
+  return SCAPE_OK;
+}
+
+// fold the recorded event pairs into the running totals (synchronises on the events)
+int prof_drain(scape* h) {
+  for (int i = 0; i < h->prof_pending; ++i) {
+    float a = 0.f, b = 0.f;
+    CU_TRY(cudaEventSynchronize(h->prof_ev[i][2]));
+    CU_TRY(cudaEventElapsedTime(&a, h->prof_ev[i][0], h->prof_ev[i][1]));
+    CU_TRY(cudaEventElapsedTime(&b, h->prof_ev[i][1], h->prof_ev[i][2]));
+    h->prof_fused_ms += a; h->prof_select_ms += b; h->prof_steps += 1;
+  }
+  h->prof_pending = 0;
   return SCAPE_OK;
 }
 
@@ -176,9 +216,11 @@ void free_all(scape* h) {
   cudaFree(h->m); cudaFree(h->e);
   for (auto& s : h->slot) { cudaFree(s.bits); cudaFree(s.rank); cudaFree(s.idx); }
   cudaFree(h->packed); cudaFree(h->packed_mean); cudaFree(h->dense_pack);
-  cudaFree(h->sel); cudaFree(h->ghist); cudaFree(h->block_sum); cudaFree(h->total);
+  cudaFree(h->sel); cudaFree(h->cand); cudaFree(h->seg_count); cudaFree(h->seg_above); cudaFree(h->ghist); cudaFree(h->block_sum); cudaFree(h->total);
   cudaFree(h->st_param);
   for (auto& g : h->st_grad) cudaFree(g);
+  if (h->prof_have_events)
+    for (auto& row : h->prof_ev) for (auto& ev : row) cudaEventDestroy(ev);
 }
 
 }  // namespace
@@ -231,12 +273,33 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
     alloc((void**)&h->packed_mean, sizeof(float) * h->packed_stride, true);
   }
   alloc((void**)&h->sel, sizeof(SelState), true);
+  if (sparse) {
+    // candidates of the fused select: room for ~4k keys (bracket of +-25 % around the threshold
+    // holds ~1.5k for power-law tails), never more than N/2, never fewer than 64 Ki
+    int64_t cc = 4 * h->k;
+    if (cc > N / 2) cc = N / 2;
+    if (cc < 65536) cc = 65536;
+    h->cand_cap = cc;
+    h->max_seg = h->n_sm * 8 * 8;
+    alloc((void**)&h->cand, sizeof(unsigned long long) * (size_t)cc, false);
+    alloc((void**)&h->seg_count, sizeof(uint32_t) * h->max_seg, true);
+    alloc((void**)&h->seg_above, sizeof(uint32_t) * h->max_seg, true);
+  }
   alloc((void**)&h->ghist, sizeof(uint32_t) * kBins, true);
   alloc((void**)&h->block_sum, sizeof(uint32_t) * (h->n_compact_blocks + 1), true);
   alloc((void**)&h->total, sizeof(uint32_t), true);
   if (!ok) {
     fail(SCAPE_ENOMEM, "device allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
     free_all(h); delete h; return nullptr;
+  }
+  {
+    SelState init{};
+    init.delta = 0.5f;                     // no history yet: wide first bracket
+    init.lo_key = init.hi_key = 0xFFFFFFFFu;   // nothing predicted: the first sparse step decides "general"
+    if (cudaMemcpy(h->sel, &init, sizeof init, cudaMemcpyHostToDevice) != cudaSuccess) {
+      fail(SCAPE_ECUDA, "create: cannot initialise the select state");
+      free_all(h); delete h; return nullptr;
+    }
   }
   h->slot[0].all_ones = true;                                                // l.1: M_0 = 1
   h->slot[0].count = N;
@@ -329,20 +392,64 @@ extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, vo
   p.R_f = (float)h->R; p.inv_R = 1.0f / (float)h->R;
   p.r_pow2 = (h->R & (h->R - 1)) == 0;      // x / 2^n == x * 2^-n bit for bit
   p.stash = cur.all_ones && need_select;
+  p.ctl = h->sel; p.next_bits = nxt.bits; p.cand = h->cand;
+  p.seg_count = h->seg_count; p.seg_above = h->seg_above;
 
+  const bool prof = h->prof_on;
+  if (prof && h->prof_pending == scape::kProfRing) { int prc = prof_drain(h); if (prc) return prc; }
+  const int pi = h->prof_pending;
+  if (prof) CU_TRY(cudaEventRecord(h->prof_ev[pi][0], st));
   int rc = launch_fused(h, p, cur.all_ones, st);
   if (rc) return rc;
+  if (prof) CU_TRY(cudaEventRecord(h->prof_ev[pi][1], st));
 
   if (need_select) {
-    rc = run_select(h, cur, nxt, st);
+    rc = run_select(h, cur, nxt, /*force_general=*/cur.all_ones, st);
     if (rc) return rc;
     if (cur.all_ones) CU_TRY(cudaMemsetAsync(h->e, 0, sizeof(float) * h->Npad, st));   // l.8 for e^0 after the stash
   } else {
     nxt.all_ones = true; nxt.count = h->N; nxt.valid = true;                            // k = N: M_t = 1
   }
+  if (prof) { CU_TRY(cudaEventRecord(h->prof_ev[pi][2], st)); h->prof_pending = pi + 1; }
   h->last_dense = cur.all_ones;
   h->use = 1 - h->use;
   h->t += 1;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_select_stats(scape_t* h, int64_t* fast, int64_t* general, void* cuda_stream) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  DeviceGuard guard(h->dev);
+  SelState s{};
+  CU_TRY(cudaMemcpyAsync(&s, h->sel, sizeof s, cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
+  CU_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+  if (fast) *fast = (int64_t)s.n_fast;
+  if (general) *general = (int64_t)s.n_general;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_profile(scape_t* h, int on) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  DeviceGuard guard(h->dev);
+  if (on && !h->prof_have_events) {
+    for (auto& row : h->prof_ev) for (auto& ev : row) CU_TRY(cudaEventCreate(&ev));
+    h->prof_have_events = true;
+  }
+  if (h->prof_on) { int rc = prof_drain(h); if (rc) return rc; }
+  h->prof_on = on != 0;
+  h->prof_fused_ms = h->prof_select_ms = 0.0;
+  h->prof_steps = 0;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_profile_read(scape_t* h, double* fused_ms, double* select_ms, int64_t* steps) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  DeviceGuard guard(h->dev);
+  int rc = prof_drain(h);
+  if (rc) return rc;
+  if (fused_ms) *fused_ms = h->prof_fused_ms;
+  if (select_ms) *select_ms = h->prof_select_ms;
+  if (steps) *steps = h->prof_steps;
   return SCAPE_OK;
 }
 

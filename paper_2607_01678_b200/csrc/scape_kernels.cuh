@@ -23,6 +23,22 @@ constexpr int kDigitBits = 13;       // radix-select digit width
 constexpr int kBins = 1 << kDigitBits;
 constexpr int kSelPasses = 5;        // 64-bit composite key = 13+13+13+13+12 bits
 
+// Device-resident control block of the stage-2 select (never read by the host on the timed path).
+struct SelState {
+  unsigned long long prefix;  // digits of T64 fixed so far
+  unsigned long long himask;  // mask of those digits
+  long long rank;             // rank (1-based from the top) still sought inside the prefix class
+  // predicted bracket for the COMING step's fused pass: key >= hi_key is certainly selected,
+  // lo_key <= key < hi_key is a candidate, key < lo_key is certainly not selected
+  uint32_t lo_key, hi_key;
+  float delta;                // relative half-width of the bracket
+  float T_prev;               // last exact threshold |m~| value
+  int have_T;
+  int hit;                    // this step: 1 = the bracket held (candidate list), 0 = general path
+  unsigned long long n_fast, n_general;   // statistics (scape_select_stats)
+  unsigned long long n_above, n_cand;     // this step's counts from the fused pass
+};
+
 struct StepParams {
   float* theta;                 // [N] caller-owned
   float* m;                     // [Npad]
@@ -40,6 +56,13 @@ struct StepParams {
   float R_f, inv_R;
   int r_pow2;
   int stash;                    // DENSE only: leave m~^0 in e^0 (keys for the select), not 0
+  // stage 2 fused into the pass (sparse variant only)
+  const SelState* ctl;          // bracket predicted by the previous step
+  uint32_t* next_bits;          // [Npad/32] certainly-selected bits of M_t (complete overwrite)
+  unsigned long long* cand;     // [n_seg][seg_cap] candidate composite keys, one segment per warp
+  uint32_t* seg_count;          // [n_seg] candidates this warp saw (may exceed seg_cap: overflow)
+  uint32_t* seg_above;          // [n_seg] certainly-selected entries this warp saw
+  uint32_t seg_cap;
 };
 
 // ------------------------------------------------------------------------------------------
@@ -103,8 +126,15 @@ __device__ __forceinline__ void lane_mask_bits(const uint32_t* __restrict__ bits
 // ------------------------------------------------------------------------------------------
 // Stages 1, 3, 4, 5, 6 fused: one streaming pass (Alg. 1 l.6-10, l.12-17).
 // ------------------------------------------------------------------------------------------
+struct StageA {                 // per-warp running state of the fused select (registers)
+  uint32_t lo, hi;              // bracket keys
+  uint32_t n_above;             // per lane
+  uint32_t cursor;              // warp-uniform: candidates appended so far
+  unsigned long long* seg;      // this warp's candidate segment
+};
+
 template <typename G, int R, bool DENSE, bool GUARD>
-__device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int lane) {
+__device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int lane, StageA& sa) {
   const int64_t i0 = (c << 7) + ((int64_t)lane << 2);
   uint32_t mybits = 0xFu, jbase = 0;
   if (!DENSE) lane_mask_bits(p.cur_bits, p.cur_rank, c, lane, mybits, jbase);
@@ -119,6 +149,7 @@ __device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int 
   }
 
   float mn[4];
+  uint32_t key0[4];             // bits(|m~^0|): the selection statistic of l.11
 #pragma unroll
   for (int q = 0; q < 4; ++q) {
     const bool on = DENSE || ((mybits >> q) & 1u);
@@ -128,6 +159,7 @@ __device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int 
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       const float mt = __fadd_rn(__fmaf_rn(p.c1, gg[r][q], pq), ee[r][q]);   // l.6
+      if (r == 0) key0[q] = __float_as_uint(mt) & 0x7FFFFFFFu;
       ee[r][q] = on ? ((DENSE && r == 0 && p.stash) ? mt : 0.0f) : mt;       // l.7-8
       if (on) {
         if (!DENSE || p.packed != nullptr) {
@@ -154,6 +186,32 @@ __device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int 
   store4_f32<false>(p.m, i0, p.N, mn);
 #pragma unroll
   for (int r = 0; r < R; ++r) store4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
+
+  if (!DENSE) {
+    // Stage 2 (l.11) fused: classify |m~^0| against the predicted bracket.  Exactness does not
+    // depend on the prediction: sel_decide_kernel checks n_above < k <= n_above + n_cand.
+    uint32_t nib = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const bool valid = !GUARD || (i0 + q < p.N);
+      const bool above = valid && key0[q] >= sa.hi;
+      const bool cnd = valid && !above && key0[q] >= sa.lo;
+      nib |= above ? (1u << q) : 0u;
+      const uint32_t bal = __ballot_sync(0xFFFFFFFFu, cnd);
+      if (cnd) {
+        const uint32_t pos = sa.cursor + __popc(bal & ((1u << lane) - 1u));
+        if (pos < p.seg_cap)
+          sa.seg[pos] = ((unsigned long long)key0[q] << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)(i0 + q));
+      }
+      sa.cursor += __popc(bal);
+    }
+    sa.n_above += __popc(nib);
+    uint32_t w = nib << ((lane & 7) << 2);
+    w |= __shfl_xor_sync(0xFFFFFFFFu, w, 1);
+    w |= __shfl_xor_sync(0xFFFFFFFFu, w, 2);
+    w |= __shfl_xor_sync(0xFFFFFFFFu, w, 4);
+    if ((lane & 7) == 0) p.next_bits[(c << 2) + (lane >> 3)] = w;
+  }
 }
 
 template <typename G, int R, bool DENSE>
@@ -163,8 +221,19 @@ __global__ void __launch_bounds__(256) scape_fused_step_kernel(const __grid_cons
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
   const int64_t nwarps = (int64_t)gridDim.x * wpb;
   const int64_t full = p.N >> 7;
-  for (int64_t c = warp; c < full; c += nwarps) fused_chunk<G, R, DENSE, false>(p, c, lane);
-  if (full < p.n_chunks && warp == full % nwarps) fused_chunk<G, R, DENSE, true>(p, full, lane);
+  StageA sa{};
+  if (!DENSE) {
+    sa.lo = p.ctl->lo_key; sa.hi = p.ctl->hi_key;
+    sa.seg = p.cand + (size_t)warp * p.seg_cap;
+  }
+  for (int64_t c = warp; c < full; c += nwarps) fused_chunk<G, R, DENSE, false>(p, c, lane, sa);
+  if (full < p.n_chunks && warp == full % nwarps) fused_chunk<G, R, DENSE, true>(p, full, lane, sa);
+  if (!DENSE) {
+    uint32_t na = sa.n_above;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
+    if (lane == 0) { p.seg_count[warp] = sa.cursor; p.seg_above[warp] = na; }
+  }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -182,13 +251,6 @@ struct KeySrc {
   const float* packed0;       // b^0
   int64_t N;
   int64_t n_chunks;
-};
-
-struct SelState {
-  unsigned long long prefix;  // digits fixed so far
-  unsigned long long himask;  // mask of those digits
-  long long rank;             // rank (1-based from the top) still sought inside the prefix class
-  int pad[2];
 };
 
 __device__ __forceinline__ unsigned long long make_k64(float x, int64_t i) {
@@ -211,14 +273,61 @@ __device__ __forceinline__ void chunk_keys(const KeySrc& s, int64_t c, int lane,
   for (int q = 0; q < 4; ++q) { valid[q] = i0 + q < s.N; k64[q] = make_k64(x[q], i0 + q); }
 }
 
-__global__ void sel_init_kernel(SelState* st, uint32_t* ghist, long long k) {
+// Candidate list written by the fused pass: n_seg segments of seg_cap entries.
+struct CandList {
+  const unsigned long long* cand;
+  const uint32_t* seg_count;
+  const uint32_t* seg_above;
+  uint32_t seg_cap;
+  int n_seg;
+};
+
+// One block.  Sums the per-warp counts of the fused pass and decides whether the predicted bracket
+// held: hit <=> no segment overflowed and n_above < k <= n_above + n_cand.  Arms the radix select
+// with the rank sought inside the candidate list (hit) or inside the whole partition (general).
+__global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t* ghist, CandList cl, long long k, int force_general) {
+  __shared__ unsigned long long s_above[32], s_cand[32];
+  __shared__ int s_over;
   for (int b = threadIdx.x; b < kBins; b += blockDim.x) ghist[b] = 0;
-  if (threadIdx.x == 0) { st->prefix = 0; st->himask = 0; st->rank = k; }
+  if (threadIdx.x == 0) s_over = 0;
+  __syncthreads();
+  unsigned long long a = 0, c = 0;
+  int over = 0;
+  if (!force_general) {
+    for (int i = threadIdx.x; i < cl.n_seg; i += blockDim.x) {
+      const uint32_t cnt = cl.seg_count[i];
+      a += cl.seg_above[i]; c += cnt;
+      over |= cnt > cl.seg_cap;
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { a += __shfl_xor_sync(0xFFFFFFFFu, a, o); c += __shfl_xor_sync(0xFFFFFFFFu, c, o); }
+  if ((threadIdx.x & 31) == 0) { s_above[threadIdx.x >> 5] = a; s_cand[threadIdx.x >> 5] = c; }
+  if (over) s_over = 1;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    a = 0; c = 0;
+    for (int i = 0; i < 32; ++i) { a += s_above[i]; c += s_cand[i]; }
+    const bool hit = !force_general && !s_over && (long long)a < k && (long long)(a + c) >= k;
+    st->prefix = 0; st->himask = 0;
+    st->rank = hit ? k - (long long)a : k;
+    st->hit = hit ? 1 : 0;
+    st->n_above = a; st->n_cand = c;
+    if (hit) st->n_fast += 1; else st->n_general += 1;
+    if (!hit && !force_general) {
+      // adapt the bracket width for the next prediction: too many candidates -> narrower;
+      // threshold outside the bracket -> wider
+      if (s_over) st->delta = fmaxf(st->delta * 0.5f, 0.01f);
+      else st->delta = fminf(st->delta * 2.0f, 1.0f);
+    }
+  }
 }
 
-// Histogram of digit (K64 >> shift) & (kBins-1) over the keys whose higher digits equal prefix.
-__global__ void __launch_bounds__(256) sel_hist_dense_kernel(const __grid_constant__ KeySrc s, const SelState* __restrict__ st,
-                                                            uint32_t* __restrict__ ghist, int shift, int bits) {
+// Histogram of digit (K64 >> shift) & (2^bits - 1) over the keys whose higher digits equal prefix.
+// Source: the candidate list when the bracket held (st->hit), else every key of the partition.
+__global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ KeySrc s, const __grid_constant__ CandList cl,
+                                                      const SelState* __restrict__ st, uint32_t* __restrict__ ghist,
+                                                      int shift, int bits) {
   __shared__ uint32_t h[kBins];
   for (int b = threadIdx.x; b < kBins; b += blockDim.x) h[b] = 0;
   __syncthreads();
@@ -228,19 +337,30 @@ __global__ void __launch_bounds__(256) sel_hist_dense_kernel(const __grid_consta
   const int64_t wpb = blockDim.x >> 5;
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
   const int64_t nwarps = (int64_t)gridDim.x * wpb;
-  for (int64_t c = warp; c < s.n_chunks; c += nwarps) {
-    unsigned long long k64[4]; bool valid[4];
-    chunk_keys(s, c, lane, k64, valid);
+  if (st->hit) {
+    for (int64_t sg = warp; sg < cl.n_seg; sg += nwarps) {
+      const uint32_t cnt = cl.seg_count[sg];
+      const unsigned long long* seg = cl.cand + (size_t)sg * cl.seg_cap;
+      for (uint32_t j = lane; j < cnt; j += 32) {
+        const unsigned long long k64 = seg[j];
+        if ((k64 & himask) == prefix) atomicAdd(&h[(uint32_t)(k64 >> shift) & dmask], 1u);
+      }
+    }
+  } else {
+    for (int64_t c = warp; c < s.n_chunks; c += nwarps) {
+      unsigned long long k64[4]; bool valid[4];
+      chunk_keys(s, c, lane, k64, valid);
 #pragma unroll
-    for (int q = 0; q < 4; ++q)
-      if (valid[q] && (k64[q] & himask) == prefix) atomicAdd(&h[(uint32_t)(k64[q] >> shift) & dmask], 1u);
+      for (int q = 0; q < 4; ++q)
+        if (valid[q] && (k64[q] & himask) == prefix) atomicAdd(&h[(uint32_t)(k64[q] >> shift) & dmask], 1u);
+    }
   }
   __syncthreads();
   for (int b = threadIdx.x; b < kBins; b += blockDim.x) if (h[b]) atomicAdd(&ghist[b], h[b]);
 }
 
 // One block: find the digit d whose class holds the sought rank; fix it; clear the histogram.
-__global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* ghist, int shift, int bits) {
+__global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* ghist, int shift, int bits, int last) {
   constexpr int PER = kBins / 1024;                 // bins per thread
   __shared__ long long warp_tot[32];
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
@@ -272,9 +392,27 @@ __global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* 
     for (int q = 0; q < PER; ++q) {
       if (cum < rank && rank <= cum + hv[q]) {
         const unsigned long long d = (unsigned long long)(top - 1 - q);
-        st->prefix |= d << shift;
+        const unsigned long long T64 = st->prefix | (d << shift);
+        st->prefix = T64;
         st->himask |= ((1ull << bits) - 1ull) << shift;
         st->rank = rank - cum;
+        if (last) {
+          // T64 is now exact.  Predict the next step's bracket around this threshold
+          // (the top-k structure of the first moment is temporally stable).
+          const float T = __uint_as_float((uint32_t)(T64 >> 32));
+          float dl = st->delta;
+          if (st->have_T && T > 0.0f && st->T_prev > 0.0f) {
+            const float drift = fabsf(__logf(T / st->T_prev));
+            const float target = fminf(fmaxf(4.0f * drift, 0.05f), 1.0f);
+            dl = fmaxf(target, 0.8f * dl);
+          }
+          dl = fminf(fmaxf(dl, 0.05f), 1.0f);
+          const float lo = T / (1.0f + dl), hi = T * (1.0f + dl);
+          st->lo_key = __float_as_uint(lo) & 0x7FFFFFFFu;
+          st->hi_key = (hi == hi) ? (__float_as_uint(hi) & 0x7FFFFFFFu) : 0x7F800000u;
+          if (st->hi_key <= st->lo_key) st->hi_key = st->lo_key + 1u;
+          st->delta = dl; st->T_prev = T; st->have_T = 1;
+        }
       }
       cum += hv[q];
     }
@@ -283,14 +421,30 @@ __global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* 
   for (int q = 0; q < PER; ++q) ghist[top - 1 - q] = 0;
 }
 
-// next mask bits: selected(i) <=> K64(i) >= T64 (= st->prefix once every digit is fixed).
-__global__ void __launch_bounds__(256) sel_write_mask_dense_kernel(const __grid_constant__ KeySrc s, const SelState* __restrict__ st,
-                                                                  uint32_t* __restrict__ next_bits) {
+// Complete M_t once T64 (= st->prefix) is exact: selected(i) <=> K64(i) >= T64.
+//   bracket held : the fused pass already wrote the certainly-selected bits; OR in the candidates
+//   general path : rewrite every word from the keys
+__global__ void __launch_bounds__(256) sel_finish_kernel(const __grid_constant__ KeySrc s, const __grid_constant__ CandList cl,
+                                                        const SelState* __restrict__ st, uint32_t* __restrict__ next_bits) {
   const unsigned long long T64 = st->prefix;
   const int lane = threadIdx.x & 31;
   const int64_t wpb = blockDim.x >> 5;
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
   const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  if (st->hit) {
+    for (int64_t sg = warp; sg < cl.n_seg; sg += nwarps) {
+      const uint32_t cnt = cl.seg_count[sg];
+      const unsigned long long* seg = cl.cand + (size_t)sg * cl.seg_cap;
+      for (uint32_t j = lane; j < cnt; j += 32) {
+        const unsigned long long k64 = seg[j];
+        if (k64 >= T64) {
+          const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64;
+          atomicOr(&next_bits[i >> 5], 1u << (i & 31));
+        }
+      }
+    }
+    return;
+  }
   for (int64_t c = warp; c < s.n_chunks; c += nwarps) {
     unsigned long long k64[4]; bool valid[4];
     chunk_keys(s, c, lane, k64, valid);

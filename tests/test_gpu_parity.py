@@ -125,6 +125,9 @@ def test_config1_pr1_chained_parity_is_exact(B):
         gpu.step(th_gpu, grads)
         ora.step(th_ora, [to_np32(g) for g in grads])
         compare_step(gpu, ora, th_gpu, th_ora, R, f"chained step {t}")
+    fast, general = gpu.select_stats()
+    assert fast + general == 10 and general >= 1      # step 1 (all-ones mask) is always general
+    assert fast >= 5, (fast, general)                 # the predicted bracket holds in steady state
     gpu.close()
 
 
@@ -144,6 +147,8 @@ def test_chained_100_steps(B):
         ora.step(th_ora, [to_np32(g) for g in grads])
     agree = float((gpu.mask_next() == ora.mask()).mean())
     assert agree >= 0.9999, agree
+    fast, general = gpu.select_stats()
+    assert fast + general == 100 and fast >= 80, (fast, general)
     assert_close(th_gpu.cpu().numpy(), th_ora, "theta after 100 chained steps", tol=1e-4)
     assert_close(gpu.moment(), ora.m(), "m after 100 chained steps", tol=1e-4)
     gpu.close()
@@ -293,3 +298,27 @@ def test_cuda_graph_capture_of_a_step(B):
     np.testing.assert_array_equal(ref.mask_next(), cap.mask_next())
     ref.close()
     cap.close()
+
+
+def test_select_survives_threshold_jumps(B):
+    """Gradient scale jumps by 100x up and down between steps: the predicted bracket misses in both
+    directions (and overflows when everything becomes a candidate); every step must stay exact."""
+    rng = np.random.default_rng(7)
+    N, R, s = 300_000 + 5, 2, 0.99
+    gpu = B.Scape(N, R, s, **HYP)
+    gpu.keep_dense_pack(True)
+    ora = ScapeOracle(N, R, s, **HYP)
+    th_ora = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    th_gpu = torch.from_numpy(th_ora.copy()).cuda()
+    scales = [1e-3, 1e-3, 1e-3, 1e-1, 1e-1, 1e-5, 1e-5, 1e-3, 1e-3, 1e-3, 0.0, 1e-3, 1e-3]
+    for t, sc in enumerate(scales, 1):
+        base = [(sc * rng.standard_normal(N)).astype(np.float32) for _ in range(R)]
+        if t == 9:
+            for b in base:
+                b[:] = 1e-3          # constant gradient: huge tie class around the threshold
+        gpu.step(th_gpu, [torch.from_numpy(b).cuda() for b in base])
+        ora.step(th_ora, base)
+        compare_step(gpu, ora, th_gpu, th_ora, R, f"jump step {t}")
+    fast, general = gpu.select_stats()
+    assert fast >= 2 and general >= 3, (fast, general)
+    gpu.close()
