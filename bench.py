@@ -254,6 +254,7 @@ def main():
         clocks.start()
     sc.profile(True)
     launches0 = sc.launches
+    fast0, general0 = sc.select_stats()
     t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t0.record()
     for i in range(K):
@@ -264,6 +265,7 @@ def main():
     fused_ms, select_ms, psteps = sc.profile_read()
     sc.profile(False)
     gpu_launches = sc.launches - launches0
+    fast1, general1 = sc.select_stats()
     clk = clocks.stop() if rank == 0 else None
     if world > 1:
         tt = torch.tensor([elapsed_ms], device=dev, dtype=torch.float64)
@@ -289,6 +291,7 @@ def main():
         "peak_source": peak_src, "algorithmic_bytes_per_launch": fb, "kernel_ms": fused_avg_ms,
         "kernel_share_of_step": fused_avg_ms / ms_per_step,
         "select_ms": select_ms / max(1, psteps),
+        "select_steps_fast": fast1 - fast0, "select_steps_general": general1 - general0,
         "step_algorithmic_bytes": sb, "step_gbs": sb / (ms_per_step * 1e-3) / 1e9,
         "step_frac_of_peak": sb / (ms_per_step * 1e-3) / 1e9 / peak,
         "step_frac_of_8TBs_nominal": sb / (ms_per_step * 1e-3) / 1e9 / 8000.0,

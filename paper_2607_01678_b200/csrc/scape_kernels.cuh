@@ -31,9 +31,11 @@ struct SelState {
   // predicted bracket for the COMING step's fused pass: key >= hi_key is certainly selected,
   // lo_key <= key < hi_key is a candidate, key < lo_key is certainly not selected
   uint32_t lo_key, hi_key;
-  float delta;                // relative half-width of the bracket
-  float T_prev;               // last exact threshold |m~| value
-  int have_T;
+  float delta;                // half-width of the bracket in ln(threshold)
+  float lnT_prev;             // ln of the last exact threshold |m~| value
+  float ln_pred;              // ln of the threshold that was predicted for the current step
+  int have_T;                 // number of exact thresholds seen (saturates at 2)
+  unsigned long long cand_cap_total;   // n_seg * seg_cap of the last fused pass
   int hit;                    // this step: 1 = the bracket held (candidate list), 0 = general path
   unsigned long long n_fast, n_general;   // statistics (scape_select_stats)
   unsigned long long n_above, n_cand;     // this step's counts from the fused pass
@@ -313,12 +315,12 @@ __global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t
     st->rank = hit ? k - (long long)a : k;
     st->hit = hit ? 1 : 0;
     st->n_above = a; st->n_cand = c;
+    st->cand_cap_total = (unsigned long long)cl.n_seg * cl.seg_cap;
     if (hit) st->n_fast += 1; else st->n_general += 1;
     if (!hit && !force_general) {
-      // adapt the bracket width for the next prediction: too many candidates -> narrower;
-      // threshold outside the bracket -> wider
-      if (s_over) st->delta = fmaxf(st->delta * 0.5f, 0.01f);
-      else st->delta = fminf(st->delta * 2.0f, 1.0f);
+      // too many candidates for the list: narrower next time (a threshold outside the bracket
+      // widens it by itself through the prediction error, see sel_pick_kernel)
+      if (s_over) st->delta = fmaxf(st->delta * 0.5f, 0.03f);
     }
   }
 }
@@ -399,19 +401,33 @@ __global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* 
         if (last) {
           // T64 is now exact.  Predict the next step's bracket around this threshold
           // (the top-k structure of the first moment is temporally stable).
+          // The threshold moves smoothly from step to step (transient of the EMA, then
+          // stationary), so the centre is extrapolated geometrically and the half-width follows
+          // the error the previous extrapolation made.
           const float T = __uint_as_float((uint32_t)(T64 >> 32));
-          float dl = st->delta;
-          if (st->have_T && T > 0.0f && st->T_prev > 0.0f) {
-            const float drift = fabsf(__logf(T / st->T_prev));
-            const float target = fminf(fmaxf(4.0f * drift, 0.05f), 1.0f);
-            dl = fmaxf(target, 0.8f * dl);
+          float dl = st->delta, pred;
+          if (!(T > 0.0f) || !(T < 3.0e38f)) {           // zero / non-finite threshold: no prediction
+            st->lo_key = st->hi_key = 0xFFFFFFFFu; st->have_T = 0;
+          } else {
+            const float lnT = __logf(T);
+            if (st->have_T == 0) { pred = lnT; dl = 0.6f; }
+            else {
+              const float r = fminf(fmaxf(lnT - st->lnT_prev, -0.7f), 0.7f);
+              pred = lnT + r;
+              if (st->have_T == 1) dl = fmaxf(0.05f, 0.5f * fabsf(r));
+              else dl = fmaxf(3.0f * fabsf(lnT - st->ln_pred) + 0.02f, 0.6f * dl);
+            }
+            // keep the expected candidate count under half the list's capacity
+            if (st->hit && st->cand_cap_total > 0 && 2ull * st->n_cand > st->cand_cap_total)
+              dl = fminf(dl, st->delta * (float)st->cand_cap_total / (2.0f * (float)st->n_cand));
+            dl = fminf(fmaxf(dl, 0.03f), 1.0f);
+            const float lo = __expf(pred - dl), hi = __expf(pred + dl);
+            st->lo_key = __float_as_uint(lo) & 0x7FFFFFFFu;
+            st->hi_key = (hi < 3.0e38f) ? (__float_as_uint(hi) & 0x7FFFFFFFu) : 0x7F800000u;
+            if (st->hi_key <= st->lo_key) st->hi_key = st->lo_key + 1u;
+            st->delta = dl; st->lnT_prev = lnT; st->ln_pred = pred;
+            st->have_T = st->have_T < 2 ? st->have_T + 1 : 2;
           }
-          dl = fminf(fmaxf(dl, 0.05f), 1.0f);
-          const float lo = T / (1.0f + dl), hi = T * (1.0f + dl);
-          st->lo_key = __float_as_uint(lo) & 0x7FFFFFFFu;
-          st->hi_key = (hi == hi) ? (__float_as_uint(hi) & 0x7FFFFFFFu) : 0x7F800000u;
-          if (st->hi_key <= st->lo_key) st->hi_key = st->lo_key + 1u;
-          st->delta = dl; st->T_prev = T; st->have_T = 1;
         }
       }
       cum += hv[q];
