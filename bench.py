@@ -66,16 +66,22 @@ def grad_bytes(w):
 
 
 def bytes_per_param_fused(w, k, N):
-    """Fused streaming kernel, steady state: reads theta, m, g^r, e^r, mask bits, rank128; writes
-    theta, m, e^r, b^r, b-bar."""
+    """Fused streaming kernel, steady state (sparse mask in, m stored sparsely): reads theta, g^r,
+    e^r, the bits + rank128 of the current and the previous mask, the previous packed mean (= m);
+    writes theta, e^r, b^r, b-bar (= new m) and the certainly-selected bits of the next mask.
+    With sparsity 0 every step is dense: m is read and written densely, nothing is packed."""
     G, R, d = grad_bytes(w), w.R, k / N
-    return (G + 8) * R + 16 + 4 * d * (R + 1) + 1 / 8 + 4 / 128
+    if k == N:
+        return (G + 8) * R + 16
+    return (G + 8) * R + 8 + 4 * d * (R + 2) + 2 * (1 / 8 + 4 / 128) + 1 / 8
 
 
 def bytes_per_param_step(w, k, N):
-    """Whole step, the method's own traffic with dense m (SURVEY.md §8(d) B_dense)."""
+    """Whole step, the method's own minimum traffic (SURVEY.md §8(d) B_alg: m stored sparsely)."""
     G, R, d = grad_bytes(w), w.R, k / N
-    return (G + 8) * R + 16 + 8 * d + 4 * d * R + 1 / 4
+    if k == N:
+        return (G + 8) * R + 16
+    return (G + 8) * R + 8 + 16 * d + 4 * d * R + 3 / 8
 
 
 def measured_peak():

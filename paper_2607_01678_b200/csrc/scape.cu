@@ -60,11 +60,16 @@ struct scape {
 
   float* m = nullptr;          // [Npad]
   float* e = nullptr;          // [R][Npad]
-  MaskSlot slot[2];
-  int use = 0;                 // slot the coming step uses (SCAPE_MASK_NEXT); 1-use = SCAPE_MASK_LAST
+  // three mask slots rotate: `use` = M_{t-1}, the mask the coming step uses (SCAPE_MASK_NEXT);
+  // `last` = the mask the last step used (SCAPE_MASK_LAST; a sparsely stored m is addressed
+  // through it); `build` = where the coming step writes M_t
+  MaskSlot slot[3];
+  int use = 0, last = 1, build = 2;
   float* packed = nullptr;     // [R][packed_stride]
   int64_t packed_stride = 0;
-  float* packed_mean = nullptr;   // [packed_stride]
+  float* pm[2] = {nullptr, nullptr};   // packed means b- [packed_stride], alternating
+  int pm_last = 0;             // pm[pm_last] = b- of the last sparse step
+  bool m_sparse = false;       // m_{t-1} lives in pm[pm_last] addressed through slot[last]; h->m is stale
   float* dense_pack = nullptr;    // optional [R][Npad]
   bool last_dense = false;
 
@@ -105,12 +110,12 @@ int grid_for(const scape* h, int64_t n_chunks, int warps_per_block, int blocks_p
   return (int)(need < cap ? need : cap);
 }
 
-template <typename G, int R, bool DENSE>
+template <typename G, int R, bool DENSE, bool MSPARSE>
 int launch_fused_t(scape* h, StepParams& p, cudaStream_t st) {
   static int bps = 0;   // resident blocks per SM of this instantiation
   if (bps == 0) {
     int v = 0;
-    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, scape_fused_step_kernel<G, R, DENSE>, 256, 0));
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, scape_fused_step_kernel<G, R, DENSE, MSPARSE>, 256, 0));
     bps = v > 0 ? (v > 8 ? 8 : v) : 1;
   }
   const int grid = grid_for(h, p.n_chunks, 8, bps);
@@ -120,31 +125,50 @@ int launch_fused_t(scape* h, StepParams& p, cudaStream_t st) {
   if (cap > 0x7FFFFFF0) cap = 0x7FFFFFF0;
   h->seg_cap = (uint32_t)cap;
   p.seg_cap = h->seg_cap;
-  scape_fused_step_kernel<G, R, DENSE><<<grid, 256, 0, st>>>(p);
+  scape_fused_step_kernel<G, R, DENSE, MSPARSE><<<grid, 256, 0, st>>>(p);
   h->launches++;
   CU_TRY(cudaGetLastError());
   return SCAPE_OK;
 }
 
-template <typename G, bool DENSE>
+template <typename G, bool DENSE, bool MSPARSE>
 int launch_fused_r(scape* h, StepParams& p, cudaStream_t st) {
   switch (h->R) {
-    case 1: return launch_fused_t<G, 1, DENSE>(h, p, st);
-    case 2: return launch_fused_t<G, 2, DENSE>(h, p, st);
-    case 3: return launch_fused_t<G, 3, DENSE>(h, p, st);
-    case 4: return launch_fused_t<G, 4, DENSE>(h, p, st);
-    case 5: return launch_fused_t<G, 5, DENSE>(h, p, st);
-    case 6: return launch_fused_t<G, 6, DENSE>(h, p, st);
-    case 7: return launch_fused_t<G, 7, DENSE>(h, p, st);
-    case 8: return launch_fused_t<G, 8, DENSE>(h, p, st);
+    case 1: return launch_fused_t<G, 1, DENSE, MSPARSE>(h, p, st);
+    case 2: return launch_fused_t<G, 2, DENSE, MSPARSE>(h, p, st);
+    case 3: return launch_fused_t<G, 3, DENSE, MSPARSE>(h, p, st);
+    case 4: return launch_fused_t<G, 4, DENSE, MSPARSE>(h, p, st);
+    case 5: return launch_fused_t<G, 5, DENSE, MSPARSE>(h, p, st);
+    case 6: return launch_fused_t<G, 6, DENSE, MSPARSE>(h, p, st);
+    case 7: return launch_fused_t<G, 7, DENSE, MSPARSE>(h, p, st);
+    case 8: return launch_fused_t<G, 8, DENSE, MSPARSE>(h, p, st);
   }
   return fail(SCAPE_EINVAL, "R out of range");
 }
 
-int launch_fused(scape* h, StepParams& p, bool dense, cudaStream_t st) {
-  if (h->grad_dtype == SCAPE_GRAD_BF16)
-    return dense ? launch_fused_r<__nv_bfloat16, true>(h, p, st) : launch_fused_r<__nv_bfloat16, false>(h, p, st);
-  return dense ? launch_fused_r<float, true>(h, p, st) : launch_fused_r<float, false>(h, p, st);
+// variants: all-ones mask (dense m in and out) | sparse mask, dense m in | sparse mask, sparse m in
+template <typename G>
+int launch_fused_g(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t st) {
+  if (dense) return launch_fused_r<G, true, false>(h, p, st);
+  return msparse ? launch_fused_r<G, false, true>(h, p, st) : launch_fused_r<G, false, false>(h, p, st);
+}
+
+int launch_fused(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t st) {
+  if (h->grad_dtype == SCAPE_GRAD_BF16) return launch_fused_g<__nv_bfloat16>(h, p, dense, msparse, st);
+  return launch_fused_g<float>(h, p, dense, msparse, st);
+}
+
+// dense view of m in h->m when it is stored sparsely (accessors; all-ones step after sparse ones)
+int materialise_dense_m(scape* h, cudaStream_t st) {
+  if (!h->m_sparse) return SCAPE_OK;
+  const MaskSlot& s = h->slot[h->last];
+  CU_TRY(cudaMemsetAsync(h->m, 0, sizeof(float) * h->Npad, st));
+  if (s.count > 0) {
+    scatter_packed_kernel<<<1024, 256, 0, st>>>(h->m, s.idx, h->pm[h->pm_last], s.count);
+    h->launches++;
+    CU_TRY(cudaGetLastError());
+  }
+  return SCAPE_OK;
 }
 
 // rank128 (+ idx when idx != nullptr) of slot.bits; leaves the bit count in *h->total
@@ -215,7 +239,7 @@ bool finite_all(std::initializer_list<double> v) {
 void free_all(scape* h) {
   cudaFree(h->m); cudaFree(h->e);
   for (auto& s : h->slot) { cudaFree(s.bits); cudaFree(s.rank); cudaFree(s.idx); }
-  cudaFree(h->packed); cudaFree(h->packed_mean); cudaFree(h->dense_pack);
+  cudaFree(h->packed); cudaFree(h->pm[0]); cudaFree(h->pm[1]); cudaFree(h->dense_pack);
   cudaFree(h->sel); cudaFree(h->cand); cudaFree(h->seg_count); cudaFree(h->seg_above); cudaFree(h->ghist); cudaFree(h->block_sum); cudaFree(h->total);
   cudaFree(h->st_param);
   for (auto& g : h->st_grad) cudaFree(g);
@@ -270,7 +294,8 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   }
   if (sparse) {
     alloc((void**)&h->packed, sizeof(float) * h->packed_stride * R, true);
-    alloc((void**)&h->packed_mean, sizeof(float) * h->packed_stride, true);
+    alloc((void**)&h->pm[0], sizeof(float) * h->packed_stride, true);
+    alloc((void**)&h->pm[1], sizeof(float) * h->packed_stride, true);
   }
   alloc((void**)&h->sel, sizeof(SelState), true);
   if (sparse) {
@@ -304,7 +329,7 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   h->slot[0].all_ones = true;                                                // l.1: M_0 = 1
   h->slot[0].count = N;
   h->slot[0].valid = true;
-  h->use = 0;
+  h->use = 0; h->last = 1; h->build = 2;
   if (cudaDeviceSynchronize() != cudaSuccess) { fail(SCAPE_ECUDA, "create: sync failed"); free_all(h); delete h; return nullptr; }
   return h;
 }
@@ -325,8 +350,8 @@ extern "C" int64_t scape_count(const scape_t* h, int which) {
   if (!h) return fail(SCAPE_EINVAL, "NULL handle");
   if (which == SCAPE_MASK_NEXT) return h->slot[h->use].count;
   if (which == SCAPE_MASK_LAST) {
-    if (!h->slot[1 - h->use].valid || h->t == 0) return fail(SCAPE_EINVAL, "no step has run yet");
-    return h->slot[1 - h->use].count;
+    if (!h->slot[h->last].valid || h->t == 0) return fail(SCAPE_EINVAL, "no step has run yet");
+    return h->slot[h->last].count;
   }
   return fail(SCAPE_EINVAL, "scape_count: bad selector %d", which);
 }
@@ -377,8 +402,16 @@ extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, vo
   cudaStream_t st = (cudaStream_t)cuda_stream;
 
   MaskSlot& cur = h->slot[h->use];
-  MaskSlot& nxt = h->slot[1 - h->use];
+  MaskSlot& nxt = h->slot[h->build];
   const bool need_select = h->k < h->N;
+  int rc;
+  // an all-ones step reads and writes m densely
+  if (cur.all_ones && h->m_sparse) {
+    if ((rc = materialise_dense_m(h, st))) return rc;
+    h->m_sparse = false;
+  }
+  const bool msparse = h->m_sparse;
+  const int pm_out = msparse ? 1 - h->pm_last : 0;
 
   StepParams p{};
   p.theta = param; p.m = h->m; p.e = h->e; p.e_stride = h->Npad;
@@ -386,7 +419,10 @@ extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, vo
   p.cur_bits = cur.bits; p.cur_rank = cur.rank;
   p.packed = cur.all_ones ? h->dense_pack : h->packed;
   p.packed_stride = cur.all_ones ? h->Npad : h->packed_stride;
-  p.packed_mean = h->packed_mean;
+  p.packed_mean = h->pm[pm_out];
+  if (msparse) {
+    p.prev_bits = h->slot[h->last].bits; p.prev_rank = h->slot[h->last].rank; p.pm_prev = h->pm[h->pm_last];
+  }
   p.N = h->N; p.n_chunks = h->n_chunks;
   p.b1 = h->b1; p.c1 = h->c1; p.b2 = h->b2; p.c2 = h->c2; p.eps = h->eps; p.wd = h->wd; p.neg_lr = -h->lr;
   p.R_f = (float)h->R; p.inv_R = 1.0f / (float)h->R;
@@ -399,7 +435,7 @@ extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, vo
   if (prof && h->prof_pending == scape::kProfRing) { int prc = prof_drain(h); if (prc) return prc; }
   const int pi = h->prof_pending;
   if (prof) CU_TRY(cudaEventRecord(h->prof_ev[pi][0], st));
-  int rc = launch_fused(h, p, cur.all_ones, st);
+  rc = launch_fused(h, p, cur.all_ones, msparse, st);
   if (rc) return rc;
   if (prof) CU_TRY(cudaEventRecord(h->prof_ev[pi][1], st));
 
@@ -412,7 +448,8 @@ extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, vo
   }
   if (prof) { CU_TRY(cudaEventRecord(h->prof_ev[pi][2], st)); h->prof_pending = pi + 1; }
   h->last_dense = cur.all_ones;
-  h->use = 1 - h->use;
+  if (!cur.all_ones) { h->m_sparse = true; h->pm_last = pm_out; }   // m_t = b-_t, addressed through `cur`
+  { const int old_last = h->last; h->last = h->use; h->use = h->build; h->build = old_last; }
   h->t += 1;
   return SCAPE_OK;
 }
@@ -519,11 +556,12 @@ extern "C" int scape_get(scape_t* h, int what, int r, void* buf, size_t bytes, v
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t nbytes = sizeof(float) * (size_t)h->N;
   MaskSlot& nx = h->slot[h->use];
-  MaskSlot& la = h->slot[1 - h->use];
+  MaskSlot& la = h->slot[h->last];
   int rc = SCAPE_OK;
   switch (what) {
     case SCAPE_MOMENT:
       if (bytes != nbytes) return fail(SCAPE_EINVAL, "moment: expected %zu bytes", nbytes);
+      if ((rc = materialise_dense_m(h, st))) return rc;      // dense view; the sparse store stays in use
       CU_TRY(cudaMemcpyAsync(buf, h->m, bytes, cudaMemcpyDefault, st));
       break;
     case SCAPE_RESIDUAL:
@@ -563,7 +601,7 @@ extern "C" int scape_get(scape_t* h, int what, int r, void* buf, size_t bytes, v
     case SCAPE_PACKED_MEAN:
       if (h->t == 0 || !la.valid) return fail(SCAPE_EINVAL, "no step has run yet");
       if (bytes != sizeof(float) * (size_t)la.count) return fail(SCAPE_EINVAL, "packed_mean: expected %zu bytes", sizeof(float) * (size_t)la.count);
-      CU_TRY(cudaMemcpyAsync(buf, h->last_dense ? h->m : h->packed_mean, bytes, cudaMemcpyDefault, st));
+      CU_TRY(cudaMemcpyAsync(buf, h->last_dense ? h->m : h->pm[h->pm_last], bytes, cudaMemcpyDefault, st));
       break;
     default:
       return fail(SCAPE_EINVAL, "scape_get: bad selector %d", what);
@@ -581,6 +619,7 @@ extern "C" int scape_set(scape_t* h, int what, int r, const void* buf, size_t by
     case SCAPE_MOMENT:
       if (bytes != nbytes) return fail(SCAPE_EINVAL, "moment: expected %zu bytes", nbytes);
       CU_TRY(cudaMemcpyAsync(h->m, buf, bytes, cudaMemcpyDefault, st));
+      h->m_sparse = false;                                   // m is dense again until the next sparse step
       break;
     case SCAPE_RESIDUAL:
       if (r < 0 || r >= h->R) return fail(SCAPE_EINVAL, "residual: replica %d out of range", r);

@@ -51,7 +51,12 @@ struct StepParams {
   const uint32_t* cur_rank;     // [Npad/128]
   float* packed;                // [R][packed_stride] or nullptr (DENSE without keep_dense_pack)
   int64_t packed_stride;
-  float* packed_mean;           // [k]          (unused when DENSE)
+  float* packed_mean;           // [k] b- of this step = m_t in packed form (unused when DENSE)
+  // m_{t-1} stored sparsely (MSPARSE): it is zero off the mask the previous step used (Eq. 4,
+  // PAPER.md:197), so it lives as that step's packed mean, addressed through that mask
+  const uint32_t* prev_bits;    // [Npad/32]
+  const uint32_t* prev_rank;    // [Npad/128]
+  const float* pm_prev;         // [k]
   int64_t N;
   int64_t n_chunks;             // ceil(N/128)
   float b1, c1, b2, c2, eps, wd, neg_lr;
@@ -113,6 +118,15 @@ __device__ __forceinline__ void load4_grad(const void* __restrict__ base, int64_
 }
 
 // Position of this lane's 4 mask bits inside the chunk's uint4, and the packed rank before them.
+__device__ __forceinline__ void lane_bits_from_words(const uint4 mw, const uint32_t r0, int lane, uint32_t& mybits, uint32_t& jbase) {
+  const int ws = lane >> 3, sh = (lane & 7) << 2;
+  const uint32_t p0 = __popc(mw.x), p1 = p0 + __popc(mw.y), p2 = p1 + __popc(mw.z);
+  const uint32_t w = ws == 0 ? mw.x : ws == 1 ? mw.y : ws == 2 ? mw.z : mw.w;
+  const uint32_t before = ws == 0 ? 0u : ws == 1 ? p0 : ws == 2 ? p1 : p2;
+  mybits = (w >> sh) & 0xFu;
+  jbase = r0 + before + __popc(w & ((1u << sh) - 1u));
+}
+
 __device__ __forceinline__ void lane_mask_bits(const uint32_t* __restrict__ bits, const uint32_t* __restrict__ rank,
                                                int64_t c, int lane, uint32_t& mybits, uint32_t& jbase) {
   const uint4 mw = __ldg(reinterpret_cast<const uint4*>(bits) + c);
@@ -135,19 +149,34 @@ struct StageA {                 // per-warp running state of the fused select (r
   unsigned long long* seg;      // this warp's candidate segment
 };
 
-template <typename G, int R, bool DENSE, bool GUARD>
+template <typename G, int R, bool DENSE, bool MSPARSE, bool GUARD>
 __device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int lane, StageA& sa) {
   const int64_t i0 = (c << 7) + ((int64_t)lane << 2);
-  uint32_t mybits = 0xFu, jbase = 0;
-  if (!DENSE) lane_mask_bits(p.cur_bits, p.cur_rank, c, lane, mybits, jbase);
+  // Issue order matters for latency: the mask words first (L2-resident, short latency), then the
+  // 2R+1 streaming loads, and only then the gather of m_{t-1}, whose addresses depend on the
+  // mask words -- it is in flight together with the streaming loads instead of after them.
+  uint4 cw = make_uint4(~0u, ~0u, ~0u, ~0u), pw = make_uint4(0, 0, 0, 0);
+  uint32_t cr = 0, pr = 0;
+  if (!DENSE) { cw = __ldg(reinterpret_cast<const uint4*>(p.cur_bits) + c); cr = __ldg(p.cur_rank + c); }
+  if (MSPARSE) { pw = __ldg(reinterpret_cast<const uint4*>(p.prev_bits) + c); pr = __ldg(p.prev_rank + c); }
 
   float th[4], mo[4], gg[R][4], ee[R][4];
   load4_f32<GUARD>(p.theta, i0, p.N, th);
-  load4_f32<false>(p.m, i0, p.N, mo);                       // own arrays are padded to Npad
+  if (!MSPARSE) load4_f32<false>(p.m, i0, p.N, mo);         // own arrays are padded to Npad
 #pragma unroll
   for (int r = 0; r < R; ++r) {
     load4_grad<G, GUARD>(p.g[r], i0, p.N, gg[r]);
     load4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
+  }
+
+  uint32_t mybits = 0xFu, jbase = 0;
+  if (!DENSE) lane_bits_from_words(cw, cr, lane, mybits, jbase);
+  if (MSPARSE) {
+    uint32_t pbits, pbase;
+    lane_bits_from_words(pw, pr, lane, pbits, pbase);
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+      mo[q] = ((pbits >> q) & 1u) ? __ldg(p.pm_prev + pbase + __popc(pbits & ((1u << q) - 1u))) : 0.0f;
   }
 
   float mn[4];
@@ -185,7 +214,7 @@ __device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int 
   }
 
   store4_f32<GUARD>(p.theta, i0, p.N, th);
-  store4_f32<false>(p.m, i0, p.N, mn);
+  if (DENSE) store4_f32<false>(p.m, i0, p.N, mn);           // sparse steps keep m_t as b- only
 #pragma unroll
   for (int r = 0; r < R; ++r) store4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
 
@@ -216,8 +245,8 @@ __device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int 
   }
 }
 
-template <typename G, int R, bool DENSE>
-__global__ void __launch_bounds__(256) scape_fused_step_kernel(const __grid_constant__ StepParams p) {
+template <typename G, int R, bool DENSE, bool MSPARSE>
+__global__ void __launch_bounds__(256, (R <= 4 ? 3 : 2)) scape_fused_step_kernel(const __grid_constant__ StepParams p) {
   const int lane = threadIdx.x & 31;
   const int64_t wpb = blockDim.x >> 5;
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
@@ -228,8 +257,8 @@ __global__ void __launch_bounds__(256) scape_fused_step_kernel(const __grid_cons
     sa.lo = p.ctl->lo_key; sa.hi = p.ctl->hi_key;
     sa.seg = p.cand + (size_t)warp * p.seg_cap;
   }
-  for (int64_t c = warp; c < full; c += nwarps) fused_chunk<G, R, DENSE, false>(p, c, lane, sa);
-  if (full < p.n_chunks && warp == full % nwarps) fused_chunk<G, R, DENSE, true>(p, full, lane, sa);
+  for (int64_t c = warp; c < full; c += nwarps) fused_chunk<G, R, DENSE, MSPARSE, false>(p, c, lane, sa);
+  if (full < p.n_chunks && warp == full % nwarps) fused_chunk<G, R, DENSE, MSPARSE, true>(p, full, lane, sa);
   if (!DENSE) {
     uint32_t na = sa.n_above;
 #pragma unroll
@@ -579,6 +608,13 @@ __global__ void fill_u32_kernel(uint32_t* p, int64_t n, uint32_t v) {
 
 __global__ void iota_i32_kernel(int32_t* p, int64_t n) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) p[i] = (int32_t)i;
+}
+
+// dense[idx[j]] = packed[j]  (dense view of a sparsely stored m, for the accessors)
+__global__ void scatter_packed_kernel(float* __restrict__ dense, const int32_t* __restrict__ idx,
+                                      const float* __restrict__ packed, int64_t count) {
+  for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < count; j += (int64_t)gridDim.x * blockDim.x)
+    dense[idx[j]] = packed[j];
 }
 
 // all-ones mask over [0,N), zero padding bits up to n_words*32
