@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -69,6 +70,7 @@ struct scape {
   int64_t packed_stride = 0;
   float* pm[2] = {nullptr, nullptr};   // packed means b- [packed_stride], alternating
   int pm_last = 0;             // pm[pm_last] = b- of the last sparse step
+  int fused_impl = 0;          // 0 auto (bulk-copy staged kernel in steady state), 1 = LDG kernel only
   bool m_sparse = false;       // m_{t-1} lives in pm[pm_last] addressed through slot[last]; h->m is stale
   float* dense_pack = nullptr;    // optional [R][Npad]
   bool last_dense = false;
@@ -146,9 +148,65 @@ int launch_fused_r(scape* h, StepParams& p, cudaStream_t st) {
   return fail(SCAPE_EINVAL, "R out of range");
 }
 
+// steady-state front-end with shared-memory staging (bulk copies + mbarriers)
+template <typename G, int R>
+int launch_tma_t(scape* h, StepParams& p, cudaStream_t st) {
+  static int cfg_stages = 0, cfg_bps = 0;
+  constexpr uint32_t TILE = tma_tile_bytes<G, R>();
+  if (cfg_stages == 0) {
+    // two CTAs per SM when at least 3 stages each fit, else one CTA with as many stages as fit
+    const int budget = 227 * 1024;
+    int s2 = (int)((budget / 2 - 1024 - kTmaBarrierBytes) / TILE);
+    int s1 = (int)((budget - kTmaBarrierBytes) / TILE);
+    if (s2 >= 3) { cfg_stages = s2 > kTmaMaxStages ? kTmaMaxStages : s2; cfg_bps = 2; }
+    else { cfg_stages = s1 > kTmaMaxStages ? kTmaMaxStages : s1; cfg_bps = 1; }
+    // tuning overrides (experiments only)
+    if (const char* ev = getenv("SCAPE_TMA_STAGES")) { int v = atoi(ev); if (v >= 2 && v <= kTmaMaxStages && v <= s1) cfg_stages = v; }
+    if (const char* ev = getenv("SCAPE_TMA_BPS")) { int v = atoi(ev); if (v >= 1 && v <= 4) cfg_bps = v; }
+    if (cfg_stages < 2) { cfg_stages = -1; }
+    else {
+      const size_t smem = kTmaBarrierBytes + (size_t)cfg_stages * TILE;
+      CU_TRY(cudaFuncSetAttribute(scape_fused_tma_kernel<G, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    }
+  }
+  if (cfg_stages < 0) return 1;   // does not fit: caller uses the LDG kernel
+  const int64_t n_tiles = p.N / kTmaTile;
+  int64_t grid = (int64_t)h->n_sm * cfg_bps;
+  if (grid > n_tiles) grid = n_tiles;
+  h->n_seg = (int)grid * kTmaConsumerWarps;
+  int64_t cap = (h->cand_cap / h->n_seg) & ~(int64_t)15;
+  if (cap > 0x7FFFFFF0) cap = 0x7FFFFFF0;
+  h->seg_cap = (uint32_t)cap;
+  p.seg_cap = h->seg_cap;
+  const size_t smem = kTmaBarrierBytes + (size_t)cfg_stages * TILE;
+  scape_fused_tma_kernel<G, R><<<(int)grid, kTmaThreads, smem, st>>>(p, cfg_stages);
+  h->launches++;
+  CU_TRY(cudaGetLastError());
+  return SCAPE_OK;
+}
+
+template <typename G>
+int launch_tma_r(scape* h, StepParams& p, cudaStream_t st) {
+  switch (h->R) {
+    case 1: return launch_tma_t<G, 1>(h, p, st);
+    case 2: return launch_tma_t<G, 2>(h, p, st);
+    case 3: return launch_tma_t<G, 3>(h, p, st);
+    case 4: return launch_tma_t<G, 4>(h, p, st);
+    case 5: return launch_tma_t<G, 5>(h, p, st);
+    case 6: return launch_tma_t<G, 6>(h, p, st);
+    case 7: return launch_tma_t<G, 7>(h, p, st);
+    case 8: return launch_tma_t<G, 8>(h, p, st);
+  }
+  return fail(SCAPE_EINVAL, "R out of range");
+}
+
 // variants: all-ones mask (dense m in and out) | sparse mask, dense m in | sparse mask, sparse m in
 template <typename G>
 int launch_fused_g(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t st) {
+  if (!dense && msparse && h->fused_impl != 1 && p.N / kTmaTile >= (int64_t)h->n_sm) {
+    const int rc = launch_tma_r<G>(h, p, st);
+    if (rc <= 0) return rc;      // 1 = tile does not fit in shared memory: fall through
+  }
   if (dense) return launch_fused_r<G, true, false>(h, p, st);
   return msparse ? launch_fused_r<G, false, true>(h, p, st) : launch_fused_r<G, false, false>(h, p, st);
 }
@@ -266,6 +324,7 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   scape* h = new (std::nothrow) scape();
   if (!h) { fail(SCAPE_ENOMEM, "host allocation failed"); return nullptr; }
   h->dev = dev;
+  if (const char* ev = getenv("SCAPE_FUSED_IMPL")) h->fused_impl = (strcmp(ev, "ldg") == 0) ? 1 : 0;
   cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev);
   h->N = N; h->R = R;
   h->Npad = (N + kChunk - 1) / kChunk * kChunk;

@@ -149,36 +149,13 @@ struct StageA {                 // per-warp running state of the fused select (r
   unsigned long long* seg;      // this warp's candidate segment
 };
 
-template <typename G, int R, bool DENSE, bool MSPARSE, bool GUARD>
-__device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int lane, StageA& sa) {
-  const int64_t i0 = (c << 7) + ((int64_t)lane << 2);
-  // Issue order matters for latency: the mask words first (L2-resident, short latency), then the
-  // 2R+1 streaming loads, and only then the gather of m_{t-1}, whose addresses depend on the
-  // mask words -- it is in flight together with the streaming loads instead of after them.
-  uint4 cw = make_uint4(~0u, ~0u, ~0u, ~0u), pw = make_uint4(0, 0, 0, 0);
-  uint32_t cr = 0, pr = 0;
-  if (!DENSE) { cw = __ldg(reinterpret_cast<const uint4*>(p.cur_bits) + c); cr = __ldg(p.cur_rank + c); }
-  if (MSPARSE) { pw = __ldg(reinterpret_cast<const uint4*>(p.prev_bits) + c); pr = __ldg(p.prev_rank + c); }
-
-  float th[4], mo[4], gg[R][4], ee[R][4];
-  load4_f32<GUARD>(p.theta, i0, p.N, th);
-  if (!MSPARSE) load4_f32<false>(p.m, i0, p.N, mo);         // own arrays are padded to Npad
-#pragma unroll
-  for (int r = 0; r < R; ++r) {
-    load4_grad<G, GUARD>(p.g[r], i0, p.N, gg[r]);
-    load4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
-  }
-
-  uint32_t mybits = 0xFu, jbase = 0;
-  if (!DENSE) lane_bits_from_words(cw, cr, lane, mybits, jbase);
-  if (MSPARSE) {
-    uint32_t pbits, pbase;
-    lane_bits_from_words(pw, pr, lane, pbits, pbase);
-#pragma unroll
-    for (int q = 0; q < 4; ++q)
-      mo[q] = ((pbits >> q) & 1u) ? __ldg(p.pm_prev + pbase + __popc(pbits & ((1u << q) - 1u))) : 0.0f;
-  }
-
+// The arithmetic of one lane's 4 elements (Alg. 1 l.6-10, l.12-17 in the pinned order), the stores
+// of theta / m / e^r / b^r / b-, and the bracket classification of stage 2.  Shared by the two
+// load front-ends (register-staged LDG and shared-memory-staged bulk copies).
+template <int R, bool DENSE, bool GUARD>
+__device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, int lane, int64_t i0,
+                                              uint32_t mybits, uint32_t jbase, float (&th)[4], const float (&mo)[4],
+                                              float (&gg)[R][4], float (&ee)[R][4], StageA& sa) {
   float mn[4];
   uint32_t key0[4];             // bits(|m~^0|): the selection statistic of l.11
 #pragma unroll
@@ -245,6 +222,39 @@ __device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int 
   }
 }
 
+template <typename G, int R, bool DENSE, bool MSPARSE, bool GUARD>
+__device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int lane, StageA& sa) {
+  const int64_t i0 = (c << 7) + ((int64_t)lane << 2);
+  // Issue order matters for latency: the mask words first (L2-resident, short latency), then the
+  // 2R+1 streaming loads, and only then the gather of m_{t-1}, whose addresses depend on the
+  // mask words -- it is in flight together with the streaming loads instead of after them.
+  uint4 cw = make_uint4(~0u, ~0u, ~0u, ~0u), pw = make_uint4(0, 0, 0, 0);
+  uint32_t cr = 0, pr = 0;
+  if (!DENSE) { cw = __ldg(reinterpret_cast<const uint4*>(p.cur_bits) + c); cr = __ldg(p.cur_rank + c); }
+  if (MSPARSE) { pw = __ldg(reinterpret_cast<const uint4*>(p.prev_bits) + c); pr = __ldg(p.prev_rank + c); }
+
+  float th[4], mo[4], gg[R][4], ee[R][4];
+  load4_f32<GUARD>(p.theta, i0, p.N, th);
+  if (!MSPARSE) load4_f32<false>(p.m, i0, p.N, mo);         // own arrays are padded to Npad
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    load4_grad<G, GUARD>(p.g[r], i0, p.N, gg[r]);
+    load4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
+  }
+
+  uint32_t mybits = 0xFu, jbase = 0;
+  if (!DENSE) lane_bits_from_words(cw, cr, lane, mybits, jbase);
+  if (MSPARSE) {
+    uint32_t pbits, pbase;
+    lane_bits_from_words(pw, pr, lane, pbits, pbase);
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+      mo[q] = ((pbits >> q) & 1u) ? __ldg(p.pm_prev + pbase + __popc(pbits & ((1u << q) - 1u))) : 0.0f;
+  }
+
+  fused_compute<R, DENSE, GUARD>(p, c, lane, i0, mybits, jbase, th, mo, gg, ee, sa);
+}
+
 template <typename G, int R, bool DENSE, bool MSPARSE>
 __global__ void __launch_bounds__(256, (R <= 4 ? 3 : 2)) scape_fused_step_kernel(const __grid_constant__ StepParams p) {
   const int lane = threadIdx.x & 31;
@@ -265,6 +275,197 @@ __global__ void __launch_bounds__(256, (R <= 4 ? 3 : 2)) scape_fused_step_kernel
     for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
     if (lane == 0) { p.seg_count[warp] = sa.cursor; p.seg_above[warp] = na; }
   }
+}
+
+// ------------------------------------------------------------------------------------------
+// Steady-state variant with shared-memory staging (sparse mask in, m stored sparsely).
+//
+// The LDG kernel above keeps every byte in flight in registers (2R+1 128-bit loads per lane), so
+// registers bound the memory-level parallelism (80 regs -> 24 warps/SM -> ~86 KB in flight per
+// SM).  Here one producer lane per CTA streams whole tiles of 1024 parameters (theta, e^r, g^r
+// slices: 1+2R bulk copies, `cp.async.bulk` = SASS UBLKCP, completion counted in bytes on an
+// mbarrier) into a ring of shared-memory stages; 8 consumer warps wait on the stage's "full"
+// barrier, pull their 128-bit slices out of shared memory, release the stage ("empty" barrier,
+// one arrival per warp) and do the arithmetic and the (fire-and-forget) global stores from
+// registers.  Bytes in flight = (stages-1) x tile per CTA, independent of register pressure.
+// ------------------------------------------------------------------------------------------
+constexpr int kTmaConsumerWarps = 8;
+constexpr int kTmaTile = kTmaConsumerWarps * kChunk;          // 1024 parameters
+constexpr int kTmaThreads = (kTmaConsumerWarps + 1) * 32;     // + 1 producer warp
+constexpr int kTmaMaxStages = 8;
+constexpr int kTmaBarrierBytes = 128;                         // full[8] + empty[8]
+
+template <typename G, int R>
+__host__ __device__ constexpr uint32_t tma_tile_bytes() { return kTmaTile * 4u * (1u + R) + kTmaTile * (uint32_t)sizeof(G) * R; }
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// 1-D bulk copy global -> shared, completion signalled on `bar` in bytes; L2 evict-first policy
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, uint32_t bytes, uint64_t* bar, uint64_t policy) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+               ::"r"(smem_u32(dst_smem)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy) : "memory");
+}
+
+struct TmaMaskWords { uint4 cw, pw; uint32_t cr, pr; };
+struct TmaTileState { uint32_t mybits, jbase; float mo[4]; };
+
+__device__ __forceinline__ void tma_load_words(const StepParams& p, int64_t c, TmaMaskWords& w) {
+  w.cw = __ldg(reinterpret_cast<const uint4*>(p.cur_bits) + c); w.cr = __ldg(p.cur_rank + c);
+  w.pw = __ldg(reinterpret_cast<const uint4*>(p.prev_bits) + c); w.pr = __ldg(p.prev_rank + c);
+}
+// decode a chunk's mask words for this lane and start the gather of m_{t-1}
+__device__ __forceinline__ void tma_decode_gather(const StepParams& p, const TmaMaskWords& w, int lane, TmaTileState& st) {
+  uint32_t pbits, pbase;
+  lane_bits_from_words(w.cw, w.cr, lane, st.mybits, st.jbase);
+  lane_bits_from_words(w.pw, w.pr, lane, pbits, pbase);
+#pragma unroll
+  for (int q = 0; q < 4; ++q)
+    st.mo[q] = ((pbits >> q) & 1u) ? __ldg(p.pm_prev + pbase + __popc(pbits & ((1u << q) - 1u))) : 0.0f;
+}
+
+// One tile of one consumer warp: start the next tile's gather, wait for this tile's bytes, pull
+// them out of shared memory, release the stage, compute and store.
+template <typename G, int R>
+__device__ __forceinline__ void tma_consume_tile(const StepParams& p, int64_t tile, int64_t n_tiles, int64_t tstride,
+                                                 int warp, int lane, unsigned char* stage0, uint64_t* full, uint64_t* empty,
+                                                 int& s, uint32_t& ph, int n_stages, TmaMaskWords& nw,
+                                                 TmaTileState& cur, TmaTileState& nxt, StageA& sa) {
+  constexpr uint32_t TILE = tma_tile_bytes<G, R>();
+  constexpr uint32_t OFF_E = kTmaTile * 4u, OFF_G = kTmaTile * 4u * (1u + R);
+  const int64_t c = tile * kTmaConsumerWarps + warp;
+  const int64_t i0 = (c << 7) + ((int64_t)lane << 2);
+  if (tile + tstride < n_tiles) {
+    tma_decode_gather(p, nw, lane, nxt);
+    if (tile + 2 * tstride < n_tiles) tma_load_words(p, (tile + 2 * tstride) * kTmaConsumerWarps + warp, nw);
+  }
+  mbar_wait(&full[s], ph);
+  const unsigned char* base = stage0 + (size_t)s * TILE;
+  const uint32_t off = (uint32_t)(warp * kChunk + (lane << 2));
+  float th[4], gg[R][4], ee[R][4];
+  {
+    const float4 t = *reinterpret_cast<const float4*>(base + off * 4u);
+    th[0] = t.x; th[1] = t.y; th[2] = t.z; th[3] = t.w;
+  }
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    const float4 t = *reinterpret_cast<const float4*>(base + OFF_E + r * (kTmaTile * 4u) + off * 4u);
+    ee[r][0] = t.x; ee[r][1] = t.y; ee[r][2] = t.z; ee[r][3] = t.w;
+    if constexpr (sizeof(G) == 4) {
+      const float4 g = *reinterpret_cast<const float4*>(base + OFF_G + r * (kTmaTile * 4u) + off * 4u);
+      gg[r][0] = g.x; gg[r][1] = g.y; gg[r][2] = g.z; gg[r][3] = g.w;
+    } else {
+      const uint2 g = *reinterpret_cast<const uint2*>(base + OFF_G + r * (kTmaTile * 2u) + off * 2u);
+      gg[r][0] = __uint_as_float(g.x << 16); gg[r][1] = __uint_as_float(g.x & 0xFFFF0000u);
+      gg[r][2] = __uint_as_float(g.y << 16); gg[r][3] = __uint_as_float(g.y & 0xFFFF0000u);
+    }
+  }
+  __syncwarp();
+  if (lane == 0) mbar_arrive(&empty[s]);                        // this warp is done with the stage
+  if (++s == n_stages) { s = 0; ph ^= 1u; }
+  fused_compute<R, false, false>(p, c, lane, i0, cur.mybits, cur.jbase, th, cur.mo, gg, ee, sa);
+}
+
+template <typename G, int R>
+__global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const __grid_constant__ StepParams p, int n_stages) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  constexpr uint32_t TILE = tma_tile_bytes<G, R>();
+  constexpr uint32_t OFF_E = kTmaTile * 4u, OFF_G = kTmaTile * 4u * (1u + R);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem);
+  uint64_t* empty = full + kTmaMaxStages;
+  unsigned char* stage0 = smem + kTmaBarrierBytes;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t n_tiles = p.N / kTmaTile;                     // full tiles; the rest goes through the LDG path
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < n_stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], kTmaConsumerWarps); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (warp == kTmaConsumerWarps) {
+    // ===== producer: one lane streams the tiles of this CTA =====
+    if (lane == 0) {
+      uint64_t policy;
+      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+      int s = 0; uint32_t ph = 0;
+      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        mbar_wait(&empty[s], ph ^ 1u);                         // every consumer warp has read the old contents
+        mbar_expect_tx(&full[s], TILE);
+        unsigned char* base = stage0 + (size_t)s * TILE;
+        const int64_t e0 = tile * kTmaTile;
+        bulk_g2s(base, p.theta + e0, kTmaTile * 4u, &full[s], policy);
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+          bulk_g2s(base + OFF_E + r * (kTmaTile * 4u), p.e + r * p.e_stride + e0, kTmaTile * 4u, &full[s], policy);
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+          bulk_g2s(base + OFF_G + r * (kTmaTile * (uint32_t)sizeof(G)),
+                   reinterpret_cast<const unsigned char*>(p.g[r]) + e0 * (int64_t)sizeof(G),
+                   kTmaTile * (uint32_t)sizeof(G), &full[s], policy);
+        if (++s == n_stages) { s = 0; ph ^= 1u; }
+      }
+    }
+    return;
+  }
+
+  // ===== consumers =====
+  const int64_t gwarp = (int64_t)blockIdx.x * kTmaConsumerWarps + warp;     // candidate segment of this warp
+  StageA sa{};
+  sa.lo = p.ctl->lo_key; sa.hi = p.ctl->hi_key;
+  sa.seg = p.cand + (size_t)gwarp * p.seg_cap;
+
+  // Software pipeline of the small dependent accesses, so that none of their latency is exposed
+  // once a tile has landed: mask words are fetched two tiles ahead, and the gather of m_{t-1}
+  // (whose addresses come from the previous mask's words) one tile ahead.  The per-tile state
+  // ping-pongs between two register sets (A, B) so that no register move has to wait for a load.
+  const int64_t tstride = gridDim.x;
+  int64_t tile = blockIdx.x;
+  TmaMaskWords nw{};                                   // raw words of the NEXT tile
+  TmaTileState stA{}, stB{};
+  if (tile < n_tiles) {
+    TmaMaskWords w0;
+    tma_load_words(p, tile * kTmaConsumerWarps + warp, w0);
+    if (tile + tstride < n_tiles) tma_load_words(p, (tile + tstride) * kTmaConsumerWarps + warp, nw);
+    tma_decode_gather(p, w0, lane, stA);
+  }
+  int s = 0; uint32_t ph = 0;
+  while (tile < n_tiles) {
+    tma_consume_tile<G, R>(p, tile, n_tiles, tstride, warp, lane, stage0, full, empty, s, ph, n_stages, nw, stA, stB, sa);
+    tile += tstride;
+    if (tile >= n_tiles) break;
+    tma_consume_tile<G, R>(p, tile, n_tiles, tstride, warp, lane, stage0, full, empty, s, ph, n_stages, nw, stB, stA, sa);
+    tile += tstride;
+  }
+
+  // chunks past the last full tile (fewer than 8, the last one possibly ragged): LDG path
+  {
+    const int64_t c = n_tiles * kTmaConsumerWarps + warp;
+    if (c < p.n_chunks && blockIdx.x == (unsigned)(n_tiles % gridDim.x)) {
+      if (((c + 1) << 7) <= p.N) fused_chunk<G, R, false, true, false>(p, c, lane, sa);
+      else fused_chunk<G, R, false, true, true>(p, c, lane, sa);
+    }
+  }
+  uint32_t na = sa.n_above;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
+  if (lane == 0) { p.seg_count[gwarp] = sa.cursor; p.seg_above[gwarp] = na; }
 }
 
 // ------------------------------------------------------------------------------------------
