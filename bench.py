@@ -209,6 +209,22 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def max_over_ranks_ms(ms, world, device):
+    """Device time of the slowest rank (every multi-GPU number is the max over ranks)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(n_params, steps, elapsed_ms, world):
+    """params/s of the whole job: every rank processed n_params * steps in elapsed_ms (replicas only)."""
+    return world * n_params * steps / (elapsed_ms * 1e-3)
+
+
 # ---------------------------------------------------------------------------------------------
 def main():
     args = parse()
@@ -269,21 +285,20 @@ def main():
     torch.cuda.synchronize()
     elapsed_ms = t0.elapsed_time(t1)
     fused_ms, select_ms, psteps = sc.profile_read()
+    kernel_name = sc.last_kernel
     sc.profile(False)
     gpu_launches = sc.launches - launches0
     fast1, general1 = sc.select_stats()
     clk = clocks.stop() if rank == 0 else None
+    elapsed_ms = max_over_ranks_ms(elapsed_ms, world, dev)
     if world > 1:
-        tt = torch.tensor([elapsed_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        elapsed_ms = float(tt.item())
         dist.barrier()
     assert bool(torch.isfinite(theta).all()), "theta is not finite after the timed steps"
     mask_count = sc.count_next()
     assert mask_count == k, (mask_count, k)
 
     ms_per_step = elapsed_ms / K
-    value = world * N * K / (elapsed_ms * 1e-3)
+    value = whole_job_value(N, K, elapsed_ms, world)
 
     # ---- roofline of the dominant kernel -------------------------------------------------
     peak, peak_src = measured_peak()
@@ -292,7 +307,7 @@ def main():
     achieved = fb / (fused_avg_ms * 1e-3) / 1e9
     sb = bytes_per_param_step(w, k, N) * N
     roofline = {
-        "bound": "hbm", "kernel": "scape_fused_step_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+        "bound": "hbm", "kernel": kernel_name, "achieved": achieved, "peak": peak, "unit": "GB/s",
         "frac": achieved / peak, "traffic": recorded_traffic(w.name),
         "peak_source": peak_src, "algorithmic_bytes_per_launch": fb, "kernel_ms": fused_avg_ms,
         "kernel_share_of_step": fused_avg_ms / ms_per_step,
@@ -329,12 +344,9 @@ def main():
         b.record()
         torch.cuda.synchronize()
         e2e_ms = a.elapsed_time(b)
-        if world > 1:
-            tt = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            e2e_ms = float(tt.item())
+        e2e_ms = max_over_ranks_ms(e2e_ms, world, dev)
         gbytes = N * grad_bytes(w) * R
-        e2e = {"value": world * N * n_e2e / (e2e_ms * 1e-3), "unit": UNIT,
+        e2e = {"value": whole_job_value(N, n_e2e, e2e_ms, world), "unit": UNIT,
                "h2d_bytes_per_step": 4 * N + gbytes, "d2h_bytes_per_step": 4 * N,
                "steps": n_e2e, "ms_per_step": e2e_ms / n_e2e,
                "api": "scape_step_host (pinned host param + R gradient buffers in, param out)"}

@@ -95,6 +95,11 @@ int64_t scape_k(const scape_t* h);
 int64_t scape_step_count(const scape_t* h);
 int64_t scape_launch_count(const scape_t* h);
 
+/* Name of the streaming kernel the last step launched: "scape_fused_tma_kernel" (steady state:
+ * bulk-copy staged) or "scape_fused_step_kernel" (register-staged: all-ones steps, dense m, small
+ * or odd shapes), "" before the first step.  Static string, never NULL.                         */
+const char* scape_last_kernel(const scape_t* h);
+
 /* Number of entries of SCAPE_MASK_NEXT / SCAPE_MASK_LAST (N while the mask is all ones, else
  * k); `which` is one of those two selectors.  Negative code on error.                           */
 int64_t scape_count(const scape_t* h, int which);

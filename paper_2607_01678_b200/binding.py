@@ -29,6 +29,7 @@ SYMBOLS = {
     "scape_k": (_I64, [_VP]),
     "scape_step_count": (_I64, [_VP]),
     "scape_launch_count": (_I64, [_VP]),
+    "scape_last_kernel": (ctypes.c_char_p, [_VP]),
     "scape_count": (_I64, [_VP, _I]),
     "scape_set_grad_dtype": (_I, [_VP, _I]),
     "scape_set_keep_dense_pack": (_I, [_VP, _I]),
@@ -106,6 +107,10 @@ def scape_launch_count(h):
     return int(lib().scape_launch_count(h))
 
 
+def scape_last_kernel(h):
+    return lib().scape_last_kernel(h).decode()
+
+
 def scape_count(h, which):
     n = int(lib().scape_count(h, which))
     if n < 0:
@@ -177,6 +182,10 @@ class Scape:
     @property
     def t(self):
         return scape_step_count(self.h)
+
+    @property
+    def last_kernel(self):
+        return scape_last_kernel(self.h)
 
     @property
     def launches(self):

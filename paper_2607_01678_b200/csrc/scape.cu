@@ -70,6 +70,7 @@ struct scape {
   int64_t packed_stride = 0;
   float* pm[2] = {nullptr, nullptr};   // packed means b- [packed_stride], alternating
   int pm_last = 0;             // pm[pm_last] = b- of the last sparse step
+  const char* last_kernel = "";   // name of the streaming kernel the last step launched
   int fused_impl = 0;          // 0 auto (bulk-copy staged kernel in steady state), 1 = LDG kernel only
   bool m_sparse = false;       // m_{t-1} lives in pm[pm_last] addressed through slot[last]; h->m is stale
   float* dense_pack = nullptr;    // optional [R][Npad]
@@ -128,6 +129,7 @@ int launch_fused_t(scape* h, StepParams& p, cudaStream_t st) {
   h->seg_cap = (uint32_t)cap;
   p.seg_cap = h->seg_cap;
   scape_fused_step_kernel<G, R, DENSE, MSPARSE><<<grid, 256, 0, st>>>(p);
+  h->last_kernel = "scape_fused_step_kernel";
   h->launches++;
   CU_TRY(cudaGetLastError());
   return SCAPE_OK;
@@ -180,6 +182,7 @@ int launch_tma_t(scape* h, StepParams& p, cudaStream_t st) {
   p.seg_cap = h->seg_cap;
   const size_t smem = kTmaBarrierBytes + (size_t)cfg_stages * TILE;
   scape_fused_tma_kernel<G, R><<<(int)grid, kTmaThreads, smem, st>>>(p, cfg_stages);
+  h->last_kernel = "scape_fused_tma_kernel";
   h->launches++;
   CU_TRY(cudaGetLastError());
   return SCAPE_OK;
@@ -404,6 +407,7 @@ extern "C" void scape_destroy(scape_t* h) {
 extern "C" int64_t scape_k(const scape_t* h) { return h ? h->k : SCAPE_EINVAL; }
 extern "C" int64_t scape_step_count(const scape_t* h) { return h ? h->t : SCAPE_EINVAL; }
 extern "C" int64_t scape_launch_count(const scape_t* h) { return h ? h->launches : SCAPE_EINVAL; }
+extern "C" const char* scape_last_kernel(const scape_t* h) { return h ? h->last_kernel : ""; }
 
 extern "C" int64_t scape_count(const scape_t* h, int which) {
   if (!h) return fail(SCAPE_EINVAL, "NULL handle");

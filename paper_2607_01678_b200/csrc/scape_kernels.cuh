@@ -162,29 +162,40 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
   for (int q = 0; q < 4; ++q) {
     const bool on = DENSE || ((mybits >> q) & 1u);
     const float pq = __fmul_rn(p.b1, mo[q]);                // beta1 * m_{t-1}, reused by l.6 and l.13
-    const int64_t j = DENSE ? (i0 + q) : (int64_t)(jbase + __popc(mybits & ((1u << q) - 1u)));
-    float s = 0.0f;
+    float mt[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-      const float mt = __fadd_rn(__fmaf_rn(p.c1, gg[r][q], pq), ee[r][q]);   // l.6
-      if (r == 0) key0[q] = __float_as_uint(mt) & 0x7FFFFFFFu;
-      ee[r][q] = on ? ((DENSE && r == 0 && p.stash) ? mt : 0.0f) : mt;       // l.7-8
-      if (on) {
-        if (!DENSE || p.packed != nullptr) {
-          if (!GUARD || i0 + q < p.N) p.packed[r * p.packed_stride + j] = mt;   // l.9
-        }
-        s = (r == 0) ? mt : __fadd_rn(s, mt);                                // l.10, r ascending
-      }
+      mt[r] = __fadd_rn(__fmaf_rn(p.c1, gg[r][q], pq), ee[r][q]);            // l.6
+      ee[r][q] = on ? ((DENSE && r == 0 && p.stash) ? mt[r] : 0.0f) : mt[r]; // l.7-8
     }
+    key0[q] = __float_as_uint(mt[0]) & 0x7FFFFFFFu;
     float u = 0.0f;                                                          // Eq. 5: u = 0 off the mask
     mn[q] = 0.0f;                                                            // Eq. 4: m = 0 off the mask
-    if (on) {
-      const float bb = p.r_pow2 ? __fmul_rn(s, p.inv_R) : __fdiv_rn(s, p.R_f);    // l.10
-      const float gh = __fdiv_rn(__fsub_rn(bb, pq), p.c1);                          // l.13 (Eq. 3)
-      const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), __fmul_rn(p.b2, __fmul_rn(mo[q], mo[q])));  // l.15
-      u = __fdiv_rn(bb, __fadd_rn(__fsqrt_rn(v), p.eps));                           // l.16
-      mn[q] = bb;                                                                   // l.12
-      if (!DENSE) p.packed_mean[j] = bb;
+    // At 90-99 % sparsity most warps have no selected element at a given q: a warp-uniform vote
+    // skips the pack, the replica mean and the IEEE divisions / square root entirely.
+    if (DENSE || __any_sync(0xFFFFFFFFu, on)) {
+      if (on) {
+        const uint32_t j = DENSE ? 0u : jbase + __popc(mybits & ((1u << q) - 1u));
+        float s = mt[0];
+        if (DENSE) {
+          if (p.packed != nullptr && (!GUARD || i0 + q < p.N)) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) p.packed[r * p.packed_stride + (i0 + q)] = mt[r];   // l.9 (keep_dense_pack)
+          }
+        } else {
+          float* pk = p.packed + j;
+#pragma unroll
+          for (int r = 0; r < R; ++r) { *pk = mt[r]; pk += p.packed_stride; }                  // l.9
+        }
+#pragma unroll
+        for (int r = 1; r < R; ++r) s = __fadd_rn(s, mt[r]);                                   // l.10, r ascending
+        const float bb = p.r_pow2 ? __fmul_rn(s, p.inv_R) : __fdiv_rn(s, p.R_f);              // l.10
+        const float gh = __fdiv_rn(__fsub_rn(bb, pq), p.c1);                                    // l.13 (Eq. 3)
+        const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), __fmul_rn(p.b2, __fmul_rn(mo[q], mo[q])));  // l.15
+        u = __fdiv_rn(bb, __fadd_rn(__fsqrt_rn(v), p.eps));                                     // l.16
+        mn[q] = bb;                                                                             // l.12
+        if (!DENSE) p.packed_mean[j] = bb;
+      }
     }
     const float w = __fmaf_rn(p.wd, th[q], u);                                      // l.17
     th[q] = __fmaf_rn(p.neg_lr, w, th[q]);
@@ -198,20 +209,26 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
   if (!DENSE) {
     // Stage 2 (l.11) fused: classify |m~^0| against the predicted bracket.  Exactness does not
     // depend on the prediction: sel_decide_kernel checks n_above < k <= n_above + n_cand.
-    uint32_t nib = 0;
+    uint32_t nib = 0, cnib = 0;
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       const bool valid = !GUARD || (i0 + q < p.N);
       const bool above = valid && key0[q] >= sa.hi;
-      const bool cnd = valid && !above && key0[q] >= sa.lo;
       nib |= above ? (1u << q) : 0u;
-      const uint32_t bal = __ballot_sync(0xFFFFFFFFu, cnd);
-      if (cnd) {
-        const uint32_t pos = sa.cursor + __popc(bal & ((1u << lane) - 1u));
-        if (pos < p.seg_cap)
-          sa.seg[pos] = ((unsigned long long)key0[q] << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)(i0 + q));
+      cnib |= (valid && !above && key0[q] >= sa.lo) ? (1u << q) : 0u;
+    }
+    if (__any_sync(0xFFFFFFFFu, cnib != 0u)) {              // candidates are rare: usually skipped
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const bool cnd = (cnib >> q) & 1u;
+        const uint32_t bal = __ballot_sync(0xFFFFFFFFu, cnd);
+        if (cnd) {
+          const uint32_t pos = sa.cursor + __popc(bal & ((1u << lane) - 1u));
+          if (pos < p.seg_cap)
+            sa.seg[pos] = ((unsigned long long)key0[q] << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)(i0 + q));
+        }
+        sa.cursor += __popc(bal);
       }
-      sa.cursor += __popc(bal);
     }
     sa.n_above += __popc(nib);
     uint32_t w = nib << ((lane & 7) << 2);

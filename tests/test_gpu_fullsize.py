@@ -1,0 +1,130 @@
+"""Parity at BASELINE.json's full size, in the launch configuration bench.py times — `-m gpu`.
+
+The headline workload (Llama-1.8B-shaped shard: N = 1,775,239,168, R = 4 bf16 gradient buffers,
+99 % sparsity) is far too large for the CPU oracle as a whole, so the step is checked
+  (a) element by element on a SAMPLE of positions: the inputs of the sampled positions (theta, m,
+      e^r, g^r, mask bit) are gathered before the step, handed to the oracle as a small problem
+      of their own, and its outputs compared bit for bit with what the kernels wrote there; and
+  (b) through properties that hold at any size: exactly k bits in M_t, ascending in-range index
+      list, and the top-k property itself (every selected key >= every unselected key, ties to
+      the lower index), evaluated with plain torch ops on the statistic |m~^0| rebuilt from the
+      new e^0 and b^0 (pin P2).
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle.scape_oracle import ScapeOracle  # noqa: E402
+from paper_2607_01678_b200 import synth  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+
+def unpack_bits(words_t, n):
+    """uint32 words (torch, device) -> bool tensor [n]"""
+    shifts = torch.arange(32, device=words_t.device, dtype=torch.int32)
+    bits = (words_t.to(torch.int32).unsqueeze(1) >> shifts) & 1
+    return bits.reshape(-1)[:n].bool()
+
+
+def get_mask_device(B, sc, which, N):
+    nw = (N + 31) // 32
+    buf = torch.empty(nw, dtype=torch.int32, device="cuda")
+    B.scape_get(sc.h, which, 0, buf.data_ptr(), nw * 4, torch.cuda.current_stream().cuda_stream)
+    return unpack_bits(buf, N)
+
+
+def get_f32_device(B, sc, what, r, n):
+    buf = torch.empty(n, dtype=torch.float32, device="cuda")
+    B.scape_get(sc.h, what, r, buf.data_ptr(), n * 4, torch.cuda.current_stream().cuda_stream)
+    return buf
+
+
+@pytest.mark.parametrize("name", ["llama1p8b"])
+def test_fullsize_sampled_and_property_parity(name):
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    free, _ = torch.cuda.mem_get_info()
+    if free < 120e9:
+        pytest.skip("needs ~110 GB of free HBM")
+    from paper_2607_01678_b200 import binding as B
+    B.lib()
+    w = synth.workload(name)
+    N, R, k = w.numel, w.R, None
+    gs = synth.GradStream(w, device="cuda", seed=0)
+    theta = gs.theta0()
+    sc = B.Scape(N, R, w.sparsity, **w.hyper)
+    k = sc.k
+    # reach the steady state bench.py times: dense first step, then sparse steps with m stored sparsely
+    for _ in range(3):
+        sc.step(theta, gs.next())
+    torch.cuda.synchronize()
+    fast0, gen0 = sc.select_stats()
+
+    # ---- sample positions: random ones plus every kind of edge (first/last element, tile and
+    # chunk boundaries) plus a few hundred positions that ARE in the mask the step will use
+    rng = np.random.default_rng(0)
+    cur = get_mask_device(B, sc, B.SCAPE_MASK_NEXT, N)
+    on_idx = torch.nonzero(cur).flatten()
+    pick_on = on_idx[torch.from_numpy(rng.integers(0, on_idx.numel(), 600)).cuda()]
+    edges = [0, 1, 127, 128, 1023, 1024, N - 1, N - 2, N - 1024, (N // 1024) * 1024 - 1, (N // 1024) * 1024]
+    edges = [e for e in edges if 0 <= e < N]
+    samp = torch.cat([torch.from_numpy(rng.integers(0, N, 3000)).cuda(), pick_on, torch.tensor(edges, device="cuda")])
+    samp = torch.unique(samp)            # sorted ascending
+    S = samp.numel()
+
+    grads = gs.next()
+    m_before = get_f32_device(B, sc, B.SCAPE_MOMENT, 0, N)[samp].cpu().numpy()
+    e_before = [get_f32_device(B, sc, B.SCAPE_RESIDUAL, r, N)[samp].cpu().numpy() for r in range(R)]
+    th_before = theta[samp].cpu().numpy()
+    g_s = [g[samp].to(torch.float32).cpu().numpy() for g in grads]
+    cur_s = cur[samp].cpu().numpy().astype(np.uint8)
+    del cur, on_idx
+
+    sc.step(theta, grads)                # the step under test (steady state, full size)
+    torch.cuda.synchronize()
+    fast1, gen1 = sc.select_stats()
+
+    # ---- (a) sampled positions through the oracle, bit for bit
+    ora = ScapeOracle(S, R, 0.5, **w.hyper)          # its own top-k is irrelevant here
+    ora.set_m(m_before)
+    for r in range(R):
+        ora.set_e(r, e_before[r])
+    ora.set_mask(cur_s)
+    th_o = th_before.copy()
+    ora.step(th_o, g_s)
+    th_g = theta[samp].cpu().numpy()
+    assert np.array_equal(th_g.view(np.uint32), th_o.view(np.uint32)), "theta differs on sampled positions"
+    m_g = get_f32_device(B, sc, B.SCAPE_MOMENT, 0, N)[samp].cpu().numpy()
+    assert np.array_equal(m_g.view(np.uint32), ora.m().view(np.uint32)), "m differs on sampled positions"
+    e0_new = get_f32_device(B, sc, B.SCAPE_RESIDUAL, 0, N)
+    for r in range(R):
+        e_g = (e0_new if r == 0 else get_f32_device(B, sc, B.SCAPE_RESIDUAL, r, N))[samp].cpu().numpy()
+        assert np.array_equal(e_g.view(np.uint32), ora.e(r).view(np.uint32)), f"e[{r}] differs on sampled positions"
+
+    # ---- (b) properties at full size
+    assert sc.count_last() == k and sc.count_next() == k
+    nxt = get_mask_device(B, sc, B.SCAPE_MASK_NEXT, N)
+    assert int(nxt.sum()) == k
+    idx_next = torch.from_numpy(sc.idx_next()).cuda()
+    assert idx_next.numel() == k and bool((idx_next[1:] > idx_next[:-1]).all()) and int(idx_next[-1]) < N
+    assert bool(nxt[idx_next.long()].all())
+    # statistic |m~^0|: new e^0 off the mask the step used, b^0 on it
+    keys = e0_new.abs_()
+    idx_last = torch.from_numpy(sc.idx_last()).cuda().long()
+    b0 = get_f32_device(B, sc, B.SCAPE_PACKED, 0, k)
+    keys[idx_last] = b0.abs()
+    sel_min = keys[nxt].min()
+    keys_unsel = torch.where(nxt, torch.full_like(keys, -1.0), keys)
+    unsel_max = keys_unsel.max()
+    assert float(sel_min) >= float(unsel_max), (float(sel_min), float(unsel_max))
+    if float(sel_min) == float(unsel_max):           # tie class straddles the threshold: lower indices win
+        tie = keys == sel_min
+        last_sel = torch.nonzero(tie & nxt).flatten().max()
+        first_unsel = torch.nonzero(tie & ~nxt).flatten().min()
+        assert int(last_sel) < int(first_unsel)
+    # the timed configuration: fast select route with the bulk-copy staged kernel
+    assert fast1 - fast0 + gen1 - gen0 == 1
+    assert sc.last_kernel == "scape_fused_tma_kernel"
+    sc.close()
