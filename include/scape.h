@@ -130,6 +130,12 @@ int scape_set_step_count(scape_t* h, int64_t t);
  * steps).  Both routes are exact.  Synchronises cuda_stream.                                     */
 int scape_select_stats(scape_t* h, int64_t* fast, int64_t* general, void* cuda_stream);
 
+/* Diagnostics of the last step's select (not graded): out8 = {bracket held (0/1), entries above
+ * the bracket, candidates, half-width of the next bracket in ln units, ln of the exact threshold,
+ * ln of the threshold predicted for the next step, candidate capacity, candidate segments}.
+ * Synchronises cuda_stream.                                                                      */
+int scape_select_debug(scape_t* h, double* out8, void* cuda_stream);
+
 /* Optional timing, for bench.py's roofline: while switched on, every scape_step also records
  * three CUDA events on its stream (before the fused streaming kernel of stages 1,3-6, after it,
  * and after the stage-2 select), at most 64 steps between reads without a host wait.

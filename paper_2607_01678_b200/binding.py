@@ -37,6 +37,7 @@ SYMBOLS = {
     "scape_set": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
     "scape_set_step_count": (_I, [_VP, _I64]),
     "scape_select_stats": (_I, [_VP, _VP, _VP, _VP]),
+    "scape_select_debug": (_I, [_VP, _VP, _VP]),
     "scape_profile": (_I, [_VP, _I]),
     "scape_profile_read": (_I, [_VP, _VP, _VP, _VP]),
     "scape_last_error": (ctypes.c_char_p, []),
@@ -143,6 +144,13 @@ def scape_select_stats(h, stream=0):
     a, b = ctypes.c_int64(), ctypes.c_int64()
     _check(lib().scape_select_stats(h, ctypes.byref(a), ctypes.byref(b), stream), "scape_select_stats")
     return a.value, b.value
+
+
+def scape_select_debug(h, stream=0):
+    out = (ctypes.c_double * 8)()
+    _check(lib().scape_select_debug(h, out, stream), "scape_select_debug")
+    keys = ("hit", "n_above", "n_cand", "delta", "lnT", "ln_pred_next", "cand_cap", "n_seg")
+    return dict(zip(keys, list(out)))
 
 
 def scape_profile(h, on):
@@ -285,6 +293,9 @@ class Scape:
 
     def select_stats(self):
         return scape_select_stats(self.h, self._stream())
+
+    def select_debug(self):
+        return scape_select_debug(self.h, self._stream())
 
     def profile(self, on=True):
         scape_profile(self.h, on)

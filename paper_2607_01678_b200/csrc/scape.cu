@@ -160,13 +160,15 @@ int launch_tma_t(scape* h, StepParams& p, cudaStream_t st) {
     const int budget = 227 * 1024;
     int s2 = (int)((budget / 2 - 1024 - kTmaBarrierBytes) / TILE);
     int s1 = (int)((budget - kTmaBarrierBytes) / TILE);
+    // Two CTAs (16 consumer warps) per SM with >= 3 stages each, or not at all: with one CTA per
+    // SM the 8 consumer warps cannot keep up with HBM (measured: R = 8 fp32 gradients, 68 KB
+    // tiles, 4.8 TB/s staged vs 5.95 TB/s register-staged), so big tiles use the LDG kernel.
     if (s2 >= 3) { cfg_stages = s2 > kTmaMaxStages ? kTmaMaxStages : s2; cfg_bps = 2; }
-    else { cfg_stages = s1 > kTmaMaxStages ? kTmaMaxStages : s1; cfg_bps = 1; }
+    else { cfg_stages = -1; cfg_bps = 1; (void)s1; }
     // tuning overrides (experiments only)
     if (const char* ev = getenv("SCAPE_TMA_STAGES")) { int v = atoi(ev); if (v >= 2 && v <= kTmaMaxStages && v <= s1) cfg_stages = v; }
     if (const char* ev = getenv("SCAPE_TMA_BPS")) { int v = atoi(ev); if (v >= 1 && v <= 4) cfg_bps = v; }
-    if (cfg_stages < 2) { cfg_stages = -1; }
-    else {
+    if (cfg_stages >= 2) {
       const size_t smem = kTmaBarrierBytes + (size_t)cfg_stages * TILE;
       CU_TRY(cudaFuncSetAttribute(scape_fused_tma_kernel<G, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     }
@@ -261,11 +263,11 @@ int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general,
   const int grid = grid_for(h, h->n_chunks, 8, 6);
   sel_decide_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist, cl, (long long)h->k, force_general ? 1 : 0);
   h->launches++;
-  static const int shifts[kSelPasses] = {51, 38, 25, 12, 0};
-  static const int widths[kSelPasses] = {13, 13, 13, 13, 12};
+  // 64 undecided bits at most, 13 per pass; the kernels take the digit position from the state
+  // and return at once when nothing is left to decide (fast route: 4 passes are typical)
   for (int p = 0; p < kSelPasses; ++p) {
-    sel_hist_kernel<<<grid, 256, 0, st>>>(src, cl, h->sel, h->ghist, shifts[p], widths[p]);
-    sel_pick_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist, shifts[p], widths[p], p == kSelPasses - 1);
+    sel_hist_kernel<<<grid, 256, 0, st>>>(src, cl, h->sel, h->ghist);
+    sel_pick_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist);
     h->launches += 2;
   }
   sel_finish_kernel<<<grid, 256, 0, st>>>(src, cl, h->sel, nxt.bits);
@@ -525,6 +527,17 @@ extern "C" int scape_select_stats(scape_t* h, int64_t* fast, int64_t* general, v
   CU_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
   if (fast) *fast = (int64_t)s.n_fast;
   if (general) *general = (int64_t)s.n_general;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_select_debug(scape_t* h, double* out8, void* cuda_stream) {
+  if (!h || !out8) return fail(SCAPE_EINVAL, "NULL argument");
+  DeviceGuard guard(h->dev);
+  SelState s{};
+  CU_TRY(cudaMemcpyAsync(&s, h->sel, sizeof s, cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
+  CU_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+  out8[0] = s.hit; out8[1] = (double)s.n_above; out8[2] = (double)s.n_cand; out8[3] = s.delta;
+  out8[4] = s.lnT_prev; out8[5] = s.ln_pred; out8[6] = (double)s.cand_cap_total; out8[7] = (double)h->n_seg;
   return SCAPE_OK;
 }
 

@@ -28,6 +28,8 @@ struct SelState {
   unsigned long long prefix;  // digits of T64 fixed so far
   unsigned long long himask;  // mask of those digits
   long long rank;             // rank (1-based from the top) still sought inside the prefix class
+  int top;                    // bits [0, top) of K64 are still undecided; 0 = T64 is complete
+  int pad0;
   // predicted bracket for the COMING step's fused pass: key >= hi_key is certainly selected,
   // lo_key <= key < hi_key is a candidate, key < lo_key is certainly not selected
   uint32_t lo_key, hi_key;
@@ -522,6 +524,8 @@ __device__ __forceinline__ void chunk_keys(const KeySrc& s, int64_t c, int lane,
   for (int q = 0; q < 4; ++q) { valid[q] = i0 + q < s.N; k64[q] = make_k64(x[q], i0 + q); }
 }
 
+constexpr int kListBlocks = 296;     // CTAs that work on the candidate list in the radix passes
+
 // Candidate list written by the fused pass: n_seg segments of seg_cap entries.
 struct CandList {
   const unsigned long long* cand;
@@ -558,7 +562,23 @@ __global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t
     a = 0; c = 0;
     for (int i = 0; i < 32; ++i) { a += s_above[i]; c += s_cand[i]; }
     const bool hit = !force_general && !s_over && (long long)a < k && (long long)(a + c) >= k;
-    st->prefix = 0; st->himask = 0;
+    // On the fast route every candidate key lies in [lo_key, hi_key): the bits those two bounds
+    // share are already known, so the radix passes start below them (fewer passes, and the first
+    // digit spreads the candidates over the whole histogram instead of two or three bins).
+    unsigned long long prefix0 = 0, himask0 = 0;
+    int top = 64;
+    if (hit) {
+      const uint32_t lo = st->lo_key, hi1 = st->hi_key - 1u;
+      const uint32_t diff = lo ^ hi1;
+      const int common = diff ? __clz(diff) : 32;             // leading key bits shared by all candidates
+      if (common > 0) {
+        const uint32_t km = common >= 32 ? 0xFFFFFFFFu : ~(0xFFFFFFFFu >> common);
+        himask0 = (unsigned long long)km << 32;
+        prefix0 = (unsigned long long)(lo & km) << 32;
+      }
+      top = 64 - common;
+    }
+    st->prefix = prefix0; st->himask = himask0; st->top = top;
     st->rank = hit ? k - (long long)a : k;
     st->hit = hit ? 1 : 0;
     st->n_above = a; st->n_cand = c;
@@ -575,9 +595,17 @@ __global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t
 // Histogram of digit (K64 >> shift) & (2^bits - 1) over the keys whose higher digits equal prefix.
 // Source: the candidate list when the bracket held (st->hit), else every key of the partition.
 __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ KeySrc s, const __grid_constant__ CandList cl,
-                                                      const SelState* __restrict__ st, uint32_t* __restrict__ ghist,
-                                                      int shift, int bits) {
+                                                      const SelState* __restrict__ st, uint32_t* __restrict__ ghist) {
   __shared__ uint32_t h[kBins];
+  const int hit = st->hit;
+  const int top = st->top;
+  if (top <= 0) return;                                   // every digit is fixed already
+  const int bits = top < kDigitBits ? top : kDigitBits;
+  const int shift = top - bits;
+  // the candidate list is small: a fraction of the grid is enough, and every extra CTA would
+  // only zero and flush an empty histogram
+  const int list_blocks = min((int)gridDim.x, kListBlocks);
+  if (hit && (int)blockIdx.x >= list_blocks) return;
   for (int b = threadIdx.x; b < kBins; b += blockDim.x) h[b] = 0;
   __syncthreads();
   const unsigned long long prefix = st->prefix, himask = st->himask;
@@ -585,8 +613,8 @@ __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ K
   const int lane = threadIdx.x & 31;
   const int64_t wpb = blockDim.x >> 5;
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
-  const int64_t nwarps = (int64_t)gridDim.x * wpb;
-  if (st->hit) {
+  const int64_t nwarps = (int64_t)(hit ? list_blocks : (int)gridDim.x) * wpb;
+  if (hit) {
     for (int64_t sg = warp; sg < cl.n_seg; sg += nwarps) {
       const uint32_t cnt = cl.seg_count[sg];
       const unsigned long long* seg = cl.cand + (size_t)sg * cl.seg_cap;
@@ -609,8 +637,13 @@ __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ K
 }
 
 // One block: find the digit d whose class holds the sought rank; fix it; clear the histogram.
-__global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* ghist, int shift, int bits, int last) {
+__global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* ghist) {
   constexpr int PER = kBins / 1024;                 // bins per thread
+  const int top_in = st->top;
+  if (top_in <= 0) return;
+  const int bits = top_in < kDigitBits ? top_in : kDigitBits;
+  const int shift = top_in - bits;
+  const int last = shift == 0;
   __shared__ long long warp_tot[32];
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
   // thread t owns bins [kBins - PER*(t+1), kBins - PER*t): thread 0 owns the TOP bins
@@ -645,6 +678,7 @@ __global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* 
         st->prefix = T64;
         st->himask |= ((1ull << bits) - 1ull) << shift;
         st->rank = rank - cum;
+        st->top = shift;
         if (last) {
           // T64 is now exact.  Predict the next step's bracket around this threshold
           // (the top-k structure of the first moment is temporally stable).
@@ -662,12 +696,12 @@ __global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* 
               const float r = fminf(fmaxf(lnT - st->lnT_prev, -0.7f), 0.7f);
               pred = lnT + r;
               if (st->have_T == 1) dl = fmaxf(0.05f, 0.5f * fabsf(r));
-              else dl = fmaxf(3.0f * fabsf(lnT - st->ln_pred) + 0.02f, 0.6f * dl);
+              else dl = fmaxf(3.0f * fabsf(lnT - st->ln_pred) + 0.01f, 0.6f * dl);
             }
             // keep the expected candidate count under half the list's capacity
             if (st->hit && st->cand_cap_total > 0 && 2ull * st->n_cand > st->cand_cap_total)
               dl = fminf(dl, st->delta * (float)st->cand_cap_total / (2.0f * (float)st->n_cand));
-            dl = fminf(fmaxf(dl, 0.03f), 1.0f);
+            dl = fminf(fmaxf(dl, 0.02f), 1.0f);
             const float lo = __expf(pred - dl), hi = __expf(pred + dl);
             st->lo_key = __float_as_uint(lo) & 0x7FFFFFFFu;
             st->hi_key = (hi < 3.0e38f) ? (__float_as_uint(hi) & 0x7FFFFFFFu) : 0x7F800000u;
