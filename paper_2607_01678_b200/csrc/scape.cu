@@ -71,7 +71,8 @@ struct scape {
   float* pm[2] = {nullptr, nullptr};   // packed means b- [packed_stride], alternating
   int pm_last = 0;             // pm[pm_last] = b- of the last sparse step
   const char* last_kernel = "";   // name of the streaming kernel the last step launched
-  int fused_impl = 0;          // 0 auto (bulk-copy staged kernel in steady state), 1 = LDG kernel only
+  int fused_impl = 0;          // SCAPE_FUSED_IMPL (experiments): 0 auto, 1 "ldg" = register-staged kernel only,
+                               // 2 "directstore" = staged loads but direct global stores
   bool m_sparse = false;       // m_{t-1} lives in pm[pm_last] addressed through slot[last]; h->m is stale
   float* dense_pack = nullptr;    // optional [R][Npad]
   bool last_dense = false;
@@ -170,7 +171,8 @@ int launch_tma_t(scape* h, StepParams& p, cudaStream_t st) {
     if (const char* ev = getenv("SCAPE_TMA_BPS")) { int v = atoi(ev); if (v >= 1 && v <= 4) cfg_bps = v; }
     if (cfg_stages >= 2) {
       const size_t smem = kTmaBarrierBytes + (size_t)cfg_stages * TILE;
-      CU_TRY(cudaFuncSetAttribute(scape_fused_tma_kernel<G, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      CU_TRY(cudaFuncSetAttribute(scape_fused_tma_kernel<G, R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      CU_TRY(cudaFuncSetAttribute(scape_fused_tma_kernel<G, R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     }
   }
   if (cfg_stages < 0) return 1;   // does not fit: caller uses the LDG kernel
@@ -183,7 +185,9 @@ int launch_tma_t(scape* h, StepParams& p, cudaStream_t st) {
   h->seg_cap = (uint32_t)cap;
   p.seg_cap = h->seg_cap;
   const size_t smem = kTmaBarrierBytes + (size_t)cfg_stages * TILE;
-  scape_fused_tma_kernel<G, R><<<(int)grid, kTmaThreads, smem, st>>>(p, cfg_stages);
+  // results leave through the stage as whole-tile bulk stores (default) or as direct 128-bit stores
+  if (h->fused_impl == 2) scape_fused_tma_kernel<G, R, false><<<(int)grid, kTmaThreads, smem, st>>>(p, cfg_stages);
+  else scape_fused_tma_kernel<G, R, true><<<(int)grid, kTmaThreads, smem, st>>>(p, cfg_stages);
   h->last_kernel = "scape_fused_tma_kernel";
   h->launches++;
   CU_TRY(cudaGetLastError());
@@ -329,7 +333,7 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   scape* h = new (std::nothrow) scape();
   if (!h) { fail(SCAPE_ENOMEM, "host allocation failed"); return nullptr; }
   h->dev = dev;
-  if (const char* ev = getenv("SCAPE_FUSED_IMPL")) h->fused_impl = (strcmp(ev, "ldg") == 0) ? 1 : 0;
+  if (const char* ev = getenv("SCAPE_FUSED_IMPL")) h->fused_impl = (strcmp(ev, "ldg") == 0) ? 1 : (strcmp(ev, "directstore") == 0) ? 2 : 0;
   cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev);
   h->N = N; h->R = R;
   h->Npad = (N + kChunk - 1) / kChunk * kChunk;

@@ -154,7 +154,7 @@ struct StageA {                 // per-warp running state of the fused select (r
 // The arithmetic of one lane's 4 elements (Alg. 1 l.6-10, l.12-17 in the pinned order), the stores
 // of theta / m / e^r / b^r / b-, and the bracket classification of stage 2.  Shared by the two
 // load front-ends (register-staged LDG and shared-memory-staged bulk copies).
-template <int R, bool DENSE, bool GUARD>
+template <int R, bool DENSE, bool GUARD, bool STORE = true>
 __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, int lane, int64_t i0,
                                               uint32_t mybits, uint32_t jbase, float (&th)[4], const float (&mo)[4],
                                               float (&gg)[R][4], float (&ee)[R][4], StageA& sa) {
@@ -203,10 +203,12 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
     th[q] = __fmaf_rn(p.neg_lr, w, th[q]);
   }
 
-  store4_f32<GUARD>(p.theta, i0, p.N, th);
-  if (DENSE) store4_f32<false>(p.m, i0, p.N, mn);           // sparse steps keep m_t as b- only
+  if (STORE) {                                              // else the caller stores th / ee (staged bulk stores)
+    store4_f32<GUARD>(p.theta, i0, p.N, th);
 #pragma unroll
-  for (int r = 0; r < R; ++r) store4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
+    for (int r = 0; r < R; ++r) store4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
+  }
+  if (DENSE) store4_f32<false>(p.m, i0, p.N, mn);           // sparse steps keep m_t as b- only
 
   if (!DENSE) {
     // Stage 2 (l.11) fused: classify |m~^0| against the predicted bracket.  Exactness does not
@@ -361,7 +363,12 @@ __device__ __forceinline__ void tma_decode_gather(const StepParams& p, const Tma
 
 // One tile of one consumer warp: start the next tile's gather, wait for this tile's bytes, pull
 // them out of shared memory, release the stage, compute and store.
-template <typename G, int R>
+__device__ __forceinline__ void bulk_s2g(void* dst, const void* src_smem, uint32_t bytes, uint64_t policy) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+               ::"l"(dst), "r"(smem_u32(src_smem)), "r"(bytes), "l"(policy) : "memory");
+}
+
+template <typename G, int R, bool TSTORE>
 __device__ __forceinline__ void tma_consume_tile(const StepParams& p, int64_t tile, int64_t n_tiles, int64_t tstride,
                                                  int warp, int lane, unsigned char* stage0, uint64_t* full, uint64_t* empty,
                                                  int& s, uint32_t& ph, int n_stages, TmaMaskWords& nw,
@@ -395,13 +402,39 @@ __device__ __forceinline__ void tma_consume_tile(const StepParams& p, int64_t ti
       gg[r][2] = __uint_as_float(g.y << 16); gg[r][3] = __uint_as_float(g.y & 0xFFFF0000u);
     }
   }
-  __syncwarp();
-  if (lane == 0) mbar_arrive(&empty[s]);                        // this warp is done with the stage
-  if (++s == n_stages) { s = 0; ph ^= 1u; }
-  fused_compute<R, false, false>(p, c, lane, i0, cur.mybits, cur.jbase, th, cur.mo, gg, ee, sa);
+  if (!TSTORE) {
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[s]);                      // this warp is done with the stage
+    if (++s == n_stages) { s = 0; ph ^= 1u; }
+    fused_compute<R, false, false, true>(p, c, lane, i0, cur.mybits, cur.jbase, th, cur.mo, gg, ee, sa);
+  } else {
+    // Results go back into the stage (in place) and leave as whole-tile bulk stores: 4 KB bursts
+    // per stream instead of 512-byte warp stores.
+    fused_compute<R, false, false, false>(p, c, lane, i0, cur.mybits, cur.jbase, th, cur.mo, gg, ee, sa);
+    unsigned char* wbase = stage0 + (size_t)s * TILE;
+    *reinterpret_cast<float4*>(wbase + off * 4u) = make_float4(th[0], th[1], th[2], th[3]);
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+      *reinterpret_cast<float4*>(wbase + OFF_E + r * (kTmaTile * 4u) + off * 4u) = make_float4(ee[r][0], ee[r][1], ee[r][2], ee[r][3]);
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumerWarps * 32) : "memory");
+    if (threadIdx.x == 0) {
+      uint64_t pol;
+      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+      const int64_t e0 = tile * kTmaTile;
+      bulk_s2g(p.theta + e0, wbase, kTmaTile * 4u, pol);
+#pragma unroll
+      for (int r = 0; r < R; ++r) bulk_s2g(p.e + r * p.e_stride + e0, wbase + OFF_E + r * (kTmaTile * 4u), kTmaTile * 4u, pol);
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+      // the stores of the PREVIOUS tile have finished reading their stage: hand it back
+      asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+      if (tile != (int64_t)blockIdx.x) mbar_arrive(&empty[s == 0 ? n_stages - 1 : s - 1]);
+    }
+    if (++s == n_stages) { s = 0; ph ^= 1u; }
+  }
 }
 
-template <typename G, int R>
+template <typename G, int R, bool TSTORE>
 __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const __grid_constant__ StepParams p, int n_stages) {
   extern __shared__ __align__(128) unsigned char smem[];
   constexpr uint32_t TILE = tma_tile_bytes<G, R>();
@@ -413,7 +446,7 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
   const int64_t n_tiles = p.N / kTmaTile;                     // full tiles; the rest goes through the LDG path
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < n_stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], kTmaConsumerWarps); }
+    for (int s = 0; s < n_stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], TSTORE ? 1 : kTmaConsumerWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -466,12 +499,13 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
   }
   int s = 0; uint32_t ph = 0;
   while (tile < n_tiles) {
-    tma_consume_tile<G, R>(p, tile, n_tiles, tstride, warp, lane, stage0, full, empty, s, ph, n_stages, nw, stA, stB, sa);
+    tma_consume_tile<G, R, TSTORE>(p, tile, n_tiles, tstride, warp, lane, stage0, full, empty, s, ph, n_stages, nw, stA, stB, sa);
     tile += tstride;
     if (tile >= n_tiles) break;
-    tma_consume_tile<G, R>(p, tile, n_tiles, tstride, warp, lane, stage0, full, empty, s, ph, n_stages, nw, stB, stA, sa);
+    tma_consume_tile<G, R, TSTORE>(p, tile, n_tiles, tstride, warp, lane, stage0, full, empty, s, ph, n_stages, nw, stB, stA, sa);
     tile += tstride;
   }
+  if (TSTORE && threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // stores have landed
 
   // chunks past the last full tile (fewer than 8, the last one possibly ragged): LDG path
   {
