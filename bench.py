@@ -47,6 +47,11 @@ def parse():
     ap.add_argument("--cpu-div", type=int, default=64, help="oracle sample: every tensor this many times smaller")
     ap.add_argument("--cpu-steps", type=int, default=3)
     ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--sweep", default=None, metavar="CSV",
+                    help="run BASELINE.json config 5 (sizes 2^20..2^30 x sparsity x R, Gaussian grads) and write one CSV row per point")
+    ap.add_argument("--sweep-log2n", default="20,21,22,23,24,25,26,27,28,29,30")
+    ap.add_argument("--sweep-sparsity", default="0,0.9,0.99,0.999")
+    ap.add_argument("--sweep-R", default="1,2,4,8")
     return ap.parse_args()
 
 
@@ -209,6 +214,53 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def run_sweep(args):
+    """BASELINE.json config 5: 3 warm-up + 10 timed steps per point (after the dense first step),
+    i.i.d. Gaussian gradients std 1e-3, fixed seed.  Points whose footprint fits the 126 MB L2 run
+    above the DRAM roofline and are labelled l2_resident."""
+    import torch
+    from paper_2607_01678_b200 import binding, synth
+    torch.cuda.set_device(0)
+    peak, _ = measured_peak()
+    rows = ["log2n,N,sparsity,R,k,ms_per_step,params_per_s,step_gbs_alg,frac_of_measured_peak,footprint_mib,l2_resident,kernel,select_fast,select_general"]
+    for l2 in [int(x) for x in args.sweep_log2n.split(",")]:
+        for sp in [float(x) for x in args.sweep_sparsity.split(",")]:
+            for R in [int(x) for x in args.sweep_R.split(",")]:
+                w = synth.sweep_point(l2, sp, R)
+                N = w.numel
+                gs = synth.GradStream(w, device="cuda", seed=args.seed)
+                theta = gs.theta0()
+                # as many distinct gradient sets as fit comfortably (each is 4 R N bytes)
+                n_sets = max(1, min(4, int((120e9 - (8 + 4 * R) * N) // (4 * R * N))))
+                ring = [gs.next() for _ in range(n_sets)]
+                del gs
+                sc = binding.Scape(N, R, sp, **w.hyper)
+                k = sc.k
+                sc.step(theta, ring[0])
+                for i in range(3):
+                    sc.step(theta, ring[(1 + i) % n_sets])
+                torch.cuda.synchronize()
+                f0, g0 = sc.select_stats() if k < N else (0, 0)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                for i in range(10):
+                    sc.step(theta, ring[i % n_sets])
+                b.record()
+                torch.cuda.synchronize()
+                ms = a.elapsed_time(b) / 10
+                f1, g1 = sc.select_stats() if k < N else (0, 0)
+                gbs = bytes_per_param_step(w, k, N) * N / (ms * 1e-3) / 1e9
+                foot = (8 + 8 * R) * N / 2**20
+                rows.append(f"{l2},{N},{sp},{R},{k},{ms:.5f},{N / (ms * 1e-3):.4e},{gbs:.1f},{gbs / peak:.4f},{foot:.1f},"
+                            f"{int(foot < 126)},{sc.last_kernel},{f1 - f0},{g1 - g0}")
+                print(rows[-1], flush=True)
+                sc.close()
+                del sc, ring, theta
+                torch.cuda.empty_cache()
+    with open(args.sweep, "w") as f:
+        f.write("\n".join(rows) + "\n")
+
+
 def max_over_ranks_ms(ms, world, device):
     """Device time of the slowest rank (every multi-GPU number is the max over ranks)."""
     if world <= 1:
@@ -230,6 +282,8 @@ def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
 
     import torch
     import torch.distributed as dist

@@ -212,7 +212,11 @@ int launch_tma_r(scape* h, StepParams& p, cudaStream_t st) {
 // variants: all-ones mask (dense m in and out) | sparse mask, dense m in | sparse mask, sparse m in
 template <typename G>
 int launch_fused_g(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t st) {
-  if (!dense && msparse && h->fused_impl != 1 && p.N / kTmaTile >= (int64_t)h->n_sm) {
+  // The staged kernel wins when there are enough bytes per parameter to be HBM-bound (R >= 3);
+  // with one or two replicas the step is issue-bound and the register-staged kernel's higher
+  // occupancy (40 warps/SM vs 16 consumer warps) is worth more (measured at N = 2^28, 99 %:
+  // R = 1: 1.49 vs 2.02 ms, R = 2: 1.95 vs 2.08 ms, R = 4: 2.94 vs 2.72 ms).
+  if (!dense && msparse && h->fused_impl != 1 && h->R >= 3 && p.N / kTmaTile >= (int64_t)h->n_sm) {
     const int rc = launch_tma_r<G>(h, p, st);
     if (rc <= 0) return rc;      // 1 = tile does not fit in shared memory: fall through
   }
@@ -367,9 +371,10 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   }
   alloc((void**)&h->sel, sizeof(SelState), true);
   if (sparse) {
-    // candidates of the fused select: room for ~4k keys (bracket of +-25 % around the threshold
-    // holds ~1.5k for power-law tails), never more than N/2, never fewer than 64 Ki
+    // candidates of the fused select: room for 4k keys (a bracket of +-3 % around the threshold
+    // holds ~0.8k: error feedback piles residuals up just below it), at least N/8, at most N/2
     int64_t cc = 4 * h->k;
+    if (cc < N / 8) cc = N / 8;            // very sparse masks / transients: keep room per warp segment
     if (cc > N / 2) cc = N / 2;
     if (cc < 65536) cc = 65536;
     h->cand_cap = cc;

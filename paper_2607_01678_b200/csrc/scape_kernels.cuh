@@ -36,6 +36,7 @@ struct SelState {
   float delta;                // half-width of the bracket in ln(threshold)
   float lnT_prev;             // ln of the last exact threshold |m~| value
   float ln_pred;              // ln of the threshold that was predicted for the current step
+  float r_prev;               // previous step-to-step change of ln(threshold)
   int have_T;                 // number of exact thresholds seen (saturates at 2)
   unsigned long long cand_cap_total;   // n_seg * seg_cap of the last fused pass
   int hit;                    // this step: 1 = the bracket held (candidate list), 0 = general path
@@ -727,10 +728,20 @@ __global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* 
             const float lnT = __logf(T);
             if (st->have_T == 0) { pred = lnT; dl = 0.6f; }
             else {
+              // Step-to-step change r of ln T.  In the transient of the EMA r decays geometrically,
+              // so the next change is predicted as r * (r / r_prev) (ratio clamped to [0, 1]; no
+              // extrapolation at all when the sign flips, e.g. for alternating inputs).
               const float r = fminf(fmaxf(lnT - st->lnT_prev, -0.7f), 0.7f);
-              pred = lnT + r;
+              float rn = r;
+              if (st->have_T >= 2) {
+                const float rp = st->r_prev;
+                const float ratio = (rp != 0.0f && (r > 0.0f) == (rp > 0.0f)) ? fminf(fmaxf(r / rp, 0.0f), 1.0f) : 0.0f;
+                rn = r * ratio;
+              }
+              pred = lnT + rn;
+              st->r_prev = r;
               if (st->have_T == 1) dl = fmaxf(0.05f, 0.5f * fabsf(r));
-              else dl = fmaxf(3.0f * fabsf(lnT - st->ln_pred) + 0.01f, 0.6f * dl);
+              else dl = fmaxf(3.0f * fabsf(lnT - st->ln_pred) + 0.01f, 0.85f * dl);   // widen at once, narrow slowly
             }
             // keep the expected candidate count under half the list's capacity
             if (st->hit && st->cand_cap_total > 0 && 2ull * st->n_cand > st->cand_cap_total)
