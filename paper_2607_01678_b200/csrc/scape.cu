@@ -78,6 +78,7 @@ struct scape {
   bool last_dense = false;
 
   SelState* sel = nullptr;
+  unsigned long long* cls = nullptr;    // [kClsCap] small list of the radix select
   unsigned long long* cand = nullptr;   // [cand_cap] candidate composite keys of the fused select
   int64_t cand_cap = 0;
   uint32_t* seg_count = nullptr;  // [max_seg]
@@ -266,7 +267,7 @@ int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general,
   src.N = h->N;
   src.n_chunks = h->n_chunks;
   CandList cl;
-  cl.cand = h->cand; cl.seg_count = h->seg_count; cl.seg_above = h->seg_above;
+  cl.cls = h->cls; cl.cand = h->cand; cl.seg_count = h->seg_count; cl.seg_above = h->seg_above;
   cl.seg_cap = h->seg_cap; cl.n_seg = force_general ? 0 : h->n_seg;
   const int grid = grid_for(h, h->n_chunks, 8, 6);
   sel_decide_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist, cl, (long long)h->k, force_general ? 1 : 0);
@@ -311,7 +312,7 @@ void free_all(scape* h) {
   cudaFree(h->m); cudaFree(h->e);
   for (auto& s : h->slot) { cudaFree(s.bits); cudaFree(s.rank); cudaFree(s.idx); }
   cudaFree(h->packed); cudaFree(h->pm[0]); cudaFree(h->pm[1]); cudaFree(h->dense_pack);
-  cudaFree(h->sel); cudaFree(h->cand); cudaFree(h->seg_count); cudaFree(h->seg_above); cudaFree(h->ghist); cudaFree(h->block_sum); cudaFree(h->total);
+  cudaFree(h->sel); cudaFree(h->cand); cudaFree(h->cls); cudaFree(h->seg_count); cudaFree(h->seg_above); cudaFree(h->ghist); cudaFree(h->block_sum); cudaFree(h->total);
   cudaFree(h->st_param);
   for (auto& g : h->st_grad) cudaFree(g);
   if (h->prof_have_events)
@@ -380,6 +381,7 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
     h->cand_cap = cc;
     h->max_seg = h->n_sm * 8 * 8;
     alloc((void**)&h->cand, sizeof(unsigned long long) * (size_t)cc, false);
+    alloc((void**)&h->cls, sizeof(unsigned long long) * (size_t)kClsCap, false);
     alloc((void**)&h->seg_count, sizeof(uint32_t) * h->max_seg, true);
     alloc((void**)&h->seg_above, sizeof(uint32_t) * h->max_seg, true);
   }

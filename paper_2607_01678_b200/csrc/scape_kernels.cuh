@@ -29,7 +29,10 @@ struct SelState {
   unsigned long long himask;  // mask of those digits
   long long rank;             // rank (1-based from the top) still sought inside the prefix class
   int top;                    // bits [0, top) of K64 are still undecided; 0 = T64 is complete
-  int pad0;
+  int use_cls;                // the surviving class has been collected into the small list
+  unsigned long long class_count;   // keys in the class chosen by the last pick
+  unsigned int cls_n;         // entries in the small list
+  unsigned int pad1;
   // predicted bracket for the COMING step's fused pass: key >= hi_key is certainly selected,
   // lo_key <= key < hi_key is a candidate, key < lo_key is certainly not selected
   uint32_t lo_key, hi_key;
@@ -559,10 +562,28 @@ __device__ __forceinline__ void chunk_keys(const KeySrc& s, int64_t c, int lane,
   for (int q = 0; q < 4; ++q) { valid[q] = i0 + q < s.N; k64[q] = make_k64(x[q], i0 + q); }
 }
 
-constexpr int kListBlocks = 296;     // CTAs that work on the candidate list in the radix passes
-
 // Candidate list written by the fused pass: n_seg segments of seg_cap entries.
+constexpr uint32_t kClsCap = 1u << 20;   // entries of the small list the surviving class is collected into
+
+// strided, 4-deep unrolled scan of the candidate segments (4 independent 8-byte loads per lane)
+template <typename F>
+__device__ __forceinline__ void scan_segments(const unsigned long long* cand, const uint32_t* seg_count, uint32_t seg_cap,
+                                              int n_seg, int64_t warp, int64_t nwarps, int lane, F f) {
+  for (int64_t sg = warp; sg < n_seg; sg += nwarps) {
+    const uint32_t cnt = min(seg_count[sg], seg_cap);
+    const unsigned long long* seg = cand + (size_t)sg * seg_cap;
+    for (uint32_t j0 = 0; j0 < cnt; j0 += 128) {
+      unsigned long long v[4]; bool ok[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { const uint32_t j = j0 + u * 32 + lane; ok[u] = j < cnt; v[u] = ok[u] ? __ldcs(seg + j) : 0ull; }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) if (ok[u]) f(v[u]);
+    }
+  }
+}
+
 struct CandList {
+  unsigned long long* cls;      // [kClsCap] small list (see sel_hist_kernel)
   const unsigned long long* cand;
   const uint32_t* seg_count;
   const uint32_t* seg_above;
@@ -614,6 +635,7 @@ __global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t
       top = 64 - common;
     }
     st->prefix = prefix0; st->himask = himask0; st->top = top;
+    st->use_cls = 0; st->cls_n = 0; st->class_count = ~0ull;
     st->rank = hit ? k - (long long)a : k;
     st->hit = hit ? 1 : 0;
     st->n_above = a; st->n_cand = c;
@@ -628,19 +650,22 @@ __global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t
 }
 
 // Histogram of digit (K64 >> shift) & (2^bits - 1) over the keys whose higher digits equal prefix.
-// Source: the candidate list when the bracket held (st->hit), else every key of the partition.
+// Source: the small list once the surviving class has been collected into it; else the candidate
+// list when the bracket held (st->hit); else every key of the partition.  The pass that first
+// sees a class of at most kClsCap keys also collects that class into the small list, so the
+// remaining passes touch a few thousand keys instead of re-reading everything.
 __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ KeySrc s, const __grid_constant__ CandList cl,
-                                                      const SelState* __restrict__ st, uint32_t* __restrict__ ghist) {
+                                                      SelState* __restrict__ st, uint32_t* __restrict__ ghist) {
   __shared__ uint32_t h[kBins];
   const int hit = st->hit;
   const int top = st->top;
   if (top <= 0) return;                                   // every digit is fixed already
   const int bits = top < kDigitBits ? top : kDigitBits;
   const int shift = top - bits;
-  // the candidate list is small: a fraction of the grid is enough, and every extra CTA would
-  // only zero and flush an empty histogram
-  const int list_blocks = min((int)gridDim.x, kListBlocks);
-  if (hit && (int)blockIdx.x >= list_blocks) return;
+  const int use_cls = st->use_cls;
+  const bool collect = !use_cls && st->class_count <= (unsigned long long)kClsCap;
+  const uint32_t cls_blocks = min(8u, gridDim.x);         // a handful of CTAs is plenty for the small list
+  if (use_cls && blockIdx.x >= cls_blocks) return;
   for (int b = threadIdx.x; b < kBins; b += blockDim.x) h[b] = 0;
   __syncthreads();
   const unsigned long long prefix = st->prefix, himask = st->himask;
@@ -648,23 +673,24 @@ __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ K
   const int lane = threadIdx.x & 31;
   const int64_t wpb = blockDim.x >> 5;
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
-  const int64_t nwarps = (int64_t)(hit ? list_blocks : (int)gridDim.x) * wpb;
-  if (hit) {
-    for (int64_t sg = warp; sg < cl.n_seg; sg += nwarps) {
-      const uint32_t cnt = cl.seg_count[sg];
-      const unsigned long long* seg = cl.cand + (size_t)sg * cl.seg_cap;
-      for (uint32_t j = lane; j < cnt; j += 32) {
-        const unsigned long long k64 = seg[j];
-        if ((k64 & himask) == prefix) atomicAdd(&h[(uint32_t)(k64 >> shift) & dmask], 1u);
-      }
+  const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  auto visit = [&](unsigned long long k64) {
+    if ((k64 & himask) == prefix) {
+      atomicAdd(&h[(uint32_t)(k64 >> shift) & dmask], 1u);
+      if (collect) { const uint32_t pos = atomicAdd(&st->cls_n, 1u); if (pos < kClsCap) cl.cls[pos] = k64; }
     }
+  };
+  if (use_cls) {
+    const uint32_t n = min(st->cls_n, kClsCap);
+    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += cls_blocks * blockDim.x) visit(cl.cls[j]);
+  } else if (hit) {
+    scan_segments(cl.cand, cl.seg_count, cl.seg_cap, cl.n_seg, warp, nwarps, lane, visit);
   } else {
     for (int64_t c = warp; c < s.n_chunks; c += nwarps) {
       unsigned long long k64[4]; bool valid[4];
       chunk_keys(s, c, lane, k64, valid);
 #pragma unroll
-      for (int q = 0; q < 4; ++q)
-        if (valid[q] && (k64[q] & himask) == prefix) atomicAdd(&h[(uint32_t)(k64[q] >> shift) & dmask], 1u);
+      for (int q = 0; q < 4; ++q) if (valid[q]) visit(k64[q]);
     }
   }
   __syncthreads();
@@ -714,6 +740,9 @@ __global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* 
         st->himask |= ((1ull << bits) - 1ull) << shift;
         st->rank = rank - cum;
         st->top = shift;
+        // the pass that just ran collected its class iff that class was known to be small enough
+        if (!st->use_cls && st->class_count <= (unsigned long long)kClsCap) st->use_cls = 1;
+        st->class_count = hv[q];
         if (last) {
           // T64 is now exact.  Predict the next step's bracket around this threshold
           // (the top-k structure of the first moment is temporally stable).
@@ -774,17 +803,12 @@ __global__ void __launch_bounds__(256) sel_finish_kernel(const __grid_constant__
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
   const int64_t nwarps = (int64_t)gridDim.x * wpb;
   if (st->hit) {
-    for (int64_t sg = warp; sg < cl.n_seg; sg += nwarps) {
-      const uint32_t cnt = cl.seg_count[sg];
-      const unsigned long long* seg = cl.cand + (size_t)sg * cl.seg_cap;
-      for (uint32_t j = lane; j < cnt; j += 32) {
-        const unsigned long long k64 = seg[j];
-        if (k64 >= T64) {
-          const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64;
-          atomicOr(&next_bits[i >> 5], 1u << (i & 31));
-        }
+    scan_segments(cl.cand, cl.seg_count, cl.seg_cap, cl.n_seg, warp, nwarps, lane, [&](unsigned long long k64) {
+      if (k64 >= T64) {
+        const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64;
+        atomicOr(&next_bits[i >> 5], 1u << (i & 31));
       }
-    }
+    });
     return;
   }
   for (int64_t c = warp; c < s.n_chunks; c += nwarps) {
