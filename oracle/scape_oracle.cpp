@@ -14,8 +14,11 @@
 //   P5 Eq. 4-6 off-mask behaviour           P6 telescoped error feedback (nothing lost)
 //   P7 one-step mask delay                  P8 R = 1
 //   P9 worked example tests/golden/p9_worked_example.json
-// Unpinned by the paper (decisions): S3 clip_grad omitted,
-// S4 no bias correction, S8 replica 0 owns the statistic, S9 flat (not per-layer) top-k.
+//   P10 bias correction / learning-rate schedule == independent numpy Eq. 2 + PAPER.md:77 (dense)
+//   P11 clip_grad: norm and factor vs numpy; no-op below the threshold; theta vs numpy (dense)
+// Unpinned by the paper (decisions): S3 clip_grad off by default and,
+// when switched on, the torch/Megatron rule; S4 bias correction off by default; S8 replica 0 owns
+// the statistic; S9 flat (not per-layer) top-k.
 //
 // The algorithm is instantiated twice from the same template: T = float is the graded
 // arithmetic (operation order pinned below);
@@ -58,6 +61,12 @@ struct Oracle {
   int64_t t = 0;      // steps taken
   T beta1, beta2, eps, lr, wd;
   T c1, c2;           // 1 - beta1, 1 - beta2, evaluated in T
+  double beta1_d, beta2_d;   // as given, for the bias-correction powers
+  // Optional parts of Alg. 1 / Eq. 2 that the default configuration leaves out (readings S3, S4):
+  bool bias_correction = false;   // m_t/(1-beta1^t), v_t/(1-beta2^t)
+  double clip_max_norm = 0.0;     // l.14 clip_grad, 0 = off (PAPER.md:165; "gradient clip of 1", :279)
+  double last_norm = 0.0;         // ||g^||_2 of the last step and the factor applied
+  T last_coef = (T)1;
 
   std::vector<T> m;                 // m_{t-1}, zero off the previous mask (Eq. 4)
   std::vector<std::vector<T>> e;    // e^r_{t-1}, one residual per replica (Alg. 1 l.2, :141)
@@ -74,6 +83,7 @@ struct Oracle {
       : N(N_), R(R_) {
     // Hyper-parameters are cast to T once; 1 - beta is evaluated in T.
     beta1 = (T)b1; beta2 = (T)b2; eps = (T)eps_; lr = (T)lr_; wd = (T)wd_;
+    beta1_d = b1; beta2_d = b2;
     c1 = (T)1 - beta1;
     c2 = (T)1 - beta2;
     // Reading S6: k = N - floor(s*N) in IEEE double.
@@ -133,13 +143,42 @@ struct Oracle {
       for (int r = 1; r < R; ++r) s = s + b[r][j];
       T bb = s / (T)R;
       T p = beta1 * m[i];
-      T gh = (bb - p) / c1;                              // l.13 (Eq. 3, :188)
+      bbar[j] = bb;
+      ghat[j] = (bb - p) / c1;                           // l.13 (Eq. 3, :188)
+    }
+    // l.14 clip_grad(b-bar): global-norm clip of the reconstructed gradient over the mask.
+    // The paper does not define it; this is the usual rule (torch / Megatron clip_grad_norm):
+    // coef = max_norm / (||g^||_2 + 1e-6), applied only when coef < 1.  The norm is accumulated in
+    // double, in index order.
+    T coef = (T)1;
+    {
+      double ss = 0.0;
+      for (int64_t j = 0; j < K; ++j) ss += (double)ghat[j] * (double)ghat[j];
+      last_norm = std::sqrt(ss);
+      if (clip_max_norm > 0.0) {
+        const double cc = clip_max_norm / (last_norm + 1e-6);
+        if (cc < 1.0) coef = (T)cc;
+      }
+      last_coef = coef;
+    }
+    // Bias correction, off by default (reading S4): factors 1/(1-beta^t) evaluated in
+    // double from the step number, cast to T once.
+    T bc1 = (T)1, bc2 = (T)1;
+    if (bias_correction) {
+      bc1 = (T)(1.0 / (1.0 - std::pow(beta1_d, (double)t)));
+      bc2 = (T)(1.0 / (1.0 - std::pow(beta2_d, (double)t)));
+    }
+    for (int64_t j = 0; j < K; ++j) {
+      const int64_t i = idx[j];
+      const T bb = bbar[j];
+      T gh = ghat[j];
+      if (clip_max_norm > 0.0) gh = gh * coef;           // l.14
       T vv = std::fma(c2, gh * gh, beta2 * (m[i] * m[i]));   // l.15
-      T uu = bb / (std::sqrt(vv) + eps);                 // l.16 with m_t = bbar (l.12)
+      T uu = (bb * bc1) / (std::sqrt(vv * bc2) + eps);   // l.16 with m_t = bbar (l.12)
       T w = std::fma(wd, theta[i], uu);                  // l.17
       theta[i] = std::fma(-lr, w, theta[i]);
       m_new[i] = bb;                                     // l.12
-      bbar[j] = bb; ghat[j] = gh; v[j] = vv; u[j] = uu;
+      ghat[j] = gh; v[j] = vv; u[j] = uu;
     }
     // Off the mask: u = 0 (Eq. 5, :202), so l.17 is pure weight decay (Eq. 6, :207-211).
     for (int64_t i = 0; i < N; ++i) {
@@ -188,6 +227,11 @@ template <class T> void copy_out(const std::vector<T>& v, T* dst) {
     auto* o = (Oracle<T>*)h; std::memcpy(o->cur.data(), src, o->N);                                 \
   }                                                                                                 \
   extern "C" void oracle_set_t_##SUF(void* h, int64_t t) { ((Oracle<T>*)h)->t = t; }                \
+  extern "C" void oracle_set_lr_##SUF(void* h, double lr) { ((Oracle<T>*)h)->lr = (T)lr; }         \
+  extern "C" void oracle_set_bias_correction_##SUF(void* h, int on) { ((Oracle<T>*)h)->bias_correction = on != 0; } \
+  extern "C" void oracle_set_clip_grad_##SUF(void* h, double c) { ((Oracle<T>*)h)->clip_max_norm = c; } \
+  extern "C" double oracle_last_norm_##SUF(void* h) { return ((Oracle<T>*)h)->last_norm; }          \
+  extern "C" double oracle_last_coef_##SUF(void* h) { return (double)((Oracle<T>*)h)->last_coef; }                \
   extern "C" void oracle_get_idx_##SUF(void* h, int32_t* dst) { copy_out(((Oracle<T>*)h)->idx, dst); } \
   extern "C" void oracle_get_mt_##SUF(void* h, int r, T* dst) { copy_out(((Oracle<T>*)h)->mt[r], dst); } \
   extern "C" void oracle_get_b_##SUF(void* h, int r, T* dst) { copy_out(((Oracle<T>*)h)->b[r], dst); } \

@@ -68,6 +68,31 @@ class ScapeOracle:
         fn.argtypes = [ctypes.c_void_p, ctypes.c_int64]
         fn(self.h, int(t))
 
+    def set_lr(self, lr):
+        fn = self._f("set_lr")
+        fn.argtypes = [ctypes.c_void_p, ctypes.c_double]
+        fn(self.h, float(lr))
+
+    def set_bias_correction(self, on):
+        fn = self._f("set_bias_correction")
+        fn.argtypes = [ctypes.c_void_p, ctypes.c_int]
+        fn(self.h, int(on))
+
+    def set_clip_grad(self, max_norm):
+        fn = self._f("set_clip_grad")
+        fn.argtypes = [ctypes.c_void_p, ctypes.c_double]
+        fn(self.h, float(max_norm))
+
+    def last_norm(self):
+        fn = self._f("last_norm")
+        fn.restype, fn.argtypes = ctypes.c_double, [ctypes.c_void_p]
+        return fn(self.h)
+
+    def last_coef(self):
+        fn = self._f("last_coef")
+        fn.restype, fn.argtypes = ctypes.c_double, [ctypes.c_void_p]
+        return fn(self.h)
+
     # ---- the step ------------------------------------------------------------------
     def step(self, theta, grads):
         """theta: contiguous array [N] of self.dtype, updated in place. grads: R arrays [N]."""

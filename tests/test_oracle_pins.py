@@ -338,3 +338,85 @@ def test_f32_and_f64_instantiations_track_each_other():
         o32.step(th32, g)
         o64.step(th64, [x.astype(np.float64) for x in g])
     np.testing.assert_allclose(th32, th64, rtol=2e-4, atol=1e-7)
+
+
+# ------------------------------------------------------------------------------------ P10
+def dense_adams_full_f64(theta, m, gbar, t, beta1, beta2, eps, lr, wd, bias_correction, clip):
+    """Eq. 2 + bias correction + global-norm clip of the gradient (Alg. 1 l.14 at
+    density 1, where g-hat = g-bar), written independently of the oracle."""
+    g = gbar
+    norm = float(np.sqrt(np.sum(g * g)))
+    coef = 1.0
+    if clip > 0 and clip / (norm + 1e-6) < 1.0:
+        coef = clip / (norm + 1e-6)
+    g = g * coef if clip > 0 else g
+    m_new = beta1 * m + (1 - beta1) * gbar          # l.12: the first moment is NOT clipped (clip follows it)
+    v = beta2 * m * m + (1 - beta2) * g * g
+    if bias_correction:
+        mhat, vhat = m_new / (1 - beta1 ** t), v / (1 - beta2 ** t)
+    else:
+        mhat, vhat = m_new, v
+    return theta - lr * (mhat / (np.sqrt(vhat) + eps) + wd * theta), m_new, norm, coef
+
+
+@pytest.mark.parametrize("bc,clip", [(True, 0.0), (False, 0.05), (True, 0.05), (False, 1e9)])
+def test_p10_p11_bias_correction_clip_and_lr_schedule_dense_double(bc, clip):
+    rng = np.random.default_rng(13)
+    N, R, T = 2500, 3, 7
+    o = ScapeOracle(N, R, 0.0, dtype=np.float64, **HYP)
+    o.set_bias_correction(bc)
+    o.set_clip_grad(clip)
+    th = 0.02 * rng.standard_normal(N)
+    th_ref, m_ref = th.copy(), np.zeros(N)
+    clipped_once = False
+    for t, g in enumerate(make_grads(rng, N, R, T, dtype=np.float64), 1):
+        lr = HYP["lr"] * (0.5 + 0.1 * t)             # a schedule
+        o.set_lr(lr)
+        o.step(th, g)
+        gbar = sum(g) / R
+        hyp = dict(HYP, lr=lr)
+        th_ref, m_ref, norm, coef = dense_adams_full_f64(th_ref, m_ref, gbar, t, bias_correction=bc, clip=clip, **hyp)
+        np.testing.assert_allclose(o.last_norm(), norm, rtol=1e-9)       # g-hat = g-bar up to the l.13 round trip
+        np.testing.assert_allclose(o.last_coef(), coef, rtol=1e-9)
+        clipped_once |= coef < 1.0
+        np.testing.assert_allclose(o.m(), m_ref, rtol=1e-12, atol=1e-300)
+        np.testing.assert_allclose(th, th_ref, rtol=1e-9, atol=1e-300)
+    assert clipped_once == (0 < clip < 1)             # the 0.05 threshold does bite, 1e9 never does
+
+
+def test_p11_clip_below_threshold_is_bitwise_noop_fp32():
+    rng = np.random.default_rng(14)
+    N, R = 3000, 2
+    a, b = ScapeOracle(N, R, 0.9, **HYP), ScapeOracle(N, R, 0.9, **HYP)
+    b.set_clip_grad(1e6)
+    tha = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    thb = tha.copy()
+    for g in make_grads(rng, N, R, 4):
+        a.step(tha, g)
+        b.step(thb, g)
+        assert b.last_coef() == 1.0
+        assert np.array_equal(tha.view(np.uint32), thb.view(np.uint32))
+        np.testing.assert_allclose(b.last_norm(), np.sqrt(np.sum(b.ghat().astype(np.float64) ** 2)), rtol=1e-12)
+
+
+def test_p11_clip_scales_only_the_second_moment_input_sparse():
+    """On a sparse step: m_t = b-bar is unchanged by the clip (l.12 precedes l.14); g-hat is scaled by
+    coef = c / (||g-hat|| + 1e-6); off-mask parameters are untouched by it."""
+    rng = np.random.default_rng(15)
+    N, R = 3000, 2
+    a, b = ScapeOracle(N, R, 0.9, **HYP), ScapeOracle(N, R, 0.9, **HYP)
+    b.set_clip_grad(1e-3)
+    tha = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    thb = tha.copy()
+    gs = make_grads(rng, N, R, 3)
+    for g in gs[:2]:
+        a.step(tha, g)
+        b.set_clip_grad(0.0); b.step(thb, g); b.set_clip_grad(1e-3)      # identical history
+    a.step(tha, gs[2]); b.step(thb, gs[2])
+    assert b.last_coef() < 1.0
+    np.testing.assert_array_equal(a.m(), b.m())
+    np.testing.assert_allclose(b.ghat(), a.ghat() * np.float32(b.last_coef()), rtol=2e-7)
+    np.testing.assert_allclose(b.last_coef(), 1e-3 / (a.last_norm() + 1e-6), rtol=1e-6)
+    off = np.ones(N, bool); off[a.idx()] = False
+    np.testing.assert_array_equal(tha[off], thb[off])
+    assert not np.array_equal(tha[~off], thb[~off])
