@@ -108,6 +108,25 @@ int64_t scape_count(const scape_t* h, int which);
  * bf16 is widened exactly to fp32 in registers).                                               */
 int scape_set_grad_dtype(scape_t* h, int dtype);
 
+/* Optional parts of Algorithm 1 / Eq. 2 that the default configuration leaves out (DESIGN.md
+ * readings S3, S4); each takes effect from the next scape_step.
+ *   scape_set_lr              learning rate eta for the following steps (schedules).
+ *   scape_set_bias_correction m_t/(1-beta1^t), v_t/(1-beta2^t) in l.16; t = number of
+ *                             the step being taken (scape_step_count + 1).
+ *   scape_set_clip_grad       l.14 clip_grad(b-bar) (PAPER.md:165; "gradient clip of 1", :279): the
+ *                             reconstructed gradient g^ of the selected entries is multiplied by
+ *                             max_norm / (||g^||_2 + 1e-6) when that is < 1 (the torch / Megatron
+ *                             rule; the paper does not define it).  0 switches it off.  Allocates
+ *                             2 N floats on first use.  With clipping on, theta of the selected
+ *                             entries is updated by a second small kernel after the norm is known;
+ *                             the norm is summed in double in a fixed order, so results are
+ *                             reproducible run to run and agree with the oracle to ~1 ulp.
+ *   scape_last_grad_norm      ||g^||_2 and the factor applied by the last step (synchronises).   */
+int scape_set_lr(scape_t* h, double lr);
+int scape_set_bias_correction(scape_t* h, int on);
+int scape_set_clip_grad(scape_t* h, double max_norm);
+int scape_last_grad_norm(scape_t* h, double* norm, double* coef, void* cuda_stream);
+
 /* Option: also materialise b^r on steps whose mask is all ones (step 1, or sparsity 0), where
  * the packed buffer would be R*N floats.  Off by default: on such steps SCAPE_PACKED is then
  * unavailable (SCAPE_EINVAL) and SCAPE_PACKED_MEAN equals SCAPE_MOMENT.  Allocates R*N floats

@@ -33,6 +33,10 @@ SYMBOLS = {
     "scape_count": (_I64, [_VP, _I]),
     "scape_set_grad_dtype": (_I, [_VP, _I]),
     "scape_set_keep_dense_pack": (_I, [_VP, _I]),
+    "scape_set_lr": (_I, [_VP, _D]),
+    "scape_set_bias_correction": (_I, [_VP, _I]),
+    "scape_set_clip_grad": (_I, [_VP, _D]),
+    "scape_last_grad_norm": (_I, [_VP, _VP, _VP, _VP]),
     "scape_get": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
     "scape_set": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
     "scape_set_step_count": (_I, [_VP, _I64]),
@@ -125,6 +129,25 @@ def scape_set_grad_dtype(h, dtype):
 
 def scape_set_keep_dense_pack(h, on):
     _check(lib().scape_set_keep_dense_pack(h, int(on)), "scape_set_keep_dense_pack")
+
+
+def scape_set_lr(h, lr):
+    _check(lib().scape_set_lr(h, float(lr)), "scape_set_lr")
+
+
+def scape_set_bias_correction(h, on):
+    _check(lib().scape_set_bias_correction(h, int(on)), "scape_set_bias_correction")
+
+
+def scape_set_clip_grad(h, max_norm):
+    _check(lib().scape_set_clip_grad(h, float(max_norm)), "scape_set_clip_grad")
+
+
+def scape_last_grad_norm(h, stream=0):
+    """-> (||g^||_2, factor applied) of the last step"""
+    a, b = ctypes.c_double(), ctypes.c_double()
+    _check(lib().scape_last_grad_norm(h, ctypes.byref(a), ctypes.byref(b), stream), "scape_last_grad_norm")
+    return a.value, b.value
 
 
 def scape_set_step_count(h, t):
@@ -290,6 +313,18 @@ class Scape:
 
     def set_step_count(self, t):
         scape_set_step_count(self.h, t)
+
+    def set_lr(self, lr):
+        scape_set_lr(self.h, lr)
+
+    def set_bias_correction(self, on=True):
+        scape_set_bias_correction(self.h, on)
+
+    def set_clip_grad(self, max_norm):
+        scape_set_clip_grad(self.h, max_norm)
+
+    def last_grad_norm(self):
+        return scape_last_grad_norm(self.h, self._stream())
 
     def select_stats(self):
         return scape_select_stats(self.h, self._stream())

@@ -71,8 +71,14 @@ struct scape {
   float* pm[2] = {nullptr, nullptr};   // packed means b- [packed_stride], alternating
   int pm_last = 0;             // pm[pm_last] = b- of the last sparse step
   const char* last_kernel = "";   // name of the streaming kernel the last step launched
-  int fused_impl = 0;          // SCAPE_FUSED_IMPL (experiments): 0 auto, 1 "ldg" = register-staged kernel only,
-                               // 2 "directstore" = staged loads but direct global stores
+  // optional parts of Alg. 1 (off by default: readings S3, S4)
+  bool bias_correction = false;
+  double beta1_d = 0.0, beta2_d = 0.0, clip_max_norm = 0.0;
+  float* ghat = nullptr;       // [Npad] clip mode: g^ of the selected entries (packed; dense steps use all N)
+  float* vm = nullptr;         // [Npad] clip mode: beta2 * m_old^2 of the selected entries
+  double* sumsq = nullptr;     // [max_seg] clip mode: per-warp partial sums of g^^2
+  ClipState* clip_state = nullptr;
+  int fused_impl = 0;          // SCAPE_FUSED_IMPL (experiments): 0 auto, 1 "ldg" = register-staged kernel only
   bool m_sparse = false;       // m_{t-1} lives in pm[pm_last] addressed through slot[last]; h->m is stale
   float* dense_pack = nullptr;    // optional [R][Npad]
   bool last_dense = false;
@@ -89,6 +95,7 @@ struct scape {
   uint32_t* total = nullptr;      // [1]
   int n_compact_blocks = 0;
   int n_seg = 0;                  // segments (= warps) of the last fused launch
+  int n_slots = 0;                // warps of the last streaming launch (clip-mode partial sums)
   uint32_t seg_cap = 0;
 
   // optional per-step CUDA-event timing of the fused kernel and of the select stage
@@ -126,6 +133,7 @@ int launch_fused_t(scape* h, StepParams& p, cudaStream_t st) {
   const int grid = grid_for(h, p.n_chunks, 8, bps);
   // one candidate segment per warp of this launch
   h->n_seg = grid * 8;
+  h->n_slots = grid * 8;
   int64_t cap = (h->cand_cap / h->n_seg) & ~(int64_t)15;
   if (cap > 0x7FFFFFF0) cap = 0x7FFFFFF0;
   h->seg_cap = (uint32_t)cap;
@@ -181,14 +189,15 @@ int launch_tma_t(scape* h, StepParams& p, cudaStream_t st) {
   int64_t grid = (int64_t)h->n_sm * cfg_bps;
   if (grid > n_tiles) grid = n_tiles;
   h->n_seg = (int)grid * kTmaConsumerWarps;
+  h->n_slots = h->n_seg;
   int64_t cap = (h->cand_cap / h->n_seg) & ~(int64_t)15;
   if (cap > 0x7FFFFFF0) cap = 0x7FFFFFF0;
   h->seg_cap = (uint32_t)cap;
   p.seg_cap = h->seg_cap;
   const size_t smem = kTmaBarrierBytes + (size_t)cfg_stages * TILE;
-  // results leave through the stage as whole-tile bulk stores (default) or as direct 128-bit stores
-  if (h->fused_impl == 2) scape_fused_tma_kernel<G, R, false><<<(int)grid, kTmaThreads, smem, st>>>(p, cfg_stages);
-  else scape_fused_tma_kernel<G, R, true><<<(int)grid, kTmaThreads, smem, st>>>(p, cfg_stages);
+  // the clip_grad variant is a separate instantiation so that the default path carries none of it
+  if (p.clip) scape_fused_tma_kernel<G, R, true><<<(int)grid, kTmaThreads, smem, st>>>(p, cfg_stages);
+  else scape_fused_tma_kernel<G, R, false><<<(int)grid, kTmaThreads, smem, st>>>(p, cfg_stages);
   h->last_kernel = "scape_fused_tma_kernel";
   h->launches++;
   CU_TRY(cudaGetLastError());
@@ -313,6 +322,7 @@ void free_all(scape* h) {
   for (auto& s : h->slot) { cudaFree(s.bits); cudaFree(s.rank); cudaFree(s.idx); }
   cudaFree(h->packed); cudaFree(h->pm[0]); cudaFree(h->pm[1]); cudaFree(h->dense_pack);
   cudaFree(h->sel); cudaFree(h->cand); cudaFree(h->cls); cudaFree(h->seg_count); cudaFree(h->seg_above); cudaFree(h->ghist); cudaFree(h->block_sum); cudaFree(h->total);
+  cudaFree(h->ghat); cudaFree(h->vm); cudaFree(h->sumsq); cudaFree(h->clip_state);
   cudaFree(h->st_param);
   for (auto& g : h->st_grad) cudaFree(g);
   if (h->prof_have_events)
@@ -338,7 +348,7 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   scape* h = new (std::nothrow) scape();
   if (!h) { fail(SCAPE_ENOMEM, "host allocation failed"); return nullptr; }
   h->dev = dev;
-  if (const char* ev = getenv("SCAPE_FUSED_IMPL")) h->fused_impl = (strcmp(ev, "ldg") == 0) ? 1 : (strcmp(ev, "directstore") == 0) ? 2 : 0;
+  if (const char* ev = getenv("SCAPE_FUSED_IMPL")) h->fused_impl = (strcmp(ev, "ldg") == 0) ? 1 : 0;
   cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev);
   h->N = N; h->R = R;
   h->Npad = (N + kChunk - 1) / kChunk * kChunk;
@@ -348,6 +358,7 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   // hyper-parameters are cast to fp32 once; 1 - beta is evaluated in fp32
   h->b1 = (float)beta1; h->b2 = (float)beta2; h->eps = (float)eps; h->lr = (float)lr; h->wd = (float)wd;
   h->c1 = 1.0f - h->b1; h->c2 = 1.0f - h->b2;
+  h->beta1_d = beta1; h->beta2_d = beta2;
   h->n_compact_blocks = (int)((h->n_chunks + kCompactChunksPerBlock - 1) / kCompactChunksPerBlock);
   const bool sparse = h->k < N;
   h->packed_stride = sparse ? (h->k + 31) / 32 * 32 : 0;
@@ -459,6 +470,51 @@ extern "C" int scape_set_keep_dense_pack(scape_t* h, int on) {
   return SCAPE_OK;
 }
 
+extern "C" int scape_set_lr(scape_t* h, double lr) {
+  if (!h || !std::isfinite(lr)) return fail(SCAPE_EINVAL, "bad argument");
+  h->lr = (float)lr;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_set_bias_correction(scape_t* h, int on) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  h->bias_correction = on != 0;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_set_clip_grad(scape_t* h, double max_norm) {
+  if (!h || !(max_norm >= 0.0) || !std::isfinite(max_norm)) return fail(SCAPE_EINVAL, "max_norm must be finite and >= 0");
+  DeviceGuard g(h->dev);
+  if (max_norm > 0.0 && !h->ghat) {
+    const int slots = h->n_sm * 8 * 8;
+    bool ok = cudaMalloc((void**)&h->ghat, sizeof(float) * h->Npad) == cudaSuccess &&
+              cudaMalloc((void**)&h->vm, sizeof(float) * h->Npad) == cudaSuccess &&
+              cudaMalloc((void**)&h->sumsq, sizeof(double) * slots) == cudaSuccess &&
+              cudaMalloc((void**)&h->clip_state, sizeof(ClipState)) == cudaSuccess;
+    if (!ok) {
+      cudaGetLastError();
+      cudaFree(h->ghat); cudaFree(h->vm); cudaFree(h->sumsq); cudaFree(h->clip_state);
+      h->ghat = h->vm = nullptr; h->sumsq = nullptr; h->clip_state = nullptr;
+      return fail(SCAPE_ENOMEM, "clip_grad: allocation of 2 N floats failed");
+    }
+    cudaMemset(h->clip_state, 0, sizeof(ClipState));
+  }
+  h->clip_max_norm = max_norm;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_last_grad_norm(scape_t* h, double* norm, double* coef, void* cuda_stream) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (!h->clip_state) return fail(SCAPE_EINVAL, "clip_grad has never been switched on");
+  DeviceGuard g(h->dev);
+  ClipState cs{};
+  CU_TRY(cudaMemcpyAsync(&cs, h->clip_state, sizeof cs, cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
+  CU_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+  if (norm) *norm = cs.norm;
+  if (coef) *coef = (double)cs.coef;
+  return SCAPE_OK;
+}
+
 extern "C" int scape_set_step_count(scape_t* h, int64_t t) {
   if (!h || t < 0) return fail(SCAPE_EINVAL, "bad argument");
   h->t = t;
@@ -504,6 +560,14 @@ extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, vo
   p.R_f = (float)h->R; p.inv_R = 1.0f / (float)h->R;
   p.r_pow2 = (h->R & (h->R - 1)) == 0;      // x / 2^n == x * 2^-n bit for bit
   p.stash = cur.all_ones && need_select;
+  p.bc1 = 1.0f; p.bc2 = 1.0f;
+  if (h->bias_correction) {      // PAPER.md:77; factors evaluated in double from the step number, cast once
+    const double t = (double)(h->t + 1);
+    p.bc1 = (float)(1.0 / (1.0 - std::pow(h->beta1_d, t)));
+    p.bc2 = (float)(1.0 / (1.0 - std::pow(h->beta2_d, t)));
+  }
+  const bool clip = h->clip_max_norm > 0.0;
+  p.clip = clip ? 1 : 0; p.ghat = h->ghat; p.vm = h->vm; p.sumsq = h->sumsq;
   p.ctl = h->sel; p.next_bits = nxt.bits; p.cand = h->cand;
   p.seg_count = h->seg_count; p.seg_above = h->seg_above;
 
@@ -513,6 +577,16 @@ extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, vo
   if (prof) CU_TRY(cudaEventRecord(h->prof_ev[pi][0], st));
   rc = launch_fused(h, p, cur.all_ones, msparse, st);
   if (rc) return rc;
+  if (clip) {
+    // l.14-17 on the mask: norm of g^ (fixed-order reduction), then the deferred update
+    const int64_t K = cur.count;
+    clip_norm_kernel<<<1, 1024, 0, st>>>(h->sumsq, h->n_slots, h->clip_max_norm, h->clip_state);
+    int g2 = (int)((K + 255) / 256); if (g2 > h->n_sm * 16) g2 = h->n_sm * 16; if (g2 < 1) g2 = 1;
+    clip_update_kernel<<<g2, 256, 0, st>>>(param, cur.all_ones ? nullptr : cur.idx, cur.all_ones ? h->m : h->pm[pm_out],
+                                           h->ghat, h->vm, K, h->clip_state, h->c2, h->eps, h->wd, -h->lr, p.bc1, p.bc2);
+    h->launches += 2;
+    CU_TRY(cudaGetLastError());
+  }
   if (prof) CU_TRY(cudaEventRecord(h->prof_ev[pi][1], st));
 
   if (need_select) {

@@ -68,6 +68,13 @@ struct StepParams {
   float b1, c1, b2, c2, eps, wd, neg_lr;
   float R_f, inv_R;
   int r_pow2;
+  float bc1, bc2;               // bias-correction factors 1/(1-beta^t); 1.0f when off
+  // l.14 clip_grad (optional): the pass stores g^ and beta2*m^2 of every selected entry, sums g^^2
+  // in double, and leaves theta on the mask alone; clip_update_kernel finishes l.14-17 there
+  int clip;
+  float* ghat;                  // [K] packed
+  float* vm;                    // [K] packed
+  double* sumsq;                // one slot per warp of the launch
   int stash;                    // DENSE only: leave m~^0 in e^0 (keys for the select), not 0
   // stage 2 fused into the pass (sparse variant only)
   const SelState* ctl;          // bracket predicted by the previous step
@@ -153,17 +160,27 @@ struct StageA {                 // per-warp running state of the fused select (r
   uint32_t n_above;             // per lane
   uint32_t cursor;              // warp-uniform: candidates appended so far
   unsigned long long* seg;      // this warp's candidate segment
+  double sumsq;                 // per lane: sum of g^^2 (clip mode)
 };
+
+// clip mode: this warp's share of sum g^^2, lanes added in a fixed butterfly order
+__device__ __forceinline__ void warp_store_sumsq(const StepParams& p, const StageA& sa, int64_t slot, int lane) {
+  double v = sa.sumsq;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+  if (lane == 0) p.sumsq[slot] = v;
+}
 
 // The arithmetic of one lane's 4 elements (Alg. 1 l.6-10, l.12-17 in the pinned order), the stores
 // of theta / m / e^r / b^r / b-, and the bracket classification of stage 2.  Shared by the two
 // load front-ends (register-staged LDG and shared-memory-staged bulk copies).
-template <int R, bool DENSE, bool GUARD, bool STORE = true>
+template <int R, bool DENSE, bool GUARD, bool STORE = true, bool CLIPT = true>
 __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, int lane, int64_t i0,
                                               uint32_t mybits, uint32_t jbase, float (&th)[4], const float (&mo)[4],
                                               float (&gg)[R][4], float (&ee)[R][4], StageA& sa) {
   float mn[4];
   uint32_t key0[4];             // bits(|m~^0|): the selection statistic of l.11
+  uint32_t deferred = 0;        // clip mode: entries whose theta update is left to clip_update_kernel
 #pragma unroll
   for (int q = 0; q < 4; ++q) {
     const bool on = DENSE || ((mybits >> q) & 1u);
@@ -197,12 +214,24 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
         for (int r = 1; r < R; ++r) s = __fadd_rn(s, mt[r]);                                   // l.10, r ascending
         const float bb = p.r_pow2 ? __fmul_rn(s, p.inv_R) : __fdiv_rn(s, p.R_f);              // l.10
         const float gh = __fdiv_rn(__fsub_rn(bb, pq), p.c1);                                    // l.13 (Eq. 3)
-        const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), __fmul_rn(p.b2, __fmul_rn(mo[q], mo[q])));  // l.15
-        u = __fdiv_rn(bb, __fadd_rn(__fsqrt_rn(v), p.eps));                                     // l.16
+        const float vmq = __fmul_rn(p.b2, __fmul_rn(mo[q], mo[q]));
         mn[q] = bb;                                                                             // l.12
         if (!DENSE) p.packed_mean[j] = bb;
+        if (CLIPT && p.clip) {
+          // l.14 needs the norm of g^ over the whole mask first: park what l.15-17 need
+          const int64_t jj = DENSE ? (i0 + q) : (int64_t)j;
+          if (!GUARD || i0 + q < p.N) {
+            p.ghat[jj] = gh; p.vm[jj] = vmq;
+            sa.sumsq += (double)gh * (double)gh;
+          }
+          deferred |= 1u << q;
+        } else {
+          const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), vmq);                              // l.15
+          u = __fdiv_rn(__fmul_rn(bb, p.bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, p.bc2)), p.eps));   // l.16 (+ :77)
+        }
       }
     }
+    if (CLIPT && ((deferred >> q) & 1u)) continue;          // theta of this entry is updated by clip_update_kernel
     const float w = __fmaf_rn(p.wd, th[q], u);                                      // l.17
     th[q] = __fmaf_rn(p.neg_lr, w, th[q]);
   }
@@ -300,6 +329,7 @@ __global__ void __launch_bounds__(256, (R <= 4 ? 3 : 2)) scape_fused_step_kernel
     for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
     if (lane == 0) { p.seg_count[warp] = sa.cursor; p.seg_above[warp] = na; }
   }
+  if (p.clip) warp_store_sumsq(p, sa, warp, lane);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -372,7 +402,7 @@ __device__ __forceinline__ void bulk_s2g(void* dst, const void* src_smem, uint32
                ::"l"(dst), "r"(smem_u32(src_smem)), "r"(bytes), "l"(policy) : "memory");
 }
 
-template <typename G, int R, bool TSTORE>
+template <typename G, int R, bool CLIPT>
 __device__ __forceinline__ void tma_consume_tile(const StepParams& p, int64_t tile, int64_t n_tiles, int64_t tstride,
                                                  int warp, int lane, unsigned char* stage0, uint64_t* full, uint64_t* empty,
                                                  int& s, uint32_t& ph, int n_stages, TmaMaskWords& nw,
@@ -406,39 +436,32 @@ __device__ __forceinline__ void tma_consume_tile(const StepParams& p, int64_t ti
       gg[r][2] = __uint_as_float(g.y << 16); gg[r][3] = __uint_as_float(g.y & 0xFFFF0000u);
     }
   }
-  if (!TSTORE) {
-    __syncwarp();
-    if (lane == 0) mbar_arrive(&empty[s]);                      // this warp is done with the stage
-    if (++s == n_stages) { s = 0; ph ^= 1u; }
-    fused_compute<R, false, false, true>(p, c, lane, i0, cur.mybits, cur.jbase, th, cur.mo, gg, ee, sa);
-  } else {
-    // Results go back into the stage (in place) and leave as whole-tile bulk stores: 4 KB bursts
-    // per stream instead of 512-byte warp stores.
-    fused_compute<R, false, false, false>(p, c, lane, i0, cur.mybits, cur.jbase, th, cur.mo, gg, ee, sa);
-    unsigned char* wbase = stage0 + (size_t)s * TILE;
-    *reinterpret_cast<float4*>(wbase + off * 4u) = make_float4(th[0], th[1], th[2], th[3]);
+  // Results go back into the stage (in place) and leave as whole-tile bulk stores: 4 KB bursts
+  // per stream instead of 512-byte warp stores.
+  fused_compute<R, false, false, false, CLIPT>(p, c, lane, i0, cur.mybits, cur.jbase, th, cur.mo, gg, ee, sa);
+  unsigned char* wbase = stage0 + (size_t)s * TILE;
+  *reinterpret_cast<float4*>(wbase + off * 4u) = make_float4(th[0], th[1], th[2], th[3]);
 #pragma unroll
-    for (int r = 0; r < R; ++r)
-      *reinterpret_cast<float4*>(wbase + OFF_E + r * (kTmaTile * 4u) + off * 4u) = make_float4(ee[r][0], ee[r][1], ee[r][2], ee[r][3]);
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumerWarps * 32) : "memory");
-    if (threadIdx.x == 0) {
-      uint64_t pol;
-      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-      const int64_t e0 = tile * kTmaTile;
-      bulk_s2g(p.theta + e0, wbase, kTmaTile * 4u, pol);
+  for (int r = 0; r < R; ++r)
+    *reinterpret_cast<float4*>(wbase + OFF_E + r * (kTmaTile * 4u) + off * 4u) = make_float4(ee[r][0], ee[r][1], ee[r][2], ee[r][3]);
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumerWarps * 32) : "memory");
+  if (threadIdx.x == 0) {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    const int64_t e0 = tile * kTmaTile;
+    bulk_s2g(p.theta + e0, wbase, kTmaTile * 4u, pol);
 #pragma unroll
-      for (int r = 0; r < R; ++r) bulk_s2g(p.e + r * p.e_stride + e0, wbase + OFF_E + r * (kTmaTile * 4u), kTmaTile * 4u, pol);
-      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-      // the stores of the PREVIOUS tile have finished reading their stage: hand it back
-      asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
-      if (tile != (int64_t)blockIdx.x) mbar_arrive(&empty[s == 0 ? n_stages - 1 : s - 1]);
-    }
-    if (++s == n_stages) { s = 0; ph ^= 1u; }
+    for (int r = 0; r < R; ++r) bulk_s2g(p.e + r * p.e_stride + e0, wbase + OFF_E + r * (kTmaTile * 4u), kTmaTile * 4u, pol);
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    // the stores of the PREVIOUS tile have finished reading their stage: hand it back
+    asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+    if (tile != (int64_t)blockIdx.x) mbar_arrive(&empty[s == 0 ? n_stages - 1 : s - 1]);
   }
+  if (++s == n_stages) { s = 0; ph ^= 1u; }
 }
 
-template <typename G, int R, bool TSTORE>
+template <typename G, int R, bool CLIPT>
 __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const __grid_constant__ StepParams p, int n_stages) {
   extern __shared__ __align__(128) unsigned char smem[];
   constexpr uint32_t TILE = tma_tile_bytes<G, R>();
@@ -450,7 +473,7 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
   const int64_t n_tiles = p.N / kTmaTile;                     // full tiles; the rest goes through the LDG path
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < n_stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], TSTORE ? 1 : kTmaConsumerWarps); }
+    for (int s = 0; s < n_stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -503,13 +526,13 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
   }
   int s = 0; uint32_t ph = 0;
   while (tile < n_tiles) {
-    tma_consume_tile<G, R, TSTORE>(p, tile, n_tiles, tstride, warp, lane, stage0, full, empty, s, ph, n_stages, nw, stA, stB, sa);
+    tma_consume_tile<G, R, CLIPT>(p, tile, n_tiles, tstride, warp, lane, stage0, full, empty, s, ph, n_stages, nw, stA, stB, sa);
     tile += tstride;
     if (tile >= n_tiles) break;
-    tma_consume_tile<G, R, TSTORE>(p, tile, n_tiles, tstride, warp, lane, stage0, full, empty, s, ph, n_stages, nw, stB, stA, sa);
+    tma_consume_tile<G, R, CLIPT>(p, tile, n_tiles, tstride, warp, lane, stage0, full, empty, s, ph, n_stages, nw, stB, stA, sa);
     tile += tstride;
   }
-  if (TSTORE && threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // stores have landed
+  if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // stores have landed
 
   // chunks past the last full tile (fewer than 8, the last one possibly ragged): LDG path
   {
@@ -523,6 +546,7 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
   if (lane == 0) { p.seg_count[gwarp] = sa.cursor; p.seg_above[gwarp] = na; }
+  if (CLIPT && p.clip) warp_store_sumsq(p, sa, gwarp, lane);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -919,6 +943,43 @@ __global__ void __launch_bounds__(1024) mask_rank_idx_kernel(const uint32_t* __r
       if ((int64_t)j < idx_cap) idx[j] = (int32_t)(base + (q << 5) + b);
       ++j;
     }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// l.14 clip_grad (optional, reading S3'): global-norm clip of the reconstructed gradient
+// ------------------------------------------------------------------------------------------
+struct ClipState { double norm; float coef; int pad; };
+
+// one block: sum the per-warp partial sums in a fixed order, derive the factor
+__global__ void __launch_bounds__(1024) clip_norm_kernel(const double* __restrict__ sumsq, int n_slots, double max_norm, ClipState* out) {
+  __shared__ double sh[1024];
+  double a = 0.0;
+  for (int i = threadIdx.x; i < n_slots; i += 1024) a += sumsq[i];
+  sh[threadIdx.x] = a;
+  __syncthreads();
+  for (int o = 512; o > 0; o >>= 1) { if ((int)threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o]; __syncthreads(); }
+  if (threadIdx.x == 0) {
+    const double nrm = sqrt(sh[0]);
+    const double cc = max_norm / (nrm + 1e-6);              // the torch / Megatron clip_grad_norm rule
+    out->norm = nrm;
+    out->coef = cc < 1.0 ? (float)cc : 1.0f;
+  }
+}
+
+// l.14-17 for the K entries of the mask: scale g^, second moment, update, parameter step
+__global__ void __launch_bounds__(256) clip_update_kernel(float* __restrict__ theta, const int32_t* __restrict__ idx,
+                                                         const float* __restrict__ bb, const float* __restrict__ ghat,
+                                                         const float* __restrict__ vm, int64_t K, const ClipState* __restrict__ cs,
+                                                         float c2, float eps, float wd, float neg_lr, float bc1, float bc2) {
+  const float coef = cs->coef;
+  for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < K; j += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t i = idx ? (int64_t)idx[j] : j;
+    const float gh = __fmul_rn(ghat[j], coef);                                              // l.14
+    const float v = __fmaf_rn(c2, __fmul_rn(gh, gh), vm[j]);                               // l.15
+    const float u = __fdiv_rn(__fmul_rn(bb[j], bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, bc2)), eps));   // l.16 (+ :77)
+    const float t = theta[i];
+    theta[i] = __fmaf_rn(neg_lr, __fmaf_rn(wd, t, u), t);                                   // l.17
   }
 }
 

@@ -322,3 +322,77 @@ def test_select_survives_threshold_jumps(B):
     fast, general = gpu.select_stats()
     assert fast >= 2 and general >= 3, (fast, general)
     gpu.close()
+
+
+# ------------------------------------------------------------------------------------------
+# Optional parts of Alg. 1: learning-rate schedule, bias correction, clip_grad (l.14)
+# ------------------------------------------------------------------------------------------
+def run_options_parity(B, w, steps, seed, bias_correction=False, clip=0.0, lr_schedule=False, exact=True):
+    N, R = w.numel, w.R
+    gs = synth.GradStream(w, device="cuda", seed=seed)
+    th_gpu = gs.theta0()
+    th_ora = th_gpu.cpu().numpy().copy()
+    gpu = B.Scape(N, R, w.sparsity, **HYP)
+    gpu.keep_dense_pack(True)
+    ora = ScapeOracle(N, R, w.sparsity, **HYP)
+    for o in (gpu, ora):
+        o.set_bias_correction(bias_correction)
+        o.set_clip_grad(clip)
+    clipped = 0
+    for t in range(1, steps + 1):
+        if lr_schedule:
+            lr = HYP["lr"] * (0.25 + 0.25 * t)
+            gpu.set_lr(lr)
+            ora.set_lr(lr)
+        grads = gs.next()
+        gpu.step(th_gpu, grads)
+        ora.step(th_ora, [to_np32(g) for g in grads])
+        if clip > 0:
+            norm, coef = gpu.last_grad_norm()
+            np.testing.assert_allclose(norm, ora.last_norm(), rtol=1e-12)
+            np.testing.assert_allclose(coef, ora.last_coef(), rtol=2e-7)
+            clipped += coef < 1.0
+            same_coef = np.float32(coef) == np.float32(ora.last_coef())
+        else:
+            same_coef = True
+        compare_step(gpu, ora, th_gpu, th_ora, R, f"{w.name} opt step {t}", exact=exact and same_coef)
+    gpu.close()
+    return clipped
+
+
+def small_workload(name, N, R, s, gdt="f32"):
+    return synth.Workload(name, [("a", N // 3), ("b", N - N // 3)], R=R, sparsity=s, dist="t4", rho=0.9,
+                          grad_dtype=gdt, steps=6)
+
+
+def test_bias_correction_and_lr_schedule(B):
+    run_options_parity(B, small_workload("bc", 200_003, 3, 0.99), 6, seed=21, bias_correction=True, lr_schedule=True)
+    run_options_parity(B, small_workload("bc_dense", 50_001, 2, 0.0, "bf16"), 4, seed=22, bias_correction=True, lr_schedule=True)
+
+
+@pytest.mark.parametrize("N,R,s,gdt,clip", [
+    (300_007, 4, 0.99, "bf16", 1e-3),      # staged kernel, clip bites every step
+    (300_007, 2, 0.9, "f32", 2e-3),        # register-staged kernel
+    (40_001, 3, 0.0, "f32", 1e-2),         # all-ones mask every step: the deferred update covers all N
+])
+def test_clip_grad(B, N, R, s, gdt, clip):
+    clipped = run_options_parity(B, small_workload("clip", N, R, s, gdt), 6, seed=N, clip=clip, bias_correction=True)
+    assert clipped >= 3
+
+
+def test_clip_grad_above_the_norm_is_a_bitwise_noop(B):
+    w = small_workload("clip_noop", 150_011, 3, 0.99)
+    gs = synth.GradStream(w, device="cuda", seed=5)
+    th_a = gs.theta0()
+    th_b = th_a.clone()
+    a, b = B.Scape(w.numel, w.R, w.sparsity, **HYP), B.Scape(w.numel, w.R, w.sparsity, **HYP)
+    b.set_clip_grad(1e9)
+    for _ in range(5):
+        grads = gs.next()
+        a.step(th_a, grads)
+        b.step(th_b, grads)
+        assert b.last_grad_norm()[1] == 1.0
+        assert torch.equal(th_a, th_b)
+    np.testing.assert_array_equal(a.mask_next(), b.mask_next())
+    a.close()
+    b.close()
