@@ -78,6 +78,7 @@ struct scape {
   float* vm = nullptr;         // [Npad] clip mode: beta2 * m_old^2 of the selected entries
   double* sumsq = nullptr;     // [max_seg] clip mode: per-warp partial sums of g^^2
   ClipState* clip_state = nullptr;
+  uint32_t compact_min = 3;    // SCAPE_COMPACT_MIN (experiments)
   int fused_impl = 0;          // SCAPE_FUSED_IMPL (experiments): 0 auto, 1 "ldg" = register-staged kernel only
   bool m_sparse = false;       // m_{t-1} lives in pm[pm_last] addressed through slot[last]; h->m is stale
   float* dense_pack = nullptr;    // optional [R][Npad]
@@ -348,6 +349,7 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   scape* h = new (std::nothrow) scape();
   if (!h) { fail(SCAPE_ENOMEM, "host allocation failed"); return nullptr; }
   h->dev = dev;
+  if (const char* ev = getenv("SCAPE_COMPACT_MIN")) { int v = atoi(ev); if (v >= 1) h->compact_min = (uint32_t)v; }
   if (const char* ev = getenv("SCAPE_FUSED_IMPL")) h->fused_impl = (strcmp(ev, "ldg") == 0) ? 1 : 0;
   cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev);
   h->N = N; h->R = R;
@@ -560,6 +562,7 @@ extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, vo
   p.R_f = (float)h->R; p.inv_R = 1.0f / (float)h->R;
   p.r_pow2 = (h->R & (h->R - 1)) == 0;      // x / 2^n == x * 2^-n bit for bit
   p.stash = cur.all_ones && need_select;
+  p.compact_min = h->compact_min;
   p.bc1 = 1.0f; p.bc2 = 1.0f;
   if (h->bias_correction) {      // PAPER.md:77; factors evaluated in double from the step number, cast once
     const double t = (double)(h->t + 1);

@@ -76,6 +76,7 @@ struct StepParams {
   float* vm;                    // [K] packed
   double* sumsq;                // one slot per warp of the launch
   int stash;                    // DENSE only: leave m~^0 in e^0 (keys for the select), not 0
+  uint32_t compact_min;         // selected entries per chunk from which l.10-16 run in compacted form
   // stage 2 fused into the pass (sparse variant only)
   const SelState* ctl;          // bracket predicted by the previous step
   uint32_t* next_bits;          // [Npad/32] certainly-selected bits of M_t (complete overwrite)
@@ -139,6 +140,7 @@ __device__ __forceinline__ void lane_bits_from_words(const uint4 mw, const uint3
   mybits = (w >> sh) & 0xFu;
   jbase = r0 + before + __popc(w & ((1u << sh) - 1u));
 }
+__device__ __forceinline__ uint32_t chunk_popc(const uint4 mw) { return __popc(mw.x) + __popc(mw.y) + __popc(mw.z) + __popc(mw.w); }
 
 __device__ __forceinline__ void lane_mask_bits(const uint32_t* __restrict__ bits, const uint32_t* __restrict__ rank,
                                                int64_t c, int lane, uint32_t& mybits, uint32_t& jbase) {
@@ -174,76 +176,172 @@ __device__ __forceinline__ void warp_store_sumsq(const StepParams& p, const Stag
 // The arithmetic of one lane's 4 elements (Alg. 1 l.6-10, l.12-17 in the pinned order), the stores
 // of theta / m / e^r / b^r / b-, and the bracket classification of stage 2.  Shared by the two
 // load front-ends (register-staged LDG and shared-memory-staged bulk copies).
-template <int R, bool DENSE, bool GUARD, bool STORE = true, bool CLIPT = true>
+//
+// Sparse steps: the selected entries of a chunk (cnt of 128; ~13 at 90 % sparsity, ~1 at 99 %) are
+// scattered over the lanes, so running l.10-16 (IEEE divisions, square root) where they sit would
+// mean four divergent passes with a few active lanes each.  Instead every lane parks (sum_r m~^r,
+// m_old) of its selected entries in a warp-private scratch at the entry's rank inside the chunk,
+// and lane l then runs l.10-16 for the entry of rank l: one pass, consecutive lanes, b- stored
+// coalesced.  The update u comes back through the same scratch.
+//   r0 = rank128[c]; cnt = set bits of the chunk; scs, scm = 128 floats each, private to this warp
+template <int R, bool DENSE, bool GUARD, bool STORE = true, bool CLIPT = true, bool COMPACT = true>
 __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, int lane, int64_t i0,
-                                              uint32_t mybits, uint32_t jbase, float (&th)[4], const float (&mo)[4],
+                                              uint32_t mybits, uint32_t jbase, uint32_t r0, uint32_t cnt, float* scs, float* scm,
+                                              float (&th)[4], const float (&mo)[4],
                                               float (&gg)[R][4], float (&ee)[R][4], StageA& sa) {
-  float mn[4];
   uint32_t key0[4];             // bits(|m~^0|): the selection statistic of l.11
-  uint32_t deferred = 0;        // clip mode: entries whose theta update is left to clip_update_kernel
+  if constexpr (DENSE) {
+    float mn[4];
 #pragma unroll
-  for (int q = 0; q < 4; ++q) {
-    const bool on = DENSE || ((mybits >> q) & 1u);
-    const float pq = __fmul_rn(p.b1, mo[q]);                // beta1 * m_{t-1}, reused by l.6 and l.13
-    float mt[R];
+    for (int q = 0; q < 4; ++q) {
+      const float pq = __fmul_rn(p.b1, mo[q]);                // beta1 * m_{t-1}, reused by l.6 and l.13
+      float mt[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-      mt[r] = __fadd_rn(__fmaf_rn(p.c1, gg[r][q], pq), ee[r][q]);            // l.6
-      ee[r][q] = on ? ((DENSE && r == 0 && p.stash) ? mt[r] : 0.0f) : mt[r]; // l.7-8
-    }
-    key0[q] = __float_as_uint(mt[0]) & 0x7FFFFFFFu;
-    float u = 0.0f;                                                          // Eq. 5: u = 0 off the mask
-    mn[q] = 0.0f;                                                            // Eq. 4: m = 0 off the mask
-    // At 90-99 % sparsity most warps have no selected element at a given q: a warp-uniform vote
-    // skips the pack, the replica mean and the IEEE divisions / square root entirely.
-    if (DENSE || __any_sync(0xFFFFFFFFu, on)) {
-      if (on) {
-        const uint32_t j = DENSE ? 0u : jbase + __popc(mybits & ((1u << q) - 1u));
-        float s = mt[0];
-        if (DENSE) {
-          if (p.packed != nullptr && (!GUARD || i0 + q < p.N)) {
+      for (int r = 0; r < R; ++r) {
+        mt[r] = __fadd_rn(__fmaf_rn(p.c1, gg[r][q], pq), ee[r][q]);            // l.6
+        ee[r][q] = (r == 0 && p.stash) ? mt[r] : 0.0f;                         // l.8 (M = 1); stash: keys for the select
+      }
+      key0[q] = __float_as_uint(mt[0]) & 0x7FFFFFFFu;
+      if (p.packed != nullptr && (!GUARD || i0 + q < p.N)) {
 #pragma unroll
-            for (int r = 0; r < R; ++r) p.packed[r * p.packed_stride + (i0 + q)] = mt[r];   // l.9 (keep_dense_pack)
-          }
-        } else {
-          float* pk = p.packed + j;
+        for (int r = 0; r < R; ++r) p.packed[r * p.packed_stride + (i0 + q)] = mt[r];   // l.9 (keep_dense_pack)
+      }
+      float s = mt[0];
 #pragma unroll
-          for (int r = 0; r < R; ++r) { *pk = mt[r]; pk += p.packed_stride; }                  // l.9
+      for (int r = 1; r < R; ++r) s = __fadd_rn(s, mt[r]);                                   // l.10, r ascending
+      const float bb = p.r_pow2 ? __fmul_rn(s, p.inv_R) : __fdiv_rn(s, p.R_f);              // l.10
+      const float gh = __fdiv_rn(__fsub_rn(bb, pq), p.c1);                                    // l.13 (Eq. 3)
+      const float vmq = __fmul_rn(p.b2, __fmul_rn(mo[q], mo[q]));
+      mn[q] = bb;                                                                             // l.12
+      if (CLIPT && p.clip) {
+        // l.14 needs the norm of g^ over the whole mask first: park what l.15-17 need; theta of
+        // this entry is updated by clip_update_kernel
+        if (!GUARD || i0 + q < p.N) {
+          p.ghat[i0 + q] = gh; p.vm[i0 + q] = vmq;
+          sa.sumsq += (double)gh * (double)gh;
         }
-#pragma unroll
-        for (int r = 1; r < R; ++r) s = __fadd_rn(s, mt[r]);                                   // l.10, r ascending
-        const float bb = p.r_pow2 ? __fmul_rn(s, p.inv_R) : __fdiv_rn(s, p.R_f);              // l.10
-        const float gh = __fdiv_rn(__fsub_rn(bb, pq), p.c1);                                    // l.13 (Eq. 3)
-        const float vmq = __fmul_rn(p.b2, __fmul_rn(mo[q], mo[q]));
-        mn[q] = bb;                                                                             // l.12
-        if (!DENSE) p.packed_mean[j] = bb;
-        if (CLIPT && p.clip) {
-          // l.14 needs the norm of g^ over the whole mask first: park what l.15-17 need
-          const int64_t jj = DENSE ? (i0 + q) : (int64_t)j;
-          if (!GUARD || i0 + q < p.N) {
-            p.ghat[jj] = gh; p.vm[jj] = vmq;
-            sa.sumsq += (double)gh * (double)gh;
-          }
-          deferred |= 1u << q;
-        } else {
-          const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), vmq);                              // l.15
-          u = __fdiv_rn(__fmul_rn(bb, p.bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, p.bc2)), p.eps));   // l.16 (+ :77)
-        }
+      } else {
+        const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), vmq);                              // l.15
+        const float u = __fdiv_rn(__fmul_rn(bb, p.bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, p.bc2)), p.eps));   // l.16 (+ :77)
+        const float w = __fmaf_rn(p.wd, th[q], u);                                            // l.17
+        th[q] = __fmaf_rn(p.neg_lr, w, th[q]);
       }
     }
-    if (CLIPT && ((deferred >> q) & 1u)) continue;          // theta of this entry is updated by clip_update_kernel
-    const float w = __fmaf_rn(p.wd, th[q], u);                                      // l.17
-    th[q] = __fmaf_rn(p.neg_lr, w, th[q]);
-  }
-
-  if (STORE) {                                              // else the caller stores th / ee (staged bulk stores)
-    store4_f32<GUARD>(p.theta, i0, p.N, th);
+    if (STORE) {
+      store4_f32<GUARD>(p.theta, i0, p.N, th);
 #pragma unroll
-    for (int r = 0; r < R; ++r) store4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
-  }
-  if (DENSE) store4_f32<false>(p.m, i0, p.N, mn);           // sparse steps keep m_t as b- only
+      for (int r = 0; r < R; ++r) store4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
+    }
+    store4_f32<false>(p.m, i0, p.N, mn);                    // sparse steps keep m_t as b- only
+    return;
+  } else {
+    const bool deferred = CLIPT && p.clip;                  // theta on the mask is left to clip_update_kernel
+    if (COMPACT && cnt == 0) {
+      // no selected entry in this chunk (88 % of the chunks at 99.9 % sparsity): l.6-8 and l.17 only
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const float pq = __fmul_rn(p.b1, mo[q]);
+#pragma unroll
+        for (int r = 0; r < R; ++r) ee[r][q] = __fadd_rn(__fmaf_rn(p.c1, gg[r][q], pq), ee[r][q]);   // l.6-7
+        key0[q] = __float_as_uint(ee[0][q]) & 0x7FFFFFFFu;
+        th[q] = __fmaf_rn(p.neg_lr, __fmaf_rn(p.wd, th[q], 0.0f), th[q]);                            // l.17, u = 0 (Eq. 5)
+      }
+    } else if (!COMPACT || cnt < p.compact_min) {
+      // one or two selected entries: l.10-16 in place, on the few lanes that own them
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const bool on = (mybits >> q) & 1u;
+        const float pq = __fmul_rn(p.b1, mo[q]);
+        float mt[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          mt[r] = __fadd_rn(__fmaf_rn(p.c1, gg[r][q], pq), ee[r][q]);            // l.6
+          ee[r][q] = on ? 0.0f : mt[r];                                          // l.7-8
+        }
+        key0[q] = __float_as_uint(mt[0]) & 0x7FFFFFFFu;
+        float u = 0.0f;                                                          // Eq. 5: u = 0 off the mask
+        if (__any_sync(0xFFFFFFFFu, on)) {
+          if (on) {
+            const uint32_t j = jbase + __popc(mybits & ((1u << q) - 1u));
+            float* pk = p.packed + j;
+            float sm = mt[0];
+#pragma unroll
+            for (int r = 0; r < R; ++r) { *pk = mt[r]; pk += p.packed_stride; }                 // l.9
+#pragma unroll
+            for (int r = 1; r < R; ++r) sm = __fadd_rn(sm, mt[r]);                              // l.10, r ascending
+            const float bb = p.r_pow2 ? __fmul_rn(sm, p.inv_R) : __fdiv_rn(sm, p.R_f);          // l.10
+            const float gh = __fdiv_rn(__fsub_rn(bb, pq), p.c1);                                // l.13 (Eq. 3)
+            const float vmq = __fmul_rn(p.b2, __fmul_rn(mo[q], mo[q]));
+            p.packed_mean[j] = bb;                                                              // l.12: m_t = b-
+            if (deferred) {
+              p.ghat[j] = gh; p.vm[j] = vmq;
+              sa.sumsq += (double)gh * (double)gh;
+            } else {
+              const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), vmq);                          // l.15
+              u = __fdiv_rn(__fmul_rn(bb, p.bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, p.bc2)), p.eps));   // l.16 (+ :77)
+            }
+          }
+        }
+        if (deferred && on) continue;
+        th[q] = __fmaf_rn(p.neg_lr, __fmaf_rn(p.wd, th[q], u), th[q]);                         // l.17
+      }
+    } else {
+      const uint32_t lbase = jbase - r0;                    // rank of this lane's first entry inside the chunk
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const bool on = (mybits >> q) & 1u;
+        const float pq = __fmul_rn(p.b1, mo[q]);
+        float mt[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          mt[r] = __fadd_rn(__fmaf_rn(p.c1, gg[r][q], pq), ee[r][q]);            // l.6
+          ee[r][q] = on ? 0.0f : mt[r];                                          // l.7-8
+        }
+        key0[q] = __float_as_uint(mt[0]) & 0x7FFFFFFFu;
+        if (on) {
+          const uint32_t lj = lbase + __popc(mybits & ((1u << q) - 1u));
+          float* pk = p.packed + (r0 + lj);
+          float sm = mt[0];
+#pragma unroll
+          for (int r = 0; r < R; ++r) { *pk = mt[r]; pk += p.packed_stride; }                   // l.9
+#pragma unroll
+          for (int r = 1; r < R; ++r) sm = __fadd_rn(sm, mt[r]);                                // l.10, r ascending
+          scs[lj] = sm; scm[lj] = mo[q];
+        }
+      }
+      __syncwarp();
+      for (uint32_t l = lane; l < cnt; l += 32) {           // lane l: the chunk's selected entry of rank l
+        const float sm = scs[l], mq = scm[l];
+        const float pq = __fmul_rn(p.b1, mq);
+        const float bb = p.r_pow2 ? __fmul_rn(sm, p.inv_R) : __fdiv_rn(sm, p.R_f);          // l.10
+        const float gh = __fdiv_rn(__fsub_rn(bb, pq), p.c1);                                  // l.13 (Eq. 3)
+        const float vmq = __fmul_rn(p.b2, __fmul_rn(mq, mq));
+        p.packed_mean[r0 + l] = bb;                                                           // l.12: m_t = b-
+        if (deferred) {
+          p.ghat[r0 + l] = gh; p.vm[r0 + l] = vmq;
+          sa.sumsq += (double)gh * (double)gh;
+        } else {
+          const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), vmq);                            // l.15
+          scs[l] = __fdiv_rn(__fmul_rn(bb, p.bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, p.bc2)), p.eps));   // l.16 (+ :77)
+        }
+      }
+      __syncwarp();
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const bool on = (mybits >> q) & 1u;
+        if (deferred && on) continue;
+        const float u = on ? scs[lbase + __popc(mybits & ((1u << q) - 1u))] : 0.0f;            // Eq. 5 off the mask
+        th[q] = __fmaf_rn(p.neg_lr, __fmaf_rn(p.wd, th[q], u), th[q]);                         // l.17
+      }
+      __syncwarp();                                         // the scratch is reused by the next chunk
+    }
 
-  if (!DENSE) {
+    if (STORE) {                                            // else the caller stores th / ee (staged bulk stores)
+      store4_f32<GUARD>(p.theta, i0, p.N, th);
+#pragma unroll
+      for (int r = 0; r < R; ++r) store4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
+    }
+
     // Stage 2 (l.11) fused: classify |m~^0| against the predicted bracket.  Exactness does not
     // depend on the prediction: sel_decide_kernel checks n_above < k <= n_above + n_cand.
     uint32_t nib = 0, cnib = 0;
@@ -277,7 +375,7 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
 }
 
 template <typename G, int R, bool DENSE, bool MSPARSE, bool GUARD>
-__device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int lane, StageA& sa) {
+__device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int lane, float* sc, StageA& sa) {
   const int64_t i0 = (c << 7) + ((int64_t)lane << 2);
   // Issue order matters for latency: the mask words first (L2-resident, short latency), then the
   // 2R+1 streaming loads, and only then the gather of m_{t-1}, whose addresses depend on the
@@ -306,23 +404,28 @@ __device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int 
       mo[q] = ((pbits >> q) & 1u) ? __ldg(p.pm_prev + pbase + __popc(pbits & ((1u << q) - 1u))) : 0.0f;
   }
 
-  fused_compute<R, DENSE, GUARD>(p, c, lane, i0, mybits, jbase, th, mo, gg, ee, sa);
+  constexpr bool COMPACT = R >= 3;      // one or two replicas: latency-bound, the plain in-place path is shorter
+  fused_compute<R, DENSE, GUARD, true, true, COMPACT>(p, c, lane, i0, mybits, jbase, cr, (DENSE || !COMPACT) ? 0u : chunk_popc(cw), sc, sc + kChunk, th, mo, gg, ee, sa);
 }
 
 template <typename G, int R, bool DENSE, bool MSPARSE>
-__global__ void __launch_bounds__(256, (R <= 4 ? 3 : 2)) scape_fused_step_kernel(const __grid_constant__ StepParams p) {
+// resident CTAs per SM: sparse steps with one or two replicas are latency-bound (12-24 bytes per parameter in
+// flight per lane), so they trade registers for a fourth CTA (measured, N = 2^28, R = 2, 90 %: 2.54 -> 2.29 ms)
+__global__ void __launch_bounds__(256, ((!DENSE && R <= 2) ? 4 : R <= 4 ? 3 : 2)) scape_fused_step_kernel(const __grid_constant__ StepParams p) {
   const int lane = threadIdx.x & 31;
   const int64_t wpb = blockDim.x >> 5;
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
   const int64_t nwarps = (int64_t)gridDim.x * wpb;
   const int64_t full = p.N >> 7;
+  __shared__ float scratch[DENSE ? 1 : 8 * 2 * kChunk];     // per warp: (sum_r m~^r, m_old) of the selected entries
+  float* sc = DENSE ? scratch : scratch + (threadIdx.x >> 5) * (2 * kChunk);
   StageA sa{};
   if (!DENSE) {
     sa.lo = p.ctl->lo_key; sa.hi = p.ctl->hi_key;
     sa.seg = p.cand + (size_t)warp * p.seg_cap;
   }
-  for (int64_t c = warp; c < full; c += nwarps) fused_chunk<G, R, DENSE, MSPARSE, false>(p, c, lane, sa);
-  if (full < p.n_chunks && warp == full % nwarps) fused_chunk<G, R, DENSE, MSPARSE, true>(p, full, lane, sa);
+  for (int64_t c = warp; c < full; c += nwarps) fused_chunk<G, R, DENSE, MSPARSE, false>(p, c, lane, sc, sa);
+  if (full < p.n_chunks && warp == full % nwarps) fused_chunk<G, R, DENSE, MSPARSE, true>(p, full, lane, sc, sa);
   if (!DENSE) {
     uint32_t na = sa.n_above;
 #pragma unroll
@@ -379,7 +482,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, uint32
 }
 
 struct TmaMaskWords { uint4 cw, pw; uint32_t cr, pr; };
-struct TmaTileState { uint32_t mybits, jbase; float mo[4]; };
+struct TmaTileState { uint32_t mybits, jbase, r0, cnt; float mo[4]; };
 
 __device__ __forceinline__ void tma_load_words(const StepParams& p, int64_t c, TmaMaskWords& w) {
   w.cw = __ldg(reinterpret_cast<const uint4*>(p.cur_bits) + c); w.cr = __ldg(p.cur_rank + c);
@@ -389,6 +492,7 @@ __device__ __forceinline__ void tma_load_words(const StepParams& p, int64_t c, T
 __device__ __forceinline__ void tma_decode_gather(const StepParams& p, const TmaMaskWords& w, int lane, TmaTileState& st) {
   uint32_t pbits, pbase;
   lane_bits_from_words(w.cw, w.cr, lane, st.mybits, st.jbase);
+  st.r0 = w.cr; st.cnt = chunk_popc(w.cw);
   lane_bits_from_words(w.pw, w.pr, lane, pbits, pbase);
 #pragma unroll
   for (int q = 0; q < 4; ++q)
@@ -438,8 +542,13 @@ __device__ __forceinline__ void tma_consume_tile(const StepParams& p, int64_t ti
   }
   // Results go back into the stage (in place) and leave as whole-tile bulk stores: 4 KB bursts
   // per stream instead of 512-byte warp stores.
-  fused_compute<R, false, false, false, CLIPT>(p, c, lane, i0, cur.mybits, cur.jbase, th, cur.mo, gg, ee, sa);
+  // scratch of the on-mask arithmetic: this warp's own theta and e^0 slices of the stage (their
+  // contents are in registers now and are written back only after fused_compute)
   unsigned char* wbase = stage0 + (size_t)s * TILE;
+  __syncwarp();
+  fused_compute<R, false, false, false, CLIPT>(p, c, lane, i0, cur.mybits, cur.jbase, cur.r0, cur.cnt,
+                                               reinterpret_cast<float*>(wbase) + warp * kChunk,
+                                               reinterpret_cast<float*>(wbase + OFF_E) + warp * kChunk, th, cur.mo, gg, ee, sa);
   *reinterpret_cast<float4*>(wbase + off * 4u) = make_float4(th[0], th[1], th[2], th[3]);
 #pragma unroll
   for (int r = 0; r < R; ++r)
@@ -533,13 +642,16 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
     tile += tstride;
   }
   if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // stores have landed
+  asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumerWarps * 32) : "memory");          // ... and every consumer warp knows
 
   // chunks past the last full tile (fewer than 8, the last one possibly ragged): LDG path
   {
     const int64_t c = n_tiles * kTmaConsumerWarps + warp;
     if (c < p.n_chunks && blockIdx.x == (unsigned)(n_tiles % gridDim.x)) {
-      if (((c + 1) << 7) <= p.N) fused_chunk<G, R, false, true, false>(p, c, lane, sa);
-      else fused_chunk<G, R, false, true, true>(p, c, lane, sa);
+      // (all bulk stores of this CTA have completed: the first stage serves as scratch)
+      float* sc = reinterpret_cast<float*>(stage0) + warp * (2 * kChunk);
+      if (((c + 1) << 7) <= p.N) fused_chunk<G, R, false, true, false>(p, c, lane, sc, sa);
+      else fused_chunk<G, R, false, true, true>(p, c, lane, sc, sa);
     }
   }
   uint32_t na = sa.n_above;
