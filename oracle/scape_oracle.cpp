@@ -16,9 +16,13 @@
 //   P9 worked example tests/golden/p9_worked_example.json
 //   P10 bias correction / learning-rate schedule == independent numpy Eq. 2 + PAPER.md:77 (dense)
 //   P11 clip_grad: norm and factor vs numpy; no-op below the threshold; theta vs numpy (dense)
+//   P12 per-layer refresh vs brute force per layer; exactly k_l per layer; one layer == flat
+//   P13 an uncompressed layer is dense AdamS (Eq. 2) on its slice while the others are sparse
+//   P14 sparsity schedule: mask counts follow the schedule with the one-step delay; P6 still holds
 // Unpinned by the paper (decisions): S3 clip_grad off by default and,
 // when switched on, the torch/Megatron rule; S4 bias correction off by default; S8 replica 0 owns
-// the statistic; S9 flat (not per-layer) top-k.
+// the statistic; S9 flat top-k by default, per-layer top-k with uncompressed
+// layers (:246, :279, :286) after set_layers; S19 the density warm-up schedule (:279) is the caller's.
 //
 // The algorithm is instantiated twice from the same template: T = float is the graded
 // arithmetic (operation order pinned below);
@@ -68,6 +72,16 @@ struct Oracle {
   double last_norm = 0.0;         // ||g^||_2 of the last step and the factor applied
   T last_coef = (T)1;
 
+  // Per-layer refresh (PAPER.md:89 "per-layer style", :138 "number of layers in model L"): the
+  // shard is cut into layers [off[l], off[l+1]); refresh_mask runs inside each layer with
+  // k_l = n_l - floor(s * n_l); a layer with compress[l] == 0 is never sparsified (LayerNorm,
+  // RMSNorm, bias: PAPER.md:246, :279, :286): all its entries are selected.  Empty = one layer.
+  std::vector<int64_t> layer_off;
+  std::vector<uint8_t> layer_compress;
+  // Sparsity used by the NEXT refresh (density warm-up: "exponentially decrease
+  // density d from 1 to 0.1 or 0.01"; the schedule itself is the caller's).
+  double sparsity_now = 0.0;
+
   std::vector<T> m;                 // m_{t-1}, zero off the previous mask (Eq. 4)
   std::vector<std::vector<T>> e;    // e^r_{t-1}, one residual per replica (Alg. 1 l.2, :141)
   std::vector<uint8_t> cur;         // M_{t-1}, the mask used by the coming step (l.1: all ones)
@@ -88,6 +102,7 @@ struct Oracle {
     c2 = (T)1 - beta2;
     // Reading S6: k = N - floor(s*N) in IEEE double.
     k = N - (int64_t)std::floor(sparsity * (double)N);
+    sparsity_now = sparsity;
     m.assign(N, (T)0);                                   // reading S5: m_0 = 0
     e.assign(R, std::vector<T>(N, (T)0));                // l.2: e_0 = 0
     cur.assign(N, 1);                                    // l.1: M_0 = 1
@@ -103,6 +118,21 @@ struct Oracle {
     });
     std::vector<uint8_t> mask(n, 0);
     for (int64_t j = 0; j < kk; ++j) mask[order[j]] = 1;
+    return mask;
+  }
+
+  static int64_t k_of(int64_t n, double sparsity) { return n - (int64_t)std::floor(sparsity * (double)n); }   // S6
+
+  // l.11 with the per-layer reading: refresh_mask inside every layer, at the current sparsity.
+  std::vector<uint8_t> refresh(const T* x) const {
+    if (layer_off.empty()) return topk_mask(x, N, k_of(N, sparsity_now));
+    std::vector<uint8_t> mask(N, 0);
+    for (size_t l = 0; l + 1 < layer_off.size(); ++l) {
+      const int64_t a = layer_off[l], n = layer_off[l + 1] - a;
+      if (!layer_compress[l]) { std::fill(mask.begin() + a, mask.begin() + a + n, (uint8_t)1); continue; }
+      std::vector<uint8_t> ml = topk_mask(x + a, n, k_of(n, sparsity_now));
+      std::copy(ml.begin(), ml.end(), mask.begin() + a);
+    }
     return mask;
   }
 
@@ -132,7 +162,8 @@ struct Oracle {
 
     // l.11: M_t <- refresh_mask(density, abs(m-tilde)) from the owner's (replica 0) statistic,
     // over all N positions (readings S8, S11).  Used from the next step on (§IV-A, :178).
-    std::vector<uint8_t> next = topk_mask(mt[0].data(), N, k);
+    // With layers set: the same inside every layer.
+    std::vector<uint8_t> next = refresh(mt[0].data());
 
     // l.10, l.12-17 on the mask.
     std::vector<T> m_new(N, (T)0);                       // l.12 / Eq. 4: zero off the mask
@@ -227,6 +258,17 @@ template <class T> void copy_out(const std::vector<T>& v, T* dst) {
     auto* o = (Oracle<T>*)h; std::memcpy(o->cur.data(), src, o->N);                                 \
   }                                                                                                 \
   extern "C" void oracle_set_t_##SUF(void* h, int64_t t) { ((Oracle<T>*)h)->t = t; }                \
+  extern "C" int oracle_set_layers_##SUF(void* h, int L, const int64_t* off, const uint8_t* compress) { \
+    auto* o = (Oracle<T>*)h;                                                                        \
+    if (L < 1 || off[0] != 0 || off[L] != o->N) return -1;                                          \
+    for (int l = 0; l < L; ++l) if (off[l + 1] <= off[l]) return -1;                                \
+    o->layer_off.assign(off, off + L + 1); o->layer_compress.assign(compress, compress + L);        \
+    return 0;                                                                                       \
+  }                                                                                                 \
+  extern "C" int oracle_set_sparsity_##SUF(void* h, double s) {                                     \
+    if (!(s >= 0.0 && s < 1.0)) return -1;                                                          \
+    auto* o = (Oracle<T>*)h; o->sparsity_now = s; o->k = Oracle<T>::k_of(o->N, s); return 0;        \
+  }                                                                                                 \
   extern "C" void oracle_set_lr_##SUF(void* h, double lr) { ((Oracle<T>*)h)->lr = (T)lr; }         \
   extern "C" void oracle_set_bias_correction_##SUF(void* h, int on) { ((Oracle<T>*)h)->bias_correction = on != 0; } \
   extern "C" void oracle_set_clip_grad_##SUF(void* h, double c) { ((Oracle<T>*)h)->clip_max_norm = c; } \

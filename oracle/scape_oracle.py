@@ -68,6 +68,27 @@ class ScapeOracle:
         fn.argtypes = [ctypes.c_void_p, ctypes.c_int64]
         fn(self.h, int(t))
 
+    def set_layers(self, offsets, compress=None):
+        """Per-layer refresh: layers [offsets[l], offsets[l+1]); compress[l] == 0
+        marks a layer that is never sparsified."""
+        off = np.ascontiguousarray(offsets, dtype=np.int64)
+        L = off.size - 1
+        cp = np.ones(L, np.uint8) if compress is None else np.ascontiguousarray(compress, dtype=np.uint8)
+        assert cp.size == L
+        fn = self._f("set_layers")
+        fn.restype = ctypes.c_int
+        fn.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
+        if fn(self.h, int(L), off.ctypes.data, cp.ctypes.data) != 0:
+            raise ValueError("oracle_set_layers rejected the offsets")
+
+    def set_sparsity(self, s):
+        """Sparsity of the coming refreshes (density warm-up)."""
+        fn = self._f("set_sparsity")
+        fn.restype = ctypes.c_int
+        fn.argtypes = [ctypes.c_void_p, ctypes.c_double]
+        if fn(self.h, float(s)) != 0:
+            raise ValueError("sparsity must be in [0, 1)")
+
     def set_lr(self, lr):
         fn = self._f("set_lr")
         fn.argtypes = [ctypes.c_void_p, ctypes.c_double]

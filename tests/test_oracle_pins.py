@@ -420,3 +420,132 @@ def test_p11_clip_scales_only_the_second_moment_input_sparse():
     off = np.ones(N, bool); off[a.idx()] = False
     np.testing.assert_array_equal(tha[off], thb[off])
     assert not np.array_equal(tha[~off], thb[~off])
+
+
+# ------------------------------------------------------------------------------------ P12
+def layered_brute_force(x, offsets, compress, s):
+    """Per-layer refresh written from the definition: inside each compressed layer the
+    k_l = n_l - floor(s n_l) entries of largest |x| (ties to the lower index), every entry of an
+    uncompressed layer."""
+    mask = np.zeros(len(x), np.uint8)
+    for l in range(len(offsets) - 1):
+        a, b = offsets[l], offsets[l + 1]
+        if not compress[l]:
+            mask[a:b] = 1
+        else:
+            n = b - a
+            mask[a:b] = brute_force_topk(x[a:b], n - int(np.floor(s * n)))
+    return mask
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_p12_per_layer_refresh_vs_brute_force(seed):
+    rng = np.random.default_rng(100 + seed)
+    N, R = 300, 2
+    cuts = np.sort(rng.choice(np.arange(1, N), size=5, replace=False))
+    offsets = np.concatenate([[0], cuts, [N]])
+    compress = np.array([1, 1, 0, 1, 1, 1], np.uint8)
+    s = [0.9, 0.5, 0.75, 0.99][seed]
+    o = ScapeOracle(N, R, s, **HYP)
+    o.set_layers(offsets, compress)
+    th = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    scale = np.repeat(10.0 ** rng.uniform(-3, 0, 6), np.diff(offsets)).astype(np.float32)
+    for g in make_grads(rng, N, R, 4):
+        g = [x * scale for x in g]
+        if seed == 0:                      # ties inside and across layers
+            g = [np.round(x * 2e3) / 2e3 for x in g]
+        o.step(th, g)
+        mk = o.mask()
+        np.testing.assert_array_equal(mk, layered_brute_force(o.mt(0), offsets, compress, s))
+        for l in range(6):                 # exactly k_l per layer
+            n = offsets[l + 1] - offsets[l]
+            want = n if not compress[l] else n - int(np.floor(s * n))
+            assert mk[offsets[l]:offsets[l + 1]].sum() == want
+
+
+def test_p12_one_layer_is_the_flat_refresh_and_layers_differ_from_flat():
+    rng = np.random.default_rng(12)
+    N, R, T = 2000, 2, 5
+    grads = make_grads(rng, N, R, T)
+    th0 = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    flat = ScapeOracle(N, R, 0.9, **HYP)
+    one = ScapeOracle(N, R, 0.9, **HYP)
+    one.set_layers([0, N])
+    two = ScapeOracle(N, R, 0.9, **HYP)
+    two.set_layers([0, 700, N])
+    tha, thb, thc = th0.copy(), th0.copy(), th0.copy()
+    scale = np.where(np.arange(N) < 700, 1.0, 30.0).astype(np.float32)   # a flat top-k would starve layer 0
+    for g in grads:
+        g = [x * scale for x in g]
+        flat.step(tha, g); one.step(thb, g); two.step(thc, g)
+        np.testing.assert_array_equal(flat.mask(), one.mask())
+        assert np.array_equal(tha.view(np.uint32), thb.view(np.uint32))
+        assert two.mask()[:700].sum() == 70 and two.mask()[700:].sum() == 130
+    assert flat.mask()[:700].sum() < 70
+
+
+def test_set_layers_rejects_bad_offsets():
+    o = ScapeOracle(100, 1, 0.5, **HYP)
+    for bad in ([0, 50], [1, 100], [0, 50, 50, 100], [0, 60, 40, 100]):
+        with pytest.raises(ValueError):
+            o.set_layers(bad)
+    with pytest.raises(ValueError):
+        o.set_sparsity(1.0)
+
+
+# ------------------------------------------------------------------------------------ P13
+def test_p13_uncompressed_layer_is_dense_adams_on_its_slice_double():
+    """A layer that is not sparsified stays in every mask, so on its slice
+    e = 0 and the step is Eq. 2 with the replica-mean gradient."""
+    rng = np.random.default_rng(13)
+    N, R, T = 1200, 3, 7
+    a, b = 500, 640
+    o = ScapeOracle(N, R, 0.95, dtype=np.float64, **HYP)
+    o.set_layers([0, a, b, N], [1, 0, 1])
+    th = 0.02 * rng.standard_normal(N)
+    th_ref, m_ref = th[a:b].copy(), np.zeros(b - a)
+    for g in make_grads(rng, N, R, T, dtype=np.float64):
+        o.step(th, g)
+        gbar = sum(x[a:b] for x in g) / R
+        th_ref, m_ref = dense_adams_f64(th_ref, m_ref, gbar, **HYP)
+        assert o.mask()[a:b].all()
+        for r in range(R):
+            assert not o.e(r)[a:b].any()
+        np.testing.assert_allclose(o.m()[a:b], m_ref, rtol=1e-12, atol=1e-300)
+        np.testing.assert_allclose(th[a:b], th_ref, rtol=1e-12, atol=1e-300)
+    # the sparsified layers hold exactly their k_l
+    assert o.mask()[:a].sum() == a - int(np.floor(0.95 * a))
+    assert o.mask()[b:].sum() == (N - b) - int(np.floor(0.95 * (N - b)))
+
+
+# ------------------------------------------------------------------------------------ P14
+def warmup_density(t, d_final, T_w):
+    """Exponential density warm-up 1 -> d_final over T_w steps (PAPER.md:279 gives the shape only)."""
+    return max(d_final, d_final ** (t / T_w))
+
+
+def test_p14_sparsity_schedule_counts_delay_and_conservation_double():
+    rng = np.random.default_rng(14)
+    N, R, T = 1000, 2, 12
+    offsets, compress = [0, 300, 364, N], [1, 0, 1]
+    o = ScapeOracle(N, R, 0.0, dtype=np.float64, **HYP)
+    o.set_layers(offsets, compress)
+    th = 0.02 * rng.standard_normal(N)
+    c1 = 1 - HYP["beta1"]
+    sum_g, sum_m_before = np.zeros(N), np.zeros(N)
+    want_prev = N                                   # M_0 = 1
+    for t, g in enumerate(make_grads(rng, N, R, T, dtype=np.float64), start=1):
+        s = 1.0 - warmup_density(t, 0.05, 8)
+        o.set_sparsity(s)                           # used by this step's refresh (M_t)
+        sum_m_before += o.m()
+        o.step(th, g)
+        assert o.K_last == want_prev                # the step used the mask made one step earlier
+        want_prev = sum((b - a) if not c else (b - a) - int(np.floor(s * (b - a)))
+                        for a, b, c in zip(offsets[:-1], offsets[1:], compress))
+        assert o.mask().sum() == want_prev
+        np.testing.assert_array_equal(o.mask(), layered_brute_force(o.mt(0), offsets, compress, s))
+        # P6 under a changing mask size: nothing is lost
+        sum_g += sum(g) / R
+        ebar = sum(o.e(r) for r in range(R)) / R
+        np.testing.assert_allclose(c1 * sum_g, ebar + o.m() + c1 * sum_m_before, rtol=1e-10, atol=1e-14)
+    assert want_prev == 15 + 64 + 32               # 5 % of 300 and of 636, all 64 of the uncompressed layer
