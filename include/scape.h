@@ -127,6 +127,31 @@ int scape_set_bias_correction(scape_t* h, int on);
 int scape_set_clip_grad(scape_t* h, double max_norm);
 int scape_last_grad_norm(scape_t* h, double* norm, double* coef, void* cuda_stream);
 
+/* Per-layer refresh and density warm-up (readings S9, S19).
+ *   scape_set_layers    PAPER.md:89 ("the top-k sparsification is performed in a per-layer style"),
+ *                       :138 ("number of layers in model L"): cut the shard into n_layers layers
+ *                       [offsets[l], offsets[l+1]) (HOST array of n_layers+1 entries, offsets[0] = 0,
+ *                       offsets[n_layers] = shard_numel, strictly increasing; any alignment) and run
+ *                       refresh_mask (l.11) inside every layer: k_l = n_l - floor(sparsity * n_l)
+ *                       entries of largest |m~^0|, ties to the lower index.  compress (HOST array of
+ *                       n_layers bytes, or NULL = all ones): compress[l] == 0 marks a layer that is
+ *                       never sparsified (LayerNorm, RMSNorm, bias: PAPER.md:246, :279, :286): all
+ *                       its entries stay selected, so it takes dense AdamS steps.  Takes effect with
+ *                       the next step's refresh; masks already made stay as they are.  n_layers = 0
+ *                       returns to one flat top-k.  At most SCAPE_MAX_LAYERS layers.  Synchronises
+ *                       the device; allocates 32 KB per layer + 4 bytes per 128 parameters.
+ *   scape_set_sparsity  sparsity of the following refreshes (density warm-up: "we use
+ *                       sparsity warmup to exponentially decrease density d from 1 to 0.1 or 0.01";
+ *                       the schedule is the caller's).  The mask made by step t at sparsity s_t is
+ *                       used by step t+1.  Grows the packed buffers when the new masks are larger
+ *                       than any before (then it synchronises the device); never shrinks them.
+ *   scape_layer_k       k_l of a layer at the current sparsity (layer 0 = the whole shard when no
+ *                       layers are set); scape_k is their sum.                                       */
+#define SCAPE_MAX_LAYERS 4096
+int scape_set_layers(scape_t* h, int n_layers, const int64_t* offsets, const uint8_t* compress);
+int scape_set_sparsity(scape_t* h, double sparsity);
+int64_t scape_layer_k(const scape_t* h, int layer);
+
 /* Option: also materialise b^r on steps whose mask is all ones (step 1, or sparsity 0), where
  * the packed buffer would be R*N floats.  Off by default: on such steps SCAPE_PACKED is then
  * unavailable (SCAPE_EINVAL) and SCAPE_PACKED_MEAN equals SCAPE_MOMENT.  Allocates R*N floats
@@ -137,7 +162,8 @@ int scape_set_keep_dense_pack(scape_t* h, int on);
  * may be a host or a device pointer (unified addressing); `bytes` must equal the size of the
  * selected object; `r` is the replica for SCAPE_RESIDUAL / SCAPE_PACKED and ignored otherwise.
  * Both calls synchronise `cuda_stream` before returning.  Not part of the timed path.
- * scape_set(SCAPE_MASK_NEXT) accepts a mask with at most k set bits, or with all N bits set;
+ * scape_set(SCAPE_MASK_NEXT) accepts a mask with at most as many set bits as the largest mask so
+ * far (scape_k at creation, grown by scape_set_sparsity / scape_set_layers), or with all N bits set;
  * bits at positions >= N are ignored.                                                          */
 int scape_get(scape_t* h, int what, int r, void* buf, size_t bytes, void* cuda_stream);
 int scape_set(scape_t* h, int what, int r, const void* buf, size_t bytes, void* cuda_stream);
@@ -146,7 +172,8 @@ int scape_set_step_count(scape_t* h, int64_t t);
 /* How often the stage-2 select could use the candidate list gathered by the fused pass (the
  * threshold predicted from the previous step bracketed the true one: `fast`) and how often it
  * fell back to radix passes over the whole partition (`general`; always the case on all-ones
- * steps).  Both routes are exact.  Synchronises cuda_stream.                                     */
+ * steps).  With layers set the counts are per layer and step.  Both routes are exact.
+ * Synchronises cuda_stream.                                     */
 int scape_select_stats(scape_t* h, int64_t* fast, int64_t* general, void* cuda_stream);
 
 /* Diagnostics of the last step's select (not graded): out8 = {bracket held (0/1), entries above

@@ -37,6 +37,9 @@ SYMBOLS = {
     "scape_set_bias_correction": (_I, [_VP, _I]),
     "scape_set_clip_grad": (_I, [_VP, _D]),
     "scape_last_grad_norm": (_I, [_VP, _VP, _VP, _VP]),
+    "scape_set_layers": (_I, [_VP, _I, _VP, _VP]),
+    "scape_set_sparsity": (_I, [_VP, _D]),
+    "scape_layer_k": (_I64, [_VP, _I]),
     "scape_get": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
     "scape_set": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
     "scape_set_step_count": (_I, [_VP, _I64]),
@@ -148,6 +151,25 @@ def scape_last_grad_norm(h, stream=0):
     a, b = ctypes.c_double(), ctypes.c_double()
     _check(lib().scape_last_grad_norm(h, ctypes.byref(a), ctypes.byref(b), stream), "scape_last_grad_norm")
     return a.value, b.value
+
+
+def scape_set_layers(h, offsets, compress=None):
+    """offsets: n_layers+1 ints (0 ... shard_numel); compress: n_layers flags or None (all compressed)."""
+    n = len(offsets) - 1
+    off = (ctypes.c_int64 * (n + 1))(*[int(x) for x in offsets])
+    cp = None if compress is None else (ctypes.c_uint8 * n)(*[int(bool(x)) for x in compress])
+    _check(lib().scape_set_layers(h, n, off, cp), "scape_set_layers")
+
+
+def scape_set_sparsity(h, sparsity):
+    _check(lib().scape_set_sparsity(h, float(sparsity)), "scape_set_sparsity")
+
+
+def scape_layer_k(h, layer):
+    n = int(lib().scape_layer_k(h, int(layer)))
+    if n < 0:
+        raise ScapeError(f"scape_layer_k failed ({n}): {scape_last_error()}")
+    return n
 
 
 def scape_set_step_count(h, t):
@@ -313,6 +335,18 @@ class Scape:
 
     def set_step_count(self, t):
         scape_set_step_count(self.h, t)
+
+    def set_layers(self, offsets, compress=None):
+        scape_set_layers(self.h, offsets, compress)
+
+    def clear_layers(self):
+        _check(lib().scape_set_layers(self.h, 0, None, None), "scape_set_layers")
+
+    def set_sparsity(self, sparsity):
+        scape_set_sparsity(self.h, sparsity)
+
+    def layer_k(self, layer):
+        return scape_layer_k(self.h, layer)
 
     def set_lr(self, lr):
         scape_set_lr(self.h, lr)

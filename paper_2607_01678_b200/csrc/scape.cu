@@ -3,12 +3,14 @@
 // No CPU fallback exists: every stage runs in the kernels of scape_kernels.cuh.
 #include "../../include/scape.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "scape_kernels.cuh"
 
@@ -98,6 +100,18 @@ struct scape {
   int n_seg = 0;                  // segments (= warps) of the last fused launch
   int n_slots = 0;                // warps of the last streaming launch (clip-mode partial sums)
   uint32_t seg_cap = 0;
+
+  // per-layer refresh (scape_set_layers) and per-step sparsity (scape_set_sparsity)
+  double sparsity = 0.0;          // sparsity of the coming refreshes
+  int n_layers = 0;               // 0 = one flat top-k over the shard
+  std::vector<int64_t> lay_off;   // host copy [n_layers + 1]
+  std::vector<uint8_t> lay_compress;
+  LayerState* layers = nullptr;   // [n_layers]
+  LayerCtl* lctl = nullptr;
+  uint32_t* chunk_layer = nullptr;   // [n_chunks]
+  uint32_t* lhist = nullptr;      // [n_layers][kBins]
+  int4* items = nullptr;
+  int n_items = 0;
 
   // optional per-step CUDA-event timing of the fused kernel and of the select stage
   bool prof_on = false;
@@ -300,6 +314,103 @@ int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general,
   return SCAPE_OK;
 }
 
+// Storage whose size follows the number of selected entries: index lists, packed b^r, the two
+// packed means, the candidate list.  Grows (never shrinks) so that masks of up to K entries fit;
+// live contents are kept.  Synchronises the device when it has to reallocate.  Masks with all N
+// bits set need none of it.
+int ensure_capacity(scape* h, int64_t K) {
+  if (K >= h->N) return SCAPE_OK;
+  const int64_t stride = (K + 31) / 32 * 32;
+  if (stride > h->packed_stride) {
+    CU_TRY(cudaDeviceSynchronize());
+    const int64_t old = h->packed_stride;
+    auto grow = [&](void** p, size_t elem, int64_t rows) -> bool {
+      void* q = nullptr;
+      if (cudaMalloc(&q, elem * (size_t)stride * rows) != cudaSuccess) { cudaGetLastError(); return false; }
+      if (cudaMemset(q, 0, elem * (size_t)stride * rows) != cudaSuccess) { cudaFree(q); return false; }
+      if (*p && old > 0)
+        for (int64_t r = 0; r < rows; ++r)
+          if (cudaMemcpy((char*)q + elem * (size_t)stride * r, (char*)*p + elem * (size_t)old * r, elem * (size_t)old,
+                         cudaMemcpyDeviceToDevice) != cudaSuccess) { cudaFree(q); return false; }
+      cudaFree(*p);
+      *p = q;
+      return true;
+    };
+    bool ok = true;
+    for (auto& s : h->slot) ok = ok && grow((void**)&s.idx, sizeof(int32_t), 1);
+    ok = ok && grow((void**)&h->pm[0], sizeof(float), 1) && grow((void**)&h->pm[1], sizeof(float), 1);
+    ok = ok && grow((void**)&h->packed, sizeof(float), h->R);
+    if (!ok) return fail(SCAPE_ENOMEM, "device allocation failed (packed buffers for %lld selected entries)", (long long)K);
+    h->packed_stride = stride;
+  }
+  if (!h->cand) {
+    // candidates of the fused select: room for 4k keys (a bracket of +-3 % around the threshold
+    // holds ~0.8k: error feedback piles residuals up just below it), at least N/8, at most N/2
+    int64_t cc = 4 * K;
+    if (cc < h->N / 8) cc = h->N / 8;      // very sparse masks / transients: keep room per warp segment
+    if (cc > h->N / 2) cc = h->N / 2;
+    if (cc < 65536) cc = 65536;
+    if (cudaMalloc((void**)&h->cand, sizeof(unsigned long long) * (size_t)cc) != cudaSuccess ||
+        cudaMalloc((void**)&h->cls, sizeof(unsigned long long) * (size_t)kClsCap) != cudaSuccess) {
+      cudaGetLastError();
+      cudaFree(h->cand); h->cand = nullptr;
+      return fail(SCAPE_ENOMEM, "device allocation failed (candidate list)");
+    }
+    h->cand_cap = cc;
+  }
+  return SCAPE_OK;
+}
+
+// entries the refresh selects at sparsity s: reading S6, inside every layer when layers are set
+int64_t total_k(const scape* h, double s) {
+  if (h->n_layers == 0) return h->N - (int64_t)std::floor(s * (double)h->N);
+  int64_t K = 0;
+  for (int l = 0; l < h->n_layers; ++l) {
+    const int64_t n = h->lay_off[l + 1] - h->lay_off[l];
+    K += h->lay_compress[l] ? n - (int64_t)std::floor(s * (double)n) : n;
+  }
+  return K;
+}
+
+// Stage 2 with layers: the same exact select inside every layer at once.
+int run_select_layered(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st) {
+  KeySrc src;
+  src.e0 = h->e;
+  src.cur_bits = cur.all_ones ? nullptr : cur.bits;
+  src.cur_rank = cur.all_ones ? nullptr : cur.rank;
+  src.packed0 = h->packed;
+  src.N = h->N;
+  src.n_chunks = h->n_chunks;
+  CandList cl;
+  cl.cls = h->cls; cl.cand = h->cand; cl.seg_count = h->seg_count; cl.seg_above = h->seg_above;
+  cl.seg_cap = h->seg_cap; cl.n_seg = force_general ? 0 : h->n_seg;
+  LayerWork w;
+  w.chunk_layer = h->chunk_layer; w.layers = h->layers; w.n_layers = h->n_layers; w.ctl = h->lctl;
+  w.hist = h->lhist; w.items = h->items; w.n_items = h->n_items;
+  const int grid_c = h->n_sm * 2;
+  int grid_f = h->n_sm * 6; if (grid_f > h->n_items) grid_f = h->n_items;
+  lsel_decide_kernel<<<1, 1024, 0, st>>>(w, cl, h->sparsity, force_general ? 1 : 0);
+  h->launches++;
+  // 5 digits at most, plus one round for layers whose bracket turns out (first pick) to have
+  // missed and that restart on the general route; kernels with nothing to do return at once
+  for (int round = 0; round < kSelPasses + 1; ++round) {
+    if (!force_general) { lsel_hist_cand_kernel<<<grid_c, 256, 0, st>>>(w, cl); h->launches++; }
+    lsel_hist_full_kernel<<<grid_f, 256, 0, st>>>(src, w);
+    lsel_pick_kernel<<<h->n_layers, 1024, 0, st>>>(w);
+    h->launches += 2;
+  }
+  lsel_finish_full_kernel<<<grid_f, 256, 0, st>>>(src, w, nxt.bits);
+  h->launches++;
+  if (!force_general) { lsel_finish_cand_kernel<<<grid_c, 256, 0, st>>>(w, cl, nxt.bits); h->launches++; }
+  CU_TRY(cudaGetLastError());
+  int rc = compact_mask(h, nxt, true, st);
+  if (rc) return rc;
+  nxt.count = h->k;
+  nxt.all_ones = false;
+  nxt.valid = true;
+  return SCAPE_OK;
+}
+
 // fold the recorded event pairs into the running totals (synchronises on the events)
 int prof_drain(scape* h) {
   for (int i = 0; i < h->prof_pending; ++i) {
@@ -324,6 +435,7 @@ void free_all(scape* h) {
   cudaFree(h->packed); cudaFree(h->pm[0]); cudaFree(h->pm[1]); cudaFree(h->dense_pack);
   cudaFree(h->sel); cudaFree(h->cand); cudaFree(h->cls); cudaFree(h->seg_count); cudaFree(h->seg_above); cudaFree(h->ghist); cudaFree(h->block_sum); cudaFree(h->total);
   cudaFree(h->ghat); cudaFree(h->vm); cudaFree(h->sumsq); cudaFree(h->clip_state);
+  cudaFree(h->layers); cudaFree(h->lctl); cudaFree(h->chunk_layer); cudaFree(h->lhist); cudaFree(h->items);
   cudaFree(h->st_param);
   for (auto& g : h->st_grad) cudaFree(g);
   if (h->prof_have_events)
@@ -362,8 +474,8 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   h->c1 = 1.0f - h->b1; h->c2 = 1.0f - h->b2;
   h->beta1_d = beta1; h->beta2_d = beta2;
   h->n_compact_blocks = (int)((h->n_chunks + kCompactChunksPerBlock - 1) / kCompactChunksPerBlock);
-  const bool sparse = h->k < N;
-  h->packed_stride = sparse ? (h->k + 31) / 32 * 32 : 0;
+  h->sparsity = sparsity;
+  h->max_seg = h->n_sm * 8 * 8;
 
   bool ok = true;
   auto alloc = [&](void** p, size_t bytes, bool zero) {
@@ -376,28 +488,11 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   for (auto& s : h->slot) {
     alloc((void**)&s.bits, sizeof(uint32_t) * h->n_words, true);
     alloc((void**)&s.rank, sizeof(uint32_t) * h->n_chunks, true);
-    if (sparse) alloc((void**)&s.idx, sizeof(int32_t) * h->packed_stride, true);
-  }
-  if (sparse) {
-    alloc((void**)&h->packed, sizeof(float) * h->packed_stride * R, true);
-    alloc((void**)&h->pm[0], sizeof(float) * h->packed_stride, true);
-    alloc((void**)&h->pm[1], sizeof(float) * h->packed_stride, true);
   }
   alloc((void**)&h->sel, sizeof(SelState), true);
-  if (sparse) {
-    // candidates of the fused select: room for 4k keys (a bracket of +-3 % around the threshold
-    // holds ~0.8k: error feedback piles residuals up just below it), at least N/8, at most N/2
-    int64_t cc = 4 * h->k;
-    if (cc < N / 8) cc = N / 8;            // very sparse masks / transients: keep room per warp segment
-    if (cc > N / 2) cc = N / 2;
-    if (cc < 65536) cc = 65536;
-    h->cand_cap = cc;
-    h->max_seg = h->n_sm * 8 * 8;
-    alloc((void**)&h->cand, sizeof(unsigned long long) * (size_t)cc, false);
-    alloc((void**)&h->cls, sizeof(unsigned long long) * (size_t)kClsCap, false);
-    alloc((void**)&h->seg_count, sizeof(uint32_t) * h->max_seg, true);
-    alloc((void**)&h->seg_above, sizeof(uint32_t) * h->max_seg, true);
-  }
+  alloc((void**)&h->seg_count, sizeof(uint32_t) * h->max_seg, true);
+  alloc((void**)&h->seg_above, sizeof(uint32_t) * h->max_seg, true);
+  if (ok && ensure_capacity(h, h->k) != SCAPE_OK) ok = false;                // index lists, packed buffers, candidates
   alloc((void**)&h->ghist, sizeof(uint32_t) * kBins, true);
   alloc((void**)&h->block_sum, sizeof(uint32_t) * (h->n_compact_blocks + 1), true);
   alloc((void**)&h->total, sizeof(uint32_t), true);
@@ -407,8 +502,8 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   }
   {
     SelState init{};
-    init.delta = 0.5f;                     // no history yet: wide first bracket
-    init.lo_key = init.hi_key = 0xFFFFFFFFu;   // nothing predicted: the first sparse step decides "general"
+    init.br.delta = 0.5f;                     // no history yet: wide first bracket
+    init.br.lo_key = init.br.hi_key = 0xFFFFFFFFu;   // nothing predicted: the first sparse step decides "general"
     if (cudaMemcpy(h->sel, &init, sizeof init, cudaMemcpyHostToDevice) != cudaSuccess) {
       fail(SCAPE_ECUDA, "create: cannot initialise the select state");
       free_all(h); delete h; return nullptr;
@@ -505,6 +600,96 @@ extern "C" int scape_set_clip_grad(scape_t* h, double max_norm) {
   return SCAPE_OK;
 }
 
+extern "C" int scape_set_sparsity(scape_t* h, double sparsity) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (!(sparsity >= 0.0 && sparsity < 1.0)) return fail(SCAPE_EINVAL, "sparsity must be in [0, 1)");
+  DeviceGuard g(h->dev);
+  const int64_t K = total_k(h, sparsity);
+  int rc = ensure_capacity(h, K);
+  if (rc) return rc;
+  h->sparsity = sparsity;
+  h->k = K;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_set_layers(scape_t* h, int n_layers, const int64_t* offsets, const uint8_t* compress) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  DeviceGuard g(h->dev);
+  CU_TRY(cudaDeviceSynchronize());
+  if (n_layers == 0) {                       // back to one flat top-k
+    h->n_layers = 0; h->lay_off.clear(); h->lay_compress.clear();
+    h->k = total_k(h, h->sparsity);
+    return ensure_capacity(h, h->k);
+  }
+  if (n_layers < 0 || n_layers > SCAPE_MAX_LAYERS) return fail(SCAPE_EINVAL, "n_layers must be in [0, %d]", SCAPE_MAX_LAYERS);
+  if (!offsets) return fail(SCAPE_EINVAL, "NULL offsets");
+  if (offsets[0] != 0 || offsets[n_layers] != h->N) return fail(SCAPE_EINVAL, "offsets must run from 0 to shard_numel");
+  for (int l = 0; l < n_layers; ++l)
+    if (offsets[l + 1] <= offsets[l]) return fail(SCAPE_EINVAL, "offsets must be strictly increasing (layer %d is empty)", l);
+
+  // host tables: layer of every chunk's first entry (bit 31: the chunk holds several layers), and
+  // work items of at most kItemChunks chunks that never cross a layer boundary
+  std::vector<uint32_t> cl((size_t)h->n_chunks);
+  std::vector<int4> items;
+  std::vector<LayerState> ls((size_t)n_layers);
+  {
+    int l = 0;
+    for (int64_t c = 0; c < h->n_chunks; ++c) {
+      const int64_t a = c * kChunk, b = std::min<int64_t>(a + kChunk, h->N);
+      while (offsets[l + 1] <= a) ++l;
+      cl[(size_t)c] = (uint32_t)l | (offsets[l + 1] < b ? 0x80000000u : 0u);
+    }
+  }
+  for (int l = 0; l < n_layers; ++l) {
+    LayerState& S = ls[(size_t)l];
+    std::memset(&S, 0, sizeof S);
+    S.begin = offsets[l]; S.end = offsets[l + 1];
+    S.compress = compress ? (compress[l] != 0) : 1;
+    S.br.delta = 0.5f;
+    // nothing predicted yet for a compressed layer; every key of an uncompressed one is "above"
+    S.br.lo_key = S.br.hi_key = S.compress ? 0xFFFFFFFFu : 0u;
+    const int64_t c0 = S.begin / kChunk, c1 = (S.end + kChunk - 1) / kChunk;
+    for (int64_t c = c0; c < c1; c += kItemChunks)
+      items.push_back(make_int4(l, (int)c, (int)std::min<int64_t>(c + kItemChunks, c1), 0));
+  }
+  cudaFree(h->layers); cudaFree(h->lctl); cudaFree(h->chunk_layer); cudaFree(h->lhist); cudaFree(h->items);
+  h->layers = nullptr; h->lctl = nullptr; h->chunk_layer = nullptr; h->lhist = nullptr; h->items = nullptr;
+  h->n_layers = 0;
+  bool ok = cudaMalloc((void**)&h->layers, sizeof(LayerState) * ls.size()) == cudaSuccess &&
+            cudaMalloc((void**)&h->lctl, sizeof(LayerCtl)) == cudaSuccess &&
+            cudaMalloc((void**)&h->chunk_layer, sizeof(uint32_t) * cl.size()) == cudaSuccess &&
+            cudaMalloc((void**)&h->lhist, sizeof(uint32_t) * (size_t)kBins * ls.size()) == cudaSuccess &&
+            cudaMalloc((void**)&h->items, sizeof(int4) * items.size()) == cudaSuccess;
+  ok = ok && cudaMemcpy(h->layers, ls.data(), sizeof(LayerState) * ls.size(), cudaMemcpyHostToDevice) == cudaSuccess &&
+       cudaMemset(h->lctl, 0, sizeof(LayerCtl)) == cudaSuccess &&
+       cudaMemcpy(h->chunk_layer, cl.data(), sizeof(uint32_t) * cl.size(), cudaMemcpyHostToDevice) == cudaSuccess &&
+       cudaMemset(h->lhist, 0, sizeof(uint32_t) * (size_t)kBins * ls.size()) == cudaSuccess &&
+       cudaMemcpy(h->items, items.data(), sizeof(int4) * items.size(), cudaMemcpyHostToDevice) == cudaSuccess;
+  if (!ok) {
+    cudaGetLastError();
+    cudaFree(h->layers); cudaFree(h->lctl); cudaFree(h->chunk_layer); cudaFree(h->lhist); cudaFree(h->items);
+    h->layers = nullptr; h->lctl = nullptr; h->chunk_layer = nullptr; h->lhist = nullptr; h->items = nullptr;
+    h->lay_off.clear(); h->lay_compress.clear();
+    h->k = total_k(h, h->sparsity);
+    return fail(SCAPE_ENOMEM, "set_layers: device allocation failed");
+  }
+  h->n_layers = n_layers;
+  h->n_items = (int)items.size();
+  h->lay_off.assign(offsets, offsets + n_layers + 1);
+  h->lay_compress.resize((size_t)n_layers);
+  for (int l = 0; l < n_layers; ++l) h->lay_compress[(size_t)l] = ls[(size_t)l].compress ? 1 : 0;
+  h->k = total_k(h, h->sparsity);
+  return ensure_capacity(h, h->k);
+}
+
+extern "C" int64_t scape_layer_k(const scape_t* h, int layer) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (h->n_layers == 0) return layer == 0 ? h->k : fail(SCAPE_EINVAL, "no layers are set");
+  if (layer < 0 || layer >= h->n_layers) return fail(SCAPE_EINVAL, "layer %d out of range", layer);
+  const int64_t n = h->lay_off[layer + 1] - h->lay_off[layer];
+  return h->lay_compress[layer] ? n - (int64_t)std::floor(h->sparsity * (double)n) : n;
+}
+
 extern "C" int scape_last_grad_norm(scape_t* h, double* norm, double* coef, void* cuda_stream) {
   if (!h) return fail(SCAPE_EINVAL, "NULL handle");
   if (!h->clip_state) return fail(SCAPE_EINVAL, "clip_grad has never been switched on");
@@ -573,6 +758,7 @@ extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, vo
   p.clip = clip ? 1 : 0; p.ghat = h->ghat; p.vm = h->vm; p.sumsq = h->sumsq;
   p.ctl = h->sel; p.next_bits = nxt.bits; p.cand = h->cand;
   p.seg_count = h->seg_count; p.seg_above = h->seg_above;
+  if (h->n_layers > 0) { p.chunk_layer = h->chunk_layer; p.layers = h->layers; }
 
   const bool prof = h->prof_on;
   if (prof && h->prof_pending == scape::kProfRing) { int prc = prof_drain(h); if (prc) return prc; }
@@ -593,7 +779,8 @@ extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, vo
   if (prof) CU_TRY(cudaEventRecord(h->prof_ev[pi][1], st));
 
   if (need_select) {
-    rc = run_select(h, cur, nxt, /*force_general=*/cur.all_ones, st);
+    rc = h->n_layers > 0 ? run_select_layered(h, cur, nxt, /*force_general=*/cur.all_ones, st)
+                         : run_select(h, cur, nxt, /*force_general=*/cur.all_ones, st);
     if (rc) return rc;
     if (cur.all_ones) CU_TRY(cudaMemsetAsync(h->e, 0, sizeof(float) * h->Npad, st));   // l.8 for e^0 after the stash
   } else {
@@ -611,10 +798,12 @@ extern "C" int scape_select_stats(scape_t* h, int64_t* fast, int64_t* general, v
   if (!h) return fail(SCAPE_EINVAL, "NULL handle");
   DeviceGuard guard(h->dev);
   SelState s{};
+  LayerCtl lc{};
   CU_TRY(cudaMemcpyAsync(&s, h->sel, sizeof s, cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
+  if (h->lctl) CU_TRY(cudaMemcpyAsync(&lc, h->lctl, sizeof lc, cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
   CU_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
-  if (fast) *fast = (int64_t)s.n_fast;
-  if (general) *general = (int64_t)s.n_general;
+  if (fast) *fast = (int64_t)(s.n_fast + lc.n_fast);
+  if (general) *general = (int64_t)(s.n_general + lc.n_general);
   return SCAPE_OK;
 }
 
@@ -624,8 +813,8 @@ extern "C" int scape_select_debug(scape_t* h, double* out8, void* cuda_stream) {
   SelState s{};
   CU_TRY(cudaMemcpyAsync(&s, h->sel, sizeof s, cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
   CU_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
-  out8[0] = s.hit; out8[1] = (double)s.n_above; out8[2] = (double)s.n_cand; out8[3] = s.delta;
-  out8[4] = s.lnT_prev; out8[5] = s.ln_pred; out8[6] = (double)s.cand_cap_total; out8[7] = (double)h->n_seg;
+  out8[0] = s.hit; out8[1] = (double)s.n_above; out8[2] = (double)s.n_cand; out8[3] = s.br.delta;
+  out8[4] = s.br.lnT_prev; out8[5] = s.br.ln_pred; out8[6] = (double)s.cand_cap_total; out8[7] = (double)h->n_seg;
   return SCAPE_OK;
 }
 
@@ -806,12 +995,12 @@ extern "C" int scape_set(scape_t* h, int what, int r, const void* buf, size_t by
       CU_TRY(cudaStreamSynchronize(st));
       if ((int64_t)total == h->N) {
         s.all_ones = true; s.count = h->N; s.valid = true;
-      } else if ((int64_t)total <= h->k && h->k < h->N) {
+      } else if ((int64_t)total <= h->packed_stride) {
         s.all_ones = false; s.count = total; s.valid = true;
         if ((rc = compact_mask(h, s, true, st))) return rc;
       } else {
         s.all_ones = true; s.count = h->N; s.valid = true;   // fall back to a defined state
-        return fail(SCAPE_EINVAL, "mask: %u bits set, at most k = %lld (or all N) allowed", total, (long long)h->k);
+        return fail(SCAPE_EINVAL, "mask: %u bits set, at most %lld (the packed capacity) or all N allowed", total, (long long)h->packed_stride);
       }
       break;
     }

@@ -23,6 +23,18 @@ constexpr int kDigitBits = 13;       // radix-select digit width
 constexpr int kBins = 1 << kDigitBits;
 constexpr int kSelPasses = 5;        // 64-bit composite key = 13+13+13+13+12 bits
 
+// Predicted threshold bracket of one top-k problem (the flat partition, or one layer): in the coming
+// step's fused pass key >= hi_key is certainly selected, lo_key <= key < hi_key is a candidate,
+// key < lo_key is certainly not selected.  lo_key = hi_key = 0xFFFFFFFF: nothing predicted.
+struct Bracket {
+  uint32_t lo_key, hi_key;
+  float delta;                // half-width of the bracket in ln(threshold)
+  float lnT_prev;             // ln of the last exact threshold |m~| value
+  float ln_pred;              // ln of the threshold that was predicted for the current step
+  float r_prev;               // previous step-to-step change of ln(threshold)
+  int have_T;                 // number of exact thresholds seen (saturates at 2)
+};
+
 // Device-resident control block of the stage-2 select (never read by the host on the timed path).
 struct SelState {
   unsigned long long prefix;  // digits of T64 fixed so far
@@ -33,18 +45,35 @@ struct SelState {
   unsigned long long class_count;   // keys in the class chosen by the last pick
   unsigned int cls_n;         // entries in the small list
   unsigned int pad1;
-  // predicted bracket for the COMING step's fused pass: key >= hi_key is certainly selected,
-  // lo_key <= key < hi_key is a candidate, key < lo_key is certainly not selected
-  uint32_t lo_key, hi_key;
-  float delta;                // half-width of the bracket in ln(threshold)
-  float lnT_prev;             // ln of the last exact threshold |m~| value
-  float ln_pred;              // ln of the threshold that was predicted for the current step
-  float r_prev;               // previous step-to-step change of ln(threshold)
-  int have_T;                 // number of exact thresholds seen (saturates at 2)
+  Bracket br;                 // predicted bracket for the COMING step's fused pass
   unsigned long long cand_cap_total;   // n_seg * seg_cap of the last fused pass
   int hit;                    // this step: 1 = the bracket held (candidate list), 0 = general path
   unsigned long long n_fast, n_general;   // statistics (scape_select_stats)
   unsigned long long n_above, n_cand;     // this step's counts from the fused pass
+};
+
+// Per-layer top-k (PAPER.md:89 "per-layer style", :138): one of these per layer, device-resident.
+struct LayerState {
+  long long begin, end;       // the layer is [begin, end) of the flattened shard
+  long long k;                // entries the current refresh selects in this layer (end - begin when not compressed)
+  int compress;               // 0: never sparsified (LayerNorm, RMSNorm, bias: PAPER.md:246, :279, :286)
+  int hit;                    // this step: 1 = the layer's bracket held (candidate list), 0 = general route
+  unsigned long long prefix;  // digits of the layer's T64 fixed so far
+  unsigned long long himask;
+  long long rank;
+  int top;                    // bits [0, top) of K64 still undecided; 0 = T64 complete
+  int pad;
+  unsigned long long n_above; // certainly-selected entries counted by the fused pass (reset by lsel_decide)
+  Bracket br;
+};
+
+// Control block of the per-layer select.
+struct LayerCtl {
+  int any_general;            // some layer takes the general route in this step
+  int overflow;               // a candidate segment overflowed: every compressed layer goes general
+  float shrink;               // > 0: the candidate list was more than half full, narrow every bracket
+  int pad;
+  unsigned long long n_fast, n_general;   // layer-steps on each route (statistics)
 };
 
 struct StepParams {
@@ -84,6 +113,10 @@ struct StepParams {
   uint32_t* seg_count;          // [n_seg] candidates this warp saw (may exceed seg_cap: overflow)
   uint32_t* seg_above;          // [n_seg] certainly-selected entries this warp saw
   uint32_t seg_cap;
+  // per-layer refresh (nullptr = one flat top-k): layer of each chunk's first element, bit 31 set
+  // when the chunk holds entries of more than one layer
+  const uint32_t* chunk_layer;  // [Npad/128]
+  LayerState* layers;
 };
 
 // ------------------------------------------------------------------------------------------
@@ -163,7 +196,18 @@ struct StageA {                 // per-warp running state of the fused select (r
   uint32_t cursor;              // warp-uniform: candidates appended so far
   unsigned long long* seg;      // this warp's candidate segment
   double sumsq;                 // per lane: sum of g^^2 (clip mode)
+  uint32_t layer;               // per-layer refresh: layer whose bracket is loaded (kNoLayer: none yet)
 };
+constexpr uint32_t kNoLayer = 0xFFFFFFFFu;
+
+// per-layer refresh: add this warp's count of certainly-selected entries to its layer
+__device__ __forceinline__ void warp_flush_layer(const StepParams& p, StageA& sa, int lane) {
+  uint32_t na = sa.n_above;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
+  if (lane == 0 && na != 0u && sa.layer != kNoLayer) atomicAdd(&p.layers[sa.layer].n_above, (unsigned long long)na);
+  sa.n_above = 0;
+}
 
 // clip mode: this warp's share of sum g^^2, lanes added in a fixed butterfly order
 __device__ __forceinline__ void warp_store_sumsq(const StepParams& p, const StageA& sa, int64_t slot, int lane) {
@@ -344,13 +388,38 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
 
     // Stage 2 (l.11) fused: classify |m~^0| against the predicted bracket.  Exactness does not
     // depend on the prediction: sel_decide_kernel checks n_above < k <= n_above + n_cand.
+    bool mixed = false;                                     // chunk with entries of several layers (warp-uniform)
+    if (p.chunk_layer != nullptr) {
+      // per-layer refresh: the bracket is the one of this chunk's layer.  Warps walk the shard in
+      // ascending order, so a layer change is rare: flush the count, load the new bracket.
+      const uint32_t cl = __ldg(p.chunk_layer + c);
+      const uint32_t l = cl & 0x7FFFFFFFu;
+      mixed = (cl >> 31) != 0u;
+      if (l != sa.layer) {
+        warp_flush_layer(p, sa, lane);
+        sa.layer = l;
+        sa.lo = p.layers[l].br.lo_key; sa.hi = p.layers[l].br.hi_key;
+      }
+    }
     uint32_t nib = 0, cnib = 0;
+    if (!mixed) {
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      const bool valid = !GUARD || (i0 + q < p.N);
-      const bool above = valid && key0[q] >= sa.hi;
-      nib |= above ? (1u << q) : 0u;
-      cnib |= (valid && !above && key0[q] >= sa.lo) ? (1u << q) : 0u;
+      for (int q = 0; q < 4; ++q) {
+        const bool valid = !GUARD || (i0 + q < p.N);
+        const bool above = valid && key0[q] >= sa.hi;
+        nib |= above ? (1u << q) : 0u;
+        cnib |= (valid && !above && key0[q] >= sa.lo) ? (1u << q) : 0u;
+      }
+    } else {
+      // a chunk shared by several layers (at most one per layer boundary): bracket and count per entry
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        if (GUARD && i0 + q >= p.N) continue;
+        uint32_t l = sa.layer;
+        while (i0 + q >= p.layers[l].end) ++l;
+        if (key0[q] >= p.layers[l].br.hi_key) { nib |= 1u << q; atomicAdd(&p.layers[l].n_above, 1ull); }
+        else if (key0[q] >= p.layers[l].br.lo_key) cnib |= 1u << q;
+      }
     }
     if (__any_sync(0xFFFFFFFFu, cnib != 0u)) {              // candidates are rare: usually skipped
 #pragma unroll
@@ -365,7 +434,7 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
         sa.cursor += __popc(bal);
       }
     }
-    sa.n_above += __popc(nib);
+    if (!mixed) sa.n_above += __popc(nib);
     uint32_t w = nib << ((lane & 7) << 2);
     w |= __shfl_xor_sync(0xFFFFFFFFu, w, 1);
     w |= __shfl_xor_sync(0xFFFFFFFFu, w, 2);
@@ -420,13 +489,15 @@ __global__ void __launch_bounds__(256, ((!DENSE && R <= 2) ? 4 : R <= 4 ? 3 : 2)
   __shared__ float scratch[DENSE ? 1 : 8 * 2 * kChunk];     // per warp: (sum_r m~^r, m_old) of the selected entries
   float* sc = DENSE ? scratch : scratch + (threadIdx.x >> 5) * (2 * kChunk);
   StageA sa{};
+  sa.layer = kNoLayer;
   if (!DENSE) {
-    sa.lo = p.ctl->lo_key; sa.hi = p.ctl->hi_key;
+    sa.lo = p.ctl->br.lo_key; sa.hi = p.ctl->br.hi_key;
     sa.seg = p.cand + (size_t)warp * p.seg_cap;
   }
   for (int64_t c = warp; c < full; c += nwarps) fused_chunk<G, R, DENSE, MSPARSE, false>(p, c, lane, sc, sa);
   if (full < p.n_chunks && warp == full % nwarps) fused_chunk<G, R, DENSE, MSPARSE, true>(p, full, lane, sc, sa);
   if (!DENSE) {
+    if (p.chunk_layer != nullptr) warp_flush_layer(p, sa, lane);      // per-layer counts; seg_above stays 0
     uint32_t na = sa.n_above;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
@@ -616,7 +687,8 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
   // ===== consumers =====
   const int64_t gwarp = (int64_t)blockIdx.x * kTmaConsumerWarps + warp;     // candidate segment of this warp
   StageA sa{};
-  sa.lo = p.ctl->lo_key; sa.hi = p.ctl->hi_key;
+  sa.layer = kNoLayer;
+  sa.lo = p.ctl->br.lo_key; sa.hi = p.ctl->br.hi_key;
   sa.seg = p.cand + (size_t)gwarp * p.seg_cap;
 
   // Software pipeline of the small dependent accesses, so that none of their latency is exposed
@@ -654,6 +726,7 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
       else fused_chunk<G, R, false, true, true>(p, c, lane, sc, sa);
     }
   }
+  if (p.chunk_layer != nullptr) warp_flush_layer(p, sa, lane);        // per-layer counts; seg_above stays 0
   uint32_t na = sa.n_above;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
@@ -760,7 +833,7 @@ __global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t
     unsigned long long prefix0 = 0, himask0 = 0;
     int top = 64;
     if (hit) {
-      const uint32_t lo = st->lo_key, hi1 = st->hi_key - 1u;
+      const uint32_t lo = st->br.lo_key, hi1 = st->br.hi_key - 1u;
       const uint32_t diff = lo ^ hi1;
       const int common = diff ? __clz(diff) : 32;             // leading key bits shared by all candidates
       if (common > 0) {
@@ -780,7 +853,7 @@ __global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t
     if (!hit && !force_general) {
       // too many candidates for the list: narrower next time (a threshold outside the bracket
       // widens it by itself through the prediction error, see sel_pick_kernel)
-      if (s_over) st->delta = fmaxf(st->delta * 0.5f, 0.03f);
+      if (s_over) st->br.delta = fmaxf(st->br.delta * 0.5f, 0.03f);
     }
   }
 }
@@ -833,6 +906,46 @@ __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ K
   for (int b = threadIdx.x; b < kBins; b += blockDim.x) if (h[b]) atomicAdd(&ghist[b], h[b]);
 }
 
+// Predict the next step's bracket around the exact threshold just found (the top-k
+// structure of the first moment is temporally stable).  The threshold moves smoothly from step to
+// step (transient of the EMA, then stationary), so the centre is extrapolated geometrically and the
+// half-width follows the error the previous extrapolation made.  shrink > 0: cap the half-width at
+// shrink x the old one (the candidate list was more than half full).
+__device__ __forceinline__ void predict_bracket(Bracket& b, uint32_t Tkey, float shrink) {
+  const float T = __uint_as_float(Tkey);
+  float dl = b.delta, pred;
+  if (!(T > 0.0f) || !(T < 3.0e38f)) {           // zero / non-finite threshold: no prediction
+    b.lo_key = b.hi_key = 0xFFFFFFFFu; b.have_T = 0;
+    return;
+  }
+  const float lnT = __logf(T);
+  if (b.have_T == 0) { pred = lnT; dl = 0.6f; }
+  else {
+    // Step-to-step change r of ln T.  In the transient of the EMA r decays geometrically,
+    // so the next change is predicted as r * (r / r_prev) (ratio clamped to [0, 1]; no
+    // extrapolation at all when the sign flips, e.g. for alternating inputs).
+    const float r = fminf(fmaxf(lnT - b.lnT_prev, -0.7f), 0.7f);
+    float rn = r;
+    if (b.have_T >= 2) {
+      const float rp = b.r_prev;
+      const float ratio = (rp != 0.0f && (r > 0.0f) == (rp > 0.0f)) ? fminf(fmaxf(r / rp, 0.0f), 1.0f) : 0.0f;
+      rn = r * ratio;
+    }
+    pred = lnT + rn;
+    b.r_prev = r;
+    if (b.have_T == 1) dl = fmaxf(0.05f, 0.5f * fabsf(r));
+    else dl = fmaxf(3.0f * fabsf(lnT - b.ln_pred) + 0.01f, 0.85f * dl);   // widen at once, narrow slowly
+  }
+  if (shrink > 0.0f) dl = fminf(dl, b.delta * shrink);
+  dl = fminf(fmaxf(dl, 0.02f), 1.0f);
+  const float lo = __expf(pred - dl), hi = __expf(pred + dl);
+  b.lo_key = __float_as_uint(lo) & 0x7FFFFFFFu;
+  b.hi_key = (hi < 3.0e38f) ? (__float_as_uint(hi) & 0x7FFFFFFFu) : 0x7F800000u;
+  if (b.hi_key <= b.lo_key) b.hi_key = b.lo_key + 1u;
+  b.delta = dl; b.lnT_prev = lnT; b.ln_pred = pred;
+  b.have_T = b.have_T < 2 ? b.have_T + 1 : 2;
+}
+
 // One block: find the digit d whose class holds the sought rank; fix it; clear the histogram.
 __global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* ghist) {
   constexpr int PER = kBins / 1024;                 // bins per thread
@@ -880,45 +993,11 @@ __global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* 
         if (!st->use_cls && st->class_count <= (unsigned long long)kClsCap) st->use_cls = 1;
         st->class_count = hv[q];
         if (last) {
-          // T64 is now exact.  Predict the next step's bracket around this threshold
-          // (the top-k structure of the first moment is temporally stable).
-          // The threshold moves smoothly from step to step (transient of the EMA, then
-          // stationary), so the centre is extrapolated geometrically and the half-width follows
-          // the error the previous extrapolation made.
-          const float T = __uint_as_float((uint32_t)(T64 >> 32));
-          float dl = st->delta, pred;
-          if (!(T > 0.0f) || !(T < 3.0e38f)) {           // zero / non-finite threshold: no prediction
-            st->lo_key = st->hi_key = 0xFFFFFFFFu; st->have_T = 0;
-          } else {
-            const float lnT = __logf(T);
-            if (st->have_T == 0) { pred = lnT; dl = 0.6f; }
-            else {
-              // Step-to-step change r of ln T.  In the transient of the EMA r decays geometrically,
-              // so the next change is predicted as r * (r / r_prev) (ratio clamped to [0, 1]; no
-              // extrapolation at all when the sign flips, e.g. for alternating inputs).
-              const float r = fminf(fmaxf(lnT - st->lnT_prev, -0.7f), 0.7f);
-              float rn = r;
-              if (st->have_T >= 2) {
-                const float rp = st->r_prev;
-                const float ratio = (rp != 0.0f && (r > 0.0f) == (rp > 0.0f)) ? fminf(fmaxf(r / rp, 0.0f), 1.0f) : 0.0f;
-                rn = r * ratio;
-              }
-              pred = lnT + rn;
-              st->r_prev = r;
-              if (st->have_T == 1) dl = fmaxf(0.05f, 0.5f * fabsf(r));
-              else dl = fmaxf(3.0f * fabsf(lnT - st->ln_pred) + 0.01f, 0.85f * dl);   // widen at once, narrow slowly
-            }
-            // keep the expected candidate count under half the list's capacity
-            if (st->hit && st->cand_cap_total > 0 && 2ull * st->n_cand > st->cand_cap_total)
-              dl = fminf(dl, st->delta * (float)st->cand_cap_total / (2.0f * (float)st->n_cand));
-            dl = fminf(fmaxf(dl, 0.02f), 1.0f);
-            const float lo = __expf(pred - dl), hi = __expf(pred + dl);
-            st->lo_key = __float_as_uint(lo) & 0x7FFFFFFFu;
-            st->hi_key = (hi < 3.0e38f) ? (__float_as_uint(hi) & 0x7FFFFFFFu) : 0x7F800000u;
-            if (st->hi_key <= st->lo_key) st->hi_key = st->lo_key + 1u;
-            st->delta = dl; st->lnT_prev = lnT; st->ln_pred = pred;
-            st->have_T = st->have_T < 2 ? st->have_T + 1 : 2;
-          }
+          // T64 is now exact: predict the next step's bracket around this threshold
+          float shrink = 0.0f;              // keep the expected candidate count under half the list's capacity
+          if (st->hit && st->cand_cap_total > 0 && 2ull * st->n_cand > st->cand_cap_total)
+            shrink = (float)st->cand_cap_total / (2.0f * (float)st->n_cand);
+          predict_bracket(st->br, (uint32_t)(T64 >> 32), shrink);
         }
       }
       cum += hv[q];
@@ -959,6 +1038,271 @@ __global__ void __launch_bounds__(256) sel_finish_kernel(const __grid_constant__
     w |= __shfl_xor_sync(0xFFFFFFFFu, w, 4);
     if ((lane & 7) == 0) next_bits[(c << 2) + (lane >> 3)] = w;
   }
+}
+
+// ------------------------------------------------------------------------------------------
+// Per-layer refresh ("the top-k sparsification is performed in a per-layer style",
+// :138 "number of layers in model L"; uncompressed LayerNorm / RMSNorm / bias layers: :246, :279,
+// :286).  The same exact radix select on the same composite keys, run for every layer at once:
+// one LayerState per layer, one histogram per layer in global memory.  A layer whose predicted
+// bracket held works on the candidates the fused pass collected; the others (no prediction yet,
+// a miss, an all-ones step) read their keys back from e^0 / b^0 in work items that never cross a
+// layer boundary, so that a CTA can keep a private shared-memory histogram per item.
+// ------------------------------------------------------------------------------------------
+struct LayerWork {
+  const uint32_t* chunk_layer;  // [Npad/128]
+  LayerState* layers;
+  int n_layers;
+  LayerCtl* ctl;
+  uint32_t* hist;               // [n_layers][kBins]
+  const int4* items;            // {layer, first chunk, end chunk, 0}: <= kItemChunks chunks of one layer
+  int n_items;
+};
+constexpr int kItemChunks = 2048;
+
+__device__ __forceinline__ uint32_t layer_of(const LayerWork& w, uint32_t i) {
+  const uint32_t cl = __ldg(w.chunk_layer + (i >> 7));
+  uint32_t l = cl & 0x7FFFFFFFu;
+  if (cl >> 31) while ((long long)i >= w.layers[l].end) ++l;          // chunk shared by several layers
+  return l;
+}
+
+// One block.  Per layer: k_l of this refresh (reading S6 inside the layer, evaluated in double
+// like the host does), route, and the armed radix state.
+__global__ void __launch_bounds__(1024) lsel_decide_kernel(LayerWork w, CandList cl, double sparsity, int force_general) {
+  __shared__ unsigned long long s_cand[32];
+  __shared__ int s_over;
+  if (threadIdx.x == 0) s_over = 0;
+  __syncthreads();
+  unsigned long long c = 0;
+  int over = 0;
+  if (!force_general)
+    for (int i = threadIdx.x; i < cl.n_seg; i += blockDim.x) { const uint32_t cnt = cl.seg_count[i]; c += cnt; over |= cnt > cl.seg_cap; }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, o);
+  if ((threadIdx.x & 31) == 0) s_cand[threadIdx.x >> 5] = c;
+  if (over) s_over = 1;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    c = 0;
+    for (int i = 0; i < 32; ++i) c += s_cand[i];
+    const unsigned long long cap = (unsigned long long)cl.n_seg * cl.seg_cap;
+    w.ctl->overflow = s_over;
+    w.ctl->shrink = (!force_general && cap > 0 && 2ull * c > cap) ? (float)cap / (2.0f * (float)c) : 0.0f;
+    w.ctl->any_general = 0;
+  }
+  __syncthreads();
+  unsigned long long nf = 0, ng = 0;
+  for (int l = threadIdx.x; l < w.n_layers; l += blockDim.x) {
+    LayerState& S = w.layers[l];
+    const long long n = S.end - S.begin;
+    const long long k = S.compress ? n - (long long)floor(sparsity * (double)n) : n;
+    const long long a = (long long)S.n_above;
+    S.n_above = 0;
+    S.k = k;
+    const bool predicted = !(S.br.lo_key == 0xFFFFFFFFu && S.br.hi_key == 0xFFFFFFFFu);
+    const bool hit = !force_general && !s_over && predicted && a <= k;
+    S.hit = hit ? 1 : 0;
+    if (hit) {
+      nf += 1;
+      S.rank = k - a;                                  // still to be found among the layer's candidates
+      if (S.rank == 0) { S.top = 0; S.prefix = ~0ull; S.himask = ~0ull; }     // nothing more to select
+      else {
+        // every candidate of the layer lies in [lo_key, hi_key): start below the bits they share
+        const uint32_t lo = S.br.lo_key, diff = lo ^ (S.br.hi_key - 1u);
+        const int common = diff ? __clz(diff) : 32;
+        const uint32_t km = common == 0 ? 0u : common >= 32 ? 0xFFFFFFFFu : ~(0xFFFFFFFFu >> common);
+        S.himask = (unsigned long long)km << 32;
+        S.prefix = (unsigned long long)(lo & km) << 32;
+        S.top = 64 - common;
+      }
+    } else {
+      ng += 1;
+      S.rank = k; S.top = 64; S.prefix = 0; S.himask = 0;
+      atomicOr(&w.ctl->any_general, 1);
+      if (!force_general && s_over && S.compress) S.br.delta = fmaxf(S.br.delta * 0.5f, 0.03f);
+    }
+  }
+  if (nf) atomicAdd(&w.ctl->n_fast, nf);
+  if (ng) atomicAdd(&w.ctl->n_general, ng);
+}
+
+__device__ __forceinline__ bool layer_digit(const LayerState& S, unsigned long long k64, uint32_t& d) {
+  const int top = S.top;
+  if (top <= 0 || (k64 & S.himask) != S.prefix) return false;
+  const int bits = top < kDigitBits ? top : kDigitBits;
+  d = (uint32_t)(k64 >> (top - bits)) & ((1u << bits) - 1u);
+  return true;
+}
+
+// Digit histograms of the layers on the candidate route.  The candidates of one layer fall into a
+// handful of bins in the first pass, so equal (layer, digit) pairs of a warp are merged before the
+// global atomic.
+__global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_constant__ LayerWork w, const __grid_constant__ CandList cl) {
+  const int lane = threadIdx.x & 31;
+  const int64_t wpb = blockDim.x >> 5;
+  const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
+  const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  for (int64_t sg = warp; sg < cl.n_seg; sg += nwarps) {
+    const uint32_t cnt = min(cl.seg_count[sg], cl.seg_cap);
+    const unsigned long long* seg = cl.cand + (size_t)sg * cl.seg_cap;
+    for (uint32_t j0 = 0; j0 < cnt; j0 += 32) {
+      const uint32_t j = j0 + lane;
+      uint32_t tag = 0xFFFFFFFFu;
+      if (j < cnt) {
+        const unsigned long long k64 = __ldcs(seg + j);
+        const uint32_t l = layer_of(w, 0xFFFFFFFFu - (uint32_t)k64);
+        uint32_t d;
+        if (w.layers[l].hit && layer_digit(w.layers[l], k64, d)) tag = (l << kDigitBits) | d;
+      }
+      const uint32_t same = __match_any_sync(0xFFFFFFFFu, tag);
+      if (tag != 0xFFFFFFFFu && (__ffs(same) - 1) == lane) atomicAdd(&w.hist[tag], (uint32_t)__popc(same));
+    }
+  }
+}
+
+// Digit histograms of the layers on the general route: every key of the layer, item by item.
+__global__ void __launch_bounds__(256) lsel_hist_full_kernel(const __grid_constant__ KeySrc s, const __grid_constant__ LayerWork w) {
+  __shared__ uint32_t h[kBins];
+  if (!w.ctl->any_general) return;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, wpb = blockDim.x >> 5;
+  for (int it = blockIdx.x; it < w.n_items; it += gridDim.x) {
+    const int4 item = __ldg(w.items + it);
+    const LayerState& S = w.layers[item.x];
+    if (S.hit || S.top <= 0) continue;                      // block-uniform
+    for (int b = threadIdx.x; b < kBins; b += blockDim.x) h[b] = 0;
+    __syncthreads();
+    const long long lb = S.begin, le = S.end;
+    for (int64_t c = item.y + wid; c < item.z; c += wpb) {
+      unsigned long long k64[4]; bool valid[4];
+      chunk_keys(s, c, lane, k64, valid);
+      const int64_t i0 = (c << 7) + ((int64_t)lane << 2);
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        uint32_t d;
+        if (valid[q] && i0 + q >= lb && i0 + q < le && layer_digit(S, k64[q], d)) atomicAdd(&h[d], 1u);
+      }
+    }
+    __syncthreads();
+    uint32_t* gh = w.hist + (size_t)item.x * kBins;
+    for (int b = threadIdx.x; b < kBins; b += blockDim.x) if (h[b]) atomicAdd(&gh[b], h[b]);
+    __syncthreads();
+  }
+}
+
+// One block per layer: find the digit whose class holds the sought rank; fix it; clear the
+// layer's histogram.  A layer on the candidate route whose candidates turn out to be fewer than
+// the rank sought (the bracket missed) restarts on the general route.
+__global__ void __launch_bounds__(1024) lsel_pick_kernel(LayerWork w) {
+  constexpr int PER = kBins / 1024;
+  LayerState& S = w.layers[blockIdx.x];
+  uint32_t* ghist = w.hist + (size_t)blockIdx.x * kBins;
+  const int top_in = S.top;
+  if (top_in <= 0) return;
+  const int bits = top_in < kDigitBits ? top_in : kDigitBits;
+  const int shift = top_in - bits;
+  __shared__ long long warp_tot[32];
+  __shared__ long long s_total;
+  const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
+  const int topb = kBins - PER * t;                 // thread 0 owns the TOP bins
+  uint32_t hv[PER];
+  long long local = 0;
+#pragma unroll
+  for (int q = 0; q < PER; ++q) { hv[q] = ghist[topb - 1 - q]; local += hv[q]; ghist[topb - 1 - q] = 0; }
+  long long incl = local;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { long long v = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += v; }
+  if (lane == 31) warp_tot[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    long long v = warp_tot[lane], iv = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { long long x = __shfl_up_sync(0xFFFFFFFFu, iv, o); if (lane >= o) iv += x; }
+    warp_tot[lane] = iv - v;
+    if (lane == 31) s_total = iv;
+  }
+  __syncthreads();
+  const long long above = warp_tot[wid] + incl - local;
+  const long long rank = S.rank;
+  const long long total = s_total;
+  const int hit = S.hit;
+  __syncthreads();
+  if (total < rank) {
+    // only possible on the candidate route, first pass: fewer candidates than entries still to
+    // select, i.e. the true threshold lies below the bracket
+    if (t == 0) {
+      S.hit = 0; S.rank = S.k; S.top = 64; S.prefix = 0; S.himask = 0;
+      atomicOr(&w.ctl->any_general, 1);
+      atomicAdd(&w.ctl->n_general, 1ull);
+      atomicAdd(&w.ctl->n_fast, ~0ull);              // - 1
+    }
+    return;
+  }
+  if (above < rank && rank <= above + local) {
+    long long cum = above;
+#pragma unroll
+    for (int q = 0; q < PER; ++q) {
+      if (cum < rank && rank <= cum + hv[q]) {
+        const unsigned long long d = (unsigned long long)(topb - 1 - q);
+        const unsigned long long T64 = S.prefix | (d << shift);
+        S.prefix = T64;
+        S.himask |= ((1ull << bits) - 1ull) << shift;
+        S.rank = rank - cum;
+        S.top = shift;
+        if (shift == 0 && S.compress) predict_bracket(S.br, (uint32_t)(T64 >> 32), hit ? w.ctl->shrink : 0.0f);
+      }
+      cum += hv[q];
+    }
+  }
+}
+
+// M_t of the layers on the general route: rewrite every bit of the layer from its keys.
+__global__ void __launch_bounds__(256) lsel_finish_full_kernel(const __grid_constant__ KeySrc s, const __grid_constant__ LayerWork w,
+                                                              uint32_t* __restrict__ next_bits) {
+  if (!w.ctl->any_general) return;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, wpb = blockDim.x >> 5;
+  for (int it = blockIdx.x; it < w.n_items; it += gridDim.x) {
+    const int4 item = __ldg(w.items + it);
+    const LayerState& S = w.layers[item.x];
+    if (S.hit) continue;
+    const unsigned long long T64 = S.prefix;
+    const long long lb = S.begin, le = S.end;
+    for (int64_t c = item.y + wid; c < item.z; c += wpb) {
+      unsigned long long k64[4]; bool valid[4];
+      chunk_keys(s, c, lane, k64, valid);
+      const int64_t i0 = (c << 7) + ((int64_t)lane << 2);
+      uint32_t nib = 0, own = 0;                            // own: positions of this word that belong to the layer
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const bool in = i0 + q >= lb && i0 + q < le;
+        own |= in ? (1u << q) : 0u;
+        nib |= (in && valid[q] && k64[q] >= T64) ? (1u << q) : 0u;
+      }
+      uint32_t v = nib << ((lane & 7) << 2), m = own << ((lane & 7) << 2);
+#pragma unroll
+      for (int o = 1; o < 8; o <<= 1) { v |= __shfl_xor_sync(0xFFFFFFFFu, v, o); m |= __shfl_xor_sync(0xFFFFFFFFu, m, o); }
+      if ((lane & 7) == 0 && m != 0u) {
+        uint32_t* wp = next_bits + (c << 2) + (lane >> 3);
+        if (m == 0xFFFFFFFFu) *wp = v;
+        else { atomicAnd(wp, ~m); atomicOr(wp, v); }       // word shared with a neighbouring layer
+      }
+    }
+  }
+}
+
+// M_t of the layers on the candidate route: the fused pass wrote the certainly-selected bits;
+// OR in the candidates at or above the layer's threshold.
+__global__ void __launch_bounds__(256) lsel_finish_cand_kernel(const __grid_constant__ LayerWork w, const __grid_constant__ CandList cl,
+                                                              uint32_t* __restrict__ next_bits) {
+  const int lane = threadIdx.x & 31;
+  const int64_t wpb = blockDim.x >> 5;
+  const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
+  const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  scan_segments(cl.cand, cl.seg_count, cl.seg_cap, cl.n_seg, warp, nwarps, lane, [&](unsigned long long k64) {
+    const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64;
+    const LayerState& S = w.layers[layer_of(w, i)];
+    if (S.hit && k64 >= S.prefix) atomicOr(&next_bits[i >> 5], 1u << (i & 31));
+  });
 }
 
 // ------------------------------------------------------------------------------------------

@@ -82,6 +82,18 @@ class Workload:
     def numel(self) -> int:
         return sum(n for _, n in self.tensors)
 
+    def offsets(self) -> List[int]:
+        """Tensor boundaries in the flattened shard: the layers of a per-layer refresh."""
+        off = [0]
+        for _, n in self.tensors:
+            off.append(off[-1] + n)
+        return off
+
+    def compress_flags(self) -> List[int]:
+        """0 for the tensors the paper leaves uncompressed (LayerNorm, RMSNorm, bias: PAPER.md:246,
+        :279, :286), recognised by name; 1 for the weight matrices."""
+        return [0 if any(t in name for t in ("norm", "bias", "ln_")) else 1 for name, _ in self.tensors]
+
 
 def scaled(tensors: List[Tuple[str, int]], div: int) -> List[Tuple[str, int]]:
     """Same structure, every tensor `div` times smaller (kept a multiple of 8 elements, so
