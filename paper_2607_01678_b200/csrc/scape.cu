@@ -142,7 +142,7 @@ int launch_fused_t(scape* h, StepParams& p, cudaStream_t st) {
   static int bps = 0;   // resident blocks per SM of this instantiation
   if (bps == 0) {
     int v = 0;
-    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, scape_fused_step_kernel<G, R, DENSE, MSPARSE>, 256, 0));
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, scape_fused_step_kernel<G, R, DENSE, MSPARSE, false>, 256, 0));
     bps = v > 0 ? (v > 8 ? 8 : v) : 1;
   }
   const int grid = grid_for(h, p.n_chunks, 8, bps);
@@ -153,7 +153,9 @@ int launch_fused_t(scape* h, StepParams& p, cudaStream_t st) {
   if (cap > 0x7FFFFFF0) cap = 0x7FFFFFF0;
   h->seg_cap = (uint32_t)cap;
   p.seg_cap = h->seg_cap;
-  scape_fused_step_kernel<G, R, DENSE, MSPARSE><<<grid, 256, 0, st>>>(p);
+  // the clip_grad variant is a separate instantiation so that the default path carries none of it
+  if (p.clip) scape_fused_step_kernel<G, R, DENSE, MSPARSE, true><<<grid, 256, 0, st>>>(p);
+  else scape_fused_step_kernel<G, R, DENSE, MSPARSE, false><<<grid, 256, 0, st>>>(p);
   h->last_kernel = "scape_fused_step_kernel";
   h->launches++;
   CU_TRY(cudaGetLastError());

@@ -178,13 +178,19 @@ __device__ __forceinline__ uint32_t chunk_popc(const uint4 mw) { return __popc(m
 __device__ __forceinline__ void lane_mask_bits(const uint32_t* __restrict__ bits, const uint32_t* __restrict__ rank,
                                                int64_t c, int lane, uint32_t& mybits, uint32_t& jbase) {
   const uint4 mw = __ldg(reinterpret_cast<const uint4*>(bits) + c);
-  const uint32_t r0 = __ldg(rank + c);
-  const int ws = lane >> 3, sh = (lane & 7) << 2;
-  const uint32_t p0 = __popc(mw.x), p1 = p0 + __popc(mw.y), p2 = p1 + __popc(mw.z);
-  const uint32_t w = ws == 0 ? mw.x : ws == 1 ? mw.y : ws == 2 ? mw.z : mw.w;
-  const uint32_t before = ws == 0 ? 0u : ws == 1 ? p0 : ws == 2 ? p1 : p2;
-  mybits = (w >> sh) & 0xFu;
-  jbase = r0 + before + __popc(w & ((1u << sh) - 1u));
+  lane_bits_from_words(mw, __ldg(rank + c), lane, mybits, jbase);
+}
+
+// Gather of m_{t-1} for this lane's 4 elements from the previous step's packed mean: selected
+// entries sit at consecutive packed positions from pbase on, so one pointer walks them.
+__device__ __forceinline__ void gather_prev_m(const float* __restrict__ pm, uint32_t pbits, uint32_t pbase, float (&mo)[4]) {
+  const float* ptr = pm + pbase;
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const bool on = (pbits >> q) & 1u;
+    mo[q] = on ? __ldg(ptr) : 0.0f;
+    ptr += on ? 1 : 0;
+  }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -304,8 +310,8 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
         }
         key0[q] = __float_as_uint(mt[0]) & 0x7FFFFFFFu;
         float u = 0.0f;                                                          // Eq. 5: u = 0 off the mask
-        if (__any_sync(0xFFFFFFFFu, on)) {
-          if (on) {
+        if (on) {                                                                // divergent: only the owning lanes run it
+          {
             const uint32_t j = jbase + __popc(mybits & ((1u << q) - 1u));
             float* pk = p.packed + j;
             float sm = mt[0];
@@ -421,17 +427,42 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
         else if (key0[q] >= p.layers[l].br.lo_key) cnib |= 1u << q;
       }
     }
-    if (__any_sync(0xFFFFFFFFu, cnib != 0u)) {              // candidates are rare: usually skipped
+    // Append this chunk's candidates to the warp's segment (their order inside the segment is
+    // irrelevant: the composite keys carry the index).  Two forms, chosen by measurement: the
+    // register-staged front-end is issue-bound and takes the shorter one (one prefix over the lanes
+    // from three ballots on the bits of the per-lane count); the bulk-copy front-end is register-
+    // bound (96 registers per thread) and keeps the one with the shortest live ranges.
+    if constexpr (STORE) {
+      if (__any_sync(0xFFFFFFFFu, cnib != 0u)) {
+        const uint32_t n = __popc(cnib), lt = (1u << lane) - 1u;
+        const uint32_t b0 = __ballot_sync(0xFFFFFFFFu, n & 1u), b1 = __ballot_sync(0xFFFFFFFFu, n & 2u),
+                       b2 = __ballot_sync(0xFFFFFFFFu, n & 4u);
+        uint32_t pos = sa.cursor + __popc(b0 & lt) + 2u * __popc(b1 & lt) + 4u * __popc(b2 & lt);
+        if (cnib != 0u) {
+          const uint32_t inv = 0xFFFFFFFFu - (uint32_t)i0;
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const bool cnd = (cnib >> q) & 1u;
-        const uint32_t bal = __ballot_sync(0xFFFFFFFFu, cnd);
-        if (cnd) {
-          const uint32_t pos = sa.cursor + __popc(bal & ((1u << lane) - 1u));
-          if (pos < p.seg_cap)
-            sa.seg[pos] = ((unsigned long long)key0[q] << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)(i0 + q));
+          for (int q = 0; q < 4; ++q) {
+            if ((cnib >> q) & 1u) {
+              if (pos < p.seg_cap) sa.seg[pos] = ((unsigned long long)key0[q] << 32) | (unsigned long long)(inv - q);
+              ++pos;
+            }
+          }
         }
-        sa.cursor += __popc(bal);
+        sa.cursor += __popc(b0) + 2u * __popc(b1) + 4u * __popc(b2);
+      }
+    } else {
+      if (__any_sync(0xFFFFFFFFu, cnib != 0u)) {              // candidates are rare: usually skipped
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const bool cnd = (cnib >> q) & 1u;
+          const uint32_t bal = __ballot_sync(0xFFFFFFFFu, cnd);
+          if (cnd) {
+            const uint32_t pos = sa.cursor + __popc(bal & ((1u << lane) - 1u));
+            if (pos < p.seg_cap)
+              sa.seg[pos] = ((unsigned long long)key0[q] << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)(i0 + q));
+          }
+          sa.cursor += __popc(bal);
+        }
       }
     }
     if (!mixed) sa.n_above += __popc(nib);
@@ -443,7 +474,7 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
   }
 }
 
-template <typename G, int R, bool DENSE, bool MSPARSE, bool GUARD>
+template <typename G, int R, bool DENSE, bool MSPARSE, bool GUARD, bool CLIPT>
 __device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int lane, float* sc, StageA& sa) {
   const int64_t i0 = (c << 7) + ((int64_t)lane << 2);
   // Issue order matters for latency: the mask words first (L2-resident, short latency), then the
@@ -468,16 +499,13 @@ __device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int 
   if (MSPARSE) {
     uint32_t pbits, pbase;
     lane_bits_from_words(pw, pr, lane, pbits, pbase);
-#pragma unroll
-    for (int q = 0; q < 4; ++q)
-      mo[q] = ((pbits >> q) & 1u) ? __ldg(p.pm_prev + pbase + __popc(pbits & ((1u << q) - 1u))) : 0.0f;
+    gather_prev_m(p.pm_prev, pbits, pbase, mo);
   }
 
-  constexpr bool COMPACT = R >= 3;      // one or two replicas: latency-bound, the plain in-place path is shorter
-  fused_compute<R, DENSE, GUARD, true, true, COMPACT>(p, c, lane, i0, mybits, jbase, cr, (DENSE || !COMPACT) ? 0u : chunk_popc(cw), sc, sc + kChunk, th, mo, gg, ee, sa);
+  fused_compute<R, DENSE, GUARD, true, CLIPT>(p, c, lane, i0, mybits, jbase, cr, DENSE ? 0u : chunk_popc(cw), sc, sc + kChunk, th, mo, gg, ee, sa);
 }
 
-template <typename G, int R, bool DENSE, bool MSPARSE>
+template <typename G, int R, bool DENSE, bool MSPARSE, bool CLIPT>
 // resident CTAs per SM: sparse steps with one or two replicas are latency-bound (12-24 bytes per parameter in
 // flight per lane), so they trade registers for a fourth CTA (measured, N = 2^28, R = 2, 90 %: 2.54 -> 2.29 ms)
 __global__ void __launch_bounds__(256, ((!DENSE && R <= 2) ? 4 : R <= 4 ? 3 : 2)) scape_fused_step_kernel(const __grid_constant__ StepParams p) {
@@ -494,8 +522,8 @@ __global__ void __launch_bounds__(256, ((!DENSE && R <= 2) ? 4 : R <= 4 ? 3 : 2)
     sa.lo = p.ctl->br.lo_key; sa.hi = p.ctl->br.hi_key;
     sa.seg = p.cand + (size_t)warp * p.seg_cap;
   }
-  for (int64_t c = warp; c < full; c += nwarps) fused_chunk<G, R, DENSE, MSPARSE, false>(p, c, lane, sc, sa);
-  if (full < p.n_chunks && warp == full % nwarps) fused_chunk<G, R, DENSE, MSPARSE, true>(p, full, lane, sc, sa);
+  for (int64_t c = warp; c < full; c += nwarps) fused_chunk<G, R, DENSE, MSPARSE, false, CLIPT>(p, c, lane, sc, sa);
+  if (full < p.n_chunks && warp == full % nwarps) fused_chunk<G, R, DENSE, MSPARSE, true, CLIPT>(p, full, lane, sc, sa);
   if (!DENSE) {
     if (p.chunk_layer != nullptr) warp_flush_layer(p, sa, lane);      // per-layer counts; seg_above stays 0
     uint32_t na = sa.n_above;
@@ -503,7 +531,7 @@ __global__ void __launch_bounds__(256, ((!DENSE && R <= 2) ? 4 : R <= 4 ? 3 : 2)
     for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
     if (lane == 0) { p.seg_count[warp] = sa.cursor; p.seg_above[warp] = na; }
   }
-  if (p.clip) warp_store_sumsq(p, sa, warp, lane);
+  if (CLIPT && p.clip) warp_store_sumsq(p, sa, warp, lane);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -565,9 +593,7 @@ __device__ __forceinline__ void tma_decode_gather(const StepParams& p, const Tma
   lane_bits_from_words(w.cw, w.cr, lane, st.mybits, st.jbase);
   st.r0 = w.cr; st.cnt = chunk_popc(w.cw);
   lane_bits_from_words(w.pw, w.pr, lane, pbits, pbase);
-#pragma unroll
-  for (int q = 0; q < 4; ++q)
-    st.mo[q] = ((pbits >> q) & 1u) ? __ldg(p.pm_prev + pbase + __popc(pbits & ((1u << q) - 1u))) : 0.0f;
+  gather_prev_m(p.pm_prev, pbits, pbase, st.mo);
 }
 
 // One tile of one consumer warp: start the next tile's gather, wait for this tile's bytes, pull
@@ -722,8 +748,8 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
     if (c < p.n_chunks && blockIdx.x == (unsigned)(n_tiles % gridDim.x)) {
       // (all bulk stores of this CTA have completed: the first stage serves as scratch)
       float* sc = reinterpret_cast<float*>(stage0) + warp * (2 * kChunk);
-      if (((c + 1) << 7) <= p.N) fused_chunk<G, R, false, true, false>(p, c, lane, sc, sa);
-      else fused_chunk<G, R, false, true, true>(p, c, lane, sc, sa);
+      if (((c + 1) << 7) <= p.N) fused_chunk<G, R, false, true, false, CLIPT>(p, c, lane, sc, sa);
+      else fused_chunk<G, R, false, true, true, CLIPT>(p, c, lane, sc, sa);
     }
   }
   if (p.chunk_layer != nullptr) warp_flush_layer(p, sa, lane);        // per-layer counts; seg_above stays 0
