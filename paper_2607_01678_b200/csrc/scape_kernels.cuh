@@ -45,6 +45,7 @@ struct SelState {
   unsigned long long class_count;   // keys in the class chosen by the last pick
   unsigned int cls_n;         // entries in the small list
   unsigned int pad1;
+  unsigned long long base;    // fast route: the radix passes run on K64 - base (base = lo_key << 32), see sel_decide_kernel
   Bracket br;                 // predicted bracket for the COMING step's fused pass
   unsigned long long cand_cap_total;   // n_seg * seg_cap of the last fused pass
   int hit;                    // this step: 1 = the bracket held (candidate list), 0 = general path
@@ -800,17 +801,44 @@ __device__ __forceinline__ void chunk_keys(const KeySrc& s, int64_t c, int lane,
 // Candidate list written by the fused pass: n_seg segments of seg_cap entries.
 constexpr uint32_t kClsCap = 1u << 20;   // entries of the small list the surviving class is collected into
 
-// strided, 4-deep unrolled scan of the candidate segments (4 independent 8-byte loads per lane)
+// Scan of the candidate segments by the whole grid.  The fused pass leaves one segment per warp
+// (a few thousand of them).  Long segments (large shards: ~10^4 entries each): a work item is one
+// of P equal slices of one segment, items are dealt round-robin to the CTAs, and the threads of a
+// CTA stride through a slice with 4 independent 8-byte loads each (one warp per segment left two
+// thirds of the grid idle and the rest walking long chains of dependent trips).  Short segments
+// (small shards: the pass is latency-bound): one warp per segment, all segments at once.
 template <typename F>
 __device__ __forceinline__ void scan_segments(const unsigned long long* cand, const uint32_t* seg_count, uint32_t seg_cap,
-                                              int n_seg, int64_t warp, int64_t nwarps, int lane, F f) {
-  for (int64_t sg = warp; sg < n_seg; sg += nwarps) {
+                                              int n_seg, unsigned long long n_cand, F f) {
+  if (n_cand <= 256ull * (unsigned long long)n_seg) {
+    const int lane = threadIdx.x & 31;
+    const int64_t wpb = blockDim.x >> 5;
+    const int64_t nwarps = (int64_t)gridDim.x * wpb;
+    for (int64_t sg = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5); sg < n_seg; sg += nwarps) {
+      const uint32_t cnt = min(seg_count[sg], seg_cap);
+      const unsigned long long* seg = cand + (size_t)sg * seg_cap;
+      for (uint32_t j0 = 0; j0 < cnt; j0 += 128) {
+        unsigned long long v[4]; bool ok[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { const uint32_t j = j0 + u * 32 + lane; ok[u] = j < cnt; v[u] = ok[u] ? __ldcs(seg + j) : 0ull; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) if (ok[u]) f(v[u]);
+      }
+    }
+    return;
+  }
+  const uint32_t P = max(1u, (2u * gridDim.x + (uint32_t)n_seg - 1u) / (uint32_t)n_seg);
+  const uint32_t n_items = (uint32_t)n_seg * P;
+  for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
+    const uint32_t sg = it % (uint32_t)n_seg, part = it / (uint32_t)n_seg;
     const uint32_t cnt = min(seg_count[sg], seg_cap);
+    const uint32_t per = ((cnt + P - 1u) / P + 31u) & ~31u;      // slice length, whole 256-byte lines
+    const uint32_t b = part * per, e = min(cnt, b + per);
     const unsigned long long* seg = cand + (size_t)sg * seg_cap;
-    for (uint32_t j0 = 0; j0 < cnt; j0 += 128) {
+    for (uint32_t j0 = b + threadIdx.x; j0 < e; j0 += 4u * blockDim.x) {
       unsigned long long v[4]; bool ok[4];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) { const uint32_t j = j0 + u * 32 + lane; ok[u] = j < cnt; v[u] = ok[u] ? __ldcs(seg + j) : 0ull; }
+      for (int u = 0; u < 4; ++u) { const uint32_t j = j0 + u * blockDim.x; ok[u] = j < e; v[u] = ok[u] ? __ldcs(seg + j) : 0ull; }
 #pragma unroll
       for (int u = 0; u < 4; ++u) if (ok[u]) f(v[u]);
     }
@@ -853,22 +881,20 @@ __global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t
     a = 0; c = 0;
     for (int i = 0; i < 32; ++i) { a += s_above[i]; c += s_cand[i]; }
     const bool hit = !force_general && !s_over && (long long)a < k && (long long)(a + c) >= k;
-    // On the fast route every candidate key lies in [lo_key, hi_key): the bits those two bounds
-    // share are already known, so the radix passes start below them (fewer passes, and the first
-    // digit spreads the candidates over the whole histogram instead of two or three bins).
-    unsigned long long prefix0 = 0, himask0 = 0;
+    // On the fast route every candidate key lies in [lo_key, hi_key): the passes run on
+    // K64 - (lo_key << 32), whose bits above 32 + ceil(log2(hi_key - lo_key)) are all zero, and start
+    // there.  Fewer passes, and the first digit spreads the candidates over at least half of the
+    // histogram wherever the bracket sits (skipping only the bits lo and hi share leaves a few
+    // hundred crowded bins when the bracket straddles a power of two: contended shared-memory
+    // atomics, and a surviving class of 10^5 keys for the second pass to collect).
+    unsigned long long prefix0 = 0, himask0 = 0, base = 0;
     int top = 64;
     if (hit) {
-      const uint32_t lo = st->br.lo_key, hi1 = st->br.hi_key - 1u;
-      const uint32_t diff = lo ^ hi1;
-      const int common = diff ? __clz(diff) : 32;             // leading key bits shared by all candidates
-      if (common > 0) {
-        const uint32_t km = common >= 32 ? 0xFFFFFFFFu : ~(0xFFFFFFFFu >> common);
-        himask0 = (unsigned long long)km << 32;
-        prefix0 = (unsigned long long)(lo & km) << 32;
-      }
-      top = 64 - common;
+      const uint32_t lo = st->br.lo_key, span1 = st->br.hi_key - 1u - lo;      // largest key - lo
+      base = (unsigned long long)lo << 32;
+      top = 32 + (span1 ? 32 - __clz(span1) : 0);
     }
+    st->base = base;
     st->prefix = prefix0; st->himask = himask0; st->top = top;
     st->use_cls = 0; st->cls_n = 0; st->class_count = ~0ull;
     st->rank = hit ? k - (long long)a : k;
@@ -909,9 +935,11 @@ __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ K
   const int64_t wpb = blockDim.x >> 5;
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
   const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  const unsigned long long base = st->base;
   auto visit = [&](unsigned long long k64) {
-    if ((k64 & himask) == prefix) {
-      atomicAdd(&h[(uint32_t)(k64 >> shift) & dmask], 1u);
+    const unsigned long long kr = k64 - base;
+    if ((kr & himask) == prefix) {
+      atomicAdd(&h[(uint32_t)(kr >> shift) & dmask], 1u);
       if (collect) { const uint32_t pos = atomicAdd(&st->cls_n, 1u); if (pos < kClsCap) cl.cls[pos] = k64; }
     }
   };
@@ -919,7 +947,7 @@ __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ K
     const uint32_t n = min(st->cls_n, kClsCap);
     for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += cls_blocks * blockDim.x) visit(cl.cls[j]);
   } else if (hit) {
-    scan_segments(cl.cand, cl.seg_count, cl.seg_cap, cl.n_seg, warp, nwarps, lane, visit);
+    scan_segments(cl.cand, cl.seg_count, cl.seg_cap, cl.n_seg, st->n_cand, visit);
   } else {
     for (int64_t c = warp; c < s.n_chunks; c += nwarps) {
       unsigned long long k64[4]; bool valid[4];
@@ -1019,11 +1047,13 @@ __global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* 
         if (!st->use_cls && st->class_count <= (unsigned long long)kClsCap) st->use_cls = 1;
         st->class_count = hv[q];
         if (last) {
-          // T64 is now exact: predict the next step's bracket around this threshold
+          // T64 is now exact (back in the key domain): predict the next step's bracket around it
+          const unsigned long long Tk = T64 + st->base;
+          st->prefix = Tk; st->base = 0;
           float shrink = 0.0f;              // keep the expected candidate count under half the list's capacity
           if (st->hit && st->cand_cap_total > 0 && 2ull * st->n_cand > st->cand_cap_total)
             shrink = (float)st->cand_cap_total / (2.0f * (float)st->n_cand);
-          predict_bracket(st->br, (uint32_t)(T64 >> 32), shrink);
+          predict_bracket(st->br, (uint32_t)(Tk >> 32), shrink);
         }
       }
       cum += hv[q];
@@ -1044,7 +1074,7 @@ __global__ void __launch_bounds__(256) sel_finish_kernel(const __grid_constant__
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
   const int64_t nwarps = (int64_t)gridDim.x * wpb;
   if (st->hit) {
-    scan_segments(cl.cand, cl.seg_count, cl.seg_cap, cl.n_seg, warp, nwarps, lane, [&](unsigned long long k64) {
+    scan_segments(cl.cand, cl.seg_count, cl.seg_cap, cl.n_seg, st->n_cand, [&](unsigned long long k64) {
       if (k64 >= T64) {
         const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64;
         atomicOr(&next_bits[i >> 5], 1u << (i & 31));
@@ -1169,13 +1199,19 @@ __global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_consta
   const int64_t wpb = blockDim.x >> 5;
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
   const int64_t nwarps = (int64_t)gridDim.x * wpb;
-  for (int64_t sg = warp; sg < cl.n_seg; sg += nwarps) {
+  // work item = one of P equal slices of one segment (see scan_segments), one warp per item
+  const uint32_t n_seg = (uint32_t)cl.n_seg;
+  const uint32_t P = max(1u, (uint32_t)((4 * nwarps + n_seg - 1) / n_seg));
+  for (int64_t it = warp; it < (int64_t)n_seg * P; it += nwarps) {
+    const uint32_t sg = (uint32_t)(it % n_seg), part = (uint32_t)(it / n_seg);
     const uint32_t cnt = min(cl.seg_count[sg], cl.seg_cap);
+    const uint32_t per = ((cnt + P - 1u) / P + 31u) & ~31u;
+    const uint32_t b = part * per, e = min(cnt, b + per);
     const unsigned long long* seg = cl.cand + (size_t)sg * cl.seg_cap;
-    for (uint32_t j0 = 0; j0 < cnt; j0 += 32) {
+    for (uint32_t j0 = b; j0 < e; j0 += 32) {
       const uint32_t j = j0 + lane;
       uint32_t tag = 0xFFFFFFFFu;
-      if (j < cnt) {
+      if (j < e) {
         const unsigned long long k64 = __ldcs(seg + j);
         const uint32_t l = layer_of(w, 0xFFFFFFFFu - (uint32_t)k64);
         uint32_t d;
@@ -1324,7 +1360,7 @@ __global__ void __launch_bounds__(256) lsel_finish_cand_kernel(const __grid_cons
   const int64_t wpb = blockDim.x >> 5;
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
   const int64_t nwarps = (int64_t)gridDim.x * wpb;
-  scan_segments(cl.cand, cl.seg_count, cl.seg_cap, cl.n_seg, warp, nwarps, lane, [&](unsigned long long k64) {
+  scan_segments(cl.cand, cl.seg_count, cl.seg_cap, cl.n_seg, ~0ull, [&](unsigned long long k64) {
     const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64;
     const LayerState& S = w.layers[layer_of(w, i)];
     if (S.hit && k64 >= S.prefix) atomicOr(&next_bits[i >> 5], 1u << (i & 31));
