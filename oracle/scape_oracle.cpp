@@ -19,6 +19,8 @@
 //   P12 per-layer refresh vs brute force per layer; exactly k_l per layer; one layer == flat
 //   P13 an uncompressed layer is dense AdamS (Eq. 2) on its slice while the others are sparse
 //   P14 sparsity schedule: mask counts follow the schedule with the one-step delay; P6 still holds
+//   P15 workers: every layer's mask == brute force on ITS OWNER's |m-tilde|; the
+//       two-level sum equals the flat mean (double, 1e-15); W = R with one owner == the plain step
 // Unpinned by the paper (decisions): S3 clip_grad off by default and,
 // when switched on, the torch/Megatron rule; S4 bias correction off by default; S8 replica 0 owns
 // the statistic; S9 flat top-k by default, per-layer top-k with uncompressed
@@ -78,6 +80,15 @@ struct Oracle {
   // RMSNorm, bias: PAPER.md:246, :279, :286): all its entries are selected.  Empty = one layer.
   std::vector<int64_t> layer_off;
   std::vector<uint8_t> layer_compress;
+  // Workers ("N workers", §IV-A :178 "each worker only computes a portion of the
+  // top-k operations ... the new local masks from all workers are gathered"): the R replicas are
+  // `workers` groups of R/workers consecutive replicas (one group = the gradient buffers of one
+  // worker); layer l's statistic is the m-tilde of the FIRST replica of worker layer_owner[l]; the
+  // mean of l.10 is taken the way an all-reduce over workers takes it: each worker sums its own
+  // replicas in order, the workers' sums are added in worker order, one division by R.
+  // workers = 1 (default) is the plain reading S8 / S14.
+  int workers = 1;
+  std::vector<int32_t> layer_owner;
   // Sparsity used by the NEXT refresh (density warm-up: "exponentially decrease
   // density d from 1 to 0.1 or 0.01"; the schedule itself is the caller's).
   double sparsity_now = 0.0;
@@ -123,14 +134,17 @@ struct Oracle {
 
   static int64_t k_of(int64_t n, double sparsity) { return n - (int64_t)std::floor(sparsity * (double)n); }   // S6
 
-  // l.11 with the per-layer reading: refresh_mask inside every layer, at the current sparsity.
-  std::vector<uint8_t> refresh(const T* x) const {
-    if (layer_off.empty()) return topk_mask(x, N, k_of(N, sparsity_now));
+  // l.11 with the per-layer reading: refresh_mask inside every layer, at the current sparsity,
+  // from the statistic of the worker that owns the layer (worker 0 unless set_workers said otherwise).
+  std::vector<uint8_t> refresh(const std::vector<std::vector<T>>& x) const {
+    if (layer_off.empty()) return topk_mask(x[0].data(), N, k_of(N, sparsity_now));
     std::vector<uint8_t> mask(N, 0);
+    const int Rl = R / workers;
     for (size_t l = 0; l + 1 < layer_off.size(); ++l) {
       const int64_t a = layer_off[l], n = layer_off[l + 1] - a;
       if (!layer_compress[l]) { std::fill(mask.begin() + a, mask.begin() + a + n, (uint8_t)1); continue; }
-      std::vector<uint8_t> ml = topk_mask(x + a, n, k_of(n, sparsity_now));
+      const int owner = layer_owner.empty() ? 0 : layer_owner[l];
+      std::vector<uint8_t> ml = topk_mask(x[owner * Rl].data() + a, n, k_of(n, sparsity_now));
       std::copy(ml.begin(), ml.end(), mask.begin() + a);
     }
     return mask;
@@ -163,15 +177,20 @@ struct Oracle {
     // l.11: M_t <- refresh_mask(density, abs(m-tilde)) from the owner's (replica 0) statistic,
     // over all N positions (readings S8, S11).  Used from the next step on (§IV-A, :178).
     // With layers set: the same inside every layer.
-    std::vector<uint8_t> next = refresh(mt[0].data());
+    std::vector<uint8_t> next = refresh(mt);
 
     // l.10, l.12-17 on the mask.
     std::vector<T> m_new(N, (T)0);                       // l.12 / Eq. 4: zero off the mask
     bbar.assign(K, (T)0); ghat.assign(K, (T)0); v.assign(K, (T)0); u.assign(K, (T)0);
     for (int64_t j = 0; j < K; ++j) {
       const int64_t i = idx[j];
-      T s = b[0][j];                                     // l.10: sum over replicas, r ascending
-      for (int r = 1; r < R; ++r) s = s + b[r][j];
+      const int Rl = R / workers;                        // replicas per worker (R when workers = 1)
+      T s = (T)0;
+      for (int w = 0; w < workers; ++w) {                // l.10: all-reduce = sum of the workers' sums
+        T sw = b[w * Rl][j];                             //   one worker: its replicas, r ascending
+        for (int r = 1; r < Rl; ++r) sw = sw + b[w * Rl + r][j];
+        s = w == 0 ? sw : s + sw;
+      }
       T bb = s / (T)R;
       T p = beta1 * m[i];
       bbar[j] = bb;
@@ -263,6 +282,16 @@ template <class T> void copy_out(const std::vector<T>& v, T* dst) {
     if (L < 1 || off[0] != 0 || off[L] != o->N) return -1;                                          \
     for (int l = 0; l < L; ++l) if (off[l + 1] <= off[l]) return -1;                                \
     o->layer_off.assign(off, off + L + 1); o->layer_compress.assign(compress, compress + L);        \
+    o->layer_owner.clear();                                                                         \
+    return 0;                                                                                       \
+  }                                                                                                 \
+  extern "C" int oracle_set_workers_##SUF(void* h, int W, const int32_t* owner) {                  \
+    auto* o = (Oracle<T>*)h;                                                                        \
+    if (W < 1 || o->R % W != 0) return -1;                                                          \
+    const size_t L = o->layer_off.empty() ? 0 : o->layer_off.size() - 1;                            \
+    if (owner) { if (L == 0) return -1; for (size_t l = 0; l < L; ++l) if (owner[l] < 0 || owner[l] >= W) return -1; } \
+    o->workers = W;                                                                                 \
+    if (owner) o->layer_owner.assign(owner, owner + L); else o->layer_owner.clear();                \
     return 0;                                                                                       \
   }                                                                                                 \
   extern "C" int oracle_set_sparsity_##SUF(void* h, double s) {                                     \

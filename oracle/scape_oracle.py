@@ -81,6 +81,16 @@ class ScapeOracle:
         if fn(self.h, int(L), off.ctypes.data, cp.ctypes.data) != 0:
             raise ValueError("oracle_set_layers rejected the offsets")
 
+    def set_workers(self, workers, layer_owner=None):
+        """the R replicas are `workers` groups of R/workers replicas; layer l's
+        mask comes from worker layer_owner[l]'s statistic; l.10 sums per worker, then over workers."""
+        fn = self._f("set_workers")
+        fn.restype = ctypes.c_int
+        fn.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]
+        ow = None if layer_owner is None else np.ascontiguousarray(layer_owner, dtype=np.int32)
+        if fn(self.h, int(workers), None if ow is None else ow.ctypes.data) != 0:
+            raise ValueError("oracle_set_workers rejected the arguments")
+
     def set_sparsity(self, s):
         """Sparsity of the coming refreshes (density warm-up)."""
         fn = self._f("set_sparsity")

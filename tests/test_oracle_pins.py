@@ -549,3 +549,72 @@ def test_p14_sparsity_schedule_counts_delay_and_conservation_double():
         ebar = sum(o.e(r) for r in range(R)) / R
         np.testing.assert_allclose(c1 * sum_g, ebar + o.m() + c1 * sum_m_before, rtol=1e-10, atol=1e-14)
     assert want_prev == 15 + 64 + 32               # 5 % of 300 and of 636, all 64 of the uncompressed layer
+
+
+# ---------------------------------------------------------------------------------------------
+# P15 workers ("N workers"; §IV-A :178 "each worker only computes a portion of the
+# top-k operations ... the new local masks from all workers are gathered")
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("W,Rl", [(2, 1), (2, 2), (4, 1), (3, 2)])
+def test_p15_every_layer_follows_its_owner_and_the_two_level_mean(W, Rl):
+    rng = np.random.default_rng(1500 + 10 * W + Rl)
+    N, R, s = 400, W * Rl, 0.9
+    cuts = np.sort(rng.choice(np.arange(1, N), size=5, replace=False))
+    offsets = np.concatenate([[0], cuts, [N]])
+    compress = np.array([1, 1, 1, 0, 1, 1], np.uint8)
+    owner = np.array([l % W for l in range(6)], np.int32)
+    o = ScapeOracle(N, R, s, **HYP, dtype=np.float64)
+    o.set_layers(offsets, compress)
+    o.set_workers(W, owner)
+    th = 0.02 * rng.standard_normal(N)
+    for g in make_grads(rng, N, R, 5, dtype=np.float64):
+        # replicas that disagree strongly, so that the owner matters
+        g = [x * (1.0 + 3.0 * r) for r, x in enumerate(g)]
+        o.step(th, g)
+        mk = o.mask()
+        want = np.zeros(N, np.uint8)
+        for l in range(6):                       # brute force inside the layer on ITS OWNER's statistic
+            a, b = offsets[l], offsets[l + 1]
+            if not compress[l]:
+                want[a:b] = 1
+                continue
+            x = o.mt(int(owner[l]) * Rl)[a:b]
+            want[a:b] = brute_force_topk(x, (b - a) - int(np.floor(s * (b - a))))
+        np.testing.assert_array_equal(mk, want)
+        # l.10: the two-level sum is the mean over all R replicas
+        flat = np.mean(np.stack([o.b(r) for r in range(R)]), axis=0)
+        np.testing.assert_allclose(o.bbar(), flat, rtol=1e-12, atol=1e-18)   # sums may cancel
+    # a different owner gives a different mask (the pin has teeth)
+    assert not np.array_equal(want, layered_brute_force(o.mt(0), offsets, compress, s))
+
+
+def test_p15_one_worker_or_one_replica_per_worker_is_the_plain_step_fp32():
+    rng = np.random.default_rng(1515)
+    N, R, T = 500, 4, 5
+    offsets = [0, 100, 333, N]
+    grads = make_grads(rng, N, R, T)
+    th0 = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    plain = ScapeOracle(N, R, 0.9, **HYP); plain.set_layers(offsets)
+    one = ScapeOracle(N, R, 0.9, **HYP); one.set_layers(offsets); one.set_workers(1)
+    # R workers of one replica each, all layers owned by worker 0: the same left-to-right sum
+    per = ScapeOracle(N, R, 0.9, **HYP); per.set_layers(offsets); per.set_workers(R, [0, 0, 0])
+    tha, thb, thc = th0.copy(), th0.copy(), th0.copy()
+    for g in grads:
+        plain.step(tha, g); one.step(thb, g); per.step(thc, g)
+        for o in (one, per):
+            np.testing.assert_array_equal(o.mask(), plain.mask())
+            assert np.array_equal(o.bbar().view(np.uint32), plain.bbar().view(np.uint32))
+    assert np.array_equal(tha.view(np.uint32), thb.view(np.uint32))
+    assert np.array_equal(tha.view(np.uint32), thc.view(np.uint32))
+
+
+def test_p15_set_workers_rejects_bad_arguments():
+    o = ScapeOracle(64, 4, 0.5, **HYP)
+    with pytest.raises(ValueError):
+        o.set_workers(3)                         # R not divisible
+    with pytest.raises(ValueError):
+        o.set_workers(2, [0, 1])                 # owners need layers
+    o.set_layers([0, 32, 64])
+    with pytest.raises(ValueError):
+        o.set_workers(2, [0, 2])                 # owner out of range
+    o.set_workers(2, [1, 0])
