@@ -152,6 +152,40 @@ int scape_set_layers(scape_t* h, int n_layers, const int64_t* offsets, const uin
 int scape_set_sparsity(scape_t* h, double sparsity);
 int64_t scape_layer_k(const scape_t* h, int layer);
 
+/* Workers: the exchange step of Algorithm 1 across processes (not part of
+ * the north-star path, which sums R replicas inside one GPU).  PAPER.md:136 ("N workers"), :155
+ * (l.10: all-reduce of b), §IV-A :178 and Fig. 7 :218 ("each worker only computes a portion of the
+ * top-k operations ... the new local masks from all workers are gathered").
+ *   scape_set_workers   this handle is worker `rank` of `world`; every worker holds the whole
+ *                       shard (theta, m, masks are identical on all of them) and its own R gradient
+ *                       buffers and residuals.  layer_owner: HOST array of n_layers worker numbers
+ *                       (scape_set_layers first): worker layer_owner[l] refreshes the mask of layer
+ *                       l from ITS replica 0's statistic; NULL = this worker owns every layer (only
+ *                       with world = 1).  The mean of l.10 becomes the sum over all R * world
+ *                       replicas -- each worker's own replicas in order, then the workers' sums --
+ *                       divided by R * world.  Allocates 2 N floats once.  Synchronises the device.
+ *   scape_step_local    everything of a step that needs no other worker: l.6-9 for the local
+ *                       replicas, the local sums of l.10, theta off the mask (l.17 with u = 0), this
+ *                       worker's portion of the refresh (l.11).  Same arguments and rules as
+ *                       scape_step.  clip_grad is not available in this mode (SCAPE_EINVAL).
+ *   scape_exchange_buffers  what has to be summed over the workers before scape_step_apply, as
+ *                       DEVICE pointers owned by the handle: `sums` = n_sums floats (the local sum of
+ *                       m~^r at every selected position, in index order: the payload of l.10; an
+ *                       all-reduce SUM makes it the global sum), `mask_words` = n_mask_words uint32
+ *                       words of M_t in which only this worker's layers have bits (the portions are
+ *                       disjoint, so an integer all-reduce SUM, or an all-gather of word-aligned
+ *                       portions, completes the mask); n_mask_words = 0 when the sparsity is 0.
+ *                       Valid between scape_step_local and scape_step_apply.
+ *   scape_step_apply    l.10 (division), l.12-17 on the mask from the summed buffer, rank and index
+ *                       list of the completed M_t; advances t.  `param` as in scape_step_local.
+ * With world = 1 the pair step_local / step_apply computes exactly what scape_step computes.
+ * scape_step itself refuses a handle with world > 1.  scape_set_layers / scape_set_sparsity are
+ * refused between the two halves.                                                              */
+int scape_set_workers(scape_t* h, int world, int rank, const int32_t* layer_owner);
+int scape_step_local(scape_t* h, float* param, const void* const* grads, void* cuda_stream);
+int scape_exchange_buffers(scape_t* h, float** sums, int64_t* n_sums, uint32_t** mask_words, int64_t* n_mask_words);
+int scape_step_apply(scape_t* h, float* param, void* cuda_stream);
+
 /* Option: also materialise b^r on steps whose mask is all ones (step 1, or sparsity 0), where
  * the packed buffer would be R*N floats.  Off by default: on such steps SCAPE_PACKED is then
  * unavailable (SCAPE_EINVAL) and SCAPE_PACKED_MEAN equals SCAPE_MOMENT.  Allocates R*N floats

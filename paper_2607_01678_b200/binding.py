@@ -40,6 +40,10 @@ SYMBOLS = {
     "scape_set_layers": (_I, [_VP, _I, _VP, _VP]),
     "scape_set_sparsity": (_I, [_VP, _D]),
     "scape_layer_k": (_I64, [_VP, _I]),
+    "scape_set_workers": (_I, [_VP, _I, _I, _VP]),
+    "scape_step_local": (_I, [_VP, _VP, _VP, _VP]),
+    "scape_exchange_buffers": (_I, [_VP, _VP, _VP, _VP, _VP]),
+    "scape_step_apply": (_I, [_VP, _VP, _VP]),
     "scape_get": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
     "scape_set": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
     "scape_set_step_count": (_I, [_VP, _I64]),
@@ -51,6 +55,18 @@ SYMBOLS = {
 }
 
 _LIB = None
+
+
+def _device_view(ptr, n, dtype):
+    """torch tensor over n elements of device memory owned by the library (current device)."""
+    import torch
+
+    class _Mem:
+        pass
+    m = _Mem()
+    m.__cuda_array_interface__ = {"shape": (int(n),), "typestr": "<f4" if dtype == "float32" else "<i4",
+                                  "data": (int(ptr), False), "version": 3, "strides": None}
+    return torch.as_tensor(m, device="cuda")
 
 
 class ScapeError(RuntimeError):
@@ -161,6 +177,29 @@ def scape_set_layers(h, offsets, compress=None):
     _check(lib().scape_set_layers(h, n, off, cp), "scape_set_layers")
 
 
+def scape_set_workers(h, world, rank, layer_owner=None):
+    ow = None if layer_owner is None else np.ascontiguousarray(layer_owner, dtype=np.int32)
+    _check(lib().scape_set_workers(h, int(world), int(rank), None if ow is None else ow.ctypes.data), "scape_set_workers")
+
+
+def scape_step_local(h, param_ptr, grad_ptrs, stream=0):
+    arr = (ctypes.c_void_p * len(grad_ptrs))(*grad_ptrs)
+    _check(lib().scape_step_local(h, param_ptr, arr, stream), "scape_step_local")
+
+
+def scape_exchange_buffers(h):
+    """-> (sums device pointer, n_sums, mask words device pointer, n_mask_words)"""
+    ps, pw = ctypes.c_void_p(), ctypes.c_void_p()
+    ns, nw = ctypes.c_int64(), ctypes.c_int64()
+    _check(lib().scape_exchange_buffers(h, ctypes.byref(ps), ctypes.byref(ns), ctypes.byref(pw), ctypes.byref(nw)),
+           "scape_exchange_buffers")
+    return ps.value or 0, ns.value, pw.value or 0, nw.value
+
+
+def scape_step_apply(h, param_ptr, stream=0):
+    _check(lib().scape_step_apply(h, param_ptr, stream), "scape_step_apply")
+
+
 def scape_set_sparsity(h, sparsity):
     _check(lib().scape_set_sparsity(h, float(sparsity)), "scape_set_sparsity")
 
@@ -266,6 +305,41 @@ class Scape:
             assert g.is_cuda and g.is_contiguous() and g.numel() == self.N and g.dtype == grads[0].dtype
         self._set_dtype_for(grads[0])
         scape_step(self.h, param.data_ptr(), [g.data_ptr() for g in grads], self._stream())
+
+    # ---- workers: split step (include/scape.h "Workers") ---------------------------------
+    def set_workers(self, world, rank, layer_owner=None):
+        scape_set_workers(self.h, world, rank, layer_owner)
+
+    def step_local(self, param, grads):
+        import torch
+        assert param.is_cuda and param.dtype == torch.float32 and param.is_contiguous() and param.numel() == self.N
+        assert len(grads) == self.R
+        for g in grads:
+            assert g.is_cuda and g.is_contiguous() and g.numel() == self.N and g.dtype == grads[0].dtype
+        self._set_dtype_for(grads[0])
+        scape_step_local(self.h, param.data_ptr(), [g.data_ptr() for g in grads], self._stream())
+
+    def exchange_tensors(self):
+        """The two buffers to be summed over the workers, as torch views of the handle's device
+        memory (no copy): (float32 [n_sums], int32 [n_mask_words] or None)."""
+        ps, ns, pw, nw = scape_exchange_buffers(self.h)
+        sums = _device_view(ps, ns, "float32")
+        words = _device_view(pw, nw, "int32") if nw else None
+        return sums, words
+
+    def step_apply(self, param):
+        scape_step_apply(self.h, param.data_ptr(), self._stream())
+
+    def step_workers(self, param, grads, group=None):
+        """One step of worker `rank` of `world` (torch.distributed, NCCL): the local half, the two
+        all-reduces of PAPER.md:155 / :178 on the handle's own buffers, the apply half."""
+        import torch.distributed as dist
+        self.step_local(param, grads)
+        sums, words = self.exchange_tensors()
+        dist.all_reduce(sums, op=dist.ReduceOp.SUM, group=group)
+        if words is not None:
+            dist.all_reduce(words, op=dist.ReduceOp.SUM, group=group)      # disjoint portions: SUM == OR
+        self.step_apply(param)
 
     def step_host(self, param, grads):
         """param / grads: CPU tensors (pinned for async DMA). Synchronises before returning."""

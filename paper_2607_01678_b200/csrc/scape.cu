@@ -113,6 +113,15 @@ struct scape {
   int4* items = nullptr;
   int n_items = 0;
 
+  // workers (scape_set_workers): this handle is worker `rank` of `world`; the step is split into
+  // scape_step_local / [all-reduce of the exchange buffers] / scape_step_apply
+  int world = 1, rank = 0;
+  std::vector<uint8_t> lay_skip;  // host copy: layers whose mask another worker makes
+  bool pending = false;           // step_local has run, step_apply has not
+  bool pending_need_select = false;
+  int pending_pm_out = 0;
+  float pending_bc1 = 1.0f, pending_bc2 = 1.0f;
+
   // optional per-step CUDA-event timing of the fused kernel and of the select stage
   bool prof_on = false;
   static constexpr int kProfRing = 64;
@@ -284,7 +293,7 @@ int compact_mask(scape* h, MaskSlot& s, bool want_idx, cudaStream_t st) {
 // Stage 2 (Alg. 1 l.11): exact top-k of |m~^0| -> nxt.bits / rank / idx.  When the fused pass ran
 // with a predicted bracket (sparse step) the radix select works on its candidate list if the
 // bracket held; otherwise (or on all-ones steps: force_general) on every key of the partition.
-int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st) {
+int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st, bool compact = true) {
   KeySrc src;
   src.e0 = h->e;
   src.cur_bits = cur.all_ones ? nullptr : cur.bits;
@@ -308,6 +317,7 @@ int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general,
   sel_finish_kernel<<<grid, 256, 0, st>>>(src, cl, h->sel, nxt.bits);
   h->launches++;
   CU_TRY(cudaGetLastError());
+  if (!compact) return SCAPE_OK;
   int rc = compact_mask(h, nxt, true, st);
   if (rc) return rc;
   nxt.count = h->k;
@@ -375,7 +385,7 @@ int64_t total_k(const scape* h, double s) {
 }
 
 // Stage 2 with layers: the same exact select inside every layer at once.
-int run_select_layered(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st) {
+int run_select_layered(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st, bool compact = true) {
   KeySrc src;
   src.e0 = h->e;
   src.cur_bits = cur.all_ones ? nullptr : cur.bits;
@@ -405,6 +415,7 @@ int run_select_layered(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_
   h->launches++;
   if (!force_general) { lsel_finish_cand_kernel<<<grid_c, 256, 0, st>>>(w, cl, nxt.bits); h->launches++; }
   CU_TRY(cudaGetLastError());
+  if (!compact) return SCAPE_OK;          // workers: the other workers' bits are still missing (scape_step_apply)
   int rc = compact_mask(h, nxt, true, st);
   if (rc) return rc;
   nxt.count = h->k;
@@ -584,12 +595,12 @@ extern "C" int scape_set_bias_correction(scape_t* h, int on) {
 extern "C" int scape_set_clip_grad(scape_t* h, double max_norm) {
   if (!h || !(max_norm >= 0.0) || !std::isfinite(max_norm)) return fail(SCAPE_EINVAL, "max_norm must be finite and >= 0");
   DeviceGuard g(h->dev);
-  if (max_norm > 0.0 && !h->ghat) {
+  if (max_norm > 0.0 && (!h->ghat || !h->sumsq)) {
     const int slots = h->n_sm * 8 * 8;
-    bool ok = cudaMalloc((void**)&h->ghat, sizeof(float) * h->Npad) == cudaSuccess &&
-              cudaMalloc((void**)&h->vm, sizeof(float) * h->Npad) == cudaSuccess &&
-              cudaMalloc((void**)&h->sumsq, sizeof(double) * slots) == cudaSuccess &&
-              cudaMalloc((void**)&h->clip_state, sizeof(ClipState)) == cudaSuccess;
+    bool ok = (h->ghat || cudaMalloc((void**)&h->ghat, sizeof(float) * h->Npad) == cudaSuccess) &&
+              (h->vm || cudaMalloc((void**)&h->vm, sizeof(float) * h->Npad) == cudaSuccess) &&
+              (h->sumsq || cudaMalloc((void**)&h->sumsq, sizeof(double) * slots) == cudaSuccess) &&
+              (h->clip_state || cudaMalloc((void**)&h->clip_state, sizeof(ClipState)) == cudaSuccess);
     if (!ok) {
       cudaGetLastError();
       cudaFree(h->ghat); cudaFree(h->vm); cudaFree(h->sumsq); cudaFree(h->clip_state);
@@ -605,6 +616,7 @@ extern "C" int scape_set_clip_grad(scape_t* h, double max_norm) {
 extern "C" int scape_set_sparsity(scape_t* h, double sparsity) {
   if (!h) return fail(SCAPE_EINVAL, "NULL handle");
   if (!(sparsity >= 0.0 && sparsity < 1.0)) return fail(SCAPE_EINVAL, "sparsity must be in [0, 1)");
+  if (h->pending) return fail(SCAPE_EINVAL, "a split step is in flight");
   DeviceGuard g(h->dev);
   const int64_t K = total_k(h, sparsity);
   int rc = ensure_capacity(h, K);
@@ -616,6 +628,8 @@ extern "C" int scape_set_sparsity(scape_t* h, double sparsity) {
 
 extern "C" int scape_set_layers(scape_t* h, int n_layers, const int64_t* offsets, const uint8_t* compress) {
   if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (h->pending) return fail(SCAPE_EINVAL, "a split step is in flight");
+  if (h->world > 1) return fail(SCAPE_EINVAL, "this handle is one of %d workers: scape_set_workers(h, 1, 0, NULL) before changing the layers", h->world);
   DeviceGuard g(h->dev);
   CU_TRY(cudaDeviceSynchronize());
   if (n_layers == 0) {                       // back to one flat top-k
@@ -710,8 +724,18 @@ extern "C" int scape_set_step_count(scape_t* h, int64_t t) {
   return SCAPE_OK;
 }
 
-extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, void* cuda_stream) {
+namespace {
+
+// The step.  local = false: all of it (scape_step).  local = true (scape_step_local): everything
+// that needs no other worker -- l.6-9 for the local replicas, the local sums of l.10 parked for the
+// all-reduce, theta off the mask, this worker's share of the refresh (l.11) -- and the rest is left
+// to scape_step_apply.
+int step_impl(scape_t* h, float* param, const void* const* grads, void* cuda_stream, bool local) {
   if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (h->pending) return fail(SCAPE_EINVAL, "scape_step_local has run: call scape_step_apply first");
+  if (!local && h->world > 1) return fail(SCAPE_EINVAL, "this handle is one of %d workers: use scape_step_local / scape_step_apply", h->world);
+  if (local && h->clip_max_norm > 0.0) return fail(SCAPE_EINVAL, "clip_grad is not available with scape_step_local");
+  if (local && !h->ghat) return fail(SCAPE_EINVAL, "call scape_set_workers before scape_step_local");
   if (!param || !grads) return fail(SCAPE_EINVAL, "NULL param/grads");
   if ((uintptr_t)param & 15) return fail(SCAPE_EINVAL, "param must be 16-byte aligned");
   for (int r = 0; r < h->R; ++r) {
@@ -756,8 +780,8 @@ extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, vo
     p.bc1 = (float)(1.0 / (1.0 - std::pow(h->beta1_d, t)));
     p.bc2 = (float)(1.0 / (1.0 - std::pow(h->beta2_d, t)));
   }
-  const bool clip = h->clip_max_norm > 0.0;
-  p.clip = clip ? 1 : 0; p.ghat = h->ghat; p.vm = h->vm; p.sumsq = h->sumsq;
+  const bool clip = !local && h->clip_max_norm > 0.0;
+  p.clip = local ? 2 : clip ? 1 : 0; p.ghat = h->ghat; p.vm = h->vm; p.sumsq = h->sumsq;
   p.ctl = h->sel; p.next_bits = nxt.bits; p.cand = h->cand;
   p.seg_count = h->seg_count; p.seg_above = h->seg_above;
   if (h->n_layers > 0) { p.chunk_layer = h->chunk_layer; p.layers = h->layers; }
@@ -781,16 +805,121 @@ extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, vo
   if (prof) CU_TRY(cudaEventRecord(h->prof_ev[pi][1], st));
 
   if (need_select) {
-    rc = h->n_layers > 0 ? run_select_layered(h, cur, nxt, /*force_general=*/cur.all_ones, st)
-                         : run_select(h, cur, nxt, /*force_general=*/cur.all_ones, st);
+    // workers: an all-ones step does not write M_t in the fused pass, and the select only writes
+    // this worker's layers: the others' words must read zero for the exchange
+    if (local && cur.all_ones && h->n_layers > 0) CU_TRY(cudaMemsetAsync(nxt.bits, 0, sizeof(uint32_t) * h->n_words, st));
+    rc = h->n_layers > 0 ? run_select_layered(h, cur, nxt, /*force_general=*/cur.all_ones, st, /*compact=*/!local)
+                         : run_select(h, cur, nxt, /*force_general=*/cur.all_ones, st, /*compact=*/!local);
     if (rc) return rc;
     if (cur.all_ones) CU_TRY(cudaMemsetAsync(h->e, 0, sizeof(float) * h->Npad, st));   // l.8 for e^0 after the stash
-  } else {
+  } else if (!local) {
     nxt.all_ones = true; nxt.count = h->N; nxt.valid = true;                            // k = N: M_t = 1
   }
   if (prof) { CU_TRY(cudaEventRecord(h->prof_ev[pi][2], st)); h->prof_pending = pi + 1; }
+  if (local) {
+    h->pending = true; h->pending_pm_out = pm_out; h->pending_bc1 = p.bc1; h->pending_bc2 = p.bc2;
+    h->pending_need_select = need_select;
+    return SCAPE_OK;
+  }
   h->last_dense = cur.all_ones;
   if (!cur.all_ones) { h->m_sparse = true; h->pm_last = pm_out; }   // m_t = b-_t, addressed through `cur`
+  { const int old_last = h->last; h->last = h->use; h->use = h->build; h->build = old_last; }
+  h->t += 1;
+  return SCAPE_OK;
+}
+
+}  // namespace
+
+extern "C" int scape_step(scape_t* h, float* param, const void* const* grads, void* cuda_stream) {
+  return step_impl(h, param, grads, cuda_stream, /*local=*/false);
+}
+
+// ---- workers: PAPER.md:136 (N workers), :155 (all-reduce of b), :178 / :218 (each worker refreshes
+// ---- a portion of the mask, the portions are gathered)  --  SURVEY.md §8(f) rank 3
+extern "C" int scape_set_workers(scape_t* h, int world, int rank, const int32_t* layer_owner) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (world < 1 || rank < 0 || rank >= world) return fail(SCAPE_EINVAL, "need 0 <= rank < world");
+  if (h->pending) return fail(SCAPE_EINVAL, "a split step is in flight");
+  if (world > 1 && (h->n_layers == 0 || !layer_owner))
+    return fail(SCAPE_EINVAL, "more than one worker needs layers (scape_set_layers) and an owner per layer");
+  if (layer_owner && h->n_layers == 0) return fail(SCAPE_EINVAL, "layer owners need layers (scape_set_layers)");
+  if (layer_owner)
+    for (int l = 0; l < h->n_layers; ++l)
+      if (layer_owner[l] < 0 || layer_owner[l] >= world) return fail(SCAPE_EINVAL, "layer_owner[%d] out of range", l);
+  DeviceGuard g(h->dev);
+  CU_TRY(cudaDeviceSynchronize());
+  if (!h->ghat) {                      // exchange buffers: the local sums and m_old of the selected entries
+    if (cudaMalloc((void**)&h->ghat, sizeof(float) * h->Npad) != cudaSuccess ||
+        cudaMalloc((void**)&h->vm, sizeof(float) * h->Npad) != cudaSuccess) {
+      cudaGetLastError();
+      cudaFree(h->ghat); cudaFree(h->vm); h->ghat = h->vm = nullptr;
+      return fail(SCAPE_ENOMEM, "set_workers: allocation of 2 N floats failed");
+    }
+  }
+  if (h->n_layers > 0) {
+    std::vector<LayerState> ls((size_t)h->n_layers);
+    CU_TRY(cudaMemcpy(ls.data(), h->layers, sizeof(LayerState) * ls.size(), cudaMemcpyDeviceToHost));
+    h->lay_skip.assign((size_t)h->n_layers, 0);
+    for (int l = 0; l < h->n_layers; ++l) {
+      LayerState& S = ls[(size_t)l];
+      const int skip = layer_owner ? (layer_owner[l] != rank) : 0;
+      if (skip != S.skip) {            // ownership changed: forget the prediction
+        S.skip = skip;
+        S.br = Bracket{};
+        S.br.delta = 0.5f;
+        S.br.lo_key = S.br.hi_key = (skip || S.compress) ? 0xFFFFFFFFu : 0u;
+      }
+      h->lay_skip[(size_t)l] = (uint8_t)skip;
+    }
+    CU_TRY(cudaMemcpy(h->layers, ls.data(), sizeof(LayerState) * ls.size(), cudaMemcpyHostToDevice));
+  }
+  h->world = world; h->rank = rank;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_step_local(scape_t* h, float* param, const void* const* grads, void* cuda_stream) {
+  return step_impl(h, param, grads, cuda_stream, /*local=*/true);
+}
+
+extern "C" int scape_exchange_buffers(scape_t* h, float** sums, int64_t* n_sums, uint32_t** mask_words, int64_t* n_mask_words) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (!h->pending) return fail(SCAPE_EINVAL, "no split step is in flight (call scape_step_local first)");
+  const MaskSlot& cur = h->slot[h->use];
+  if (sums) *sums = h->ghat;
+  if (n_sums) *n_sums = cur.all_ones ? h->N : cur.count;
+  if (mask_words) *mask_words = h->pending_need_select ? h->slot[h->build].bits : nullptr;
+  if (n_mask_words) *n_mask_words = h->pending_need_select ? h->n_words : 0;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_step_apply(scape_t* h, float* param, void* cuda_stream) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (!param) return fail(SCAPE_EINVAL, "NULL param");
+  if (!h->pending) return fail(SCAPE_EINVAL, "no split step is in flight (call scape_step_local first)");
+  DeviceGuard guard(h->dev);
+  if (!guard.ok) return fail(SCAPE_ECUDA, "cannot select the handle's device");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  MaskSlot& cur = h->slot[h->use];
+  MaskSlot& nxt = h->slot[h->build];
+  const int pm_out = h->pending_pm_out;
+  const int64_t K = cur.all_ones ? h->N : cur.count;
+  const int Rt = h->R * h->world;
+  int g2 = (int)((K + 255) / 256); if (g2 > h->n_sm * 16) g2 = h->n_sm * 16; if (g2 < 1) g2 = 1;
+  dist_update_kernel<<<g2, 256, 0, st>>>(param, cur.all_ones ? nullptr : cur.idx, cur.all_ones ? h->m : h->pm[pm_out],
+                                         h->ghat, h->vm, K, (float)Rt, 1.0f / (float)Rt, (Rt & (Rt - 1)) == 0 ? 1 : 0,
+                                         h->b1, h->c1, h->b2, h->c2, h->eps, h->wd, -h->lr, h->pending_bc1, h->pending_bc2);
+  h->launches++;
+  CU_TRY(cudaGetLastError());
+  if (h->pending_need_select) {
+    int rc = compact_mask(h, nxt, true, st);       // M_t is complete now: rank128 + the index list
+    if (rc) return rc;
+    nxt.count = h->k; nxt.all_ones = false; nxt.valid = true;
+  } else {
+    nxt.all_ones = true; nxt.count = h->N; nxt.valid = true;
+  }
+  h->pending = false;
+  h->last_dense = cur.all_ones;
+  if (!cur.all_ones) { h->m_sparse = true; h->pm_last = pm_out; }
   { const int old_last = h->last; h->last = h->use; h->use = h->build; h->build = old_last; }
   h->t += 1;
   return SCAPE_OK;

@@ -63,7 +63,7 @@ struct LayerState {
   unsigned long long himask;
   long long rank;
   int top;                    // bits [0, top) of K64 still undecided; 0 = T64 complete
-  int pad;
+  int skip;                   // workers: another worker makes this layer's mask (scape_set_workers); no bit is set here
   unsigned long long n_above; // certainly-selected entries counted by the fused pass (reset by lsel_decide)
   Bracket br;
 };
@@ -101,6 +101,9 @@ struct StepParams {
   float bc1, bc2;               // bias-correction factors 1/(1-beta^t); 1.0f when off
   // l.14 clip_grad (optional): the pass stores g^ and beta2*m^2 of every selected entry, sums g^^2
   // in double, and leaves theta on the mask alone; clip_update_kernel finishes l.14-17 there
+  // clip = 2 (workers, scape_step_local): the mean of l.10 needs the other workers' sums first, so
+  // the pass parks the LOCAL sum over its replicas in ghat and m_old in vm, and leaves theta on the
+  // mask to dist_update_kernel (scape_step_apply), which runs after the all-reduce
   int clip;
   float* ghat;                  // [K] packed
   float* vm;                    // [K] packed
@@ -268,8 +271,11 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
         // l.14 needs the norm of g^ over the whole mask first: park what l.15-17 need; theta of
         // this entry is updated by clip_update_kernel
         if (!GUARD || i0 + q < p.N) {
-          p.ghat[i0 + q] = gh; p.vm[i0 + q] = vmq;
-          sa.sumsq += (double)gh * (double)gh;
+          if (p.clip == 2) { p.ghat[i0 + q] = s; p.vm[i0 + q] = mo[q]; }
+          else {
+            p.ghat[i0 + q] = gh; p.vm[i0 + q] = vmq;
+            sa.sumsq += (double)gh * (double)gh;
+          }
         }
       } else {
         const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), vmq);                              // l.15
@@ -325,8 +331,11 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
             const float vmq = __fmul_rn(p.b2, __fmul_rn(mo[q], mo[q]));
             p.packed_mean[j] = bb;                                                              // l.12: m_t = b-
             if (deferred) {
-              p.ghat[j] = gh; p.vm[j] = vmq;
-              sa.sumsq += (double)gh * (double)gh;
+              if (p.clip == 2) { p.ghat[j] = sm; p.vm[j] = mo[q]; }
+              else {
+                p.ghat[j] = gh; p.vm[j] = vmq;
+                sa.sumsq += (double)gh * (double)gh;
+              }
             } else {
               const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), vmq);                          // l.15
               u = __fdiv_rn(__fmul_rn(bb, p.bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, p.bc2)), p.eps));   // l.16 (+ :77)
@@ -369,8 +378,11 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
         const float vmq = __fmul_rn(p.b2, __fmul_rn(mq, mq));
         p.packed_mean[r0 + l] = bb;                                                           // l.12: m_t = b-
         if (deferred) {
-          p.ghat[r0 + l] = gh; p.vm[r0 + l] = vmq;
-          sa.sumsq += (double)gh * (double)gh;
+          if (p.clip == 2) { p.ghat[r0 + l] = sm; p.vm[r0 + l] = mq; }
+          else {
+            p.ghat[r0 + l] = gh; p.vm[r0 + l] = vmq;
+            sa.sumsq += (double)gh * (double)gh;
+          }
         } else {
           const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), vmq);                            // l.15
           scs[l] = __fdiv_rn(__fmul_rn(bb, p.bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, p.bc2)), p.eps));   // l.16 (+ :77)
@@ -532,7 +544,7 @@ __global__ void __launch_bounds__(256, ((!DENSE && R <= 2) ? 4 : R <= 4 ? 3 : 2)
     for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
     if (lane == 0) { p.seg_count[warp] = sa.cursor; p.seg_above[warp] = na; }
   }
-  if (CLIPT && p.clip) warp_store_sumsq(p, sa, warp, lane);
+  if (CLIPT && p.clip == 1) warp_store_sumsq(p, sa, warp, lane);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -758,7 +770,7 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
   if (lane == 0) { p.seg_count[gwarp] = sa.cursor; p.seg_above[gwarp] = na; }
-  if (CLIPT && p.clip) warp_store_sumsq(p, sa, gwarp, lane);
+  if (CLIPT && p.clip == 1) warp_store_sumsq(p, sa, gwarp, lane);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1156,6 +1168,10 @@ __global__ void __launch_bounds__(1024) lsel_decide_kernel(LayerWork w, CandList
     const long long a = (long long)S.n_above;
     S.n_above = 0;
     S.k = k;
+    if (S.skip) {            // not this worker's layer: nothing to find, no bit to set (its bracket stays "none")
+      S.hit = 1; S.rank = 0; S.top = 0; S.prefix = ~0ull; S.himask = ~0ull;
+      continue;
+    }
     const bool predicted = !(S.br.lo_key == 0xFFFFFFFFu && S.br.hi_key == 0xFFFFFFFFu);
     const bool hit = !force_general && !s_over && predicted && a <= k;
     S.hit = hit ? 1 : 0;
@@ -1502,6 +1518,29 @@ __global__ void __launch_bounds__(256) clip_update_kernel(float* __restrict__ th
 }
 
 // scatter / gather helpers for the dense <-> packed views used by the accessors
+// Workers ("all-reduce", §8(f) rank 3): l.10 and l.12-17 for the K selected entries once
+// the workers' sums have been added up.  S[j] = sum over ALL R_total replicas of m~^r at idx[j]
+// (each worker's own replicas in order, then the workers: the oracle's two-level sum), mold[j] =
+// m_{t-1} there.  Same pinned operation order as fused_compute.  idx == nullptr: all-ones step.
+__global__ void __launch_bounds__(256) dist_update_kernel(float* __restrict__ theta, const int32_t* __restrict__ idx,
+                                                         float* __restrict__ m_out, const float* __restrict__ S,
+                                                         const float* __restrict__ mold, int64_t K, float R_f, float inv_R,
+                                                         int r_pow2, float b1, float c1, float b2, float c2, float eps, float wd,
+                                                         float neg_lr, float bc1, float bc2) {
+  for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < K; j += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t i = idx ? (int64_t)idx[j] : j;
+    const float sm = S[j], mo = mold[j];
+    const float pq = __fmul_rn(b1, mo);
+    const float bb = r_pow2 ? __fmul_rn(sm, inv_R) : __fdiv_rn(sm, R_f);                      // l.10
+    const float gh = __fdiv_rn(__fsub_rn(bb, pq), c1);                                         // l.13 (Eq. 3)
+    const float v = __fmaf_rn(c2, __fmul_rn(gh, gh), __fmul_rn(b2, __fmul_rn(mo, mo)));      // l.15
+    const float u = __fdiv_rn(__fmul_rn(bb, bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, bc2)), eps));   // l.16 (+ :77)
+    const float th = theta[i];
+    theta[i] = __fmaf_rn(neg_lr, __fmaf_rn(wd, th, u), th);                                   // l.17
+    m_out[j] = bb;                                                                             // l.12: m_t = b- (packed, or dense when idx == nullptr)
+  }
+}
+
 __global__ void fill_u32_kernel(uint32_t* p, int64_t n, uint32_t v) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) p[i] = v;
 }

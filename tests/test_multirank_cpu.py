@@ -53,3 +53,80 @@ def test_single_rank_helpers():
     import bench
     assert bench.max_over_ranks_ms(7.5, 1, torch.device("cpu")) == 7.5
     assert bench.whole_job_value(10, 2, 1000.0, 1) == 20.0
+
+
+# ---------------------------------------------------------------------------------------------
+# Workers mode (include/scape.h "Workers"): the host-side protocol on two gloo ranks.  The kernels
+# need a GPU (tests/test_gpu_workers.py); what runs here is everything around them: every rank
+# derives the same layer owners, the mask portions the owners produce are disjoint, and the
+# integer all-reduce SUM the binding uses for them is a bitwise OR.
+# ---------------------------------------------------------------------------------------------
+WORKER_PROTOCOL = r"""
+import os, sys
+sys.path.insert(0, os.environ["SCAPE_ROOT"])
+import numpy as np, torch, torch.distributed as dist
+from paper_2607_01678_b200 import workers
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+sizes = [1000, 1, 5, 127, 129, 4099, 64, 20011, 2]
+owner = workers.balance_layers(sizes, world)
+got = [None] * world
+dist.all_gather_object(got, owner)
+assert all(g == owner for g in got), got                      # the same decision on every rank
+offsets = np.concatenate([[0], np.cumsum(sizes)])
+N = int(offsets[-1])
+rng = np.random.default_rng(7)                                # same stream on both ranks
+full = rng.integers(0, 2, N).astype(np.uint8)                 # a "true" M_t
+mine = np.zeros(N, np.uint8)
+for l, o in enumerate(owner):
+    if o == rank:
+        mine[offsets[l]:offsets[l + 1]] = full[offsets[l]:offsets[l + 1]]
+pad = (-N) % 32
+bits = np.packbits(np.concatenate([mine, np.zeros(pad, np.uint8)]), bitorder="little").view(np.uint32)
+words = torch.from_numpy(bits.view(np.int32).copy())
+dist.all_reduce(words, op=dist.ReduceOp.SUM)                  # disjoint portions: SUM == OR
+out = np.unpackbits(words.numpy().view(np.uint8), bitorder="little")[:N]
+assert np.array_equal(out, full)
+# the word ranges a rank may touch cover its layers and nothing is lost when only those are exchanged
+rngs = workers.owned_word_ranges(offsets, owner, rank)
+cover = np.zeros(bits.size, bool)
+for a, b in rngs:
+    cover[a:b] = True
+assert not bits[~cover].any()
+sums = torch.full((5,), float(rank + 1))
+dist.all_reduce(sums, op=dist.ReduceOp.SUM)
+assert float(sums[0]) == sum(range(1, world + 1))
+dist.barrier()
+dist.destroy_process_group()
+print("ok", rank)
+"""
+
+
+def test_two_gloo_ranks_workers_protocol():
+    port = free_port()
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), WORLD_SIZE="2", LOCAL_RANK=str(r), MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port), SCAPE_ROOT=ROOT)
+        procs.append(subprocess.Popen([sys.executable, "-c", WORKER_PROTOCOL], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.STDOUT, text=True))
+    outs = [p.communicate(timeout=180)[0] for p in procs]
+    for p, o in zip(procs, outs):
+        assert p.returncode == 0, o
+        assert "ok" in o
+
+
+def test_balance_layers_is_even_and_deterministic():
+    sys.path.insert(0, ROOT)
+    from paper_2607_01678_b200 import workers
+    sizes = [50257 * 1024, 1024 * 1024] + [3072 * 1024, 1024 * 1024, 4096 * 1024, 4096 * 1024] * 24
+    for world in (1, 2, 4, 8, 64):
+        owner = workers.balance_layers(sizes, world)
+        assert owner == workers.balance_layers(list(sizes), world)
+        load = [0] * world
+        for s, o in zip(sizes, owner):
+            load[o] += s
+        assert max(load) - min(load) <= max(sizes)            # within one (largest) layer of even
+    assert workers.owned_word_ranges([0, 40, 64, 100], [0, 1, 0], 0) == [(0, 4)]
+    assert workers.owned_word_ranges([0, 40, 64, 100], [0, 1, 0], 1) == [(1, 2)]
+    assert workers.owned_word_ranges([0, 64, 640, 700], [0, 1, 0], 0) == [(0, 2), (20, 22)]
