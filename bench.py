@@ -47,6 +47,13 @@ def parse():
     ap.add_argument("--cpu-div", type=int, default=64, help="oracle sample: every tensor this many times smaller")
     ap.add_argument("--cpu-steps", type=int, default=3)
     ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--layers", action="store_true",
+                    help="per-layer refresh (scape_set_layers: one top-k per tensor of the workload, PAPER.md:89, :138) instead of "
+                         "the north star's flat top-k")
+    ap.add_argument("--workers", action="store_true",
+                    help="workers mode (include/scape.h 'Workers', not the north-star path): every rank holds the whole shard and its "
+                         "own R gradient buffers, per-layer refresh split over the ranks, NCCL all-reduce of the k local sums and of the "
+                         "mask words between scape_step_local and scape_step_apply")
     ap.add_argument("--sweep", default=None, metavar="CSV",
                     help="run BASELINE.json config 5 (sizes 2^20..2^30 x sparsity x R, Gaussian grads) and write one CSV row per point")
     ap.add_argument("--sweep-log2n", default="20,21,22,23,24,25,26,27,28,29,30")
@@ -297,6 +304,9 @@ def main():
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    elif args.workers:                      # a world of one: the same NCCL calls, nothing to wait for
+        dist.init_process_group("nccl", init_method="file://" + tempfile.mktemp(prefix="scape_pg_"), rank=0, world_size=1,
+                                device_id=torch.device("cuda", local))
     binding.lib()
 
     w = get_workload(args)
@@ -307,19 +317,29 @@ def main():
     # ---- inputs resident in HBM before the timed region --------------------------------
     gs = synth.GradStream(w, device=dev, seed=args.seed + rank)
     theta = gs.theta0()
+    if args.workers and world > 1:          # every worker holds the same parameters
+        theta = synth.GradStream(w, device=dev, seed=args.seed).theta0()
     n_sets = max(1, min(args.sets, K + W + 1))
     ring = [gs.next() for _ in range(n_sets)]
     del gs
     torch.cuda.empty_cache()
 
     sc = binding.Scape(N, R, w.sparsity, **w.hyper)
+    step = sc.step
+    if args.layers and not args.workers:
+        sc.set_layers(w.offsets(), w.compress_flags())
+    if args.workers:
+        from paper_2607_01678_b200 import workers as wk
+        sc.set_layers(w.offsets(), w.compress_flags())          # per-layer refresh, one layer per tensor
+        sc.set_workers(world, rank, wk.balance_layers([n for _, n in w.tensors], world))
+        step = sc.step_workers
     k = sc.k
     # the first step of Alg. 1 is dense (M_0 = 1): always warm-up, reported separately
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(); sc.step(theta, ring[0]); e1.record(); torch.cuda.synchronize()
+    e0.record(); step(theta, ring[0]); e1.record(); torch.cuda.synchronize()
     first_step_ms = e0.elapsed_time(e1)
     for i in range(W):
-        sc.step(theta, ring[(1 + i) % n_sets])
+        step(theta, ring[(1 + i) % n_sets])
     torch.cuda.synchronize()
 
     if world > 1:
@@ -334,7 +354,7 @@ def main():
     t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t0.record()
     for i in range(K):
-        sc.step(theta, ring[(1 + W + i) % n_sets])
+        step(theta, ring[(1 + W + i) % n_sets])
     t1.record()
     torch.cuda.synchronize()
     elapsed_ms = t0.elapsed_time(t1)
@@ -352,7 +372,8 @@ def main():
     assert mask_count == k, (mask_count, k)
 
     ms_per_step = elapsed_ms / K
-    value = whole_job_value(N, K, elapsed_ms, world)
+    # replicas: every rank updates its own copy of the shard; workers: the ranks update ONE shard together
+    value = whole_job_value(N, K, elapsed_ms, 1 if args.workers else world)
 
     # ---- roofline of the dominant kernel -------------------------------------------------
     peak, peak_src = measured_peak()
@@ -378,7 +399,7 @@ def main():
 
     # ---- end to end through the C-ABI with HOST buffers ---------------------------------------
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not args.workers:
         gs = synth.GradStream(w, device=dev, seed=args.seed + rank)
         th_h = gs.theta0().cpu().pin_memory()
         g_h = [g.cpu().pin_memory() for g in gs.next()]
@@ -422,12 +443,15 @@ def main():
             "config": {"workload": w.name, "shard_numel": N, "R": R, "sparsity": w.sparsity, "k": k,
                        "grad_dtype": w.grad_dtype, "dist": w.dist, "ar1_rho": w.rho, "hyper": w.hyper,
                        "gradient_sets_cycled": n_sets, "l2": "inputs (tens of GB) exceed the 126 MB L2; no flush needed",
-                       "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU",
+                       "parallelism": (f"workers: {world} rank(s) x {R} replicas, per-layer refresh split over the ranks, NCCL all-reduce "
+                                       f"of {k} fp32 sums + {(N + 31) // 32} mask words per step") if args.workers else
+                                      "replicas only (no sharding, no collective)" if world > 1 else "single GPU",
+                       "refresh": "per layer (one top-k per tensor)" if (args.layers or args.workers) else "flat top-k over the shard",
                        "first_dense_step_ms": first_step_ms},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": gpu_launches, "clocks": clk,
         }
         print(json.dumps(line), flush=True)
-    if world > 1:
+    if world > 1 or args.workers:
         dist.destroy_process_group()
 
 

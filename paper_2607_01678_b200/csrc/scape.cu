@@ -16,6 +16,8 @@
 
 using namespace scapek;
 
+static_assert(scapek::SCAPE_MAX_LAYERS_K == SCAPE_MAX_LAYERS, "layer-end table of the select kernels");
+
 namespace {
 
 thread_local char g_err[512] = "";
@@ -80,7 +82,7 @@ struct scape {
   float* vm = nullptr;         // [Npad] clip mode: beta2 * m_old^2 of the selected entries
   double* sumsq = nullptr;     // [max_seg] clip mode: per-warp partial sums of g^^2
   ClipState* clip_state = nullptr;
-  uint32_t compact_min = 3;    // SCAPE_COMPACT_MIN (experiments)
+  uint32_t compact_min = 1;    // selected entries per chunk from which l.10-16 run compacted (SCAPE_COMPACT_MIN: experiments)
   int fused_impl = 0;          // SCAPE_FUSED_IMPL (experiments): 0 auto, 1 "ldg" = register-staged kernel only
   bool m_sparse = false;       // m_{t-1} lives in pm[pm_last] addressed through slot[last]; h->m is stale
   float* dense_pack = nullptr;    // optional [R][Npad]
@@ -399,7 +401,7 @@ int run_select_layered(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_
   LayerWork w;
   w.chunk_layer = h->chunk_layer; w.layers = h->layers; w.n_layers = h->n_layers; w.ctl = h->lctl;
   w.hist = h->lhist; w.items = h->items; w.n_items = h->n_items;
-  const int grid_c = h->n_sm * 2;
+  const int grid_c = h->n_sm * 6;      // 6 CTAs of 256 threads per SM (the 32 KB layer-end table bounds it)
   int grid_f = h->n_sm * 6; if (grid_f > h->n_items) grid_f = h->n_items;
   lsel_decide_kernel<<<1, 1024, 0, st>>>(w, cl, h->sparsity, force_general ? 1 : 0);
   h->launches++;

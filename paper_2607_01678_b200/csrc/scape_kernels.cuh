@@ -65,6 +65,7 @@ struct LayerState {
   int top;                    // bits [0, top) of K64 still undecided; 0 = T64 complete
   int skip;                   // workers: another worker makes this layer's mask (scape_set_workers); no bit is set here
   unsigned long long n_above; // certainly-selected entries counted by the fused pass (reset by lsel_decide)
+  unsigned long long base;    // candidate route: the radix passes run on K64 - base (base = lo_key << 32); 0 otherwise
   Bracket br;
 };
 
@@ -75,6 +76,11 @@ struct LayerCtl {
   float shrink;               // > 0: the candidate list was more than half full, narrow every bracket
   int pad;
   unsigned long long n_fast, n_general;   // layer-steps on each route (statistics)
+  // small list: once the surviving classes of all candidate-route layers together hold at most
+  // kClsCap keys, the next pass copies them out and the remaining passes read only that list
+  unsigned long long cls_total; // keys in the classes the last picks chose (candidate-route layers)
+  unsigned int cls_n;           // entries in the small list
+  int use_cls;                  // the small list is complete: read it instead of the segments
 };
 
 struct StepParams {
@@ -1127,6 +1133,23 @@ struct LayerWork {
   int n_items;
 };
 constexpr int kItemChunks = 2048;
+constexpr int SCAPE_MAX_LAYERS_K = 4096;           // == SCAPE_MAX_LAYERS (include/scape.h; static_assert in scape.cu)
+
+// Layer of element i by binary search over the layer ends held in shared memory (the candidate
+// lists are visited in an order that makes the chunk_layer table, N/32 bytes, a stream of L2
+// misses: one random 4-byte load per candidate; the ends are at most 32 KB and stay on chip).
+__device__ __forceinline__ void load_layer_ends(const LayerWork& w, long long* ends) {
+  for (int l = threadIdx.x; l < w.n_layers; l += blockDim.x) ends[l] = w.layers[l].end;
+  __syncthreads();
+}
+__device__ __forceinline__ uint32_t layer_of_sorted(const long long* ends, int n_layers, uint32_t i) {
+  int lo = 0, hi = n_layers - 1;                   // first l with ends[l] > i
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (ends[mid] > (long long)i) hi = mid; else lo = mid + 1;
+  }
+  return (uint32_t)lo;
+}
 
 __device__ __forceinline__ uint32_t layer_of(const LayerWork& w, uint32_t i) {
   const uint32_t cl = __ldg(w.chunk_layer + (i >> 7));
@@ -1158,6 +1181,7 @@ __global__ void __launch_bounds__(1024) lsel_decide_kernel(LayerWork w, CandList
     w.ctl->overflow = s_over;
     w.ctl->shrink = (!force_general && cap > 0 && 2ull * c > cap) ? (float)cap / (2.0f * (float)c) : 0.0f;
     w.ctl->any_general = 0;
+    w.ctl->cls_total = 0; w.ctl->cls_n = 0; w.ctl->use_cls = 0;
   }
   __syncthreads();
   unsigned long long nf = 0, ng = 0;
@@ -1169,7 +1193,7 @@ __global__ void __launch_bounds__(1024) lsel_decide_kernel(LayerWork w, CandList
     S.n_above = 0;
     S.k = k;
     if (S.skip) {            // not this worker's layer: nothing to find, no bit to set (its bracket stays "none")
-      S.hit = 1; S.rank = 0; S.top = 0; S.prefix = ~0ull; S.himask = ~0ull;
+      S.hit = 1; S.rank = 0; S.top = 0; S.prefix = ~0ull; S.himask = ~0ull; S.base = 0;
       continue;
     }
     const bool predicted = !(S.br.lo_key == 0xFFFFFFFFu && S.br.hi_key == 0xFFFFFFFFu);
@@ -1178,19 +1202,19 @@ __global__ void __launch_bounds__(1024) lsel_decide_kernel(LayerWork w, CandList
     if (hit) {
       nf += 1;
       S.rank = k - a;                                  // still to be found among the layer's candidates
+      S.base = 0;
       if (S.rank == 0) { S.top = 0; S.prefix = ~0ull; S.himask = ~0ull; }     // nothing more to select
       else {
-        // every candidate of the layer lies in [lo_key, hi_key): start below the bits they share
-        const uint32_t lo = S.br.lo_key, diff = lo ^ (S.br.hi_key - 1u);
-        const int common = diff ? __clz(diff) : 32;
-        const uint32_t km = common == 0 ? 0u : common >= 32 ? 0xFFFFFFFFu : ~(0xFFFFFFFFu >> common);
-        S.himask = (unsigned long long)km << 32;
-        S.prefix = (unsigned long long)(lo & km) << 32;
-        S.top = 64 - common;
+        // every candidate of the layer lies in [lo_key, hi_key): the passes run on K64 - (lo_key << 32)
+        // and start at the top of that difference (see sel_decide_kernel)
+        const uint32_t lo = S.br.lo_key, span1 = S.br.hi_key - 1u - lo;
+        S.base = (unsigned long long)lo << 32;
+        S.himask = 0; S.prefix = 0;
+        S.top = 32 + (span1 ? 32 - __clz(span1) : 0);
       }
     } else {
       ng += 1;
-      S.rank = k; S.top = 64; S.prefix = 0; S.himask = 0;
+      S.rank = k; S.top = 64; S.prefix = 0; S.himask = 0; S.base = 0;
       atomicOr(&w.ctl->any_general, 1);
       if (!force_general && s_over && S.compress) S.br.delta = fmaxf(S.br.delta * 0.5f, 0.03f);
     }
@@ -1201,9 +1225,10 @@ __global__ void __launch_bounds__(1024) lsel_decide_kernel(LayerWork w, CandList
 
 __device__ __forceinline__ bool layer_digit(const LayerState& S, unsigned long long k64, uint32_t& d) {
   const int top = S.top;
-  if (top <= 0 || (k64 & S.himask) != S.prefix) return false;
+  const unsigned long long kr = k64 - S.base;
+  if (top <= 0 || (kr & S.himask) != S.prefix) return false;
   const int bits = top < kDigitBits ? top : kDigitBits;
-  d = (uint32_t)(k64 >> (top - bits)) & ((1u << bits) - 1u);
+  d = (uint32_t)(kr >> (top - bits)) & ((1u << bits) - 1u);
   return true;
 }
 
@@ -1211,10 +1236,39 @@ __device__ __forceinline__ bool layer_digit(const LayerState& S, unsigned long l
 // handful of bins in the first pass, so equal (layer, digit) pairs of a warp are merged before the
 // global atomic.
 __global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_constant__ LayerWork w, const __grid_constant__ CandList cl) {
+  __shared__ long long ends[SCAPE_MAX_LAYERS_K];
+  load_layer_ends(w, ends);
   const int lane = threadIdx.x & 31;
   const int64_t wpb = blockDim.x >> 5;
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
   const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  // small list (LayerCtl): nobody changes these two fields while this kernel runs, so every CTA
+  // takes the same decision; lsel_hist_full_kernel's bookkeeping repeats it afterwards
+  const bool use_cls = w.ctl->use_cls != 0;
+  const unsigned long long ctot = w.ctl->cls_total;
+  const bool collect = !use_cls && ctot > 0 && ctot <= (unsigned long long)kClsCap;
+  // one warp-wide step: 32 keys (ok = this lane has one), equal (layer, digit) pairs merged
+  auto visit32 = [&](bool ok, unsigned long long k64) {
+    uint32_t tag = 0xFFFFFFFFu;
+    if (ok) {
+      const uint32_t l = layer_of_sorted(ends, w.n_layers, 0xFFFFFFFFu - (uint32_t)k64);
+      uint32_t d;
+      if (w.layers[l].hit && layer_digit(w.layers[l], k64, d)) {
+        tag = (l << kDigitBits) | d;
+        if (collect) { const uint32_t pos = atomicAdd(&w.ctl->cls_n, 1u); if (pos < kClsCap) cl.cls[pos] = k64; }
+      }
+    }
+    const uint32_t same = __match_any_sync(0xFFFFFFFFu, tag);
+    if (tag != 0xFFFFFFFFu && (__ffs(same) - 1) == lane) atomicAdd(&w.hist[tag], (uint32_t)__popc(same));
+  };
+  if (use_cls) {
+    const uint32_t n = min(w.ctl->cls_n, kClsCap);
+    for (int64_t j0 = warp * 32; j0 < (int64_t)n; j0 += nwarps * 32) {
+      const int64_t j = j0 + lane;
+      visit32(j < (int64_t)n, j < (int64_t)n ? cl.cls[j] : 0ull);
+    }
+    return;
+  }
   // work item = one of P equal slices of one segment (see scan_segments), one warp per item
   const uint32_t n_seg = (uint32_t)cl.n_seg;
   const uint32_t P = max(1u, (uint32_t)((4 * nwarps + n_seg - 1) / n_seg));
@@ -1226,15 +1280,7 @@ __global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_consta
     const unsigned long long* seg = cl.cand + (size_t)sg * cl.seg_cap;
     for (uint32_t j0 = b; j0 < e; j0 += 32) {
       const uint32_t j = j0 + lane;
-      uint32_t tag = 0xFFFFFFFFu;
-      if (j < e) {
-        const unsigned long long k64 = __ldcs(seg + j);
-        const uint32_t l = layer_of(w, 0xFFFFFFFFu - (uint32_t)k64);
-        uint32_t d;
-        if (w.layers[l].hit && layer_digit(w.layers[l], k64, d)) tag = (l << kDigitBits) | d;
-      }
-      const uint32_t same = __match_any_sync(0xFFFFFFFFu, tag);
-      if (tag != 0xFFFFFFFFu && (__ffs(same) - 1) == lane) atomicAdd(&w.hist[tag], (uint32_t)__popc(same));
+      visit32(j < e, j < e ? __ldcs(seg + j) : 0ull);
     }
   }
 }
@@ -1242,6 +1288,13 @@ __global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_consta
 // Digit histograms of the layers on the general route: every key of the layer, item by item.
 __global__ void __launch_bounds__(256) lsel_hist_full_kernel(const __grid_constant__ KeySrc s, const __grid_constant__ LayerWork w) {
   __shared__ uint32_t h[kBins];
+  // Bookkeeping of the small list, between the candidate pass that just ran and the picks that
+  // follow: a pass that was collecting has completed the list; the class sizes are summed afresh.
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    const unsigned long long ctot = w.ctl->cls_total;
+    if (!w.ctl->use_cls && ctot > 0 && ctot <= (unsigned long long)kClsCap) w.ctl->use_cls = 1;   // the pass before this copied them
+    w.ctl->cls_total = 0;
+  }
   if (!w.ctl->any_general) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, wpb = blockDim.x >> 5;
   for (int it = blockIdx.x; it < w.n_items; it += gridDim.x) {
@@ -1309,7 +1362,7 @@ __global__ void __launch_bounds__(1024) lsel_pick_kernel(LayerWork w) {
     // only possible on the candidate route, first pass: fewer candidates than entries still to
     // select, i.e. the true threshold lies below the bracket
     if (t == 0) {
-      S.hit = 0; S.rank = S.k; S.top = 64; S.prefix = 0; S.himask = 0;
+      S.hit = 0; S.rank = S.k; S.top = 64; S.prefix = 0; S.himask = 0; S.base = 0;
       atomicOr(&w.ctl->any_general, 1);
       atomicAdd(&w.ctl->n_general, 1ull);
       atomicAdd(&w.ctl->n_fast, ~0ull);              // - 1
@@ -1322,11 +1375,13 @@ __global__ void __launch_bounds__(1024) lsel_pick_kernel(LayerWork w) {
     for (int q = 0; q < PER; ++q) {
       if (cum < rank && rank <= cum + hv[q]) {
         const unsigned long long d = (unsigned long long)(topb - 1 - q);
-        const unsigned long long T64 = S.prefix | (d << shift);
+        unsigned long long T64 = S.prefix | (d << shift);
+        if (shift == 0) { T64 += S.base; S.base = 0; }       // exact: back in the key domain
         S.prefix = T64;
         S.himask |= ((1ull << bits) - 1ull) << shift;
         S.rank = rank - cum;
         S.top = shift;
+        if (hit && shift > 0) atomicAdd(&w.ctl->cls_total, (unsigned long long)hv[q]);   // size of the surviving class
         if (shift == 0 && S.compress) predict_bracket(S.br, (uint32_t)(T64 >> 32), hit ? w.ctl->shrink : 0.0f);
       }
       cum += hv[q];
@@ -1372,13 +1427,11 @@ __global__ void __launch_bounds__(256) lsel_finish_full_kernel(const __grid_cons
 // OR in the candidates at or above the layer's threshold.
 __global__ void __launch_bounds__(256) lsel_finish_cand_kernel(const __grid_constant__ LayerWork w, const __grid_constant__ CandList cl,
                                                               uint32_t* __restrict__ next_bits) {
-  const int lane = threadIdx.x & 31;
-  const int64_t wpb = blockDim.x >> 5;
-  const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
-  const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  __shared__ long long ends[SCAPE_MAX_LAYERS_K];
+  load_layer_ends(w, ends);
   scan_segments(cl.cand, cl.seg_count, cl.seg_cap, cl.n_seg, ~0ull, [&](unsigned long long k64) {
     const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64;
-    const LayerState& S = w.layers[layer_of(w, i)];
+    const LayerState& S = w.layers[layer_of_sorted(ends, w.n_layers, i)];
     if (S.hit && k64 >= S.prefix) atomicOr(&next_bits[i >> 5], 1u << (i & 31));
   });
 }
