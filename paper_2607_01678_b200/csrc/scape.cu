@@ -477,6 +477,8 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   if (!h) { fail(SCAPE_ENOMEM, "host allocation failed"); return nullptr; }
   h->dev = dev;
   if (const char* ev = getenv("SCAPE_COMPACT_MIN")) { int v = atoi(ev); if (v >= 1) h->compact_min = (uint32_t)v; }
+  if (const char* ev = getenv("SCAPE_NARROW")) { float v = (float)atof(ev); if (v > 0.1f && v < 1.0f) cudaMemcpyToSymbol(g_narrow, &v, sizeof v); }
+  if (const char* ev = getenv("SCAPE_ERR_MULT")) { float v = (float)atof(ev); if (v >= 1.0f && v < 100.0f) cudaMemcpyToSymbol(g_err_mult, &v, sizeof v); }
   if (const char* ev = getenv("SCAPE_FUSED_IMPL")) h->fused_impl = (strcmp(ev, "ldg") == 0) ? 1 : 0;
   cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev);
   h->N = N; h->R = R;

@@ -983,6 +983,8 @@ __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ K
 // step (transient of the EMA, then stationary), so the centre is extrapolated geometrically and the
 // half-width follows the error the previous extrapolation made.  shrink > 0: cap the half-width at
 // shrink x the old one (the candidate list was more than half full).
+__device__ float g_narrow = 0.7f;        // factor by which the half-width may shrink per step (SCAPE_NARROW: experiments; 0.55 missed once in the sweep)
+__device__ float g_err_mult = 3.0f;      // half-width >= g_err_mult x the last prediction error + 0.01 (SCAPE_ERR_MULT)
 __device__ __forceinline__ void predict_bracket(Bracket& b, uint32_t Tkey, float shrink) {
   const float T = __uint_as_float(Tkey);
   float dl = b.delta, pred;
@@ -1006,7 +1008,7 @@ __device__ __forceinline__ void predict_bracket(Bracket& b, uint32_t Tkey, float
     pred = lnT + rn;
     b.r_prev = r;
     if (b.have_T == 1) dl = fmaxf(0.05f, 0.5f * fabsf(r));
-    else dl = fmaxf(3.0f * fabsf(lnT - b.ln_pred) + 0.01f, 0.85f * dl);   // widen at once, narrow slowly
+    else dl = fmaxf(g_err_mult * fabsf(lnT - b.ln_pred) + 0.01f, g_narrow * dl);   // widen at once, narrow slowly
   }
   if (shrink > 0.0f) dl = fminf(dl, b.delta * shrink);
   dl = fminf(fmaxf(dl, 0.02f), 1.0f);
@@ -1580,17 +1582,32 @@ __global__ void __launch_bounds__(256) dist_update_kernel(float* __restrict__ th
                                                          const float* __restrict__ mold, int64_t K, float R_f, float inv_R,
                                                          int r_pow2, float b1, float c1, float b2, float c2, float eps, float wd,
                                                          float neg_lr, float bc1, float bc2) {
-  for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < K; j += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t i = idx ? (int64_t)idx[j] : j;
-    const float sm = S[j], mo = mold[j];
-    const float pq = __fmul_rn(b1, mo);
-    const float bb = r_pow2 ? __fmul_rn(sm, inv_R) : __fdiv_rn(sm, R_f);                      // l.10
-    const float gh = __fdiv_rn(__fsub_rn(bb, pq), c1);                                         // l.13 (Eq. 3)
-    const float v = __fmaf_rn(c2, __fmul_rn(gh, gh), __fmul_rn(b2, __fmul_rn(mo, mo)));      // l.15
-    const float u = __fdiv_rn(__fmul_rn(bb, bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, bc2)), eps));   // l.16 (+ :77)
-    const float th = theta[i];
-    theta[i] = __fmaf_rn(neg_lr, __fmaf_rn(wd, th, u), th);                                   // l.17
-    m_out[j] = bb;                                                                             // l.12: m_t = b- (packed, or dense when idx == nullptr)
+  // 4 entries per thread and trip: the gather of theta depends on the index load, so the loads of
+  // four entries are issued together (one entry per trip left the kernel latency-bound)
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t j0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j0 < K; j0 += 4 * stride) {
+    int64_t i[4]; float sm[4], mo[4], th[4]; bool ok[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int64_t j = j0 + u * stride;
+      ok[u] = j < K;
+      i[u] = ok[u] ? (idx ? (int64_t)__ldg(idx + j) : j) : 0;
+      sm[u] = ok[u] ? __ldcs(S + j) : 0.0f;
+      mo[u] = ok[u] ? __ldcs(mold + j) : 0.0f;
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) th[u] = ok[u] ? theta[i[u]] : 0.0f;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      if (!ok[u]) continue;
+      const float pq = __fmul_rn(b1, mo[u]);
+      const float bb = r_pow2 ? __fmul_rn(sm[u], inv_R) : __fdiv_rn(sm[u], R_f);               // l.10
+      const float gh = __fdiv_rn(__fsub_rn(bb, pq), c1);                                       // l.13 (Eq. 3)
+      const float v = __fmaf_rn(c2, __fmul_rn(gh, gh), __fmul_rn(b2, __fmul_rn(mo[u], mo[u])));   // l.15
+      const float uu = __fdiv_rn(__fmul_rn(bb, bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, bc2)), eps));   // l.16 (+ :77)
+      theta[i[u]] = __fmaf_rn(neg_lr, __fmaf_rn(wd, th[u], uu), th[u]);                        // l.17
+      m_out[j0 + u * stride] = bb;                                                             // l.12: m_t = b- (packed, or dense when idx == nullptr)
+    }
   }
 }
 
