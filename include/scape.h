@@ -186,6 +186,18 @@ int scape_step_local(scape_t* h, float* param, const void* const* grads, void* c
 int scape_exchange_buffers(scape_t* h, float** sums, int64_t* n_sums, uint32_t** mask_words, int64_t* n_mask_words);
 int scape_step_apply(scape_t* h, float* param, void* cuda_stream);
 
+/* Mask bit pack / unpack, stand-alone (no handle).  PAPER.md:250-252: "we convert the masks from INT8
+ * to 1-bit values and pack 8 mask values into one byte" (the paper's Triton kernels, K1 of SURVEY.md
+ * §2).  The packed form is the one SCAPE_MASK_NEXT / SCAPE_MASK_LAST and scape_exchange_buffers use:
+ * bit i % 32 of little-endian word i / 32, bits at positions >= n zero.
+ *   scape_mask_pack    mask_bytes: DEVICE, n bytes, non-zero = selected; words: DEVICE,
+ *                      ceil(n / 32) uint32, completely overwritten.
+ *   scape_mask_unpack  the inverse: writes n bytes of 0 / 1.
+ * Both enqueue one kernel on cuda_stream of the CURRENT device and return without synchronising.
+ * Buffers are caller-owned.  n = 0 is a no-op.  SCAPE_EINVAL for n < 0, NULL or misaligned words.  */
+int scape_mask_pack(const uint8_t* mask_bytes, int64_t n, uint32_t* words, void* cuda_stream);
+int scape_mask_unpack(const uint32_t* words, int64_t n, uint8_t* mask_bytes, void* cuda_stream);
+
 /* Option: also materialise b^r on steps whose mask is all ones (step 1, or sparsity 0), where
  * the packed buffer would be R*N floats.  Off by default: on such steps SCAPE_PACKED is then
  * unavailable (SCAPE_EINVAL) and SCAPE_PACKED_MEAN equals SCAPE_MOMENT.  Allocates R*N floats

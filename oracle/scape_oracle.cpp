@@ -21,6 +21,7 @@
 //   P14 sparsity schedule: mask counts follow the schedule with the one-step delay; P6 still holds
 //   P15 workers: every layer's mask == brute force on ITS OWNER's |m-tilde|; the
 //       two-level sum equals the flat mean (double, 1e-15); W = R with one owner == the plain step
+//   P16 mask bit pack / unpack (oracle/scape_oracle.py, a plain loop) vs numpy packbits and an example
 // Unpinned by the paper (decisions): S3 clip_grad off by default and,
 // when switched on, the torch/Megatron rule; S4 bias correction off by default; S8 replica 0 owns
 // the statistic; S9 flat top-k by default, per-layer top-k with uncompressed

@@ -209,3 +209,22 @@ def topk_mask(x, k):
     out = np.zeros(x.size, dtype=np.uint8)
     fn(x.ctypes.data, x.size, int(k), out.ctypes.data)
     return out
+
+
+def mask_pack(mask_bytes):
+    """Mask bit pack written out from its definition (INT8 mask values to 1 bit
+    each, 8 per byte; layout of include/scape.h: bit i % 32 of little-endian word i / 32): a plain
+    loop over the entries, no library routine.  Returns uint32 words, ceil(n / 32) of them."""
+    m = np.asarray(mask_bytes)
+    n = m.size
+    words = [0] * ((n + 31) // 32)
+    for i in range(n):
+        if m[i] != 0:
+            words[i // 32] |= 1 << (i % 32)
+    return np.array(words, dtype=np.uint32)
+
+
+def mask_unpack(words, n):
+    """The inverse of mask_pack, entry by entry: uint8 [n] of 0 / 1."""
+    w = np.asarray(words, dtype=np.uint32)
+    return np.array([(int(w[i // 32]) >> (i % 32)) & 1 for i in range(n)], dtype=np.uint8)

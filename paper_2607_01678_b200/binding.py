@@ -44,6 +44,8 @@ SYMBOLS = {
     "scape_step_local": (_I, [_VP, _VP, _VP, _VP]),
     "scape_exchange_buffers": (_I, [_VP, _VP, _VP, _VP, _VP]),
     "scape_step_apply": (_I, [_VP, _VP, _VP]),
+    "scape_mask_pack": (_I, [_VP, _I64, _VP, _VP]),
+    "scape_mask_unpack": (_I, [_VP, _I64, _VP, _VP]),
     "scape_get": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
     "scape_set": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
     "scape_set_step_count": (_I, [_VP, _I64]),
@@ -198,6 +200,35 @@ def scape_exchange_buffers(h):
 
 def scape_step_apply(h, param_ptr, stream=0):
     _check(lib().scape_step_apply(h, param_ptr, stream), "scape_step_apply")
+
+
+def scape_mask_pack(mask_bytes_ptr, n, words_ptr, stream=0):
+    _check(lib().scape_mask_pack(mask_bytes_ptr, int(n), words_ptr, stream), "scape_mask_pack")
+
+
+def scape_mask_unpack(words_ptr, n, mask_bytes_ptr, stream=0):
+    _check(lib().scape_mask_unpack(words_ptr, int(n), mask_bytes_ptr, stream), "scape_mask_unpack")
+
+
+def mask_pack(mask_bytes):
+    """torch uint8 [n] on the GPU -> torch int32 [ceil(n/32)] bit-packed."""
+    import torch
+    assert mask_bytes.is_cuda and mask_bytes.dtype == torch.uint8 and mask_bytes.is_contiguous()
+    n = mask_bytes.numel()
+    words = torch.empty((n + 31) // 32, dtype=torch.int32, device=mask_bytes.device)
+    with torch.cuda.device(mask_bytes.device):
+        scape_mask_pack(mask_bytes.data_ptr(), n, words.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    return words
+
+
+def mask_unpack(words, n):
+    """torch int32 bit-packed words on the GPU -> torch uint8 [n] of 0 / 1."""
+    import torch
+    assert words.is_cuda and words.dtype == torch.int32 and words.is_contiguous() and words.numel() >= (n + 31) // 32
+    out = torch.empty(n, dtype=torch.uint8, device=words.device)
+    with torch.cuda.device(words.device):
+        scape_mask_unpack(words.data_ptr(), n, out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    return out
 
 
 def scape_set_sparsity(h, sparsity):

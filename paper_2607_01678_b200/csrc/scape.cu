@@ -929,6 +929,31 @@ extern "C" int scape_step_apply(scape_t* h, float* param, void* cuda_stream) {
   return SCAPE_OK;
 }
 
+// ---- mask bit pack / unpack, stand-alone: no handle ----------------------
+extern "C" int scape_mask_pack(const uint8_t* mask_bytes, int64_t n, uint32_t* words, void* cuda_stream) {
+  if (n < 0) return fail(SCAPE_EINVAL, "n must be >= 0");
+  if (n == 0) return SCAPE_OK;
+  if (!mask_bytes || !words) return fail(SCAPE_EINVAL, "NULL argument");
+  if ((uintptr_t)words & 3) return fail(SCAPE_EINVAL, "words must be 4-byte aligned");
+  const int64_t groups = (n + 31) >> 5;
+  int64_t grid = (groups + 255) / 256; if (grid > 148 * 32) grid = 148 * 32;
+  mask_pack_kernel<<<(int)grid, 256, 0, (cudaStream_t)cuda_stream>>>(mask_bytes, n, words);
+  CU_TRY(cudaGetLastError());
+  return SCAPE_OK;
+}
+
+extern "C" int scape_mask_unpack(const uint32_t* words, int64_t n, uint8_t* mask_bytes, void* cuda_stream) {
+  if (n < 0) return fail(SCAPE_EINVAL, "n must be >= 0");
+  if (n == 0) return SCAPE_OK;
+  if (!mask_bytes || !words) return fail(SCAPE_EINVAL, "NULL argument");
+  if ((uintptr_t)words & 3) return fail(SCAPE_EINVAL, "words must be 4-byte aligned");
+  const int64_t groups = (n + 15) >> 4;
+  int64_t grid = (groups + 255) / 256; if (grid > 148 * 32) grid = 148 * 32;
+  mask_unpack_kernel<<<(int)grid, 256, 0, (cudaStream_t)cuda_stream>>>(words, n, mask_bytes);
+  CU_TRY(cudaGetLastError());
+  return SCAPE_OK;
+}
+
 extern "C" int scape_select_stats(scape_t* h, int64_t* fast, int64_t* general, void* cuda_stream) {
   if (!h) return fail(SCAPE_EINVAL, "NULL handle");
   DeviceGuard guard(h->dev);

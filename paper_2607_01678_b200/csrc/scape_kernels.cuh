@@ -1626,6 +1626,61 @@ __global__ void scatter_packed_kernel(float* __restrict__ dense, const int32_t* 
     dense[idx[j]] = packed[j];
 }
 
+// ------------------------------------------------------------------------------------------
+// Mask bit pack / unpack ("we convert the masks from INT8 to 1-bit values and pack
+// 8 mask values into one byte"; the paper's Triton kernels).  The bit-packed form -- bit i % 32 of
+// word i / 32 -- is this library's native mask; these two kernels convert to and from one byte
+// per parameter for callers that keep masks that way.  HBM-bound: N bytes on one side, N/8 on the
+// other; a thread handles one word = 32 mask values (two independent 16-byte accesses).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t nonzero_bytes_to_bits16(const uint4 t) {
+  const uint32_t x[4] = {t.x, t.y, t.z, t.w};
+  uint32_t v = 0;
+#pragma unroll
+  for (int q = 0; q < 4; ++q)
+#pragma unroll
+    for (int b = 0; b < 4; ++b) v |= ((x[q] >> (8 * b)) & 0xFFu) ? (1u << (4 * q + b)) : 0u;
+  return v;
+}
+__device__ __forceinline__ uint4 bits16_to_bytes(uint32_t v) {
+  uint32_t x[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const uint32_t n4 = (v >> (4 * q)) & 0xFu;
+    x[q] = (n4 & 1u) | ((n4 & 2u) << 7) | ((n4 & 4u) << 14) | ((n4 & 8u) << 21);
+  }
+  return make_uint4(x[0], x[1], x[2], x[3]);
+}
+
+__global__ void __launch_bounds__(256) mask_pack_kernel(const uint8_t* __restrict__ bytes, int64_t N, uint32_t* __restrict__ words) {
+  const int64_t n_words = (N + 31) >> 5;
+  const bool aligned = ((uintptr_t)bytes & 15) == 0;
+  for (int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; w < n_words; w += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t i0 = w << 5;
+    uint32_t v = 0;
+    if (aligned && i0 + 32 <= N) {
+      const uint4 lo = __ldcs(reinterpret_cast<const uint4*>(bytes + i0));
+      const uint4 hi = __ldcs(reinterpret_cast<const uint4*>(bytes + i0 + 16));
+      v = nonzero_bytes_to_bits16(lo) | (nonzero_bytes_to_bits16(hi) << 16);
+    } else {
+      for (int b = 0; b < 32; ++b) if (i0 + b < N && bytes[i0 + b]) v |= 1u << b;
+    }
+    words[w] = v;
+  }
+}
+
+// a thread writes 16 values (one 16-byte store; two stores of 32-byte stride per lane wrote half sectors)
+__global__ void __launch_bounds__(256) mask_unpack_kernel(const uint32_t* __restrict__ words, int64_t N, uint8_t* __restrict__ bytes) {
+  const int64_t n_half = (N + 15) >> 4;
+  const bool aligned = ((uintptr_t)bytes & 15) == 0;
+  for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g < n_half; g += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t i0 = g << 4;
+    const uint32_t v = (__ldg(words + (g >> 1)) >> ((g & 1) << 4)) & 0xFFFFu;
+    if (aligned && i0 + 16 <= N) __stcs(reinterpret_cast<uint4*>(bytes + i0), bits16_to_bytes(v));
+    else for (int b = 0; b < 16; ++b) if (i0 + b < N) bytes[i0 + b] = (uint8_t)((v >> b) & 1u);
+  }
+}
+
 // all-ones mask over [0,N), zero padding bits up to n_words*32
 __global__ void mask_all_ones_kernel(uint32_t* bits, int64_t n_words, int64_t N) {
   for (int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; w < n_words; w += (int64_t)gridDim.x * blockDim.x) {

@@ -618,3 +618,22 @@ def test_p15_set_workers_rejects_bad_arguments():
     with pytest.raises(ValueError):
         o.set_workers(2, [0, 2])                 # owner out of range
     o.set_workers(2, [1, 0])
+
+
+# ---------------------------------------------------------------------------------------------
+# P16 mask bit pack / unpack: the oracle's plain loop against numpy's packbits
+# (a library routine, another route to the same definition), a hand-written example, the round trip
+# ---------------------------------------------------------------------------------------------
+def test_p16_mask_pack_unpack():
+    from oracle.scape_oracle import mask_pack, mask_unpack
+    # by hand: entries 0, 5, 31 -> word 0 = 1 + 32 + 2^31; entry 32 -> word 1 bit 0; entry 70 -> word 2 bit 6
+    m = np.zeros(71, np.uint8); m[[0, 5, 31, 32, 70]] = [1, 9, 255, 1, 1]
+    np.testing.assert_array_equal(mask_pack(m), np.array([1 + 32 + 2**31, 1, 64], np.uint32))
+    rng = np.random.default_rng(16)
+    for n in (1, 31, 32, 33, 64, 1000, 4099):
+        m = (rng.random(n) < 0.3).astype(np.uint8) * rng.integers(1, 255, n).astype(np.uint8)
+        w = mask_pack(m)
+        lib = np.packbits(np.concatenate([m != 0, np.zeros((-n) % 32, bool)]), bitorder="little").view(np.uint32)
+        np.testing.assert_array_equal(w, lib)
+        np.testing.assert_array_equal(mask_unpack(w, n), (m != 0).astype(np.uint8))
+        assert w.size == (n + 31) // 32
