@@ -49,10 +49,14 @@ def _workload(name):
     if name == "max_int32_index_R1":
         return synth.Workload(name, [("a", 2**31 - 1)], R=1, sparsity=0.999, dist="gauss", rho=0.9,
                               grad_dtype="f32", steps=4, per_tensor_scale=False), "scape_fused_step_kernel", 60e9
+    if name == "llama1p8b_layers_split":
+        # the same shard with the per-layer refresh (one top-k per tensor: 194 layers) and the split step of
+        # the workers mode (a world of one): SURVEY.md §8(f) ranks 2 and 3 at full size
+        return synth.workload("llama1p8b"), "scape_fused_tma_kernel", 130e9
     return synth.workload(name), "scape_fused_tma_kernel", 120e9
 
 
-@pytest.mark.parametrize("name", ["llama1p8b", "max_int32_index", "max_int32_index_R1"])
+@pytest.mark.parametrize("name", ["llama1p8b", "llama1p8b_layers_split", "max_int32_index", "max_int32_index_R1"])
 def test_fullsize_sampled_and_property_parity(name):
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
@@ -66,10 +70,22 @@ def test_fullsize_sampled_and_property_parity(name):
     gs = synth.GradStream(w, device="cuda", seed=0)
     theta = gs.theta0()
     sc = B.Scape(N, R, w.sparsity, **w.hyper)
+    layered = name.endswith("_layers_split")
+    offsets = w.offsets()
+    if layered:
+        sc.set_layers(offsets, w.compress_flags())
+        sc.set_workers(1, 0, [0] * (len(offsets) - 1))
+
+    def step(th, g):
+        if layered:
+            sc.step_local(th, g)
+            sc.step_apply(th)
+        else:
+            sc.step(th, g)
     k = sc.k
     # reach the steady state bench.py times: dense first step, then sparse steps with m stored sparsely
     for _ in range(3):
-        sc.step(theta, gs.next())
+        step(theta, gs.next())
     torch.cuda.synchronize()
     fast0, gen0 = sc.select_stats()
 
@@ -93,7 +109,7 @@ def test_fullsize_sampled_and_property_parity(name):
     cur_s = cur[samp].cpu().numpy().astype(np.uint8)
     del cur, on_idx
 
-    sc.step(theta, grads)                # the step under test (steady state, full size)
+    step(theta, grads)                   # the step under test (steady state, full size)
     torch.cuda.synchronize()
     fast1, gen1 = sc.select_stats()
 
@@ -126,18 +142,29 @@ def test_fullsize_sampled_and_property_parity(name):
     idx_last = torch.from_numpy(sc.idx_last()).cuda().long()
     b0 = get_f32_device(B, sc, B.SCAPE_PACKED, 0, k)
     keys[idx_last] = b0.abs()
-    sel_min = keys[nxt].min()
-    keys_unsel = torch.where(nxt, torch.full_like(keys, -1.0), keys)
-    unsel_max = keys_unsel.max()
-    assert float(sel_min) >= float(unsel_max), (float(sel_min), float(unsel_max))
-    if float(sel_min) == float(unsel_max):           # tie class straddles the threshold: lower indices win
-        tie = keys == sel_min
-        last_sel = torch.nonzero(tie & nxt).flatten().max()
-        first_unsel = torch.nonzero(tie & ~nxt).flatten().min()
-        assert int(last_sel) < int(first_unsel)
-    # the timed configuration: fast select route with the bulk-copy staged kernel
-    assert fast1 - fast0 + gen1 - gen0 == 1
+    def check_topk(keys_l, nxt_l, k_l):
+        assert int(nxt_l.sum()) == k_l
+        if k_l == keys_l.numel():
+            return
+        sel_min = keys_l[nxt_l].min()
+        unsel_max = torch.where(nxt_l, torch.full_like(keys_l, -1.0), keys_l).max()
+        assert float(sel_min) >= float(unsel_max), (float(sel_min), float(unsel_max))
+        if float(sel_min) == float(unsel_max):       # tie class straddles the threshold: lower indices win
+            tie = keys_l == sel_min
+            last_sel = torch.nonzero(tie & nxt_l).flatten().max()
+            first_unsel = torch.nonzero(tie & ~nxt_l).flatten().min()
+            assert int(last_sel) < int(first_unsel)
+
+    if layered:                                      # the top-k property inside every layer, exactly k_l each
+        for l in range(len(offsets) - 1):
+            a, b = offsets[l], offsets[l + 1]
+            check_topk(keys[a:b], nxt[a:b], sc.layer_k(l))
+        assert fast1 - fast0 + gen1 - gen0 == len(offsets) - 1      # counted per layer and step
+    else:
+        check_topk(keys, nxt, k)
+        # the timed configuration: fast select route with the bulk-copy staged kernel
+        assert fast1 - fast0 + gen1 - gen0 == 1
     assert sc.last_kernel == want_kernel
     sc.close()
-    del theta, grads, keys, keys_unsel, nxt, e0_new
+    del theta, grads, keys, nxt, e0_new
     torch.cuda.empty_cache()
