@@ -97,7 +97,10 @@ struct scape {
   int max_seg = 0;
   uint32_t* ghist = nullptr;      // [kBins]
   uint32_t* block_sum = nullptr;  // [n_compact_blocks]
-  uint32_t* total = nullptr;      // [1]
+  uint32_t* total = nullptr;      // [2]: number of set bits, ticket of mask_compact_kernel
+  unsigned long long* scan_state = nullptr;   // [n_compact_blocks] look-back state of mask_compact_kernel
+  uint32_t compact_epoch = 0;
+  int compact_impl = 0;           // 1 single pass (small shards), 0 count / scan / rank; SCAPE_COMPACT_IMPL overrides
   int n_compact_blocks = 0;
   int n_seg = 0;                  // segments (= warps) of the last fused launch
   int n_slots = 0;                // warps of the last streaming launch (clip-mode partial sums)
@@ -283,6 +286,14 @@ int materialise_dense_m(scape* h, cudaStream_t st) {
 // rank128 (+ idx when idx != nullptr) of slot.bits; leaves the bit count in *h->total
 int compact_mask(scape* h, MaskSlot& s, bool want_idx, cudaStream_t st) {
   const int nb = h->n_compact_blocks;
+  if (h->compact_impl == 1) {       // single pass (chained scan with look-back)
+    h->compact_epoch = (h->compact_epoch + 1u) & 0x3FFFFFFFu;
+    mask_compact_kernel<<<nb, 1024, 0, st>>>(s.bits, h->n_chunks, h->scan_state, h->total, h->compact_epoch, s.rank,
+                                            want_idx ? s.idx : nullptr, h->packed_stride);
+    h->launches += 1;
+    CU_TRY(cudaGetLastError());
+    return SCAPE_OK;
+  }
   mask_block_count_kernel<<<nb, 1024, 0, st>>>(s.bits, h->n_chunks, h->block_sum);
   mask_scan_blocks_kernel<<<1, 1024, 0, st>>>(h->block_sum, nb, h->total);
   mask_rank_idx_kernel<<<nb, 1024, 0, st>>>(s.bits, h->n_chunks, h->block_sum, s.rank, want_idx ? s.idx : nullptr,
@@ -448,7 +459,7 @@ void free_all(scape* h) {
   cudaFree(h->m); cudaFree(h->e);
   for (auto& s : h->slot) { cudaFree(s.bits); cudaFree(s.rank); cudaFree(s.idx); }
   cudaFree(h->packed); cudaFree(h->pm[0]); cudaFree(h->pm[1]); cudaFree(h->dense_pack);
-  cudaFree(h->sel); cudaFree(h->cand); cudaFree(h->cls); cudaFree(h->seg_count); cudaFree(h->seg_above); cudaFree(h->ghist); cudaFree(h->block_sum); cudaFree(h->total);
+  cudaFree(h->sel); cudaFree(h->cand); cudaFree(h->cls); cudaFree(h->seg_count); cudaFree(h->seg_above); cudaFree(h->ghist); cudaFree(h->block_sum); cudaFree(h->total); cudaFree(h->scan_state);
   cudaFree(h->ghat); cudaFree(h->vm); cudaFree(h->sumsq); cudaFree(h->clip_state);
   cudaFree(h->layers); cudaFree(h->lctl); cudaFree(h->chunk_layer); cudaFree(h->lhist); cudaFree(h->items);
   cudaFree(h->st_param);
@@ -512,7 +523,12 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   if (ok && ensure_capacity(h, h->k) != SCAPE_OK) ok = false;                // index lists, packed buffers, candidates
   alloc((void**)&h->ghist, sizeof(uint32_t) * kBins, true);
   alloc((void**)&h->block_sum, sizeof(uint32_t) * (h->n_compact_blocks + 1), true);
-  alloc((void**)&h->total, sizeof(uint32_t), true);
+  alloc((void**)&h->total, 2 * sizeof(uint32_t), true);
+  alloc((void**)&h->scan_state, sizeof(unsigned long long) * (h->n_compact_blocks + 1), true);
+  // measured: the single pass wins while launch count matters (pr1: select stage 99 -> 94 us) and loses on
+  // large shards, where 13.5 k CTAs wait on one another's prefixes (headline: 0.44 -> 0.50 ms)
+  h->compact_impl = h->n_compact_blocks <= 512 ? 1 : 0;
+  if (const char* ev = getenv("SCAPE_COMPACT_IMPL")) h->compact_impl = atoi(ev) != 0;
   if (!ok) {
     fail(SCAPE_ENOMEM, "device allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
     free_all(h); delete h; return nullptr;

@@ -1535,6 +1535,91 @@ __global__ void __launch_bounds__(1024) mask_rank_idx_kernel(const uint32_t* __r
   }
 }
 
+// Single-pass variant of the three kernels above (chained scan with decoupled look-back): every CTA
+// takes a ticket (so that all its predecessors have started), scans its 1024 chunk counts,
+// publishes its total, looks back over the predecessors' totals / inclusive prefixes until it has its
+// own exclusive prefix, publishes the inclusive one and writes rank128 and the index list.  The
+// mask bits are read once instead of twice and two launches go away.
+//   state[b] = (tag << 32) | value, tag = 2 * epoch + 1: total of block b, 2 * epoch + 2: inclusive
+//   prefix through block b; any other tag: nothing yet (epoch changes every call: no clearing).
+//   ctl[0] = total number of set bits (out), ctl[1] = ticket (returns to 0).
+__global__ void __launch_bounds__(1024) mask_compact_kernel(const uint32_t* __restrict__ bits, int64_t n_chunks,
+                                                           unsigned long long* state, uint32_t* ctl, uint32_t epoch,
+                                                           uint32_t* __restrict__ rank128, int32_t* __restrict__ idx, int64_t idx_cap) {
+  __shared__ uint32_t ws[32];
+  __shared__ uint32_t s_bid, s_prefix;
+  if (threadIdx.x == 0) s_bid = atomicAdd(&ctl[1], 1u);
+  __syncthreads();
+  const uint32_t bid = s_bid;
+  const int64_t c = (int64_t)bid * 1024 + threadIdx.x;
+  uint4 w = make_uint4(0, 0, 0, 0);
+  if (c < n_chunks) w = __ldg(reinterpret_cast<const uint4*>(bits) + c);
+  const uint32_t n = __popc(w.x) + __popc(w.y) + __popc(w.z) + __popc(w.w);
+  uint32_t incl = n;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += x; }
+  if (lane == 31) ws[wid] = incl;
+  __syncthreads();
+  const unsigned long long tag_total = (unsigned long long)(2u * epoch + 1u) << 32, tag_incl = (unsigned long long)(2u * epoch + 2u) << 32;
+  if (wid == 0) {
+    uint32_t x = ws[lane], ix = x;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xFFFFFFFFu, ix, o); if (lane >= o) ix += y; }
+    ws[lane] = ix - x;
+    const uint32_t total = __shfl_sync(0xFFFFFFFFu, ix, 31);
+    // publish the total (block 0: already the inclusive prefix), then look back, 32 predecessors at a time
+    volatile unsigned long long* vs = state;
+    if (lane == 0) { vs[bid] = (bid == 0 ? tag_incl : tag_total) | total; __threadfence(); }
+    uint32_t prefix = 0;
+    if (bid > 0) {
+      int64_t b0 = (int64_t)bid - 1;                    // newest predecessor not yet accounted for
+      while (true) {
+        const int64_t b = b0 - lane;
+        unsigned long long v = 0;
+        bool ready, is_incl;
+        do {                                            // wait until every predecessor in the window has published
+          v = b >= 0 ? vs[b] : tag_incl;                // before block 0: an inclusive prefix of 0
+          const unsigned long long tg = v & 0xFFFFFFFF00000000ull;
+          is_incl = tg == tag_incl;
+          ready = is_incl || tg == tag_total;
+        } while (!__all_sync(0xFFFFFFFFu, ready));
+        const uint32_t incl_mask = __ballot_sync(0xFFFFFFFFu, is_incl);
+        // lanes 0 .. first inclusive one (nearest predecessors first) contribute
+        const int stop = incl_mask ? __ffs(incl_mask) - 1 : 31;
+        uint32_t val = lane <= stop ? (uint32_t)v : 0u;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(0xFFFFFFFFu, val, o);
+        prefix += val;
+        if (incl_mask) break;
+        b0 -= 32;
+      }
+      if (lane == 0) { __threadfence(); vs[bid] = tag_incl | (prefix + total); }
+    }
+    if (lane == 0) {
+      s_prefix = prefix;
+      if (bid == gridDim.x - 1) { ctl[0] = prefix + total; ctl[1] = 0; }     // every CTA has its ticket by now
+    }
+  }
+  __syncthreads();
+  if (c >= n_chunks) return;
+  uint32_t j = s_prefix + ws[wid] + incl - n;
+  rank128[c] = j;
+  if (idx == nullptr) return;
+  const uint32_t words[4] = {w.x, w.y, w.z, w.w};
+  const int64_t base = c << 7;
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    uint32_t x = words[q];
+    while (x) {
+      const int b = __ffs(x) - 1;
+      x &= x - 1;
+      if ((int64_t)j < idx_cap) idx[j] = (int32_t)(base + (q << 5) + b);
+      ++j;
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------
 // l.14 clip_grad (optional, reading S3'): global-norm clip of the reconstructed gradient
 // ------------------------------------------------------------------------------------------

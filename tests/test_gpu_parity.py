@@ -396,3 +396,13 @@ def test_clip_grad_above_the_norm_is_a_bitwise_noop(B):
     np.testing.assert_array_equal(a.mask_next(), b.mask_next())
     a.close()
     b.close()
+
+
+@pytest.mark.parametrize("impl", ["0", "1"])
+def test_both_compaction_forms(B, monkeypatch, impl):
+    """rank128 + index list from the mask bits: the three-kernel form (large shards) and the single-pass
+    chained scan (small shards) are chosen by size; both run here on the same ragged shard."""
+    monkeypatch.setenv("SCAPE_COMPACT_IMPL", impl)
+    w = synth.Workload(f"compact{impl}", [("a", 300_000), ("b", 1024 * 700 + 77)], R=2, sparsity=0.97, dist="t3", rho=0.9,
+                       grad_dtype="f32", steps=5)
+    run_reload_parity(B, w, steps=5, seed=int(impl))
