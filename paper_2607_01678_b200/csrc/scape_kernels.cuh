@@ -459,11 +459,18 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
         uint32_t pos = sa.cursor + __popc(b0 & lt) + 2u * __popc(b1 & lt) + 4u * __popc(b2 & lt);
         if (cnib != 0u) {
           const uint32_t inv = 0xFFFFFFFFu - (uint32_t)i0;
+          if (pos + 4u <= p.seg_cap) {                      // room for all four: one pointer, no bound checks
+            uint2* dst = reinterpret_cast<uint2*>(sa.seg + pos);
 #pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            if ((cnib >> q) & 1u) {
-              if (pos < p.seg_cap) sa.seg[pos] = ((unsigned long long)key0[q] << 32) | (unsigned long long)(inv - q);
-              ++pos;
+            for (int q = 0; q < 4; ++q)
+              if ((cnib >> q) & 1u) { *dst = make_uint2(inv - q, key0[q]); ++dst; }      // little endian: low word = index part
+          } else {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              if ((cnib >> q) & 1u) {
+                if (pos < p.seg_cap) sa.seg[pos] = ((unsigned long long)key0[q] << 32) | (unsigned long long)(inv - q);
+                ++pos;
+              }
             }
           }
         }
