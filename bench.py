@@ -107,12 +107,16 @@ def measured_peak():
 
 def recorded_traffic(workload_name):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed
-    `ncu --set full` capture (profiles/traffic.json), or None."""
+    `ncu --set full` captures (profiles/traffic.csv: workload, kernel, bytes, source), or None."""
+    import csv
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(workload_name, {}).get("fused_dram_bytes_per_launch")
+        with open(os.path.join(ROOT, "profiles", "traffic.csv"), newline="") as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload_name:
+                    return int(row["fused_dram_bytes_per_launch"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 # ---------------------------------------------------------------------------------------------
