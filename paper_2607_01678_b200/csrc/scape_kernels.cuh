@@ -353,6 +353,7 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
       }
     } else {
       const uint32_t lbase = jbase - r0;                    // rank of this lane's first entry inside the chunk
+      uint32_t lj = lbase;                                  // walks this lane's selected entries
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         const bool on = (mybits >> q) & 1u;
@@ -365,7 +366,6 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
         }
         key0[q] = __float_as_uint(mt[0]) & 0x7FFFFFFFu;
         if (on) {
-          const uint32_t lj = lbase + __popc(mybits & ((1u << q) - 1u));
           float* pk = p.packed + (r0 + lj);
           float sm = mt[0];
 #pragma unroll
@@ -373,6 +373,7 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
 #pragma unroll
           for (int r = 1; r < R; ++r) sm = __fadd_rn(sm, mt[r]);                                // l.10, r ascending
           scs[lj] = sm; scm[lj] = mo[q];
+          ++lj;
         }
       }
       __syncwarp();
@@ -395,11 +396,13 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
         }
       }
       __syncwarp();
+      lj = lbase;
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         const bool on = (mybits >> q) & 1u;
+        const float u = on ? scs[lj] : 0.0f;                                                   // Eq. 5 off the mask
+        lj += on ? 1u : 0u;
         if (deferred && on) continue;
-        const float u = on ? scs[lbase + __popc(mybits & ((1u << q) - 1u))] : 0.0f;            // Eq. 5 off the mask
         th[q] = __fmaf_rn(p.neg_lr, __fmaf_rn(p.wd, th[q], u), th[q]);                         // l.17
       }
       __syncwarp();                                         // the scratch is reused by the next chunk
