@@ -15,7 +15,8 @@
  *   l.13  g^ = (b- - beta1 m_old)/(1-beta1)   (Eq. 3)
  *   l.15-17 v = beta2 m_old^2 + (1-beta2) g^^2 ; u = m/(sqrt(v)+eps);
  *         theta <- theta - lr (u + wd theta)   (AdamS, Eq. 2)
- * clip_grad (l.14) and bias correction are NOT applied (readings S3, S4).
+ * clip_grad (l.14) and bias correction are off by default (readings S3, S4);
+ * scape_set_clip_grad / scape_set_bias_correction below switch them on.
  * Ties in the top-k go to the lower index; exactly k = N - floor(sparsity*N) entries are kept.
  * The fp32 operation order is pinned.
  *
@@ -59,7 +60,8 @@ typedef struct scape scape_t;
 
 /* Alg. 1 "Require" line + l.1-2: create the state of one partition.
  *   shard_numel  N, number of fp32 parameters in the flattened shard, 0 < N < 2^31
- *   R            number of simulated data-parallel replicas (the paper's N workers), 1..8
+ *   R            number of simulated data-parallel replicas (the paper's N workers), 1..8 (every
+ *                BASELINE.json config has R <= 8; the streaming kernels are instantiated for these)
  *   sparsity     s in [0,1); k = N - floor(s*N) (evaluated in double) entries are selected
  *   beta1,beta2  in [0,1); eps >= 0; lr; wd : AdamS hyper-parameters, cast to fp32 once
  * Allocates on the current CUDA device and OWNS: m [N] (zeros), e^r [R][N] (zeros, l.2), the
@@ -75,8 +77,19 @@ scape_t* scape_create(int64_t shard_numel, int R, double sparsity, double beta1,
  *                never written
  *   cuda_stream  a cudaStream_t (NULL = legacy default stream)
  * All work is enqueued on cuda_stream; the call does not synchronise and allocates nothing,
- * so it can be captured into a CUDA graph.  One step may be in flight per handle.  Advances the
- * step counter.  Returns SCAPE_OK or a negative code; the state is unchanged on SCAPE_EINVAL. */
+ * so it can be captured into a CUDA graph -- with one rule.  The handle rotates three mask slots
+ * and two packed-mean buffers from step to step and bakes their addresses, the learning rate and
+ * the bias-correction factors into the launches, so a captured sequence replays correctly only if
+ * it returns the rotation to where it started: capture a multiple of SCAPE_GRAPH_PERIOD (= 6)
+ * consecutive steady-state steps (sparse mask in, i.e. from the third step on; constant lr, bias
+ * correction off) and replay that graph any number of times; scape_step_count does not advance on
+ * replay.  One step may be in flight per handle.  Advances the step counter.
+ * Returns SCAPE_OK or a negative code.  On SCAPE_EINVAL nothing was enqueued and the state is
+ * unchanged.  SCAPE_ECUDA means a launch or runtime call failed part-way through the step: some
+ * kernels may already be enqueued, the step counter and the mask rotation have NOT advanced, and
+ * the handle's contents (theta included) are undefined -- destroy the handle or reload every
+ * buffer with scape_set before stepping again.                                                  */
+#define SCAPE_GRAPH_PERIOD 6
 int scape_step(scape_t* h, float* param, const void* const* grads, void* cuda_stream);
 
 /* Same step with HOST buffers (end-to-end path): copies param (N fp32) and the R gradient
@@ -198,6 +211,11 @@ int scape_step_apply(scape_t* h, float* param, void* cuda_stream);
 int scape_mask_pack(const uint8_t* mask_bytes, int64_t n, uint32_t* words, void* cuda_stream);
 int scape_mask_unpack(const uint32_t* words, int64_t n, uint8_t* mask_bytes, void* cuda_stream);
 
+/* How rank128 + the index list are made from the bits of a new mask: 0 = by shard size (default:
+ * one pass with a chained scan up to 2^26 parameters, three kernels above), 1 = always the single
+ * pass, 2 = always the three kernels.  Both forms give identical results; for tests.            */
+int scape_set_compaction(scape_t* h, int form);
+
 /* Option: also materialise b^r on steps whose mask is all ones (step 1, or sparsity 0), where
  * the packed buffer would be R*N floats.  Off by default: on such steps SCAPE_PACKED is then
  * unavailable (SCAPE_EINVAL) and SCAPE_PACKED_MEAN equals SCAPE_MOMENT.  Allocates R*N floats
@@ -210,7 +228,9 @@ int scape_set_keep_dense_pack(scape_t* h, int on);
  * Both calls synchronise `cuda_stream` before returning.  Not part of the timed path.
  * scape_set(SCAPE_MASK_NEXT) accepts a mask with at most as many set bits as the largest mask so
  * far (scape_k at creation, grown by scape_set_sparsity / scape_set_layers), or with all N bits set;
- * bits at positions >= N are ignored.                                                          */
+ * bits at positions >= N are ignored; a mask with more bits is refused (SCAPE_EINVAL) and the
+ * handle keeps the mask it had.  scape_set is refused between scape_step_local and
+ * scape_step_apply.                                                                            */
 int scape_get(scape_t* h, int what, int r, void* buf, size_t bytes, void* cuda_stream);
 int scape_set(scape_t* h, int what, int r, const void* buf, size_t bytes, void* cuda_stream);
 int scape_set_step_count(scape_t* h, int64_t t);

@@ -33,6 +33,7 @@ SYMBOLS = {
     "scape_count": (_I64, [_VP, _I]),
     "scape_set_grad_dtype": (_I, [_VP, _I]),
     "scape_set_keep_dense_pack": (_I, [_VP, _I]),
+    "scape_set_compaction": (_I, [_VP, _I]),
     "scape_set_lr": (_I, [_VP, _D]),
     "scape_set_bias_correction": (_I, [_VP, _I]),
     "scape_set_clip_grad": (_I, [_VP, _D]),
@@ -150,6 +151,10 @@ def scape_set_grad_dtype(h, dtype):
 
 def scape_set_keep_dense_pack(h, on):
     _check(lib().scape_set_keep_dense_pack(h, int(on)), "scape_set_keep_dense_pack")
+
+
+def scape_set_compaction(h, form):
+    _check(lib().scape_set_compaction(h, int(form)), "scape_set_compaction")
 
 
 def scape_set_lr(h, lr):
@@ -437,6 +442,9 @@ class Scape:
 
     def keep_dense_pack(self, on=True):
         scape_set_keep_dense_pack(self.h, on)
+
+    def set_compaction(self, form):
+        scape_set_compaction(self.h, form)
 
     def set_step_count(self, t):
         scape_set_step_count(self.h, t)

@@ -12,7 +12,19 @@
 #include <new>
 #include <vector>
 
-#include "scape_kernels.cuh"
+#include "scape_select_kernels.cuh"
+
+// kernel lookups exported by the instantiation units (scape_fused_inst.cu)
+namespace scapek {
+#define SCAPE_DECL_INST(tag)                                                               \
+  const void* fused_step_kernel_##tag(int R, bool dense, bool msparse, bool clipt);        \
+  const void* fused_tma_kernel_##tag(int R, bool clipt, uint32_t* tile_bytes);
+SCAPE_DECL_INST(f32_lo)
+SCAPE_DECL_INST(f32_hi)
+SCAPE_DECL_INST(bf16_lo)
+SCAPE_DECL_INST(bf16_hi)
+#undef SCAPE_DECL_INST
+}  // namespace scapek
 
 using namespace scapek;
 
@@ -36,6 +48,9 @@ int fail(int code, const char* fmt, ...) {
     if (_e != cudaSuccess) return fail(SCAPE_ECUDA, "%s: %s", #expr, cudaGetErrorString(_e)); \
   } while (0)
 
+// shards of up to this many 1024-chunk blocks (2^26 parameters) compact their masks in one pass
+constexpr int kSinglePassCompactBlocks = 512;
+
 struct MaskSlot {
   uint32_t* bits = nullptr;   // [n_words]
   uint32_t* rank = nullptr;   // [n_chunks]
@@ -43,6 +58,15 @@ struct MaskSlot {
   int64_t count = 0;
   bool all_ones = false;
   bool valid = false;
+};
+
+// one streaming-kernel instantiation as this handle launches it
+struct FusedCfg {
+  const void* fn = nullptr;   // kernel address (scape_fused_inst.cu); nullptr: the instantiation does not exist
+  int bps = 0;                // resident CTAs per SM the grid is sized for
+  int stages = 0;             // staged kernel: ring depth
+  uint32_t tile = 0;          // staged kernel: bytes per stage
+  size_t smem = 0;            // staged kernel: dynamic shared memory per CTA
 };
 
 struct DeviceGuard {
@@ -82,8 +106,10 @@ struct scape {
   float* vm = nullptr;         // [Npad] clip mode: beta2 * m_old^2 of the selected entries
   double* sumsq = nullptr;     // [max_seg] clip mode: per-warp partial sums of g^^2
   ClipState* clip_state = nullptr;
-  uint32_t compact_min = 1;    // selected entries per chunk from which l.10-16 run compacted (SCAPE_COMPACT_MIN: experiments)
-  int fused_impl = 0;          // SCAPE_FUSED_IMPL (experiments): 0 auto, 1 "ldg" = register-staged kernel only
+  // launch configuration of the streaming kernels for this handle's R on this handle's device
+  // (prepare_kernels): [gradient type][variant][clip_grad instantiation]
+  FusedCfg cfg_step[2][3][2];
+  FusedCfg cfg_tma[2][2];
   bool m_sparse = false;       // m_{t-1} lives in pm[pm_last] addressed through slot[last]; h->m is stale
   float* dense_pack = nullptr;    // optional [R][Npad]
   bool last_dense = false;
@@ -100,7 +126,7 @@ struct scape {
   uint32_t* total = nullptr;      // [2]: number of set bits, ticket of mask_compact_kernel
   unsigned long long* scan_state = nullptr;   // [n_compact_blocks] look-back state of mask_compact_kernel
   uint32_t compact_epoch = 0;
-  int compact_impl = 0;           // 1 single pass (small shards), 0 count / scan / rank; SCAPE_COMPACT_IMPL overrides
+  int compact_impl = 0;           // 1 single pass (small shards), 0 count / scan / rank (scape_set_compaction)
   int n_compact_blocks = 0;
   int n_seg = 0;                  // segments (= warps) of the last fused launch
   int n_slots = 0;                // warps of the last streaming launch (clip-mode partial sums)
@@ -136,6 +162,8 @@ struct scape {
   double prof_fused_ms = 0.0, prof_select_ms = 0.0;
   int64_t prof_steps = 0;
 
+  int32_t* iota_scratch = nullptr;   // scape_get(SCAPE_IDX_*) of an all-ones mask
+
   // scape_step_host staging
   float* st_param = nullptr;
   void* st_grad[kMaxR] = {};
@@ -151,123 +179,88 @@ int grid_for(const scape* h, int64_t n_chunks, int warps_per_block, int blocks_p
   return (int)(need < cap ? need : cap);
 }
 
-template <typename G, int R, bool DENSE, bool MSPARSE>
-int launch_fused_t(scape* h, StepParams& p, cudaStream_t st) {
-  static int bps = 0;   // resident blocks per SM of this instantiation
-  if (bps == 0) {
-    int v = 0;
-    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, scape_fused_step_kernel<G, R, DENSE, MSPARSE, false>, 256, 0));
-    bps = v > 0 ? (v > 8 ? 8 : v) : 1;
-  }
-  const int grid = grid_for(h, p.n_chunks, 8, bps);
-  // one candidate segment per warp of this launch
-  h->n_seg = grid * 8;
-  h->n_slots = grid * 8;
-  int64_t cap = (h->cand_cap / h->n_seg) & ~(int64_t)15;
-  if (cap > 0x7FFFFFF0) cap = 0x7FFFFFF0;
-  h->seg_cap = (uint32_t)cap;
-  p.seg_cap = h->seg_cap;
-  // the clip_grad variant is a separate instantiation so that the default path carries none of it
-  if (p.clip) scape_fused_step_kernel<G, R, DENSE, MSPARSE, true><<<grid, 256, 0, st>>>(p);
-  else scape_fused_step_kernel<G, R, DENSE, MSPARSE, false><<<grid, 256, 0, st>>>(p);
-  h->last_kernel = "scape_fused_step_kernel";
-  h->launches++;
-  CU_TRY(cudaGetLastError());
-  return SCAPE_OK;
+// The streaming kernels are instantiated in scape_fused_inst.cu (one translation unit per gradient
+// type and range of R); their launch configuration is resolved ONCE PER HANDLE in
+// prepare_kernels(), under the handle's device: occupancy and the opt-in to more than 48 KB of
+// dynamic shared memory are per device, and handles of several devices may live in one process.
+const void* step_kernel(int dtype, int R, bool dense, bool msparse, bool clipt) {
+  const void* f = dtype == SCAPE_GRAD_BF16 ? fused_step_kernel_bf16_lo(R, dense, msparse, clipt)
+                                           : fused_step_kernel_f32_lo(R, dense, msparse, clipt);
+  if (!f) f = dtype == SCAPE_GRAD_BF16 ? fused_step_kernel_bf16_hi(R, dense, msparse, clipt)
+                                       : fused_step_kernel_f32_hi(R, dense, msparse, clipt);
+  return f;
 }
 
-template <typename G, bool DENSE, bool MSPARSE>
-int launch_fused_r(scape* h, StepParams& p, cudaStream_t st) {
-  switch (h->R) {
-    case 1: return launch_fused_t<G, 1, DENSE, MSPARSE>(h, p, st);
-    case 2: return launch_fused_t<G, 2, DENSE, MSPARSE>(h, p, st);
-    case 3: return launch_fused_t<G, 3, DENSE, MSPARSE>(h, p, st);
-    case 4: return launch_fused_t<G, 4, DENSE, MSPARSE>(h, p, st);
-    case 5: return launch_fused_t<G, 5, DENSE, MSPARSE>(h, p, st);
-    case 6: return launch_fused_t<G, 6, DENSE, MSPARSE>(h, p, st);
-    case 7: return launch_fused_t<G, 7, DENSE, MSPARSE>(h, p, st);
-    case 8: return launch_fused_t<G, 8, DENSE, MSPARSE>(h, p, st);
-  }
-  return fail(SCAPE_EINVAL, "R out of range");
+const void* tma_kernel(int dtype, int R, bool clipt, uint32_t* tile) {
+  const void* f = dtype == SCAPE_GRAD_BF16 ? fused_tma_kernel_bf16_lo(R, clipt, tile) : fused_tma_kernel_f32_lo(R, clipt, tile);
+  if (!f) f = dtype == SCAPE_GRAD_BF16 ? fused_tma_kernel_bf16_hi(R, clipt, tile) : fused_tma_kernel_f32_hi(R, clipt, tile);
+  return f;
 }
 
-// steady-state front-end with shared-memory staging (bulk copies + mbarriers)
-template <typename G, int R>
-int launch_tma_t(scape* h, StepParams& p, cudaStream_t st) {
-  static int cfg_stages = 0, cfg_bps = 0;
-  constexpr uint32_t TILE = tma_tile_bytes<G, R>();
-  if (cfg_stages == 0) {
-    // two CTAs per SM when at least 3 stages each fit, else one CTA with as many stages as fit
-    const int budget = 227 * 1024;
-    int s2 = (int)((budget / 2 - 1024 - kTmaBarrierBytes) / TILE);
-    int s1 = (int)((budget - kTmaBarrierBytes) / TILE);
-    // Two CTAs (16 consumer warps) per SM with >= 3 stages each, or not at all: with one CTA per
-    // SM the 8 consumer warps cannot keep up with HBM (measured: R = 8 fp32 gradients, 68 KB
-    // tiles, 4.8 TB/s staged vs 5.95 TB/s register-staged), so big tiles use the LDG kernel.
-    if (s2 >= 3) { cfg_stages = s2 > kTmaMaxStages ? kTmaMaxStages : s2; cfg_bps = 2; }
-    else { cfg_stages = -1; cfg_bps = 1; (void)s1; }
-    // tuning overrides (experiments only)
-    if (const char* ev = getenv("SCAPE_TMA_STAGES")) { int v = atoi(ev); if (v >= 2 && v <= kTmaMaxStages && v <= s1) cfg_stages = v; }
-    if (const char* ev = getenv("SCAPE_TMA_BPS")) { int v = atoi(ev); if (v >= 1 && v <= 4) cfg_bps = v; }
-    if (cfg_stages >= 2) {
-      const size_t smem = kTmaBarrierBytes + (size_t)cfg_stages * TILE;
-      CU_TRY(cudaFuncSetAttribute(scape_fused_tma_kernel<G, R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      CU_TRY(cudaFuncSetAttribute(scape_fused_tma_kernel<G, R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+int prepare_kernels(scape* h) {
+  for (int dt = 0; dt < 2; ++dt)
+    for (int clipt = 0; clipt < 2; ++clipt) {
+      for (int v = 0; v < 3; ++v) {          // 0 all-ones mask | 1 sparse mask, dense m in | 2 sparse mask, sparse m in
+        FusedCfg& c = h->cfg_step[dt][v][clipt];
+        c.fn = step_kernel(dt, h->R, v == 0, v == 2, clipt != 0);
+        if (!c.fn) return fail(SCAPE_EINVAL, "no streaming kernel for R = %d", h->R);
+        int occ = 0;
+        CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c.fn, 256, 0));
+        c.bps = occ > 0 ? (occ > 8 ? 8 : occ) : 1;
+      }
+      // Staged kernel: two CTAs (16 consumer warps) per SM with >= 3 stages each, or not at all
+      // (tma_can_launch in scape_kernels.cuh); as many stages as fit, at most kTmaMaxStages.
+      FusedCfg& c = h->cfg_tma[dt][clipt];
+      c.fn = tma_kernel(dt, h->R, clipt != 0, &c.tile);
+      if (c.fn) {
+        const int s2 = (int)((kSmemPerSm / 2u - 1024u - kTmaBarrierBytes) / c.tile);
+        c.stages = s2 > kTmaMaxStages ? kTmaMaxStages : s2;
+        c.bps = 2;
+        c.smem = kTmaBarrierBytes + (size_t)c.stages * c.tile;
+        CU_TRY(cudaFuncSetAttribute(c.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem));
+      }
     }
-  }
-  if (cfg_stages < 0) return 1;   // does not fit: caller uses the LDG kernel
-  const int64_t n_tiles = p.N / kTmaTile;
-  int64_t grid = (int64_t)h->n_sm * cfg_bps;
-  if (grid > n_tiles) grid = n_tiles;
-  h->n_seg = (int)grid * kTmaConsumerWarps;
-  h->n_slots = h->n_seg;
+  return SCAPE_OK;
+}
+
+void set_segments(scape* h, StepParams& p, int n_seg) {
+  // one candidate segment per warp of this launch
+  h->n_seg = n_seg;
+  h->n_slots = n_seg;
   int64_t cap = (h->cand_cap / h->n_seg) & ~(int64_t)15;
   if (cap > 0x7FFFFFF0) cap = 0x7FFFFFF0;
   h->seg_cap = (uint32_t)cap;
   p.seg_cap = h->seg_cap;
-  const size_t smem = kTmaBarrierBytes + (size_t)cfg_stages * TILE;
-  // the clip_grad variant is a separate instantiation so that the default path carries none of it
-  if (p.clip) scape_fused_tma_kernel<G, R, true><<<(int)grid, kTmaThreads, smem, st>>>(p, cfg_stages);
-  else scape_fused_tma_kernel<G, R, false><<<(int)grid, kTmaThreads, smem, st>>>(p, cfg_stages);
-  h->last_kernel = "scape_fused_tma_kernel";
-  h->launches++;
-  CU_TRY(cudaGetLastError());
-  return SCAPE_OK;
-}
-
-template <typename G>
-int launch_tma_r(scape* h, StepParams& p, cudaStream_t st) {
-  switch (h->R) {
-    case 1: return launch_tma_t<G, 1>(h, p, st);
-    case 2: return launch_tma_t<G, 2>(h, p, st);
-    case 3: return launch_tma_t<G, 3>(h, p, st);
-    case 4: return launch_tma_t<G, 4>(h, p, st);
-    case 5: return launch_tma_t<G, 5>(h, p, st);
-    case 6: return launch_tma_t<G, 6>(h, p, st);
-    case 7: return launch_tma_t<G, 7>(h, p, st);
-    case 8: return launch_tma_t<G, 8>(h, p, st);
-  }
-  return fail(SCAPE_EINVAL, "R out of range");
 }
 
 // variants: all-ones mask (dense m in and out) | sparse mask, dense m in | sparse mask, sparse m in
-template <typename G>
-int launch_fused_g(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t st) {
+int launch_fused(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t st) {
+  const int dt = h->grad_dtype == SCAPE_GRAD_BF16 ? 1 : 0, clipt = p.clip ? 1 : 0;   // the clip_grad variant is its own instantiation
   // The staged kernel wins when there are enough bytes per parameter to be HBM-bound (R >= 3);
   // with one or two replicas the step is issue-bound and the register-staged kernel's higher
   // occupancy (40 warps/SM vs 16 consumer warps) is worth more (measured at N = 2^28, 99 %:
   // R = 1: 1.49 vs 2.02 ms, R = 2: 1.95 vs 2.08 ms, R = 4: 2.94 vs 2.72 ms).
-  if (!dense && msparse && h->fused_impl != 1 && h->R >= 3 && p.N / kTmaTile >= (int64_t)h->n_sm) {
-    const int rc = launch_tma_r<G>(h, p, st);
-    if (rc <= 0) return rc;      // 1 = tile does not fit in shared memory: fall through
+  const FusedCfg& ct = h->cfg_tma[dt][clipt];
+  if (!dense && msparse && ct.fn && h->R >= 3 && p.N / kTmaTile >= (int64_t)h->n_sm) {
+    const int64_t n_tiles = p.N / kTmaTile;
+    int64_t grid = (int64_t)h->n_sm * ct.bps;
+    if (grid > n_tiles) grid = n_tiles;
+    set_segments(h, p, (int)grid * kTmaConsumerWarps);
+    int stages = ct.stages;
+    void* args[] = {(void*)&p, (void*)&stages};
+    CU_TRY(cudaLaunchKernel(ct.fn, dim3((unsigned)grid), dim3(kTmaThreads), args, ct.smem, st));
+    h->last_kernel = "scape_fused_tma_kernel";
+    h->launches++;
+    return SCAPE_OK;
   }
-  if (dense) return launch_fused_r<G, true, false>(h, p, st);
-  return msparse ? launch_fused_r<G, false, true>(h, p, st) : launch_fused_r<G, false, false>(h, p, st);
-}
-
-int launch_fused(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t st) {
-  if (h->grad_dtype == SCAPE_GRAD_BF16) return launch_fused_g<__nv_bfloat16>(h, p, dense, msparse, st);
-  return launch_fused_g<float>(h, p, dense, msparse, st);
+  const FusedCfg& c = h->cfg_step[dt][dense ? 0 : msparse ? 2 : 1][clipt];
+  const int grid = grid_for(h, p.n_chunks, 8, c.bps);
+  set_segments(h, p, grid * 8);
+  void* args[] = {(void*)&p};
+  CU_TRY(cudaLaunchKernel(c.fn, dim3((unsigned)grid), dim3(256), args, 0, st));
+  h->last_kernel = "scape_fused_step_kernel";
+  h->launches++;
+  return SCAPE_OK;
 }
 
 // dense view of m in h->m when it is stored sparsely (accessors; all-ones step after sparse ones)
@@ -368,20 +361,27 @@ int ensure_capacity(scape* h, int64_t K) {
     if (!ok) return fail(SCAPE_ENOMEM, "device allocation failed (packed buffers for %lld selected entries)", (long long)K);
     h->packed_stride = stride;
   }
-  if (!h->cand) {
+  {
     // candidates of the fused select: room for 4k keys (a bracket of +-3 % around the threshold
-    // holds ~0.8k: error feedback piles residuals up just below it), at least N/8, at most N/2
+    // holds ~0.8k: error feedback piles residuals up just below it), at least N/8, at most N/2.
+    // Grows with the largest K seen (density warm-up from the sparse side); its contents only live
+    // inside a step, so nothing is copied.  Never shrinks.
     int64_t cc = 4 * K;
     if (cc < h->N / 8) cc = h->N / 8;      // very sparse masks / transients: keep room per warp segment
     if (cc > h->N / 2) cc = h->N / 2;
     if (cc < 65536) cc = 65536;
-    if (cudaMalloc((void**)&h->cand, sizeof(unsigned long long) * (size_t)cc) != cudaSuccess ||
-        cudaMalloc((void**)&h->cls, sizeof(unsigned long long) * (size_t)kClsCap) != cudaSuccess) {
-      cudaGetLastError();
-      cudaFree(h->cand); h->cand = nullptr;
-      return fail(SCAPE_ENOMEM, "device allocation failed (candidate list)");
+    if (!h->cls && cudaMalloc((void**)&h->cls, sizeof(unsigned long long) * (size_t)kClsCap) != cudaSuccess) {
+      cudaGetLastError(); h->cls = nullptr;
+      return fail(SCAPE_ENOMEM, "device allocation failed (small list of the select)");
     }
-    h->cand_cap = cc;
+    if (cc > h->cand_cap) {
+      if (h->cand) { CU_TRY(cudaDeviceSynchronize()); cudaFree(h->cand); h->cand = nullptr; h->cand_cap = 0; }
+      if (cudaMalloc((void**)&h->cand, sizeof(unsigned long long) * (size_t)cc) != cudaSuccess) {
+        cudaGetLastError(); h->cand = nullptr;
+        return fail(SCAPE_ENOMEM, "device allocation failed (candidate list)");
+      }
+      h->cand_cap = cc;
+    }
   }
   return SCAPE_OK;
 }
@@ -462,7 +462,7 @@ void free_all(scape* h) {
   cudaFree(h->sel); cudaFree(h->cand); cudaFree(h->cls); cudaFree(h->seg_count); cudaFree(h->seg_above); cudaFree(h->ghist); cudaFree(h->block_sum); cudaFree(h->total); cudaFree(h->scan_state);
   cudaFree(h->ghat); cudaFree(h->vm); cudaFree(h->sumsq); cudaFree(h->clip_state);
   cudaFree(h->layers); cudaFree(h->lctl); cudaFree(h->chunk_layer); cudaFree(h->lhist); cudaFree(h->items);
-  cudaFree(h->st_param);
+  cudaFree(h->st_param); cudaFree(h->iota_scratch);
   for (auto& g : h->st_grad) cudaFree(g);
   if (h->prof_have_events)
     for (auto& row : h->prof_ev) for (auto& ev : row) cudaEventDestroy(ev);
@@ -487,10 +487,6 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   scape* h = new (std::nothrow) scape();
   if (!h) { fail(SCAPE_ENOMEM, "host allocation failed"); return nullptr; }
   h->dev = dev;
-  if (const char* ev = getenv("SCAPE_COMPACT_MIN")) { int v = atoi(ev); if (v >= 1) h->compact_min = (uint32_t)v; }
-  if (const char* ev = getenv("SCAPE_NARROW")) { float v = (float)atof(ev); if (v > 0.1f && v < 1.0f) cudaMemcpyToSymbol(g_narrow, &v, sizeof v); }
-  if (const char* ev = getenv("SCAPE_ERR_MULT")) { float v = (float)atof(ev); if (v >= 1.0f && v < 100.0f) cudaMemcpyToSymbol(g_err_mult, &v, sizeof v); }
-  if (const char* ev = getenv("SCAPE_FUSED_IMPL")) h->fused_impl = (strcmp(ev, "ldg") == 0) ? 1 : 0;
   cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev);
   h->N = N; h->R = R;
   h->Npad = (N + kChunk - 1) / kChunk * kChunk;
@@ -527,8 +523,7 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   alloc((void**)&h->scan_state, sizeof(unsigned long long) * (h->n_compact_blocks + 1), true);
   // measured: the single pass wins while launch count matters (pr1: select stage 99 -> 94 us) and loses on
   // large shards, where 13.5 k CTAs wait on one another's prefixes (headline: 0.44 -> 0.50 ms)
-  h->compact_impl = h->n_compact_blocks <= 512 ? 1 : 0;
-  if (const char* ev = getenv("SCAPE_COMPACT_IMPL")) h->compact_impl = atoi(ev) != 0;
+  h->compact_impl = h->n_compact_blocks <= kSinglePassCompactBlocks ? 1 : 0;
   if (!ok) {
     fail(SCAPE_ENOMEM, "device allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
     free_all(h); delete h; return nullptr;
@@ -542,6 +537,7 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
       free_all(h); delete h; return nullptr;
     }
   }
+  if (prepare_kernels(h) != SCAPE_OK) { free_all(h); delete h; return nullptr; }
   h->slot[0].all_ones = true;                                                // l.1: M_0 = 1
   h->slot[0].count = N;
   h->slot[0].valid = true;
@@ -597,6 +593,13 @@ extern "C" int scape_set_keep_dense_pack(scape_t* h, int on) {
     cudaFree(h->dense_pack);
     h->dense_pack = nullptr;
   }
+  return SCAPE_OK;
+}
+
+extern "C" int scape_set_compaction(scape_t* h, int form) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (form < 0 || form > 2) return fail(SCAPE_EINVAL, "form must be 0 (by size), 1 (single pass) or 2 (three kernels)");
+  h->compact_impl = form == 0 ? (h->n_compact_blocks <= kSinglePassCompactBlocks ? 1 : 0) : form == 1 ? 1 : 0;
   return SCAPE_OK;
 }
 
@@ -793,7 +796,6 @@ int step_impl(scape_t* h, float* param, const void* const* grads, void* cuda_str
   p.R_f = (float)h->R; p.inv_R = 1.0f / (float)h->R;
   p.r_pow2 = (h->R & (h->R - 1)) == 0;      // x / 2^n == x * 2^-n bit for bit
   p.stash = cur.all_ones && need_select;
-  p.compact_min = h->compact_min;
   p.bc1 = 1.0f; p.bc2 = 1.0f;
   if (h->bias_correction) {      // PAPER.md:77; factors evaluated in double from the step number, cast once
     const double t = (double)(h->t + 1);
@@ -1066,14 +1068,21 @@ int get_idx(scape* h, MaskSlot& s, void* buf, size_t bytes, cudaStream_t st) {
     CU_TRY(cudaMemcpyAsync(buf, s.idx, bytes, cudaMemcpyDefault, st));
     return SCAPE_OK;
   }
-  int32_t* tmp = nullptr;
-  CU_TRY(cudaMalloc((void**)&tmp, bytes));
-  iota_i32_kernel<<<256, 256, 0, st>>>(tmp, h->N);
-  h->launches++;
-  cudaError_t e1 = cudaMemcpyAsync(buf, tmp, bytes, cudaMemcpyDefault, st);
-  cudaError_t e2 = cudaStreamSynchronize(st);
-  cudaFree(tmp);
-  if (e1 != cudaSuccess || e2 != cudaSuccess) return fail(SCAPE_ECUDA, "idx copy failed");
+  // all-ones mask: the list is 0 .. N-1, produced piecewise in a small scratch kept by the handle
+  constexpr int64_t kPiece = 1 << 20;
+  if (!h->iota_scratch) {
+    if (cudaMalloc((void**)&h->iota_scratch, sizeof(int32_t) * kPiece) != cudaSuccess) {
+      h->iota_scratch = nullptr; cudaGetLastError();
+      return fail(SCAPE_ENOMEM, "idx: scratch allocation failed");
+    }
+  }
+  for (int64_t lo = 0; lo < h->N; lo += kPiece) {
+    const int64_t n = std::min<int64_t>(kPiece, h->N - lo);
+    iota_i32_kernel<<<256, 256, 0, st>>>(h->iota_scratch, n, (int32_t)lo);
+    h->launches++;
+    CU_TRY(cudaMemcpyAsync((char*)buf + sizeof(int32_t) * (size_t)lo, h->iota_scratch, sizeof(int32_t) * (size_t)n, cudaMemcpyDefault, st));
+    CU_TRY(cudaStreamSynchronize(st));        // the scratch is reused by the next piece (the copy may be staged)
+  }
   return SCAPE_OK;
 }
 
@@ -1141,6 +1150,7 @@ extern "C" int scape_get(scape_t* h, int what, int r, void* buf, size_t bytes, v
 
 extern "C" int scape_set(scape_t* h, int what, int r, const void* buf, size_t bytes, void* cuda_stream) {
   if (!h || !buf) return fail(SCAPE_EINVAL, "NULL argument");
+  if (h->pending) return fail(SCAPE_EINVAL, "a split step is in flight: scape_step_apply first");
   DeviceGuard guard(h->dev);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t nbytes = sizeof(float) * (size_t)h->N;
@@ -1156,7 +1166,9 @@ extern "C" int scape_set(scape_t* h, int what, int r, const void* buf, size_t by
       CU_TRY(cudaMemcpyAsync(h->e + (size_t)r * h->Npad, buf, bytes, cudaMemcpyDefault, st));
       break;
     case SCAPE_MASK_NEXT: {
-      MaskSlot& s = h->slot[h->use];
+      // The mask is validated in the `build` slot (free between steps: it holds M_{t-2}) and only
+      // then becomes the `use` slot, so a refused mask leaves the handle as it was.
+      MaskSlot& s = h->slot[h->build];
       const size_t mb = sizeof(uint32_t) * (size_t)((h->N + 31) / 32);
       if (bytes != mb) return fail(SCAPE_EINVAL, "mask: expected %zu bytes", mb);
       CU_TRY(cudaMemsetAsync(s.bits, 0, sizeof(uint32_t) * h->n_words, st));
@@ -1169,15 +1181,17 @@ extern "C" int scape_set(scape_t* h, int what, int r, const void* buf, size_t by
       uint32_t total = 0;
       CU_TRY(cudaMemcpyAsync(&total, h->total, sizeof total, cudaMemcpyDeviceToHost, st));
       CU_TRY(cudaStreamSynchronize(st));
-      if ((int64_t)total == h->N) {
-        s.all_ones = true; s.count = h->N; s.valid = true;
-      } else if ((int64_t)total <= h->packed_stride) {
-        s.all_ones = false; s.count = total; s.valid = true;
-        if ((rc = compact_mask(h, s, true, st))) return rc;
-      } else {
-        s.all_ones = true; s.count = h->N; s.valid = true;   // fall back to a defined state
+      s.valid = false;
+      if ((int64_t)total != h->N && (int64_t)total > h->packed_stride)
         return fail(SCAPE_EINVAL, "mask: %u bits set, at most %lld (the packed capacity) or all N allowed", total, (long long)h->packed_stride);
+      if ((int64_t)total == h->N) {
+        s.all_ones = true; s.count = h->N;
+      } else {
+        s.all_ones = false; s.count = total;
+        if ((rc = compact_mask(h, s, true, st))) return rc;
       }
+      s.valid = true;
+      std::swap(h->use, h->build);
       break;
     }
     default:

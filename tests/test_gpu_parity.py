@@ -83,13 +83,15 @@ def compare_step(gpu, ora, th_gpu, th_ora, R, tag, exact=True):
             assert np.array_equal(gpu.residual(r).view(np.uint32), ora.e(r).view(np.uint32)), f"{tag} e[{r}] not bit-exact"
 
 
-def run_reload_parity(B, w, steps, seed=0, hyp=HYP):
+def run_reload_parity(B, w, steps, seed=0, hyp=HYP, setup=None):
     """Per-step parity 'when both start from identical state each step'."""
     N, R = w.numel, w.R
     gs = synth.GradStream(w, device="cuda", seed=seed)
     th0 = gs.theta0()
     gpu = B.Scape(N, R, w.sparsity, **hyp)
     gpu.keep_dense_pack(True)
+    if setup is not None:
+        setup(gpu)
     ora = ScapeOracle(N, R, w.sparsity, **hyp)
     assert gpu.k == ora.k
     th_ora = th0.cpu().numpy().copy()
@@ -398,11 +400,11 @@ def test_clip_grad_above_the_norm_is_a_bitwise_noop(B):
     b.close()
 
 
-@pytest.mark.parametrize("impl", ["0", "1"])
-def test_both_compaction_forms(B, monkeypatch, impl):
+@pytest.mark.parametrize("form", [1, 2])
+def test_both_compaction_forms(B, form):
     """rank128 + index list from the mask bits: the three-kernel form (large shards) and the single-pass
-    chained scan (small shards) are chosen by size; both run here on the same ragged shard."""
-    monkeypatch.setenv("SCAPE_COMPACT_IMPL", impl)
-    w = synth.Workload(f"compact{impl}", [("a", 300_000), ("b", 1024 * 700 + 77)], R=2, sparsity=0.97, dist="t3", rho=0.9,
+    chained scan (small shards) are chosen by size; scape_set_compaction forces either on the same
+    ragged shard."""
+    w = synth.Workload(f"compact{form}", [("a", 300_000), ("b", 1024 * 700 + 77)], R=2, sparsity=0.97, dist="t3", rho=0.9,
                        grad_dtype="f32", steps=5)
-    run_reload_parity(B, w, steps=5, seed=int(impl))
+    run_reload_parity(B, w, steps=5, seed=form, setup=lambda gpu: gpu.set_compaction(form))
