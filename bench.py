@@ -59,6 +59,12 @@ def parse():
     ap.add_argument("--sweep-log2n", default="20,21,22,23,24,25,26,27,28,29,30")
     ap.add_argument("--sweep-sparsity", default="0,0.9,0.99,0.999")
     ap.add_argument("--sweep-R", default="1,2,4,8")
+    ap.add_argument("--no-also", action="store_true",
+                    help="skip `also_measured` (the other BASELINE.json configs timed after the headline region, N = 1 only)")
+    ap.add_argument("--also-steps", type=int, default=10)
+    ap.add_argument("--plumbing-only", action="store_true",
+                    help="launcher / rendezvous / barrier / max-over-ranks / JSON line WITHOUT the CUDA step, on the gloo backend: "
+                         "what tests/test_multirank_cpu.py runs on a CPU box; the line says so and carries no measurement")
     return ap.parse_args()
 
 
@@ -288,6 +294,105 @@ def whole_job_value(n_params, steps, elapsed_ms, world):
     return world * n_params * steps / (elapsed_ms * 1e-3)
 
 
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without a launcher around it: start the N ranks here, exactly as the
+    driver's own command line does (torch.distributed.run, one node, 127.0.0.1), and hand on their
+    output and exit code.  Under torchrun (WORLD_SIZE set) this is never reached."""
+    import socket
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+def run_plumbing_only(args):
+    """The N > 1 host logic with no GPU: rendezvous, barrier, max over ranks, whole-job aggregate, one
+    JSON line from rank 0.  Every rank pretends its region took (10 + 5 rank) ms."""
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    if world > 1:
+        dist.init_process_group("gloo")
+        dist.barrier()
+    K = args.steps
+    ms = max_over_ranks_ms(10.0 + 5.0 * rank, world, torch.device("cpu"))
+    if world > 1:
+        dist.barrier()
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": None, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+                          "ms_per_step": None, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                          "plumbing_only": {"note": "no CUDA step was run (CPU test of the launcher)", "max_over_ranks_ms": ms,
+                                            "aggregate_of_fake_region": whole_job_value(1000, K, ms, world)},
+                          "gpu_launches": 0}), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def timed_region(step, theta, ring, first, K):
+    """K back-to-back steps, one CUDA event before each and one after the last (all on torch's current
+    stream, the one the step is enqueued on).  -> (elapsed ms of the whole region, per-step ms list)."""
+    import torch
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
+    n_sets = len(ring)
+    for i in range(K):
+        ev[i].record()
+        step(theta, ring[(first + i) % n_sets])
+    ev[K].record()
+    torch.cuda.synchronize()
+    per = [ev[i].elapsed_time(ev[i + 1]) for i in range(K)]
+    return ev[0].elapsed_time(ev[K]), per
+
+
+def step_stats(per):
+    s = sorted(per)
+    return {"ms_median": s[len(s) // 2] if len(s) % 2 else 0.5 * (s[len(s) // 2 - 1] + s[len(s) // 2]),
+            "ms_min": s[0], "ms_max": s[-1]}
+
+
+def measure_also(name, w, theta, ring, K, W, peak, layers=False):
+    """One more workload timed like the headline (dense first step, W warm-up steps, K timed steps
+    with per-step events), reported in `also_measured`."""
+    import torch
+    from paper_2607_01678_b200 import binding
+    N, R = w.numel, w.R
+    sc = binding.Scape(N, R, w.sparsity, **w.hyper)
+    if layers:
+        sc.set_layers(w.offsets(), w.compress_flags())
+    k = sc.k
+    n_sets = len(ring)
+    sc.step(theta, ring[0])
+    for i in range(W):
+        sc.step(theta, ring[(1 + i) % n_sets])
+    torch.cuda.synchronize()
+    sc.profile(True)
+    f0, g0 = sc.select_stats()
+    l0 = sc.launches
+    elapsed, per = timed_region(sc.step, theta, ring, 1 + W, K)
+    fused_ms, select_ms, psteps = sc.profile_read()
+    sc.profile(False)
+    f1, g1 = sc.select_stats()
+    ms = elapsed / K
+    kms = fused_ms / max(1, psteps)
+    fb = bytes_per_param_fused(w, k, N) * N
+    sb = bytes_per_param_step(w, k, N) * N
+    out = {"workload": name, "shard_numel": N, "R": R, "grad_dtype": w.grad_dtype, "sparsity": w.sparsity, "k": k,
+           "refresh": "per layer (one top-k per tensor)" if layers else "flat top-k over the shard",
+           "steps": K, "warmup": W, "ms_per_step": ms, **step_stats(per), "params_per_s": N / (ms * 1e-3),
+           "kernel": sc.last_kernel, "kernel_ms": kms, "kernel_share_of_step": kms / ms,
+           "kernel_gbs": fb / (kms * 1e-3) / 1e9, "kernel_frac_of_peak": fb / (kms * 1e-3) / 1e9 / peak,
+           "select_ms": select_ms / max(1, psteps), "step_gbs": sb / (ms * 1e-3) / 1e9,
+           "step_frac_of_peak": sb / (ms * 1e-3) / 1e9 / peak,
+           "select_fast": f1 - f0, "select_general": g1 - g0, "gpu_launches": sc.launches - l0,
+           "l2_resident": (8 + (grad_bytes(w) + 4) * R) * N < 126e6}
+    assert bool(torch.isfinite(theta).all())
+    sc.close()
+    return out
+
+
 # ---------------------------------------------------------------------------------------------
 def main():
     args = parse()
@@ -295,6 +400,10 @@ def main():
         return run_reference(args)
     if args.sweep:
         return run_sweep(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(spawn_ranks(args))
+    if args.plumbing_only:
+        return run_plumbing_only(args)
 
     import torch
     import torch.distributed as dist
@@ -355,13 +464,7 @@ def main():
     sc.profile(True)
     launches0 = sc.launches
     fast0, general0 = sc.select_stats()
-    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t0.record()
-    for i in range(K):
-        step(theta, ring[(1 + W + i) % n_sets])
-    t1.record()
-    torch.cuda.synchronize()
-    elapsed_ms = t0.elapsed_time(t1)
+    elapsed_ms, per_step = timed_region(step, theta, ring, 1 + W, K)
     fused_ms, select_ms, psteps = sc.profile_read()
     kernel_name = sc.last_kernel
     sc.profile(False)
@@ -398,7 +501,29 @@ def main():
     }
 
     sc.close()
-    del ring, sc
+    del sc
+
+    # ---- the rest of `metric` ("at 90 %/99 % sparsity", the other model shapes), same run, N = 1 only
+    also = None
+    if world == 1 and not args.no_also and not args.workers and not args.layers and w.name == "llama1p8b":
+        Ka, Wa = max(1, args.also_steps), 6
+        also = [measure_also("llama1p8b --layers", w, theta, ring, Ka, Wa, peak, layers=True)]
+        del ring, theta
+        torch.cuda.empty_cache()
+        cache = {}                                   # llama500m at 99 % re-uses the inputs drawn for 90 %
+        for nm, sp in (("llama500m", 0.9), ("llama500m", None), ("gpt345m", None), ("pr1", None)):
+            wa = synth.workload(nm, sparsity=sp)
+            if nm not in cache:
+                cache.clear()
+                torch.cuda.empty_cache()
+                ga = synth.GradStream(wa, device=dev, seed=args.seed)
+                th0 = ga.theta0()
+                cache[nm] = (th0, [ga.next() for _ in range(2)])
+                del ga, th0
+            also.append(measure_also(nm, wa, cache[nm][0].clone(), cache[nm][1], Ka, Wa, peak))
+        cache.clear()
+    else:
+        del ring, theta
     torch.cuda.empty_cache()
 
     # ---- end to end through the C-ABI with HOST buffers ---------------------------------------
@@ -442,7 +567,7 @@ def main():
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_per_step, **step_stats(per_step), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic (seeded; shapes and distributions of BASELINE.json configs)",
             "config": {"workload": w.name, "shard_numel": N, "R": R, "sparsity": w.sparsity, "k": k,
                        "grad_dtype": w.grad_dtype, "dist": w.dist, "ar1_rho": w.rho, "hyper": w.hyper,
@@ -453,6 +578,7 @@ def main():
                        "refresh": "per layer (one top-k per tensor)" if (args.layers or args.workers) else "flat top-k over the shard",
                        "first_dense_step_ms": first_step_ms},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": gpu_launches, "clocks": clk,
+            "also_measured": also,
         }
         print(json.dumps(line), flush=True)
     if world > 1 or args.workers:

@@ -22,6 +22,12 @@
 //   P15 workers: every layer's mask == brute force on ITS OWNER's |m-tilde|; the
 //       two-level sum equals the flat mean (double, 1e-15); W = R with one owner == the plain step
 //   P16 mask bit pack / unpack (oracle/scape_oracle.py, a plain loop) vs numpy packbits and an example
+//   P17 bf16 round-to-nearest-even vs the torch CPU conversion, crafted ties, denormals, +-0
+//   P18 Algorithm 2 parameter side: a non-owner's FP32 copy kept up by pack / all-gather / apply equals
+//       the owner's theta of Algorithm 1 bit for bit, every step (fp32 payload); with a bf16 payload
+//       the compute copy equals bf16(theta) on the mask; the mask of the exchange is the one the last
+//       update used (any other mask breaks it)
+//   P19 hand example tests/golden/p19_alg2_param_example.json;  P20 Eq. 6 literal vs l.17 with u = 0: <= 1 ulp
 // Unpinned by the paper (decisions): S3 clip_grad off by default and,
 // when switched on, the torch/Megatron rule; S4 bias correction off by default; S8 replica 0 owns
 // the statistic; S9 flat top-k by default, per-layer top-k with uncompressed
@@ -317,3 +323,81 @@ template <class T> void copy_out(const std::vector<T>& v, T* dst) {
 
 ORACLE_API(f32, float)
 ORACLE_API(f64, double)
+
+// ---------------------------------------------------------------------------------------------
+// Algorithm 2, parameter side (PAPER.md:222-242; Eq. 6, :207-211; "Use FP32 w to compute
+// untransmitted params", :231-232).  With a partitioned (distributed) optimizer only the OWNER of a
+// partition holds its updated parameters w'.  Every other worker keeps a full FP32 copy w and the
+// compute copy w^ (BF16 parameters), and brings both up to date from
+//   l.2  w~ <- w'[M]                      the owner's updated parameters on the mask, packed in
+//                                         ascending index order (fp32, or rounded to bf16: RNE)
+//   l.3  w^[M] <- AllGather(w~)           (the all-gather itself is the caller's)
+//   l.4  w^[not M] <- (1 - eta lambda) w^[not M], computed from the FP32 copy w
+// where M is the mask the last update used (Eq. 6 is about theta_{t+1}[not M_{t-1}]; DESIGN.md
+// reading S22).  Reading S21: the FP32 copy is updated in place, w[M] <- payload, w[not M] by
+// Alg. 1 l.17 with u = 0 -- fma(-eta, lambda*w, w), the arithmetic the owner itself applies off the
+// mask (reading S13) -- so that with an fp32 payload the copy equals the owner's theta to the bit;
+// w^ = bf16(w) everywhere.  form = 1 computes Eq. 6 literally, (1 - eta*lambda) * w, for pin P20.
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+// float -> bfloat16, round to nearest, ties to even, written out from the definition: keep the upper
+// 16 bits; the dropped 16 bits are compared with one half (0x8000); above -> up, below -> down,
+// exactly half -> towards the even kept value.  NaN keeps its sign and gets a quiet payload.
+uint16_t bf16_rne(float x) {
+  uint32_t u;
+  std::memcpy(&u, &x, sizeof u);
+  if ((u & 0x7F800000u) == 0x7F800000u && (u & 0x007FFFFFu) != 0u) return (uint16_t)((u >> 16) | 0x0040u);   // NaN
+  const uint32_t kept = u >> 16, dropped = u & 0xFFFFu;
+  uint32_t r = kept;
+  if (dropped > 0x8000u) r = kept + 1u;
+  else if (dropped == 0x8000u) r = kept + (kept & 1u);
+  return (uint16_t)r;          // a carry out of the mantissa moves to the next exponent (or to inf): correct by construction
+}
+
+float bf16_widen(uint16_t b) {
+  const uint32_t u = (uint32_t)b << 16;
+  float x;
+  std::memcpy(&x, &u, sizeof x);
+  return x;
+}
+
+}  // namespace
+
+extern "C" uint16_t oracle_bf16_rne(float x) { return bf16_rne(x); }
+extern "C" float oracle_bf16_widen(uint16_t b) { return bf16_widen(b); }
+extern "C" void oracle_bf16_rne_array(const float* x, int64_t n, uint16_t* out) { for (int64_t i = 0; i < n; ++i) out[i] = bf16_rne(x[i]); }
+
+// l.2: out[j] = w_local[i_j], i_0 < i_1 < ... the positions with mask[i] != 0.  Returns the count.
+// out_f32 or out_bf16 (exactly one non-null).
+extern "C" int64_t oracle_param_pack(const float* w_local, const uint8_t* mask, int64_t N, float* out_f32, uint16_t* out_bf16) {
+  int64_t j = 0;
+  for (int64_t i = 0; i < N; ++i) {
+    if (!mask[i]) continue;
+    if (out_f32) out_f32[j] = w_local[i];
+    if (out_bf16) out_bf16[j] = bf16_rne(w_local[i]);
+    ++j;
+  }
+  return j;
+}
+
+// l.3-4 on a non-owner: w [N] FP32 copy, updated in place; w_hat [N] bf16 compute copy (may be null);
+// payload in ascending index order of the mask, fp32 or bf16 (exactly one non-null).
+extern "C" void oracle_param_apply(float* w, uint16_t* w_hat, const uint8_t* mask, int64_t N, const float* payload_f32,
+                                   const uint16_t* payload_bf16, double lr_d, double wd_d, int form) {
+  const float lr = (float)lr_d, wd = (float)wd_d;           // cast once, like Alg. 1's hyper-parameters
+  int64_t j = 0;
+  for (int64_t i = 0; i < N; ++i) {
+    if (mask[i]) {                                           // l.3
+      w[i] = payload_f32 ? payload_f32[j] : bf16_widen(payload_bf16[j]);
+      ++j;
+    } else if (form == 0) {                                  // l.4 as Alg. 1 l.17 with u = 0 (S13, S21)
+      const float d = std::fma(wd, w[i], 0.0f);
+      w[i] = std::fma(-lr, d, w[i]);
+    } else {                                                 // l.4 / Eq. 6 literally
+      const float f = 1.0f - lr * wd;
+      w[i] = f * w[i];
+    }
+    if (w_hat) w_hat[i] = bf16_rne(w[i]);
+  }
+}

@@ -228,3 +228,57 @@ def mask_unpack(words, n):
     """The inverse of mask_pack, entry by entry: uint8 [n] of 0 / 1."""
     w = np.asarray(words, dtype=np.uint32)
     return np.array([(int(w[i // 32]) >> (i % 32)) & 1 for i in range(n)], dtype=np.uint8)
+
+
+# ---- Algorithm 2, parameter side (PAPER.md:222-242; scape_oracle.cpp "Algorithm 2") ----------------
+def bf16_rne(x):
+    """float32 array -> uint16 array of bfloat16 bit patterns, round to nearest even (the C++ definition, entry by entry)."""
+    a = np.ascontiguousarray(x, dtype=np.float32).ravel()
+    out = np.empty(a.size, np.uint16)
+    fn = _lib().oracle_bf16_rne_array
+    fn.restype, fn.argtypes = None, [ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p]
+    fn(a.ctypes.data, a.size, out.ctypes.data)
+    return out
+
+
+def bf16_widen(b):
+    """uint16 bfloat16 bit patterns -> float32 (exact)."""
+    return (np.asarray(b, dtype=np.uint16).astype(np.uint32) << 16).view(np.float32)
+
+
+def param_pack(w_local, mask, dtype="f32"):
+    """Alg. 2 l.2: the owner's parameters on the mask, packed in ascending index order.
+    dtype "f32" -> float32 array, "bf16" -> uint16 bit patterns (RNE)."""
+    w = np.ascontiguousarray(w_local, dtype=np.float32)
+    m = np.ascontiguousarray(mask, dtype=np.uint8)
+    assert w.size == m.size
+    K = int(np.count_nonzero(m))
+    fn = _lib().oracle_param_pack
+    fn.restype = ctypes.c_int64
+    fn.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
+    if dtype == "f32":
+        out = np.empty(K, np.float32)
+        n = fn(w.ctypes.data, m.ctypes.data, w.size, out.ctypes.data, None)
+    else:
+        out = np.empty(K, np.uint16)
+        n = fn(w.ctypes.data, m.ctypes.data, w.size, None, out.ctypes.data)
+    assert n == K
+    return out
+
+
+def param_apply(w, mask, payload, lr, wd, w_hat=None, form=0):
+    """Alg. 2 l.3-4 on a non-owner: `w` (float32 [N]) is updated in place, `w_hat` (uint16 [N], optional)
+    receives bf16(w).  payload: float32 or uint16 (bf16 bits), one value per set mask entry, index order."""
+    assert w.dtype == np.float32 and w.flags.c_contiguous
+    m = np.ascontiguousarray(mask, dtype=np.uint8)
+    p = np.ascontiguousarray(payload)
+    assert p.dtype in (np.float32, np.uint16) and p.size == int(np.count_nonzero(m)) and m.size == w.size
+    if w_hat is not None:
+        assert w_hat.dtype == np.uint16 and w_hat.flags.c_contiguous and w_hat.size == w.size
+    fn = _lib().oracle_param_apply
+    fn.restype = None
+    fn.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p,
+                   ctypes.c_double, ctypes.c_double, ctypes.c_int]
+    fn(w.ctypes.data, None if w_hat is None else w_hat.ctypes.data, m.ctypes.data, w.size,
+       p.ctypes.data if p.dtype == np.float32 else None, p.ctypes.data if p.dtype == np.uint16 else None,
+       float(lr), float(wd), int(form))

@@ -142,6 +142,19 @@ def test_fullsize_sampled_and_property_parity(name):
     idx_last = torch.from_numpy(sc.idx_last()).cuda().long()
     b0 = get_f32_device(B, sc, B.SCAPE_PACKED, 0, k)
     keys[idx_last] = b0.abs()
+    # ---- (a') the sparse buffer itself at the sampled on-mask positions: b^r and b- (l.9, l.10) sit at
+    # packed position j with idx_last[j] = i; the small oracle's packed order is the sampled positions'
+    on_s = torch.from_numpy(cur_s.astype(bool)).cuda()
+    samp_on = samp[on_s]
+    j_on = torch.searchsorted(idx_last, samp_on)
+    assert bool((idx_last[j_on] == samp_on).all()), "a sampled on-mask position is missing from the index list"
+    assert samp_on.numel() == ora.K_last and samp_on.numel() >= 300
+    for r in range(R):
+        b_g = (b0 if r == 0 else get_f32_device(B, sc, B.SCAPE_PACKED, r, k))[j_on].cpu().numpy()
+        assert np.array_equal(b_g.view(np.uint32), ora.b(r).view(np.uint32)), f"b[{r}] differs on sampled on-mask positions"
+    bb_g = get_f32_device(B, sc, B.SCAPE_PACKED_MEAN, 0, k)[j_on].cpu().numpy()
+    assert np.array_equal(bb_g.view(np.uint32), ora.bbar().view(np.uint32)), "b-bar differs on sampled on-mask positions"
+
     def check_topk(keys_l, nxt_l, k_l):
         assert int(nxt_l.sum()) == k_l
         if k_l == keys_l.numel():

@@ -51,9 +51,13 @@ def to_np32(g):
     return g.detach().to(torch.float32).cpu().numpy()
 
 
-def load_state(gpu, ora, R):
-    """Copy the oracle's state (m, e^r, mask the coming step uses, t) into the CUDA handle."""
-    gpu.set_moment(ora.m())
+def load_state(gpu, ora, R, moment=True):
+    """Copy the oracle's state (m, e^r, mask the coming step uses, t) into the CUDA handle.
+    moment=False leaves m as the handle carries it (sparsely, as the previous step's packed mean:
+    loading a dense m would switch the next step to the dense-m kernel variant); compare_step has
+    already shown it equal to the oracle's to the bit."""
+    if moment:
+        gpu.set_moment(ora.m())
     for r in range(R):
         gpu.set_residual(r, ora.e(r))
     gpu.set_mask_next(ora.mask())
@@ -83,8 +87,9 @@ def compare_step(gpu, ora, th_gpu, th_ora, R, tag, exact=True):
             assert np.array_equal(gpu.residual(r).view(np.uint32), ora.e(r).view(np.uint32)), f"{tag} e[{r}] not bit-exact"
 
 
-def run_reload_parity(B, w, steps, seed=0, hyp=HYP, setup=None):
-    """Per-step parity 'when both start from identical state each step'."""
+def run_reload_parity(B, w, steps, seed=0, hyp=HYP, setup=None, reload_moment=True, kernels=None):
+    """Per-step parity 'when both start from identical state each step'.
+    kernels: optional {step number: expected scape_last_kernel}."""
     N, R = w.numel, w.R
     gs = synth.GradStream(w, device="cuda", seed=seed)
     th0 = gs.theta0()
@@ -97,12 +102,14 @@ def run_reload_parity(B, w, steps, seed=0, hyp=HYP, setup=None):
     th_ora = th0.cpu().numpy().copy()
     for t in range(1, steps + 1):
         grads = gs.next()
-        load_state(gpu, ora, R)
+        load_state(gpu, ora, R, moment=reload_moment)
         th_gpu = torch.from_numpy(th_ora.copy()).cuda()
         gpu.step(th_gpu, grads)
         ora.step(th_ora, [to_np32(g) for g in grads])
         torch.cuda.synchronize()
         compare_step(gpu, ora, th_gpu, th_ora, R, f"{w.name} step {t}")
+        if kernels and t in kernels:
+            assert gpu.last_kernel == kernels[t], (t, gpu.last_kernel)
     gpu.close()
 
 
@@ -169,9 +176,54 @@ def test_ragged_sizes_replica_counts_and_dtypes(B, N, R, s, gdt):
 
 @pytest.mark.parametrize("name,div", [("gpt345m", 256), ("llama500m", 256), ("llama1p8b", 512)])
 def test_scaled_model_shaped_shards(B, name, div):
-    """Configs 2-4 with every tensor `div` times smaller (same structure, scales, distributions)."""
+    """Configs 2-4 with every tensor `div` times smaller (same structure, scales, distributions).
+    Loading a dense m makes every sparse step take the register-staged kernel with dense m in."""
     w = synth.workload(name, div=div)
-    run_reload_parity(B, w, steps=3, seed=1)
+    run_reload_parity(B, w, steps=3, seed=1, kernels={2: "scape_fused_step_kernel", 3: "scape_fused_step_kernel"})
+
+
+@pytest.mark.parametrize("name,div,sparsity", [("gpt345m", 256, None), ("llama500m", 256, 0.9), ("llama500m", 256, None),
+                                               ("llama1p8b", 512, None)])
+def test_scaled_model_shaped_shards_reload_keeps_m_sparse(B, name, div, sparsity):
+    """The same per-step reload (e^r, mask, theta, t from the oracle) but m stays as the handle keeps it
+    in steady state -- the previous step's packed mean -- so from step 3 on the step under test is the
+    steady-state instantiation bench.py times (m gathered through the previous mask)."""
+    w = synth.workload(name, div=div, sparsity=sparsity)
+    steady = STEADY_KERNEL[name]
+    run_reload_parity(B, w, steps=5, seed=2, reload_moment=False,
+                      kernels={1: "scape_fused_step_kernel", 2: "scape_fused_step_kernel", 3: steady, 4: steady, 5: steady})
+
+
+# streaming kernel each model-shaped workload takes in steady state (what bench.py times)
+STEADY_KERNEL = {"gpt345m": "scape_fused_tma_kernel", "llama500m": "scape_fused_step_kernel", "llama1p8b": "scape_fused_tma_kernel"}
+
+
+@pytest.mark.parametrize("name,div,sparsity", [("llama1p8b", 512, None), ("gpt345m", 128, None), ("llama500m", 128, 0.9),
+                                               ("llama500m", 128, None)])
+def test_headline_instantiations_chained_element_by_element(B, name, div, sparsity):
+    """The exact instantiations bench.py times (llama1p8b: staged kernel <bf16, R = 4>, flat select;
+    gpt345m: <f32, 4>; llama500m: <f32, 8> at 90 % and 99 %), chained for 8 steps WITHOUT reloading any
+    state, every output of every step compared with the oracle element by element: masks, index lists,
+    theta, m, e^r, b^r, b-bar.  N = 2.8-3.9 M: thousands of tiles per CTA ring and a ragged tail."""
+    w = synth.workload(name, div=div, sparsity=sparsity)
+    w.tensors.append(("ragged_tail", 1024 * 3 + 128 * 2 + 77))       # chunks past the last full tile, the last one ragged
+    N, R = w.numel, w.R
+    gs = synth.GradStream(w, device="cuda", seed=11)
+    th_gpu = gs.theta0()
+    th_ora = th_gpu.cpu().numpy().copy()
+    gpu = B.Scape(N, R, w.sparsity, **w.hyper)
+    gpu.keep_dense_pack(True)
+    ora = ScapeOracle(N, R, w.sparsity, **w.hyper)
+    for t in range(1, 9):
+        grads = gs.next()
+        gpu.step(th_gpu, grads)
+        ora.step(th_ora, [to_np32(g) for g in grads])
+        compare_step(gpu, ora, th_gpu, th_ora, R, f"{w.name} chained step {t}")
+        if t >= 3:
+            assert gpu.last_kernel == STEADY_KERNEL[name], (t, gpu.last_kernel)
+    fast, general = gpu.select_stats()
+    assert fast + general == 8 and fast >= 3, (fast, general)
+    gpu.close()
 
 
 def test_crafted_ties_and_zeros(B):
@@ -298,6 +350,61 @@ def test_cuda_graph_capture_of_a_step(B):
     torch.cuda.synchronize()
     assert torch.equal(th, th2)
     np.testing.assert_array_equal(ref.mask_next(), cap.mask_next())
+    ref.close()
+    cap.close()
+
+
+def test_cuda_graph_replays_a_whole_rotation_period(B):
+    """include/scape.h: the handle rotates three mask slots and two packed-mean buffers and bakes their
+    addresses into the launches, so a graph must hold a multiple of SCAPE_GRAPH_PERIOD = 6 steady-state
+    steps.  Capture 6 steps once, replay the graph three times on fresh gradients (18 steps) and compare
+    with 18 eager steps of a second handle and with the oracle."""
+    w = synth.Workload("graph6", [("a", 200_000), ("b", 131_072 + 333)], R=3, sparsity=0.99, dist="t4", rho=0.9,
+                       grad_dtype="f32", steps=24)
+    N, R = w.numel, w.R
+    gs = synth.GradStream(w, device="cuda", seed=8)
+    th_ref = gs.theta0()
+    th_cap = th_ref.clone()
+    th_ora = th_ref.cpu().numpy().copy()
+    ref, cap = B.Scape(N, R, w.sparsity, **HYP), B.Scape(N, R, w.sparsity, **HYP)
+    ora = ScapeOracle(N, R, w.sparsity, **HYP)
+    static = [[torch.empty(N, device="cuda") for _ in range(R)] for _ in range(6)]     # the graph's gradient buffers
+
+    def feed(i):
+        grads = gs.next()
+        for dst, src in zip(static[i], grads):
+            dst.copy_(src)
+        return grads
+
+    for i in range(4):                                   # dense step, dense-m step, two steady-state steps: eagerly
+        grads = feed(i)
+        ref.step(th_ref, grads)
+        cap.step(th_cap, static[i])
+        ora.step(th_ora, [to_np32(g) for g in grads])
+    assert cap.last_kernel == "scape_fused_tma_kernel"
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(graph, stream=s):
+            for i in range(6):
+                cap.step(th_cap, static[i])
+    torch.cuda.current_stream().wait_stream(s)
+    for rep in range(3):
+        for i in range(6):
+            grads = feed(i)
+            ref.step(th_ref, grads)
+            ora.step(th_ora, [to_np32(g) for g in grads])
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(th_ref, th_cap), f"replay {rep + 1}: theta of the replayed graph differs from eager steps"
+        np.testing.assert_array_equal(cap.mask_next(), ora.mask(), err_msg=f"replay {rep + 1} mask")
+        np.testing.assert_array_equal(cap.idx_next(), np.nonzero(ora.mask())[0].astype(np.int32))
+        assert np.array_equal(th_cap.cpu().numpy().view(np.uint32), th_ora.view(np.uint32)), f"replay {rep + 1}: theta vs oracle"
+        assert np.array_equal(cap.moment().view(np.uint32), ora.m().view(np.uint32)), f"replay {rep + 1}: m vs oracle"
+        for r in range(R):
+            assert np.array_equal(cap.residual(r).view(np.uint32), ora.e(r).view(np.uint32)), f"replay {rep + 1}: e[{r}]"
     ref.close()
     cap.close()
 

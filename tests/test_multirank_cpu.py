@@ -47,6 +47,23 @@ def test_two_gloo_ranks_aggregate():
         assert "ok" in o
 
 
+def test_bench_gpus_2_launches_two_ranks_itself():
+    """`python bench.py --gpus 2` with no launcher around it (WORLD_SIZE unset) must start two ranks:
+    the line it prints says n_gpus = 2 and carries the max over the two ranks' (fake) region times.
+    --plumbing-only keeps the CUDA step out so that this runs on a CPU box with the gloo backend."""
+    import json
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "4", "--plumbing-only"],
+                         env=env, cwd=ROOT, capture_output=True, text=True, timeout=300)
+    assert res.returncode == 0, res.stdout + res.stderr
+    lines = [l for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, res.stdout                       # rank 0 alone prints
+    line = json.loads(lines[0])
+    assert line["n_gpus"] == 2 and line["steps"] == 4
+    assert line["plumbing_only"]["max_over_ranks_ms"] == 15.0          # rank 1's 15 ms, not rank 0's 10 ms
+    assert abs(line["plumbing_only"]["aggregate_of_fake_region"] - 2 * 1000 * 4 / 0.015) < 1e-6
+
+
 def test_single_rank_helpers():
     import torch
     sys.path.insert(0, ROOT)

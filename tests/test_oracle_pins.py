@@ -637,3 +637,118 @@ def test_p16_mask_pack_unpack():
         np.testing.assert_array_equal(w, lib)
         np.testing.assert_array_equal(mask_unpack(w, n), (m != 0).astype(np.uint8))
         assert w.size == (n + 31) // 32
+
+
+# ------------------------------------------------------------------------------------ P17-P20
+# Algorithm 2, parameter side (PAPER.md:222-242; Eq. 6 :207-211; "Use FP32 w", :231-232)
+def test_p17_bf16_round_to_nearest_even_vs_torch_and_crafted_ties():
+    """The oracle's float -> bfloat16 (written out from the definition) against (i) the torch CPU
+    conversion, a library routine, on random values of every magnitude, denormals, +-0, +-inf, and
+    (ii) hand-checked ties: exactly half goes to the even neighbour, anything above half goes up."""
+    import torch
+    from oracle.scape_oracle import bf16_rne, bf16_widen
+    rng = np.random.default_rng(17)
+    bits = rng.integers(0, 2**32, 400_000, dtype=np.uint64).astype(np.uint32)
+    x = bits.view(np.float32)
+    x = x[np.isfinite(x)]
+    x = np.concatenate([x, np.array([0.0, -0.0, np.inf, -np.inf, 1e-45, -1e-45, 1e-40, 3.3895314e38, -3.4e38], np.float32),
+                        (1e-3 * rng.standard_normal(100_000)).astype(np.float32)])
+    got = bf16_rne(x)
+    want = torch.from_numpy(x.copy()).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+    np.testing.assert_array_equal(got, want)
+    # (ii) by hand: bf16 keeps 8 significant bits
+    cases = {1.0: 1.0, 1.0 + 2.0**-8: 1.0, 1.0 + 2.0**-8 + 2.0**-23: 1.0 + 2.0**-7, 1.0 + 2.0**-7 + 2.0**-8: 1.0 + 2.0**-6,
+             1.0 + 2.0**-7: 1.0 + 2.0**-7, -(1.0 + 2.0**-8 + 2.0**-16): -(1.0 + 2.0**-7), 2.0 - 2.0**-9: 2.0,
+             2.0 - 2.0**-8: 2.0, 2.0 - 2.0**-8 - 2.0**-20: 2.0 - 2.0**-7}
+    xs = np.array(list(cases), np.float32)
+    np.testing.assert_array_equal(bf16_widen(bf16_rne(xs)), np.array(list(cases.values()), np.float32))
+    # widening is exact and rounding a bf16 value is the identity
+    b = rng.integers(0, 2**16, 5000).astype(np.uint16)
+    b = b[np.isfinite(bf16_widen(b))]
+    np.testing.assert_array_equal(bf16_rne(bf16_widen(b)), b)
+
+
+def test_p19_alg2_parameter_hand_example():
+    """tests/golden/p19_alg2_param_example.json: 8 parameters, dyadic values, worked by hand."""
+    from oracle.scape_oracle import bf16_rne, bf16_widen, param_apply, param_pack
+    with open(os.path.join(HERE, "golden", "p19_alg2_param_example.json")) as f:
+        G = json.load(f)
+    mask = np.array(G["mask"], np.uint8)
+    th = np.array(G["theta_owner"], np.float32)
+    pf = param_pack(th, mask, "f32")
+    pb = param_pack(th, mask, "bf16")
+    np.testing.assert_array_equal(pf, np.array(G["pack_f32"], np.float32))          # ascending index order
+    np.testing.assert_array_equal(bf16_widen(pb), np.array(G["pack_bf16_as_f32"], np.float32))
+    for payload, tag in ((pf, "f32"), (pb, "bf16")):
+        for form in (0, 1):                              # l.17 with u = 0 and Eq. 6 literally: identical here (all exact)
+            w = np.array(G["w_before"], np.float32)
+            w_hat = np.zeros(G["N"], np.uint16)
+            param_apply(w, mask, payload, G["lr"], G["wd"], w_hat=w_hat, form=form)
+            np.testing.assert_array_equal(w, np.array(G[f"w_after_{tag}_payload"], np.float32))
+            np.testing.assert_array_equal(bf16_widen(w_hat), np.array(G[f"w_hat_after_{tag}_payload_as_f32"], np.float32))
+
+
+def test_p20_eq6_literal_vs_l17_with_u_zero_within_one_ulp():
+    """Eq. 6: theta[not M] = (1 - eta lambda) theta.  The graded form is Alg. 1 l.17
+    with u = 0, fma(-eta, lambda*theta, theta) (readings S13, S21); the two differ by at most 1 ulp, and
+    both agree with the exact product to 1 ulp."""
+    from oracle.scape_oracle import param_apply
+    rng = np.random.default_rng(20)
+    N = 200_000
+    w0 = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    w0[:7] = [0.0, -0.0, 1e-40, -1e-38, 3e38, 1.0, -1.0]
+    mask = np.zeros(N, np.uint8)
+    for lr, wd in ((1e-3, 0.1), (3e-4, 0.1), (1.5e-4, 0.01), (0.5, 0.25)):
+        a, b = w0.copy(), w0.copy()
+        param_apply(a, mask, np.zeros(0, np.float32), lr, wd, form=0)
+        param_apply(b, mask, np.zeros(0, np.float32), lr, wd, form=1)
+        exact = (1.0 - np.float64(np.float32(lr)) * np.float64(np.float32(wd))) * w0.astype(np.float64)
+        assert np.all(np.abs(a.astype(np.float64) - b.astype(np.float64)) <= ulp32(exact))
+        assert np.all(np.abs(a.astype(np.float64) - exact) <= ulp32(exact))
+        assert np.all(np.abs(b.astype(np.float64) - exact) <= ulp32(exact))
+        assert np.array_equal(np.signbit(a), np.signbit(w0))
+
+
+@pytest.mark.parametrize("R,sparsity", [(2, 0.9), (1, 0.99), (3, 0.0)])
+def test_p18_alg2_copy_tracks_the_owner_bitwise(R, sparsity):
+    """Algorithm 2 l.2-4 with Algorithm 1 as the owner's update.  The owner steps theta with the SCAPE
+    step; a non-owner keeps the FP32 copy w and the bf16 compute copy w^ and, after every step, gets the
+    owner's theta on the mask THAT STEP USED (M_{t-1}: Eq. 6, reading S22) and decays the rest locally.
+      fp32 payload: w == theta bit for bit after every step, w^ == bf16(theta) everywhere;
+      bf16 payload: w^ == bf16(theta) on the mask, w == widen(bf16(theta)) there;
+      wrong mask (the refreshed M_t instead of M_{t-1}): the copy drifts at once -- the pin has teeth."""
+    from oracle.scape_oracle import bf16_rne, bf16_widen, param_apply, param_pack
+    rng = np.random.default_rng(18 + R)
+    N, T = 3001, 6
+    grads = make_grads(rng, N, R, T)
+    ora = ScapeOracle(N, R, sparsity, **HYP)
+    theta = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    w = theta.copy()                       # the non-owner starts from the same parameters
+    w_bf = theta.copy()                    # a second copy fed with bf16 payloads
+    w_wrong = theta.copy()
+    drifted = False
+    for t in range(T):
+        used = ora.mask().copy()           # M_{t-1}: the mask the coming step uses
+        ora.step(theta, grads[t])
+        refreshed = ora.mask()             # M_t
+        # fp32 payload
+        w_hat = np.zeros(N, np.uint16)
+        param_apply(w, used, param_pack(theta, used, "f32"), HYP["lr"], HYP["wd"], w_hat=w_hat)
+        assert np.array_equal(w.view(np.uint32), theta.view(np.uint32)), f"step {t + 1}: the FP32 copy left the owner's theta"
+        np.testing.assert_array_equal(w_hat, bf16_rne(theta))
+        # bf16 payload
+        w_hat_b = np.zeros(N, np.uint16)
+        pb = param_pack(theta, used, "bf16")
+        np.testing.assert_array_equal(pb, bf16_rne(theta[used.astype(bool)]))
+        param_apply(w_bf, used, pb, HYP["lr"], HYP["wd"], w_hat=w_hat_b)
+        on = used.astype(bool)
+        np.testing.assert_array_equal(w_hat_b[on], bf16_rne(theta[on]))
+        np.testing.assert_array_equal(w_bf[on], bf16_widen(bf16_rne(theta[on])))
+        # the wrong mask
+        if sparsity > 0 and t >= 1:
+            param_apply(w_wrong, refreshed, param_pack(theta, refreshed, "f32"), HYP["lr"], HYP["wd"])
+            drifted = drifted or not np.array_equal(w_wrong, theta)
+        else:
+            w_wrong[:] = theta
+    if sparsity > 0:
+        assert drifted, "exchanging on M_t instead of M_{t-1} went unnoticed"
