@@ -199,6 +199,39 @@ int scape_step_local(scape_t* h, float* param, const void* const* grads, void* c
 int scape_exchange_buffers(scape_t* h, float** sums, int64_t* n_sums, uint32_t** mask_words, int64_t* n_mask_words);
 int scape_step_apply(scape_t* h, float* param, void* cuda_stream);
 
+/* Algorithm 2, parameter side (Eq. 6 :207-211).  With
+ * Megatron-LM's distributed optimizer only the OWNER of a partition holds its updated parameters
+ * w'; before the next forward pass the others need them.  Eq. 6: after the update of step t,
+ * theta differs from (1 - eta lambda) theta only on M_{t-1}, the mask that update used -- so only
+ * those k values travel (Alg. 2 l.2-3) and every worker decays the rest itself from its full FP32
+ * copy (l.4, "Use FP32 w to compute untransmitted params", :231-232).  Both calls work on the mask
+ * the handle's LAST completed step used (SCAPE_MASK_LAST / SCAPE_IDX_LAST; all N entries after the
+ * first step, whose mask is all ones), enqueue one kernel on cuda_stream and return without
+ * synchronising.  The all-gather between them is the caller's.  DESIGN.md readings S21-S23.
+ *   scape_param_pack    l.2  w~ <- w'[M_{t-1}]: out[j] = param[idx_last[first + j]], 0 <= j < count,
+ *                       ascending index order (the order of the sparse buffer), as fp32
+ *                       (SCAPE_PARAM_F32) or rounded to nearest even to bf16 (SCAPE_PARAM_BF16).
+ *                       param: DEVICE, N fp32 (the array scape_step updates); out: DEVICE, count
+ *                       elements, caller-owned.  [first, first + count) must lie inside
+ *                       [0, scape_count(h, SCAPE_MASK_LAST)): a worker that owns a range of the
+ *                       sparse buffer packs just that range.
+ *   scape_param_apply   l.3-4 on a copy of the shard that did NOT take the update: w (DEVICE, N
+ *                       fp32, 16-byte aligned, the full FP32 copy, updated IN PLACE) gets
+ *                       w[i] = payload[j] on the mask (payload: DEVICE, scape_count(MASK_LAST)
+ *                       elements of `dtype` in index order, i.e. the gathered w~) and
+ *                       w[i] = fma(-eta, lambda w[i], w[i]) off it -- Alg. 1 l.17 with u = 0, the
+ *                       arithmetic the owner itself applies there, so that with an fp32 payload w
+ *                       equals the owner's parameters bit for bit ((1 - eta lambda) w of Eq. 6
+ *                       differs from it by at most 1 ulp); eta is the learning rate the last step
+ *                       applied.  w_hat (DEVICE, N bf16, 8-byte aligned, or NULL): the compute
+ *                       copy, w_hat[i] = bf16(w[i]) (round to nearest even) for every i.
+ * SCAPE_EINVAL before the first step, during a split step, for a bad range, dtype or alignment.   */
+#define SCAPE_PARAM_F32   0
+#define SCAPE_PARAM_BF16  1
+int scape_param_pack(scape_t* h, const float* param, int64_t first, int64_t count, void* out, int dtype,
+                     void* cuda_stream);
+int scape_param_apply(scape_t* h, float* w, void* w_hat, const void* payload, int dtype, void* cuda_stream);
+
 /* Mask bit pack / unpack, stand-alone (no handle).  PAPER.md:250-252: "we convert the masks from INT8
  * to 1-bit values and pack 8 mask values into one byte" (the paper's Triton kernels, K1 of SURVEY.md
  * §2).  The packed form is the one SCAPE_MASK_NEXT / SCAPE_MASK_LAST and scape_exchange_buffers use:

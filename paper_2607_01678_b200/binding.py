@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libscape.so")
 
 SCAPE_OK, SCAPE_EINVAL, SCAPE_ECUDA, SCAPE_ENOMEM = 0, -1, -2, -3
 SCAPE_GRAD_F32, SCAPE_GRAD_BF16 = 0, 1
+SCAPE_PARAM_F32, SCAPE_PARAM_BF16 = 0, 1
 (SCAPE_MOMENT, SCAPE_RESIDUAL, SCAPE_MASK_NEXT, SCAPE_MASK_LAST, SCAPE_IDX_NEXT, SCAPE_IDX_LAST,
  SCAPE_PACKED, SCAPE_PACKED_MEAN) = range(8)
 
@@ -45,6 +46,8 @@ SYMBOLS = {
     "scape_step_local": (_I, [_VP, _VP, _VP, _VP]),
     "scape_exchange_buffers": (_I, [_VP, _VP, _VP, _VP, _VP]),
     "scape_step_apply": (_I, [_VP, _VP, _VP]),
+    "scape_param_pack": (_I, [_VP, _VP, _I64, _I64, _VP, _I, _VP]),
+    "scape_param_apply": (_I, [_VP, _VP, _VP, _VP, _I, _VP]),
     "scape_mask_pack": (_I, [_VP, _I64, _VP, _VP]),
     "scape_mask_unpack": (_I, [_VP, _I64, _VP, _VP]),
     "scape_get": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
@@ -207,6 +210,14 @@ def scape_step_apply(h, param_ptr, stream=0):
     _check(lib().scape_step_apply(h, param_ptr, stream), "scape_step_apply")
 
 
+def scape_param_pack(h, param_ptr, first, count, out_ptr, dtype, stream=0):
+    _check(lib().scape_param_pack(h, param_ptr, int(first), int(count), out_ptr, int(dtype), stream), "scape_param_pack")
+
+
+def scape_param_apply(h, w_ptr, w_hat_ptr, payload_ptr, dtype, stream=0):
+    _check(lib().scape_param_apply(h, w_ptr, w_hat_ptr, payload_ptr, int(dtype), stream), "scape_param_apply")
+
+
 def scape_mask_pack(mask_bytes_ptr, n, words_ptr, stream=0):
     _check(lib().scape_mask_pack(mask_bytes_ptr, int(n), words_ptr, stream), "scape_mask_pack")
 
@@ -298,7 +309,10 @@ class Scape:
 
     def close(self):
         if getattr(self, "h", None):
-            scape_destroy(self.h)
+            try:
+                scape_destroy(self.h)
+            except TypeError:       # interpreter shutdown: the module globals are already gone
+                pass
             self.h = None
 
     __del__ = close
@@ -376,6 +390,33 @@ class Scape:
         if words is not None:
             dist.all_reduce(words, op=dist.ReduceOp.SUM, group=group)      # disjoint portions: SUM == OR
         self.step_apply(param)
+
+    # ---- Algorithm 2, parameter side (include/scape.h) -----------------------------------
+    def param_pack(self, param, dtype=None, first=0, count=None, out=None):
+        """Alg. 2 l.2: the updated parameters on the mask the last step used, packed in index order.
+        dtype: torch.float32 (default) or torch.bfloat16.  Returns the torch tensor written."""
+        import torch
+        dtype = dtype or torch.float32
+        assert param.is_cuda and param.dtype == torch.float32 and param.is_contiguous() and param.numel() == self.N
+        if count is None:
+            count = self.count_last() - first
+        if out is None:
+            out = torch.empty(count, dtype=dtype, device=param.device)
+        assert out.is_cuda and out.is_contiguous() and out.dtype == dtype and out.numel() >= count
+        scape_param_pack(self.h, param.data_ptr(), first, count, out.data_ptr(),
+                         SCAPE_PARAM_BF16 if dtype == torch.bfloat16 else SCAPE_PARAM_F32, self._stream())
+        return out
+
+    def param_apply(self, w, payload, w_hat=None):
+        """Alg. 2 l.3-4 on a copy that did not take the update: w (fp32 [N]) in place, w_hat (bf16 [N]) optional."""
+        import torch
+        assert w.is_cuda and w.dtype == torch.float32 and w.is_contiguous() and w.numel() == self.N
+        assert payload.is_cuda and payload.is_contiguous() and payload.dtype in (torch.float32, torch.bfloat16)
+        assert payload.numel() == self.count_last()
+        if w_hat is not None:
+            assert w_hat.is_cuda and w_hat.dtype == torch.bfloat16 and w_hat.is_contiguous() and w_hat.numel() == self.N
+        scape_param_apply(self.h, w.data_ptr(), None if w_hat is None else w_hat.data_ptr(), payload.data_ptr(),
+                          SCAPE_PARAM_BF16 if payload.dtype == torch.bfloat16 else SCAPE_PARAM_F32, self._stream())
 
     def step_host(self, param, grads):
         """param / grads: CPU tensors (pinned for async DMA). Synchronises before returning."""

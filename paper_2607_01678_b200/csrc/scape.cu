@@ -86,6 +86,7 @@ struct scape {
   int R = 0, dev = 0, n_sm = 148, grad_dtype = SCAPE_GRAD_F32;
   int64_t t = 0, launches = 0;
   float b1, b2, eps, lr, wd, c1, c2;
+  float lr_last = 0.0f;        // learning rate the last completed step applied (scape_param_apply decays with it)
 
   float* m = nullptr;          // [Npad]
   float* e = nullptr;          // [R][Npad]
@@ -151,7 +152,7 @@ struct scape {
   bool pending = false;           // step_local has run, step_apply has not
   bool pending_need_select = false;
   int pending_pm_out = 0;
-  float pending_bc1 = 1.0f, pending_bc2 = 1.0f;
+  float pending_bc1 = 1.0f, pending_bc2 = 1.0f, pending_lr = 0.0f;
 
   // optional per-step CUDA-event timing of the fused kernel and of the select stage
   bool prof_on = false;
@@ -839,13 +840,14 @@ int step_impl(scape_t* h, float* param, const void* const* grads, void* cuda_str
   }
   if (prof) { CU_TRY(cudaEventRecord(h->prof_ev[pi][2], st)); h->prof_pending = pi + 1; }
   if (local) {
-    h->pending = true; h->pending_pm_out = pm_out; h->pending_bc1 = p.bc1; h->pending_bc2 = p.bc2;
+    h->pending = true; h->pending_pm_out = pm_out; h->pending_bc1 = p.bc1; h->pending_bc2 = p.bc2; h->pending_lr = h->lr;
     h->pending_need_select = need_select;
     return SCAPE_OK;
   }
   h->last_dense = cur.all_ones;
   if (!cur.all_ones) { h->m_sparse = true; h->pm_last = pm_out; }   // m_t = b-_t, addressed through `cur`
   { const int old_last = h->last; h->last = h->use; h->use = h->build; h->build = old_last; }
+  h->lr_last = h->lr;
   h->t += 1;
   return SCAPE_OK;
 }
@@ -929,7 +931,7 @@ extern "C" int scape_step_apply(scape_t* h, float* param, void* cuda_stream) {
   int g2 = (int)((K + 255) / 256); if (g2 > h->n_sm * 16) g2 = h->n_sm * 16; if (g2 < 1) g2 = 1;
   dist_update_kernel<<<g2, 256, 0, st>>>(param, cur.all_ones ? nullptr : cur.idx, cur.all_ones ? h->m : h->pm[pm_out],
                                          h->ghat, h->vm, K, (float)Rt, 1.0f / (float)Rt, (Rt & (Rt - 1)) == 0 ? 1 : 0,
-                                         h->b1, h->c1, h->b2, h->c2, h->eps, h->wd, -h->lr, h->pending_bc1, h->pending_bc2);
+                                         h->b1, h->c1, h->b2, h->c2, h->eps, h->wd, -h->pending_lr, h->pending_bc1, h->pending_bc2);
   h->launches++;
   CU_TRY(cudaGetLastError());
   if (h->pending_need_select) {
@@ -943,7 +945,62 @@ extern "C" int scape_step_apply(scape_t* h, float* param, void* cuda_stream) {
   h->last_dense = cur.all_ones;
   if (!cur.all_ones) { h->m_sparse = true; h->pm_last = pm_out; }
   { const int old_last = h->last; h->last = h->use; h->use = h->build; h->build = old_last; }
+  h->lr_last = h->pending_lr;
   h->t += 1;
+  return SCAPE_OK;
+}
+
+// ---- Algorithm 2, parameter side (Eq. 6 :207-211)  --  SURVEY.md §8(f) rank 4
+extern "C" int scape_param_pack(scape_t* h, const float* param, int64_t first, int64_t count, void* out, int dtype,
+                                void* cuda_stream) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (h->pending) return fail(SCAPE_EINVAL, "a split step is in flight: scape_step_apply first");
+  if (dtype != SCAPE_PARAM_F32 && dtype != SCAPE_PARAM_BF16) return fail(SCAPE_EINVAL, "unknown payload dtype %d", dtype);
+  const MaskSlot& la = h->slot[h->last];
+  if (h->t == 0 || !la.valid) return fail(SCAPE_EINVAL, "no step has run yet: there is no updated parameter to send");
+  if (first < 0 || count < 0 || first + count > la.count)
+    return fail(SCAPE_EINVAL, "range [%lld, %lld) outside the %lld entries of the mask the last step used", (long long)first,
+                (long long)(first + count), (long long)la.count);
+  if (count == 0) return SCAPE_OK;
+  if (!param || !out) return fail(SCAPE_EINVAL, "NULL param/out");
+  if ((uintptr_t)out & (dtype == SCAPE_PARAM_BF16 ? 1 : 3)) return fail(SCAPE_EINVAL, "out is misaligned for its element type");
+  DeviceGuard guard(h->dev);
+  if (!guard.ok) return fail(SCAPE_ECUDA, "cannot select the handle's device");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int64_t grid = (count + 1023) / 1024; if (grid > h->n_sm * 16) grid = h->n_sm * 16;
+  const int32_t* idx = la.all_ones ? nullptr : la.idx;
+  if (dtype == SCAPE_PARAM_BF16) param_pack_kernel<true><<<(int)grid, 256, 0, st>>>(param, idx, first, count, out);
+  else param_pack_kernel<false><<<(int)grid, 256, 0, st>>>(param, idx, first, count, out);
+  h->launches++;
+  CU_TRY(cudaGetLastError());
+  return SCAPE_OK;
+}
+
+extern "C" int scape_param_apply(scape_t* h, float* w, void* w_hat, const void* payload, int dtype, void* cuda_stream) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (h->pending) return fail(SCAPE_EINVAL, "a split step is in flight: scape_step_apply first");
+  if (dtype != SCAPE_PARAM_F32 && dtype != SCAPE_PARAM_BF16) return fail(SCAPE_EINVAL, "unknown payload dtype %d", dtype);
+  MaskSlot& la = h->slot[h->last];
+  if (h->t == 0 || !la.valid) return fail(SCAPE_EINVAL, "no step has run yet");
+  if (!w || (!payload && la.count > 0)) return fail(SCAPE_EINVAL, "NULL w/payload");
+  if ((uintptr_t)w & 15) return fail(SCAPE_EINVAL, "w must be 16-byte aligned");
+  if ((uintptr_t)w_hat & 7) return fail(SCAPE_EINVAL, "w_hat must be 8-byte aligned");
+  if ((uintptr_t)payload & (dtype == SCAPE_PARAM_BF16 ? 1 : 3)) return fail(SCAPE_EINVAL, "payload is misaligned for its element type");
+  DeviceGuard guard(h->dev);
+  if (!guard.ok) return fail(SCAPE_ECUDA, "cannot select the handle's device");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int grid = grid_for(h, (h->n_chunks + kApplyChunks - 1) / kApplyChunks, 8, 4);
+  const bool bf = dtype == SCAPE_PARAM_BF16, hat = w_hat != nullptr, ones = la.all_ones;
+  const float wd = h->wd, neg_lr = -h->lr_last;
+  uint16_t* wh = (uint16_t*)w_hat;
+#define SCAPE_APPLY(B_, H_, O_) param_apply_kernel<B_, H_, O_><<<grid, 256, 0, st>>>(w, wh, la.bits, la.rank, payload, h->N, h->n_chunks, wd, neg_lr)
+  if (ones) { if (bf) { if (hat) SCAPE_APPLY(true, true, true); else SCAPE_APPLY(true, false, true); }
+              else    { if (hat) SCAPE_APPLY(false, true, true); else SCAPE_APPLY(false, false, true); } }
+  else      { if (bf) { if (hat) SCAPE_APPLY(true, true, false); else SCAPE_APPLY(true, false, false); }
+              else    { if (hat) SCAPE_APPLY(false, true, false); else SCAPE_APPLY(false, false, false); } }
+#undef SCAPE_APPLY
+  h->launches++;
+  CU_TRY(cudaGetLastError());
   return SCAPE_OK;
 }
 

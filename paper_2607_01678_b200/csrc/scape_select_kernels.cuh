@@ -996,6 +996,127 @@ __global__ void __launch_bounds__(256) mask_unpack_kernel(const uint32_t* __rest
   }
 }
 
+// ------------------------------------------------------------------------------------------
+// Algorithm 2, parameter side (PAPER.md:222-242; Eq. 6, :207-211).  With a partitioned optimizer
+// only the owner of a partition holds its updated parameters; the others bring their copies up to
+// date from the owner's values on the mask the last update used (l.2-3) and decay the rest locally
+// from their FP32 copy (l.4, "Use FP32 w to compute untransmitted params").
+// ------------------------------------------------------------------------------------------
+// l.2: out[j] = theta[idx[first + j]], j < count (ascending index order = the order of the sparse
+// buffer); idx == nullptr: the mask is all ones and the payload is theta[first .. first + count).
+// Four entries per thread in flight: the gather depends on the index load.
+template <bool BF16>
+__global__ void __launch_bounds__(256) param_pack_kernel(const float* __restrict__ theta, const int32_t* __restrict__ idx,
+                                                        int64_t first, int64_t count, void* __restrict__ out) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t j0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j0 < count; j0 += 4 * stride) {
+    int64_t i[4]; float v[4]; bool ok[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int64_t j = j0 + u * stride;
+      ok[u] = j < count;
+      i[u] = ok[u] ? (idx ? (int64_t)__ldg(idx + first + j) : first + j) : 0;
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) v[u] = ok[u] ? __ldg(theta + i[u]) : 0.0f;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      if (!ok[u]) continue;
+      const int64_t j = j0 + u * stride;
+      if (BF16) reinterpret_cast<__nv_bfloat16*>(out)[j] = __float2bfloat16_rn(v[u]);
+      else reinterpret_cast<float*>(out)[j] = v[u];
+    }
+  }
+}
+
+__device__ __forceinline__ float payload_at(const void* __restrict__ p, bool bf16, int64_t j) {
+  if (bf16) return __uint_as_float(((uint32_t)__ldg(reinterpret_cast<const uint16_t*>(p) + j)) << 16);
+  return __ldg(reinterpret_cast<const float*>(p) + j);
+}
+
+// l.3-4 for one lane's 4 parameters of chunk c: on the mask w <- payload (packed position = rank128[c]
+// + set bits before it), off the mask Alg. 1 l.17 with u = 0 (the owner's own arithmetic there:
+// readings S13, S21); w^ = bf16(w).  mw / r0: the chunk's mask words and rank (all ones: unused).
+template <bool BF16, bool HAT, bool ALLONES, bool GUARD>
+__device__ __forceinline__ void param_apply_lane(float* __restrict__ w, uint16_t* __restrict__ w_hat, const void* __restrict__ payload,
+                                                 int64_t N, int64_t c, int lane, const uint4 mw, const uint32_t r0, float (&v)[4],
+                                                 float wd, float neg_lr) {
+  const int64_t i0 = (c << 7) + ((int64_t)lane << 2);
+  if (ALLONES) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) if (!GUARD || i0 + q < N) v[q] = payload_at(payload, BF16, i0 + q);
+  } else {
+    uint32_t mybits, jbase;
+    lane_bits_from_words(mw, r0, lane, mybits, jbase);
+    int64_t j = jbase;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const bool on = (mybits >> q) & 1u;
+      const float dec = __fmaf_rn(neg_lr, __fmaf_rn(wd, v[q], 0.0f), v[q]);        // l.4 (Eq. 6 as l.17 with u = 0)
+      v[q] = on ? payload_at(payload, BF16, j) : dec;                                // l.3
+      j += on ? 1 : 0;
+    }
+  }
+  store4_f32<GUARD>(w, i0, N, v);
+  if (HAT) {
+    if (!GUARD) {
+      const uint32_t lo = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(v[0])) | ((uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(v[1])) << 16);
+      const uint32_t hi = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(v[2])) | ((uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(v[3])) << 16);
+      __stcs(reinterpret_cast<uint2*>(w_hat + i0), make_uint2(lo, hi));
+    } else {
+#pragma unroll
+      for (int q = 0; q < 4; ++q) if (i0 + q < N) w_hat[i0 + q] = __bfloat16_as_ushort(__float2bfloat16_rn(v[q]));
+    }
+  }
+}
+
+// Streaming pass over the shard: reads w (4 B), writes w (4 B) and w^ (2 B) per parameter, plus the
+// mask words, rank128 and the payload (k values).  HBM-bound; a warp takes kApplyChunks chunks per
+// trip so that as many 128-bit loads per lane are in flight (10 bytes per parameter are too few
+// for one: 2 per trip reached 84 % of the measured copy bandwidth).
+constexpr int kApplyChunks = 4;
+template <bool BF16, bool HAT, bool ALLONES>
+__global__ void __launch_bounds__(256, 4) param_apply_kernel(float* __restrict__ w, uint16_t* __restrict__ w_hat,
+                                                         const uint32_t* __restrict__ bits, const uint32_t* __restrict__ rank,
+                                                         const void* __restrict__ payload, int64_t N, int64_t n_chunks,
+                                                         float wd, float neg_lr) {
+  const int lane = threadIdx.x & 31;
+  const int64_t wpb = blockDim.x >> 5;
+  const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
+  const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  const int64_t full = N >> 7;
+  int64_t c = warp;
+  for (; c + (kApplyChunks - 1) * nwarps < full; c += kApplyChunks * nwarps) {
+    uint4 mw[kApplyChunks];
+    uint32_t r0[kApplyChunks];
+    float v[kApplyChunks][4];
+#pragma unroll
+    for (int u = 0; u < kApplyChunks; ++u) {
+      mw[u] = make_uint4(0, 0, 0, 0); r0[u] = 0;
+      if (!ALLONES) { mw[u] = __ldg(reinterpret_cast<const uint4*>(bits) + (c + u * nwarps)); r0[u] = __ldg(rank + (c + u * nwarps)); }
+    }
+#pragma unroll
+    for (int u = 0; u < kApplyChunks; ++u)
+      if (!ALLONES) load4_f32<false>(w, ((c + u * nwarps) << 7) + ((int64_t)lane << 2), N, v[u]);
+#pragma unroll
+    for (int u = 0; u < kApplyChunks; ++u)
+      param_apply_lane<BF16, HAT, ALLONES, false>(w, w_hat, payload, N, c + u * nwarps, lane, mw[u], r0[u], v[u], wd, neg_lr);
+  }
+  for (; c < n_chunks; c += nwarps) {                        // the last trips, and the ragged last chunk
+    uint4 ma = make_uint4(0, 0, 0, 0);
+    uint32_t ra = 0;
+    if (!ALLONES) { ma = __ldg(reinterpret_cast<const uint4*>(bits) + c); ra = __ldg(rank + c); }
+    float va[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+    if (c < full) {
+      if (!ALLONES) load4_f32<false>(w, (c << 7) + ((int64_t)lane << 2), N, va);
+      param_apply_lane<BF16, HAT, ALLONES, false>(w, w_hat, payload, N, c, lane, ma, ra, va, wd, neg_lr);
+    } else {
+      if (!ALLONES) load4_f32<true>(w, (c << 7) + ((int64_t)lane << 2), N, va);
+      param_apply_lane<BF16, HAT, ALLONES, true>(w, w_hat, payload, N, c, lane, ma, ra, va, wd, neg_lr);
+    }
+  }
+}
+
 // all-ones mask over [0,N), zero padding bits up to n_words*32
 __global__ void mask_all_ones_kernel(uint32_t* bits, int64_t n_words, int64_t N) {
   for (int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; w < n_words; w += (int64_t)gridDim.x * blockDim.x) {
