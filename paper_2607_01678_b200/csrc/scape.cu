@@ -53,7 +53,7 @@ constexpr int kSinglePassCompactBlocks = 512;
 
 struct MaskSlot {
   uint32_t* bits = nullptr;   // [n_words]
-  uint32_t* rank = nullptr;   // [n_chunks]
+  uint2* rank = nullptr;      // [n_chunks] {set bits before the chunk, running popcounts of its words}
   int32_t* idx = nullptr;     // [k]   (not materialised while all_ones)
   int64_t count = 0;
   bool all_ones = false;
@@ -66,7 +66,7 @@ struct FusedCfg {
   int bps = 0;                // resident CTAs per SM the grid is sized for
   int stages = 0;             // staged kernel: ring depth
   uint32_t tile = 0;          // staged kernel: bytes per stage
-  size_t smem = 0;            // staged kernel: dynamic shared memory per CTA
+  size_t smem = 0;            // dynamic shared memory per CTA
 };
 
 struct DeviceGuard {
@@ -205,8 +205,11 @@ int prepare_kernels(scape* h) {
         FusedCfg& c = h->cfg_step[dt][v][clipt];
         c.fn = step_kernel(dt, h->R, v == 0, v == 2, clipt != 0);
         if (!c.fn) return fail(SCAPE_EINVAL, "no streaming kernel for R = %d", h->R);
+        // sparse variants: per-warp scratch of the on-mask arithmetic + candidate ring (dynamic shared memory)
+        c.smem = step_smem_bytes(h->R, v == 0);
+        if (c.smem > 48u * 1024u) CU_TRY(cudaFuncSetAttribute(c.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem));
         int occ = 0;
-        CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c.fn, 256, 0));
+        CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c.fn, 256, c.smem));
         c.bps = occ > 0 ? (occ > 8 ? 8 : occ) : 1;
       }
       // Staged kernel: two CTAs (16 consumer warps) per SM with >= 3 stages each, or not at all
@@ -258,7 +261,7 @@ int launch_fused(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t
   const int grid = grid_for(h, p.n_chunks, 8, c.bps);
   set_segments(h, p, grid * 8);
   void* args[] = {(void*)&p};
-  CU_TRY(cudaLaunchKernel(c.fn, dim3((unsigned)grid), dim3(256), args, 0, st));
+  CU_TRY(cudaLaunchKernel(c.fn, dim3((unsigned)grid), dim3(256), args, c.smem, st));
   h->last_kernel = "scape_fused_step_kernel";
   h->launches++;
   return SCAPE_OK;
@@ -304,7 +307,7 @@ int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general,
   KeySrc src;
   src.e0 = h->e;
   src.cur_bits = cur.all_ones ? nullptr : cur.bits;
-  src.cur_rank = cur.all_ones ? nullptr : cur.rank;
+  src.cur_rk = cur.all_ones ? nullptr : cur.rank;
   src.packed0 = h->packed;
   src.N = h->N;
   src.n_chunks = h->n_chunks;
@@ -403,7 +406,7 @@ int run_select_layered(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_
   KeySrc src;
   src.e0 = h->e;
   src.cur_bits = cur.all_ones ? nullptr : cur.bits;
-  src.cur_rank = cur.all_ones ? nullptr : cur.rank;
+  src.cur_rk = cur.all_ones ? nullptr : cur.rank;
   src.packed0 = h->packed;
   src.N = h->N;
   src.n_chunks = h->n_chunks;
@@ -512,7 +515,7 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   alloc((void**)&h->e, sizeof(float) * h->Npad * R, true);                   // l.2: e_0 = 0
   for (auto& s : h->slot) {
     alloc((void**)&s.bits, sizeof(uint32_t) * h->n_words, true);
-    alloc((void**)&s.rank, sizeof(uint32_t) * h->n_chunks, true);
+    alloc((void**)&s.rank, sizeof(uint2) * h->n_chunks, true);
   }
   alloc((void**)&h->sel, sizeof(SelState), true);
   alloc((void**)&h->seg_count, sizeof(uint32_t) * h->max_seg, true);
@@ -785,12 +788,12 @@ int step_impl(scape_t* h, float* param, const void* const* grads, void* cuda_str
   StepParams p{};
   p.theta = param; p.m = h->m; p.e = h->e; p.e_stride = h->Npad;
   for (int r = 0; r < h->R; ++r) p.g[r] = grads[r];
-  p.cur_bits = cur.bits; p.cur_rank = cur.rank;
+  p.cur_bits = cur.bits; p.cur_rk = cur.rank;
   p.packed = cur.all_ones ? h->dense_pack : h->packed;
   p.packed_stride = cur.all_ones ? h->Npad : h->packed_stride;
   p.packed_mean = h->pm[pm_out];
   if (msparse) {
-    p.prev_bits = h->slot[h->last].bits; p.prev_rank = h->slot[h->last].rank; p.pm_prev = h->pm[h->pm_last];
+    p.prev_bits = h->slot[h->last].bits; p.prev_rk = h->slot[h->last].rank; p.pm_prev = h->pm[h->pm_last];
   }
   p.N = h->N; p.n_chunks = h->n_chunks;
   p.b1 = h->b1; p.c1 = h->c1; p.b2 = h->b2; p.c2 = h->c2; p.eps = h->eps; p.wd = h->wd; p.neg_lr = -h->lr;

@@ -3,10 +3,11 @@
 // Data layout: the shard is cut into CHUNKS of 128 consecutive
 // parameters; one warp handles one chunk per loop trip, lane l owning elements 4l..4l+3
 // (one 128-bit access per fp32 array, one 64-bit access per bf16 array).  A mask is stored as
-// bits (word i/32, bit i%32 => one uint4 per chunk) plus `rank128[c]`, the number of set bits
-// before chunk c, so the packed position of a selected element is rank128[c] + popc(bits
-// before it inside the chunk): the pack of Alg. 1 l.9 needs no atomics and keeps ascending
-// index order.
+// bits (word i/32, bit i%32 => one uint4 per chunk) plus `rk[c]` = {the number of set bits before
+// chunk c ("rank128"), the running popcounts of the chunk's four words, one byte each}, so the
+// packed position of a selected element is rank128 + words before + popc(bits before it inside
+// its word): the pack of Alg. 1 l.9 needs no atomics and keeps ascending index order, and a lane
+// finds its position from ONE word and ONE uint2 (no popcounts over the other words).
 //
 // Every fp32 operation of the method is written with a _rn intrinsic so that nvcc cannot
 // contract or reorder it; the order is the one pinned in DESIGN.md and followed by the oracle.
@@ -90,14 +91,14 @@ struct StepParams {
   int64_t e_stride;
   const void* g[kMaxR];         // R caller-owned gradient buffers
   const uint32_t* cur_bits;     // [Npad/32]   (unused when DENSE)
-  const uint32_t* cur_rank;     // [Npad/128]
+  const uint2* cur_rk;          // [Npad/128] {rank128, word prefixes}: see chunk_prefix_bytes
   float* packed;                // [R][packed_stride] or nullptr (DENSE without keep_dense_pack)
   int64_t packed_stride;
   float* packed_mean;           // [k] b- of this step = m_t in packed form (unused when DENSE)
   // m_{t-1} stored sparsely (MSPARSE): it is zero off the mask the previous step used (Eq. 4,
   // PAPER.md:197), so it lives as that step's packed mean, addressed through that mask
   const uint32_t* prev_bits;    // [Npad/32]
-  const uint32_t* prev_rank;    // [Npad/128]
+  const uint2* prev_rk;         // [Npad/128]
   const float* pm_prev;         // [k]
   int64_t N;
   int64_t n_chunks;             // ceil(N/128)
@@ -134,7 +135,7 @@ struct StepParams {
 // (mask bits, rank128, packed buffers) from L2.
 // ------------------------------------------------------------------------------------------
 template <bool GUARD>
-__device__ __forceinline__ void load4_f32(const float* __restrict__ p, int64_t i0, int64_t N, float (&v)[4]) {
+__device__ __forceinline__ void load4_f32(const float* __restrict__ p, uint32_t i0, int64_t N, float (&v)[4]) {
   if (!GUARD) {
     const float4 t = __ldcs(reinterpret_cast<const float4*>(p + i0));
     v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
@@ -145,7 +146,7 @@ __device__ __forceinline__ void load4_f32(const float* __restrict__ p, int64_t i
 }
 
 template <bool GUARD>
-__device__ __forceinline__ void store4_f32(float* __restrict__ p, int64_t i0, int64_t N, const float (&v)[4]) {
+__device__ __forceinline__ void store4_f32(float* __restrict__ p, uint32_t i0, int64_t N, const float (&v)[4]) {
   if (!GUARD) {
     __stcs(reinterpret_cast<float4*>(p + i0), make_float4(v[0], v[1], v[2], v[3]));
   } else {
@@ -156,7 +157,7 @@ __device__ __forceinline__ void store4_f32(float* __restrict__ p, int64_t i0, in
 
 // Gradient loads: fp32, or bf16 widened exactly (S16) by placing the 16 bits in the high half.
 template <typename G, bool GUARD>
-__device__ __forceinline__ void load4_grad(const void* __restrict__ base, int64_t i0, int64_t N, float (&v)[4]) {
+__device__ __forceinline__ void load4_grad(const void* __restrict__ base, uint32_t i0, int64_t N, float (&v)[4]) {
   if constexpr (sizeof(G) == 4) {
     load4_f32<GUARD>(reinterpret_cast<const float*>(base), i0, N, v);
   } else {
@@ -184,10 +185,31 @@ __device__ __forceinline__ void lane_bits_from_words(const uint4 mw, const uint3
 }
 __device__ __forceinline__ uint32_t chunk_popc(const uint4 mw) { return __popc(mw.x) + __popc(mw.y) + __popc(mw.z) + __popc(mw.w); }
 
-__device__ __forceinline__ void lane_mask_bits(const uint32_t* __restrict__ bits, const uint32_t* __restrict__ rank,
+__device__ __forceinline__ void lane_mask_bits(const uint32_t* __restrict__ bits, const uint2* __restrict__ rk,
                                                int64_t c, int lane, uint32_t& mybits, uint32_t& jbase) {
   const uint4 mw = __ldg(reinterpret_cast<const uint4*>(bits) + c);
-  lane_bits_from_words(mw, __ldg(rank + c), lane, mybits, jbase);
+  lane_bits_from_words(mw, __ldg(rk + c).x, lane, mybits, jbase);
+}
+
+// rk[c].y: running popcounts of the chunk's words, one byte each (byte 3 = the chunk's total, <= 128)
+__host__ __device__ __forceinline__ uint32_t chunk_prefix_bytes(uint32_t p0, uint32_t p1, uint32_t p2, uint32_t p3) {
+  return p0 | ((p0 + p1) << 8) | ((p0 + p1 + p2) << 16) | ((p0 + p1 + p2 + p3) << 24);
+}
+
+// Where a lane's 4 mask bits sit: word ws of the chunk, bits sh..sh+3.  Loop-invariant per lane, so the
+// streaming kernels decode a chunk's mask with one 32-bit load of the lane's OWN word, one uint2 load
+// of rk[c] (same address for the whole warp), a byte pick (PRMT), a shift, two ANDs and one POPC.
+struct LaneMap { uint32_t ws, sh, lowmask, sel; };
+__device__ __forceinline__ LaneMap lane_map(int lane) {
+  LaneMap lm;
+  lm.ws = (uint32_t)lane >> 3; lm.sh = ((uint32_t)lane & 7u) << 2;
+  lm.lowmask = (1u << lm.sh) - 1u;
+  lm.sel = lm.ws == 0 ? 0x4444u : 0x4440u + (lm.ws - 1u);      // __byte_perm selector: byte ws-1 of rk.y, or 0
+  return lm;
+}
+__device__ __forceinline__ void lane_decode(uint32_t w, uint2 rk, const LaneMap& lm, uint32_t& mybits, uint32_t& jbase) {
+  mybits = (w >> lm.sh) & 0xFu;
+  jbase = rk.x + __byte_perm(rk.y, 0u, lm.sel) + __popc(w & lm.lowmask);
 }
 
 // Gather of m_{t-1} for this lane's 4 elements from the previous step's packed mean: selected
@@ -235,82 +257,115 @@ __device__ __forceinline__ void warp_store_sumsq(const StepParams& p, const Stag
 // The arithmetic of one lane's 4 elements (Alg. 1 l.6-10, l.12-17 in the pinned order), the stores
 // of theta / m / e^r / b^r / b-, and the bracket classification of stage 2.  Shared by the two
 // load front-ends (register-staged LDG and shared-memory-staged bulk copies).
-//
-// Sparse steps: the selected entries of a chunk (cnt of 128; ~13 at 90 % sparsity, ~1 at 99 %) are
-// scattered over the lanes, so running l.10-16 (IEEE divisions, square root) where they sit would
-// mean four divergent passes with a few active lanes each.  Instead every lane parks (sum_r m~^r,
-// m_old) of its selected entries in a warp-private scratch at the entry's rank inside the chunk,
-// and lane l then runs l.10-16 for the entry of rank l: one pass, consecutive lanes, b- stored
-// coalesced.  The update u comes back through the same scratch.
-//   r0 = rank128[c]; cnt = set bits of the chunk; scs, scm = 128 floats each, private to this warp
-template <int R, bool DENSE, bool GUARD, bool STORE = true, bool CLIPT = true>
-__device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, int lane, int64_t i0,
-                                              uint32_t mybits, uint32_t jbase, uint32_t r0, uint32_t cnt, float* scs, float* scm,
-                                              float (&th)[4], const float (&mo)[4],
+
+// All-ones mask (step 1, sparsity 0): dense m in and out, nothing is packed, no classification.
+template <int R, bool GUARD, bool CLIPT>
+__device__ __forceinline__ void dense_compute(const StepParams& p, uint32_t i0, float (&th)[4], const float (&mo)[4],
                                               float (&gg)[R][4], float (&ee)[R][4], StageA& sa) {
-  uint32_t key0[4];             // bits(|m~^0|): the selection statistic of l.11
-  if constexpr (DENSE) {
-    float mn[4];
+  float mn[4];
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      const float pq = __fmul_rn(p.b1, mo[q]);                // beta1 * m_{t-1}, reused by l.6 and l.13
-      float mt[R];
+  for (int q = 0; q < 4; ++q) {
+    const float pq = __fmul_rn(p.b1, mo[q]);                // beta1 * m_{t-1}, reused by l.6 and l.13
+    float mt[R];
 #pragma unroll
-      for (int r = 0; r < R; ++r) {
-        mt[r] = __fadd_rn(__fmaf_rn(p.c1, gg[r][q], pq), ee[r][q]);            // l.6
-        ee[r][q] = (r == 0 && p.stash) ? mt[r] : 0.0f;                         // l.8 (M = 1); stash: keys for the select
-      }
-      key0[q] = __float_as_uint(mt[0]) & 0x7FFFFFFFu;
-      if (p.packed != nullptr && (!GUARD || i0 + q < p.N)) {
+    for (int r = 0; r < R; ++r) {
+      mt[r] = __fadd_rn(__fmaf_rn(p.c1, gg[r][q], pq), ee[r][q]);            // l.6
+      ee[r][q] = (r == 0 && p.stash) ? mt[r] : 0.0f;                         // l.8 (M = 1); stash: keys for the select
+    }
+    if (p.packed != nullptr && (!GUARD || i0 + q < p.N)) {
 #pragma unroll
-        for (int r = 0; r < R; ++r) p.packed[r * p.packed_stride + (i0 + q)] = mt[r];   // l.9 (keep_dense_pack)
-      }
-      float s = mt[0];
+      for (int r = 0; r < R; ++r) p.packed[r * p.packed_stride + (i0 + q)] = mt[r];   // l.9 (keep_dense_pack)
+    }
+    float s = mt[0];
 #pragma unroll
-      for (int r = 1; r < R; ++r) s = __fadd_rn(s, mt[r]);                                   // l.10, r ascending
-      const float bb = p.r_pow2 ? __fmul_rn(s, p.inv_R) : __fdiv_rn(s, p.R_f);              // l.10
-      const float gh = __fdiv_rn(__fsub_rn(bb, pq), p.c1);                                    // l.13 (Eq. 3)
-      const float vmq = __fmul_rn(p.b2, __fmul_rn(mo[q], mo[q]));
-      mn[q] = bb;                                                                             // l.12
-      if (CLIPT && p.clip) {
-        // l.14 needs the norm of g^ over the whole mask first: park what l.15-17 need; theta of
-        // this entry is updated by clip_update_kernel
-        if (!GUARD || i0 + q < p.N) {
-          if (p.clip == 2) { p.ghat[i0 + q] = s; p.vm[i0 + q] = mo[q]; }
-          else {
-            p.ghat[i0 + q] = gh; p.vm[i0 + q] = vmq;
-            sa.sumsq += (double)gh * (double)gh;
-          }
+    for (int r = 1; r < R; ++r) s = __fadd_rn(s, mt[r]);                                   // l.10, r ascending
+    const float bb = p.r_pow2 ? __fmul_rn(s, p.inv_R) : __fdiv_rn(s, p.R_f);              // l.10
+    const float gh = __fdiv_rn(__fsub_rn(bb, pq), p.c1);                                    // l.13 (Eq. 3)
+    const float vmq = __fmul_rn(p.b2, __fmul_rn(mo[q], mo[q]));
+    mn[q] = bb;                                                                             // l.12
+    if (CLIPT && p.clip) {
+      // l.14 needs the norm of g^ over the whole mask first: park what l.15-17 need; theta of
+      // this entry is updated by clip_update_kernel
+      if (!GUARD || i0 + q < p.N) {
+        if (p.clip == 2) { p.ghat[i0 + q] = s; p.vm[i0 + q] = mo[q]; }
+        else {
+          p.ghat[i0 + q] = gh; p.vm[i0 + q] = vmq;
+          sa.sumsq += (double)gh * (double)gh;
         }
-      } else {
-        const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), vmq);                              // l.15
-        const float u = __fdiv_rn(__fmul_rn(bb, p.bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, p.bc2)), p.eps));   // l.16 (+ :77)
-        const float w = __fmaf_rn(p.wd, th[q], u);                                            // l.17
-        th[q] = __fmaf_rn(p.neg_lr, w, th[q]);
-      }
-    }
-    if (STORE) {
-      store4_f32<GUARD>(p.theta, i0, p.N, th);
-#pragma unroll
-      for (int r = 0; r < R; ++r) store4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
-    }
-    store4_f32<false>(p.m, i0, p.N, mn);                    // sparse steps keep m_t as b- only
-    return;
-  } else {
-    const bool deferred = CLIPT && p.clip;                  // theta on the mask is left to clip_update_kernel
-    if (cnt == 0) {
-      // no selected entry in this chunk (88 % of the chunks at 99.9 % sparsity): l.6-8 and l.17 only
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const float pq = __fmul_rn(p.b1, mo[q]);
-#pragma unroll
-        for (int r = 0; r < R; ++r) ee[r][q] = __fadd_rn(__fmaf_rn(p.c1, gg[r][q], pq), ee[r][q]);   // l.6-7
-        key0[q] = __float_as_uint(ee[0][q]) & 0x7FFFFFFFu;
-        th[q] = __fmaf_rn(p.neg_lr, __fmaf_rn(p.wd, th[q], 0.0f), th[q]);                            // l.17, u = 0 (Eq. 5)
       }
     } else {
-      const uint32_t lbase = jbase - r0;                    // rank of this lane's first entry inside the chunk
-      uint32_t lj = lbase;                                  // walks this lane's selected entries
+      const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), vmq);                              // l.15
+      const float u = __fdiv_rn(__fmul_rn(bb, p.bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, p.bc2)), p.eps));   // l.16 (+ :77)
+      const float w = __fmaf_rn(p.wd, th[q], u);                                            // l.17
+      th[q] = __fmaf_rn(p.neg_lr, w, th[q]);
+    }
+  }
+  store4_f32<GUARD>(p.theta, i0, p.N, th);
+#pragma unroll
+  for (int r = 0; r < R; ++r) store4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
+  store4_f32<false>(p.m, i0, p.N, mn);                    // sparse steps keep m_t as b- only
+}
+
+// Candidate keys of the register-staged front-end are staged in a per-warp shared-memory ring and
+// leave for the warp's segment in global memory 32 at a time (one 256-byte store per warp): a lane
+// with candidates takes its ring positions with ONE shared-memory atomic (no votes, no prefix over
+// the lanes; the order inside a segment is irrelevant, the composite keys carry the index).
+// The ring holds the < 32 keys not yet flushed plus the <= 128 a chunk can add.
+constexpr uint32_t kRing = 256;
+struct CandRing {
+  unsigned long long* ring;     // [kRing] shared memory, private to the warp
+  uint32_t* head;               // keys appended so far (shared memory); StageA::cursor = keys flushed so far
+};
+
+__device__ __forceinline__ void ring_flush32(const StepParams& p, StageA& sa, const CandRing& cr, int lane) {
+  const uint32_t j = sa.cursor + (uint32_t)lane;
+  const unsigned long long v = cr.ring[j & (kRing - 1u)];
+  if (j < p.seg_cap) sa.seg[j] = v;                         // a full segment drops keys; seg_count still counts them (overflow)
+  sa.cursor += 32u;
+}
+// end of the kernel: the < 32 keys still in the ring; returns the number of keys the warp appended
+__device__ __forceinline__ uint32_t ring_drain(const StepParams& p, StageA& sa, const CandRing& cr, int lane) {
+  __syncwarp();
+  const uint32_t head = *reinterpret_cast<volatile uint32_t*>(cr.head);
+  while (head - sa.cursor >= 32u) ring_flush32(p, sa, cr, lane);
+  const uint32_t j = sa.cursor + (uint32_t)lane;
+  if (j < head && j < p.seg_cap) sa.seg[j] = cr.ring[j & (kRing - 1u)];
+  return head;
+}
+
+// Sparse mask.  The selected entries of a chunk (cnt of 128; ~13 at 90 % sparsity, ~1 at 99 %) are
+// scattered over the lanes, so running l.10-16 (IEEE divisions, square root) where they sit would
+// mean four divergent passes with a few active lanes each, and b^r would leave as scattered 4-byte
+// stores.  Instead every lane parks (m_old, m~^0 .. m~^{R-1}) of its selected entries in a
+// warp-private scratch at the entry's rank inside the chunk, and lane l then handles the entry of
+// rank l: b^r (l.9), b- (l.10, l.12) stored coalesced, l.13-16 in one pass over consecutive lanes.
+// The update u comes back through the same scratch.
+//   r0 = rank128[c]; cnt = set bits of the chunk
+//   scm = 128 floats (m_old), sc = R arrays of 128 floats SCS floats apart (m~^r), private to this warp
+//   RING: candidates go through the shared-memory ring `cr` (register-staged front-end), else straight
+//   to the segment with one ballot per element (bulk-copy front-end: register-bound, shared memory full)
+template <int R, bool GUARD, bool STORE, bool CLIPT, bool RING, int SCS>
+__device__ __forceinline__ void sparse_compute(const StepParams& p, uint32_t c, int lane, const LaneMap& lm, uint32_t i0,
+                                               uint32_t mybits, uint32_t jbase, uint32_t r0, uint32_t cnt, float* scm, float* sc,
+                                               float (&th)[4], const float (&mo)[4],
+                                               float (&gg)[R][4], float (&ee)[R][4], StageA& sa, const CandRing& cr) {
+  uint32_t key0[4];             // bits(|m~^0|): the selection statistic of l.11
+  const bool deferred = CLIPT && p.clip;                  // theta on the mask is left to clip_update_kernel / dist_update_kernel
+  if (cnt == 0) {
+    // no selected entry in this chunk (88 % of the chunks at 99.9 % sparsity): l.6-8 and l.17 only
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const float pq = __fmul_rn(p.b1, mo[q]);
+#pragma unroll
+      for (int r = 0; r < R; ++r) ee[r][q] = __fadd_rn(__fmaf_rn(p.c1, gg[r][q], pq), ee[r][q]);   // l.6-7
+      key0[q] = __float_as_uint(ee[0][q]) & 0x7FFFFFFFu;
+      th[q] = __fmaf_rn(p.neg_lr, __fmaf_rn(p.wd, th[q], 0.0f), th[q]);                            // l.17, u = 0 (Eq. 5)
+    }
+  } else {
+    const uint32_t lbase = jbase - r0;                    // rank of this lane's first entry inside the chunk
+    {
+      float* ps = sc + lbase;                             // walks this lane's selected entries
+      float* pm = scm + lbase;
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         const bool on = (mybits >> q) & 1u;
@@ -323,153 +378,165 @@ __device__ __forceinline__ void fused_compute(const StepParams& p, int64_t c, in
         }
         key0[q] = __float_as_uint(mt[0]) & 0x7FFFFFFFu;
         if (on) {
-          float* pk = p.packed + (r0 + lj);
-          float sm = mt[0];
+          *pm = mo[q];
 #pragma unroll
-          for (int r = 0; r < R; ++r) { *pk = mt[r]; pk += p.packed_stride; }                   // l.9
-#pragma unroll
-          for (int r = 1; r < R; ++r) sm = __fadd_rn(sm, mt[r]);                                // l.10, r ascending
-          scs[lj] = sm; scm[lj] = mo[q];
-          ++lj;
+          for (int r = 0; r < R; ++r) ps[r * SCS] = mt[r];
+          ++ps; ++pm;
         }
       }
-      __syncwarp();
-      for (uint32_t l = lane; l < cnt; l += 32) {           // lane l: the chunk's selected entry of rank l
-        const float sm = scs[l], mq = scm[l];
-        const float pq = __fmul_rn(p.b1, mq);
-        const float bb = p.r_pow2 ? __fmul_rn(sm, p.inv_R) : __fdiv_rn(sm, p.R_f);          // l.10
-        const float gh = __fdiv_rn(__fsub_rn(bb, pq), p.c1);                                  // l.13 (Eq. 3)
-        const float vmq = __fmul_rn(p.b2, __fmul_rn(mq, mq));
-        p.packed_mean[r0 + l] = bb;                                                           // l.12: m_t = b-
-        if (deferred) {
-          if (p.clip == 2) { p.ghat[r0 + l] = sm; p.vm[r0 + l] = mq; }
-          else {
-            p.ghat[r0 + l] = gh; p.vm[r0 + l] = vmq;
-            sa.sumsq += (double)gh * (double)gh;
-          }
-        } else {
-          const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), vmq);                            // l.15
-          scs[l] = __fdiv_rn(__fmul_rn(bb, p.bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, p.bc2)), p.eps));   // l.16 (+ :77)
-        }
+    }
+    __syncwarp();
+    for (uint32_t l = lane; l < cnt; l += 32) {           // lane l: the chunk's selected entry of rank l
+      const float mq = scm[l];
+      float* pk = p.packed + (r0 + l);
+      float sm = sc[l];
+      *pk = sm;                                                                             // l.9, r = 0
+#pragma unroll
+      for (int r = 1; r < R; ++r) {
+        const float v = sc[r * SCS + l];
+        pk += p.packed_stride;
+        *pk = v;                                                                            // l.9
+        sm = __fadd_rn(sm, v);                                                              // l.10, r ascending
       }
-      __syncwarp();
-      lj = lbase;
+      const float pq = __fmul_rn(p.b1, mq);
+      const float bb = p.r_pow2 ? __fmul_rn(sm, p.inv_R) : __fdiv_rn(sm, p.R_f);          // l.10
+      const float gh = __fdiv_rn(__fsub_rn(bb, pq), p.c1);                                  // l.13 (Eq. 3)
+      const float vmq = __fmul_rn(p.b2, __fmul_rn(mq, mq));
+      p.packed_mean[r0 + l] = bb;                                                           // l.12: m_t = b-
+      if (deferred) {
+        if (p.clip == 2) { p.ghat[r0 + l] = sm; p.vm[r0 + l] = mq; }
+        else {
+          p.ghat[r0 + l] = gh; p.vm[r0 + l] = vmq;
+          sa.sumsq += (double)gh * (double)gh;
+        }
+      } else {
+        const float v = __fmaf_rn(p.c2, __fmul_rn(gh, gh), vmq);                            // l.15
+        sc[l] = __fdiv_rn(__fmul_rn(bb, p.bc1), __fadd_rn(__fsqrt_rn(__fmul_rn(v, p.bc2)), p.eps));   // l.16 (+ :77)
+      }
+    }
+    __syncwarp();
+    {
+      const float* pu = sc + lbase;
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         const bool on = (mybits >> q) & 1u;
-        const float u = on ? scs[lj] : 0.0f;                                                   // Eq. 5 off the mask
-        lj += on ? 1u : 0u;
+        const float u = on ? *pu : 0.0f;                                                     // Eq. 5 off the mask
+        pu += on ? 1 : 0;
         if (deferred && on) continue;
-        th[q] = __fmaf_rn(p.neg_lr, __fmaf_rn(p.wd, th[q], u), th[q]);                         // l.17
-      }
-      __syncwarp();                                         // the scratch is reused by the next chunk
-    }
-
-    if (STORE) {                                            // else the caller stores th / ee (staged bulk stores)
-      store4_f32<GUARD>(p.theta, i0, p.N, th);
-#pragma unroll
-      for (int r = 0; r < R; ++r) store4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
-    }
-
-    // Stage 2 (l.11) fused: classify |m~^0| against the predicted bracket.  Exactness does not
-    // depend on the prediction: sel_decide_kernel checks n_above < k <= n_above + n_cand.
-    bool mixed = false;                                     // chunk with entries of several layers (warp-uniform)
-    if (p.chunk_layer != nullptr) {
-      // per-layer refresh: the bracket is the one of this chunk's layer.  Warps walk the shard in
-      // ascending order, so a layer change is rare: flush the count, load the new bracket.
-      const uint32_t cl = __ldg(p.chunk_layer + c);
-      const uint32_t l = cl & 0x7FFFFFFFu;
-      mixed = (cl >> 31) != 0u;
-      if (l != sa.layer) {
-        warp_flush_layer(p, sa, lane);
-        sa.layer = l;
-        sa.lo = p.layers[l].br.lo_key; sa.hi = p.layers[l].br.hi_key;
+        th[q] = __fmaf_rn(p.neg_lr, __fmaf_rn(p.wd, th[q], u), th[q]);                       // l.17
       }
     }
-    uint32_t nib = 0, cnib = 0;
-    if (!mixed) {
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const bool valid = !GUARD || (i0 + q < p.N);
-        const bool above = valid && key0[q] >= sa.hi;
-        nib |= above ? (1u << q) : 0u;
-        cnib |= (valid && !above && key0[q] >= sa.lo) ? (1u << q) : 0u;
-      }
-    } else {
-      // a chunk shared by several layers (at most one per layer boundary): bracket and count per entry
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        if (GUARD && i0 + q >= p.N) continue;
-        uint32_t l = sa.layer;
-        while (i0 + q >= p.layers[l].end) ++l;
-        if (key0[q] >= p.layers[l].br.hi_key) { nib |= 1u << q; atomicAdd(&p.layers[l].n_above, 1ull); }
-        else if (key0[q] >= p.layers[l].br.lo_key) cnib |= 1u << q;
-      }
-    }
-    // Append this chunk's candidates to the warp's segment (their order inside the segment is
-    // irrelevant: the composite keys carry the index).  Two forms, chosen by measurement: the
-    // register-staged front-end is issue-bound and takes the shorter one (one prefix over the lanes
-    // from three ballots on the bits of the per-lane count); the bulk-copy front-end is register-
-    // bound (96 registers per thread) and keeps the one with the shortest live ranges.
-    if constexpr (STORE) {
-      if (__any_sync(0xFFFFFFFFu, cnib != 0u)) {
-        const uint32_t n = __popc(cnib), lt = (1u << lane) - 1u;
-        const uint32_t b0 = __ballot_sync(0xFFFFFFFFu, n & 1u), b1 = __ballot_sync(0xFFFFFFFFu, n & 2u),
-                       b2 = __ballot_sync(0xFFFFFFFFu, n & 4u);
-        uint32_t pos = sa.cursor + __popc(b0 & lt) + 2u * __popc(b1 & lt) + 4u * __popc(b2 & lt);
-        if (cnib != 0u) {
-          const uint32_t inv = 0xFFFFFFFFu - (uint32_t)i0;
-          if (pos + 4u <= p.seg_cap) {                      // room for all four: one pointer, no bound checks
-            uint2* dst = reinterpret_cast<uint2*>(sa.seg + pos);
-#pragma unroll
-            for (int q = 0; q < 4; ++q)
-              if ((cnib >> q) & 1u) { *dst = make_uint2(inv - q, key0[q]); ++dst; }      // little endian: low word = index part
-          } else {
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-              if ((cnib >> q) & 1u) {
-                if (pos < p.seg_cap) sa.seg[pos] = ((unsigned long long)key0[q] << 32) | (unsigned long long)(inv - q);
-                ++pos;
-              }
-            }
-          }
-        }
-        sa.cursor += __popc(b0) + 2u * __popc(b1) + 4u * __popc(b2);
-      }
-    } else {
-      if (__any_sync(0xFFFFFFFFu, cnib != 0u)) {              // candidates are rare: usually skipped
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const bool cnd = (cnib >> q) & 1u;
-          const uint32_t bal = __ballot_sync(0xFFFFFFFFu, cnd);
-          if (cnd) {
-            const uint32_t pos = sa.cursor + __popc(bal & ((1u << lane) - 1u));
-            if (pos < p.seg_cap)
-              sa.seg[pos] = ((unsigned long long)key0[q] << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)(i0 + q));
-          }
-          sa.cursor += __popc(bal);
-        }
-      }
-    }
-    if (!mixed) sa.n_above += __popc(nib);
-    uint32_t w = nib << ((lane & 7) << 2);
-    w |= __shfl_xor_sync(0xFFFFFFFFu, w, 1);
-    w |= __shfl_xor_sync(0xFFFFFFFFu, w, 2);
-    w |= __shfl_xor_sync(0xFFFFFFFFu, w, 4);
-    if ((lane & 7) == 0) p.next_bits[(c << 2) + (lane >> 3)] = w;
+    __syncwarp();                                         // the scratch is reused by the next chunk
   }
+
+  if (STORE) {                                            // else the caller stores th / ee (staged bulk stores)
+    store4_f32<GUARD>(p.theta, i0, p.N, th);
+#pragma unroll
+    for (int r = 0; r < R; ++r) store4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
+  }
+
+  // Stage 2 (l.11) fused: classify |m~^0| against the predicted bracket.  Exactness does not
+  // depend on the prediction: sel_decide_kernel checks n_above < k <= n_above + n_cand.
+  bool mixed = false;                                     // chunk with entries of several layers (warp-uniform)
+  if (p.chunk_layer != nullptr) {
+    // per-layer refresh: the bracket is the one of this chunk's layer.  Warps walk the shard in
+    // ascending order, so a layer change is rare: flush the count, load the new bracket.
+    const uint32_t cl = __ldg(p.chunk_layer + c);
+    const uint32_t l = cl & 0x7FFFFFFFu;
+    mixed = (cl >> 31) != 0u;
+    if (l != sa.layer) {
+      warp_flush_layer(p, sa, lane);
+      sa.layer = l;
+      sa.lo = p.layers[l].br.lo_key; sa.hi = p.layers[l].br.hi_key;
+    }
+  }
+  uint32_t nib = 0, cnib = 0;
+  if (!mixed) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const bool valid = !GUARD || (i0 + q < p.N);
+      const bool above = valid && key0[q] >= sa.hi;
+      nib |= above ? (1u << q) : 0u;
+      cnib |= (valid && !above && key0[q] >= sa.lo) ? (1u << q) : 0u;
+    }
+  } else {
+    // a chunk shared by several layers (at most one per layer boundary): bracket and count per entry
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      if (GUARD && i0 + q >= p.N) continue;
+      uint32_t l = sa.layer;
+      while (i0 + q >= p.layers[l].end) ++l;
+      if (key0[q] >= p.layers[l].br.hi_key) { nib |= 1u << q; atomicAdd(&p.layers[l].n_above, 1ull); }
+      else if (key0[q] >= p.layers[l].br.lo_key) cnib |= 1u << q;
+    }
+  }
+  // Append this chunk's candidates (their order inside the segment is irrelevant: the composite
+  // keys carry the index).
+  if constexpr (RING) {
+    if (cnib != 0u) {
+      uint32_t pos = atomicAdd(cr.head, (uint32_t)__popc(cnib));
+      const uint32_t inv = 0xFFFFFFFFu - (uint32_t)i0;
+      uint2* ring2 = reinterpret_cast<uint2*>(cr.ring);
+#pragma unroll
+      for (int q = 0; q < 4; ++q)
+        if ((cnib >> q) & 1u) { ring2[pos & (kRing - 1u)] = make_uint2(inv - q, key0[q]); ++pos; }   // little endian: low word = index part
+    }
+    __syncwarp();
+    const uint32_t head = *reinterpret_cast<volatile uint32_t*>(cr.head);
+    while (head - sa.cursor >= 32u) ring_flush32(p, sa, cr, lane);
+  } else {
+    if (__any_sync(0xFFFFFFFFu, cnib != 0u)) {              // candidates are rare here: usually skipped
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const bool cnd = (cnib >> q) & 1u;
+        const uint32_t bal = __ballot_sync(0xFFFFFFFFu, cnd);
+        if (cnd) {
+          const uint32_t pos = sa.cursor + __popc(bal & ((1u << lane) - 1u));
+          if (pos < p.seg_cap)
+            sa.seg[pos] = ((unsigned long long)key0[q] << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)(i0 + q));
+        }
+        sa.cursor += __popc(bal);
+      }
+    }
+  }
+  if (!mixed) sa.n_above += __popc(nib);
+  // the word of M_t this lane's group of 8 shares: OR of the nibbles (a REDUX per group of 8 lanes
+  // compiles to four serialised collectives: slower than three shuffles)
+  uint32_t w = nib << lm.sh;
+  w |= __shfl_xor_sync(0xFFFFFFFFu, w, 1);
+  w |= __shfl_xor_sync(0xFFFFFFFFu, w, 2);
+  w |= __shfl_xor_sync(0xFFFFFFFFu, w, 4);
+  if (lm.sh == 0u) p.next_bits[(c << 2) + lm.ws] = w;
 }
 
-template <typename G, int R, bool DENSE, bool MSPARSE, bool GUARD, bool CLIPT>
-__device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int lane, float* sc, StageA& sa) {
-  const int64_t i0 = (c << 7) + ((int64_t)lane << 2);
+// A chunk's mask words as one lane needs them: its own word of the current (and, MSPARSE, the previous) mask + rk[c]
+struct MaskWords { uint32_t cw, pw; uint2 crk, prk; };
+template <bool CUR, bool PREV>
+__device__ __forceinline__ void load_mask_words(const StepParams& p, uint32_t c, const LaneMap& lm, MaskWords& w) {
+  if (CUR) { w.cw = __ldg(p.cur_bits + (c << 2) + lm.ws); w.crk = __ldg(p.cur_rk + c); }
+  if (PREV) { w.pw = __ldg(p.prev_bits + (c << 2) + lm.ws); w.prk = __ldg(p.prev_rk + c); }
+}
+// Which mask words the register-staged kernel fetches one trip ahead: 2 = both masks' (R = 1: 6 more live
+// registers still fit the 64 of four CTAs per SM), 1 = the previous mask's only (they feed the gather of m),
+// 0 = none (R >= 3: the registers are worth more to the streaming loads; measured)
+__host__ __device__ constexpr int step_prefetch(int R) { return R == 1 ? 2 : R == 2 ? 1 : 0; }
+
+// One chunk of the register-staged front-end.  sc: this warp's scratch, (R + 1) x 128 floats.
+// mw: this chunk's mask words, fetched during the previous trip (their L2 latency would otherwise sit
+// in front of the gather of m and, as ptxas schedules it, of the streaming loads too: 23 % of the
+// stall samples at R = 1); c_next: the chunk whose words to fetch now (0xFFFFFFFF: none).
+template <typename G, int R, bool DENSE, bool MSPARSE, bool GUARD, bool CLIPT, bool RING, int PF>
+__device__ __forceinline__ void fused_chunk(const StepParams& p, uint32_t c, uint32_t c_next, int lane, const LaneMap& lm, float* sc,
+                                            StageA& sa, const CandRing& cr, MaskWords& mw) {
+  // chunk and element indices are 32-bit (scape_create: N < 2^31), so that every address is ONE
+  // IMAD.WIDE.U32 off a kernel-parameter base instead of 64-bit index arithmetic
+  const uint32_t i0 = (c << 7) + ((uint32_t)lane << 2);
   // Issue order matters for latency: the mask words first (L2-resident, short latency), then the
   // 2R+1 streaming loads, and only then the gather of m_{t-1}, whose addresses depend on the
   // mask words -- it is in flight together with the streaming loads instead of after them.
-  uint4 cw = make_uint4(~0u, ~0u, ~0u, ~0u), pw = make_uint4(0, 0, 0, 0);
-  uint32_t cr = 0, pr = 0;
-  if (!DENSE) { cw = __ldg(reinterpret_cast<const uint4*>(p.cur_bits) + c); cr = __ldg(p.cur_rank + c); }
-  if (MSPARSE) { pw = __ldg(reinterpret_cast<const uint4*>(p.prev_bits) + c); pr = __ldg(p.prev_rank + c); }
+  if (!DENSE) load_mask_words<PF < 2, MSPARSE && PF < 1>(p, c, lm, mw);      // whatever was not fetched ahead
+  const uint32_t cw = mw.cw, pw = mw.pw;
+  const uint2 crk = mw.crk, prk = mw.prk;
 
   float th[4], mo[4], gg[R][4], ee[R][4];
   load4_f32<GUARD>(p.theta, i0, p.N, th);
@@ -480,45 +547,75 @@ __device__ __forceinline__ void fused_chunk(const StepParams& p, int64_t c, int 
     load4_f32<false>(p.e + r * p.e_stride, i0, p.N, ee[r]);
   }
 
-  uint32_t mybits = 0xFu, jbase = 0;
-  if (!DENSE) lane_bits_from_words(cw, cr, lane, mybits, jbase);
-  if (MSPARSE) {
-    uint32_t pbits, pbase;
-    lane_bits_from_words(pw, pr, lane, pbits, pbase);
-    gather_prev_m(p.pm_prev, pbits, pbase, mo);
+  if constexpr (DENSE) {
+    dense_compute<R, GUARD, CLIPT>(p, i0, th, mo, gg, ee, sa);
+  } else {
+    uint32_t mybits, jbase;
+    lane_decode(cw, crk, lm, mybits, jbase);
+    if (MSPARSE) {
+      uint32_t pbits, pbase;
+      lane_decode(pw, prk, lm, pbits, pbase);
+      gather_prev_m(p.pm_prev, pbits, pbase, mo);
+    }
+    if (PF > 0 && c_next != 0xFFFFFFFFu) load_mask_words<PF >= 2, MSPARSE && PF >= 1>(p, c_next, lm, mw);
+    sparse_compute<R, GUARD, true, CLIPT, RING, kChunk>(p, c, lane, lm, i0, mybits, jbase, crk.x, crk.y >> 24, sc, sc + kChunk,
+                                                        th, mo, gg, ee, sa, cr);
   }
+}
 
-  fused_compute<R, DENSE, GUARD, true, CLIPT>(p, c, lane, i0, mybits, jbase, cr, DENSE ? 0u : chunk_popc(cw), sc, sc + kChunk, th, mo, gg, ee, sa);
+// Dynamic shared memory of the register-staged kernel (sparse variants): per warp the scratch of the
+// on-mask arithmetic ((R + 1) x 128 floats) and the candidate ring, then the 8 ring heads.
+__host__ __device__ constexpr uint32_t step_scratch_bytes(int R) { return (uint32_t)(R + 1) * kChunk * 4u; }
+__host__ __device__ constexpr uint32_t step_smem_bytes(int R, bool dense) {
+  return dense ? 0u : 8u * (step_scratch_bytes(R) + kRing * 8u) + 8u * 4u;
 }
 
 template <typename G, int R, bool DENSE, bool MSPARSE, bool CLIPT>
 // resident CTAs per SM: sparse steps with one or two replicas are latency-bound (12-24 bytes per parameter in
 // flight per lane), so they trade registers for a fourth CTA (measured, N = 2^28, R = 2, 90 %: 2.54 -> 2.29 ms)
 __global__ void __launch_bounds__(256, ((!DENSE && R <= 2) ? 4 : R <= 4 ? 3 : 2)) scape_fused_step_kernel(const __grid_constant__ StepParams p) {
-  const int lane = threadIdx.x & 31;
-  const int64_t wpb = blockDim.x >> 5;
-  const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
-  const int64_t nwarps = (int64_t)gridDim.x * wpb;
-  const int64_t full = p.N >> 7;
-  __shared__ float scratch[DENSE ? 1 : 8 * 2 * kChunk];     // per warp: (sum_r m~^r, m_old) of the selected entries
-  float* sc = DENSE ? scratch : scratch + (threadIdx.x >> 5) * (2 * kChunk);
+  extern __shared__ __align__(16) unsigned char step_smem[];
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const uint32_t wpb = blockDim.x >> 5;
+  const uint32_t warp = blockIdx.x * wpb + wib;
+  const uint32_t nwarps = gridDim.x * wpb;
+  const uint32_t full = (uint32_t)(p.N >> 7);
+  const LaneMap lm = lane_map(lane);
+  float* sc = reinterpret_cast<float*>(step_smem + (size_t)wib * step_scratch_bytes(R));
+  CandRing cr{};
   StageA sa{};
   sa.layer = kNoLayer;
   if (!DENSE) {
+    cr.ring = reinterpret_cast<unsigned long long*>(step_smem + 8u * step_scratch_bytes(R)) + (size_t)wib * kRing;
+    cr.head = reinterpret_cast<uint32_t*>(step_smem + 8u * (step_scratch_bytes(R) + kRing * 8u)) + wib;
+    if (lane == 0) *cr.head = 0u;
+    __syncwarp();
     sa.lo = p.ctl->br.lo_key; sa.hi = p.ctl->br.hi_key;
     sa.seg = p.cand + (size_t)warp * p.seg_cap;
   }
-  for (int64_t c = warp; c < full; c += nwarps) fused_chunk<G, R, DENSE, MSPARSE, false, CLIPT>(p, c, lane, sc, sa);
-  if (full < p.n_chunks && warp == full % nwarps) fused_chunk<G, R, DENSE, MSPARSE, true, CLIPT>(p, full, lane, sc, sa);
+  // this warp's chunks: warp, warp + nwarps, ... (full chunks), then possibly the ragged last one
+  const bool tail = (int64_t)full < p.n_chunks && warp == full % nwarps;
+  MaskWords mw{};
+  constexpr int PF = DENSE ? 0 : step_prefetch(R);
+  if (PF > 0 && (warp < full || tail)) load_mask_words<PF >= 2, MSPARSE && PF >= 1>(p, warp < full ? warp : full, lm, mw);
+  // (c < full before c += nwarps wraps: full + nwarps < 2^25)
+  for (uint32_t c = warp; c < full; c += nwarps) {
+    uint32_t cn = 0xFFFFFFFFu;
+    if constexpr (PF > 0) cn = c + nwarps < full ? c + nwarps : tail ? full : 0xFFFFFFFFu;
+    fused_chunk<G, R, DENSE, MSPARSE, false, CLIPT, true, PF>(p, c, cn, lane, lm, sc, sa, cr, mw);
+  }
+  if (tail) fused_chunk<G, R, DENSE, MSPARSE, true, CLIPT, true, PF>(p, full, 0xFFFFFFFFu, lane, lm, sc, sa, cr, mw);
   if (!DENSE) {
+    const uint32_t n_cand = ring_drain(p, sa, cr, lane);
     if (p.chunk_layer != nullptr) warp_flush_layer(p, sa, lane);      // per-layer counts; seg_above stays 0
     uint32_t na = sa.n_above;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
-    if (lane == 0) { p.seg_count[warp] = sa.cursor; p.seg_above[warp] = na; }
+    if (lane == 0) { p.seg_count[warp] = n_cand; p.seg_above[warp] = na; }
   }
   if (CLIPT && p.clip == 1) warp_store_sumsq(p, sa, warp, lane);
 }
+
 
 // ------------------------------------------------------------------------------------------
 // Steady-state variant with shared-memory staging (sparse mask in, m stored sparsely).
@@ -538,8 +635,9 @@ __global__ void __launch_bounds__(256, ((!DENSE && R <= 2) ? 4 : R <= 4 ? 3 : 2)
 //              stage's empty barrier, which hands it back to the producer
 // So a stage is reusable one tile after its consumers are done with it, the stores of tile i overlap
 // the compute of tile i+1, and the bytes in flight are (stages - 1) x tile per CTA, independent of
-// register pressure.  The scratch of the on-mask arithmetic is the warp's own theta / e^0 slice of
-// the stage (its contents are in registers by then and are written back after fused_compute).
+// register pressure.  The scratch of the on-mask arithmetic is the warp's own theta slice (m_old)
+// and e^r slices (m~^r) of the stage (their contents are in registers by then and are written back after
+// sparse_compute).
 // ------------------------------------------------------------------------------------------
 constexpr int kTmaConsumerWarps = 8;
 constexpr int kTmaTile = kTmaConsumerWarps * kChunk;          // 1024 parameters
@@ -584,19 +682,18 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, uint32
                ::"r"(smem_u32(dst_smem)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy) : "memory");
 }
 
-struct TmaMaskWords { uint4 cw, pw; uint32_t cr, pr; };
+using TmaMaskWords = MaskWords;
 struct TmaTileState { uint32_t mybits, jbase, r0, cnt; float mo[4]; };
 
-__device__ __forceinline__ void tma_load_words(const StepParams& p, int64_t c, TmaMaskWords& w) {
-  w.cw = __ldg(reinterpret_cast<const uint4*>(p.cur_bits) + c); w.cr = __ldg(p.cur_rank + c);
-  w.pw = __ldg(reinterpret_cast<const uint4*>(p.prev_bits) + c); w.pr = __ldg(p.prev_rank + c);
+__device__ __forceinline__ void tma_load_words(const StepParams& p, uint32_t c, const LaneMap& lm, TmaMaskWords& w) {
+  load_mask_words<true, true>(p, c, lm, w);
 }
 // decode a chunk's mask words for this lane and start the gather of m_{t-1}
-__device__ __forceinline__ void tma_decode_gather(const StepParams& p, const TmaMaskWords& w, int lane, TmaTileState& st) {
+__device__ __forceinline__ void tma_decode_gather(const StepParams& p, const TmaMaskWords& w, const LaneMap& lm, TmaTileState& st) {
   uint32_t pbits, pbase;
-  lane_bits_from_words(w.cw, w.cr, lane, st.mybits, st.jbase);
-  st.r0 = w.cr; st.cnt = chunk_popc(w.cw);
-  lane_bits_from_words(w.pw, w.pr, lane, pbits, pbase);
+  lane_decode(w.cw, w.crk, lm, st.mybits, st.jbase);
+  st.r0 = w.crk.x; st.cnt = w.crk.y >> 24;
+  lane_decode(w.pw, w.prk, lm, pbits, pbase);
   gather_prev_m(p.pm_prev, pbits, pbase, st.mo);
 }
 
@@ -611,16 +708,16 @@ __device__ __forceinline__ void bulk_s2g(void* dst, const void* src_smem, uint32
 // the tile's bulk stores and releases the previous stage (protocol above).
 template <typename G, int R, bool CLIPT>
 __device__ __forceinline__ void tma_consume_tile(const StepParams& p, int64_t tile, int64_t n_tiles, int64_t tstride,
-                                                 int warp, int lane, unsigned char* stage0, uint64_t* full, uint64_t* empty,
+                                                 int warp, int lane, const LaneMap& lm, unsigned char* stage0, uint64_t* full, uint64_t* empty,
                                                  int& s, uint32_t& ph, int n_stages, TmaMaskWords& nw,
                                                  TmaTileState& cur, TmaTileState& nxt, StageA& sa) {
   constexpr uint32_t TILE = tma_tile_bytes<G, R>();
   constexpr uint32_t OFF_E = kTmaTile * 4u, OFF_G = kTmaTile * 4u * (1u + R);
-  const int64_t c = tile * kTmaConsumerWarps + warp;
-  const int64_t i0 = (c << 7) + ((int64_t)lane << 2);
+  const uint32_t c = (uint32_t)tile * kTmaConsumerWarps + warp;
+  const uint32_t i0 = (c << 7) + ((uint32_t)lane << 2);
   if (tile + tstride < n_tiles) {
-    tma_decode_gather(p, nw, lane, nxt);
-    if (tile + 2 * tstride < n_tiles) tma_load_words(p, (tile + 2 * tstride) * kTmaConsumerWarps + warp, nw);
+    tma_decode_gather(p, nw, lm, nxt);
+    if (tile + 2 * tstride < n_tiles) tma_load_words(p, (uint32_t)(tile + 2 * tstride) * kTmaConsumerWarps + warp, lm, nw);
   }
   mbar_wait(&full[s], ph);
   const unsigned char* base = stage0 + (size_t)s * TILE;
@@ -645,13 +742,14 @@ __device__ __forceinline__ void tma_consume_tile(const StepParams& p, int64_t ti
   }
   // Results go back into the stage (in place) and leave as whole-tile bulk stores: 4 KB bursts
   // per stream instead of 512-byte warp stores.
-  // scratch of the on-mask arithmetic: this warp's own theta and e^0 slices of the stage (their
-  // contents are in registers now and are written back only after fused_compute)
+  // scratch of the on-mask arithmetic: this warp's own theta slice (m_old) and e^r slices (m~^r) of
+  // the stage (their contents are in registers now and are written back only after sparse_compute)
   unsigned char* wbase = stage0 + (size_t)s * TILE;
   __syncwarp();
-  fused_compute<R, false, false, false, CLIPT>(p, c, lane, i0, cur.mybits, cur.jbase, cur.r0, cur.cnt,
-                                               reinterpret_cast<float*>(wbase) + warp * kChunk,
-                                               reinterpret_cast<float*>(wbase + OFF_E) + warp * kChunk, th, cur.mo, gg, ee, sa);
+  sparse_compute<R, false, false, CLIPT, false, kTmaTile>(p, c, lane, lm, i0, cur.mybits, cur.jbase, cur.r0, cur.cnt,
+                                                          reinterpret_cast<float*>(wbase) + warp * kChunk,
+                                                          reinterpret_cast<float*>(wbase + OFF_E) + warp * kChunk, th, cur.mo, gg, ee, sa,
+                                                          CandRing{});
   *reinterpret_cast<float4*>(wbase + off * 4u) = make_float4(th[0], th[1], th[2], th[3]);
 #pragma unroll
   for (int r = 0; r < R; ++r)
@@ -717,6 +815,7 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
   }
 
   // ===== consumers =====
+  const LaneMap lm = lane_map(lane);
   const int64_t gwarp = (int64_t)blockIdx.x * kTmaConsumerWarps + warp;     // candidate segment of this warp
   StageA sa{};
   sa.layer = kNoLayer;
@@ -733,16 +832,16 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
   TmaTileState stA{}, stB{};
   if (tile < n_tiles) {
     TmaMaskWords w0;
-    tma_load_words(p, tile * kTmaConsumerWarps + warp, w0);
-    if (tile + tstride < n_tiles) tma_load_words(p, (tile + tstride) * kTmaConsumerWarps + warp, nw);
-    tma_decode_gather(p, w0, lane, stA);
+    tma_load_words(p, (uint32_t)tile * kTmaConsumerWarps + warp, lm, w0);
+    if (tile + tstride < n_tiles) tma_load_words(p, (uint32_t)(tile + tstride) * kTmaConsumerWarps + warp, lm, nw);
+    tma_decode_gather(p, w0, lm, stA);
   }
   int s = 0; uint32_t ph = 0;
   while (tile < n_tiles) {
-    tma_consume_tile<G, R, CLIPT>(p, tile, n_tiles, tstride, warp, lane, stage0, full, empty, s, ph, n_stages, nw, stA, stB, sa);
+    tma_consume_tile<G, R, CLIPT>(p, tile, n_tiles, tstride, warp, lane, lm, stage0, full, empty, s, ph, n_stages, nw, stA, stB, sa);
     tile += tstride;
     if (tile >= n_tiles) break;
-    tma_consume_tile<G, R, CLIPT>(p, tile, n_tiles, tstride, warp, lane, stage0, full, empty, s, ph, n_stages, nw, stB, stA, sa);
+    tma_consume_tile<G, R, CLIPT>(p, tile, n_tiles, tstride, warp, lane, lm, stage0, full, empty, s, ph, n_stages, nw, stB, stA, sa);
     tile += tstride;
   }
   if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // stores have landed
@@ -750,12 +849,13 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
 
   // chunks past the last full tile (fewer than 8, the last one possibly ragged): LDG path
   {
-    const int64_t c = n_tiles * kTmaConsumerWarps + warp;
-    if (c < p.n_chunks && blockIdx.x == (unsigned)(n_tiles % gridDim.x)) {
+    const uint32_t c = (uint32_t)n_tiles * kTmaConsumerWarps + warp;
+    if ((int64_t)c < p.n_chunks && blockIdx.x == (unsigned)(n_tiles % gridDim.x)) {
       // (all bulk stores of this CTA have completed: the first stage serves as scratch)
-      float* sc = reinterpret_cast<float*>(stage0) + warp * (2 * kChunk);
-      if (((c + 1) << 7) <= p.N) fused_chunk<G, R, false, true, false, CLIPT>(p, c, lane, sc, sa);
-      else fused_chunk<G, R, false, true, true, CLIPT>(p, c, lane, sc, sa);
+      float* sc = reinterpret_cast<float*>(stage0) + warp * ((R + 1) * kChunk);
+      MaskWords mw;
+      if (((int64_t)(c + 1) << 7) <= p.N) fused_chunk<G, R, false, true, false, CLIPT, false, 0>(p, c, 0xFFFFFFFFu, lane, lm, sc, sa, CandRing{}, mw);
+      else fused_chunk<G, R, false, true, true, CLIPT, false, 0>(p, c, 0xFFFFFFFFu, lane, lm, sc, sa, CandRing{}, mw);
     }
   }
   if (p.chunk_layer != nullptr) warp_flush_layer(p, sa, lane);        // per-layer counts; seg_above stays 0

@@ -1,6 +1,6 @@
 // scape_select_kernels.cuh — the kernels of the SCAPE step that are not the streaming pass: the exact
 // top-k select of stage 2 (Alg. 1 l.11), the ordered compaction of a bit mask into
-// rank128 + the ascending index list (the int32 half of the sparse buffer, l.9), the deferred
+// rk (rank128 + word prefixes) + the ascending index list (the int32 half of the sparse buffer, l.9), the deferred
 // updates (clip_grad l.14, workers l.10-17), the mask bit pack / unpack and the
 // Algorithm 2 parameter kernels.  Plain (non-template) kernels: this header is
 // included by scape.cu only.
@@ -20,7 +20,7 @@ namespace scapek {
 struct KeySrc {
   const float* e0;            // [Npad]
   const uint32_t* cur_bits;   // mask the step used (nullptr => treat every position as "off":
-  const uint32_t* cur_rank;   //   all-ones step with m~^0 stashed in e^0)
+  const uint2* cur_rk;        //   all-ones step with m~^0 stashed in e^0)
   const float* packed0;       // b^0
   int64_t N;
   int64_t n_chunks;
@@ -37,7 +37,7 @@ __device__ __forceinline__ void chunk_keys(const KeySrc& s, int64_t c, int lane,
   float x[4] = {ev.x, ev.y, ev.z, ev.w};
   if (s.cur_bits != nullptr) {
     uint32_t mybits, jbase;
-    lane_mask_bits(s.cur_bits, s.cur_rank, c, lane, mybits, jbase);
+    lane_mask_bits(s.cur_bits, s.cur_rk, c, lane, mybits, jbase);
 #pragma unroll
     for (int q = 0; q < 4; ++q)
       if ((mybits >> q) & 1u) x[q] = __ldg(s.packed0 + jbase + __popc(mybits & ((1u << q) - 1u)));
@@ -728,7 +728,7 @@ __global__ void __launch_bounds__(1024) mask_scan_blocks_kernel(uint32_t* __rest
 
 __global__ void __launch_bounds__(1024) mask_rank_idx_kernel(const uint32_t* __restrict__ bits, int64_t n_chunks,
                                                             const uint32_t* __restrict__ block_off,
-                                                            uint32_t* __restrict__ rank128, int32_t* __restrict__ idx, int64_t idx_cap) {
+                                                            uint2* __restrict__ rk, int32_t* __restrict__ idx, int64_t idx_cap) {
   __shared__ uint32_t ws[32];
   const int64_t c = (int64_t)blockIdx.x * kCompactChunksPerBlock + threadIdx.x;
   uint4 w = make_uint4(0, 0, 0, 0);
@@ -749,7 +749,7 @@ __global__ void __launch_bounds__(1024) mask_rank_idx_kernel(const uint32_t* __r
   __syncthreads();
   if (c >= n_chunks) return;
   uint32_t j = block_off[blockIdx.x] + ws[wid] + incl - n;
-  rank128[c] = j;
+  rk[c] = make_uint2(j, chunk_prefix_bytes(__popc(w.x), __popc(w.y), __popc(w.z), __popc(w.w)));
   if (idx == nullptr) return;
   const uint32_t words[4] = {w.x, w.y, w.z, w.w};
   const int64_t base = c << 7;
@@ -775,7 +775,7 @@ __global__ void __launch_bounds__(1024) mask_rank_idx_kernel(const uint32_t* __r
 //   ctl[0] = total number of set bits (out), ctl[1] = ticket (returns to 0).
 __global__ void __launch_bounds__(1024) mask_compact_kernel(const uint32_t* __restrict__ bits, int64_t n_chunks,
                                                            unsigned long long* state, uint32_t* ctl, uint32_t epoch,
-                                                           uint32_t* __restrict__ rank128, int32_t* __restrict__ idx, int64_t idx_cap) {
+                                                           uint2* __restrict__ rk, int32_t* __restrict__ idx, int64_t idx_cap) {
   __shared__ uint32_t ws[32];
   __shared__ uint32_t s_bid, s_prefix;
   if (threadIdx.x == 0) s_bid = atomicAdd(&ctl[1], 1u);
@@ -834,7 +834,7 @@ __global__ void __launch_bounds__(1024) mask_compact_kernel(const uint32_t* __re
   __syncthreads();
   if (c >= n_chunks) return;
   uint32_t j = s_prefix + ws[wid] + incl - n;
-  rank128[c] = j;
+  rk[c] = make_uint2(j, chunk_prefix_bytes(__popc(w.x), __popc(w.y), __popc(w.z), __popc(w.w)));
   if (idx == nullptr) return;
   const uint32_t words[4] = {w.x, w.y, w.z, w.w};
   const int64_t base = c << 7;
@@ -1077,7 +1077,7 @@ __device__ __forceinline__ void param_apply_lane(float* __restrict__ w, uint16_t
 constexpr int kApplyChunks = 4;
 template <bool BF16, bool HAT, bool ALLONES>
 __global__ void __launch_bounds__(256, 4) param_apply_kernel(float* __restrict__ w, uint16_t* __restrict__ w_hat,
-                                                         const uint32_t* __restrict__ bits, const uint32_t* __restrict__ rank,
+                                                         const uint32_t* __restrict__ bits, const uint2* __restrict__ rank,
                                                          const void* __restrict__ payload, int64_t N, int64_t n_chunks,
                                                          float wd, float neg_lr) {
   const int lane = threadIdx.x & 31;
@@ -1093,7 +1093,7 @@ __global__ void __launch_bounds__(256, 4) param_apply_kernel(float* __restrict__
 #pragma unroll
     for (int u = 0; u < kApplyChunks; ++u) {
       mw[u] = make_uint4(0, 0, 0, 0); r0[u] = 0;
-      if (!ALLONES) { mw[u] = __ldg(reinterpret_cast<const uint4*>(bits) + (c + u * nwarps)); r0[u] = __ldg(rank + (c + u * nwarps)); }
+      if (!ALLONES) { mw[u] = __ldg(reinterpret_cast<const uint4*>(bits) + (c + u * nwarps)); r0[u] = __ldg(rank + (c + u * nwarps)).x; }
     }
 #pragma unroll
     for (int u = 0; u < kApplyChunks; ++u)
@@ -1105,7 +1105,7 @@ __global__ void __launch_bounds__(256, 4) param_apply_kernel(float* __restrict__
   for (; c < n_chunks; c += nwarps) {                        // the last trips, and the ragged last chunk
     uint4 ma = make_uint4(0, 0, 0, 0);
     uint32_t ra = 0;
-    if (!ALLONES) { ma = __ldg(reinterpret_cast<const uint4*>(bits) + c); ra = __ldg(rank + c); }
+    if (!ALLONES) { ma = __ldg(reinterpret_cast<const uint4*>(bits) + c); ra = __ldg(rank + c).x; }
     float va[4] = {0.0f, 0.0f, 0.0f, 0.0f};
     if (c < full) {
       if (!ALLONES) load4_f32<false>(w, (c << 7) + ((int64_t)lane << 2), N, va);
