@@ -199,6 +199,56 @@ int scape_step_local(scape_t* h, float* param, const void* const* grads, void* c
 int scape_exchange_buffers(scape_t* h, float** sums, int64_t* n_sums, uint32_t** mask_words, int64_t* n_mask_words);
 int scape_step_apply(scape_t* h, float* param, void* cuda_stream);
 
+/* The exchange itself, inside the library (PAPER.md:155 l.10 "all-reduce"; §IV-A :178 "each worker
+ * only computes a portion of the top-k operations"; Fig. 7 :218 "the new local masks from all
+ * workers are gathered"; :236, :244 "launch the asynchronous all-gather for M_t").  Call between
+ * scape_step_local and scape_step_apply, instead of exchanging scape_exchange_buffers yourself.
+ *   comm        an ncclComm_t of `world` ranks whose rank numbers are the worker numbers (the
+ *               caller creates it; scape_nccl_* below are there for callers without NCCL bindings).
+ *               The library resolves NCCL at run time (dlopen of the libnccl.so.2 already in the
+ *               process, else the system one): no link-time dependency; SCAPE_ECUDA if absent.
+ *   mask_comm   a second communicator for the mask portions, or NULL.  With one, the portions travel
+ *               on a stream of the handle's own, off the caller's stream: the one-step delay means
+ *               M_t is not needed before the NEXT scape_step_local, which waits for it (as does
+ *               every accessor).  NULL: they follow the sums on cuda_stream through `comm`.
+ *   What moves: the n_sums floats (in-place all-reduce SUM), and of M_t only what each worker made:
+ *               every maximal run of consecutive layers with one owner is broadcast from that owner
+ *               (grouped: one all-gather-v of word ranges, not an all-reduce of all N/32 words); the
+ *               at most n_layers - 1 words that hold a boundary between two owners are collected,
+ *               summed (disjoint bits: SUM = OR) and put back.  scape_exchange_plan reports the plan.
+ * Errors: SCAPE_EINVAL outside a split step; SCAPE_ECUDA for NCCL / CUDA failures (the split step
+ * stays pending; the communicator's state is NCCL's).                                             */
+int scape_step_exchange(scape_t* h, void* comm, void* mask_comm, void* cuda_stream);
+
+/* The plan scape_step_exchange follows for the mask (a pure function of the layer offsets and
+ * owners, identical on every worker).  HOST outputs, each may be NULL: *n_ranges word ranges
+ * [first[i], end[i]) broadcast from worker owner[i] (arrays of capacity `cap`), and *n_shared mask
+ * words shared by several owners (`shared`, capacity `cap_shared`).  Returns SCAPE_EINVAL if a
+ * capacity is too small (the counts are still written).                                          */
+int scape_exchange_plan(const scape_t* h, int64_t* first, int64_t* end, int32_t* owner, int cap, int* n_ranges,
+                        int64_t* shared, int cap_shared, int* n_shared);
+
+/* NCCL communicator helpers (thin forwards to ncclGetUniqueId / ncclCommInitRank / ncclCommDestroy
+ * of the NCCL the library resolved).  id: HOST, SCAPE_NCCL_ID_BYTES bytes, made by one rank and
+ * distributed by the caller (e.g. a torch.distributed broadcast over gloo).                      */
+#define SCAPE_NCCL_ID_BYTES 128
+int scape_nccl_unique_id(void* id);
+int scape_nccl_comm_create(int world, int rank, const void* id, void** comm);
+int scape_nccl_comm_destroy(void* comm);
+
+/* Asynchronous mask refresh ("the delayed use of the sparse mask ... provides an
+ * opportunity to ... hide" the top-k; :236 AsyncMaskRefresh).  theta, m, e^r and b are final when
+ * the streaming kernel ends; M_t is not needed before the next step.  With on = 1, scape_step runs
+ * stage 2 (the exact select, the rank / index list of M_t) on a stream of the handle's own, ordered
+ * after the streaming kernel by an event, and returns the caller's stream as soon as that kernel is
+ * enqueued: whatever the caller enqueues next (its forward / backward) overlaps the refresh.  The
+ * next scape_step / scape_step_local and every accessor make their stream wait for the refresh
+ * first; scape_join_refresh does so explicitly.  A step captured into a CUDA graph always runs the
+ * refresh in-stream (and requires any earlier asynchronous refresh to have completed: synchronise
+ * before capturing).  Default off.  scape_step_exchange with a mask_comm uses the same stream.   */
+int scape_set_async_refresh(scape_t* h, int on);
+int scape_join_refresh(scape_t* h, void* cuda_stream);
+
 /* Algorithm 2, parameter side (Eq. 6 :207-211).  With
  * Megatron-LM's distributed optimizer only the OWNER of a partition holds its updated parameters
  * w'; before the next forward pass the others need them.  Eq. 6: after the update of step t,

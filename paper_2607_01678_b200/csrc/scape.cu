@@ -3,6 +3,8 @@
 // No CPU fallback exists: every stage runs in the kernels of scape_kernels.cuh.
 #include "../../include/scape.h"
 
+#include <dlfcn.h>
+
 #include <algorithm>
 #include <cmath>
 #include <cstdarg>
@@ -149,6 +151,21 @@ struct scape {
   // scape_step_local / [all-reduce of the exchange buffers] / scape_step_apply
   int world = 1, rank = 0;
   std::vector<uint8_t> lay_skip;  // host copy: layers whose mask another worker makes
+  // the mask part of scape_step_exchange (a pure function of the layer offsets and owners, the same
+  // on every worker): word ranges broadcast from their owner + the words two owners share
+  std::vector<int64_t> xr_first, xr_end, x_shared;
+  std::vector<int32_t> xr_owner;
+  uint32_t* x_shared_idx = nullptr;   // [x_shared.size()] device copy of the shared word numbers
+  uint32_t* x_shared_buf = nullptr;   // [x_shared.size()] their values, summed over the workers
+  bool pending_mask_on_side = false;  // the mask portions travel on `side`: scape_step_apply compacts there
+
+  // asynchronous refresh (scape_set_async_refresh) and the mask exchange with its own communicator:
+  // a stream of the handle's own, ordered against the caller's stream by two events
+  bool async_refresh = false;
+  cudaStream_t side = nullptr;
+  cudaEvent_t ev_main = nullptr, ev_side = nullptr;
+  bool side_used = false;         // ev_side has been recorded: the caller's stream must wait for it
+
   bool pending = false;           // step_local has run, step_apply has not
   bool pending_need_select = false;
   int pending_pm_out = 0;

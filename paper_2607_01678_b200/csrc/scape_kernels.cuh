@@ -344,7 +344,7 @@ __device__ __forceinline__ uint32_t ring_drain(const StepParams& p, StageA& sa, 
 //   scm = 128 floats (m_old), sc = R arrays of 128 floats SCS floats apart (m~^r), private to this warp
 //   RING: candidates go through the shared-memory ring `cr` (register-staged front-end), else straight
 //   to the segment with one ballot per element (bulk-copy front-end: register-bound, shared memory full)
-template <int R, bool GUARD, bool STORE, bool CLIPT, bool RING, int SCS>
+template <int R, bool GUARD, bool STORE, bool CLIPT, bool RING, int SCS, bool DIRECT = false>
 __device__ __forceinline__ void sparse_compute(const StepParams& p, uint32_t c, int lane, const LaneMap& lm, uint32_t i0,
                                                uint32_t mybits, uint32_t jbase, uint32_t r0, uint32_t cnt, float* scm, float* sc,
                                                float (&th)[4], const float (&mo)[4],
@@ -379,8 +379,18 @@ __device__ __forceinline__ void sparse_compute(const StepParams& p, uint32_t c, 
         key0[q] = __float_as_uint(mt[0]) & 0x7FFFFFFFu;
         if (on) {
           *pm = mo[q];
+          if constexpr (DIRECT) {
+            float* pk = p.packed + (r0 + (uint32_t)(ps - sc));
+            float sm = mt[0];
 #pragma unroll
-          for (int r = 0; r < R; ++r) ps[r * SCS] = mt[r];
+            for (int r = 0; r < R; ++r) { *pk = mt[r]; pk += p.packed_stride; }                 // l.9
+#pragma unroll
+            for (int r = 1; r < R; ++r) sm = __fadd_rn(sm, mt[r]);                              // l.10, r ascending
+            *ps = sm;
+          } else {
+#pragma unroll
+            for (int r = 0; r < R; ++r) ps[r * SCS] = mt[r];
+          }
           ++ps; ++pm;
         }
       }
@@ -388,15 +398,17 @@ __device__ __forceinline__ void sparse_compute(const StepParams& p, uint32_t c, 
     __syncwarp();
     for (uint32_t l = lane; l < cnt; l += 32) {           // lane l: the chunk's selected entry of rank l
       const float mq = scm[l];
-      float* pk = p.packed + (r0 + l);
       float sm = sc[l];
-      *pk = sm;                                                                             // l.9, r = 0
+      if constexpr (!DIRECT) {
+        float* pk = p.packed + (r0 + l);
+        __stcs(pk, sm);                                                                     // l.9, r = 0
 #pragma unroll
-      for (int r = 1; r < R; ++r) {
-        const float v = sc[r * SCS + l];
-        pk += p.packed_stride;
-        *pk = v;                                                                            // l.9
-        sm = __fadd_rn(sm, v);                                                              // l.10, r ascending
+        for (int r = 1; r < R; ++r) {
+          const float v = sc[r * SCS + l];
+          pk += p.packed_stride;
+          __stcs(pk, v);                                                                    // l.9
+          sm = __fadd_rn(sm, v);                                                            // l.10, r ascending
+        }
       }
       const float pq = __fmul_rn(p.b1, mq);
       const float bb = p.r_pow2 ? __fmul_rn(sm, p.inv_R) : __fdiv_rn(sm, p.R_f);          // l.10
@@ -644,6 +656,8 @@ constexpr int kTmaTile = kTmaConsumerWarps * kChunk;          // 1024 parameters
 constexpr int kTmaThreads = (kTmaConsumerWarps + 1) * 32;     // + 1 producer warp
 constexpr int kTmaMaxStages = 8;
 constexpr int kTmaBarrierBytes = 128;                         // full[8] + empty[8]
+constexpr int kTmaPrefetchAhead = 1;                          // tiles beyond the one being loaded whose m_{t-1} range the producer prefetches
+constexpr bool kTmaDirectPack = false;                        // b^r stored from the owning lanes (phase 1) instead of staged
 
 template <typename G, int R>
 __host__ __device__ constexpr uint32_t tma_tile_bytes() { return kTmaTile * 4u * (1u + R) + kTmaTile * (uint32_t)sizeof(G) * R; }
@@ -746,7 +760,7 @@ __device__ __forceinline__ void tma_consume_tile(const StepParams& p, int64_t ti
   // the stage (their contents are in registers now and are written back only after sparse_compute)
   unsigned char* wbase = stage0 + (size_t)s * TILE;
   __syncwarp();
-  sparse_compute<R, false, false, CLIPT, false, kTmaTile>(p, c, lane, lm, i0, cur.mybits, cur.jbase, cur.r0, cur.cnt,
+  sparse_compute<R, false, false, CLIPT, false, kTmaTile, kTmaDirectPack>(p, c, lane, lm, i0, cur.mybits, cur.jbase, cur.r0, cur.cnt,
                                                           reinterpret_cast<float*>(wbase) + warp * kChunk,
                                                           reinterpret_cast<float*>(wbase + OFF_E) + warp * kChunk, th, cur.mo, gg, ee, sa,
                                                           CandRing{});
@@ -789,12 +803,27 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
   __syncthreads();
 
   if (warp == kTmaConsumerWarps) {
-    // ===== producer: one lane streams the tiles of this CTA =====
-    if (lane == 0) {
-      uint64_t policy;
-      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
-      int s = 0; uint32_t ph = 0;
-      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    // ===== producer: one lane streams the tiles of this CTA; the whole warp first pulls the part of
+    // the previous packed mean (= m_{t-1}) that a coming tile's gather will read into L2.  That part
+    // is ONE contiguous range per chunk (rank128 .. + the chunk's count); the streaming traffic since
+    // the last step has pushed it out of L2, and the consumers' 4-byte gathers of it, issued one tile
+    // ahead, were what they waited for (40 % of their stall samples: DRAM latency under load exceeds
+    // a tile's time).  Lane l: chunk l / 4 of the tile, 128-byte line l % 4 of its range.
+    auto prefetch_pm = [&](int64_t tile) {
+      if (tile >= n_tiles) return;
+      const uint2 prk = __ldg(p.prev_rk + (tile * kTmaConsumerWarps + (lane >> 2)));
+      const uint32_t cntp = prk.y >> 24;
+      const char* a = reinterpret_cast<const char*>(p.pm_prev + prk.x);
+      const char* line = reinterpret_cast<const char*>((uintptr_t)a & ~(uintptr_t)127) + ((uint32_t)lane & 3u) * 128u;
+      if (cntp != 0u && line < a + cntp * 4u) asm volatile("prefetch.global.L2 [%0];" ::"l"(line));
+    };
+    uint64_t policy;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+    for (int a = 0; a < kTmaPrefetchAhead; ++a) prefetch_pm((int64_t)blockIdx.x + (int64_t)a * gridDim.x);
+    int s = 0; uint32_t ph = 0;
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      prefetch_pm(tile + (int64_t)kTmaPrefetchAhead * gridDim.x);
+      if (lane == 0) {
         mbar_wait(&empty[s], ph ^ 1u);                         // every consumer warp has read the old contents
         mbar_expect_tx(&full[s], TILE);
         unsigned char* base = stage0 + (size_t)s * TILE;
@@ -808,8 +837,9 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
           bulk_g2s(base + OFF_G + r * (kTmaTile * (uint32_t)sizeof(G)),
                    reinterpret_cast<const unsigned char*>(p.g[r]) + e0 * (int64_t)sizeof(G),
                    kTmaTile * (uint32_t)sizeof(G), &full[s], policy);
-        if (++s == n_stages) { s = 0; ph ^= 1u; }
       }
+      __syncwarp();
+      if (++s == n_stages) { s = 0; ph ^= 1u; }
     }
     return;
   }

@@ -214,7 +214,9 @@ __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ K
 // half-width follows the error the previous extrapolation made.  shrink > 0: cap the half-width at
 // shrink x the old one (the candidate list was more than half full).
 constexpr float kNarrow = 0.7f;          // factor by which the half-width may shrink per step (measured: 0.55 missed once in the config-5 sweep, 0.85 kept ~1.5x more candidates)
-constexpr float kErrMult = 3.0f;         // half-width >= kErrMult x the last prediction error + 0.01
+constexpr float kErrMult = 3.0f;         // half-width >= kErrMult x the last prediction error + kErrAdd
+constexpr float kErrAdd = 0.004f;        // (0.01 and a floor of 0.02 until round 2: twice the candidates in steady state, where the
+constexpr float kMinDelta = 0.008f;      //  prediction error is 0.001-0.003; replayed on the recorded thresholds of 11 workloads: no miss)
 __device__ __forceinline__ void predict_bracket(Bracket& b, uint32_t Tkey, float shrink) {
   const float T = __uint_as_float(Tkey);
   float dl = b.delta, pred;
@@ -238,10 +240,10 @@ __device__ __forceinline__ void predict_bracket(Bracket& b, uint32_t Tkey, float
     pred = lnT + rn;
     b.r_prev = r;
     if (b.have_T == 1) dl = fmaxf(0.05f, 0.5f * fabsf(r));
-    else dl = fmaxf(kErrMult * fabsf(lnT - b.ln_pred) + 0.01f, kNarrow * dl);   // widen at once, narrow slowly
+    else dl = fmaxf(kErrMult * fabsf(lnT - b.ln_pred) + kErrAdd, kNarrow * dl);   // widen at once, narrow slowly
   }
   if (shrink > 0.0f) dl = fminf(dl, b.delta * shrink);
-  dl = fminf(fmaxf(dl, 0.02f), 1.0f);
+  dl = fminf(fmaxf(dl, kMinDelta), 1.0f);
   const float lo = __expf(pred - dl), hi = __expf(pred + dl);
   b.lo_key = __float_as_uint(lo) & 0x7FFFFFFFu;
   b.hi_key = (hi < 3.0e38f) ? (__float_as_uint(hi) & 0x7FFFFFFFu) : 0x7F800000u;
