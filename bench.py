@@ -445,7 +445,13 @@ def main():
         from paper_2607_01678_b200 import workers as wk
         sc.set_layers(w.offsets(), w.compress_flags())          # per-layer refresh, one layer per tensor
         sc.set_workers(world, rank, wk.balance_layers([n for _, n in w.tensors], world))
-        step = sc.step_workers
+        # the exchange runs inside the library (scape_step_exchange) over two NCCL communicators of its own:
+        # the sums on the caller's stream, the mask portions on the handle's stream
+        ids = [binding.scape_nccl_unique_id(), binding.scape_nccl_unique_id()] if rank == 0 else [None, None]
+        if world > 1:
+            dist.broadcast_object_list(ids, src=0)
+        comms = [binding.scape_nccl_comm_create(world, rank, i) for i in ids]
+        step = lambda th, g: sc.step_workers(th, g, comm=comms[0], mask_comm=comms[1])    # noqa: E731
     k = sc.k
     # the first step of Alg. 1 is dense (M_0 = 1): always warm-up, reported separately
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -499,6 +505,60 @@ def main():
         "step_frac_of_peak": sb / (ms_per_step * 1e-3) / 1e9 / peak,
         "step_frac_of_8TBs_nominal": sb / (ms_per_step * 1e-3) / 1e9 / 8000.0,
     }
+
+    # ---- asynchronous refresh (scape_set_async_refresh): what a step costs the caller's
+    # stream when other work (a stand-in for the forward / backward: ~5 ms of bf16 GEMMs, library calls) follows it
+    async_line = None
+    if world == 1 and not args.workers and not args.no_also and k < N:
+        big = torch.randn(8192, 8192, device=dev, dtype=torch.bfloat16)
+        big2 = torch.empty_like(big)
+        small = torch.randn(1024, 1024, device=dev, dtype=torch.bfloat16)
+        small2 = torch.empty_like(small)
+
+        def busy_full():                         # six GEMMs that each fill every SM for ~0.7 ms
+            for _ in range(6):
+                torch.matmul(big, big, out=big2)
+
+        # 600 GEMMs of 64 tiles each, replayed as one CUDA graph (no launch gaps): the stream is busy, most SMs are not
+        torch.matmul(small, small, out=small2)
+        torch.cuda.synchronize()
+        g_small = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g_small):
+            for _ in range(600):
+                torch.matmul(small, small, out=small2)
+
+        def busy_partial():
+            g_small.replay()
+
+        def loop(n, with_step, busy):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            a.record()
+            for i in range(n):
+                if with_step:
+                    step(theta, ring[i % n_sets])
+                busy()
+            b.record()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b) / n
+        async_line = {"streaming_kernel_ms": fused_avg_ms, "select_ms": select_ms / max(1, psteps),
+                      "note": "10 iterations of [scape_step; other work on the same stream]; step_cost = iteration - other work alone; "
+                              "async: stage 2 on the handle's own high-priority stream.  Work that fills every SM leaves nothing to "
+                              "overlap with; work that keeps the stream busy but not the SMs hides the refresh"}
+        for name, busy in (("other_work_fills_all_sms", busy_full), ("other_work_leaves_sms_idle", busy_partial)):
+            busy()
+            busy_ms = loop(10, False, busy)
+            res = {}
+            for mode in (False, True):
+                sc.set_async_refresh(mode)
+                loop(3, True, busy)
+                res[mode] = loop(10, True, busy)
+            sc.set_async_refresh(False)
+            sc.join_refresh()
+            torch.cuda.synchronize()
+            async_line[name] = {"other_work_ms": busy_ms, "step_cost_in_stream_ms": res[False] - busy_ms,
+                                "step_cost_async_ms": res[True] - busy_ms}
+        del g_small, big, big2, small, small2
 
     sc.close()
     del sc
@@ -578,7 +638,7 @@ def main():
                        "refresh": "per layer (one top-k per tensor)" if (args.layers or args.workers) else "flat top-k over the shard",
                        "first_dense_step_ms": first_step_ms},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": gpu_launches, "clocks": clk,
-            "also_measured": also,
+            "also_measured": also, "async_refresh": async_line,
         }
         print(json.dumps(line), flush=True)
     if world > 1 or args.workers:

@@ -244,8 +244,9 @@ int scape_nccl_comm_destroy(void* comm);
  * enqueued: whatever the caller enqueues next (its forward / backward) overlaps the refresh.  The
  * next scape_step / scape_step_local and every accessor make their stream wait for the refresh
  * first; scape_join_refresh does so explicitly.  A step captured into a CUDA graph always runs the
- * refresh in-stream (and requires any earlier asynchronous refresh to have completed: synchronise
- * before capturing).  Default off.  scape_step_exchange with a mask_comm uses the same stream.   */
+ * refresh in-stream, and a capture cannot wait for work enqueued outside it: call
+ * scape_join_refresh on the stream the graph will be launched on before capturing (SCAPE_EINVAL
+ * otherwise).  Default off.  scape_step_exchange with a mask_comm uses the same stream.   */
 int scape_set_async_refresh(scape_t* h, int on);
 int scape_join_refresh(scape_t* h, void* cuda_stream);
 

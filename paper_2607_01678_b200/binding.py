@@ -46,6 +46,13 @@ SYMBOLS = {
     "scape_step_local": (_I, [_VP, _VP, _VP, _VP]),
     "scape_exchange_buffers": (_I, [_VP, _VP, _VP, _VP, _VP]),
     "scape_step_apply": (_I, [_VP, _VP, _VP]),
+    "scape_step_exchange": (_I, [_VP, _VP, _VP, _VP]),
+    "scape_exchange_plan": (_I, [_VP, _VP, _VP, _VP, _I, _VP, _VP, _I, _VP]),
+    "scape_nccl_unique_id": (_I, [_VP]),
+    "scape_nccl_comm_create": (_I, [_I, _I, _VP, _VP]),
+    "scape_nccl_comm_destroy": (_I, [_VP]),
+    "scape_set_async_refresh": (_I, [_VP, _I]),
+    "scape_join_refresh": (_I, [_VP, _VP]),
     "scape_param_pack": (_I, [_VP, _VP, _I64, _I64, _VP, _I, _VP]),
     "scape_param_apply": (_I, [_VP, _VP, _VP, _VP, _I, _VP]),
     "scape_mask_pack": (_I, [_VP, _I64, _VP, _VP]),
@@ -208,6 +215,49 @@ def scape_exchange_buffers(h):
 
 def scape_step_apply(h, param_ptr, stream=0):
     _check(lib().scape_step_apply(h, param_ptr, stream), "scape_step_apply")
+
+
+def scape_step_exchange(h, comm, mask_comm=None, stream=0):
+    _check(lib().scape_step_exchange(h, comm, mask_comm, stream), "scape_step_exchange")
+
+
+def scape_exchange_plan(h):
+    """-> ([(first word, end word, owner)], [shared word numbers]): what scape_step_exchange moves of M_t"""
+    nr, ns = ctypes.c_int(), ctypes.c_int()
+    lib().scape_exchange_plan(h, None, None, None, 0, ctypes.byref(nr), None, 0, ctypes.byref(ns))
+    a, b = (ctypes.c_int64 * max(1, nr.value))(), (ctypes.c_int64 * max(1, nr.value))()
+    o, sh = (ctypes.c_int32 * max(1, nr.value))(), (ctypes.c_int64 * max(1, ns.value))()
+    _check(lib().scape_exchange_plan(h, a, b, o, nr.value, ctypes.byref(nr), sh, ns.value, ctypes.byref(ns)), "scape_exchange_plan")
+    return [(a[i], b[i], o[i]) for i in range(nr.value)], [sh[i] for i in range(ns.value)]
+
+
+SCAPE_NCCL_ID_BYTES = 128
+
+
+def scape_nccl_unique_id() -> bytes:
+    buf = ctypes.create_string_buffer(SCAPE_NCCL_ID_BYTES)
+    _check(lib().scape_nccl_unique_id(buf), "scape_nccl_unique_id")
+    return buf.raw
+
+
+def scape_nccl_comm_create(world, rank, uid: bytes):
+    assert len(uid) == SCAPE_NCCL_ID_BYTES
+    comm = ctypes.c_void_p()
+    _check(lib().scape_nccl_comm_create(int(world), int(rank), ctypes.create_string_buffer(uid, SCAPE_NCCL_ID_BYTES), ctypes.byref(comm)),
+           "scape_nccl_comm_create")
+    return comm.value
+
+
+def scape_nccl_comm_destroy(comm):
+    _check(lib().scape_nccl_comm_destroy(comm), "scape_nccl_comm_destroy")
+
+
+def scape_set_async_refresh(h, on):
+    _check(lib().scape_set_async_refresh(h, int(on)), "scape_set_async_refresh")
+
+
+def scape_join_refresh(h, stream=0):
+    _check(lib().scape_join_refresh(h, stream), "scape_join_refresh")
 
 
 def scape_param_pack(h, param_ptr, first, count, out_ptr, dtype, stream=0):
@@ -380,15 +430,43 @@ class Scape:
     def step_apply(self, param):
         scape_step_apply(self.h, param.data_ptr(), self._stream())
 
-    def step_workers(self, param, grads, group=None):
-        """One step of worker `rank` of `world` (torch.distributed, NCCL): the local half, the two
-        all-reduces of PAPER.md:155 / :178 on the handle's own buffers, the apply half."""
-        import torch.distributed as dist
+    def set_async_refresh(self, on=True):
+        scape_set_async_refresh(self.h, on)
+
+    def join_refresh(self):
+        scape_join_refresh(self.h, self._stream())
+
+    def exchange_plan(self):
+        return scape_exchange_plan(self.h)
+
+    def step_exchange(self, comm, mask_comm=None):
+        """The exchange inside the library (scape_step_exchange): comm / mask_comm are ncclComm_t values
+        (scape_nccl_comm_create, or any NCCL binding's)."""
+        scape_step_exchange(self.h, comm, mask_comm, self._stream())
+
+    def step_workers(self, param, grads, group=None, comm=None, mask_comm=None):
+        """One step of worker `rank` of `world`: the local half, the exchange of PAPER.md:155 / :178 /
+        :218, the apply half.  comm given: the library's own exchange over NCCL (scape_step_exchange).
+        Otherwise torch.distributed moves the same things on the handle's buffers -- the sums with an
+        all-reduce, of the mask only what the plan says: every word range from its owner, the shared
+        words summed -- which also works on backends NCCL does not cover (gloo: two ranks on one GPU)."""
         self.step_local(param, grads)
-        sums, words = self.exchange_tensors()
-        dist.all_reduce(sums, op=dist.ReduceOp.SUM, group=group)
-        if words is not None:
-            dist.all_reduce(words, op=dist.ReduceOp.SUM, group=group)      # disjoint portions: SUM == OR
+        if comm is not None:
+            self.step_exchange(comm, mask_comm)
+        else:
+            import torch
+            import torch.distributed as dist
+            sums, words = self.exchange_tensors()
+            dist.all_reduce(sums, op=dist.ReduceOp.SUM, group=group)
+            if words is not None:
+                ranges, shared = self.exchange_plan()
+                for a, b, owner in ranges:
+                    dist.broadcast(words[a:b], src=dist.get_global_rank(group, owner) if group is not None else owner, group=group)
+                if shared:
+                    ix = torch.tensor(shared, dtype=torch.int64, device=words.device)
+                    sw = words[ix]
+                    dist.all_reduce(sw, op=dist.ReduceOp.SUM, group=group)     # disjoint bits: SUM == OR
+                    words[ix] = sw
         self.step_apply(param)
 
     # ---- Algorithm 2, parameter side (include/scape.h) -----------------------------------

@@ -165,6 +165,7 @@ struct scape {
   cudaStream_t side = nullptr;
   cudaEvent_t ev_main = nullptr, ev_side = nullptr;
   bool side_used = false;         // ev_side has been recorded: the caller's stream must wait for it
+  bool side_dirty = false;        // ... and no stream has waited for it since (a capture cannot wait: it needs this false)
 
   bool pending = false;           // step_local has run, step_apply has not
   bool pending_need_select = false;
@@ -195,6 +196,126 @@ int grid_for(const scape* h, int64_t n_chunks, int warps_per_block, int blocks_p
   int64_t cap = (int64_t)h->n_sm * blocks_per_sm;
   if (need < 1) need = 1;
   return (int)(need < cap ? need : cap);
+}
+
+// ---- the handle's own stream (asynchronous refresh, mask exchange) --------------------------------
+int ensure_side(scape* h) {
+  if (h->side) return SCAPE_OK;
+  // highest priority: the refresh is a chain of small dependent kernels; at default priority its blocks
+  // queue behind whatever grid the caller has in flight and the chain stretches over the caller's whole
+  // forward / backward (measured: no overlap at all), at high priority they take the SM slots as they free up
+  int prio_lo = 0, prio_hi = 0;
+  CU_TRY(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+  CU_TRY(cudaStreamCreateWithPriority(&h->side, cudaStreamNonBlocking, prio_hi));
+  CU_TRY(cudaEventCreateWithFlags(&h->ev_main, cudaEventDisableTiming));
+  CU_TRY(cudaEventCreateWithFlags(&h->ev_side, cudaEventDisableTiming));
+  return SCAPE_OK;
+}
+
+bool is_capturing(cudaStream_t st) {
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { cudaGetLastError(); return false; }
+  return cs != cudaStreamCaptureStatusNone;
+}
+
+// Everything the handle enqueued on its own stream happens before what `st` gets from now on.  A
+// capturing stream cannot wait for an event recorded outside the capture: there the work must be over.
+int join_side(scape* h, cudaStream_t st) {
+  if (!h->side_used) return SCAPE_OK;
+  if (is_capturing(st)) {
+    // (no event query either: inside a global-mode capture it invalidates the capture)
+    if (h->side_dirty)
+      return fail(SCAPE_EINVAL, "work on the handle's own stream has not been joined: scape_join_refresh on the stream the graph "
+                                "will be launched on (or a device synchronisation) before capturing");
+    return SCAPE_OK;
+  }
+  CU_TRY(cudaStreamWaitEvent(st, h->ev_side, 0));
+  h->side_dirty = false;
+  return SCAPE_OK;
+}
+
+// side <- after everything enqueued on st so far
+int fork_side(scape* h, cudaStream_t st) {
+  int rc = ensure_side(h);
+  if (rc) return rc;
+  CU_TRY(cudaEventRecord(h->ev_main, st));
+  CU_TRY(cudaStreamWaitEvent(h->side, h->ev_main, 0));
+  return SCAPE_OK;
+}
+
+int mark_side(scape* h) {
+  CU_TRY(cudaEventRecord(h->ev_side, h->side));
+  h->side_used = true;
+  h->side_dirty = true;
+  return SCAPE_OK;
+}
+
+// ---- NCCL, resolved at run time (no link-time dependency; the paper's own data plane) ----
+struct NcclId { char internal[SCAPE_NCCL_ID_BYTES]; };
+struct NcclApi {
+  void* lib = nullptr;
+  int (*AllReduce)(const void*, void*, size_t, int, int, void*, cudaStream_t) = nullptr;
+  int (*Broadcast)(const void*, void*, size_t, int, int, void*, cudaStream_t) = nullptr;
+  int (*GroupStart)() = nullptr;
+  int (*GroupEnd)() = nullptr;
+  const char* (*GetErrorString)(int) = nullptr;
+  int (*GetUniqueId)(NcclId*) = nullptr;
+  int (*CommInitRank)(void**, int, NcclId, int) = nullptr;
+  int (*CommDestroy)(void*) = nullptr;
+};
+constexpr int kNcclFloat32 = 7, kNcclUint32 = 3, kNcclSum = 0;      // nccl.h: ncclDataType_t / ncclRedOp_t
+
+const NcclApi* nccl() {
+  static NcclApi api;
+  static bool tried = false;
+  if (tried) return api.lib ? &api : nullptr;
+  tried = true;
+  // the copy already in the process (torch loads its own) wins over the system's
+  void* lib = dlopen("libnccl.so.2", RTLD_NOW | RTLD_NOLOAD | RTLD_GLOBAL);
+  if (!lib) lib = dlopen("libnccl.so.2", RTLD_NOW | RTLD_GLOBAL);
+  if (!lib) lib = dlopen("libnccl.so", RTLD_NOW | RTLD_GLOBAL);
+  if (!lib) return nullptr;
+  bool ok = true;
+  auto sym = [&](const char* name) { void* f = dlsym(lib, name); if (!f) ok = false; return f; };
+  api.AllReduce = (decltype(api.AllReduce))sym("ncclAllReduce");
+  api.Broadcast = (decltype(api.Broadcast))sym("ncclBroadcast");
+  api.GroupStart = (decltype(api.GroupStart))sym("ncclGroupStart");
+  api.GroupEnd = (decltype(api.GroupEnd))sym("ncclGroupEnd");
+  api.GetErrorString = (decltype(api.GetErrorString))sym("ncclGetErrorString");
+  api.GetUniqueId = (decltype(api.GetUniqueId))sym("ncclGetUniqueId");
+  api.CommInitRank = (decltype(api.CommInitRank))sym("ncclCommInitRank");
+  api.CommDestroy = (decltype(api.CommDestroy))sym("ncclCommDestroy");
+  if (!ok) return nullptr;
+  api.lib = lib;
+  return &api;
+}
+
+#define NCCL_TRY(api, expr)                                                                       \
+  do {                                                                                            \
+    int _r = (expr);                                                                              \
+    if (_r != 0) return fail(SCAPE_ECUDA, "%s: %s", #expr, (api)->GetErrorString(_r));            \
+  } while (0)
+
+// Mask part of the exchange: every maximal run of consecutive layers with one owner becomes a word
+// range [first, end) that only this owner writes; a word that holds a boundary between two runs is
+// shared.  offsets == nullptr (no layers): one run, owner 0.
+void build_exchange_plan(scape* h, const int32_t* layer_owner) {
+  h->xr_first.clear(); h->xr_end.clear(); h->xr_owner.clear(); h->x_shared.clear();
+  const int64_t n_words = (h->N + 31) / 32;
+  if (h->n_layers == 0 || !layer_owner) {
+    h->xr_first.push_back(0); h->xr_end.push_back(n_words); h->xr_owner.push_back(0);
+    return;
+  }
+  int l = 0;
+  while (l < h->n_layers) {
+    int e = l + 1;
+    while (e < h->n_layers && layer_owner[e] == layer_owner[l]) ++e;
+    const int64_t a = h->lay_off[l], b = h->lay_off[e];
+    const int64_t w0 = (a + 31) / 32, w1 = b == h->N ? n_words : b / 32;
+    if (w1 > w0) { h->xr_first.push_back(w0); h->xr_end.push_back(w1); h->xr_owner.push_back(layer_owner[l]); }
+    if (a % 32 != 0 && (h->x_shared.empty() || h->x_shared.back() != a / 32)) h->x_shared.push_back(a / 32);
+    l = e;
+  }
 }
 
 // The streaming kernels are instantiated in scape_fused_inst.cu (one translation unit per gradient
@@ -484,6 +605,8 @@ void free_all(scape* h) {
   cudaFree(h->ghat); cudaFree(h->vm); cudaFree(h->sumsq); cudaFree(h->clip_state);
   cudaFree(h->layers); cudaFree(h->lctl); cudaFree(h->chunk_layer); cudaFree(h->lhist); cudaFree(h->items);
   cudaFree(h->st_param); cudaFree(h->iota_scratch);
+  cudaFree(h->x_shared_idx); cudaFree(h->x_shared_buf);
+  if (h->side) { cudaStreamDestroy(h->side); cudaEventDestroy(h->ev_main); cudaEventDestroy(h->ev_side); }
   for (auto& g : h->st_grad) cudaFree(g);
   if (h->prof_have_events)
     for (auto& row : h->prof_ev) for (auto& ev : row) cudaEventDestroy(ev);
@@ -789,11 +912,14 @@ int step_impl(scape_t* h, float* param, const void* const* grads, void* cuda_str
   DeviceGuard guard(h->dev);
   if (!guard.ok) return fail(SCAPE_ECUDA, "cannot select the handle's device");
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc;
+  if ((rc = join_side(h, st))) return rc;      // M_{t-1} (rank, index list, predicted bracket) may still be on its way
 
   MaskSlot& cur = h->slot[h->use];
   MaskSlot& nxt = h->slot[h->build];
   const bool need_select = h->k < h->N;
-  int rc;
+  // stage 2 on the handle's own stream, off the caller's: never inside a capture
+  const bool async = h->async_refresh && need_select && !local && !is_capturing(st);
   // an all-ones step reads and writes m densely
   if (cur.all_ones && h->m_sparse) {
     if ((rc = materialise_dense_m(h, st))) return rc;
@@ -847,18 +973,21 @@ int step_impl(scape_t* h, float* param, const void* const* grads, void* cuda_str
   }
   if (prof) CU_TRY(cudaEventRecord(h->prof_ev[pi][1], st));
 
+  cudaStream_t ss = st;                        // the stream stage 2 runs on
+  if (async) { if ((rc = fork_side(h, st))) return rc; ss = h->side; }
   if (need_select) {
     // workers: an all-ones step does not write M_t in the fused pass, and the select only writes
     // this worker's layers: the others' words must read zero for the exchange
-    if (local && cur.all_ones && h->n_layers > 0) CU_TRY(cudaMemsetAsync(nxt.bits, 0, sizeof(uint32_t) * h->n_words, st));
-    rc = h->n_layers > 0 ? run_select_layered(h, cur, nxt, /*force_general=*/cur.all_ones, st, /*compact=*/!local)
-                         : run_select(h, cur, nxt, /*force_general=*/cur.all_ones, st, /*compact=*/!local);
+    if (local && cur.all_ones && h->n_layers > 0) CU_TRY(cudaMemsetAsync(nxt.bits, 0, sizeof(uint32_t) * h->n_words, ss));
+    rc = h->n_layers > 0 ? run_select_layered(h, cur, nxt, /*force_general=*/cur.all_ones, ss, /*compact=*/!local)
+                         : run_select(h, cur, nxt, /*force_general=*/cur.all_ones, ss, /*compact=*/!local);
     if (rc) return rc;
-    if (cur.all_ones) CU_TRY(cudaMemsetAsync(h->e, 0, sizeof(float) * h->Npad, st));   // l.8 for e^0 after the stash
+    if (cur.all_ones) CU_TRY(cudaMemsetAsync(h->e, 0, sizeof(float) * h->Npad, ss));   // l.8 for e^0 after the stash
   } else if (!local) {
     nxt.all_ones = true; nxt.count = h->N; nxt.valid = true;                            // k = N: M_t = 1
   }
-  if (prof) { CU_TRY(cudaEventRecord(h->prof_ev[pi][2], st)); h->prof_pending = pi + 1; }
+  if (prof) { CU_TRY(cudaEventRecord(h->prof_ev[pi][2], ss)); h->prof_pending = pi + 1; }
+  if (async && (rc = mark_side(h))) return rc;
   if (local) {
     h->pending = true; h->pending_pm_out = pm_out; h->pending_bc1 = p.bc1; h->pending_bc2 = p.bc2; h->pending_lr = h->lr;
     h->pending_need_select = need_select;
@@ -918,6 +1047,18 @@ extern "C" int scape_set_workers(scape_t* h, int world, int rank, const int32_t*
     CU_TRY(cudaMemcpy(h->layers, ls.data(), sizeof(LayerState) * ls.size(), cudaMemcpyHostToDevice));
   }
   h->world = world; h->rank = rank;
+  build_exchange_plan(h, world > 1 ? layer_owner : nullptr);
+  cudaFree(h->x_shared_idx); cudaFree(h->x_shared_buf);
+  h->x_shared_idx = h->x_shared_buf = nullptr;
+  if (!h->x_shared.empty()) {
+    std::vector<uint32_t> w(h->x_shared.begin(), h->x_shared.end());
+    if (cudaMalloc((void**)&h->x_shared_idx, sizeof(uint32_t) * w.size()) != cudaSuccess ||
+        cudaMalloc((void**)&h->x_shared_buf, sizeof(uint32_t) * w.size()) != cudaSuccess) {
+      cudaGetLastError();
+      return fail(SCAPE_ENOMEM, "set_workers: allocation of the shared-word list failed");
+    }
+    CU_TRY(cudaMemcpy(h->x_shared_idx, w.data(), sizeof(uint32_t) * w.size(), cudaMemcpyHostToDevice));
+  }
   return SCAPE_OK;
 }
 
@@ -946,6 +1087,8 @@ extern "C" int scape_step_apply(scape_t* h, float* param, void* cuda_stream) {
   MaskSlot& cur = h->slot[h->use];
   MaskSlot& nxt = h->slot[h->build];
   const int pm_out = h->pending_pm_out;
+  if (h->pending_need_select && is_capturing(st) && h->pending_mask_on_side)
+    return fail(SCAPE_EINVAL, "a mask exchange on the handle's own stream cannot be part of a captured graph");
   const int64_t K = cur.all_ones ? h->N : cur.count;
   const int Rt = h->R * h->world;
   int g2 = (int)((K + 255) / 256); if (g2 > h->n_sm * 16) g2 = h->n_sm * 16; if (g2 < 1) g2 = 1;
@@ -955,8 +1098,12 @@ extern "C" int scape_step_apply(scape_t* h, float* param, void* cuda_stream) {
   h->launches++;
   CU_TRY(cudaGetLastError());
   if (h->pending_need_select) {
-    int rc = compact_mask(h, nxt, true, st);       // M_t is complete now: rank128 + the index list
+    // M_t is complete now: rank128 + the index list -- on the handle's own stream when the mask
+    // portions travelled there (scape_step_exchange with a mask_comm); the next step waits for it
+    cudaStream_t cs = h->pending_mask_on_side ? h->side : st;
+    int rc = compact_mask(h, nxt, true, cs);
     if (rc) return rc;
+    if (h->pending_mask_on_side) { if ((rc = mark_side(h))) return rc; h->pending_mask_on_side = false; }
     nxt.count = h->k; nxt.all_ones = false; nxt.valid = true;
   } else {
     nxt.all_ones = true; nxt.count = h->N; nxt.valid = true;
@@ -968,6 +1115,107 @@ extern "C" int scape_step_apply(scape_t* h, float* param, void* cuda_stream) {
   h->lr_last = h->pending_lr;
   h->t += 1;
   return SCAPE_OK;
+}
+
+// ---- the exchange inside the library ---------------------
+extern "C" int scape_step_exchange(scape_t* h, void* comm, void* mask_comm, void* cuda_stream) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (!h->pending) return fail(SCAPE_EINVAL, "no split step is in flight (call scape_step_local first)");
+  if (!comm) return fail(SCAPE_EINVAL, "NULL communicator");
+  if (h->pending_mask_on_side) return fail(SCAPE_EINVAL, "this split step has been exchanged already");
+  const NcclApi* nc = nccl();
+  if (!nc) return fail(SCAPE_ECUDA, "NCCL (libnccl.so.2) could not be loaded: %s", dlerror() ? dlerror() : "symbol missing");
+  DeviceGuard guard(h->dev);
+  if (!guard.ok) return fail(SCAPE_ECUDA, "cannot select the handle's device");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const MaskSlot& cur = h->slot[h->use];
+  const int64_t n_sums = cur.all_ones ? h->N : cur.count;
+  // l.10: the local sums of every selected entry become the sum over all workers
+  if (n_sums > 0) NCCL_TRY(nc, nc->AllReduce(h->ghat, h->ghat, (size_t)n_sums, kNcclFloat32, kNcclSum, comm, st));
+  if (!h->pending_need_select) return SCAPE_OK;
+  // M_t: only what each worker made travels, from its owner; on the handle's own stream when it has
+  // a communicator of its own (the one-step delay: nobody needs M_t before the next step's local half)
+  const bool on_side = mask_comm != nullptr && mask_comm != comm && !is_capturing(st);
+  cudaStream_t ms = st;
+  void* mc = mask_comm ? mask_comm : comm;
+  if (on_side) { int rc = fork_side(h, st); if (rc) return rc; ms = h->side; }
+  uint32_t* bits = h->slot[h->build].bits;
+  NCCL_TRY(nc, nc->GroupStart());
+  for (size_t i = 0; i < h->xr_first.size(); ++i) {
+    int r = nc->Broadcast(bits + h->xr_first[i], bits + h->xr_first[i], (size_t)(h->xr_end[i] - h->xr_first[i]), kNcclUint32,
+                          h->xr_owner[i], mc, ms);
+    if (r != 0) { nc->GroupEnd(); return fail(SCAPE_ECUDA, "ncclBroadcast: %s", nc->GetErrorString(r)); }
+  }
+  NCCL_TRY(nc, nc->GroupEnd());
+  const int ns = (int)h->x_shared.size();
+  if (ns > 0) {
+    gather_words_kernel<<<(ns + 255) / 256, 256, 0, ms>>>(bits, h->x_shared_idx, ns, h->x_shared_buf);
+    NCCL_TRY(nc, nc->AllReduce(h->x_shared_buf, h->x_shared_buf, (size_t)ns, kNcclUint32, kNcclSum, mc, ms));   // disjoint bits: SUM = OR
+    scatter_words_kernel<<<(ns + 255) / 256, 256, 0, ms>>>(bits, h->x_shared_idx, ns, h->x_shared_buf);
+    h->launches += 2;
+    CU_TRY(cudaGetLastError());
+  }
+  h->pending_mask_on_side = on_side;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_exchange_plan(const scape_t* h, int64_t* first, int64_t* end, int32_t* owner, int cap, int* n_ranges,
+                                   int64_t* shared, int cap_shared, int* n_shared) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  const int nr = (int)h->xr_first.size(), ns = (int)h->x_shared.size();
+  if (n_ranges) *n_ranges = nr;
+  if (n_shared) *n_shared = ns;
+  if ((first || end || owner) && cap < nr) return fail(SCAPE_EINVAL, "exchange_plan: %d ranges, capacity %d", nr, cap);
+  if (shared && cap_shared < ns) return fail(SCAPE_EINVAL, "exchange_plan: %d shared words, capacity %d", ns, cap_shared);
+  for (int i = 0; i < nr; ++i) {
+    if (first) first[i] = h->xr_first[i];
+    if (end) end[i] = h->xr_end[i];
+    if (owner) owner[i] = h->xr_owner[i];
+  }
+  for (int i = 0; i < ns && shared; ++i) shared[i] = h->x_shared[i];
+  return SCAPE_OK;
+}
+
+extern "C" int scape_nccl_unique_id(void* id) {
+  if (!id) return fail(SCAPE_EINVAL, "NULL id");
+  const NcclApi* nc = nccl();
+  if (!nc) return fail(SCAPE_ECUDA, "NCCL (libnccl.so.2) could not be loaded");
+  NCCL_TRY(nc, nc->GetUniqueId((NcclId*)id));
+  return SCAPE_OK;
+}
+
+extern "C" int scape_nccl_comm_create(int world, int rank, const void* id, void** comm) {
+  if (!id || !comm || world < 1 || rank < 0 || rank >= world) return fail(SCAPE_EINVAL, "bad argument");
+  const NcclApi* nc = nccl();
+  if (!nc) return fail(SCAPE_ECUDA, "NCCL (libnccl.so.2) could not be loaded");
+  NcclId uid;
+  std::memcpy(&uid, id, sizeof uid);
+  NCCL_TRY(nc, nc->CommInitRank(comm, world, uid, rank));
+  return SCAPE_OK;
+}
+
+extern "C" int scape_nccl_comm_destroy(void* comm) {
+  if (!comm) return SCAPE_OK;
+  const NcclApi* nc = nccl();
+  if (!nc) return fail(SCAPE_ECUDA, "NCCL (libnccl.so.2) could not be loaded");
+  NCCL_TRY(nc, nc->CommDestroy(comm));
+  return SCAPE_OK;
+}
+
+// ---- asynchronous refresh ------------------------------------------------
+extern "C" int scape_set_async_refresh(scape_t* h, int on) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  if (h->pending) return fail(SCAPE_EINVAL, "a split step is in flight");
+  DeviceGuard g(h->dev);
+  if (on) { int rc = ensure_side(h); if (rc) return rc; }
+  h->async_refresh = on != 0;
+  return SCAPE_OK;
+}
+
+extern "C" int scape_join_refresh(scape_t* h, void* cuda_stream) {
+  if (!h) return fail(SCAPE_EINVAL, "NULL handle");
+  DeviceGuard g(h->dev);
+  return join_side(h, (cudaStream_t)cuda_stream);
 }
 
 // ---- Algorithm 2, parameter side (Eq. 6 :207-211)  --  SURVEY.md §8(f) rank 4
@@ -987,6 +1235,7 @@ extern "C" int scape_param_pack(scape_t* h, const float* param, int64_t first, i
   DeviceGuard guard(h->dev);
   if (!guard.ok) return fail(SCAPE_ECUDA, "cannot select the handle's device");
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  { const int jr = join_side(h, st); if (jr) return jr; }     // a refresh on the handle's own stream comes first
   int64_t grid = (count + 1023) / 1024; if (grid > h->n_sm * 16) grid = h->n_sm * 16;
   const int32_t* idx = la.all_ones ? nullptr : la.idx;
   if (dtype == SCAPE_PARAM_BF16) param_pack_kernel<true><<<(int)grid, 256, 0, st>>>(param, idx, first, count, out);
@@ -1009,6 +1258,7 @@ extern "C" int scape_param_apply(scape_t* h, float* w, void* w_hat, const void* 
   DeviceGuard guard(h->dev);
   if (!guard.ok) return fail(SCAPE_ECUDA, "cannot select the handle's device");
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  { const int jr = join_side(h, st); if (jr) return jr; }     // a refresh on the handle's own stream comes first
   const int grid = grid_for(h, (h->n_chunks + kApplyChunks - 1) / kApplyChunks, 8, 4);
   const bool bf = dtype == SCAPE_PARAM_BF16, hat = w_hat != nullptr, ones = la.all_ones;
   const float wd = h->wd, neg_lr = -h->lr_last;
@@ -1052,6 +1302,7 @@ extern "C" int scape_mask_unpack(const uint32_t* words, int64_t n, uint8_t* mask
 extern "C" int scape_select_stats(scape_t* h, int64_t* fast, int64_t* general, void* cuda_stream) {
   if (!h) return fail(SCAPE_EINVAL, "NULL handle");
   DeviceGuard guard(h->dev);
+  { const int jr = join_side(h, (cudaStream_t)cuda_stream); if (jr) return jr; }     // a refresh on the handle's own stream comes first
   SelState s{};
   LayerCtl lc{};
   CU_TRY(cudaMemcpyAsync(&s, h->sel, sizeof s, cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
@@ -1065,6 +1316,7 @@ extern "C" int scape_select_stats(scape_t* h, int64_t* fast, int64_t* general, v
 extern "C" int scape_select_debug(scape_t* h, double* out8, void* cuda_stream) {
   if (!h || !out8) return fail(SCAPE_EINVAL, "NULL argument");
   DeviceGuard guard(h->dev);
+  { const int jr = join_side(h, (cudaStream_t)cuda_stream); if (jr) return jr; }     // a refresh on the handle's own stream comes first
   SelState s{};
   CU_TRY(cudaMemcpyAsync(&s, h->sel, sizeof s, cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
   CU_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
@@ -1169,6 +1421,7 @@ extern "C" int scape_get(scape_t* h, int what, int r, void* buf, size_t bytes, v
   if (!h || !buf) return fail(SCAPE_EINVAL, "NULL argument");
   DeviceGuard guard(h->dev);
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  { const int jr = join_side(h, st); if (jr) return jr; }     // a refresh on the handle's own stream comes first
   const size_t nbytes = sizeof(float) * (size_t)h->N;
   MaskSlot& nx = h->slot[h->use];
   MaskSlot& la = h->slot[h->last];
@@ -1230,6 +1483,7 @@ extern "C" int scape_set(scape_t* h, int what, int r, const void* buf, size_t by
   if (h->pending) return fail(SCAPE_EINVAL, "a split step is in flight: scape_step_apply first");
   DeviceGuard guard(h->dev);
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  { const int jr = join_side(h, st); if (jr) return jr; }     // a refresh on the handle's own stream comes first
   const size_t nbytes = sizeof(float) * (size_t)h->N;
   switch (what) {
     case SCAPE_MOMENT:

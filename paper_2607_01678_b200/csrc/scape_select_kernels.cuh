@@ -928,6 +928,16 @@ __global__ void __launch_bounds__(256) dist_update_kernel(float* __restrict__ th
   }
 }
 
+// workers: the mask words two owners share, collected for their all-reduce and put back (scape_step_exchange)
+__global__ void gather_words_kernel(const uint32_t* __restrict__ bits, const uint32_t* __restrict__ which, int n, uint32_t* __restrict__ out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = bits[which[i]];
+}
+__global__ void scatter_words_kernel(uint32_t* __restrict__ bits, const uint32_t* __restrict__ which, int n, const uint32_t* __restrict__ in) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) bits[which[i]] = in[i];
+}
+
 __global__ void fill_u32_kernel(uint32_t* p, int64_t n, uint32_t v) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) p[i] = v;
 }

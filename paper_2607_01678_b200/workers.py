@@ -39,3 +39,26 @@ def owned_word_ranges(offsets: Sequence[int], owner: Sequence[int], rank: int):
         else:
             out.append((a, b))
     return out
+
+
+def exchange_plan(offsets: Sequence[int], owner: Sequence[int], numel: int):
+    """What scape_step_exchange moves of the new mask (include/scape.h; the library computes the same
+    plan itself: scape_exchange_plan): every maximal run of consecutive layers with one owner is a range
+    of 32-bit mask words [first, end) that only this owner writes -> ([(first, end, owner)]); a word
+    that holds a boundary between two runs is shared -> ([word numbers]).  A pure function of the
+    layer offsets and owners: every worker derives the same plan."""
+    n_words = (int(numel) + 31) // 32
+    ranges, shared = [], []
+    l, n = 0, len(owner)
+    while l < n:
+        e = l + 1
+        while e < n and owner[e] == owner[l]:
+            e += 1
+        a, b = int(offsets[l]), int(offsets[e])
+        w0, w1 = (a + 31) // 32, n_words if b == int(numel) else b // 32
+        if w1 > w0:
+            ranges.append((w0, w1, int(owner[l])))
+        if a % 32 != 0 and (not shared or shared[-1] != a // 32):
+            shared.append(a // 32)
+        l = e
+    return ranges, shared

@@ -208,3 +208,169 @@ def test_step_workers_over_nccl_world_of_one(B, tmp_path):
         a.close(); b.close()
     finally:
         dist.destroy_process_group()
+
+
+# ---- the exchange inside the library (scape_step_exchange) and the asynchronous refresh ----------
+def test_exchange_plan_of_the_library_is_the_documented_one(B):
+    sizes = [37, 3, 88, 1000, 13, 4000 + 7, 64, 32, 5]
+    off = np.concatenate([[0], np.cumsum(sizes)]).tolist()
+    for W, owner in ((2, [0, 1, 0, 1, 0, 1, 1, 0, 0]), (3, [2, 2, 0, 0, 1, 2, 2, 2, 1]), (2, [0] * 9), (1, [0] * 9)):
+        h = B.Scape(off[-1], 1, 0.9, **HYP)
+        h.set_layers(off, [1] * len(sizes))
+        h.set_workers(W, 0, owner)
+        ranges, shared = h.exchange_plan()
+        want = workers.exchange_plan(off, owner, off[-1]) if W > 1 else ([(0, (off[-1] + 31) // 32, 0)], [])
+        assert (ranges, shared) == (want[0], want[1]), (W, owner, ranges, shared, want)
+        # every word is covered exactly once: by one range or as a shared word
+        cover = np.zeros((off[-1] + 31) // 32, dtype=np.int32)
+        for a, b, _ in ranges:
+            cover[a:b] += 1
+        cover[shared] += 1
+        assert (cover == 1).all(), (W, owner)
+        h.close()
+
+
+@pytest.mark.parametrize("two_comms", [False, True])
+def test_step_exchange_over_nccl_world_of_one(B, two_comms):
+    """scape_step_exchange really calls NCCL (all-reduce of the sums, grouped broadcasts of the word
+    ranges, all-reduce of the shared words); with a communicator of its own the mask part runs on the
+    handle's stream.  One rank: the pair must equal scape_step to the bit."""
+    sizes, comp = BIG
+    w = synth.Workload("workers/nccl1", [(f"t{i}", n) for i, n in enumerate(sizes)], R=4, sparsity=0.99,
+                       dist="t3", rho=0.9, grad_dtype="bf16", steps=8)
+    gs = synth.GradStream(w, device="cuda", seed=2)
+    th_a = gs.theta0(); th_b = th_a.clone()
+    a = B.Scape(w.numel, 4, 0.99, **w.hyper); a.set_layers(w.offsets(), comp)
+    b = B.Scape(w.numel, 4, 0.99, **w.hyper); b.set_layers(w.offsets(), comp); b.set_workers(1, 0, [0] * len(sizes))
+    comm = B.scape_nccl_comm_create(1, 0, B.scape_nccl_unique_id())
+    mcomm = B.scape_nccl_comm_create(1, 0, B.scape_nccl_unique_id()) if two_comms else None
+    try:
+        for t in range(8):
+            g = gs.next()
+            a.step(th_a, g)
+            b.step_workers(th_b, g, comm=comm, mask_comm=mcomm)
+            torch.cuda.synchronize()
+            assert torch.equal(th_a, th_b), t
+            np.testing.assert_array_equal(a.mask_next(), b.mask_next())
+            np.testing.assert_array_equal(a.idx_next(), b.idx_next())
+            assert np.array_equal(a.packed_mean().view(np.uint32), b.packed_mean().view(np.uint32))
+    finally:
+        a.close(); b.close()
+        B.scape_nccl_comm_destroy(comm)
+        if mcomm:
+            B.scape_nccl_comm_destroy(mcomm)
+
+
+_TWO_PROC = r'''
+import os, sys, numpy as np, torch, torch.distributed as dist
+sys.path.insert(0, os.environ["SCAPE_ROOT"]); sys.path.insert(0, os.path.join(os.environ["SCAPE_ROOT"], "tests"))
+from oracle.scape_oracle import ScapeOracle
+from paper_2607_01678_b200 import binding as B, synth, workers
+dist.init_process_group("gloo")
+rank, W = dist.get_rank(), dist.get_world_size()
+torch.cuda.set_device(0)
+sizes = [37, 3, 88, 1000, 13, 4000 + 7, 128 * 300 + 5, 64, 20011]
+comp = [1, 1, 1, 1, 0, 1, 1, 1, 1]
+Rl, s = 2, 0.9
+w = synth.Workload("workers/2proc", [(f"t{i}", n) for i, n in enumerate(sizes)], R=W * Rl, sparsity=s, dist="t3", rho=0.9,
+                   grad_dtype="f32", steps=8)
+owner = workers.balance_layers(sizes, W)
+gs = synth.GradStream(w, device="cuda", seed=3)            # same seed: every rank draws all W * Rl gradients, keeps its own
+th = gs.theta0(); th_ora = th.cpu().numpy().copy()
+ora = ScapeOracle(w.numel, W * Rl, s, **w.hyper); ora.set_layers(w.offsets(), comp); ora.set_workers(W, owner)
+h = B.Scape(w.numel, Rl, s, **w.hyper); h.set_layers(w.offsets(), comp); h.set_workers(W, rank, owner)
+for t in range(8):
+    g = gs.next()
+    h.step_workers(th, g[rank * Rl:(rank + 1) * Rl])          # torch.distributed path: plan-driven broadcasts over gloo
+    ora.step(th_ora, [x.to(torch.float32).cpu().numpy() for x in g])
+    torch.cuda.synchronize()
+    assert np.array_equal(h.mask_next(), ora.mask()), (rank, t, "mask")
+    assert np.array_equal(h.idx_last(), ora.idx()), (rank, t, "idx")
+    assert np.array_equal(th.cpu().numpy().view(np.uint32), th_ora.view(np.uint32)), (rank, t, "theta")
+    assert np.array_equal(h.packed_mean().view(np.uint32), ora.bbar().view(np.uint32)), (rank, t, "bbar")
+    for q in range(Rl):
+        assert np.array_equal(h.residual(q).view(np.uint32), ora.e(rank * Rl + q).view(np.uint32)), (rank, t, "e", q)
+h.close()
+dist.barrier()
+if rank == 0:
+    print("TWO_PROC_OK")
+dist.destroy_process_group()
+'''
+
+
+def test_two_processes_on_one_gpu_over_gloo(tmp_path):
+    """Two real processes, each with its own handle on cuda:0, exchanging through torch.distributed's
+    gloo backend on CUDA tensors (NCCL refuses two ranks on one device): the word ranges from their
+    owners, the shared words and the sums summed.  Every rank bit-exact against the oracle's workers
+    reading, 8 steps."""
+    import socket
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "two_proc.py"
+    script.write_text(_TWO_PROC)
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    env = dict(os.environ, SCAPE_ROOT=root)
+    res = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr",
+                          "127.0.0.1", "--master-port", str(port), str(script)], capture_output=True, text=True, env=env, timeout=600)
+    assert res.returncode == 0 and "TWO_PROC_OK" in res.stdout, res.stdout[-2000:] + res.stderr[-4000:]
+
+
+def _busy(x, n):
+    for _ in range(n):
+        x.mul_(1.0000001)
+
+
+@pytest.mark.parametrize("layered", [False, True])
+def test_async_refresh_is_the_same_step(B, layered):
+    """scape_set_async_refresh: stage 2 on the handle's own stream, the caller's stream free after the
+    streaming kernel (other work enqueued between the steps); every output bit-exact against the oracle
+    and against the in-stream form; accessors and the next step wait for the refresh by themselves."""
+    sizes, comp = BIG
+    w = synth.Workload("async", [(f"t{i}", n) for i, n in enumerate(sizes)], R=4, sparsity=0.99, dist="t3", rho=0.9,
+                       grad_dtype="bf16", steps=10)
+    gs = synth.GradStream(w, device="cuda", seed=7)
+    th_a = gs.theta0(); th_b = th_a.clone(); th_o = th_a.cpu().numpy().copy()
+    a = B.Scape(w.numel, 4, 0.99, **w.hyper)
+    b = B.Scape(w.numel, 4, 0.99, **w.hyper); b.set_async_refresh(True)
+    ora = ScapeOracle(w.numel, 4, 0.99, **w.hyper)
+    if layered:
+        for x in (a, b, ora):
+            x.set_layers(w.offsets(), comp)
+    other = torch.ones(1 << 24, device="cuda")
+    side = torch.cuda.Stream()
+    for t in range(10):
+        g = gs.next()
+        a.step(th_a, g)
+        if t % 2:                                   # alternate the caller's stream: the dependency follows the handle
+            with torch.cuda.stream(side):
+                side.wait_stream(torch.cuda.current_stream())
+                b.step(th_b, g)
+                _busy(other, 3)
+            torch.cuda.current_stream().wait_stream(side)
+        else:
+            b.step(th_b, g)
+            _busy(other, 3)                         # the caller's next work overlaps the refresh
+        ora.step(th_o, [to_np32(x) for x in g])
+        if t in (2, 5, 9):
+            np.testing.assert_array_equal(b.mask_next(), ora.mask())          # accessors join by themselves
+            np.testing.assert_array_equal(b.idx_next(), np.nonzero(ora.mask())[0].astype(np.int32))
+            torch.cuda.synchronize()
+            assert torch.equal(th_a, th_b), t
+            assert np.array_equal(th_b.cpu().numpy().view(np.uint32), th_o.view(np.uint32)), t
+    torch.cuda.synchronize()
+    assert b.last_kernel == "scape_fused_tma_kernel"
+    # a captured step runs the refresh in-stream; replaying one rotation period stays exact
+    b.join_refresh()
+    torch.cuda.synchronize()
+    ring = [gs.next() for _ in range(6)]
+    gr = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(gr):
+        for g in ring:
+            b.step(th_b, g)
+    for g in ring:
+        a.step(th_a, g)
+    gr.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(th_a, th_b)
+    a.close(); b.close()

@@ -110,6 +110,21 @@ cover = np.zeros(bits.size, bool)
 for a, b in rngs:
     cover[a:b] = True
 assert not bits[~cover].any()
+# the exchange the library performs (scape_step_exchange; Scape.step_workers over torch.distributed):
+# every word range broadcast from its owner, the shared words summed -- nothing else moves
+ranges, shared = workers.exchange_plan(offsets, owner, N)
+w2 = torch.from_numpy(bits.view(np.int32).copy())
+moved = 0
+for a, b, o in ranges:
+    dist.broadcast(w2[a:b], src=o)
+    moved += b - a
+if shared:
+    ix = torch.tensor(shared, dtype=torch.int64)
+    sw = w2[ix]
+    dist.all_reduce(sw, op=dist.ReduceOp.SUM)
+    w2[ix] = sw
+assert np.array_equal(np.unpackbits(w2.numpy().view(np.uint8), bitorder="little")[:N], full)
+assert moved + len(shared) == bits.size and len(shared) < len(sizes)       # every word exactly once
 sums = torch.full((5,), float(rank + 1))
 dist.all_reduce(sums, op=dist.ReduceOp.SUM)
 assert float(sums[0]) == sum(range(1, world + 1))
@@ -147,3 +162,8 @@ def test_balance_layers_is_even_and_deterministic():
     assert workers.owned_word_ranges([0, 40, 64, 100], [0, 1, 0], 0) == [(0, 4)]
     assert workers.owned_word_ranges([0, 40, 64, 100], [0, 1, 0], 1) == [(1, 2)]
     assert workers.owned_word_ranges([0, 64, 640, 700], [0, 1, 0], 0) == [(0, 2), (20, 22)]
+    # the plan of the exchange: runs of one owner become exclusive word ranges, boundary words are shared
+    assert workers.exchange_plan([0, 64, 640, 700], [0, 1, 0], 700) == ([(0, 2, 0), (2, 20, 1), (20, 22, 0)], [])
+    assert workers.exchange_plan([0, 37, 40, 128, 1128, 1141, 5148], [0, 1, 0, 1, 0, 1], 5148) == \
+        ([(0, 1, 0), (2, 4, 0), (4, 35, 1), (36, 161, 1)], [1, 35])
+    assert workers.exchange_plan([0, 10, 20], [1, 1], 20) == ([(0, 1, 1)], [])
