@@ -20,7 +20,7 @@
 namespace scapek {
 #define SCAPE_DECL_INST(tag)                                                               \
   const void* fused_step_kernel_##tag(int R, bool dense, bool msparse, bool clipt);        \
-  const void* fused_tma_kernel_##tag(int R, bool clipt, uint32_t* tile_bytes);
+  const void* fused_tma_kernel_##tag(int R, bool clipt, bool rkview, uint32_t* tile_bytes);
 SCAPE_DECL_INST(f32_lo)
 SCAPE_DECL_INST(f32_hi)
 SCAPE_DECL_INST(bf16_lo)
@@ -56,6 +56,8 @@ constexpr int kSinglePassCompactBlocks = 512;
 struct MaskSlot {
   uint32_t* bits = nullptr;   // [n_words]
   uint2* rank = nullptr;      // [n_chunks] {set bits before the chunk, running popcounts of its words}
+  uint32_t* pre = nullptr;    // [8 * n_tiles] the second half of `rank` on its own (zero past n_chunks)
+  uint32_t* trank = nullptr;  // [n_tiles + 1] set bits before every tile of 8 chunks; last entry: all of them
   int32_t* idx = nullptr;     // [k]   (not materialised while all_ones)
   int64_t count = 0;
   bool all_ones = false;
@@ -112,7 +114,7 @@ struct scape {
   // launch configuration of the streaming kernels for this handle's R on this handle's device
   // (prepare_kernels): [gradient type][variant][clip_grad instantiation]
   FusedCfg cfg_step[2][3][2];
-  FusedCfg cfg_tma[2][2];
+  FusedCfg cfg_tma[2][2][2];   // ... [table view: 0 pre + trank (flat top-k), 1 rk (per-layer refresh)]
   bool m_sparse = false;       // m_{t-1} lives in pm[pm_last] addressed through slot[last]; h->m is stale
   float* dense_pack = nullptr;    // optional [R][Npad]
   bool last_dense = false;
@@ -330,9 +332,9 @@ const void* step_kernel(int dtype, int R, bool dense, bool msparse, bool clipt) 
   return f;
 }
 
-const void* tma_kernel(int dtype, int R, bool clipt, uint32_t* tile) {
-  const void* f = dtype == SCAPE_GRAD_BF16 ? fused_tma_kernel_bf16_lo(R, clipt, tile) : fused_tma_kernel_f32_lo(R, clipt, tile);
-  if (!f) f = dtype == SCAPE_GRAD_BF16 ? fused_tma_kernel_bf16_hi(R, clipt, tile) : fused_tma_kernel_f32_hi(R, clipt, tile);
+const void* tma_kernel(int dtype, int R, bool clipt, bool rkview, uint32_t* tile) {
+  const void* f = dtype == SCAPE_GRAD_BF16 ? fused_tma_kernel_bf16_lo(R, clipt, rkview, tile) : fused_tma_kernel_f32_lo(R, clipt, rkview, tile);
+  if (!f) f = dtype == SCAPE_GRAD_BF16 ? fused_tma_kernel_bf16_hi(R, clipt, rkview, tile) : fused_tma_kernel_f32_hi(R, clipt, rkview, tile);
   return f;
 }
 
@@ -352,14 +354,16 @@ int prepare_kernels(scape* h) {
       }
       // Staged kernel: two CTAs (16 consumer warps) per SM with >= 3 stages each, or not at all
       // (tma_can_launch in scape_kernels.cuh); as many stages as fit, at most kTmaMaxStages.
-      FusedCfg& c = h->cfg_tma[dt][clipt];
-      c.fn = tma_kernel(dt, h->R, clipt != 0, &c.tile);
+      for (int view = 0; view < 2; ++view) {
+      FusedCfg& c = h->cfg_tma[dt][clipt][view];
+      c.fn = tma_kernel(dt, h->R, clipt != 0, view != 0, &c.tile);
       if (c.fn) {
         const int s2 = (int)((kSmemPerSm / 2u - 1024u - kTmaBarrierBytes) / c.tile);
         c.stages = s2 > kTmaMaxStages ? kTmaMaxStages : s2;
         c.bps = 2;
         c.smem = kTmaBarrierBytes + (size_t)c.stages * c.tile;
         CU_TRY(cudaFuncSetAttribute(c.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem));
+      }
       }
     }
   return SCAPE_OK;
@@ -382,7 +386,7 @@ int launch_fused(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t
   // with one or two replicas the step is issue-bound and the register-staged kernel's higher
   // occupancy (40 warps/SM vs 16 consumer warps) is worth more (measured at N = 2^28, 99 %:
   // R = 1: 1.49 vs 2.02 ms, R = 2: 1.95 vs 2.08 ms, R = 4: 2.94 vs 2.72 ms).
-  const FusedCfg& ct = h->cfg_tma[dt][clipt];
+  const FusedCfg& ct = h->cfg_tma[dt][clipt][h->n_layers > 0 ? 1 : 0];
   if (!dense && msparse && ct.fn && h->R >= 3 && p.N / kTmaTile >= (int64_t)h->n_sm) {
     const int64_t n_tiles = p.N / kTmaTile;
     int64_t grid = (int64_t)h->n_sm * ct.bps;
@@ -423,7 +427,7 @@ int compact_mask(scape* h, MaskSlot& s, bool want_idx, cudaStream_t st) {
   const int nb = h->n_compact_blocks;
   if (h->compact_impl == 1) {       // single pass (chained scan with look-back)
     h->compact_epoch = (h->compact_epoch + 1u) & 0x3FFFFFFFu;
-    mask_compact_kernel<<<nb, 1024, 0, st>>>(s.bits, h->n_chunks, h->scan_state, h->total, h->compact_epoch, s.rank,
+    mask_compact_kernel<<<nb, 1024, 0, st>>>(s.bits, h->n_chunks, h->scan_state, h->total, h->compact_epoch, s.rank, s.pre, s.trank,
                                             want_idx ? s.idx : nullptr, h->packed_stride);
     h->launches += 1;
     CU_TRY(cudaGetLastError());
@@ -431,7 +435,7 @@ int compact_mask(scape* h, MaskSlot& s, bool want_idx, cudaStream_t st) {
   }
   mask_block_count_kernel<<<nb, 1024, 0, st>>>(s.bits, h->n_chunks, h->block_sum);
   mask_scan_blocks_kernel<<<1, 1024, 0, st>>>(h->block_sum, nb, h->total);
-  mask_rank_idx_kernel<<<nb, 1024, 0, st>>>(s.bits, h->n_chunks, h->block_sum, s.rank, want_idx ? s.idx : nullptr,
+  mask_rank_idx_kernel<<<nb, 1024, 0, st>>>(s.bits, h->n_chunks, h->block_sum, s.rank, s.pre, s.trank, want_idx ? s.idx : nullptr,
                                             h->packed_stride);
   h->launches += 3;
   CU_TRY(cudaGetLastError());
@@ -599,7 +603,7 @@ bool finite_all(std::initializer_list<double> v) {
 
 void free_all(scape* h) {
   cudaFree(h->m); cudaFree(h->e);
-  for (auto& s : h->slot) { cudaFree(s.bits); cudaFree(s.rank); cudaFree(s.idx); }
+  for (auto& s : h->slot) { cudaFree(s.bits); cudaFree(s.rank); cudaFree(s.pre); cudaFree(s.trank); cudaFree(s.idx); }
   cudaFree(h->packed); cudaFree(h->pm[0]); cudaFree(h->pm[1]); cudaFree(h->dense_pack);
   cudaFree(h->sel); cudaFree(h->cand); cudaFree(h->cls); cudaFree(h->seg_count); cudaFree(h->seg_above); cudaFree(h->ghist); cudaFree(h->block_sum); cudaFree(h->total); cudaFree(h->scan_state);
   cudaFree(h->ghat); cudaFree(h->vm); cudaFree(h->sumsq); cudaFree(h->clip_state);
@@ -656,6 +660,8 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   for (auto& s : h->slot) {
     alloc((void**)&s.bits, sizeof(uint32_t) * h->n_words, true);
     alloc((void**)&s.rank, sizeof(uint2) * h->n_chunks, true);
+    alloc((void**)&s.pre, sizeof(uint32_t) * 8 * ((h->n_chunks + 7) / 8), true);
+    alloc((void**)&s.trank, sizeof(uint32_t) * ((h->n_chunks + 7) / 8 + 1), true);
   }
   alloc((void**)&h->sel, sizeof(SelState), true);
   alloc((void**)&h->seg_count, sizeof(uint32_t) * h->max_seg, true);
@@ -931,12 +937,12 @@ int step_impl(scape_t* h, float* param, const void* const* grads, void* cuda_str
   StepParams p{};
   p.theta = param; p.m = h->m; p.e = h->e; p.e_stride = h->Npad;
   for (int r = 0; r < h->R; ++r) p.g[r] = grads[r];
-  p.cur_bits = cur.bits; p.cur_rk = cur.rank;
+  p.cur_bits = cur.bits; p.cur_rk = cur.rank; p.cur_pre = cur.pre; p.cur_trank = cur.trank;
   p.packed = cur.all_ones ? h->dense_pack : h->packed;
   p.packed_stride = cur.all_ones ? h->Npad : h->packed_stride;
   p.packed_mean = h->pm[pm_out];
   if (msparse) {
-    p.prev_bits = h->slot[h->last].bits; p.prev_rk = h->slot[h->last].rank; p.pm_prev = h->pm[h->pm_last];
+    p.prev_bits = h->slot[h->last].bits; p.prev_rk = h->slot[h->last].rank; p.prev_pre = h->slot[h->last].pre; p.prev_trank = h->slot[h->last].trank; p.pm_prev = h->pm[h->pm_last];
   }
   p.N = h->N; p.n_chunks = h->n_chunks;
   p.b1 = h->b1; p.c1 = h->c1; p.b2 = h->b2; p.c2 = h->c2; p.eps = h->eps; p.wd = h->wd; p.neg_lr = -h->lr;

@@ -35,10 +35,11 @@ const void* step_ptr(bool dense, bool msparse, bool clipt) {
 }
 
 template <int R>
-const void* tma_ptr(bool clipt, uint32_t* tile_bytes) {
+const void* tma_ptr(bool clipt, bool rkview, uint32_t* tile_bytes) {
   if constexpr (tma_can_launch<InstG, R>()) {
     *tile_bytes = tma_tile_bytes<InstG, R>();
-    return clipt ? (const void*)scape_fused_tma_kernel<InstG, R, true> : (const void*)scape_fused_tma_kernel<InstG, R, false>;
+    if (rkview) return clipt ? (const void*)scape_fused_tma_kernel<InstG, R, true, true> : (const void*)scape_fused_tma_kernel<InstG, R, false, true>;
+    return clipt ? (const void*)scape_fused_tma_kernel<InstG, R, true, false> : (const void*)scape_fused_tma_kernel<InstG, R, false, false>;
   } else {
     *tile_bytes = 0;
     return nullptr;
@@ -52,9 +53,9 @@ const void* step_dispatch(int r, bool dense, bool msparse, bool clipt) {
 }
 
 template <int R>
-const void* tma_dispatch(int r, bool clipt, uint32_t* tile_bytes) {
+const void* tma_dispatch(int r, bool clipt, bool rkview, uint32_t* tile_bytes) {
   if constexpr (R > SCAPE_INST_RHI) { *tile_bytes = 0; return nullptr; }
-  else return r == R ? tma_ptr<R>(clipt, tile_bytes) : tma_dispatch<R + 1>(r, clipt, tile_bytes);
+  else return r == R ? tma_ptr<R>(clipt, rkview, tile_bytes) : tma_dispatch<R + 1>(r, clipt, rkview, tile_bytes);
 }
 
 }  // namespace
@@ -64,10 +65,10 @@ const void* SCAPE_CAT(fused_step_kernel_, SCAPE_INST_TAG)(int R, bool dense, boo
   return step_dispatch<SCAPE_INST_RLO>(R, dense, msparse, clipt);
 }
 
-// bulk-copy staged kernel <InstG, R, clipt> and the bytes of one of its stages; nullptr when the
+// bulk-copy staged kernel <InstG, R, clipt, rkview> and the bytes of one of its stages; nullptr when the
 // instantiation does not exist (R outside the range, or a tile that can never be resident twice per SM)
-const void* SCAPE_CAT(fused_tma_kernel_, SCAPE_INST_TAG)(int R, bool clipt, uint32_t* tile_bytes) {
-  return tma_dispatch<SCAPE_INST_RLO>(R, clipt, tile_bytes);
+const void* SCAPE_CAT(fused_tma_kernel_, SCAPE_INST_TAG)(int R, bool clipt, bool rkview, uint32_t* tile_bytes) {
+  return tma_dispatch<SCAPE_INST_RLO>(R, clipt, rkview, tile_bytes);
 }
 
 }  // namespace scapek

@@ -3,11 +3,21 @@
 // Data layout: the shard is cut into CHUNKS of 128 consecutive
 // parameters; one warp handles one chunk per loop trip, lane l owning elements 4l..4l+3
 // (one 128-bit access per fp32 array, one 64-bit access per bf16 array).  A mask is stored as
-// bits (word i/32, bit i%32 => one uint4 per chunk) plus `rk[c]` = {the number of set bits before
-// chunk c ("rank128"), the running popcounts of the chunk's four words, one byte each}, so the
-// packed position of a selected element is rank128 + words before + popc(bits before it inside
-// its word): the pack of Alg. 1 l.9 needs no atomics and keeps ascending index order, and a lane
-// finds its position from ONE word and ONE uint2 (no popcounts over the other words).
+// bits (word i/32, bit i%32 => one uint4 per chunk) plus position tables: `pre[c]`, the running
+// popcounts of chunk c's four words, one byte each (byte 3 = the chunk's total); the number of set
+// bits before the chunk ("rank128"); and `trank[T]`, the number of set bits before TILE T = chunks
+// 8T .. 8T+7 (the 8 chunks the warps of one CTA handle together).  The packed position of a selected
+// element is rank128 + words before + popc(bits before it inside its word): the pack of Alg. 1 l.9
+// needs no atomics and keeps ascending index order, and a lane finds its position from ONE word of
+// bits and the chunk's table entry (no popcounts over other words).  Two views of the tables exist:
+//   rk[c] = {rank128, pre}   8 bytes per chunk: one load, a handful of instructions; the register-
+//                            staged kernel (issue- and register-bound) and every other kernel use it
+//   pre[c] + trank[T]        4 bytes per chunk + 4 per tile; rank128 = trank + the totals of the
+//                            tile's earlier chunks (one shuffle, one warp-wide add).  The bulk-copy
+//                            staged kernel is HBM-bound and uses this one: rk was 3.5 M more 32-byte
+//                            sector reads per step on the headline shard and cost that kernel 0.2 ms
+//                            (1.5 % for 0.13 % of the bytes: small reads between the streams' bursts
+//                            are dear).
 //
 // Every fp32 operation of the method is written with a _rn intrinsic so that nvcc cannot
 // contract or reorder it; the order is the one pinned in DESIGN.md and followed by the oracle.
@@ -91,7 +101,9 @@ struct StepParams {
   int64_t e_stride;
   const void* g[kMaxR];         // R caller-owned gradient buffers
   const uint32_t* cur_bits;     // [Npad/32]   (unused when DENSE)
-  const uint2* cur_rk;          // [Npad/128] {rank128, word prefixes}: see chunk_prefix_bytes
+  const uint2* cur_rk;          // [Npad/128] {set bits before the chunk, its word prefixes}: register-staged kernel
+  const uint32_t* cur_pre;      // [8 * n_tiles] word prefixes of every chunk (see chunk_prefix_bytes): staged kernel
+  const uint32_t* cur_trank;    // [n_tiles + 1] set bits before every tile of 8 chunks (last entry: all of them)
   float* packed;                // [R][packed_stride] or nullptr (DENSE without keep_dense_pack)
   int64_t packed_stride;
   float* packed_mean;           // [k] b- of this step = m_t in packed form (unused when DENSE)
@@ -99,6 +111,8 @@ struct StepParams {
   // PAPER.md:197), so it lives as that step's packed mean, addressed through that mask
   const uint32_t* prev_bits;    // [Npad/32]
   const uint2* prev_rk;         // [Npad/128]
+  const uint32_t* prev_pre;     // [8 * n_tiles]
+  const uint32_t* prev_trank;   // [n_tiles + 1]
   const float* pm_prev;         // [k]
   int64_t N;
   int64_t n_chunks;             // ceil(N/128)
@@ -185,20 +199,15 @@ __device__ __forceinline__ void lane_bits_from_words(const uint4 mw, const uint3
 }
 __device__ __forceinline__ uint32_t chunk_popc(const uint4 mw) { return __popc(mw.x) + __popc(mw.y) + __popc(mw.z) + __popc(mw.w); }
 
-__device__ __forceinline__ void lane_mask_bits(const uint32_t* __restrict__ bits, const uint2* __restrict__ rk,
-                                               int64_t c, int lane, uint32_t& mybits, uint32_t& jbase) {
-  const uint4 mw = __ldg(reinterpret_cast<const uint4*>(bits) + c);
-  lane_bits_from_words(mw, __ldg(rk + c).x, lane, mybits, jbase);
-}
-
-// rk[c].y: running popcounts of the chunk's words, one byte each (byte 3 = the chunk's total, <= 128)
+// pre[c]: running popcounts of the chunk's words, one byte each (byte 3 = the chunk's total, <= 128)
 __host__ __device__ __forceinline__ uint32_t chunk_prefix_bytes(uint32_t p0, uint32_t p1, uint32_t p2, uint32_t p3) {
   return p0 | ((p0 + p1) << 8) | ((p0 + p1 + p2) << 16) | ((p0 + p1 + p2 + p3) << 24);
 }
 
 // Where a lane's 4 mask bits sit: word ws of the chunk, bits sh..sh+3.  Loop-invariant per lane, so the
-// streaming kernels decode a chunk's mask with one 32-bit load of the lane's OWN word, one uint2 load
-// of rk[c] (same address for the whole warp), a byte pick (PRMT), a shift, two ANDs and one POPC.
+// streaming kernels decode a chunk's mask with one 32-bit load of the lane's OWN word, the tile's 8
+// `pre` words (lane l loads word l % 8), trank (same address for the whole warp), one shuffle, one
+// warp-wide add, a byte pick (PRMT), a shift, two ANDs and one POPC.
 struct LaneMap { uint32_t ws, sh, lowmask, sel; };
 __device__ __forceinline__ LaneMap lane_map(int lane) {
   LaneMap lm;
@@ -210,6 +219,19 @@ __device__ __forceinline__ LaneMap lane_map(int lane) {
 __device__ __forceinline__ void lane_decode(uint32_t w, uint2 rk, const LaneMap& lm, uint32_t& mybits, uint32_t& jbase) {
   mybits = (w >> lm.sh) & 0xFu;
   jbase = rk.x + __byte_perm(rk.y, 0u, lm.sel) + __popc(w & lm.lowmask);
+}
+// {set bits before chunk `pos` of its tile, the chunk's own prefix word} from what the warp holds:
+// pa = pre[8T + lane % 8], tr = trank[T].  Whole warps only (one shuffle, one warp-wide add).
+__device__ __forceinline__ uint2 chunk_rank(uint32_t pa, uint32_t tr, uint32_t pos, int lane) {
+  const uint32_t mine = __shfl_sync(0xFFFFFFFFu, pa, (int)pos);
+  const uint32_t before = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)lane < pos ? pa >> 24 : 0u);
+  return make_uint2(tr + before, mine);
+}
+// a lane's 4 mask bits of chunk c and the packed position of the first of them
+__device__ __forceinline__ void lane_mask_bits(const uint32_t* __restrict__ bits, const uint2* __restrict__ rk,
+                                               int64_t c, int lane, uint32_t& mybits, uint32_t& jbase) {
+  const uint4 mw = __ldg(reinterpret_cast<const uint4*>(bits) + c);
+  lane_bits_from_words(mw, __ldg(rk + c).x, lane, mybits, jbase);
 }
 
 // Gather of m_{t-1} for this lane's 4 elements from the previous step's packed mean: selected
@@ -522,7 +544,7 @@ __device__ __forceinline__ void sparse_compute(const StepParams& p, uint32_t c, 
 }
 
 // A chunk's mask words as one lane needs them: its own word of the current (and, MSPARSE, the previous) mask + rk[c]
-struct MaskWords { uint32_t cw, pw; uint2 crk, prk; };
+struct MaskWords { uint32_t cw, pw; uint2 crk, prk; };        // own word of bits + rk[c]: current / previous mask
 template <bool CUR, bool PREV>
 __device__ __forceinline__ void load_mask_words(const StepParams& p, uint32_t c, const LaneMap& lm, MaskWords& w) {
   if (CUR) { w.cw = __ldg(p.cur_bits + (c << 2) + lm.ws); w.crk = __ldg(p.cur_rk + c); }
@@ -548,7 +570,6 @@ __device__ __forceinline__ void fused_chunk(const StepParams& p, uint32_t c, uin
   // mask words -- it is in flight together with the streaming loads instead of after them.
   if (!DENSE) load_mask_words<PF < 2, MSPARSE && PF < 1>(p, c, lm, mw);      // whatever was not fetched ahead
   const uint32_t cw = mw.cw, pw = mw.pw;
-  const uint2 crk = mw.crk, prk = mw.prk;
 
   float th[4], mo[4], gg[R][4], ee[R][4];
   load4_f32<GUARD>(p.theta, i0, p.N, th);
@@ -563,10 +584,11 @@ __device__ __forceinline__ void fused_chunk(const StepParams& p, uint32_t c, uin
     dense_compute<R, GUARD, CLIPT>(p, i0, th, mo, gg, ee, sa);
   } else {
     uint32_t mybits, jbase;
+    const uint2 crk = mw.crk;
     lane_decode(cw, crk, lm, mybits, jbase);
     if (MSPARSE) {
       uint32_t pbits, pbase;
-      lane_decode(pw, prk, lm, pbits, pbase);
+      lane_decode(pw, mw.prk, lm, pbits, pbase);
       gather_prev_m(p.pm_prev, pbits, pbase, mo);
     }
     if (PF > 0 && c_next != 0xFFFFFFFFu) load_mask_words<PF >= 2, MSPARSE && PF >= 1>(p, c_next, lm, mw);
@@ -696,18 +718,35 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, uint32
                ::"r"(smem_u32(dst_smem)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy) : "memory");
 }
 
-using TmaMaskWords = MaskWords;
+// own word of bits of the current / previous mask + their table entries: (c0, c1) / (p0, p1) = rk[c] when
+// RKVIEW, else {pre[8T + lane % 8], trank[T]}.  RKVIEW is the instantiation for per-layer refresh: evenly
+// spread masks make the consumer warps, not HBM, the bound there, and rk decodes in fewer instructions.
+struct TmaMaskWords { uint32_t cw, pw, c0, c1, p0, p1; };
 struct TmaTileState { uint32_t mybits, jbase, r0, cnt; float mo[4]; };
 
+template <bool RKVIEW>
 __device__ __forceinline__ void tma_load_words(const StepParams& p, uint32_t c, const LaneMap& lm, TmaMaskWords& w) {
-  load_mask_words<true, true>(p, c, lm, w);
+  w.cw = __ldg(p.cur_bits + (c << 2) + lm.ws);
+  w.pw = __ldg(p.prev_bits + (c << 2) + lm.ws);
+  if constexpr (RKVIEW) {
+    const uint2 a = __ldg(p.cur_rk + c), b = __ldg(p.prev_rk + c);
+    w.c0 = a.x; w.c1 = a.y; w.p0 = b.x; w.p1 = b.y;
+  } else {
+    const uint32_t pi = (c & ~7u) + (lm.sh >> 2);             // (lm.sh >> 2 = lane % 8)
+    w.c0 = __ldg(p.cur_pre + pi); w.c1 = __ldg(p.cur_trank + (c >> 3));
+    w.p0 = __ldg(p.prev_pre + pi); w.p1 = __ldg(p.prev_trank + (c >> 3));
+  }
 }
 // decode a chunk's mask words for this lane and start the gather of m_{t-1}
-__device__ __forceinline__ void tma_decode_gather(const StepParams& p, const TmaMaskWords& w, const LaneMap& lm, TmaTileState& st) {
+template <bool RKVIEW>
+__device__ __forceinline__ void tma_decode_gather(const StepParams& p, const TmaMaskWords& w, const LaneMap& lm, uint32_t pos, TmaTileState& st) {
   uint32_t pbits, pbase;
-  lane_decode(w.cw, w.crk, lm, st.mybits, st.jbase);
-  st.r0 = w.crk.x; st.cnt = w.crk.y >> 24;
-  lane_decode(w.pw, w.prk, lm, pbits, pbase);
+  const int lane = (int)(lm.ws * 8u + (lm.sh >> 2));
+  const uint2 crk = RKVIEW ? make_uint2(w.c0, w.c1) : chunk_rank(w.c0, w.c1, pos, lane);
+  const uint2 prk = RKVIEW ? make_uint2(w.p0, w.p1) : chunk_rank(w.p0, w.p1, pos, lane);
+  lane_decode(w.cw, crk, lm, st.mybits, st.jbase);
+  st.r0 = crk.x; st.cnt = crk.y >> 24;
+  lane_decode(w.pw, prk, lm, pbits, pbase);
   gather_prev_m(p.pm_prev, pbits, pbase, st.mo);
 }
 
@@ -720,7 +759,7 @@ __device__ __forceinline__ void bulk_s2g(void* dst, const void* src_smem, uint32
 // One tile of one consumer warp: start the next tile's gather of m, wait for this tile's bytes, pull
 // them out of shared memory, compute, write the results back into the stage; thread 0 then issues
 // the tile's bulk stores and releases the previous stage (protocol above).
-template <typename G, int R, bool CLIPT>
+template <typename G, int R, bool CLIPT, bool RKVIEW>
 __device__ __forceinline__ void tma_consume_tile(const StepParams& p, int64_t tile, int64_t n_tiles, int64_t tstride,
                                                  int warp, int lane, const LaneMap& lm, unsigned char* stage0, uint64_t* full, uint64_t* empty,
                                                  int& s, uint32_t& ph, int n_stages, TmaMaskWords& nw,
@@ -730,8 +769,8 @@ __device__ __forceinline__ void tma_consume_tile(const StepParams& p, int64_t ti
   const uint32_t c = (uint32_t)tile * kTmaConsumerWarps + warp;
   const uint32_t i0 = (c << 7) + ((uint32_t)lane << 2);
   if (tile + tstride < n_tiles) {
-    tma_decode_gather(p, nw, lm, nxt);
-    if (tile + 2 * tstride < n_tiles) tma_load_words(p, (uint32_t)(tile + 2 * tstride) * kTmaConsumerWarps + warp, lm, nw);
+    tma_decode_gather<RKVIEW>(p, nw, lm, (uint32_t)warp, nxt);
+    if (tile + 2 * tstride < n_tiles) tma_load_words<RKVIEW>(p, (uint32_t)(tile + 2 * tstride) * kTmaConsumerWarps + warp, lm, nw);
   }
   mbar_wait(&full[s], ph);
   const unsigned char* base = stage0 + (size_t)s * TILE;
@@ -785,7 +824,7 @@ __device__ __forceinline__ void tma_consume_tile(const StepParams& p, int64_t ti
   if (++s == n_stages) { s = 0; ph ^= 1u; }
 }
 
-template <typename G, int R, bool CLIPT>
+template <typename G, int R, bool CLIPT, bool RKVIEW>
 __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const __grid_constant__ StepParams p, int n_stages) {
   extern __shared__ __align__(128) unsigned char smem[];
   constexpr uint32_t TILE = tma_tile_bytes<G, R>();
@@ -808,14 +847,14 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
     // is ONE contiguous range per chunk (rank128 .. + the chunk's count); the streaming traffic since
     // the last step has pushed it out of L2, and the consumers' 4-byte gathers of it, issued one tile
     // ahead, were what they waited for (40 % of their stall samples: DRAM latency under load exceeds
-    // a tile's time).  Lane l: chunk l / 4 of the tile, 128-byte line l % 4 of its range.
+    // a tile's time).  A tile's range is contiguous (trank[T] .. trank[T+1]), at most 4 KB + alignment:
+    // lane l takes its 128-byte line l.
     auto prefetch_pm = [&](int64_t tile) {
       if (tile >= n_tiles) return;
-      const uint2 prk = __ldg(p.prev_rk + (tile * kTmaConsumerWarps + (lane >> 2)));
-      const uint32_t cntp = prk.y >> 24;
-      const char* a = reinterpret_cast<const char*>(p.pm_prev + prk.x);
-      const char* line = reinterpret_cast<const char*>((uintptr_t)a & ~(uintptr_t)127) + ((uint32_t)lane & 3u) * 128u;
-      if (cntp != 0u && line < a + cntp * 4u) asm volatile("prefetch.global.L2 [%0];" ::"l"(line));
+      const uint32_t j0 = __ldg(p.prev_trank + tile), j1 = __ldg(p.prev_trank + tile + 1);
+      const char* a = reinterpret_cast<const char*>(p.pm_prev + j0);
+      const char* line = reinterpret_cast<const char*>((uintptr_t)a & ~(uintptr_t)127) + (uint32_t)lane * 128u;
+      if (line < a + (size_t)(j1 - j0) * 4u) asm volatile("prefetch.global.L2 [%0];" ::"l"(line));
     };
     uint64_t policy;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
@@ -862,16 +901,16 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
   TmaTileState stA{}, stB{};
   if (tile < n_tiles) {
     TmaMaskWords w0;
-    tma_load_words(p, (uint32_t)tile * kTmaConsumerWarps + warp, lm, w0);
-    if (tile + tstride < n_tiles) tma_load_words(p, (uint32_t)(tile + tstride) * kTmaConsumerWarps + warp, lm, nw);
-    tma_decode_gather(p, w0, lm, stA);
+    tma_load_words<RKVIEW>(p, (uint32_t)tile * kTmaConsumerWarps + warp, lm, w0);
+    if (tile + tstride < n_tiles) tma_load_words<RKVIEW>(p, (uint32_t)(tile + tstride) * kTmaConsumerWarps + warp, lm, nw);
+    tma_decode_gather<RKVIEW>(p, w0, lm, (uint32_t)warp, stA);
   }
   int s = 0; uint32_t ph = 0;
   while (tile < n_tiles) {
-    tma_consume_tile<G, R, CLIPT>(p, tile, n_tiles, tstride, warp, lane, lm, stage0, full, empty, s, ph, n_stages, nw, stA, stB, sa);
+    tma_consume_tile<G, R, CLIPT, RKVIEW>(p, tile, n_tiles, tstride, warp, lane, lm, stage0, full, empty, s, ph, n_stages, nw, stA, stB, sa);
     tile += tstride;
     if (tile >= n_tiles) break;
-    tma_consume_tile<G, R, CLIPT>(p, tile, n_tiles, tstride, warp, lane, lm, stage0, full, empty, s, ph, n_stages, nw, stB, stA, sa);
+    tma_consume_tile<G, R, CLIPT, RKVIEW>(p, tile, n_tiles, tstride, warp, lane, lm, stage0, full, empty, s, ph, n_stages, nw, stB, stA, sa);
     tile += tstride;
   }
   if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // stores have landed

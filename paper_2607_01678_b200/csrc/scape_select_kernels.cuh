@@ -1,6 +1,6 @@
 // scape_select_kernels.cuh — the kernels of the SCAPE step that are not the streaming pass: the exact
 // top-k select of stage 2 (Alg. 1 l.11), the ordered compaction of a bit mask into
-// rk (rank128 + word prefixes) + the ascending index list (the int32 half of the sparse buffer, l.9), the deferred
+// the position tables (pre, trank) + the ascending index list (the int32 half of the sparse buffer, l.9), the deferred
 // updates (clip_grad l.14, workers l.10-17), the mask bit pack / unpack and the
 // Algorithm 2 parameter kernels.  Plain (non-template) kernels: this header is
 // included by scape.cu only.
@@ -772,7 +772,8 @@ __device__ __forceinline__ void write_chunk_indices(const uint4 w, const uint32_
 
 __global__ void __launch_bounds__(1024) mask_rank_idx_kernel(const uint32_t* __restrict__ bits, int64_t n_chunks,
                                                             const uint32_t* __restrict__ block_off,
-                                                            uint2* __restrict__ rk, int32_t* __restrict__ idx, int64_t idx_cap) {
+                                                            uint2* __restrict__ rk, uint32_t* __restrict__ pre, uint32_t* __restrict__ trank,
+                                                            int32_t* __restrict__ idx, int64_t idx_cap) {
   __shared__ uint32_t ws[32];
   const int64_t c = (int64_t)blockIdx.x * kCompactChunksPerBlock + threadIdx.x;
   uint4 w = make_uint4(0, 0, 0, 0);
@@ -792,7 +793,13 @@ __global__ void __launch_bounds__(1024) mask_rank_idx_kernel(const uint32_t* __r
   }
   __syncthreads();
   const uint32_t j = block_off[blockIdx.x] + ws[wid] + incl - n;
-  if (c < n_chunks) rk[c] = make_uint2(j, chunk_prefix_bytes(__popc(w.x), __popc(w.y), __popc(w.z), __popc(w.w)));
+  if (c < n_chunks) {
+    const uint32_t pb = chunk_prefix_bytes(__popc(w.x), __popc(w.y), __popc(w.z), __popc(w.w));
+    rk[c] = make_uint2(j, pb);
+    pre[c] = pb;
+    if ((c & 7) == 0) trank[c >> 3] = j;
+    if (c == n_chunks - 1) trank[(c >> 3) + 1] = j + n;      // the table's last entry: every set bit
+  }
   write_chunk_indices(w, n, j, c, idx, idx_cap);           // whole warps (past the end: w = 0, n = 0)
 }
 
@@ -806,7 +813,8 @@ __global__ void __launch_bounds__(1024) mask_rank_idx_kernel(const uint32_t* __r
 //   ctl[0] = total number of set bits (out), ctl[1] = ticket (returns to 0).
 __global__ void __launch_bounds__(1024) mask_compact_kernel(const uint32_t* __restrict__ bits, int64_t n_chunks,
                                                            unsigned long long* state, uint32_t* ctl, uint32_t epoch,
-                                                           uint2* __restrict__ rk, int32_t* __restrict__ idx, int64_t idx_cap) {
+                                                           uint2* __restrict__ rk, uint32_t* __restrict__ pre, uint32_t* __restrict__ trank,
+                                                           int32_t* __restrict__ idx, int64_t idx_cap) {
   __shared__ uint32_t ws[32];
   __shared__ uint32_t s_bid, s_prefix;
   if (threadIdx.x == 0) s_bid = atomicAdd(&ctl[1], 1u);
@@ -864,7 +872,13 @@ __global__ void __launch_bounds__(1024) mask_compact_kernel(const uint32_t* __re
   }
   __syncthreads();
   const uint32_t j = s_prefix + ws[wid] + incl - n;
-  if (c < n_chunks) rk[c] = make_uint2(j, chunk_prefix_bytes(__popc(w.x), __popc(w.y), __popc(w.z), __popc(w.w)));
+  if (c < n_chunks) {
+    const uint32_t pb = chunk_prefix_bytes(__popc(w.x), __popc(w.y), __popc(w.z), __popc(w.w));
+    rk[c] = make_uint2(j, pb);
+    pre[c] = pb;
+    if ((c & 7) == 0) trank[c >> 3] = j;
+    if (c == n_chunks - 1) trank[(c >> 3) + 1] = j + n;      // the table's last entry: every set bit
+  }
   write_chunk_indices(w, n, j, c, idx, idx_cap);           // whole warps (past the end: w = 0, n = 0)
 }
 
