@@ -372,17 +372,40 @@ constexpr int SCAPE_MAX_LAYERS_K = 4096;           // == SCAPE_MAX_LAYERS (inclu
 // Layer of element i by binary search over the layer ends held in shared memory (the candidate
 // lists are visited in an order that makes the chunk_layer table, N/32 bytes, a stream of L2
 // misses: one random 4-byte load per candidate; the ends are at most 32 KB and stay on chip).
-__device__ __forceinline__ void load_layer_ends(const LayerWork& w, long long* ends) {
-  for (int l = threadIdx.x; l < w.n_layers; l += blockDim.x) ends[l] = w.layers[l].end;
+// (layer ends fit 32 bits: shard_numel < 2^31.)  `lite`: what a candidate's digit needs of its layer's
+// state, for the first kLiteLayers layers, so that a candidate costs shared-memory reads only (the
+// LayerState in global memory was five dependent L2 loads per candidate).
+constexpr int kLiteLayers = 512;
+struct LayerLite { unsigned long long base, himask, prefix; int top; int hit; };
+__device__ __forceinline__ LayerLite layer_lite(const LayerState& S) {
+  LayerLite L; L.base = S.base; L.himask = S.himask; L.prefix = S.prefix; L.top = S.top; L.hit = S.hit;
+  return L;
+}
+__device__ __forceinline__ void load_layer_ends(const LayerWork& w, uint32_t* ends, LayerLite* lite) {
+  for (int l = threadIdx.x; l < w.n_layers; l += blockDim.x) {
+    ends[l] = (uint32_t)w.layers[l].end;
+    if (l < kLiteLayers) lite[l] = layer_lite(w.layers[l]);
+  }
   __syncthreads();
 }
-__device__ __forceinline__ uint32_t layer_of_sorted(const long long* ends, int n_layers, uint32_t i) {
+// hint: the layer of the previous candidate this thread saw (a segment is in ascending chunk order, so
+// the layer rarely changes: one or two comparisons instead of a 12-step search)
+__device__ __forceinline__ uint32_t layer_of_sorted(const uint32_t* ends, int n_layers, uint32_t i, uint32_t hint = 0) {
+  if (i < ends[hint] && (hint == 0u || i >= ends[hint - 1u])) return hint;
   int lo = 0, hi = n_layers - 1;                   // first l with ends[l] > i
   while (lo < hi) {
     const int mid = (lo + hi) >> 1;
-    if (ends[mid] > (long long)i) hi = mid; else lo = mid + 1;
+    if (ends[mid] > i) hi = mid; else lo = mid + 1;
   }
   return (uint32_t)lo;
+}
+__device__ __forceinline__ bool lite_digit(const LayerLite& S, unsigned long long k64, uint32_t& d) {
+  const int top = S.top;
+  const unsigned long long kr = k64 - S.base;
+  if (top <= 0 || (kr & S.himask) != S.prefix) return false;
+  const int bits = top < kDigitBits ? top : kDigitBits;
+  d = (uint32_t)(kr >> (top - bits)) & ((1u << bits) - 1u);
+  return true;
 }
 
 __device__ __forceinline__ uint32_t layer_of(const LayerWork& w, uint32_t i) {
@@ -466,34 +489,36 @@ __device__ __forceinline__ bool layer_digit(const LayerState& S, unsigned long l
   return true;
 }
 
-// Digit histograms of the layers on the candidate route.  The candidates of one layer fall into a
-// handful of bins in the first pass, so equal (layer, digit) pairs of a warp are merged before the
-// global atomic.
+// Digit histograms of the layers on the candidate route: one global atomic per candidate of a live
+// class (merging equal (layer, digit) pairs of a warp with __match_any_sync first cost more than the
+// atomics it saved: first pass 511 -> 437 us on the headline shard without it).
 __global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_constant__ LayerWork w, const __grid_constant__ CandList cl) {
-  __shared__ long long ends[SCAPE_MAX_LAYERS_K];
-  load_layer_ends(w, ends);
+  __shared__ uint32_t ends[SCAPE_MAX_LAYERS_K];
+  __shared__ LayerLite lite[kLiteLayers];
+  load_layer_ends(w, ends, lite);
   const int lane = threadIdx.x & 31;
   const int64_t wpb = blockDim.x >> 5;
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
   const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  uint32_t hint = 0;
   // small list (LayerCtl): nobody changes these two fields while this kernel runs, so every CTA
   // takes the same decision; lsel_hist_full_kernel's bookkeeping repeats it afterwards
   const bool use_cls = w.ctl->use_cls != 0;
   const unsigned long long ctot = w.ctl->cls_total;
   const bool collect = !use_cls && ctot > 0 && ctot <= (unsigned long long)kClsCap;
-  // one warp-wide step: 32 keys (ok = this lane has one), equal (layer, digit) pairs merged
+  // one warp-wide step: 32 keys (ok = this lane has one)
   auto visit32 = [&](bool ok, unsigned long long k64) {
     uint32_t tag = 0xFFFFFFFFu;
     if (ok) {
-      const uint32_t l = layer_of_sorted(ends, w.n_layers, 0xFFFFFFFFu - (uint32_t)k64);
+      const uint32_t l = hint = layer_of_sorted(ends, w.n_layers, 0xFFFFFFFFu - (uint32_t)k64, hint);
+      const LayerLite L = l < (uint32_t)kLiteLayers ? lite[l] : layer_lite(w.layers[l]);
       uint32_t d;
-      if (w.layers[l].hit && layer_digit(w.layers[l], k64, d)) {
+      if (L.hit && lite_digit(L, k64, d)) {
         tag = (l << kDigitBits) | d;
         if (collect) { const uint32_t pos = atomicAdd(&w.ctl->cls_n, 1u); if (pos < kClsCap) cl.cls[pos] = k64; }
       }
     }
-    const uint32_t same = __match_any_sync(0xFFFFFFFFu, tag);
-    if (tag != 0xFFFFFFFFu && (__ffs(same) - 1) == lane) atomicAdd(&w.hist[tag], (uint32_t)__popc(same));
+    if (tag != 0xFFFFFFFFu) atomicAdd(&w.hist[tag], 1u);
   };
   if (use_cls) {
     const uint32_t n = min(w.ctl->cls_n, kClsCap);
@@ -512,9 +537,12 @@ __global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_consta
     const uint32_t per = ((cnt + P - 1u) / P + 31u) & ~31u;
     const uint32_t b = part * per, e = min(cnt, b + per);
     const unsigned long long* seg = cl.cand + (size_t)sg * cl.seg_cap;
-    for (uint32_t j0 = b; j0 < e; j0 += 32) {
-      const uint32_t j = j0 + lane;
-      visit32(j < e, j < e ? __ldcs(seg + j) : 0ull);
+    for (uint32_t j0 = b; j0 < e; j0 += 128) {            // four independent loads per lane in flight
+      unsigned long long v[4]; bool ok[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { const uint32_t j = j0 + u * 32 + lane; ok[u] = j < e; v[u] = ok[u] ? __ldcs(seg + j) : 0ull; }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) if (j0 + u * 32 < e) visit32(ok[u], v[u]);
     }
   }
 }
@@ -661,12 +689,15 @@ __global__ void __launch_bounds__(256) lsel_finish_full_kernel(const __grid_cons
 // OR in the candidates at or above the layer's threshold.
 __global__ void __launch_bounds__(256) lsel_finish_cand_kernel(const __grid_constant__ LayerWork w, const __grid_constant__ CandList cl,
                                                               uint32_t* __restrict__ next_bits) {
-  __shared__ long long ends[SCAPE_MAX_LAYERS_K];
-  load_layer_ends(w, ends);
+  __shared__ uint32_t ends[SCAPE_MAX_LAYERS_K];
+  __shared__ LayerLite lite[kLiteLayers];
+  load_layer_ends(w, ends, lite);
+  uint32_t hint = 0;
   scan_segments(cl.cand, cl.seg_count, cl.seg_cap, cl.n_seg, ~0ull, [&](unsigned long long k64) {
     const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64;
-    const LayerState& S = w.layers[layer_of_sorted(ends, w.n_layers, i)];
-    if (S.hit && k64 >= S.prefix) atomicOr(&next_bits[i >> 5], 1u << (i & 31));
+    const uint32_t l = hint = layer_of_sorted(ends, w.n_layers, i, hint);
+    const bool sel = l < (uint32_t)kLiteLayers ? (lite[l].hit && k64 >= lite[l].prefix) : (w.layers[l].hit && k64 >= w.layers[l].prefix);
+    if (sel) atomicOr(&next_bits[i >> 5], 1u << (i & 31));
   });
 }
 
