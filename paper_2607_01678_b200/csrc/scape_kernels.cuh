@@ -678,7 +678,6 @@ constexpr int kTmaTile = kTmaConsumerWarps * kChunk;          // 1024 parameters
 constexpr int kTmaThreads = (kTmaConsumerWarps + 1) * 32;     // + 1 producer warp
 constexpr int kTmaMaxStages = 8;
 constexpr int kTmaBarrierBytes = 128;                         // full[8] + empty[8]
-constexpr int kTmaPrefetchAhead = 1;                          // tiles beyond the one being loaded whose m_{t-1} range the producer prefetches
 constexpr bool kTmaDirectPack = false;                        // b^r stored from the owning lanes (phase 1) instead of staged
 
 template <typename G, int R>
@@ -842,27 +841,17 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
   __syncthreads();
 
   if (warp == kTmaConsumerWarps) {
-    // ===== producer: one lane streams the tiles of this CTA; the whole warp first pulls the part of
-    // the previous packed mean (= m_{t-1}) that a coming tile's gather will read into L2.  That part
-    // is ONE contiguous range per chunk (rank128 .. + the chunk's count); the streaming traffic since
-    // the last step has pushed it out of L2, and the consumers' 4-byte gathers of it, issued one tile
-    // ahead, were what they waited for (40 % of their stall samples: DRAM latency under load exceeds
-    // a tile's time).  A tile's range is contiguous (trank[T] .. trank[T+1]), at most 4 KB + alignment:
-    // lane l takes its 128-byte line l.
-    auto prefetch_pm = [&](int64_t tile) {
-      if (tile >= n_tiles) return;
-      const uint32_t j0 = __ldg(p.prev_trank + tile), j1 = __ldg(p.prev_trank + tile + 1);
-      const char* a = reinterpret_cast<const char*>(p.pm_prev + j0);
-      const char* line = reinterpret_cast<const char*>((uintptr_t)a & ~(uintptr_t)127) + (uint32_t)lane * 128u;
-      if (line < a + (size_t)(j1 - j0) * 4u) asm volatile("prefetch.global.L2 [%0];" ::"l"(line));
-    };
-    uint64_t policy;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
-    for (int a = 0; a < kTmaPrefetchAhead; ++a) prefetch_pm((int64_t)blockIdx.x + (int64_t)a * gridDim.x);
-    int s = 0; uint32_t ph = 0;
-    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-      prefetch_pm(tile + (int64_t)kTmaPrefetchAhead * gridDim.x);
-      if (lane == 0) {
+    // ===== producer: one lane streams the tiles of this CTA =====
+    // (Tried: the idle lanes prefetching each coming tile's range of the previous packed mean into L2,
+    // so that the consumers' gather of m hits there.  The hit rate rose from 11 to 18 %, the kernel got
+    // SLOWER -- 13.75 vs 13.62 ms on the headline shard, 2.43 vs 2.39 ms at N = 2^28, R = 4 -- because
+    // whole-line prefetches are more small reads between the streams' bursts than the sectors the
+    // gather touches.  The consumers do wait for the gather, but only while the streams are the bound.)
+    if (lane == 0) {
+      uint64_t policy;
+      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+      int s = 0; uint32_t ph = 0;
+      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         mbar_wait(&empty[s], ph ^ 1u);                         // every consumer warp has read the old contents
         mbar_expect_tx(&full[s], TILE);
         unsigned char* base = stage0 + (size_t)s * TILE;
@@ -876,9 +865,8 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
           bulk_g2s(base + OFF_G + r * (kTmaTile * (uint32_t)sizeof(G)),
                    reinterpret_cast<const unsigned char*>(p.g[r]) + e0 * (int64_t)sizeof(G),
                    kTmaTile * (uint32_t)sizeof(G), &full[s], policy);
+        if (++s == n_stages) { s = 0; ph ^= 1u; }
       }
-      __syncwarp();
-      if (++s == n_stages) { s = 0; ph ^= 1u; }
     }
     return;
   }
