@@ -560,6 +560,34 @@ def main():
                                 "step_cost_async_ms": res[True] - busy_ms}
         del g_small, big, big2, small, small2
 
+    # ---- Algorithm 2's parameter side on the same shard: the owner packs
+    # theta on the mask the last step used, a non-owner applies it to its FP32 copy and refreshes the bf16 compute copy
+    alg2_line = None
+    if world == 1 and not args.workers and not args.no_also and k < N:
+        w_copy = theta.clone()
+        w_hat = torch.empty(N, dtype=torch.bfloat16, device=dev)
+        kk = sc.count_last()
+        pay = sc.param_pack(theta, dtype=torch.bfloat16)
+        sc.param_apply(w_copy, pay, w_hat)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        torch.cuda.synchronize()
+        reps = 5
+        ev[0].record()
+        for _ in range(reps):
+            sc.param_pack(theta, dtype=torch.bfloat16, out=pay)
+        ev[1].record()
+        for _ in range(reps):
+            sc.param_apply(w_copy, pay, w_hat)
+        ev[2].record()
+        torch.cuda.synchronize()
+        pack_ms, apply_ms = ev[0].elapsed_time(ev[1]) / reps, ev[1].elapsed_time(ev[2]) / reps
+        apply_bytes = N * (4 + 4 + 2 + 1 / 8 + 8 / 128) + 2 * kk          # w in / out, w^ out, bits + rk, bf16 payload
+        alg2_line = {"k": kk, "payload": "bf16", "param_pack_ms": pack_ms, "param_apply_ms": apply_ms,
+                     "param_apply_algorithmic_bytes": apply_bytes, "param_apply_gbs": apply_bytes / (apply_ms * 1e-3) / 1e9,
+                     "param_apply_frac_of_peak": apply_bytes / (apply_ms * 1e-3) / 1e9 / peak,
+                     "param_pack_entries_per_s": kk / (pack_ms * 1e-3)}
+        del w_copy, w_hat, pay
+
     sc.close()
     del sc
 
@@ -638,7 +666,7 @@ def main():
                        "refresh": "per layer (one top-k per tensor)" if (args.layers or args.workers) else "flat top-k over the shard",
                        "first_dense_step_ms": first_step_ms},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": gpu_launches, "clocks": clk,
-            "also_measured": also, "async_refresh": async_line,
+            "also_measured": also, "async_refresh": async_line, "alg2_param_side": alg2_line,
         }
         print(json.dumps(line), flush=True)
     if world > 1 or args.workers:
