@@ -358,10 +358,18 @@ int prepare_kernels(scape* h) {
       FusedCfg& c = h->cfg_tma[dt][clipt][view];
       c.fn = tma_kernel(dt, h->R, clipt != 0, view != 0, &c.tile);
       if (c.fn) {
-        const int s2 = (int)((kSmemPerSm / 2u - 1024u - kTmaBarrierBytes) / c.tile);
-        c.stages = s2 > kTmaMaxStages ? kTmaMaxStages : s2;
+        if (view == 0) {       // flat form: barriers + as many stages as fit
+          const int s2 = (int)((kSmemPerSm / 2u - 1024u - kTmaBarrierBytes) / c.tile);
+          c.stages = s2 > kTmaMaxStages ? kTmaMaxStages : s2;
+          c.smem = kTmaBarrierBytes + (size_t)c.stages * c.tile;
+        } else {               // grouped form: + two mask buffers (a group's mask words, by bulk copy); at most kTmaGroup
+                               // stages (the producer's reuse rule for the mask buffers needs n_stages <= kTmaGroup)
+          const uint32_t mb = tma_mb_bytes<true>();
+          const int s2 = (int)((kSmemPerSm / 2u - 1024u - kTmagBarrierBytes - 2u * mb) / c.tile);
+          c.stages = s2 > kTmaGroup ? kTmaGroup : s2;
+          c.smem = kTmagBarrierBytes + 2u * mb + (size_t)c.stages * c.tile;
+        }
         c.bps = 2;
-        c.smem = kTmaBarrierBytes + (size_t)c.stages * c.tile;
         CU_TRY(cudaFuncSetAttribute(c.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem));
       }
       }
@@ -386,11 +394,13 @@ int launch_fused(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t
   // with one or two replicas the step is issue-bound and the register-staged kernel's higher
   // occupancy (40 warps/SM vs 16 consumer warps) is worth more (measured at N = 2^28, 99 %:
   // R = 1: 1.49 vs 2.02 ms, R = 2: 1.95 vs 2.08 ms, R = 4: 2.94 vs 2.72 ms).
-  const FusedCfg& ct = h->cfg_tma[dt][clipt][h->n_layers > 0 ? 1 : 0];
+  const int view = h->n_layers > 0 ? 1 : 0;          // per-layer refresh: the grouped form (consumer-bound there)
+  const FusedCfg& ct = h->cfg_tma[dt][clipt][view];
   if (!dense && msparse && ct.fn && h->R >= 3 && p.N / kTmaTile >= (int64_t)h->n_sm) {
     const int64_t n_tiles = p.N / kTmaTile;
+    const int64_t n_units = view ? (n_tiles + kTmaGroup - 1) / kTmaGroup : n_tiles;   // grouped: a CTA takes groups of kTmaGroup consecutive tiles
     int64_t grid = (int64_t)h->n_sm * ct.bps;
-    if (grid > n_tiles) grid = n_tiles;
+    if (grid > n_units) grid = n_units;
     set_segments(h, p, (int)grid * kTmaConsumerWarps);
     int stages = ct.stages;
     void* args[] = {(void*)&p, (void*)&stages};
@@ -658,10 +668,13 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   alloc((void**)&h->m, sizeof(float) * h->Npad, true);                       // S5: m_0 = 0
   alloc((void**)&h->e, sizeof(float) * h->Npad * R, true);                   // l.2: e_0 = 0
   for (auto& s : h->slot) {
-    alloc((void**)&s.bits, sizeof(uint32_t) * h->n_words, true);
-    alloc((void**)&s.rank, sizeof(uint2) * h->n_chunks, true);
-    alloc((void**)&s.pre, sizeof(uint32_t) * 8 * ((h->n_chunks + 7) / 8), true);
-    alloc((void**)&s.trank, sizeof(uint32_t) * ((h->n_chunks + 7) / 8 + 1), true);
+    // (padded with zeros to whole groups of kTmaGroup tiles = 32 chunks: the staged kernel fetches a group's
+    // mask words and table entries with fixed-size bulk copies)
+    const size_t chunks_pad = (size_t)((h->n_chunks + 8 * kTmaGroup - 1) / (8 * kTmaGroup)) * (8 * kTmaGroup);
+    alloc((void**)&s.bits, sizeof(uint32_t) * 4 * chunks_pad, true);
+    alloc((void**)&s.rank, sizeof(uint2) * chunks_pad, true);
+    alloc((void**)&s.pre, sizeof(uint32_t) * chunks_pad, true);
+    alloc((void**)&s.trank, sizeof(uint32_t) * (chunks_pad / 8 + kTmaGroup), true);
   }
   alloc((void**)&h->sel, sizeof(SelState), true);
   alloc((void**)&h->seg_count, sizeof(uint32_t) * h->max_seg, true);

@@ -38,7 +38,8 @@ template <int R>
 const void* tma_ptr(bool clipt, bool rkview, uint32_t* tile_bytes) {
   if constexpr (tma_can_launch<InstG, R>()) {
     *tile_bytes = tma_tile_bytes<InstG, R>();
-    if (rkview) return clipt ? (const void*)scape_fused_tma_kernel<InstG, R, true, true> : (const void*)scape_fused_tma_kernel<InstG, R, false, true>;
+    // rkview: the grouped form with the rk tables (per-layer refresh); else the flat form with pre + trank
+    if (rkview) return clipt ? (const void*)scape_fused_tmag_kernel<InstG, R, true, true> : (const void*)scape_fused_tmag_kernel<InstG, R, false, true>;
     return clipt ? (const void*)scape_fused_tma_kernel<InstG, R, true, false> : (const void*)scape_fused_tma_kernel<InstG, R, false, false>;
   } else {
     *tile_bytes = 0;

@@ -677,7 +677,17 @@ constexpr int kTmaConsumerWarps = 8;
 constexpr int kTmaTile = kTmaConsumerWarps * kChunk;          // 1024 parameters
 constexpr int kTmaThreads = (kTmaConsumerWarps + 1) * 32;     // + 1 producer warp
 constexpr int kTmaMaxStages = 8;
-constexpr int kTmaBarrierBytes = 128;                         // full[8] + empty[8]
+constexpr int kTmaBarrierBytes = 128;                         // flat kernel: full[8] + empty[8]
+constexpr int kTmagBarrierBytes = 256;                        // grouped kernel: + mfull[2]
+// Mask words by bulk copy: a CTA takes GROUPS of kTmaGroup consecutive tiles, and the producer fetches a
+// group's mask words and table entries of both masks as six bulk copies (512-byte bursts of bits) into
+// one of two small shared-memory buffers, one group ahead.  The consumers no longer load mask words
+// from global memory at all: those loads were 5 single-sector DRAM reads per tile and mask between
+// the streams' 4 KB bursts (see "small reads" in DESIGN.md §5.1) and six registers of prefetch state.
+constexpr int kTmaGroup = 4;
+constexpr uint32_t kMbBits = kTmaGroup * 128u;                // bytes of one mask's bits for a group (32 words per tile)
+template <bool RKVIEW> __host__ __device__ constexpr uint32_t tma_mb_tab() { return kTmaGroup * (RKVIEW ? 64u : 32u); }   // rk: 8 x uint2, pre: 8 x u32 per tile
+template <bool RKVIEW> __host__ __device__ constexpr uint32_t tma_mb_bytes() { return 2u * kMbBits + 2u * tma_mb_tab<RKVIEW>() + (RKVIEW ? 0u : 2u * 16u); }
 constexpr bool kTmaDirectPack = false;                        // b^r stored from the owning lanes (phase 1) instead of staged
 
 template <typename G, int R>
@@ -690,7 +700,11 @@ constexpr uint32_t kSmemPerSm = 227u * 1024u;
 template <typename G, int R>
 __host__ __device__ constexpr int tma_stages_two_ctas() { return (int)((kSmemPerSm / 2u - 1024u - kTmaBarrierBytes) / tma_tile_bytes<G, R>()); }
 template <typename G, int R>
-__host__ __device__ constexpr bool tma_can_launch() { return tma_stages_two_ctas<G, R>() >= 3; }
+__host__ __device__ constexpr int tmag_stages_two_ctas() {
+  return (int)((kSmemPerSm / 2u - 1024u - kTmagBarrierBytes - 2u * tma_mb_bytes<true>()) / tma_tile_bytes<G, R>());
+}
+template <typename G, int R>
+__host__ __device__ constexpr bool tma_can_launch() { return tma_stages_two_ctas<G, R>() >= 3 && tmag_stages_two_ctas<G, R>() >= 3; }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
@@ -723,6 +737,25 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, uint32
 struct TmaMaskWords { uint32_t cw, pw, c0, c1, p0, p1; };
 struct TmaTileState { uint32_t mybits, jbase, r0, cnt; float mo[4]; };
 
+// this lane's mask words of chunk `warp` of tile t (0 .. kTmaGroup-1) of the group held in buffer mb
+template <bool RKVIEW>
+__device__ __forceinline__ void tma_read_words(const unsigned char* mb, int t, int warp, const LaneMap& lm, TmaMaskWords& w) {
+  const uint32_t* cb = reinterpret_cast<const uint32_t*>(mb);
+  const uint32_t* pb = reinterpret_cast<const uint32_t*>(mb + kMbBits);
+  w.cw = cb[t * 32 + warp * 4 + lm.ws];
+  w.pw = pb[t * 32 + warp * 4 + lm.ws];
+  const unsigned char* ct = mb + 2u * kMbBits;
+  const unsigned char* pt = ct + tma_mb_tab<RKVIEW>();
+  if constexpr (RKVIEW) {
+    const uint2 a = reinterpret_cast<const uint2*>(ct)[t * 8 + warp], b = reinterpret_cast<const uint2*>(pt)[t * 8 + warp];
+    w.c0 = a.x; w.c1 = a.y; w.p0 = b.x; w.p1 = b.y;
+  } else {
+    const uint32_t li = (uint32_t)t * 8u + (lm.sh >> 2);      // (lm.sh >> 2 = lane % 8)
+    const uint32_t* tr = reinterpret_cast<const uint32_t*>(pt + tma_mb_tab<RKVIEW>());
+    w.c0 = reinterpret_cast<const uint32_t*>(ct)[li]; w.c1 = tr[t];
+    w.p0 = reinterpret_cast<const uint32_t*>(pt)[li]; w.p1 = tr[4 + t];
+  }
+}
 template <bool RKVIEW>
 __device__ __forceinline__ void tma_load_words(const StepParams& p, uint32_t c, const LaneMap& lm, TmaMaskWords& w) {
   w.cw = __ldg(p.cur_bits + (c << 2) + lm.ws);
@@ -755,6 +788,227 @@ __device__ __forceinline__ void bulk_s2g(void* dst, const void* src_smem, uint32
                ::"l"(dst), "r"(smem_u32(src_smem)), "r"(bytes), "l"(policy) : "memory");
 }
 
+// The tiles of one CTA: groups g = blockIdx.x, + gridDim.x, ... of kTmaGroup consecutive tiles (the last group
+// of the shard may be short); j = ordinal of the group within this CTA (its mask buffer is j & 1).
+struct TmaPos { int64_t g; int t; int j; };
+__device__ __forceinline__ bool tma_pos_valid(const TmaPos& q, int64_t n_tiles) { return q.g * kTmaGroup + q.t < n_tiles; }
+__device__ __forceinline__ TmaPos tma_pos_next(const TmaPos& q, int64_t n_tiles) {
+  TmaPos n = q;
+  if (++n.t == kTmaGroup || n.g * kTmaGroup + n.t >= n_tiles) { n.t = 0; n.g += gridDim.x; n.j += 1; }
+  return n;
+}
+
+// One tile of one consumer warp: read the next tile's mask words from the group's buffer and start its
+// gather of m, wait for this tile's bytes, pull them out of shared memory, compute, write the results back
+// into the stage; thread 0 then issues the tile's bulk stores and releases the previous stage (protocol above).
+template <typename G, int R, bool CLIPT, bool RKVIEW>
+__device__ __forceinline__ void tmag_consume_tile(const StepParams& p, const TmaPos& pos, int64_t n_tiles, bool first,
+                                                 int warp, int lane, const LaneMap& lm, unsigned char* stage0, const unsigned char* mb0,
+                                                 uint64_t* full, uint64_t* empty, uint64_t* mfull,
+                                                 int& s, uint32_t& ph, int n_stages,
+                                                 TmaTileState& cur, TmaTileState& nxt, StageA& sa) {
+  constexpr uint32_t TILE = tma_tile_bytes<G, R>();
+  constexpr uint32_t OFF_E = kTmaTile * 4u, OFF_G = kTmaTile * 4u * (1u + R);
+  const int64_t tile = pos.g * kTmaGroup + pos.t;
+  const uint32_t c = (uint32_t)tile * kTmaConsumerWarps + warp;
+  const uint32_t i0 = (c << 7) + ((uint32_t)lane << 2);
+  {
+    const TmaPos nx = tma_pos_next(pos, n_tiles);
+    if (tma_pos_valid(nx, n_tiles)) {
+      if (nx.t == 0) mbar_wait(&mfull[nx.j & 1], (uint32_t)(nx.j >> 1) & 1u);      // the next group's mask words have landed
+      TmaMaskWords nw;
+      tma_read_words<RKVIEW>(mb0 + (size_t)(nx.j & 1) * tma_mb_bytes<RKVIEW>(), nx.t, warp, lm, nw);
+      tma_decode_gather<RKVIEW>(p, nw, lm, (uint32_t)warp, nxt);
+    }
+  }
+  mbar_wait(&full[s], ph);
+  const unsigned char* base = stage0 + (size_t)s * TILE;
+  const uint32_t off = (uint32_t)(warp * kChunk + (lane << 2));
+  float th[4], gg[R][4], ee[R][4];
+  {
+    const float4 t = *reinterpret_cast<const float4*>(base + off * 4u);
+    th[0] = t.x; th[1] = t.y; th[2] = t.z; th[3] = t.w;
+  }
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    const float4 t = *reinterpret_cast<const float4*>(base + OFF_E + r * (kTmaTile * 4u) + off * 4u);
+    ee[r][0] = t.x; ee[r][1] = t.y; ee[r][2] = t.z; ee[r][3] = t.w;
+    if constexpr (sizeof(G) == 4) {
+      const float4 g = *reinterpret_cast<const float4*>(base + OFF_G + r * (kTmaTile * 4u) + off * 4u);
+      gg[r][0] = g.x; gg[r][1] = g.y; gg[r][2] = g.z; gg[r][3] = g.w;
+    } else {
+      const uint2 g = *reinterpret_cast<const uint2*>(base + OFF_G + r * (kTmaTile * 2u) + off * 2u);
+      gg[r][0] = __uint_as_float(g.x << 16); gg[r][1] = __uint_as_float(g.x & 0xFFFF0000u);
+      gg[r][2] = __uint_as_float(g.y << 16); gg[r][3] = __uint_as_float(g.y & 0xFFFF0000u);
+    }
+  }
+  // Results go back into the stage (in place) and leave as whole-tile bulk stores: 4 KB bursts
+  // per stream instead of 512-byte warp stores.
+  // scratch of the on-mask arithmetic: this warp's own theta slice (m_old) and e^r slices (m~^r) of
+  // the stage (their contents are in registers now and are written back only after sparse_compute)
+  unsigned char* wbase = stage0 + (size_t)s * TILE;
+  __syncwarp();
+  sparse_compute<R, false, false, CLIPT, false, kTmaTile, kTmaDirectPack>(p, c, lane, lm, i0, cur.mybits, cur.jbase, cur.r0, cur.cnt,
+                                                          reinterpret_cast<float*>(wbase) + warp * kChunk,
+                                                          reinterpret_cast<float*>(wbase + OFF_E) + warp * kChunk, th, cur.mo, gg, ee, sa,
+                                                          CandRing{});
+  *reinterpret_cast<float4*>(wbase + off * 4u) = make_float4(th[0], th[1], th[2], th[3]);
+#pragma unroll
+  for (int r = 0; r < R; ++r)
+    *reinterpret_cast<float4*>(wbase + OFF_E + r * (kTmaTile * 4u) + off * 4u) = make_float4(ee[r][0], ee[r][1], ee[r][2], ee[r][3]);
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumerWarps * 32) : "memory");
+  if (threadIdx.x == 0) {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    const int64_t e0 = tile * kTmaTile;
+    bulk_s2g(p.theta + e0, wbase, kTmaTile * 4u, pol);
+#pragma unroll
+    for (int r = 0; r < R; ++r) bulk_s2g(p.e + r * p.e_stride + e0, wbase + OFF_E + r * (kTmaTile * 4u), kTmaTile * 4u, pol);
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    // the stores of the PREVIOUS tile have finished reading their stage: hand it back
+    asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+    if (!first) mbar_arrive(&empty[s == 0 ? n_stages - 1 : s - 1]);
+  }
+  if (++s == n_stages) { s = 0; ph ^= 1u; }
+}
+
+template <typename G, int R, bool CLIPT, bool RKVIEW>
+__global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tmag_kernel(const __grid_constant__ StepParams p, int n_stages) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  constexpr uint32_t TILE = tma_tile_bytes<G, R>();
+  constexpr uint32_t OFF_E = kTmaTile * 4u, OFF_G = kTmaTile * 4u * (1u + R);
+  constexpr uint32_t MB = tma_mb_bytes<RKVIEW>();
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem);
+  uint64_t* empty = full + kTmaMaxStages;
+  uint64_t* mfull = empty + kTmaMaxStages;                    // [2]: a group's mask words have landed
+  unsigned char* mb0 = smem + kTmagBarrierBytes;              // two mask buffers
+  unsigned char* stage0 = mb0 + 2u * MB;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t n_tiles = p.N / kTmaTile;                     // full tiles; the rest goes through the LDG path
+  const int64_t n_groups = (n_tiles + kTmaGroup - 1) / kTmaGroup;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < n_stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    mbar_init(&mfull[0], 1); mbar_init(&mfull[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (warp == kTmaConsumerWarps) {
+    // ===== producer: one lane streams the tiles of this CTA and, one group ahead, the groups' mask words =====
+    // (Tried: the idle lanes prefetching each coming tile's range of the previous packed mean into L2,
+    // so that the consumers' gather of m hits there.  The hit rate rose from 11 to 18 %, the kernel got
+    // SLOWER -- 13.75 vs 13.62 ms on the headline shard, 2.43 vs 2.39 ms at N = 2^28, R = 4 -- because
+    // whole-line prefetches are more small reads between the streams' bursts than the sectors the
+    // gather touches.  The consumers do wait for the gather, but only while the streams are the bound.)
+    if (lane == 0) {
+      uint64_t policy, keep;
+      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+      asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(keep));
+      // mask words of group g -> buffer j & 1 (the table arrays are padded to whole groups: scape.cu)
+      auto load_masks = [&](int64_t g, int j) {
+        unsigned char* mb = mb0 + (size_t)(j & 1) * MB;
+        uint64_t* bar = &mfull[j & 1];
+        mbar_expect_tx(bar, MB);
+        bulk_g2s(mb, p.cur_bits + g * (kMbBits / 4u), kMbBits, bar, keep);
+        bulk_g2s(mb + kMbBits, p.prev_bits + g * (kMbBits / 4u), kMbBits, bar, keep);
+        unsigned char* ct = mb + 2u * kMbBits;
+        if constexpr (RKVIEW) {
+          bulk_g2s(ct, p.cur_rk + g * (kTmaGroup * 8), tma_mb_tab<true>(), bar, keep);
+          bulk_g2s(ct + tma_mb_tab<true>(), p.prev_rk + g * (kTmaGroup * 8), tma_mb_tab<true>(), bar, keep);
+        } else {
+          bulk_g2s(ct, p.cur_pre + g * (kTmaGroup * 8), tma_mb_tab<false>(), bar, keep);
+          bulk_g2s(ct + tma_mb_tab<false>(), p.prev_pre + g * (kTmaGroup * 8), tma_mb_tab<false>(), bar, keep);
+          bulk_g2s(ct + 2u * tma_mb_tab<false>(), p.cur_trank + g * kTmaGroup, 16u, bar, keep);
+          bulk_g2s(ct + 2u * tma_mb_tab<false>() + 16u, p.prev_trank + g * kTmaGroup, 16u, bar, keep);
+        }
+      };
+      int s = 0; uint32_t ph = 0;
+      TmaPos q{(int64_t)blockIdx.x, 0, 0};
+      if (q.g < n_groups) load_masks(q.g, 0);
+      for (; tma_pos_valid(q, n_tiles); q = tma_pos_next(q, n_tiles)) {
+        mbar_wait(&empty[s], ph ^ 1u);                         // every consumer warp has read the old contents
+        // The buffer of group j + 1 is the one group j - 1 used: free once the LAST tile of j - 1 has been
+        // released, which the wait above implies from tile n_stages - 1 of group j on (n_stages <= kTmaGroup).
+        if (q.t == n_stages - 1 && q.g + gridDim.x < n_groups) load_masks(q.g + gridDim.x, q.j + 1);
+        mbar_expect_tx(&full[s], TILE);
+        unsigned char* base = stage0 + (size_t)s * TILE;
+        const int64_t e0 = (q.g * kTmaGroup + q.t) * kTmaTile;
+        bulk_g2s(base, p.theta + e0, kTmaTile * 4u, &full[s], policy);
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+          bulk_g2s(base + OFF_E + r * (kTmaTile * 4u), p.e + r * p.e_stride + e0, kTmaTile * 4u, &full[s], policy);
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+          bulk_g2s(base + OFF_G + r * (kTmaTile * (uint32_t)sizeof(G)),
+                   reinterpret_cast<const unsigned char*>(p.g[r]) + e0 * (int64_t)sizeof(G),
+                   kTmaTile * (uint32_t)sizeof(G), &full[s], policy);
+        if (++s == n_stages) { s = 0; ph ^= 1u; }
+      }
+    }
+    return;
+  }
+
+  // ===== consumers =====
+  const LaneMap lm = lane_map(lane);
+  const int64_t gwarp = (int64_t)blockIdx.x * kTmaConsumerWarps + warp;     // candidate segment of this warp
+  StageA sa{};
+  sa.layer = kNoLayer;
+  sa.lo = p.ctl->br.lo_key; sa.hi = p.ctl->br.hi_key;
+  sa.seg = p.cand + (size_t)gwarp * p.seg_cap;
+
+  // Software pipeline of the dependent accesses: the gather of m_{t-1} (whose addresses come from the
+  // previous mask's words) is issued one tile ahead; the mask words themselves arrive by bulk copy one
+  // group ahead.  The per-tile state ping-pongs between two register sets (A, B).
+  TmaPos q{(int64_t)blockIdx.x, 0, 0};
+  TmaTileState stA{}, stB{};
+  if (tma_pos_valid(q, n_tiles)) {
+    mbar_wait(&mfull[0], 0u);
+    TmaMaskWords w0;
+    tma_read_words<RKVIEW>(mb0, 0, warp, lm, w0);
+    tma_decode_gather<RKVIEW>(p, w0, lm, (uint32_t)warp, stA);
+  }
+  int s = 0; uint32_t ph = 0;
+  bool first = true;
+  while (tma_pos_valid(q, n_tiles)) {
+    tmag_consume_tile<G, R, CLIPT, RKVIEW>(p, q, n_tiles, first, warp, lane, lm, stage0, mb0, full, empty, mfull, s, ph, n_stages, stA, stB, sa);
+    first = false;
+    q = tma_pos_next(q, n_tiles);
+    if (!tma_pos_valid(q, n_tiles)) break;
+    tmag_consume_tile<G, R, CLIPT, RKVIEW>(p, q, n_tiles, first, warp, lane, lm, stage0, mb0, full, empty, mfull, s, ph, n_stages, stB, stA, sa);
+    q = tma_pos_next(q, n_tiles);
+  }
+  if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // stores have landed
+  asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumerWarps * 32) : "memory");          // ... and every consumer warp knows
+
+  // chunks past the last full tile (fewer than 8, the last one possibly ragged): LDG path
+  {
+    const uint32_t c = (uint32_t)n_tiles * kTmaConsumerWarps + warp;
+    if ((int64_t)c < p.n_chunks && blockIdx.x == (unsigned)(n_tiles % gridDim.x)) {
+      // (all bulk stores of this CTA have completed: the first stage serves as scratch)
+      float* sc = reinterpret_cast<float*>(stage0) + warp * ((R + 1) * kChunk);
+      MaskWords mw;
+      if (((int64_t)(c + 1) << 7) <= p.N) fused_chunk<G, R, false, true, false, CLIPT, false, 0>(p, c, 0xFFFFFFFFu, lane, lm, sc, sa, CandRing{}, mw);
+      else fused_chunk<G, R, false, true, true, CLIPT, false, 0>(p, c, 0xFFFFFFFFu, lane, lm, sc, sa, CandRing{}, mw);
+    }
+  }
+  if (p.chunk_layer != nullptr) warp_flush_layer(p, sa, lane);        // per-layer counts; seg_above stays 0
+  uint32_t na = sa.n_above;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
+  if (lane == 0) { p.seg_count[gwarp] = sa.cursor; p.seg_above[gwarp] = na; }
+  if (CLIPT && p.clip == 1) warp_store_sumsq(p, sa, gwarp, lane);
+}
+
+
+// ------------------------------------------------------------------------------------------
+// The flat-top-k form of the staged kernel: tiles blockIdx.x, + gridDim.x, ...; mask words loaded from global
+// memory two tiles ahead by the consumer warps; one more stage fits.  HBM-bound there (0.97 of the measured
+// peak), and measured ahead of the grouped form above on flat masks (13.67 vs 13.93 ms on the headline
+// shard), while the grouped form wins where the consumer warps are the bound (per-layer refresh: 13.97
+// vs 14.6 ms) -- see DESIGN.md §5.1.
+// ------------------------------------------------------------------------------------------
 // One tile of one consumer warp: start the next tile's gather of m, wait for this tile's bytes, pull
 // them out of shared memory, compute, write the results back into the stage; thread 0 then issues
 // the tile's bulk stores and releases the previous stage (protocol above).
