@@ -169,6 +169,15 @@ struct scape {
   bool side_used = false;         // ev_side has been recorded: the caller's stream must wait for it
   bool side_dirty = false;        // ... and no stream has waited for it since (a capture cannot wait: it needs this false)
 
+  // The flat select + compaction is 14-16 small dependent launches whose arguments only depend on the
+  // mask rotation (which slots), the route forced or not, k and the segment layout: each distinct
+  // sequence is captured once into a CUDA graph and replayed with one launch afterwards (shards under
+  // ~2^23 parameters are launch-bound: pr1 0.113 -> see DESIGN.md ms per step)
+  struct SelGraph { long long key[8]; cudaGraphExec_t exec; int launches; };
+  std::vector<SelGraph> sel_graphs;
+  cudaStream_t cap_stream = nullptr;
+  bool use_sel_graphs = true;
+
   bool pending = false;           // step_local has run, step_apply has not
   bool pending_need_select = false;
   int pending_pm_out = 0;
@@ -455,7 +464,7 @@ int compact_mask(scape* h, MaskSlot& s, bool want_idx, cudaStream_t st) {
 // Stage 2 (Alg. 1 l.11): exact top-k of |m~^0| -> nxt.bits / rank / idx.  When the fused pass ran
 // with a predicted bracket (sparse step) the radix select works on its candidate list if the
 // bracket held; otherwise (or on all-ones steps: force_general) on every key of the partition.
-int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st, bool compact = true) {
+int run_select_direct(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st, bool compact) {
   KeySrc src;
   src.e0 = h->e;
   src.cur_bits = cur.all_ones ? nullptr : cur.bits;
@@ -488,6 +497,56 @@ int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general,
   return SCAPE_OK;
 }
 
+void drop_sel_graphs(scape* h) {
+  for (auto& g : h->sel_graphs) cudaGraphExecDestroy(g.exec);
+  h->sel_graphs.clear();
+}
+
+// run_select_direct through a cached CUDA graph (see scape::SelGraph).  Falls back to the direct launches
+// inside a caller's capture, and whenever capturing or instantiating fails.
+int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st, bool compact = true) {
+  if (!h->use_sel_graphs || is_capturing(st)) return run_select_direct(h, cur, nxt, force_general, st, compact);
+  long long key[8] = {(long long)(&cur - h->slot), (long long)(&nxt - h->slot), (force_general ? 1 : 0) | (cur.all_ones ? 2 : 0), compact ? 1 : 0,
+                      (long long)h->n_seg, (long long)h->seg_cap, (long long)h->k, (long long)h->compact_impl};
+  for (auto& g : h->sel_graphs)
+    if (std::memcmp(g.key, key, sizeof key) == 0) {
+      CU_TRY(cudaGraphLaunch(g.exec, st));
+      h->launches += g.launches;
+      if (compact) { nxt.count = h->k; nxt.all_ones = false; nxt.valid = true; }
+      return SCAPE_OK;
+    }
+  if (!h->cap_stream && cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+    cudaGetLastError(); h->cap_stream = nullptr;
+    return run_select_direct(h, cur, nxt, force_general, st, compact);
+  }
+  if (h->sel_graphs.size() >= 24) drop_sel_graphs(h);          // (a density schedule changes k every step)
+  const int64_t l0 = h->launches;
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t exec = nullptr;
+  if (cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+    cudaGetLastError();
+    return run_select_direct(h, cur, nxt, force_general, st, compact);
+  }
+  const int rc = run_select_direct(h, cur, nxt, force_general, h->cap_stream, compact);
+  const cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
+  const int n_launch = (int)(h->launches - l0);
+  h->launches = l0;
+  if (rc != SCAPE_OK || ce != cudaSuccess || !graph || cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) {
+    cudaGetLastError();
+    if (graph) cudaGraphDestroy(graph);
+    h->use_sel_graphs = false;                                   // not available here: direct launches from now on
+    return run_select_direct(h, cur, nxt, force_general, st, compact);
+  }
+  cudaGraphDestroy(graph);
+  scape::SelGraph g;
+  std::memcpy(g.key, key, sizeof key);
+  g.exec = exec; g.launches = n_launch;
+  h->sel_graphs.push_back(g);
+  CU_TRY(cudaGraphLaunch(exec, st));
+  h->launches += n_launch;
+  return SCAPE_OK;
+}
+
 // Storage whose size follows the number of selected entries: index lists, packed b^r, the two
 // packed means, the candidate list.  Grows (never shrinks) so that masks of up to K entries fit;
 // live contents are kept.  Synchronises the device when it has to reallocate.  Masks with all N
@@ -497,6 +556,7 @@ int ensure_capacity(scape* h, int64_t K) {
   const int64_t stride = (K + 31) / 32 * 32;
   if (stride > h->packed_stride) {
     CU_TRY(cudaDeviceSynchronize());
+    drop_sel_graphs(h);                                          // the graphs hold the old buffers' addresses
     const int64_t old = h->packed_stride;
     auto grow = [&](void** p, size_t elem, int64_t rows) -> bool {
       void* q = nullptr;
@@ -531,6 +591,7 @@ int ensure_capacity(scape* h, int64_t K) {
       return fail(SCAPE_ENOMEM, "device allocation failed (small list of the select)");
     }
     if (cc > h->cand_cap) {
+      drop_sel_graphs(h);
       if (h->cand) { CU_TRY(cudaDeviceSynchronize()); cudaFree(h->cand); h->cand = nullptr; h->cand_cap = 0; }
       if (cudaMalloc((void**)&h->cand, sizeof(unsigned long long) * (size_t)cc) != cudaSuccess) {
         cudaGetLastError(); h->cand = nullptr;
@@ -621,6 +682,9 @@ void free_all(scape* h) {
   cudaFree(h->st_param); cudaFree(h->iota_scratch);
   cudaFree(h->x_shared_idx); cudaFree(h->x_shared_buf);
   if (h->side) { cudaStreamDestroy(h->side); cudaEventDestroy(h->ev_main); cudaEventDestroy(h->ev_side); }
+  for (auto& g : h->sel_graphs) cudaGraphExecDestroy(g.exec);
+  h->sel_graphs.clear();
+  if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   for (auto& g : h->st_grad) cudaFree(g);
   if (h->prof_have_events)
     for (auto& row : h->prof_ev) for (auto& ev : row) cudaEventDestroy(ev);
