@@ -162,3 +162,28 @@ def test_set_layers_api_errors(B):
     gpu.clear_layers()
     assert gpu.k == 100
     gpu.close()
+
+
+@pytest.mark.parametrize("n_tiles,extra", [(149, 77), (150, 0), (151, 1023), (296 * 4 + 2, 5)])
+def test_grouped_staged_kernel_short_last_group(B, n_tiles, extra):
+    """Per-layer refresh runs the grouped form of the staged kernel (groups of 4 tiles, mask words by bulk
+    copy): shards whose number of full tiles is not a multiple of 4, with and without a ragged tail, layer
+    boundaries inside tiles and chunks, an uncompressed layer; 7 chained steps against the oracle."""
+    N = n_tiles * 1024 + extra
+    sizes = [1024 * 37 + 5, 333, 1024 * 60 - 338]
+    sizes.append(N - sum(sizes))
+    w = synth.Workload(f"grouped/{n_tiles}+{extra}", [(f"t{i}", n) for i, n in enumerate(sizes)], R=4, sparsity=0.99,
+                       dist="t3", rho=0.9, grad_dtype="bf16", steps=7)
+    gs = synth.GradStream(w, device="cuda", seed=11)
+    th_gpu = gs.theta0()
+    th_ora = th_gpu.cpu().numpy().copy()
+    gpu, ora = make_pair(B, w, w.offsets(), [1, 0, 1, 1])
+    for t in range(1, 8):
+        grads = gs.next()
+        gpu.step(th_gpu, grads)
+        ora.step(th_ora, [to_np32(g) for g in grads])
+        torch.cuda.synchronize()
+        compare_step(gpu, ora, th_gpu, th_ora, 4, f"{w.name} step {t}")
+        if t >= 3:
+            assert gpu.last_kernel == "scape_fused_tma_kernel"
+    gpu.close()
