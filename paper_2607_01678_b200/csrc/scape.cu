@@ -6,6 +6,7 @@
 #include <dlfcn.h>
 
 #include <algorithm>
+#include <functional>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -194,7 +195,10 @@ struct scape {
 
   int32_t* iota_scratch = nullptr;   // scape_get(SCAPE_IDX_*) of an all-ones mask
 
-  // scape_step_host staging
+  // scape_step_host staging and pipeline (upload / download streams, one event pair per part)
+  static constexpr int kHostParts = 8;
+  cudaStream_t up = nullptr, down = nullptr;
+  cudaEvent_t ev_up[kHostParts] = {}, ev_cmp[kHostParts] = {}, ev_host = nullptr;
   float* st_param = nullptr;
   void* st_grad[kMaxR] = {};
   size_t st_grad_bytes = 0;
@@ -387,7 +391,8 @@ int prepare_kernels(scape* h) {
 }
 
 void set_segments(scape* h, StepParams& p, int n_seg) {
-  // one candidate segment per warp of this launch
+  // one candidate segment per warp of this step's launch(es)
+  if (n_seg > h->max_seg) n_seg = h->max_seg;
   h->n_seg = n_seg;
   h->n_slots = n_seg;
   int64_t cap = (h->cand_cap / h->n_seg) & ~(int64_t)15;
@@ -397,7 +402,13 @@ void set_segments(scape* h, StepParams& p, int n_seg) {
 }
 
 // variants: all-ones mask (dense m in and out) | sparse mask, dense m in | sparse mask, sparse m in
-int launch_fused(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t st) {
+// part / n_parts: the launch covers the part-th of n_parts ranges of the shard (scape_step_host's pipeline;
+// boundaries at whole tiles); every part uses its own block of candidate segments.  1 part = the whole shard.
+int launch_fused(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t st, int part = 0, int n_parts = 1) {
+  const int64_t tiles_all = (p.n_chunks + 7) / 8;
+  p.c_begin = (uint32_t)(8 * (tiles_all * part / n_parts));
+  p.c_end = part + 1 == n_parts ? (uint32_t)p.n_chunks : (uint32_t)(8 * (tiles_all * (part + 1) / n_parts));
+  const int64_t range_chunks = (int64_t)p.c_end - (int64_t)p.c_begin;
   const int dt = h->grad_dtype == SCAPE_GRAD_BF16 ? 1 : 0, clipt = p.clip ? 1 : 0;   // the clip_grad variant is its own instantiation
   // The staged kernel wins when there are enough bytes per parameter to be HBM-bound (R >= 3);
   // with one or two replicas the step is issue-bound and the register-staged kernel's higher
@@ -405,12 +416,14 @@ int launch_fused(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t
   // R = 1: 1.49 vs 2.02 ms, R = 2: 1.95 vs 2.08 ms, R = 4: 2.94 vs 2.72 ms).
   const int view = h->n_layers > 0 ? 1 : 0;          // per-layer refresh: the grouped form (consumer-bound there)
   const FusedCfg& ct = h->cfg_tma[dt][clipt][view];
-  if (!dense && msparse && ct.fn && h->R >= 3 && p.N / kTmaTile >= (int64_t)h->n_sm) {
-    const int64_t n_tiles = p.N / kTmaTile;
+  if (!dense && msparse && ct.fn && h->R >= 3 && p.N / kTmaTile >= (int64_t)h->n_sm * n_parts && (view == 0 || n_parts == 1)) {
+    const int64_t n_tiles = n_parts == 1 ? p.N / kTmaTile : std::min<int64_t>(p.N / kTmaTile, p.c_end / 8) - p.c_begin / 8;
     const int64_t n_units = view ? (n_tiles + kTmaGroup - 1) / kTmaGroup : n_tiles;   // grouped: a CTA takes groups of kTmaGroup consecutive tiles
     int64_t grid = (int64_t)h->n_sm * ct.bps;
     if (grid > n_units) grid = n_units;
-    set_segments(h, p, (int)grid * kTmaConsumerWarps);
+    if (part == 0) set_segments(h, p, (n_parts == 1 ? (int)grid : h->n_sm * ct.bps) * kTmaConsumerWarps * n_parts);
+    p.seg_cap = h->seg_cap;
+    p.seg_base = (uint32_t)(part * h->n_sm * ct.bps * kTmaConsumerWarps);
     int stages = ct.stages;
     void* args[] = {(void*)&p, (void*)&stages};
     CU_TRY(cudaLaunchKernel(ct.fn, dim3((unsigned)grid), dim3(kTmaThreads), args, ct.smem, st));
@@ -419,8 +432,10 @@ int launch_fused(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t
     return SCAPE_OK;
   }
   const FusedCfg& c = h->cfg_step[dt][dense ? 0 : msparse ? 2 : 1][clipt];
-  const int grid = grid_for(h, p.n_chunks, 8, c.bps);
-  set_segments(h, p, grid * 8);
+  const int grid = grid_for(h, range_chunks, 8, c.bps);
+  if (part == 0) set_segments(h, p, (n_parts == 1 ? grid : h->n_sm * c.bps) * 8 * n_parts);
+  p.seg_cap = h->seg_cap;
+  p.seg_base = (uint32_t)(part * h->n_sm * c.bps * 8);
   void* args[] = {(void*)&p};
   CU_TRY(cudaLaunchKernel(c.fn, dim3((unsigned)grid), dim3(256), args, c.smem, st));
   h->last_kernel = "scape_fused_step_kernel";
@@ -685,6 +700,11 @@ void free_all(scape* h) {
   for (auto& g : h->sel_graphs) cudaGraphExecDestroy(g.exec);
   h->sel_graphs.clear();
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+  if (h->up) {
+    cudaStreamDestroy(h->up); cudaStreamDestroy(h->down); cudaEventDestroy(h->ev_host);
+    for (auto& e : h->ev_up) cudaEventDestroy(e);
+    for (auto& e : h->ev_cmp) cudaEventDestroy(e);
+  }
   for (auto& g : h->st_grad) cudaFree(g);
   if (h->prof_have_events)
     for (auto& row : h->prof_ev) for (auto& ev : row) cudaEventDestroy(ev);
@@ -721,7 +741,7 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   h->beta1_d = beta1; h->beta2_d = beta2;
   h->n_compact_blocks = (int)((h->n_chunks + kCompactChunksPerBlock - 1) / kCompactChunksPerBlock);
   h->sparsity = sparsity;
-  h->max_seg = h->n_sm * 8 * 8;
+  h->max_seg = h->n_sm * 8 * 8 * 8;          // 8 CTAs x 8 warps per SM, times the parts of scape_step_host's pipeline
 
   bool ok = true;
   auto alloc = [&](void** p, size_t bytes, bool zero) {
@@ -976,11 +996,26 @@ extern "C" int scape_set_step_count(scape_t* h, int64_t t) {
 
 namespace {
 
+// Elements [first, end) of part i of n: the same boundaries launch_fused uses (whole tiles of 1024).
+void part_range(const scape* h, int i, int n, int64_t* first, int64_t* end) {
+  const int64_t tiles_all = (h->n_chunks + 7) / 8;
+  *first = 1024 * (tiles_all * i / n);
+  *end = i + 1 == n ? h->N : std::min<int64_t>(h->N, 1024 * (tiles_all * (i + 1) / n));
+}
+
+// scape_step_host's pipeline: the streaming kernel runs part by part, `before(i, n)` / `after(i, n)` around
+// each launch (upload / download of that part); n = 1 when the step cannot be split (all-ones mask, dense m,
+// layers, clip_grad, a shard of too few tiles).
+struct PartHooks {
+  int n_parts;
+  std::function<int(int, int)> before, after;
+};
+
 // The step.  local = false: all of it (scape_step).  local = true (scape_step_local): everything
 // that needs no other worker -- l.6-9 for the local replicas, the local sums of l.10 parked for the
 // all-reduce, theta off the mask, this worker's share of the refresh (l.11) -- and the rest is left
 // to scape_step_apply.
-int step_impl(scape_t* h, float* param, const void* const* grads, void* cuda_stream, bool local) {
+int step_impl(scape_t* h, float* param, const void* const* grads, void* cuda_stream, bool local, const PartHooks* hooks = nullptr) {
   if (!h) return fail(SCAPE_EINVAL, "NULL handle");
   if (h->pending) return fail(SCAPE_EINVAL, "scape_step_local has run: call scape_step_apply first");
   if (!local && h->world > 1) return fail(SCAPE_EINVAL, "this handle is one of %d workers: use scape_step_local / scape_step_apply", h->world);
@@ -1042,8 +1077,22 @@ int step_impl(scape_t* h, float* param, const void* const* grads, void* cuda_str
   if (prof && h->prof_pending == scape::kProfRing) { int prc = prof_drain(h); if (prc) return prc; }
   const int pi = h->prof_pending;
   if (prof) CU_TRY(cudaEventRecord(h->prof_ev[pi][0], st));
-  rc = launch_fused(h, p, cur.all_ones, msparse, st);
-  if (rc) return rc;
+  if (hooks) {
+    int n = hooks->n_parts;
+    if (cur.all_ones || !msparse || h->n_layers > 0 || p.clip || p.N / kTmaTile < (int64_t)h->n_sm * 2 * n) n = 1;
+    if (n > 1) {                 // parts with fewer CTAs than the full grid leave segments untouched: their counts must read 0
+      CU_TRY(cudaMemsetAsync(h->seg_count, 0, sizeof(uint32_t) * h->max_seg, st));
+      CU_TRY(cudaMemsetAsync(h->seg_above, 0, sizeof(uint32_t) * h->max_seg, st));
+    }
+    for (int i = 0; i < n; ++i) {
+      if ((rc = hooks->before(i, n))) return rc;
+      if ((rc = launch_fused(h, p, cur.all_ones, msparse, st, i, n))) return rc;
+      if ((rc = hooks->after(i, n))) return rc;
+    }
+  } else {
+    rc = launch_fused(h, p, cur.all_ones, msparse, st);
+    if (rc) return rc;
+  }
   if (clip) {
     // l.14-17 on the mask: norm of g^ (fixed-order reduction), then the deferred update
     const int64_t K = cur.count;
@@ -1450,14 +1499,48 @@ extern "C" int scape_step_host(scape_t* h, float* param_host, const void* const*
     }
     h->st_grad_bytes = gb;
   }
-  for (int r = 0; r < h->R; ++r) {
+  for (int r = 0; r < h->R; ++r)
     if (!grads_host[r]) return fail(SCAPE_EINVAL, "grads[%d] is NULL", r);
-    CU_TRY(cudaMemcpyAsync(h->st_grad[r], grads_host[r], gb, cudaMemcpyHostToDevice, st));
+  // Upload, step and download are pipelined part by part: PCIe is full duplex and the streaming kernel is
+  // 2.5 % of the copies' time, so theta of part i travels back while the gradients of part i + 1 travel up.
+  // Two streams of the handle's own carry the copies; events order them against the kernel launches on st.
+  if (!h->up) {
+    CU_TRY(cudaStreamCreateWithFlags(&h->up, cudaStreamNonBlocking));
+    CU_TRY(cudaStreamCreateWithFlags(&h->down, cudaStreamNonBlocking));
+    for (auto& e : h->ev_up) CU_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    for (auto& e : h->ev_cmp) CU_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    CU_TRY(cudaEventCreateWithFlags(&h->ev_host, cudaEventDisableTiming));
   }
-  CU_TRY(cudaMemcpyAsync(h->st_param, param_host, sizeof(float) * h->N, cudaMemcpyHostToDevice, st));
-  int rc = scape_step(h, h->st_param, (const void* const*)h->st_grad, cuda_stream);
+  const size_t ge = h->grad_dtype == SCAPE_GRAD_BF16 ? 2 : 4;
+  CU_TRY(cudaEventRecord(h->ev_host, st));                       // the copies come after whatever st already holds
+  CU_TRY(cudaStreamWaitEvent(h->up, h->ev_host, 0));
+  CU_TRY(cudaStreamWaitEvent(h->down, h->ev_host, 0));
+  PartHooks hooks;
+  hooks.n_parts = scape::kHostParts;
+  hooks.before = [&](int i, int n) -> int {
+    int64_t a, b;
+    part_range(h, i, n, &a, &b);
+    for (int r = 0; r < h->R; ++r)
+      CU_TRY(cudaMemcpyAsync((char*)h->st_grad[r] + a * ge, (const char*)grads_host[r] + a * ge, (size_t)(b - a) * ge, cudaMemcpyHostToDevice, h->up));
+    CU_TRY(cudaMemcpyAsync(h->st_param + a, param_host + a, sizeof(float) * (size_t)(b - a), cudaMemcpyHostToDevice, h->up));
+    CU_TRY(cudaEventRecord(h->ev_up[i], h->up));
+    CU_TRY(cudaStreamWaitEvent(st, h->ev_up[i], 0));
+    return SCAPE_OK;
+  };
+  hooks.after = [&](int i, int n) -> int {
+    int64_t a, b;
+    part_range(h, i, n, &a, &b);
+    CU_TRY(cudaEventRecord(h->ev_cmp[i], st));
+    CU_TRY(cudaStreamWaitEvent(h->down, h->ev_cmp[i], 0));
+    if (h->clip_max_norm > 0.0 && n == 1) return SCAPE_OK;       // clip_grad finishes theta after the kernel: copied below
+    CU_TRY(cudaMemcpyAsync(param_host + a, h->st_param + a, sizeof(float) * (size_t)(b - a), cudaMemcpyDeviceToHost, h->down));
+    return SCAPE_OK;
+  };
+  int rc = step_impl(h, h->st_param, (const void* const*)h->st_grad, cuda_stream, /*local=*/false, &hooks);
   if (rc) return rc;
-  CU_TRY(cudaMemcpyAsync(param_host, h->st_param, sizeof(float) * h->N, cudaMemcpyDeviceToHost, st));
+  if (h->clip_max_norm > 0.0) CU_TRY(cudaMemcpyAsync(param_host, h->st_param, sizeof(float) * h->N, cudaMemcpyDeviceToHost, st));
+  CU_TRY(cudaEventRecord(h->ev_host, h->down));
+  CU_TRY(cudaStreamWaitEvent(st, h->ev_host, 0));
   CU_TRY(cudaStreamSynchronize(st));
   return SCAPE_OK;
 }

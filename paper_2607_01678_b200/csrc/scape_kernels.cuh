@@ -116,6 +116,10 @@ struct StepParams {
   const float* pm_prev;         // [k]
   int64_t N;
   int64_t n_chunks;             // ceil(N/128)
+  // Sub-range launches (scape_step_host pipelines upload / step / download part by part): this launch covers
+  // chunks [c_begin, c_end) -- multiples of 8 except c_end = n_chunks -- and its warps use the candidate
+  // segments from seg_base on.  A whole-shard launch: 0, n_chunks, 0.  (Not in the grouped staged kernel.)
+  uint32_t c_begin, c_end, seg_base;
   float b1, c1, b2, c2, eps, wd, neg_lr;
   float R_f, inv_R;
   int r_pow2;
@@ -613,7 +617,8 @@ __global__ void __launch_bounds__(256, ((!DENSE && R <= 2) ? 4 : R <= 4 ? 3 : 2)
   const uint32_t wpb = blockDim.x >> 5;
   const uint32_t warp = blockIdx.x * wpb + wib;
   const uint32_t nwarps = gridDim.x * wpb;
-  const uint32_t full = (uint32_t)(p.N >> 7);
+  const uint32_t full_all = (uint32_t)(p.N >> 7);
+  const uint32_t first = p.c_begin, full = p.c_end < full_all ? p.c_end : full_all;     // full chunks of this launch: [first, full)
   const LaneMap lm = lane_map(lane);
   float* sc = reinterpret_cast<float*>(step_smem + (size_t)wib * step_scratch_bytes(R));
   CandRing cr{};
@@ -625,15 +630,15 @@ __global__ void __launch_bounds__(256, ((!DENSE && R <= 2) ? 4 : R <= 4 ? 3 : 2)
     if (lane == 0) *cr.head = 0u;
     __syncwarp();
     sa.lo = p.ctl->br.lo_key; sa.hi = p.ctl->br.hi_key;
-    sa.seg = p.cand + (size_t)warp * p.seg_cap;
+    sa.seg = p.cand + (size_t)(p.seg_base + warp) * p.seg_cap;
   }
-  // this warp's chunks: warp, warp + nwarps, ... (full chunks), then possibly the ragged last one
-  const bool tail = (int64_t)full < p.n_chunks && warp == full % nwarps;
+  // this warp's chunks: first + warp, + nwarps, ... (full chunks), then possibly the ragged last one
+  const bool tail = (int64_t)full < p.n_chunks && (int64_t)p.c_end == p.n_chunks && warp == (full - first) % nwarps;
   MaskWords mw{};
   constexpr int PF = DENSE ? 0 : step_prefetch(R);
-  if (PF > 0 && (warp < full || tail)) load_mask_words<PF >= 2, MSPARSE && PF >= 1>(p, warp < full ? warp : full, lm, mw);
+  if (PF > 0 && (first + warp < full || tail)) load_mask_words<PF >= 2, MSPARSE && PF >= 1>(p, first + warp < full ? first + warp : full, lm, mw);
   // (c < full before c += nwarps wraps: full + nwarps < 2^25)
-  for (uint32_t c = warp; c < full; c += nwarps) {
+  for (uint32_t c = first + warp; c < full; c += nwarps) {
     uint32_t cn = 0xFFFFFFFFu;
     if constexpr (PF > 0) cn = c + nwarps < full ? c + nwarps : tail ? full : 0xFFFFFFFFu;
     fused_chunk<G, R, DENSE, MSPARSE, false, CLIPT, true, PF>(p, c, cn, lane, lm, sc, sa, cr, mw);
@@ -645,7 +650,7 @@ __global__ void __launch_bounds__(256, ((!DENSE && R <= 2) ? 4 : R <= 4 ? 3 : 2)
     uint32_t na = sa.n_above;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
-    if (lane == 0) { p.seg_count[warp] = n_cand; p.seg_above[warp] = na; }
+    if (lane == 0) { p.seg_count[p.seg_base + warp] = n_cand; p.seg_above[p.seg_base + warp] = na; }
   }
   if (CLIPT && p.clip == 1) warp_store_sumsq(p, sa, warp, lane);
 }
@@ -1072,7 +1077,7 @@ __device__ __forceinline__ void tma_consume_tile(const StepParams& p, int64_t ti
     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
     // the stores of the PREVIOUS tile have finished reading their stage: hand it back
     asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
-    if (tile != (int64_t)blockIdx.x) mbar_arrive(&empty[s == 0 ? n_stages - 1 : s - 1]);
+    if (tile - tstride >= (int64_t)(p.c_begin >> 3)) mbar_arrive(&empty[s == 0 ? n_stages - 1 : s - 1]);       // (not after this CTA's first tile)
   }
   if (++s == n_stages) { s = 0; ph ^= 1u; }
 }
@@ -1086,7 +1091,8 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
   uint64_t* empty = full + kTmaMaxStages;
   unsigned char* stage0 = smem + kTmaBarrierBytes;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t n_tiles = p.N / kTmaTile;                     // full tiles; the rest goes through the LDG path
+  const int64_t t_first = p.c_begin >> 3;                     // this launch: tiles [t_first, n_tiles)
+  const int64_t n_tiles = min((int64_t)(p.N / kTmaTile), (int64_t)(p.c_end >> 3));   // full tiles; the rest goes through the LDG path
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < n_stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
@@ -1105,7 +1111,7 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
       uint64_t policy;
       asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
       int s = 0; uint32_t ph = 0;
-      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      for (int64_t tile = t_first + blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         mbar_wait(&empty[s], ph ^ 1u);                         // every consumer warp has read the old contents
         mbar_expect_tx(&full[s], TILE);
         unsigned char* base = stage0 + (size_t)s * TILE;
@@ -1127,7 +1133,7 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
 
   // ===== consumers =====
   const LaneMap lm = lane_map(lane);
-  const int64_t gwarp = (int64_t)blockIdx.x * kTmaConsumerWarps + warp;     // candidate segment of this warp
+  const int64_t gwarp = (int64_t)p.seg_base + (int64_t)blockIdx.x * kTmaConsumerWarps + warp;     // candidate segment of this warp
   StageA sa{};
   sa.layer = kNoLayer;
   sa.lo = p.ctl->br.lo_key; sa.hi = p.ctl->br.hi_key;
@@ -1138,7 +1144,7 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
   // (whose addresses come from the previous mask's words) one tile ahead.  The per-tile state
   // ping-pongs between two register sets (A, B) so that no register move has to wait for a load.
   const int64_t tstride = gridDim.x;
-  int64_t tile = blockIdx.x;
+  int64_t tile = t_first + blockIdx.x;
   TmaMaskWords nw{};                                   // raw words of the NEXT tile
   TmaTileState stA{}, stB{};
   if (tile < n_tiles) {
@@ -1161,7 +1167,7 @@ __global__ void __launch_bounds__(kTmaThreads, 2) scape_fused_tma_kernel(const _
   // chunks past the last full tile (fewer than 8, the last one possibly ragged): LDG path
   {
     const uint32_t c = (uint32_t)n_tiles * kTmaConsumerWarps + warp;
-    if ((int64_t)c < p.n_chunks && blockIdx.x == (unsigned)(n_tiles % gridDim.x)) {
+    if ((int64_t)c < p.n_chunks && (int64_t)p.c_end == p.n_chunks && blockIdx.x == (unsigned)((n_tiles - t_first) % gridDim.x)) {
       // (all bulk stores of this CTA have completed: the first stage serves as scratch)
       float* sc = reinterpret_cast<float*>(stage0) + warp * ((R + 1) * kChunk);
       MaskWords mw;

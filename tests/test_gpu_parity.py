@@ -323,6 +323,39 @@ def test_step_host_matches_device_step(B):
     b.close()
 
 
+@pytest.mark.parametrize("R,gdt,s", [(4, "bf16", 0.99), (2, "f32", 0.9), (8, "f32", 0.99)])
+def test_step_host_pipeline_in_parts(B, R, gdt, s):
+    """scape_step_host on a shard large enough to be pipelined in 8 parts (upload / sub-range launch of the
+    streaming kernel / download, both kernels): every step equal to scape_step on device buffers -- theta, the
+    mask, the index list, b-, b^r and the residuals -- and to the oracle on the last step."""
+    n = 148 * 2 * 8 * 1024 + 3 * 1024 + 77                 # just above the pipeline's threshold, ragged tail
+    w = synth.Workload("hostparts", [("a", n // 3), ("b", n - n // 3)], R=R, sparsity=s, dist="t3", rho=0.9, grad_dtype=gdt, steps=6)
+    gs = synth.GradStream(w, device="cuda", seed=8)
+    th_d = gs.theta0()
+    th_h = th_d.cpu().pin_memory()
+    th_o = th_d.cpu().numpy().copy()
+    a, b = B.Scape(w.numel, R, s, **w.hyper), B.Scape(w.numel, R, s, **w.hyper)
+    ora = ScapeOracle(w.numel, R, s, **w.hyper)
+    for t in range(6):
+        grads = gs.next()
+        a.step(th_d, grads)
+        b.step_host(th_h, [g.cpu().pin_memory() for g in grads])
+        ora.step(th_o, [to_np32(g) for g in grads])
+        torch.cuda.synchronize()
+        assert torch.equal(th_d.cpu(), th_h), t
+        np.testing.assert_array_equal(a.mask_next(), b.mask_next())
+        np.testing.assert_array_equal(a.idx_next(), b.idx_next())
+        assert np.array_equal(a.packed_mean().view(np.uint32), b.packed_mean().view(np.uint32)), t
+        for r in range(R):
+            assert np.array_equal(a.residual(r).view(np.uint32), b.residual(r).view(np.uint32)), (t, r)
+            if t > 0:
+                assert np.array_equal(a.packed(r).view(np.uint32), b.packed(r).view(np.uint32)), (t, r)
+    assert np.array_equal(th_h.numpy().view(np.uint32), th_o.view(np.uint32))
+    np.testing.assert_array_equal(b.mask_next(), ora.mask())
+    a.close()
+    b.close()
+
+
 def test_cuda_graph_capture_of_a_step(B):
     """scape_step allocates nothing and never synchronises, so it can be captured."""
     w = synth.Workload("graph", [("flat", 100_000)], R=2, sparsity=0.9, dist="gauss", rho=0.9,
