@@ -178,6 +178,7 @@ struct scape {
   std::vector<SelGraph> sel_graphs;
   cudaStream_t cap_stream = nullptr;
   bool use_sel_graphs = true;
+  bool fused_hist_made = false;   // the last streaming launch added the candidates' first-digit histogram to ghist
 
   bool pending = false;           // step_local has run, step_apply has not
   bool pending_need_select = false;
@@ -422,6 +423,7 @@ int launch_fused(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t
     int64_t grid = (int64_t)h->n_sm * ct.bps;
     if (grid > n_units) grid = n_units;
     if (part == 0) set_segments(h, p, (n_parts == 1 ? (int)grid : h->n_sm * ct.bps) * kTmaConsumerWarps * n_parts);
+    p.fused_hist = nullptr; h->fused_hist_made = false;
     p.seg_cap = h->seg_cap;
     p.seg_base = (uint32_t)(part * h->n_sm * ct.bps * kTmaConsumerWarps);
     int stages = ct.stages;
@@ -434,6 +436,10 @@ int launch_fused(scape* h, StepParams& p, bool dense, bool msparse, cudaStream_t
   const FusedCfg& c = h->cfg_step[dt][dense ? 0 : msparse ? 2 : 1][clipt];
   const int grid = grid_for(h, range_chunks, 8, c.bps);
   if (part == 0) set_segments(h, p, (n_parts == 1 ? grid : h->n_sm * c.bps) * 8 * n_parts);
+  // flat top-k: the kernel histograms the candidates' first radix digit as it flushes them (sel_decide_kernel)
+  // (not on small shards: zeroing and merging 1024 counters per CTA costs a launch-bound kernel more than the pass it saves)
+  h->fused_hist_made = !dense && h->n_layers == 0 && h->k < h->N && h->N >= ((int64_t)1 << 24);
+  p.fused_hist = h->fused_hist_made ? h->ghist : nullptr;
   p.seg_cap = h->seg_cap;
   p.seg_base = (uint32_t)(part * h->n_sm * c.bps * 8);
   void* args[] = {(void*)&p};
@@ -491,7 +497,8 @@ int run_select_direct(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_g
   cl.cls = h->cls; cl.cand = h->cand; cl.seg_count = h->seg_count; cl.seg_above = h->seg_above;
   cl.seg_cap = h->seg_cap; cl.n_seg = force_general ? 0 : h->n_seg;
   const int grid = grid_for(h, h->n_chunks, 8, 6);
-  sel_decide_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist, cl, (long long)h->k, force_general ? 1 : 0);
+  sel_decide_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist, cl, (long long)h->k, force_general ? 1 : 0,
+                                        (!force_general && h->fused_hist_made) ? 1 : 0);
   h->launches++;
   // 64 undecided bits at most, 13 per pass; the kernels take the digit position from the state
   // and return at once when nothing is left to decide (fast route: 4 passes are typical)
@@ -522,7 +529,7 @@ void drop_sel_graphs(scape* h) {
 int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st, bool compact = true) {
   if (!h->use_sel_graphs || is_capturing(st)) return run_select_direct(h, cur, nxt, force_general, st, compact);
   long long key[8] = {(long long)(&cur - h->slot), (long long)(&nxt - h->slot), (force_general ? 1 : 0) | (cur.all_ones ? 2 : 0), compact ? 1 : 0,
-                      (long long)h->n_seg, (long long)h->seg_cap, (long long)h->k, (long long)h->compact_impl};
+                      (long long)h->n_seg, (long long)h->seg_cap, (long long)h->k, (long long)h->compact_impl | (h->fused_hist_made ? 256 : 0)};
   for (auto& g : h->sel_graphs)
     if (std::memcmp(g.key, key, sizeof key) == 0) {
       CU_TRY(cudaGraphLaunch(g.exec, st));

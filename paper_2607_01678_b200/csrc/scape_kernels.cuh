@@ -55,7 +55,7 @@ struct SelState {
   int use_cls;                // the surviving class has been collected into the small list
   unsigned long long class_count;   // keys in the class chosen by the last pick
   unsigned int cls_n;         // entries in the small list
-  unsigned int pad1;
+  unsigned int first_bits;    // > 0: the histogram of the first digit (this many bits) is already in ghist: the streaming kernel made it
   unsigned long long base;    // fast route: the radix passes run on K64 - base (base = lo_key << 32), see sel_decide_kernel
   Bracket br;                 // predicted bracket for the COMING step's fused pass
   unsigned long long cand_cap_total;   // n_seg * seg_cap of the last fused pass
@@ -136,6 +136,8 @@ struct StepParams {
   int stash;                    // DENSE only: leave m~^0 in e^0 (keys for the select), not 0
   // stage 2 fused into the pass (sparse variant only)
   const SelState* ctl;          // bracket predicted by the previous step
+  uint32_t* fused_hist;         // register-staged kernel, flat top-k: histogram of the candidates' first radix digit (kFusedBits
+                                // bits), added to these global counters at the end of the kernel; nullptr: not wanted
   uint32_t* next_bits;          // [Npad/32] certainly-selected bits of M_t (complete overwrite)
   unsigned long long* cand;     // [n_seg][seg_cap] candidate composite keys, one segment per warp
   uint32_t* seg_count;          // [n_seg] candidates this warp saw (may exceed seg_cap: overflow)
@@ -341,12 +343,29 @@ constexpr uint32_t kRing = 256;
 struct CandRing {
   unsigned long long* ring;     // [kRing] shared memory, private to the warp
   uint32_t* head;               // keys appended so far (shared memory); StageA::cursor = keys flushed so far
+  uint32_t* hist;               // [1 << kFusedBits] shared memory of the CTA, or nullptr: first-digit histogram of the candidates
+  uint32_t hist_shift;          // digit = (key - lo) >> hist_shift
 };
+// First radix digit of the candidate route, made on the fly (the radix-histogram select's first pass over the
+// candidate list costs a third of the select stage at 90 % sparsity): every candidate key lies in [lo, hi), the
+// passes run on K64 - (lo << 32) from bit top = 32 + bits(hi - 1 - lo) down (sel_decide_kernel), so a first
+// digit of kFusedBits bits is (key - lo) >> (top - 32 - kFusedBits) -- usable when that shift is >= 0 and the
+// remaining bits fit the remaining passes.
+constexpr int kFusedBits = 10;
+__host__ __device__ __forceinline__ int fused_hist_shift(uint32_t lo, uint32_t hi) {       // < 0: not usable
+  if (lo == 0xFFFFFFFFu && hi == 0xFFFFFFFFu) return -1;
+  const uint32_t span1 = hi - 1u - lo;
+  int b = 0;
+  while (b < 32 && (span1 >> b) != 0u) ++b;                   // bits of the largest key - lo
+  if (b < kFusedBits || 32 + b - kFusedBits > kDigitBits * (kSelPasses - 1)) return -1;
+  return b - kFusedBits;
+}
 
 __device__ __forceinline__ void ring_flush32(const StepParams& p, StageA& sa, const CandRing& cr, int lane) {
   const uint32_t j = sa.cursor + (uint32_t)lane;
   const unsigned long long v = cr.ring[j & (kRing - 1u)];
   if (j < p.seg_cap) sa.seg[j] = v;                         // a full segment drops keys; seg_count still counts them (overflow)
+  if (cr.hist != nullptr) atomicAdd(&cr.hist[((uint32_t)(v >> 32) - sa.lo) >> cr.hist_shift], 1u);
   sa.cursor += 32u;
 }
 // end of the kernel: the < 32 keys still in the ring; returns the number of keys the warp appended
@@ -355,7 +374,11 @@ __device__ __forceinline__ uint32_t ring_drain(const StepParams& p, StageA& sa, 
   const uint32_t head = *reinterpret_cast<volatile uint32_t*>(cr.head);
   while (head - sa.cursor >= 32u) ring_flush32(p, sa, cr, lane);
   const uint32_t j = sa.cursor + (uint32_t)lane;
-  if (j < head && j < p.seg_cap) sa.seg[j] = cr.ring[j & (kRing - 1u)];
+  if (j < head) {
+    const unsigned long long v = cr.ring[j & (kRing - 1u)];
+    if (j < p.seg_cap) sa.seg[j] = v;
+    if (cr.hist != nullptr) atomicAdd(&cr.hist[((uint32_t)(v >> 32) - sa.lo) >> cr.hist_shift], 1u);
+  }
   return head;
 }
 
@@ -605,7 +628,7 @@ __device__ __forceinline__ void fused_chunk(const StepParams& p, uint32_t c, uin
 // on-mask arithmetic ((R + 1) x 128 floats) and the candidate ring, then the 8 ring heads.
 __host__ __device__ constexpr uint32_t step_scratch_bytes(int R) { return (uint32_t)(R + 1) * kChunk * 4u; }
 __host__ __device__ constexpr uint32_t step_smem_bytes(int R, bool dense) {
-  return dense ? 0u : 8u * (step_scratch_bytes(R) + kRing * 8u) + 8u * 4u;
+  return dense ? 0u : 8u * (step_scratch_bytes(R) + kRing * 8u) + 8u * 4u + (4u << kFusedBits);
 }
 
 template <typename G, int R, bool DENSE, bool MSPARSE, bool CLIPT>
@@ -630,6 +653,13 @@ __global__ void __launch_bounds__(256, ((!DENSE && R <= 2) ? 4 : R <= 4 ? 3 : 2)
     if (lane == 0) *cr.head = 0u;
     __syncwarp();
     sa.lo = p.ctl->br.lo_key; sa.hi = p.ctl->br.hi_key;
+    const int hs = p.fused_hist != nullptr && p.chunk_layer == nullptr ? fused_hist_shift(sa.lo, sa.hi) : -1;
+    if (hs >= 0) {                                            // CTA-uniform
+      cr.hist = reinterpret_cast<uint32_t*>(step_smem + 8u * (step_scratch_bytes(R) + kRing * 8u) + 32u);
+      cr.hist_shift = (uint32_t)hs;
+      for (int b = threadIdx.x; b < (1 << kFusedBits); b += blockDim.x) cr.hist[b] = 0u;
+      __syncthreads();
+    }
     sa.seg = p.cand + (size_t)(p.seg_base + warp) * p.seg_cap;
   }
   // this warp's chunks: first + warp, + nwarps, ... (full chunks), then possibly the ragged last one
@@ -651,6 +681,10 @@ __global__ void __launch_bounds__(256, ((!DENSE && R <= 2) ? 4 : R <= 4 ? 3 : 2)
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
     if (lane == 0) { p.seg_count[p.seg_base + warp] = n_cand; p.seg_above[p.seg_base + warp] = na; }
+    if (cr.hist != nullptr) {                                 // the CTA's first-digit histogram joins the global one
+      __syncthreads();
+      for (int b = threadIdx.x; b < (1 << kFusedBits); b += blockDim.x) if (cr.hist[b]) atomicAdd(&p.fused_hist[b], cr.hist[b]);
+    }
   }
   if (CLIPT && p.clip == 1) warp_store_sumsq(p, sa, warp, lane);
 }

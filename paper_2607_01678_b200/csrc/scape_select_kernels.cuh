@@ -105,11 +105,12 @@ struct CandList {
 // One block.  Sums the per-warp counts of the fused pass and decides whether the predicted bracket
 // held: hit <=> no segment overflowed and n_above < k <= n_above + n_cand.  Arms the radix select
 // with the rank sought inside the candidate list (hit) or inside the whole partition (general).
-__global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t* ghist, CandList cl, long long k, int force_general) {
+//   fused: the streaming kernel has added the histogram of the candidates' first digit (kFusedBits bits) to
+//   ghist whenever fused_hist_shift(bracket) >= 0; it is kept if the bracket held and cleared otherwise.
+__global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t* ghist, CandList cl, long long k, int force_general, int fused) {
   __shared__ unsigned long long s_above[32], s_cand[32];
-  __shared__ int s_over;
-  for (int b = threadIdx.x; b < kBins; b += blockDim.x) ghist[b] = 0;
-  if (threadIdx.x == 0) s_over = 0;
+  __shared__ int s_over, s_keep;
+  if (threadIdx.x == 0) { s_over = 0; s_keep = 0; }
   __syncthreads();
   unsigned long long a = 0, c = 0;
   int over = 0;
@@ -142,6 +143,9 @@ __global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t
       base = (unsigned long long)lo << 32;
       top = 32 + (span1 ? 32 - __clz(span1) : 0);
     }
+    const bool keep = hit && fused && fused_hist_shift(st->br.lo_key, st->br.hi_key) >= 0;
+    st->first_bits = keep ? (unsigned int)kFusedBits : 0u;
+    s_keep = keep ? 1 : 0;
     st->base = base;
     st->prefix = prefix0; st->himask = himask0; st->top = top;
     st->use_cls = 0; st->cls_n = 0; st->class_count = ~0ull;
@@ -156,6 +160,8 @@ __global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t
       if (s_over) st->br.delta = fmaxf(st->br.delta * 0.5f, 0.03f);
     }
   }
+  __syncthreads();
+  if (!s_keep) for (int b = threadIdx.x; b < kBins; b += blockDim.x) ghist[b] = 0;
 }
 
 // Histogram of digit (K64 >> shift) & (2^bits - 1) over the keys whose higher digits equal prefix.
@@ -169,6 +175,7 @@ __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ K
   const int hit = st->hit;
   const int top = st->top;
   if (top <= 0) return;                                   // every digit is fixed already
+  if (st->first_bits != 0u) return;                       // this digit's histogram came with the streaming kernel
   const int bits = top < kDigitBits ? top : kDigitBits;
   const int shift = top - bits;
   const int use_cls = st->use_cls;
@@ -257,7 +264,8 @@ __global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* 
   constexpr int PER = kBins / 1024;                 // bins per thread
   const int top_in = st->top;
   if (top_in <= 0) return;
-  const int bits = top_in < kDigitBits ? top_in : kDigitBits;
+  const int fb = (int)st->first_bits;                 // a first digit of fb bits, histogrammed by the streaming kernel
+  const int bits = fb ? fb : top_in < kDigitBits ? top_in : kDigitBits;
   const int shift = top_in - bits;
   const int last = shift == 0;
   __shared__ long long warp_tot[32];
@@ -295,6 +303,7 @@ __global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* 
         st->himask |= ((1ull << bits) - 1ull) << shift;
         st->rank = rank - cum;
         st->top = shift;
+        st->first_bits = 0u;
         // the pass that just ran collected its class iff that class was known to be small enough
         if (!st->use_cls && st->class_count <= (unsigned long long)kClsCap) st->use_cls = 1;
         st->class_count = hv[q];

@@ -356,6 +356,31 @@ def test_step_host_pipeline_in_parts(B, R, gdt, s):
     b.close()
 
 
+def test_first_radix_digit_made_by_the_streaming_kernel(B):
+    """From 2^24 parameters on, the register-staged kernel histograms the candidates' first radix digit as it
+    flushes them and the select skips its first pass over the candidate list: 8 chained steps, every buffer
+    against the oracle, and the fast route must have been taken once the bracket exists."""
+    n = (1 << 24) + 4099
+    w = synth.Workload("fusedhist", [("a", n // 2 + 17), ("b", n - n // 2 - 17)], R=1, sparsity=0.9, dist="t3", rho=0.9,
+                       grad_dtype="f32", steps=8)
+    gs = synth.GradStream(w, device="cuda", seed=12)
+    th_gpu = gs.theta0()
+    th_ora = th_gpu.cpu().numpy().copy()
+    gpu = B.Scape(w.numel, 1, 0.9, **w.hyper)
+    gpu.keep_dense_pack(True)                      # compare_step also reads b^r of the dense first step
+    ora = ScapeOracle(w.numel, 1, 0.9, **w.hyper)
+    for t in range(1, 9):
+        grads = gs.next()
+        gpu.step(th_gpu, grads)
+        ora.step(th_ora, [to_np32(g) for g in grads])
+        torch.cuda.synchronize()
+        compare_step(gpu, ora, th_gpu, th_ora, 1, f"fusedhist step {t}")
+    fast, general = gpu.select_stats()
+    assert fast >= 5, (fast, general)
+    assert gpu.last_kernel == "scape_fused_step_kernel"
+    gpu.close()
+
+
 def test_cuda_graph_capture_of_a_step(B):
     """scape_step allocates nothing and never synchronises, so it can be captured."""
     w = synth.Workload("graph", [("flat", 100_000)], R=2, sparsity=0.9, dist="gauss", rho=0.9,
