@@ -233,7 +233,7 @@ def run_reference(args):
 
 def run_sweep(args):
     """BASELINE.json config 5: 3 warm-up + 10 timed steps per point (after the dense first step),
-    i.i.d. Gaussian gradients std 1e-3, fixed seed.  Points whose footprint fits the 126 MB L2 run
+    i.i.d. Gaussian gradients std 1e-3, fixed seed, a fresh gradient set every step.  Points whose footprint fits the 126 MB L2 run
     above the DRAM roofline and are labelled l2_resident."""
     import torch
     from paper_2607_01678_b200 import binding, synth
@@ -247,24 +247,31 @@ def run_sweep(args):
                 N = w.numel
                 gs = synth.GradStream(w, device="cuda", seed=args.seed)
                 theta = gs.theta0()
-                # as many distinct gradient sets as fit comfortably (each is 4 R N bytes)
-                n_sets = max(1, min(4, int((120e9 - (8 + 4 * R) * N) // (4 * R * N))))
-                ring = [gs.next() for _ in range(n_sets)]
-                del gs
+                # A fresh gradient set for every step (1 dense + 3 warm-up + 10 timed), drawn on the device between
+                # the steps, as in training, where a gradient never repeats.  (Cycling a few resident sets, as round 1
+                # did, makes the top-k threshold resonate with the error feedback -- period = number of sets -- and the
+                # select's predicted bracket three times wider than on non-repeating inputs: DESIGN.md §5.2.)  Each
+                # timed step has its own CUDA-event pair; the time between the pairs (the draw) is not counted.
                 sc = binding.Scape(N, R, sp, **w.hyper)
                 k = sc.k
-                sc.step(theta, ring[0])
-                for i in range(3):
-                    sc.step(theta, ring[(1 + i) % n_sets])
+                for i in range(4):
+                    grads = gs.next()
+                    sc.step(theta, grads)
+                    del grads
                 torch.cuda.synchronize()
                 f0, g0 = sc.select_stats() if k < N else (0, 0)
-                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                a.record()
+                evs = []
                 for i in range(10):
-                    sc.step(theta, ring[i % n_sets])
-                b.record()
+                    grads = gs.next()
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record()
+                    sc.step(theta, grads)
+                    b.record()
+                    evs.append((a, b))
+                    del grads
                 torch.cuda.synchronize()
-                ms = a.elapsed_time(b) / 10
+                ms = sum(a.elapsed_time(b) for a, b in evs) / 10
+                del gs
                 f1, g1 = sc.select_stats() if k < N else (0, 0)
                 gbs = bytes_per_param_step(w, k, N) * N / (ms * 1e-3) / 1e9
                 foot = (8 + 8 * R) * N / 2**20
@@ -272,7 +279,7 @@ def run_sweep(args):
                             f"{int(foot < 126)},{sc.last_kernel},{f1 - f0},{g1 - g0}")
                 print(rows[-1], flush=True)
                 sc.close()
-                del sc, ring, theta
+                del sc, theta
                 torch.cuda.empty_cache()
     with open(args.sweep, "w") as f:
         f.write("\n".join(rows) + "\n")
@@ -606,7 +613,10 @@ def main():
                 torch.cuda.empty_cache()
                 ga = synth.GradStream(wa, device=dev, seed=args.seed)
                 th0 = ga.theta0()
-                cache[nm] = (th0, [ga.next() for _ in range(2)])
+                # as many distinct gradient sets as the timed run needs, if ~100 GB hold them (else they are cycled)
+                set_bytes = wa.numel * wa.R * grad_bytes(wa)
+                n_also = int(max(2, min(1 + Wa + Ka, (100e9 - (12 + 4 * wa.R) * wa.numel) // set_bytes)))
+                cache[nm] = (th0, [ga.next() for _ in range(n_also)])
                 del ga, th0
             also.append(measure_also(nm, wa, cache[nm][0].clone(), cache[nm][1], Ka, Wa, peak))
         cache.clear()
