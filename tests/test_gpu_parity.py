@@ -356,6 +356,30 @@ def test_step_host_pipeline_in_parts(B, R, gdt, s):
     b.close()
 
 
+@pytest.mark.parametrize("R,gdt", [(2, "f32"), (1, "bf16")])
+def test_step_host_pipeline_with_the_first_digit_histogram(B, R, gdt):
+    """The pipelined scape_step_host on the register-staged kernel at N >= 2^24: every part's launch adds its
+    candidates' first-digit histogram to the global one; results equal to scape_step on device buffers."""
+    n = (1 << 24) + 5 * 1024 + 33
+    w = synth.Workload("hosthist", [("a", n)], R=R, sparsity=0.9, dist="t3", rho=0.9, grad_dtype=gdt, steps=6)
+    gs = synth.GradStream(w, device="cuda", seed=5)
+    th_d = gs.theta0()
+    th_h = th_d.cpu().pin_memory()
+    a, b = B.Scape(n, R, 0.9, **w.hyper), B.Scape(n, R, 0.9, **w.hyper)
+    for t in range(6):
+        g = gs.next()
+        a.step(th_d, g)
+        b.step_host(th_h, [x.cpu().pin_memory() for x in g])
+        torch.cuda.synchronize()
+        assert torch.equal(th_d.cpu(), th_h), t
+        np.testing.assert_array_equal(a.mask_next(), b.mask_next())
+        np.testing.assert_array_equal(a.idx_next(), b.idx_next())
+        assert np.array_equal(a.packed_mean().view(np.uint32), b.packed_mean().view(np.uint32)), t
+    assert b.select_stats()[0] >= 2
+    a.close()
+    b.close()
+
+
 def test_first_radix_digit_made_by_the_streaming_kernel(B):
     """From 2^24 parameters on, the register-staged kernel histograms the candidates' first radix digit as it
     flushes them and the select skips its first pass over the candidate list: 8 chained steps, every buffer
