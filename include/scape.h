@@ -330,6 +330,10 @@ int scape_set_step_count(scape_t* h, int64_t t);
  * steps).  With layers set the counts are per layer and step.  Both routes are exact.
  * Synchronises cuda_stream.                                     */
 int scape_select_stats(scape_t* h, int64_t* fast, int64_t* general, void* cuda_stream);
+/* Of the steps scape_select_stats counts as "general", how many the recovery pass saved from re-reading
+ * every key three to five times: a bracket taken from a sampled histogram, ONE classification pass over
+ * the keys, then the candidate route (a missed prediction, the first step).  HOST output.            */
+int scape_select_recovered(scape_t* h, int64_t* recovered, void* cuda_stream);
 
 /* Diagnostics of the last step's select (not graded): out8 = {bracket held (0/1), entries above
  * the bracket, candidates, half-width of the next bracket in ln units, ln of the exact threshold,

@@ -61,6 +61,7 @@ SYMBOLS = {
     "scape_set": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
     "scape_set_step_count": (_I, [_VP, _I64]),
     "scape_select_stats": (_I, [_VP, _VP, _VP, _VP]),
+    "scape_select_recovered": (_I, [_VP, _VP, _VP]),
     "scape_select_debug": (_I, [_VP, _VP, _VP]),
     "scape_profile": (_I, [_VP, _I]),
     "scape_profile_read": (_I, [_VP, _VP, _VP, _VP]),
@@ -325,6 +326,13 @@ def scape_select_stats(h, stream=0):
     a, b = ctypes.c_int64(), ctypes.c_int64()
     _check(lib().scape_select_stats(h, ctypes.byref(a), ctypes.byref(b), stream), "scape_select_stats")
     return a.value, b.value
+
+
+def scape_select_recovered(h, stream=0):
+    """-> "general" steps that the recovery pass (sampled bracket + one classification pass) completed"""
+    a = ctypes.c_int64()
+    _check(lib().scape_select_recovered(h, ctypes.byref(a), stream), "scape_select_recovered")
+    return a.value
 
 
 def scape_select_debug(h, stream=0):
@@ -597,6 +605,9 @@ class Scape:
 
     def select_debug(self):
         return scape_select_debug(self.h, self._stream())
+
+    def select_recovered(self):
+        return scape_select_recovered(self.h, self._stream())
 
     def profile(self, on=True):
         scape_profile(self.h, on)

@@ -496,10 +496,20 @@ int run_select_direct(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_g
   CandList cl;
   cl.cls = h->cls; cl.cand = h->cand; cl.seg_count = h->seg_count; cl.seg_above = h->seg_above;
   cl.seg_cap = h->seg_cap; cl.n_seg = force_general ? 0 : h->n_seg;
+  // the recovery pass's own segment layout: one segment per warp of its launch -- 5 CTAs per SM on large shards, one
+  // warp per 8 chunks on small ones (so that a segment keeps room for its share of the candidates)
+  cl.rec_n_seg = (int)std::min<int64_t>((int64_t)h->n_sm * 5 * 8, std::max<int64_t>(8, (h->n_chunks / 8 + 7) / 8 * 8));
+  cl.rec_seg_cap = (uint32_t)std::min<int64_t>((h->cand_cap / cl.rec_n_seg) & ~(int64_t)15, 0x7FFFFFF0);
   const int grid = grid_for(h, h->n_chunks, 8, 6);
   sel_decide_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist, cl, (long long)h->k, force_general ? 1 : 0,
                                         (!force_general && h->fused_hist_made) ? 1 : 0);
-  h->launches++;
+  // a missed bracket (or none: all-ones step): bracket from a sampled histogram, one classification pass, then the
+  // candidate route; all four return at once when the predicted bracket held (sel_sample_kernel)
+  sel_sample_kernel<<<grid, 256, 0, st>>>(src, h->sel, h->ghist);
+  sel_sample_pick_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist, (long long)h->k, (long long)h->N);
+  sel_classify_kernel<<<cl.rec_n_seg / 8, 256, 0, st>>>(src, cl, h->sel, h->cand, h->seg_count, h->seg_above, nxt.bits);
+  sel_decide2_kernel<<<1, 1024, 0, st>>>(h->sel, cl, (long long)h->k);
+  h->launches += 5;
   // 64 undecided bits at most, 13 per pass; the kernels take the digit position from the state
   // and return at once when nothing is left to decide (fast route: 4 passes are typical)
   for (int p = 0; p < kSelPasses; ++p) {
@@ -1449,6 +1459,17 @@ extern "C" int scape_select_stats(scape_t* h, int64_t* fast, int64_t* general, v
   CU_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
   if (fast) *fast = (int64_t)(s.n_fast + lc.n_fast);
   if (general) *general = (int64_t)(s.n_general + lc.n_general);
+  return SCAPE_OK;
+}
+
+extern "C" int scape_select_recovered(scape_t* h, int64_t* recovered, void* cuda_stream) {
+  if (!h || !recovered) return fail(SCAPE_EINVAL, "NULL argument");
+  DeviceGuard guard(h->dev);
+  { const int jr = join_side(h, (cudaStream_t)cuda_stream); if (jr) return jr; }
+  SelState s{};
+  CU_TRY(cudaMemcpyAsync(&s, h->sel, sizeof s, cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
+  CU_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+  *recovered = (int64_t)s.n_recovered;
   return SCAPE_OK;
 }
 

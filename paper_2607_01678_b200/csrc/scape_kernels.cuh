@@ -62,6 +62,12 @@ struct SelState {
   int hit;                    // this step: 1 = the bracket held (candidate list), 0 = general path
   unsigned long long n_fast, n_general;   // statistics (scape_select_stats)
   unsigned long long n_above, n_cand;     // this step's counts from the fused pass
+  // Recovery of a missed bracket (and the select of an all-ones step): a bracket taken from a sampled
+  // histogram, one classification pass over every key, then the candidate route (sel_sample_kernel ...)
+  int need_rec;               // this step: the predicted bracket missed (or there was none): the recovery kernels run
+  int rec;                    // this step: the candidate list is the recovery pass's (its own segment layout, bracket [lo2, hi2))
+  uint32_t lo2, hi2;
+  unsigned long long n_recovered;         // statistics: steps the recovery pass saved from the general route
 };
 
 // Per-layer top-k (PAPER.md:89 "per-layer style", :138): one of these per layer, device-resident.

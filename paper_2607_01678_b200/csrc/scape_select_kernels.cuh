@@ -100,6 +100,8 @@ struct CandList {
   const uint32_t* seg_above;
   uint32_t seg_cap;
   int n_seg;
+  uint32_t rec_seg_cap;         // layout of the recovery pass's candidate segments (SelState::rec)
+  int rec_n_seg;
 };
 
 // One block.  Sums the per-warp counts of the fused pass and decides whether the predicted bracket
@@ -151,6 +153,8 @@ __global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t
     st->use_cls = 0; st->cls_n = 0; st->class_count = ~0ull;
     st->rank = hit ? k - (long long)a : k;
     st->hit = hit ? 1 : 0;
+    st->need_rec = hit ? 0 : 1;                     // a miss (or no bracket at all): try the recovery pass before the general route
+    st->rec = 0;
     st->n_above = a; st->n_cand = c;
     st->cand_cap_total = (unsigned long long)cl.n_seg * cl.seg_cap;
     if (hit) st->n_fast += 1; else st->n_general += 1;
@@ -162,6 +166,204 @@ __global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t
   }
   __syncthreads();
   if (!s_keep) for (int b = threadIdx.x; b < kBins; b += blockDim.x) ghist[b] = 0;
+}
+
+// ------------------------------------------------------------------------------------------
+// Recovery of a missed bracket, and the select of an all-ones step (SelState::need_rec).  The general
+// route re-reads every key three to five times (8.9 ms on the headline shard, a ~26 ms step).  Instead:
+//   sel_sample_kernel       histogram of the top 13 key bits over every 64th chunk (every chunk of small shards)
+//   sel_sample_pick_kernel  the bin holding the (scaled) k-th largest sampled key; bracket = that bin
+//                           widened by a quarter bin on either side: [lo2, hi2)
+//   sel_classify_kernel     ONE pass over every key: key >= hi2 sets its bit of M_t, lo2 <= key < hi2
+//                           joins the candidate list (own segment layout), the rest is dropped
+//   sel_decide2_kernel      n_above < k <= n_above + n_cand and no overflow?  then the candidate route
+//                           takes over (rec = 1); else the general route runs as before
+// Exactness does not depend on the sample: it is the same check as for the predicted bracket.
+// All four return at once when the predicted bracket held.
+// ------------------------------------------------------------------------------------------
+constexpr int kRecStride = 64;            // large shards: every 64th chunk is sampled; at least ~2048 chunks (2.6e5 keys) always
+__host__ __device__ __forceinline__ int64_t rec_stride(int64_t n_chunks) {
+  const int64_t s = n_chunks / 2048;
+  return s < 1 ? 1 : s > kRecStride ? kRecStride : s;
+}
+constexpr int kRecShift = 32 - kDigitBits;  // digit of the sample histogram = key >> 19 (exponent + 4 mantissa bits)
+
+__global__ void __launch_bounds__(256) sel_sample_kernel(const __grid_constant__ KeySrc s, const SelState* __restrict__ st,
+                                                        uint32_t* __restrict__ ghist) {
+  if (!st->need_rec) return;
+  __shared__ uint32_t h[kBins];
+  for (int b = threadIdx.x; b < kBins; b += blockDim.x) h[b] = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  const int64_t wpb = blockDim.x >> 5;
+  const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
+  const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  const int64_t stride = rec_stride(s.n_chunks);
+  for (int64_t c = warp * stride; c < s.n_chunks; c += nwarps * stride) {
+    unsigned long long k64[4]; bool valid[4];
+    chunk_keys(s, c, lane, k64, valid);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) if (valid[q]) atomicAdd(&h[(uint32_t)(k64[q] >> (32 + kRecShift))], 1u);
+  }
+  __syncthreads();
+  for (int b = threadIdx.x; b < kBins; b += blockDim.x) if (h[b]) atomicAdd(&ghist[b], h[b]);
+}
+
+// one block of 1024 threads; clears ghist again
+__global__ void __launch_bounds__(1024) sel_sample_pick_kernel(SelState* st, uint32_t* ghist, long long k, long long N) {
+  if (!st->need_rec) return;
+  constexpr int PER = kBins / 1024;
+  __shared__ long long warp_tot[32];
+  __shared__ long long s_total;
+  const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
+  const int top = kBins - PER * t;                  // thread 0 owns the TOP bins
+  uint32_t hv[PER];
+  long long local = 0;
+#pragma unroll
+  for (int q = 0; q < PER; ++q) { hv[q] = ghist[top - 1 - q]; local += hv[q]; ghist[top - 1 - q] = 0; }
+  long long incl = local;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { long long v = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += v; }
+  if (lane == 31) warp_tot[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    long long v = warp_tot[lane], iv = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { long long x = __shfl_up_sync(0xFFFFFFFFu, iv, o); if (lane >= o) iv += x; }
+    warp_tot[lane] = iv - v;
+    if (lane == 31) s_total = iv;
+  }
+  __syncthreads();
+  const long long above = warp_tot[wid] + incl - local;
+  const long long total = s_total;                  // sampled keys
+  if (t == 0) { st->lo2 = 0xFFFFFFFFu; st->hi2 = 0xFFFFFFFFu; }
+  __syncthreads();
+  if (total <= 0) return;
+  // rank of the k-th largest key among the sampled ones, by proportion (the sample is every 64th chunk)
+  long long ks = (long long)((double)k * (double)total / (double)N);
+  if (ks < 1) ks = 1;
+  if (ks > total) ks = total;
+  if (above < ks && ks <= above + local) {
+    long long cum = above;
+#pragma unroll
+    for (int q = 0; q < PER; ++q) {
+      if (cum < ks && ks <= cum + hv[q]) {
+        const uint32_t d = (uint32_t)(top - 1 - q);
+        const uint32_t edge = d << kRecShift, quarter = 1u << (kRecShift - 2);
+        st->lo2 = edge > quarter ? edge - quarter : 0u;
+        const unsigned long long hi = (unsigned long long)edge + (1ull << kRecShift) + quarter;
+        st->hi2 = hi < 0x7F800000ull ? (uint32_t)hi : 0x7F800000u;
+      }
+      cum += hv[q];
+    }
+  }
+}
+
+// launched with exactly cl.rec_n_seg warps: warp w owns segment w
+__global__ void __launch_bounds__(256, 5) sel_classify_kernel(const __grid_constant__ KeySrc s, const __grid_constant__ CandList cl,
+                                                          const SelState* __restrict__ st, unsigned long long* __restrict__ cand,
+                                                          uint32_t* __restrict__ seg_count, uint32_t* __restrict__ seg_above,
+                                                          uint32_t* __restrict__ next_bits) {
+  if (!st->need_rec) return;
+  const uint32_t lo = st->lo2, hi = st->hi2;
+  if (lo == 0xFFFFFFFFu && hi == 0xFFFFFFFFu) return;      // no bracket from the sample
+  const int lane = threadIdx.x & 31;
+  const int64_t wpb = blockDim.x >> 5;
+  const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
+  const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  unsigned long long* seg = cand + (size_t)warp * cl.rec_seg_cap;
+  uint32_t cursor = 0, na = 0;
+  const LaneMap lm = lane_map(lane);
+  // (a lean form of chunk_keys: 32-bit keys only, the mask of the step decoded only in chunks that have
+  // selected entries, composite keys built for candidates only: 163 -> ~70 warp instructions per chunk)
+  for (int64_t c = warp; c < s.n_chunks; c += nwarps) {
+    const uint32_t i0 = (uint32_t)(c << 7) + ((uint32_t)lane << 2);
+    const float4 ev = __ldcs(reinterpret_cast<const float4*>(s.e0 + i0));
+    float x[4] = {ev.x, ev.y, ev.z, ev.w};
+    if (s.cur_bits != nullptr) {
+      const uint2 rk = __ldg(s.cur_rk + c);
+      if ((rk.y >> 24) != 0u) {                             // warp-uniform: this chunk has entries on the step's mask: their keys are b^0
+        uint32_t mybits, jbase;
+        lane_decode(__ldg(s.cur_bits + (c << 2) + lm.ws), rk, lm, mybits, jbase);
+        const float* pk = s.packed0 + jbase;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) if ((mybits >> q) & 1u) { x[q] = __ldg(pk); ++pk; }
+      }
+    }
+    const bool last = c == s.n_chunks - 1;
+    uint32_t nib = 0, cnib = 0, key[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      key[q] = __float_as_uint(x[q]) & 0x7FFFFFFFu;
+      const bool valid = !last || (int64_t)i0 + q < s.N;
+      const bool above = valid && key[q] >= hi;
+      nib |= above ? (1u << q) : 0u;
+      cnib |= (valid && !above && key[q] >= lo) ? (1u << q) : 0u;
+    }
+    if (__any_sync(0xFFFFFFFFu, cnib != 0u)) {                // candidates are a few per cent of the keys
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const bool cnd = (cnib >> q) & 1u;
+        const uint32_t bal = __ballot_sync(0xFFFFFFFFu, cnd);
+        if (cnd) {
+          const uint32_t pos = cursor + __popc(bal & ((1u << lane) - 1u));
+          if (pos < cl.rec_seg_cap) seg[pos] = ((unsigned long long)key[q] << 32) | (unsigned long long)(0xFFFFFFFFu - (i0 + q));
+        }
+        cursor += __popc(bal);
+      }
+    }
+    na += __popc(nib);
+    uint32_t w = nib << lm.sh;
+    w |= __shfl_xor_sync(0xFFFFFFFFu, w, 1);
+    w |= __shfl_xor_sync(0xFFFFFFFFu, w, 2);
+    w |= __shfl_xor_sync(0xFFFFFFFFu, w, 4);
+    if (lm.sh == 0u) next_bits[(c << 2) + lm.ws] = w;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xFFFFFFFFu, na, o);
+  if (lane == 0) { seg_count[warp] = cursor; seg_above[warp] = na; }
+}
+
+// one block: did the sampled bracket hold?
+__global__ void __launch_bounds__(1024) sel_decide2_kernel(SelState* st, CandList cl, long long k) {
+  if (!st->need_rec) return;
+  __shared__ unsigned long long s_above[32], s_cand[32];
+  __shared__ int s_over;
+  if (threadIdx.x == 0) s_over = 0;
+  __syncthreads();
+  const uint32_t lo = st->lo2, hi = st->hi2;
+  const bool have = !(lo == 0xFFFFFFFFu && hi == 0xFFFFFFFFu);
+  unsigned long long a = 0, c = 0;
+  int over = 0;
+  if (have)
+    for (int i = threadIdx.x; i < cl.rec_n_seg; i += blockDim.x) {
+      const uint32_t cnt = cl.seg_count[i];
+      a += cl.seg_above[i]; c += cnt;
+      over |= cnt > cl.rec_seg_cap;
+    }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { a += __shfl_xor_sync(0xFFFFFFFFu, a, o); c += __shfl_xor_sync(0xFFFFFFFFu, c, o); }
+  if ((threadIdx.x & 31) == 0) { s_above[threadIdx.x >> 5] = a; s_cand[threadIdx.x >> 5] = c; }
+  if (over) s_over = 1;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    a = 0; c = 0;
+    for (int i = 0; i < 32; ++i) { a += s_above[i]; c += s_cand[i]; }
+    const bool hit = have && !s_over && (long long)a < k && (long long)(a + c) >= k;
+    st->need_rec = 0;
+    if (hit) {
+      const uint32_t span1 = hi - 1u - lo;
+      st->base = (unsigned long long)lo << 32;
+      st->top = 32 + (span1 ? 32 - __clz(span1) : 0);
+      st->prefix = 0; st->himask = 0;
+      st->use_cls = 0; st->cls_n = 0; st->class_count = ~0ull;
+      st->rank = k - (long long)a;
+      st->hit = 1; st->rec = 1;
+      st->n_above = a; st->n_cand = c;
+      st->n_recovered += 1;
+    }
+    // else: the state sel_decide_kernel armed for the general route stands
+  }
 }
 
 // Histogram of digit (K64 >> shift) & (2^bits - 1) over the keys whose higher digits equal prefix.
@@ -202,7 +404,7 @@ __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ K
     const uint32_t n = min(st->cls_n, kClsCap);
     for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += cls_blocks * blockDim.x) visit(cl.cls[j]);
   } else if (hit) {
-    scan_segments(cl.cand, cl.seg_count, cl.seg_cap, cl.n_seg, st->n_cand, visit);
+    scan_segments(cl.cand, cl.seg_count, st->rec ? cl.rec_seg_cap : cl.seg_cap, st->rec ? cl.rec_n_seg : cl.n_seg, st->n_cand, visit);
   } else {
     for (int64_t c = warp; c < s.n_chunks; c += nwarps) {
       unsigned long long k64[4]; bool valid[4];
@@ -312,7 +514,7 @@ __global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* 
           const unsigned long long Tk = T64 + st->base;
           st->prefix = Tk; st->base = 0;
           float shrink = 0.0f;              // keep the expected candidate count under half the list's capacity
-          if (st->hit && st->cand_cap_total > 0 && 2ull * st->n_cand > st->cand_cap_total)
+          if (st->hit && !st->rec && st->cand_cap_total > 0 && 2ull * st->n_cand > st->cand_cap_total)
             shrink = (float)st->cand_cap_total / (2.0f * (float)st->n_cand);
           predict_bracket(st->br, (uint32_t)(Tk >> 32), shrink);
         }
@@ -335,7 +537,7 @@ __global__ void __launch_bounds__(256) sel_finish_kernel(const __grid_constant__
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
   const int64_t nwarps = (int64_t)gridDim.x * wpb;
   if (st->hit) {
-    scan_segments(cl.cand, cl.seg_count, cl.seg_cap, cl.n_seg, st->n_cand, [&](unsigned long long k64) {
+    scan_segments(cl.cand, cl.seg_count, st->rec ? cl.rec_seg_cap : cl.seg_cap, st->rec ? cl.rec_n_seg : cl.n_seg, st->n_cand, [&](unsigned long long k64) {
       if (k64 >= T64) {
         const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64;
         atomicOr(&next_bits[i >> 5], 1u << (i & 31));

@@ -249,6 +249,28 @@ def test_crafted_ties_and_zeros(B):
     gpu.close()
 
 
+def test_general_route_when_the_recovery_pass_overflows(B):
+    """All-zero gradients on a shard of 2^20: every key is 0, the sampled bracket makes every key a candidate, the
+    candidate list overflows, and the plain general route (radix passes over every key) must take over; ties go to
+    the lowest indices.  Then ordinary gradients again (recovery pass, then the predicted bracket)."""
+    N, R, s = (1 << 20) + 77, 1, 0.9
+    rng = np.random.default_rng(3)
+    gpu = B.Scape(N, R, s, **HYP)
+    gpu.keep_dense_pack(True)
+    ora = ScapeOracle(N, R, s, **HYP)
+    th_ora = (0.02 * rng.standard_normal(N)).astype(np.float32)
+    th_gpu = torch.from_numpy(th_ora.copy()).cuda()
+    for t in range(1, 8):
+        base = np.zeros(N, np.float32) if t <= 3 else (1e-3 * rng.standard_normal(N)).astype(np.float32)
+        gpu.step(th_gpu, [torch.from_numpy(base.copy()).cuda()])
+        ora.step(th_ora, [base.copy()])
+        compare_step(gpu, ora, th_gpu, th_ora, R, f"overflow step {t}")
+    fast, general = gpu.select_stats()
+    rec = gpu.select_recovered()
+    assert general - rec >= 2 and rec >= 1, (fast, general, rec)
+    gpu.close()
+
+
 def test_p9_worked_example_on_gpu(B):
     with open(os.path.join(HERE, "golden", "p9_worked_example.json")) as f:
         G = json.load(f)
@@ -512,6 +534,8 @@ def test_select_survives_threshold_jumps(B):
         compare_step(gpu, ora, th_gpu, th_ora, R, f"jump step {t}")
     fast, general = gpu.select_stats()
     assert fast >= 2 and general >= 3, (fast, general)
+    # most misses are completed by the recovery pass (sampled bracket + one classification pass) ...
+    assert gpu.select_recovered() >= 3, (fast, general, gpu.select_recovered())
     gpu.close()
 
 
