@@ -399,7 +399,7 @@ __device__ __forceinline__ uint32_t ring_drain(const StepParams& p, StageA& sa, 
 //   scm = 128 floats (m_old), sc = R arrays of 128 floats SCS floats apart (m~^r), private to this warp
 //   RING: candidates go through the shared-memory ring `cr` (register-staged front-end), else straight
 //   to the segment with one ballot per element (bulk-copy front-end: register-bound, shared memory full)
-template <int R, bool GUARD, bool STORE, bool CLIPT, bool RING, int SCS, bool DIRECT = false>
+template <int R, bool GUARD, bool STORE, bool CLIPT, bool RING, int SCS>
 __device__ __forceinline__ void sparse_compute(const StepParams& p, uint32_t c, int lane, const LaneMap& lm, uint32_t i0,
                                                uint32_t mybits, uint32_t jbase, uint32_t r0, uint32_t cnt, float* scm, float* sc,
                                                float (&th)[4], const float (&mo)[4],
@@ -434,18 +434,8 @@ __device__ __forceinline__ void sparse_compute(const StepParams& p, uint32_t c, 
         key0[q] = __float_as_uint(mt[0]) & 0x7FFFFFFFu;
         if (on) {
           *pm = mo[q];
-          if constexpr (DIRECT) {
-            float* pk = p.packed + (r0 + (uint32_t)(ps - sc));
-            float sm = mt[0];
 #pragma unroll
-            for (int r = 0; r < R; ++r) { *pk = mt[r]; pk += p.packed_stride; }                 // l.9
-#pragma unroll
-            for (int r = 1; r < R; ++r) sm = __fadd_rn(sm, mt[r]);                              // l.10, r ascending
-            *ps = sm;
-          } else {
-#pragma unroll
-            for (int r = 0; r < R; ++r) ps[r * SCS] = mt[r];
-          }
+          for (int r = 0; r < R; ++r) ps[r * SCS] = mt[r];
           ++ps; ++pm;
         }
       }
@@ -454,16 +444,14 @@ __device__ __forceinline__ void sparse_compute(const StepParams& p, uint32_t c, 
     for (uint32_t l = lane; l < cnt; l += 32) {           // lane l: the chunk's selected entry of rank l
       const float mq = scm[l];
       float sm = sc[l];
-      if constexpr (!DIRECT) {
-        float* pk = p.packed + (r0 + l);
-        __stcs(pk, sm);                                                                     // l.9, r = 0
+      float* pk = p.packed + (r0 + l);
+      __stcs(pk, sm);                                                                       // l.9, r = 0
 #pragma unroll
-        for (int r = 1; r < R; ++r) {
-          const float v = sc[r * SCS + l];
-          pk += p.packed_stride;
-          __stcs(pk, v);                                                                    // l.9
-          sm = __fadd_rn(sm, v);                                                            // l.10, r ascending
-        }
+      for (int r = 1; r < R; ++r) {
+        const float v = sc[r * SCS + l];
+        pk += p.packed_stride;
+        __stcs(pk, v);                                                                      // l.9
+        sm = __fadd_rn(sm, v);                                                              // l.10, r ascending
       }
       const float pq = __fmul_rn(p.b1, mq);
       const float bb = p.r_pow2 ? __fmul_rn(sm, p.inv_R) : __fdiv_rn(sm, p.R_f);          // l.10
@@ -733,7 +721,6 @@ constexpr int kTmaGroup = 4;
 constexpr uint32_t kMbBits = kTmaGroup * 128u;                // bytes of one mask's bits for a group (32 words per tile)
 template <bool RKVIEW> __host__ __device__ constexpr uint32_t tma_mb_tab() { return kTmaGroup * (RKVIEW ? 64u : 32u); }   // rk: 8 x uint2, pre: 8 x u32 per tile
 template <bool RKVIEW> __host__ __device__ constexpr uint32_t tma_mb_bytes() { return 2u * kMbBits + 2u * tma_mb_tab<RKVIEW>() + (RKVIEW ? 0u : 2u * 16u); }
-constexpr bool kTmaDirectPack = false;                        // b^r stored from the owning lanes (phase 1) instead of staged
 
 template <typename G, int R>
 __host__ __device__ constexpr uint32_t tma_tile_bytes() { return kTmaTile * 4u * (1u + R) + kTmaTile * (uint32_t)sizeof(G) * R; }
@@ -893,7 +880,7 @@ __device__ __forceinline__ void tmag_consume_tile(const StepParams& p, const Tma
   // the stage (their contents are in registers now and are written back only after sparse_compute)
   unsigned char* wbase = stage0 + (size_t)s * TILE;
   __syncwarp();
-  sparse_compute<R, false, false, CLIPT, false, kTmaTile, kTmaDirectPack>(p, c, lane, lm, i0, cur.mybits, cur.jbase, cur.r0, cur.cnt,
+  sparse_compute<R, false, false, CLIPT, false, kTmaTile>(p, c, lane, lm, i0, cur.mybits, cur.jbase, cur.r0, cur.cnt,
                                                           reinterpret_cast<float*>(wbase) + warp * kChunk,
                                                           reinterpret_cast<float*>(wbase + OFF_E) + warp * kChunk, th, cur.mo, gg, ee, sa,
                                                           CandRing{});
@@ -1097,7 +1084,7 @@ __device__ __forceinline__ void tma_consume_tile(const StepParams& p, int64_t ti
   // the stage (their contents are in registers now and are written back only after sparse_compute)
   unsigned char* wbase = stage0 + (size_t)s * TILE;
   __syncwarp();
-  sparse_compute<R, false, false, CLIPT, false, kTmaTile, kTmaDirectPack>(p, c, lane, lm, i0, cur.mybits, cur.jbase, cur.r0, cur.cnt,
+  sparse_compute<R, false, false, CLIPT, false, kTmaTile>(p, c, lane, lm, i0, cur.mybits, cur.jbase, cur.r0, cur.cnt,
                                                           reinterpret_cast<float*>(wbase) + warp * kChunk,
                                                           reinterpret_cast<float*>(wbase + OFF_E) + warp * kChunk, th, cur.mo, gg, ee, sa,
                                                           CandRing{});
