@@ -462,6 +462,7 @@ int materialise_dense_m(scape* h, cudaStream_t st) {
   return SCAPE_OK;
 }
 
+static_assert((int64_t)kScanMaxPer * 1024 * kCompactChunksPerBlock * 128 >= ((int64_t)1 << 31), "mask_scan_blocks_kernel: one block scans every block sum of a shard");
 // rank128 (+ idx when idx != nullptr) of slot.bits; leaves the bit count in *h->total
 int compact_mask(scape* h, MaskSlot& s, bool want_idx, cudaStream_t st) {
   const int nb = h->n_compact_blocks;
@@ -670,7 +671,7 @@ int run_select_layered(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_
   for (int round = 0; round < kSelPasses + 1; ++round) {
     if (!force_general) { lsel_hist_cand_kernel<<<grid_c, 256, 0, st>>>(w, cl); h->launches++; }
     lsel_hist_full_kernel<<<grid_f, 256, 0, st>>>(src, w);
-    lsel_pick_kernel<<<h->n_layers, 1024, 0, st>>>(w);
+    lsel_pick_kernel<<<h->n_layers, kLayerPickThreads, 0, st>>>(w);
     h->launches += 2;
   }
   lsel_finish_full_kernel<<<grid_f, 256, 0, st>>>(src, w, nxt.bits);

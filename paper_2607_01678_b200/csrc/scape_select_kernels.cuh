@@ -48,6 +48,7 @@ __device__ __forceinline__ void chunk_keys(const KeySrc& s, int64_t c, int lane,
 
 // Candidate list written by the fused pass: n_seg segments of seg_cap entries.
 constexpr uint32_t kClsCap = 1u << 20;   // entries of the small list the surviving class is collected into
+constexpr uint32_t kClsDirect = 4096;    // a small list of at most this many entries is histogrammed by one CTA with global atomics
 
 // Scan of the candidate segments by the whole grid.  The fused pass leaves one segment per warp
 // (a few thousand of them).  Long segments (large shards: ~10^4 entries each): a work item is one
@@ -384,10 +385,23 @@ __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ K
   const bool collect = !use_cls && st->class_count <= (unsigned long long)kClsCap;
   const uint32_t cls_blocks = min(8u, gridDim.x);         // a handful of CTAs is plenty for the small list
   if (use_cls && blockIdx.x >= cls_blocks) return;
-  for (int b = threadIdx.x; b < kBins; b += blockDim.x) h[b] = 0;
-  __syncthreads();
   const unsigned long long prefix = st->prefix, himask = st->himask;
   const uint32_t dmask = (1u << bits) - 1u;
+  if (use_cls && st->cls_n <= kClsDirect) {
+    // a few keys (the usual case from the third digit on: composite keys are distinct, so a class that shares
+    // 23 bits holds a handful): one CTA, straight to the global histogram -- clearing and merging a private
+    // histogram of 8192 counters was most of such a pass
+    if (blockIdx.x != 0) return;
+    const unsigned long long base = st->base;
+    const uint32_t n = st->cls_n;
+    for (uint32_t j = threadIdx.x; j < n; j += blockDim.x) {
+      const unsigned long long kr = cl.cls[j] - base;
+      if ((kr & himask) == prefix) atomicAdd(&ghist[(uint32_t)(kr >> shift) & dmask], 1u);
+    }
+    return;
+  }
+  for (int b = threadIdx.x; b < kBins; b += blockDim.x) h[b] = 0;
+  __syncthreads();
   const int lane = threadIdx.x & 31;
   const int64_t wpb = blockDim.x >> 5;
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
@@ -461,69 +475,90 @@ __device__ __forceinline__ void predict_bracket(Bracket& b, uint32_t Tkey, float
   b.have_T = b.have_T < 2 ? b.have_T + 1 : 2;
 }
 
-// One block: find the digit d whose class holds the sought rank; fix it; clear the histogram.
-__global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* ghist) {
-  constexpr int PER = kBins / 1024;                 // bins per thread
-  const int top_in = st->top;
-  if (top_in <= 0) return;
-  const int fb = (int)st->first_bits;                 // a first digit of fb bits, histogrammed by the streaming kernel
-  const int bits = fb ? fb : top_in < kDigitBits ? top_in : kDigitBits;
-  const int shift = top_in - bits;
-  const int last = shift == 0;
-  __shared__ long long warp_tot[32];
+// Block-wide scan of the kBins counters of ghist from the TOP bin downwards by NT threads: thread t owns the
+// PER = kBins / NT bins [kBins - PER (t + 1), kBins - PER t), returned top-down (hv[q] = bin kBins - PER t - 1 - q);
+// above = keys in the bins above the thread's, local = keys in its bins, total = all keys.  Clears the histogram.
+// Counts fit 32 bits: a pass counts a key of the partition at most once and N < 2^31.
+template <int NT>
+__device__ __forceinline__ void pick_scan(uint32_t* __restrict__ ghist, uint32_t (&hv)[kBins / NT], uint32_t& above, uint32_t& local,
+                                          uint32_t& total) {
+  constexpr int PER = kBins / NT;
+  static_assert(PER % 4 == 0 && NT % 32 == 0 && NT <= 1024, "pick_scan: whole 16-byte loads per thread");
+  __shared__ uint32_t warp_tot[32];
+  __shared__ uint32_t s_total;
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
-  // thread t owns bins [kBins - PER*(t+1), kBins - PER*t): thread 0 owns the TOP bins
-  const int top = kBins - PER * t;
-  uint32_t hv[PER];
-  long long local = 0;
+  uint4* g4 = reinterpret_cast<uint4*>(ghist + (kBins - PER * (t + 1)));
+  uint32_t asc[PER];
 #pragma unroll
-  for (int q = 0; q < PER; ++q) { hv[q] = ghist[top - 1 - q]; local += hv[q]; }
-  // inclusive prefix sum over threads (from the top bins downwards)
-  long long incl = local;
+  for (int j = 0; j < PER / 4; ++j) { const uint4 v = g4[j]; asc[4 * j] = v.x; asc[4 * j + 1] = v.y; asc[4 * j + 2] = v.z; asc[4 * j + 3] = v.w; }
 #pragma unroll
-  for (int o = 1; o < 32; o <<= 1) { long long v = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += v; }
+  for (int j = 0; j < PER / 4; ++j) g4[j] = make_uint4(0u, 0u, 0u, 0u);
+  local = 0;
+#pragma unroll
+  for (int q = 0; q < PER; ++q) { hv[q] = asc[PER - 1 - q]; local += hv[q]; }
+  uint32_t incl = local;                            // inclusive prefix sum over the threads (from the top bins downwards)
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += v; }
   if (lane == 31) warp_tot[wid] = incl;
   __syncthreads();
   if (wid == 0) {
-    long long v = warp_tot[lane], iv = v;
+    const uint32_t v = lane < NT / 32 ? warp_tot[lane] : 0u;
+    uint32_t iv = v;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { long long x = __shfl_up_sync(0xFFFFFFFFu, iv, o); if (lane >= o) iv += x; }
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, iv, o); if (lane >= o) iv += x; }
     warp_tot[lane] = iv - v;                        // exclusive
+    if (lane == 31) s_total = iv;
   }
   __syncthreads();
-  const long long above = warp_tot[wid] + incl - local;   // keys in bins above this thread's bins
+  above = warp_tot[wid] + incl - local;
+  total = s_total;
+}
+
+// One block: find the digit d whose class holds the sought rank; fix it; clear the histogram.
+// (What the pick needs of the state is loaded together with the histogram: one memory latency instead
+// of a chain of six in the thread that finds the digit.)
+__global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* ghist) {
+  constexpr int NT = 1024, PER = kBins / NT;        // bins per thread
+  const int top_in = st->top;
+  const int fb = (int)st->first_bits;               // a first digit of fb bits, histogrammed by the streaming kernel
   const long long rank = st->rank;
-  __syncthreads();
-  if (above < rank && rank <= above + local) {
+  const unsigned long long prefix = st->prefix, himask = st->himask, base = st->base;
+  const unsigned long long class_count = st->class_count, cap_total = st->cand_cap_total, n_cand = st->n_cand;
+  const int use_cls = st->use_cls, hit = st->hit, rec = st->rec;
+  if (top_in <= 0) return;
+  const int bits = fb ? fb : top_in < kDigitBits ? top_in : kDigitBits;
+  const int shift = top_in - bits;
+  const int last = shift == 0;
+  uint32_t hv[PER], above, local, total;
+  pick_scan<NT>(ghist, hv, above, local, total);
+  const int top = kBins - PER * (int)threadIdx.x;   // this thread's bins end here
+  if ((long long)above < rank && rank <= (long long)above + (long long)local) {
     long long cum = above;
 #pragma unroll
     for (int q = 0; q < PER; ++q) {
-      if (cum < rank && rank <= cum + hv[q]) {
+      if (cum < rank && rank <= cum + (long long)hv[q]) {
         const unsigned long long d = (unsigned long long)(top - 1 - q);
-        const unsigned long long T64 = st->prefix | (d << shift);
+        const unsigned long long T64 = prefix | (d << shift);
         st->prefix = T64;
-        st->himask |= ((1ull << bits) - 1ull) << shift;
+        st->himask = himask | (((1ull << bits) - 1ull) << shift);
         st->rank = rank - cum;
         st->top = shift;
         st->first_bits = 0u;
         // the pass that just ran collected its class iff that class was known to be small enough
-        if (!st->use_cls && st->class_count <= (unsigned long long)kClsCap) st->use_cls = 1;
+        if (!use_cls && class_count <= (unsigned long long)kClsCap) st->use_cls = 1;
         st->class_count = hv[q];
         if (last) {
           // T64 is now exact (back in the key domain): predict the next step's bracket around it
-          const unsigned long long Tk = T64 + st->base;
+          const unsigned long long Tk = T64 + base;
           st->prefix = Tk; st->base = 0;
           float shrink = 0.0f;              // keep the expected candidate count under half the list's capacity
-          if (st->hit && !st->rec && st->cand_cap_total > 0 && 2ull * st->n_cand > st->cand_cap_total)
-            shrink = (float)st->cand_cap_total / (2.0f * (float)st->n_cand);
+          if (hit && !rec && cap_total > 0 && 2ull * n_cand > cap_total) shrink = (float)cap_total / (2.0f * (float)n_cand);
           predict_bracket(st->br, (uint32_t)(Tk >> 32), shrink);
         }
       }
       cum += hv[q];
     }
   }
-#pragma unroll
-  for (int q = 0; q < PER; ++q) ghist[top - 1 - q] = 0;
 }
 
 // Complete M_t once T64 (= st->prefix) is exact: selected(i) <=> K64(i) >= T64.
@@ -706,6 +741,19 @@ __device__ __forceinline__ bool layer_digit(const LayerState& S, unsigned long l
 __global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_constant__ LayerWork w, const __grid_constant__ CandList cl) {
   __shared__ uint32_t ends[SCAPE_MAX_LAYERS_K];
   __shared__ LayerLite lite[kLiteLayers];
+  if (w.ctl->use_cls != 0 && w.ctl->cls_n <= kClsDirect) {
+    // a few keys (see sel_hist_kernel): one CTA, the layer from the chunk table, no layer tables in shared memory
+    if (blockIdx.x != 0) return;
+    const uint32_t n = w.ctl->cls_n;
+    for (uint32_t j = threadIdx.x; j < n; j += blockDim.x) {
+      const unsigned long long k64 = cl.cls[j];
+      const uint32_t l = layer_of(w, 0xFFFFFFFFu - (uint32_t)k64);
+      const LayerState& S = w.layers[l];
+      uint32_t d;
+      if (S.hit && layer_digit(S, k64, d)) atomicAdd(&w.hist[(l << kDigitBits) | d], 1u);
+    }
+    return;
+  }
   load_layer_ends(w, ends, lite);
   const int lane = threadIdx.x & 31;
   const int64_t wpb = blockDim.x >> 5;
@@ -797,41 +845,23 @@ __global__ void __launch_bounds__(256) lsel_hist_full_kernel(const __grid_consta
 // One block per layer: find the digit whose class holds the sought rank; fix it; clear the
 // layer's histogram.  A layer on the candidate route whose candidates turn out to be fewer than
 // the rank sought (the bracket missed) restarts on the general route.
-__global__ void __launch_bounds__(1024) lsel_pick_kernel(LayerWork w) {
-  constexpr int PER = kBins / 1024;
+constexpr int kLayerPickThreads = 512;              // two resident CTAs per SM: a few hundred layers are one wave
+__global__ void __launch_bounds__(kLayerPickThreads, 2) lsel_pick_kernel(LayerWork w) {
+  constexpr int NT = kLayerPickThreads, PER = kBins / NT;
   LayerState& S = w.layers[blockIdx.x];
   uint32_t* ghist = w.hist + (size_t)blockIdx.x * kBins;
   const int top_in = S.top;
+  const long long rank = S.rank;
+  const int hit = S.hit;
+  const unsigned long long prefix = S.prefix, himask = S.himask, base = S.base;
   if (top_in <= 0) return;
   const int bits = top_in < kDigitBits ? top_in : kDigitBits;
   const int shift = top_in - bits;
-  __shared__ long long warp_tot[32];
-  __shared__ long long s_total;
-  const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
+  const int t = threadIdx.x;
   const int topb = kBins - PER * t;                 // thread 0 owns the TOP bins
-  uint32_t hv[PER];
-  long long local = 0;
-#pragma unroll
-  for (int q = 0; q < PER; ++q) { hv[q] = ghist[topb - 1 - q]; local += hv[q]; ghist[topb - 1 - q] = 0; }
-  long long incl = local;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) { long long v = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += v; }
-  if (lane == 31) warp_tot[wid] = incl;
-  __syncthreads();
-  if (wid == 0) {
-    long long v = warp_tot[lane], iv = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { long long x = __shfl_up_sync(0xFFFFFFFFu, iv, o); if (lane >= o) iv += x; }
-    warp_tot[lane] = iv - v;
-    if (lane == 31) s_total = iv;
-  }
-  __syncthreads();
-  const long long above = warp_tot[wid] + incl - local;
-  const long long rank = S.rank;
-  const long long total = s_total;
-  const int hit = S.hit;
-  __syncthreads();
-  if (total < rank) {
+  uint32_t hv[PER], above, local, total;
+  pick_scan<NT>(ghist, hv, above, local, total);
+  if ((long long)total < rank) {
     // only possible on the candidate route, first pass: fewer candidates than entries still to
     // select, i.e. the true threshold lies below the bracket
     if (t == 0) {
@@ -842,16 +872,16 @@ __global__ void __launch_bounds__(1024) lsel_pick_kernel(LayerWork w) {
     }
     return;
   }
-  if (above < rank && rank <= above + local) {
+  if ((long long)above < rank && rank <= (long long)above + (long long)local) {
     long long cum = above;
 #pragma unroll
     for (int q = 0; q < PER; ++q) {
-      if (cum < rank && rank <= cum + hv[q]) {
+      if (cum < rank && rank <= cum + (long long)hv[q]) {
         const unsigned long long d = (unsigned long long)(topb - 1 - q);
-        unsigned long long T64 = S.prefix | (d << shift);
-        if (shift == 0) { T64 += S.base; S.base = 0; }       // exact: back in the key domain
+        unsigned long long T64 = prefix | (d << shift);
+        if (shift == 0) { T64 += base; S.base = 0; }         // exact: back in the key domain
         S.prefix = T64;
-        S.himask |= ((1ull << bits) - 1ull) << shift;
+        S.himask = himask | (((1ull << bits) - 1ull) << shift);
         S.rank = rank - cum;
         S.top = shift;
         if (hit && shift > 0) atomicAdd(&w.ctl->cls_total, (unsigned long long)hv[q]);   // size of the surviving class
@@ -939,35 +969,41 @@ __global__ void __launch_bounds__(1024) mask_block_count_kernel(const uint32_t* 
   }
 }
 
-// exclusive scan of block_sum[0..nb) in place, one block; total -> *total_out
+// exclusive scan of block_sum[0..nb) in place, one block; total -> *total_out.  Thread t owns the
+// ceil(nb / 1024) consecutive sums from t * per on and loads them all at once (one memory latency; a loop
+// over slabs of 1024 sums was 14 dependent round trips on the headline shard, 15 us).  nb <= 2^14: a
+// shard has fewer than 2^24 chunks (N < 2^31) and a block of the count kernel takes 1024 of them.
+constexpr int kScanMaxPer = 16;
 __global__ void __launch_bounds__(1024) mask_scan_blocks_kernel(uint32_t* __restrict__ block_sum, int nb, uint32_t* total_out) {
   __shared__ uint32_t ws[32];
-  __shared__ uint32_t carry;
-  if (threadIdx.x == 0) carry = 0;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int per = (nb + 1023) >> 10;
+  const int i0 = (int)threadIdx.x * per;
+  uint32_t v[kScanMaxPer], sum = 0;
+#pragma unroll
+  for (int q = 0; q < kScanMaxPer; ++q) v[q] = (q < per && i0 + q < nb) ? block_sum[i0 + q] : 0u;
+#pragma unroll
+  for (int q = 0; q < kScanMaxPer; ++q) sum += v[q];
+  uint32_t incl = sum;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += x; }
+  if (lane == 31) ws[wid] = incl;
   __syncthreads();
-  for (int base = 0; base < nb; base += 1024) {
-    const int i = base + threadIdx.x;
-    const uint32_t v = i < nb ? block_sum[i] : 0u;
-    uint32_t incl = v;
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (wid == 0) {
+    const uint32_t x = ws[lane];
+    uint32_t ix = x;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += x; }
-    if (lane == 31) ws[wid] = incl;
-    __syncthreads();
-    if (wid == 0) {
-      uint32_t x = ws[lane], ix = x;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xFFFFFFFFu, ix, o); if (lane >= o) ix += y; }
-      ws[lane] = ix - x;
-    }
-    __syncthreads();
-    const uint32_t excl = carry + ws[wid] + incl - v;
-    if (i < nb) block_sum[i] = excl;
-    __syncthreads();
-    if (threadIdx.x == 1023) carry = excl + v;
-    __syncthreads();
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, ix, o); if (lane >= o) ix += y; }
+    ws[lane] = ix - x;
   }
-  if (threadIdx.x == 0 && total_out) *total_out = carry;
+  __syncthreads();
+  uint32_t run = ws[wid] + incl - sum;
+#pragma unroll
+  for (int q = 0; q < kScanMaxPer; ++q) {
+    if (q < per && i0 + q < nb) block_sum[i0 + q] = run;
+    run += v[q];
+  }
+  if (threadIdx.x == 1023 && total_out) *total_out = run;
 }
 
 // The ascending index list of one chunk per thread (w: the chunk's 128 bits, n of them set, j: packed
