@@ -514,7 +514,7 @@ int run_select_direct(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_g
   // 64 undecided bits at most, 13 per pass; the kernels take the digit position from the state
   // and return at once when nothing is left to decide (fast route: 4 passes are typical)
   for (int p = 0; p < kSelPasses; ++p) {
-    sel_hist_kernel<<<grid, 256, 0, st>>>(src, cl, h->sel, h->ghist);
+    sel_hist_kernel<<<grid, 256, 0, st>>>(src, cl, h->sel, h->ghist, nxt.bits);
     sel_pick_kernel<<<1, 1024, 0, st>>>(h->sel, h->ghist);
     h->launches += 2;
   }
@@ -669,7 +669,7 @@ int run_select_layered(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_
   // 5 digits at most, plus one round for layers whose bracket turns out (first pick) to have
   // missed and that restart on the general route; kernels with nothing to do return at once
   for (int round = 0; round < kSelPasses + 1; ++round) {
-    if (!force_general) { lsel_hist_cand_kernel<<<grid_c, 256, 0, st>>>(w, cl); h->launches++; }
+    if (!force_general) { lsel_hist_cand_kernel<<<grid_c, 256, 0, st>>>(w, cl, nxt.bits); h->launches++; }
     lsel_hist_full_kernel<<<grid_f, 256, 0, st>>>(src, w);
     lsel_pick_kernel<<<h->n_layers, kLayerPickThreads, 0, st>>>(w);
     h->launches += 2;

@@ -68,6 +68,8 @@ struct SelState {
   int rec;                    // this step: the candidate list is the recovery pass's (its own segment layout, bracket [lo2, hi2))
   uint32_t lo2, hi2;
   unsigned long long n_recovered;         // statistics: steps the recovery pass saved from the general route
+  int bits_done;              // candidate route: the pass that collected the surviving class also set the bits of every candidate
+                              // above that class, so sel_finish_kernel only has the small list left to look at
 };
 
 // Per-layer top-k (PAPER.md:89 "per-layer style", :138): one of these per layer, device-resident.
@@ -98,6 +100,7 @@ struct LayerCtl {
   unsigned long long cls_total; // keys in the classes the last picks chose (candidate-route layers)
   unsigned int cls_n;           // entries in the small list
   int use_cls;                  // the small list is complete: read it instead of the segments
+  int bits_done;                // the collecting pass also set the bits of the candidates above their layer's class (see SelState)
 };
 
 struct StepParams {

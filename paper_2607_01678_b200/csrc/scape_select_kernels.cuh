@@ -151,7 +151,7 @@ __global__ void __launch_bounds__(1024) sel_decide_kernel(SelState* st, uint32_t
     s_keep = keep ? 1 : 0;
     st->base = base;
     st->prefix = prefix0; st->himask = himask0; st->top = top;
-    st->use_cls = 0; st->cls_n = 0; st->class_count = ~0ull;
+    st->use_cls = 0; st->cls_n = 0; st->class_count = ~0ull; st->bits_done = 0;
     st->rank = hit ? k - (long long)a : k;
     st->hit = hit ? 1 : 0;
     st->need_rec = hit ? 0 : 1;                     // a miss (or no bracket at all): try the recovery pass before the general route
@@ -357,7 +357,7 @@ __global__ void __launch_bounds__(1024) sel_decide2_kernel(SelState* st, CandLis
       st->base = (unsigned long long)lo << 32;
       st->top = 32 + (span1 ? 32 - __clz(span1) : 0);
       st->prefix = 0; st->himask = 0;
-      st->use_cls = 0; st->cls_n = 0; st->class_count = ~0ull;
+      st->use_cls = 0; st->cls_n = 0; st->class_count = ~0ull; st->bits_done = 0;
       st->rank = k - (long long)a;
       st->hit = 1; st->rec = 1;
       st->n_above = a; st->n_cand = c;
@@ -372,8 +372,13 @@ __global__ void __launch_bounds__(1024) sel_decide2_kernel(SelState* st, CandLis
 // list when the bracket held (st->hit); else every key of the partition.  The pass that first
 // sees a class of at most kClsCap keys also collects that class into the small list, so the
 // remaining passes touch a few thousand keys instead of re-reading everything.
+// On the candidate route that collecting pass also completes M_t for everything outside the class: a
+// candidate whose fixed digits lie ABOVE the threshold's is selected whatever the remaining digits
+// turn out to be, so its bit is set here and sel_finish_kernel is left with the small list (one pass
+// over the whole candidate list less: SelState::bits_done).
 __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ KeySrc s, const __grid_constant__ CandList cl,
-                                                      SelState* __restrict__ st, uint32_t* __restrict__ ghist) {
+                                                      SelState* __restrict__ st, uint32_t* __restrict__ ghist,
+                                                      uint32_t* __restrict__ next_bits) {
   __shared__ uint32_t h[kBins];
   const int hit = st->hit;
   const int top = st->top;
@@ -407,11 +412,15 @@ __global__ void __launch_bounds__(256) sel_hist_kernel(const __grid_constant__ K
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
   const int64_t nwarps = (int64_t)gridDim.x * wpb;
   const unsigned long long base = st->base;
+  const bool set_above = collect && hit;
   auto visit = [&](unsigned long long k64) {
     const unsigned long long kr = k64 - base;
     if ((kr & himask) == prefix) {
       atomicAdd(&h[(uint32_t)(kr >> shift) & dmask], 1u);
       if (collect) { const uint32_t pos = atomicAdd(&st->cls_n, 1u); if (pos < kClsCap) cl.cls[pos] = k64; }
+    } else if (set_above && (kr & himask) > prefix) {
+      const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64;
+      atomicOr(&next_bits[i >> 5], 1u << (i & 31));
     }
   };
   if (use_cls) {
@@ -545,7 +554,7 @@ __global__ void __launch_bounds__(1024) sel_pick_kernel(SelState* st, uint32_t* 
         st->top = shift;
         st->first_bits = 0u;
         // the pass that just ran collected its class iff that class was known to be small enough
-        if (!use_cls && class_count <= (unsigned long long)kClsCap) st->use_cls = 1;
+        if (!use_cls && class_count <= (unsigned long long)kClsCap) { st->use_cls = 1; st->bits_done = hit; }
         st->class_count = hv[q];
         if (last) {
           // T64 is now exact (back in the key domain): predict the next step's bracket around it
@@ -571,6 +580,18 @@ __global__ void __launch_bounds__(256) sel_finish_kernel(const __grid_constant__
   const int64_t wpb = blockDim.x >> 5;
   const int64_t warp = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5);
   const int64_t nwarps = (int64_t)gridDim.x * wpb;
+  if (st->hit && st->bits_done) {
+    // everything above the collected class has its bit already (sel_hist_kernel): the class itself is left
+    const uint32_t n = min(st->cls_n, kClsCap);
+    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+      const unsigned long long k64 = cl.cls[j];
+      if (k64 >= T64) {
+        const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64;
+        atomicOr(&next_bits[i >> 5], 1u << (i & 31));
+      }
+    }
+    return;
+  }
   if (st->hit) {
     scan_segments(cl.cand, cl.seg_count, st->rec ? cl.rec_seg_cap : cl.seg_cap, st->rec ? cl.rec_n_seg : cl.n_seg, st->n_cand, [&](unsigned long long k64) {
       if (k64 >= T64) {
@@ -684,7 +705,7 @@ __global__ void __launch_bounds__(1024) lsel_decide_kernel(LayerWork w, CandList
     w.ctl->overflow = s_over;
     w.ctl->shrink = (!force_general && cap > 0 && 2ull * c > cap) ? (float)cap / (2.0f * (float)c) : 0.0f;
     w.ctl->any_general = 0;
-    w.ctl->cls_total = 0; w.ctl->cls_n = 0; w.ctl->use_cls = 0;
+    w.ctl->cls_total = 0; w.ctl->cls_n = 0; w.ctl->use_cls = 0; w.ctl->bits_done = 0;
   }
   __syncthreads();
   unsigned long long nf = 0, ng = 0;
@@ -738,7 +759,10 @@ __device__ __forceinline__ bool layer_digit(const LayerState& S, unsigned long l
 // Digit histograms of the layers on the candidate route: one global atomic per candidate of a live
 // class (merging equal (layer, digit) pairs of a warp with __match_any_sync first cost more than the
 // atomics it saved: first pass 511 -> 437 us on the headline shard without it).
-__global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_constant__ LayerWork w, const __grid_constant__ CandList cl) {
+// The pass that collects the small list also sets the bit of every candidate that lies above its layer's
+// class (or at / above a threshold that is complete already): see sel_hist_kernel, LayerCtl::bits_done.
+__global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_constant__ LayerWork w, const __grid_constant__ CandList cl,
+                                                            uint32_t* __restrict__ next_bits) {
   __shared__ uint32_t ends[SCAPE_MAX_LAYERS_K];
   __shared__ LayerLite lite[kLiteLayers];
   if (w.ctl->use_cls != 0 && w.ctl->cls_n <= kClsDirect) {
@@ -775,6 +799,11 @@ __global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_consta
       if (L.hit && lite_digit(L, k64, d)) {
         tag = (l << kDigitBits) | d;
         if (collect) { const uint32_t pos = atomicAdd(&w.ctl->cls_n, 1u); if (pos < kClsCap) cl.cls[pos] = k64; }
+      } else if (collect && L.hit) {
+        // outside the layer's class: selected iff above it; a layer whose threshold is complete (top == 0:
+        // prefix is the threshold itself, base 0; ~0 when the layer has nothing left to select) decides here
+        const bool sel = L.top > 0 ? ((k64 - L.base) & L.himask) > L.prefix : k64 >= L.prefix;
+        if (sel) { const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64; atomicOr(&next_bits[i >> 5], 1u << (i & 31)); }
       }
     }
     if (tag != 0xFFFFFFFFu) atomicAdd(&w.hist[tag], 1u);
@@ -813,7 +842,7 @@ __global__ void __launch_bounds__(256) lsel_hist_full_kernel(const __grid_consta
   // follow: a pass that was collecting has completed the list; the class sizes are summed afresh.
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     const unsigned long long ctot = w.ctl->cls_total;
-    if (!w.ctl->use_cls && ctot > 0 && ctot <= (unsigned long long)kClsCap) w.ctl->use_cls = 1;   // the pass before this copied them
+    if (!w.ctl->use_cls && ctot > 0 && ctot <= (unsigned long long)kClsCap) { w.ctl->use_cls = 1; w.ctl->bits_done = 1; }   // the pass before this copied them
     w.ctl->cls_total = 0;
   }
   if (!w.ctl->any_general) return;
@@ -932,6 +961,17 @@ __global__ void __launch_bounds__(256) lsel_finish_cand_kernel(const __grid_cons
                                                               uint32_t* __restrict__ next_bits) {
   __shared__ uint32_t ends[SCAPE_MAX_LAYERS_K];
   __shared__ LayerLite lite[kLiteLayers];
+  if (w.ctl->bits_done) {
+    // the collecting pass has set every bit outside the layers' classes: the small list is left
+    const uint32_t n = min(w.ctl->cls_n, kClsCap);
+    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+      const unsigned long long k64 = cl.cls[j];
+      const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64;
+      const LayerState& S = w.layers[layer_of(w, i)];
+      if (S.hit && k64 >= S.prefix) atomicOr(&next_bits[i >> 5], 1u << (i & 31));
+    }
+    return;
+  }
   load_layer_ends(w, ends, lite);
   uint32_t hint = 0;
   scan_segments(cl.cand, cl.seg_count, cl.seg_cap, cl.n_seg, ~0ull, [&](unsigned long long k64) {
