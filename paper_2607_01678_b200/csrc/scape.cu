@@ -129,6 +129,7 @@ struct scape {
   int max_seg = 0;
   uint32_t* ghist = nullptr;      // [kBins]
   uint32_t* block_sum = nullptr;  // [n_compact_blocks]
+  uint32_t* warp_pre = nullptr;   // [n_compact_blocks * 32] set bits before each group of 32 chunks inside its block of 1024
   uint32_t* total = nullptr;      // [2]: number of set bits, ticket of mask_compact_kernel
   unsigned long long* scan_state = nullptr;   // [n_compact_blocks] look-back state of mask_compact_kernel
   uint32_t compact_epoch = 0;
@@ -474,9 +475,10 @@ int compact_mask(scape* h, MaskSlot& s, bool want_idx, cudaStream_t st) {
     CU_TRY(cudaGetLastError());
     return SCAPE_OK;
   }
-  mask_block_count_kernel<<<nb, 1024, 0, st>>>(s.bits, h->n_chunks, h->block_sum);
+  mask_block_count_kernel<<<nb, 1024, 0, st>>>(s.bits, h->n_chunks, h->block_sum, h->warp_pre);
   mask_scan_blocks_kernel<<<1, 1024, 0, st>>>(h->block_sum, nb, h->total);
-  mask_rank_idx_kernel<<<nb, 1024, 0, st>>>(s.bits, h->n_chunks, h->block_sum, s.rank, s.pre, s.trank, want_idx ? s.idx : nullptr,
+  mask_rank_idx_kernel<<<nb * (kCompactChunksPerBlock / kRankIdxThreads), kRankIdxThreads, 0, st>>>(
+                                            s.bits, h->n_chunks, h->block_sum, h->warp_pre, s.rank, s.pre, s.trank, want_idx ? s.idx : nullptr,
                                             h->packed_stride);
   h->launches += 3;
   CU_TRY(cudaGetLastError());
@@ -709,7 +711,7 @@ void free_all(scape* h) {
   cudaFree(h->m); cudaFree(h->e);
   for (auto& s : h->slot) { cudaFree(s.bits); cudaFree(s.rank); cudaFree(s.pre); cudaFree(s.trank); cudaFree(s.idx); }
   cudaFree(h->packed); cudaFree(h->pm[0]); cudaFree(h->pm[1]); cudaFree(h->dense_pack);
-  cudaFree(h->sel); cudaFree(h->cand); cudaFree(h->cls); cudaFree(h->seg_count); cudaFree(h->seg_above); cudaFree(h->ghist); cudaFree(h->block_sum); cudaFree(h->total); cudaFree(h->scan_state);
+  cudaFree(h->sel); cudaFree(h->cand); cudaFree(h->cls); cudaFree(h->seg_count); cudaFree(h->seg_above); cudaFree(h->ghist); cudaFree(h->block_sum); cudaFree(h->warp_pre); cudaFree(h->total); cudaFree(h->scan_state);
   cudaFree(h->ghat); cudaFree(h->vm); cudaFree(h->sumsq); cudaFree(h->clip_state);
   cudaFree(h->layers); cudaFree(h->lctl); cudaFree(h->chunk_layer); cudaFree(h->lhist); cudaFree(h->items);
   cudaFree(h->st_param); cudaFree(h->iota_scratch);
@@ -784,6 +786,7 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   if (ok && ensure_capacity(h, h->k) != SCAPE_OK) ok = false;                // index lists, packed buffers, candidates
   alloc((void**)&h->ghist, sizeof(uint32_t) * kBins, true);
   alloc((void**)&h->block_sum, sizeof(uint32_t) * (h->n_compact_blocks + 1), true);
+  alloc((void**)&h->warp_pre, sizeof(uint32_t) * 32 * (h->n_compact_blocks + 1), true);
   alloc((void**)&h->total, 2 * sizeof(uint32_t), true);
   alloc((void**)&h->scan_state, sizeof(unsigned long long) * (h->n_compact_blocks + 1), true);
   // measured: the single pass wins while launch count matters (pr1: select stage 99 -> 94 us) and loses on

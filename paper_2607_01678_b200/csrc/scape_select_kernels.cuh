@@ -988,8 +988,10 @@ __global__ void __launch_bounds__(256) lsel_finish_cand_kernel(const __grid_cons
 // ------------------------------------------------------------------------------------------
 constexpr int kCompactChunksPerBlock = 1024;   // one thread per chunk
 
+// block_sum[b] = set bits of block b (1024 chunks); warp_pre[c >> 5] = set bits of the block's chunks before the
+// group of 32 chunks that c belongs to -- with it mask_rank_idx_kernel needs no block-wide step
 __global__ void __launch_bounds__(1024) mask_block_count_kernel(const uint32_t* __restrict__ bits, int64_t n_chunks,
-                                                               uint32_t* __restrict__ block_sum) {
+                                                               uint32_t* __restrict__ block_sum, uint32_t* __restrict__ warp_pre) {
   __shared__ uint32_t ws[32];
   const int64_t c = (int64_t)blockIdx.x * kCompactChunksPerBlock + threadIdx.x;
   uint32_t n = 0;
@@ -1002,10 +1004,12 @@ __global__ void __launch_bounds__(1024) mask_block_count_kernel(const uint32_t* 
   if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = n;
   __syncthreads();
   if (threadIdx.x < 32) {
-    uint32_t v = ws[threadIdx.x];
+    const uint32_t v = ws[threadIdx.x];
+    uint32_t iv = v;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
-    if (threadIdx.x == 0) block_sum[blockIdx.x] = v;
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, iv, o); if ((int)threadIdx.x >= o) iv += x; }
+    warp_pre[(size_t)blockIdx.x * 32 + threadIdx.x] = iv - v;
+    if (threadIdx.x == 31) block_sum[blockIdx.x] = iv;
   }
 }
 
@@ -1088,29 +1092,33 @@ __device__ __forceinline__ void write_chunk_indices(const uint4 w, const uint32_
   }
 }
 
-__global__ void __launch_bounds__(1024) mask_rank_idx_kernel(const uint32_t* __restrict__ bits, int64_t n_chunks,
-                                                            const uint32_t* __restrict__ block_off,
+// One thread per chunk, a warp per group of 32 chunks; the packed position of a group's first set bit is
+// block_off[block] + warp_pre[group], so the warps are independent: no shared memory, no barrier (with a
+// block-wide scan in here the CTAs alternated between a load phase and a write phase, two per SM:
+// 2.6 TB/s on the headline shard).
+// The index list leaves through shared memory: the lanes' runs are laid down at their position inside the group's
+// run and the warp copies that out 128 bytes per instruction (straight from the lanes every index was a 4-byte
+// store to a sector of its own: 27 M L2 write transactions for 107 MB at N = 2^28, 90 %).  Groups with more than
+// kStageIdx set bits (dense regions of a flat top-k) write directly; their dense chunks are coalesced already.
+// (Several groups per warp, loaded together, were slower: the index writes bound the kernel, not the loads.)
+constexpr int kRankIdxThreads = 256;
+constexpr uint32_t kStageIdx = 1024;
+__global__ void __launch_bounds__(kRankIdxThreads) mask_rank_idx_kernel(const uint32_t* __restrict__ bits, int64_t n_chunks,
+                                                            const uint32_t* __restrict__ block_off, const uint32_t* __restrict__ warp_pre,
                                                             uint2* __restrict__ rk, uint32_t* __restrict__ pre, uint32_t* __restrict__ trank,
                                                             int32_t* __restrict__ idx, int64_t idx_cap) {
-  __shared__ uint32_t ws[32];
-  const int64_t c = (int64_t)blockIdx.x * kCompactChunksPerBlock + threadIdx.x;
+  __shared__ int32_t stage[kRankIdxThreads / 32][kStageIdx];
+  const int64_t c = (int64_t)blockIdx.x * kRankIdxThreads + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  if (c - lane >= n_chunks) return;                          // whole warp past the end
   uint4 w = make_uint4(0, 0, 0, 0);
   if (c < n_chunks) w = __ldg(reinterpret_cast<const uint4*>(bits) + c);
+  const uint32_t off = __ldg(block_off + (c >> 10)) + __ldg(warp_pre + (c >> 5));      // warp-uniform
   const uint32_t n = __popc(w.x) + __popc(w.y) + __popc(w.z) + __popc(w.w);
   uint32_t incl = n;
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
 #pragma unroll
-  for (int o = 1; o < 32; o <<= 1) { uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += x; }
-  if (lane == 31) ws[wid] = incl;
-  __syncthreads();
-  if (wid == 0) {
-    uint32_t x = ws[lane], ix = x;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xFFFFFFFFu, ix, o); if (lane >= o) ix += y; }
-    ws[lane] = ix - x;
-  }
-  __syncthreads();
-  const uint32_t j = block_off[blockIdx.x] + ws[wid] + incl - n;
+  for (int o = 1; o < 32; o <<= 1) { const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += x; }
+  const uint32_t j = off + incl - n;
   if (c < n_chunks) {
     const uint32_t pb = chunk_prefix_bytes(__popc(w.x), __popc(w.y), __popc(w.z), __popc(w.w));
     rk[c] = make_uint2(j, pb);
@@ -1118,7 +1126,19 @@ __global__ void __launch_bounds__(1024) mask_rank_idx_kernel(const uint32_t* __r
     if ((c & 7) == 0) trank[c >> 3] = j;
     if (c == n_chunks - 1) trank[(c >> 3) + 1] = j + n;      // the table's last entry: every set bit
   }
-  write_chunk_indices(w, n, j, c, idx, idx_cap);           // whole warps (past the end: w = 0, n = 0)
+  if (idx == nullptr) return;
+  const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31); // set bits of the group (past the end: w = 0, n = 0)
+  if (total <= kStageIdx) {
+    int32_t* sm = stage[threadIdx.x >> 5];
+    write_chunk_indices(w, n, incl - n, c, sm, (int64_t)kStageIdx);
+    __syncwarp();
+    for (uint32_t t = lane; t < total; t += 32) {
+      const uint32_t pos = off + t;
+      if ((int64_t)pos < idx_cap) idx[pos] = sm[t];
+    }
+  } else {
+    write_chunk_indices(w, n, j, c, idx, idx_cap);
+  }
 }
 
 // Single-pass variant of the three kernels above (chained scan with decoupled look-back): every CTA
