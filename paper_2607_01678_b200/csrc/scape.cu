@@ -475,7 +475,7 @@ int compact_mask(scape* h, MaskSlot& s, bool want_idx, cudaStream_t st) {
     CU_TRY(cudaGetLastError());
     return SCAPE_OK;
   }
-  mask_block_count_kernel<<<nb, 1024, 0, st>>>(s.bits, h->n_chunks, h->block_sum, h->warp_pre);
+  mask_block_count_kernel<<<nb, kCountThreads, 0, st>>>(s.bits, h->n_chunks, h->block_sum, h->warp_pre);
   mask_scan_blocks_kernel<<<1, 1024, 0, st>>>(h->block_sum, nb, h->total);
   mask_rank_idx_kernel<<<nb * (kCompactChunksPerBlock / kRankIdxThreads), kRankIdxThreads, 0, st>>>(
                                             s.bits, h->n_chunks, h->block_sum, h->warp_pre, s.rank, s.pre, s.trank, want_idx ? s.idx : nullptr,

@@ -990,18 +990,28 @@ constexpr int kCompactChunksPerBlock = 1024;   // one thread per chunk
 
 // block_sum[b] = set bits of block b (1024 chunks); warp_pre[c >> 5] = set bits of the block's chunks before the
 // group of 32 chunks that c belongs to -- with it mask_rank_idx_kernel needs no block-wide step
-__global__ void __launch_bounds__(1024) mask_block_count_kernel(const uint32_t* __restrict__ bits, int64_t n_chunks,
+// (256 threads, four chunks each, loaded together: one 16-byte load per thread and two CTAs of 1024 per SM kept
+// 32 KB per SM in flight, 3.7 TB/s on the headline shard.)
+constexpr int kCountThreads = 256;
+__global__ void __launch_bounds__(kCountThreads) mask_block_count_kernel(const uint32_t* __restrict__ bits, int64_t n_chunks,
                                                                uint32_t* __restrict__ block_sum, uint32_t* __restrict__ warp_pre) {
+  constexpr int U = kCompactChunksPerBlock / kCountThreads;
   __shared__ uint32_t ws[32];
-  const int64_t c = (int64_t)blockIdx.x * kCompactChunksPerBlock + threadIdx.x;
-  uint32_t n = 0;
-  if (c < n_chunks) {
-    const uint4 w = __ldg(reinterpret_cast<const uint4*>(bits) + c);
-    n = __popc(w.x) + __popc(w.y) + __popc(w.z) + __popc(w.w);
+  const int64_t c0 = (int64_t)blockIdx.x * kCompactChunksPerBlock + threadIdx.x;
+  uint4 w[U];
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+    const int64_t c = c0 + u * kCountThreads;
+    w[u] = make_uint4(0, 0, 0, 0);
+    if (c < n_chunks) w[u] = __ldg(reinterpret_cast<const uint4*>(bits) + c);
   }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) n += __shfl_xor_sync(0xFFFFFFFFu, n, o);
-  if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = n;
+  for (int u = 0; u < U; ++u) {
+    uint32_t n = __popc(w[u].x) + __popc(w[u].y) + __popc(w[u].z) + __popc(w[u].w);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) n += __shfl_xor_sync(0xFFFFFFFFu, n, o);
+    if ((threadIdx.x & 31) == 0) ws[(threadIdx.x >> 5) + u * (kCountThreads / 32)] = n;     // group of chunks c >> 5 inside the block
+  }
   __syncthreads();
   if (threadIdx.x < 32) {
     const uint32_t v = ws[threadIdx.x];
