@@ -477,7 +477,7 @@ int compact_mask(scape* h, MaskSlot& s, bool want_idx, cudaStream_t st) {
   }
   mask_block_count_kernel<<<nb, kCountThreads, 0, st>>>(s.bits, h->n_chunks, h->block_sum, h->warp_pre);
   mask_scan_blocks_kernel<<<1, 1024, 0, st>>>(h->block_sum, nb, h->total);
-  mask_rank_idx_kernel<<<nb * (kCompactChunksPerBlock / kRankIdxThreads), kRankIdxThreads, 0, st>>>(
+  mask_rank_idx_kernel<<<nb * (kCompactChunksPerBlock / (kRankIdxThreads * kRankIdxGroups)), kRankIdxThreads, 0, st>>>(
                                             s.bits, h->n_chunks, h->block_sum, h->warp_pre, s.rank, s.pre, s.trank, want_idx ? s.idx : nullptr,
                                             h->packed_stride);
   h->launches += 3;

@@ -1112,42 +1112,56 @@ __device__ __forceinline__ void write_chunk_indices(const uint4 w, const uint32_
 // kStageIdx set bits (dense regions of a flat top-k) write directly; their dense chunks are coalesced already.
 // (Several groups per warp, loaded together, were slower: the index writes bound the kernel, not the loads.)
 constexpr int kRankIdxThreads = 256;
+constexpr int kRankIdxGroups = 2;               // groups of 32 chunks per warp, loaded together
 constexpr uint32_t kStageIdx = 1024;
 __global__ void __launch_bounds__(kRankIdxThreads) mask_rank_idx_kernel(const uint32_t* __restrict__ bits, int64_t n_chunks,
                                                             const uint32_t* __restrict__ block_off, const uint32_t* __restrict__ warp_pre,
                                                             uint2* __restrict__ rk, uint32_t* __restrict__ pre, uint32_t* __restrict__ trank,
                                                             int32_t* __restrict__ idx, int64_t idx_cap) {
   __shared__ int32_t stage[kRankIdxThreads / 32][kStageIdx];
-  const int64_t c = (int64_t)blockIdx.x * kRankIdxThreads + threadIdx.x;
   const int lane = threadIdx.x & 31;
-  if (c - lane >= n_chunks) return;                          // whole warp past the end
-  uint4 w = make_uint4(0, 0, 0, 0);
-  if (c < n_chunks) w = __ldg(reinterpret_cast<const uint4*>(bits) + c);
-  const uint32_t off = __ldg(block_off + (c >> 10)) + __ldg(warp_pre + (c >> 5));      // warp-uniform
-  const uint32_t n = __popc(w.x) + __popc(w.y) + __popc(w.z) + __popc(w.w);
-  uint32_t incl = n;
+  const int64_t g0 = ((int64_t)blockIdx.x * (kRankIdxThreads / 32) + (threadIdx.x >> 5)) * kRankIdxGroups;   // this warp's first group
+  uint4 w[kRankIdxGroups];
+  uint32_t offs[kRankIdxGroups];
 #pragma unroll
-  for (int o = 1; o < 32; o <<= 1) { const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += x; }
-  const uint32_t j = off + incl - n;
-  if (c < n_chunks) {
-    const uint32_t pb = chunk_prefix_bytes(__popc(w.x), __popc(w.y), __popc(w.z), __popc(w.w));
-    rk[c] = make_uint2(j, pb);
-    pre[c] = pb;
-    if ((c & 7) == 0) trank[c >> 3] = j;
-    if (c == n_chunks - 1) trank[(c >> 3) + 1] = j + n;      // the table's last entry: every set bit
+  for (int u = 0; u < kRankIdxGroups; ++u) {
+    const int64_t g = g0 + u, c = (g << 5) + lane;
+    w[u] = make_uint4(0, 0, 0, 0);
+    offs[u] = 0;
+    if (c < n_chunks) w[u] = __ldg(reinterpret_cast<const uint4*>(bits) + c);
+    if ((g << 5) < n_chunks) offs[u] = __ldg(block_off + (g >> 5)) + __ldg(warp_pre + g);      // warp-uniform
   }
-  if (idx == nullptr) return;
-  const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31); // set bits of the group (past the end: w = 0, n = 0)
-  if (total <= kStageIdx) {
-    int32_t* sm = stage[threadIdx.x >> 5];
-    write_chunk_indices(w, n, incl - n, c, sm, (int64_t)kStageIdx);
-    __syncwarp();
-    for (uint32_t t = lane; t < total; t += 32) {
-      const uint32_t pos = off + t;
-      if ((int64_t)pos < idx_cap) idx[pos] = sm[t];
+#pragma unroll
+  for (int u = 0; u < kRankIdxGroups; ++u) {
+    const int64_t c = ((g0 + u) << 5) + lane;
+    if (c - lane >= n_chunks) break;                         // whole warp past the end
+    const uint32_t off = offs[u];
+    const uint32_t n = __popc(w[u].x) + __popc(w[u].y) + __popc(w[u].z) + __popc(w[u].w);
+    uint32_t incl = n;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += x; }
+    const uint32_t j = off + incl - n;
+    if (c < n_chunks) {
+      const uint32_t pb = chunk_prefix_bytes(__popc(w[u].x), __popc(w[u].y), __popc(w[u].z), __popc(w[u].w));
+      rk[c] = make_uint2(j, pb);
+      pre[c] = pb;
+      if ((c & 7) == 0) trank[c >> 3] = j;
+      if (c == n_chunks - 1) trank[(c >> 3) + 1] = j + n;    // the table's last entry: every set bit
     }
-  } else {
-    write_chunk_indices(w, n, j, c, idx, idx_cap);
+    if (idx == nullptr) continue;
+    const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31); // set bits of the group (past the end: w = 0, n = 0)
+    if (total <= kStageIdx) {
+      int32_t* sm = stage[threadIdx.x >> 5];
+      write_chunk_indices(w[u], n, incl - n, c, sm, (int64_t)kStageIdx);
+      __syncwarp();
+      for (uint32_t t = lane; t < total; t += 32) {
+        const uint32_t pos = off + t;
+        if ((int64_t)pos < idx_cap) idx[pos] = sm[t];
+      }
+      __syncwarp();                                            // the stage is reused by the warp's next group
+    } else {
+      write_chunk_indices(w[u], n, j, c, idx, idx_cap);
+    }
   }
 }
 
