@@ -300,6 +300,30 @@ int scape_param_apply(scape_t* h, float* w, void* w_hat, const void* payload, in
 int scape_mask_pack(const uint8_t* mask_bytes, int64_t n, uint32_t* words, void* cuda_stream);
 int scape_mask_unpack(const uint32_t* words, int64_t n, uint8_t* mask_bytes, void* cuda_stream);
 
+/* Ordered compaction of a bit mask WITHOUT any allocation (stage 4's index half, PAPER.md:144, :154:
+ * "indices into the flattened shard"), stand-alone (no handle), for callers that
+ * cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it.  The scratch of the scan (the look-back state of one CTA per 131,072 bits) is a file-scope
+ * __device__ array of the library, 33 KB, held by every GPU that loads the library until the
+ * process exits; hence the limit n <= SCAPE_STATIC_MAX_BITS.
+ *   mask_words  DEVICE, ceil(n / 32) uint32, 16-byte aligned: bit i % 32 of word i / 32 (the layout of
+ *               SCAPE_MASK_NEXT / scape_mask_pack); bits at positions >= n are ignored.  Read only.
+ *   idx_out     DEVICE, idx_cap int32: the positions of the set bits in ascending order (what
+ *               SCAPE_IDX_NEXT holds for the same mask).  Entries beyond idx_cap are dropped; *count_out
+ *               still counts them.  May be NULL when idx_cap = 0 (count only).
+ *   count_out   DEVICE, one uint32: the number of set bits among the first n.
+ * Enqueues two small memsets of the scratch and one kernel on cuda_stream of the CURRENT device (the one
+ * that owns the buffers) and returns without synchronising.  Calls cudaMalloc / cudaFree never; the first
+ * call on a device resolves the array's address (cudaGetSymbolAddress), later calls only launch.
+ * All calls on one device share the scratch array: calls that may OVERLAP on the GPU (different
+ * streams without an ordering between them) race and give wrong results; calls ordered on one stream,
+ * or by events, are fine.  n = 0 sets *count_out = 0.
+ * SCAPE_EINVAL for n < 0, n > SCAPE_STATIC_MAX_BITS (message names the limit), idx_cap < 0, NULL or
+ * misaligned pointers; SCAPE_ECUDA when a CUDA call fails.                                          */
+#define SCAPE_STATIC_MAX_BITS 536870912LL   /* 2^29 */
+int scape_mask_indices_static(const uint32_t* mask_words, int64_t n, int32_t* idx_out, int64_t idx_cap,
+                              uint32_t* count_out, void* cuda_stream);
+
 /* How rank128 + the index list are made from the bits of a new mask: 0 = by shard size (default:
  * one pass with a chained scan up to 2^26 parameters, three kernels above), 1 = always the single
  * pass, 2 = always the three kernels.  Both forms give identical results; for tests.            */

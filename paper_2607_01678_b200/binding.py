@@ -57,6 +57,7 @@ SYMBOLS = {
     "scape_param_apply": (_I, [_VP, _VP, _VP, _VP, _I, _VP]),
     "scape_mask_pack": (_I, [_VP, _I64, _VP, _VP]),
     "scape_mask_unpack": (_I, [_VP, _I64, _VP, _VP]),
+    "scape_mask_indices_static": (_I, [_VP, _I64, _VP, _I64, _VP, _VP]),
     "scape_get": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
     "scape_set": (_I, [_VP, _I, _I, _VP, _SZ, _VP]),
     "scape_set_step_count": (_I, [_VP, _I64]),
@@ -275,6 +276,13 @@ def scape_mask_pack(mask_bytes_ptr, n, words_ptr, stream=0):
 
 def scape_mask_unpack(words_ptr, n, mask_bytes_ptr, stream=0):
     _check(lib().scape_mask_unpack(words_ptr, int(n), mask_bytes_ptr, stream), "scape_mask_unpack")
+
+
+SCAPE_STATIC_MAX_BITS = 1 << 29
+
+
+def scape_mask_indices_static(words_ptr, n, idx_ptr, idx_cap, count_ptr, stream=0):
+    _check(lib().scape_mask_indices_static(words_ptr, n, idx_ptr, idx_cap, count_ptr, stream), "scape_mask_indices_static")
 
 
 def mask_pack(mask_bytes):

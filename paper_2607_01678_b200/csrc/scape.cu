@@ -7,6 +7,7 @@
 
 #include <algorithm>
 #include <functional>
+#include <mutex>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -1727,5 +1728,154 @@ extern "C" int scape_set(scape_t* h, int what, int r, const void* buf, size_t by
       return fail(SCAPE_EINVAL, "scape_set: selector %d is not settable", what);
   }
   CU_TRY(cudaStreamSynchronize(st));
+  return SCAPE_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// scape_mask_indices_static: the ordered compaction of a bit mask (bits -> ascending int32 index
+// list + count; stage 4's index half) for callers that cannot allocate: code under
+// CUDA graph capture, serving loops, harnesses that forbid cudaMalloc.  A variant of
+// mask_compact_kernel (single pass, chained scan with decoupled look-back) whose look-back state
+// lives in a file-scope array of the library instead of a cudaMalloc'ed buffer of a handle.
+// Every GPU that loads the library holds the array (kStaticScratchWords x 8 bytes = 33 KB) until
+// the process exits.  All calls on one device share it: calls that overlap on the GPU race.
+// ------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int kStaticMaxBlocks = (int)(SCAPE_STATIC_MAX_BITS / ((int64_t)kCompactChunksPerBlock * 128));   // 4096 CTAs of 1024 chunks
+static_assert((int64_t)kStaticMaxBlocks * kCompactChunksPerBlock * 128 == SCAPE_STATIC_MAX_BITS, "SCAPE_STATIC_MAX_BITS: whole blocks");
+constexpr int kStaticCtlWord = kStaticMaxBlocks;          // [0, kStaticMaxBlocks): look-back state; then one word: {total, ticket}
+constexpr int kStaticScratchWords = kStaticMaxBlocks + 32;
+// In host code this name is a host-side stand-in, not a device address: static_scratch_ptr() resolves it per device.
+static __device__ __align__(256) unsigned long long g_static_scratch[kStaticScratchWords];
+
+constexpr int kMaxDevices = 64;
+unsigned long long* g_static_scratch_addr[kMaxDevices] = {};
+std::mutex g_static_mu;
+
+// device address of g_static_scratch on device `dev`, which must be current; resolved once per device
+int static_scratch_ptr(int dev, unsigned long long** out) {
+  if (dev < 0 || dev >= kMaxDevices) return fail(SCAPE_EINVAL, "device ordinal %d out of range", dev);
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (g_static_scratch_addr[dev] == nullptr) {
+    void* p = nullptr;
+    CU_TRY(cudaGetSymbolAddress(&p, g_static_scratch));
+    if (p == nullptr) return fail(SCAPE_ECUDA, "cudaGetSymbolAddress returned a null address");
+    g_static_scratch_addr[dev] = static_cast<unsigned long long*>(p);
+  }
+  *out = g_static_scratch_addr[dev];
+  return SCAPE_OK;
+}
+
+// state[b] = (tag << 32) | value; tag 1: total of block b, 2: inclusive prefix through block b, 0 (cleared by the
+// entry point before every launch): nothing yet.  ctl[0] = ticket.  One thread per chunk of 128 bits.
+__global__ void __launch_bounds__(1024) mask_indices_static_kernel(const uint32_t* __restrict__ bits, int64_t n, int64_t n_words,
+                                                                  int64_t n_chunks, unsigned long long* state, uint32_t* ctl,
+                                                                  int32_t* __restrict__ idx, int64_t idx_cap, uint32_t* __restrict__ count_out) {
+  __shared__ uint32_t ws[32];
+  __shared__ uint32_t s_bid, s_prefix;
+  if (threadIdx.x == 0) s_bid = atomicAdd(&ctl[0], 1u);     // ticket: every predecessor has started
+  __syncthreads();
+  const uint32_t bid = s_bid;
+  const int64_t c = (int64_t)bid * kCompactChunksPerBlock + threadIdx.x;
+  uint4 w = make_uint4(0, 0, 0, 0);
+  if (c < n_chunks) {
+    if ((c << 2) + 4 <= n_words && (c << 7) + 128 <= n) {
+      w = __ldg(reinterpret_cast<const uint4*>(bits) + c);
+    } else {                                                 // the ragged last chunk: word by word, bits at positions >= n ignored
+      uint32_t x[4] = {0u, 0u, 0u, 0u};
+      for (int q = 0; q < 4; ++q) {
+        const int64_t wi = (c << 2) + q, lo = wi << 5;
+        if (wi < n_words && lo < n) {
+          x[q] = __ldg(bits + wi);
+          if (lo + 32 > n) x[q] &= (1u << (uint32_t)(n - lo)) - 1u;
+        }
+      }
+      w = make_uint4(x[0], x[1], x[2], x[3]);
+    }
+  }
+  const uint32_t cnt = __popc(w.x) + __popc(w.y) + __popc(w.z) + __popc(w.w);
+  uint32_t incl = cnt;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, o); if (lane >= o) incl += x; }
+  if (lane == 31) ws[wid] = incl;
+  __syncthreads();
+  constexpr unsigned long long tag_total = 1ull << 32, tag_incl = 2ull << 32;
+  if (wid == 0) {
+    const uint32_t x = ws[lane];
+    uint32_t ix = x;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, ix, o); if (lane >= o) ix += y; }
+    ws[lane] = ix - x;
+    const uint32_t total = __shfl_sync(0xFFFFFFFFu, ix, 31);
+    volatile unsigned long long* vs = state;
+    if (lane == 0) { vs[bid] = (bid == 0 ? tag_incl : tag_total) | total; __threadfence(); }
+    uint32_t prefix = 0;
+    if (bid > 0) {
+      int64_t b0 = (int64_t)bid - 1;                         // newest predecessor not yet accounted for
+      while (true) {
+        const int64_t b = b0 - lane;
+        unsigned long long v = 0;
+        bool ready, is_incl;
+        do {                                                 // until every predecessor in the window has published
+          v = b >= 0 ? vs[b] : tag_incl;                     // before block 0: an inclusive prefix of 0
+          const unsigned long long tg = v & 0xFFFFFFFF00000000ull;
+          is_incl = tg == tag_incl;
+          ready = is_incl || tg == tag_total;
+        } while (!__all_sync(0xFFFFFFFFu, ready));
+        const uint32_t incl_mask = __ballot_sync(0xFFFFFFFFu, is_incl);
+        const int stop = incl_mask ? __ffs(incl_mask) - 1 : 31;      // nearest predecessors first, up to the first inclusive one
+        uint32_t val = lane <= stop ? (uint32_t)v : 0u;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(0xFFFFFFFFu, val, o);
+        prefix += val;
+        if (incl_mask) break;
+        b0 -= 32;
+      }
+      if (lane == 0) { __threadfence(); vs[bid] = tag_incl | (prefix + total); }
+    }
+    if (lane == 0) {
+      s_prefix = prefix;
+      if (bid == gridDim.x - 1) *count_out = prefix + total;
+    }
+  }
+  __syncthreads();
+  const uint32_t j = s_prefix + ws[wid] + incl - cnt;
+  write_chunk_indices(w, cnt, j, c, idx, idx_cap);           // whole warps (past the end: w = 0, cnt = 0)
+}
+
+}  // namespace
+
+extern "C" int scape_mask_indices_static(const uint32_t* mask_words, int64_t n, int32_t* idx_out, int64_t idx_cap,
+                                         uint32_t* count_out, void* cuda_stream) {
+  if (n < 0) return fail(SCAPE_EINVAL, "n must be >= 0");
+  if (n > SCAPE_STATIC_MAX_BITS)
+    return fail(SCAPE_EINVAL, "n = %lld exceeds SCAPE_STATIC_MAX_BITS = %lld (the static scratch array holds the state of %d blocks of 131072 bits)",
+                (long long)n, (long long)SCAPE_STATIC_MAX_BITS, kStaticMaxBlocks);
+  if (idx_cap < 0) return fail(SCAPE_EINVAL, "idx_cap must be >= 0");
+  if (!count_out) return fail(SCAPE_EINVAL, "NULL count_out");
+  if ((uintptr_t)count_out & 3) return fail(SCAPE_EINVAL, "count_out must be 4-byte aligned");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (n == 0) { CU_TRY(cudaMemsetAsync(count_out, 0, sizeof(uint32_t), st)); return SCAPE_OK; }
+  if (!mask_words) return fail(SCAPE_EINVAL, "NULL mask_words");
+  if ((uintptr_t)mask_words & 15) return fail(SCAPE_EINVAL, "mask_words must be 16-byte aligned");
+  if (idx_cap > 0 && !idx_out) return fail(SCAPE_EINVAL, "NULL idx_out with idx_cap > 0");
+  if ((uintptr_t)idx_out & 3) return fail(SCAPE_EINVAL, "idx_out must be 4-byte aligned");
+  int dev = -1;
+  CU_TRY(cudaGetDevice(&dev));
+  unsigned long long* scratch = nullptr;
+  int rc = static_scratch_ptr(dev, &scratch);
+  if (rc) return rc;
+  const int64_t n_words = (n + 31) >> 5;
+  const int64_t n_chunks = (n + 127) >> 7;
+  const int nb = (int)((n_chunks + kCompactChunksPerBlock - 1) / kCompactChunksPerBlock);
+  // the array keeps the last call's contents: the state words of this call's blocks and the ticket start at zero
+  CU_TRY(cudaMemsetAsync(scratch, 0, sizeof(unsigned long long) * (size_t)nb, st));
+  CU_TRY(cudaMemsetAsync(scratch + kStaticCtlWord, 0, sizeof(unsigned long long), st));
+  mask_indices_static_kernel<<<nb, 1024, 0, st>>>(mask_words, n, n_words, n_chunks, scratch,
+                                                  reinterpret_cast<uint32_t*>(scratch + kStaticCtlWord),
+                                                  idx_cap > 0 ? idx_out : nullptr, idx_cap, count_out);
+  CU_TRY(cudaGetLastError());
   return SCAPE_OK;
 }
