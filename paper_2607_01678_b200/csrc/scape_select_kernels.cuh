@@ -666,6 +666,19 @@ __device__ __forceinline__ uint32_t layer_of_sorted(const uint32_t* ends, int n_
   }
   return (uint32_t)lo;
 }
+// Walking a slice of a segment, 32 consecutive candidates per warp step: the chunks ascend along the slice, so a
+// candidate's layer is the one of the candidate before it (hint: the layer of the last lane of the step before, the
+// same for all lanes) or one of the next few -- a scan of a step or two instead of a search whose eight dependent
+// shared-memory reads were 43 % of the stall samples of the first candidate pass.  (Inside a chunk the order is
+// arbitrary, hence the backward loop.)  kNoHint: start of a slice, search.
+constexpr uint32_t kNoHint = 0xFFFFFFFFu;
+__device__ __forceinline__ uint32_t layer_near(const uint32_t* ends, int n_layers, uint32_t i, uint32_t hint) {
+  if (hint == kNoHint) return layer_of_sorted(ends, n_layers, i, 0u);
+  uint32_t l = hint;
+  while (l > 0u && i < ends[l - 1u]) --l;
+  while (l + 1u < (uint32_t)n_layers && i >= ends[l]) ++l;
+  return l;
+}
 __device__ __forceinline__ bool lite_digit(const LayerLite& S, unsigned long long k64, uint32_t& d) {
   const int top = S.top;
   const unsigned long long kr = k64 - S.base;
@@ -790,10 +803,14 @@ __global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_consta
   const unsigned long long ctot = w.ctl->cls_total;
   const bool collect = !use_cls && ctot > 0 && ctot <= (unsigned long long)kClsCap;
   // one warp-wide step: 32 keys (ok = this lane has one)
-  auto visit32 = [&](bool ok, unsigned long long k64) {
+  // sorted: the keys come from a slice of a segment (hint = warp-uniform, see layer_near); else from the small list,
+  // in no order (hint = this lane's previous layer)
+  auto visit32 = [&](bool ok, unsigned long long k64, bool sorted) {
     uint32_t tag = 0xFFFFFFFFu;
+    uint32_t l = hint;
     if (ok) {
-      const uint32_t l = hint = layer_of_sorted(ends, w.n_layers, 0xFFFFFFFFu - (uint32_t)k64, hint);
+      const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64;
+      l = sorted ? layer_near(ends, w.n_layers, i, hint) : layer_of_sorted(ends, w.n_layers, i, hint);
       const LayerLite L = l < (uint32_t)kLiteLayers ? lite[l] : layer_lite(w.layers[l]);
       uint32_t d;
       if (L.hit && lite_digit(L, k64, d)) {
@@ -806,13 +823,14 @@ __global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_consta
         if (sel) { const uint32_t i = 0xFFFFFFFFu - (uint32_t)k64; atomicOr(&next_bits[i >> 5], 1u << (i & 31)); }
       }
     }
+    hint = sorted ? __shfl_sync(0xFFFFFFFFu, l, 31) : l;     // a lane without a key keeps the hint it had
     if (tag != 0xFFFFFFFFu) atomicAdd(&w.hist[tag], 1u);
   };
   if (use_cls) {
     const uint32_t n = min(w.ctl->cls_n, kClsCap);
     for (int64_t j0 = warp * 32; j0 < (int64_t)n; j0 += nwarps * 32) {
       const int64_t j = j0 + lane;
-      visit32(j < (int64_t)n, j < (int64_t)n ? cl.cls[j] : 0ull);
+      visit32(j < (int64_t)n, j < (int64_t)n ? cl.cls[j] : 0ull, false);
     }
     return;
   }
@@ -825,12 +843,13 @@ __global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_consta
     const uint32_t per = ((cnt + P - 1u) / P + 31u) & ~31u;
     const uint32_t b = part * per, e = min(cnt, b + per);
     const unsigned long long* seg = cl.cand + (size_t)sg * cl.seg_cap;
+    hint = kNoHint;
     for (uint32_t j0 = b; j0 < e; j0 += 128) {            // four independent loads per lane in flight
       unsigned long long v[4]; bool ok[4];
 #pragma unroll
       for (int u = 0; u < 4; ++u) { const uint32_t j = j0 + u * 32 + lane; ok[u] = j < e; v[u] = ok[u] ? __ldcs(seg + j) : 0ull; }
 #pragma unroll
-      for (int u = 0; u < 4; ++u) if (j0 + u * 32 < e) visit32(ok[u], v[u]);
+      for (int u = 0; u < 4; ++u) if (j0 + u * 32 < e) visit32(ok[u], v[u], true);
     }
   }
 }
