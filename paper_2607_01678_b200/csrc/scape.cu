@@ -176,7 +176,7 @@ struct scape {
   // mask rotation (which slots), the route forced or not, k and the segment layout: each distinct
   // sequence is captured once into a CUDA graph and replayed with one launch afterwards (shards under
   // ~2^23 parameters are launch-bound: pr1 0.113 -> see DESIGN.md ms per step)
-  struct SelGraph { long long key[8]; cudaGraphExec_t exec; int launches; };
+  struct SelGraph { long long key[11]; cudaGraphExec_t exec; int launches; };
   std::vector<SelGraph> sel_graphs;
   cudaStream_t cap_stream = nullptr;
   bool use_sel_graphs = true;
@@ -540,10 +540,20 @@ void drop_sel_graphs(scape* h) {
 
 // run_select_direct through a cached CUDA graph (see scape::SelGraph).  Falls back to the direct launches
 // inside a caller's capture, and whenever capturing or instantiating fails.
-int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st, bool compact = true) {
-  if (!h->use_sel_graphs || is_capturing(st)) return run_select_direct(h, cur, nxt, force_general, st, compact);
-  long long key[8] = {(long long)(&cur - h->slot), (long long)(&nxt - h->slot), (force_general ? 1 : 0) | (cur.all_ones ? 2 : 0), compact ? 1 : 0,
-                      (long long)h->n_seg, (long long)h->seg_cap, (long long)h->k, (long long)h->compact_impl | (h->fused_hist_made ? 256 : 0)};
+int run_select_layered_direct(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st, bool compact);
+
+// layered: the per-layer select (its 25 launches as one graph: 0.1 ms of dependency latency less on the headline shard);
+// its kernels take the layer tables' addresses, the item count and the sparsity by value (scape_set_layers drops the graphs)
+int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st, bool compact = true, bool layered = false) {
+  auto direct = [layered](scape* h_, const MaskSlot& cur_, MaskSlot& nxt_, bool fg, cudaStream_t st_, bool compact_) {
+    return layered ? run_select_layered_direct(h_, cur_, nxt_, fg, st_, compact_) : run_select_direct(h_, cur_, nxt_, fg, st_, compact_);
+  };
+  if (!h->use_sel_graphs || is_capturing(st)) return direct(h, cur, nxt, force_general, st, compact);
+  long long sparsity_bits = 0;
+  std::memcpy(&sparsity_bits, &h->sparsity, sizeof(double));
+  long long key[11] = {(long long)(&cur - h->slot), (long long)(&nxt - h->slot), (force_general ? 1 : 0) | (cur.all_ones ? 2 : 0), compact ? 1 : 0,
+                       (long long)h->n_seg, (long long)h->seg_cap, (long long)h->k, (long long)h->compact_impl | (h->fused_hist_made ? 256 : 0),
+                       layered ? 1 : 0, (long long)h->n_layers, layered ? sparsity_bits : 0};
   for (auto& g : h->sel_graphs)
     if (std::memcmp(g.key, key, sizeof key) == 0) {
       CU_TRY(cudaGraphLaunch(g.exec, st));
@@ -553,7 +563,7 @@ int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general,
     }
   if (!h->cap_stream && cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
     cudaGetLastError(); h->cap_stream = nullptr;
-    return run_select_direct(h, cur, nxt, force_general, st, compact);
+    return direct(h, cur, nxt, force_general, st, compact);
   }
   if (h->sel_graphs.size() >= 24) drop_sel_graphs(h);          // (a density schedule changes k every step)
   const int64_t l0 = h->launches;
@@ -561,9 +571,9 @@ int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general,
   cudaGraphExec_t exec = nullptr;
   if (cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
     cudaGetLastError();
-    return run_select_direct(h, cur, nxt, force_general, st, compact);
+    return direct(h, cur, nxt, force_general, st, compact);
   }
-  const int rc = run_select_direct(h, cur, nxt, force_general, h->cap_stream, compact);
+  const int rc = direct(h, cur, nxt, force_general, h->cap_stream, compact);
   const cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
   const int n_launch = (int)(h->launches - l0);
   h->launches = l0;
@@ -571,7 +581,7 @@ int run_select(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general,
     cudaGetLastError();
     if (graph) cudaGraphDestroy(graph);
     h->use_sel_graphs = false;                                   // not available here: direct launches from now on
-    return run_select_direct(h, cur, nxt, force_general, st, compact);
+    return direct(h, cur, nxt, force_general, st, compact);
   }
   cudaGraphDestroy(graph);
   scape::SelGraph g;
@@ -652,6 +662,10 @@ int64_t total_k(const scape* h, double s) {
 
 // Stage 2 with layers: the same exact select inside every layer at once.
 int run_select_layered(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st, bool compact = true) {
+  return run_select(h, cur, nxt, force_general, st, compact, /*layered=*/true);
+}
+
+int run_select_layered_direct(scape* h, const MaskSlot& cur, MaskSlot& nxt, bool force_general, cudaStream_t st, bool compact) {
   KeySrc src;
   src.e0 = h->e;
   src.cur_bits = cur.all_ones ? nullptr : cur.bits;
@@ -924,6 +938,7 @@ extern "C" int scape_set_layers(scape_t* h, int n_layers, const int64_t* offsets
   if (h->world > 1) return fail(SCAPE_EINVAL, "this handle is one of %d workers: scape_set_workers(h, 1, 0, NULL) before changing the layers", h->world);
   DeviceGuard g(h->dev);
   CU_TRY(cudaDeviceSynchronize());
+  drop_sel_graphs(h);                        // the per-layer graphs hold the layer tables' addresses and the item count
   if (n_layers == 0) {                       // back to one flat top-k
     h->n_layers = 0; h->lay_off.clear(); h->lay_compress.clear();
     h->k = total_k(h, h->sparsity);

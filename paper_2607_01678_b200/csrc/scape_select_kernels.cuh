@@ -49,6 +49,7 @@ __device__ __forceinline__ void chunk_keys(const KeySrc& s, int64_t c, int lane,
 // Candidate list written by the fused pass: n_seg segments of seg_cap entries.
 constexpr uint32_t kClsCap = 1u << 20;   // entries of the small list the surviving class is collected into
 constexpr uint32_t kClsDirect = 4096;    // a small list of at most this many entries is histogrammed by one CTA with global atomics
+constexpr uint32_t kClsDirectLayers = 1u << 16;   // per-layer select: by ceil(n / 256) CTAs
 
 // Scan of the candidate segments by the whole grid.  The fused pass leaves one segment per warp
 // (a few thousand of them).  Long segments (large shards: ~10^4 entries each): a work item is one
@@ -778,11 +779,13 @@ __global__ void __launch_bounds__(256) lsel_hist_cand_kernel(const __grid_consta
                                                             uint32_t* __restrict__ next_bits) {
   __shared__ uint32_t ends[SCAPE_MAX_LAYERS_K];
   __shared__ LayerLite lite[kLiteLayers];
-  if (w.ctl->use_cls != 0 && w.ctl->cls_n <= kClsDirect) {
-    // a few keys (see sel_hist_kernel): one CTA, the layer from the chunk table, no layer tables in shared memory
-    if (blockIdx.x != 0) return;
+  if (w.ctl->use_cls != 0 && w.ctl->cls_n <= kClsDirectLayers) {
+    // a few keys per layer (see sel_hist_kernel; a few hundred layers together: 10^3 .. 10^4): one thread per key,
+    // the layer from the chunk table, no layer tables in shared memory; the other CTAs return at once (with every
+    // CTA loading the tables first, such a pass took 25 us on the headline shard)
     const uint32_t n = w.ctl->cls_n;
-    for (uint32_t j = threadIdx.x; j < n; j += blockDim.x) {
+    if (blockIdx.x * blockDim.x >= n) return;
+    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
       const unsigned long long k64 = cl.cls[j];
       const uint32_t l = layer_of(w, 0xFFFFFFFFu - (uint32_t)k64);
       const LayerState& S = w.layers[l];
