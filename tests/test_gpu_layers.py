@@ -150,6 +150,34 @@ def test_sparsity_can_go_back_to_dense_and_up_again(B):
     run(B, w, steps=9, seed=6, schedule=lambda t: sched[t])
 
 
+def test_layers_can_change_between_steps(B):
+    """scape_set_layers in the middle of a run (the cached select graphs hold the old layer tables' addresses and
+    item counts and must go): layout A, another layout, the flat top-k, layout A again; every step against the oracle."""
+    w = synth.Workload("relayer", [("a", 128 * 700 + 77)], R=2, sparsity=0.9, dist="gauss", rho=0.9, grad_dtype="f32", steps=18)
+    N = w.numel
+    lay_a = [0, 1000, 1000 + 128 * 300 + 5, 60_000, N]
+    lay_b = [0, 128 * 100, 128 * 100 + 3, 20_000, 20_001, 70_000 + 9, N]
+    plan = {1: (lay_a, [1, 1, 0, 1]), 6: (lay_b, [1, 0, 1, 1, 1, 1]), 11: None, 14: (lay_a, [1, 1, 0, 1])}
+    gs = synth.GradStream(w, device="cuda", seed=9)
+    th_gpu = gs.theta0()
+    th_ora = th_gpu.cpu().numpy().copy()
+    gpu, ora = make_pair(B, w)
+    for t in range(1, 19):
+        if t in plan:
+            if plan[t] is None:                      # flat: one top-k over the shard = one compressed layer
+                gpu.clear_layers()
+                ora.set_layers([0, N], [1])
+            else:
+                gpu.set_layers(*plan[t])
+                ora.set_layers(*plan[t])
+        grads = gs.next()
+        gpu.step(th_gpu, grads)
+        ora.step(th_ora, [to_np32(g) for g in grads])
+        torch.cuda.synchronize()
+        compare_step(gpu, ora, th_gpu, th_ora, w.R, f"relayer step {t}")
+    gpu.close()
+
+
 def test_set_layers_api_errors(B):
     gpu = B.Scape(1000, 1, 0.9, **HYP)
     for bad in ([0, 500], [1, 1000], [0, 500, 500, 1000], [0, 600, 400, 1000]):
