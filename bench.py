@@ -400,6 +400,61 @@ def measure_also(name, w, theta, ring, K, W, peak, layers=False):
     return out
 
 
+def measure_fresh(name, w, K, W, peak, seed, layers=False):
+    """The same step with a FRESH gradient set every step, drawn on the device between the steps (as in training, where
+    a gradient never repeats; the draw is not timed: every timed step has its own CUDA-event pair).  The resident sets the
+    headline cycles keep the select's predicted brackets wide (the threshold resonates with the error feedback, period =
+    number of sets): this line shows the select stage on non-repeating inputs."""
+    import torch
+    from paper_2607_01678_b200 import binding, synth
+    N, R = w.numel, w.R
+    gs = synth.GradStream(w, device="cuda", seed=seed)
+    theta = gs.theta0()
+    sc = binding.Scape(N, R, w.sparsity, **w.hyper)
+    if layers:
+        sc.set_layers(w.offsets(), w.compress_flags())
+    k = sc.k
+    for _ in range(1 + W):
+        grads = gs.next()
+        sc.step(theta, grads)
+        del grads
+    torch.cuda.synchronize()
+    sc.profile(True)
+    f0, g0 = sc.select_stats()
+    evs = []
+    for _ in range(K):
+        grads = gs.next()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        sc.step(theta, grads)
+        b.record()
+        evs.append((a, b))
+        del grads
+    torch.cuda.synchronize()
+    per = [a.elapsed_time(b) for a, b in evs]
+    fused_ms, select_ms, psteps = sc.profile_read()
+    sc.profile(False)
+    f1, g1 = sc.select_stats()
+    ms = sum(per) / K
+    kms = fused_ms / max(1, psteps)
+    fb = bytes_per_param_fused(w, k, N) * N
+    sb = bytes_per_param_step(w, k, N) * N
+    out = {"workload": name, "gradients": "fresh every step (drawn on the device between the timed steps; per-step CUDA events)",
+           "shard_numel": N, "R": R, "grad_dtype": w.grad_dtype, "sparsity": w.sparsity, "k": k,
+           "refresh": "per layer (one top-k per tensor)" if layers else "flat top-k over the shard",
+           "steps": K, "warmup": W, "ms_per_step": ms, **step_stats(per), "params_per_s": N / (ms * 1e-3),
+           "kernel": sc.last_kernel, "kernel_ms": kms, "kernel_share_of_step": kms / ms,
+           "kernel_gbs": fb / (kms * 1e-3) / 1e9, "kernel_frac_of_peak": fb / (kms * 1e-3) / 1e9 / peak,
+           "select_ms": select_ms / max(1, psteps), "step_gbs": sb / (ms * 1e-3) / 1e9,
+           "step_frac_of_peak": sb / (ms * 1e-3) / 1e9 / peak,
+           "select_fast": f1 - f0, "select_general": g1 - g0, "l2_resident": False}
+    assert bool(torch.isfinite(theta).all())
+    sc.close()
+    del gs, theta
+    torch.cuda.empty_cache()
+    return out
+
+
 # ---------------------------------------------------------------------------------------------
 def main():
     args = parse()
@@ -605,6 +660,8 @@ def main():
         also = [measure_also("llama1p8b --layers", w, theta, ring, Ka, Wa, peak, layers=True)]
         del ring, theta
         torch.cuda.empty_cache()
+        for lay in (False, True):                    # the headline shard on non-repeating gradients
+            also.append(measure_fresh("llama1p8b, fresh gradients" + (" --layers" if lay else ""), w, Ka, 12, peak, args.seed, layers=lay))
         cache = {}                                   # llama500m at 99 % re-uses the inputs drawn for 90 %
         for nm, sp in (("llama500m", 0.9), ("llama500m", None), ("gpt345m", None), ("pr1", None)):
             wa = synth.workload(nm, sparsity=sp)
