@@ -97,7 +97,7 @@ int scape_step(scape_t* h, float* param, const void* const* grads, void* cuda_st
  * copies param back device->host, and synchronises cuda_stream before returning.  Pinned host
  * memory makes the copies asynchronous DMA; pageable memory works but is slower.
  * In steady state (sparse mask, flat top-k, no clip_grad, at least 2368 tiles of 1024 parameters)
- * the three phases are pipelined in 8 parts of whole tiles: the streaming kernel runs on sub-ranges
+ * the three phases are pipelined in 16 parts of whole tiles: the streaming kernel runs on sub-ranges
  * of the shard, so that theta of part i travels back while the gradients of part i + 1 travel up
  * (PCIe is full duplex), on two copy streams of the handle's own ordered by events; stage 2 follows
  * the last part.  The result is the same to the bit.

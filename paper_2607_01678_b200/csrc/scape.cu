@@ -199,7 +199,7 @@ struct scape {
   int32_t* iota_scratch = nullptr;   // scape_get(SCAPE_IDX_*) of an all-ones mask
 
   // scape_step_host staging and pipeline (upload / download streams, one event pair per part)
-  static constexpr int kHostParts = 8;
+  static constexpr int kHostParts = 16;
   cudaStream_t up = nullptr, down = nullptr;
   cudaEvent_t ev_up[kHostParts] = {}, ev_cmp[kHostParts] = {}, ev_host = nullptr;
   float* st_param = nullptr;
@@ -776,7 +776,7 @@ extern "C" scape_t* scape_create(int64_t N, int R, double sparsity, double beta1
   h->beta1_d = beta1; h->beta2_d = beta2;
   h->n_compact_blocks = (int)((h->n_chunks + kCompactChunksPerBlock - 1) / kCompactChunksPerBlock);
   h->sparsity = sparsity;
-  h->max_seg = h->n_sm * 8 * 8 * 8;          // 8 CTAs x 8 warps per SM, times the parts of scape_step_host's pipeline
+  h->max_seg = h->n_sm * 8 * 8 * scape::kHostParts;          // 8 CTAs x 8 warps per SM, times the parts of scape_step_host's pipeline
 
   bool ok = true;
   auto alloc = [&](void** p, size_t bytes, bool zero) {

@@ -347,10 +347,10 @@ def test_step_host_matches_device_step(B):
 
 @pytest.mark.parametrize("R,gdt,s", [(4, "bf16", 0.99), (2, "f32", 0.9), (8, "f32", 0.99)])
 def test_step_host_pipeline_in_parts(B, R, gdt, s):
-    """scape_step_host on a shard large enough to be pipelined in 8 parts (upload / sub-range launch of the
+    """scape_step_host on a shard large enough to be pipelined in 16 parts (upload / sub-range launch of the
     streaming kernel / download, both kernels): every step equal to scape_step on device buffers -- theta, the
     mask, the index list, b-, b^r and the residuals -- and to the oracle on the last step."""
-    n = 148 * 2 * 8 * 1024 + 3 * 1024 + 77                 # just above the pipeline's threshold, ragged tail
+    n = 148 * 2 * 16 * 1024 + 3 * 1024 + 77                # just above the pipeline's threshold, ragged tail
     w = synth.Workload("hostparts", [("a", n // 3), ("b", n - n // 3)], R=R, sparsity=s, dist="t3", rho=0.9, grad_dtype=gdt, steps=6)
     gs = synth.GradStream(w, device="cuda", seed=8)
     th_d = gs.theta0()
