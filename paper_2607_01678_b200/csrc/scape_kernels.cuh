@@ -575,7 +575,7 @@ __device__ __forceinline__ void load_mask_words(const StepParams& p, uint32_t c,
   if (PREV) { w.pw = __ldg(p.prev_bits + (c << 2) + lm.ws); w.prk = __ldg(p.prev_rk + c); }
 }
 // Which mask words the register-staged kernel fetches one trip ahead: 2 = both masks' (R = 1: 6 more live
-// registers still fit the 64 of four CTAs per SM), 1 = the previous mask's only (they feed the gather of m),
+// registers still fit the 48 of five CTAs per SM, step_ctas_per_sm), 1 = the previous mask's only (they feed the gather of m),
 // 0 = none (R >= 3: the registers are worth more to the streaming loads; measured)
 __host__ __device__ constexpr int step_prefetch(int R) { return R == 1 ? 2 : R == 2 ? 1 : 0; }
 
@@ -628,10 +628,19 @@ __host__ __device__ constexpr uint32_t step_smem_bytes(int R, bool dense) {
   return dense ? 0u : 8u * (step_scratch_bytes(R) + kRing * 8u) + 8u * 4u + (4u << kFusedBits);
 }
 
+// Resident CTAs per SM of the register-staged kernel: sparse steps with one or two replicas are latency-bound
+// (12-24 bytes per parameter in flight per lane), so they trade registers for a fourth CTA (measured, N = 2^28,
+// R = 2, 90 %: 2.54 -> 2.29 ms).  With one replica and no deferred update the body fits 48 registers without a
+// spill, i.e. a FIFTH CTA (40 of 64 warp slots): N = 2^28 kernel 1.111 -> 1.059 / 1.008 -> 0.956 / 0.908 -> 0.901 ms
+// at 90 / 99 / 99.9 %, N = 2^30 4.45 -> 4.25 / 4.04 -> 3.89 ms.  Not further: six CTAs (40 registers) spill 68 bytes
+// and lose (1.186 / 1.064 ms); R = 2 spills 44 bytes at five CTAs (1.540 -> 1.639 ms at 90 %); the deferred-update
+// (CLIPT) instantiations of R = 1 spill 24-52 bytes at five (workers mode 1.094 -> 1.125 ms); three CTAs (69 registers)
+// lose at R = 1 (1.223 / 1.107 ms) and at R = 2 (1.579 / 1.450 against 1.540 / 1.392).
+__host__ __device__ constexpr int step_ctas_per_sm(int R, bool dense, bool clipt) {
+  return dense ? (R <= 4 ? 3 : 2) : (R == 1 && !clipt) ? 5 : R <= 2 ? 4 : R <= 4 ? 3 : 2;
+}
 template <typename G, int R, bool DENSE, bool MSPARSE, bool CLIPT>
-// resident CTAs per SM: sparse steps with one or two replicas are latency-bound (12-24 bytes per parameter in
-// flight per lane), so they trade registers for a fourth CTA (measured, N = 2^28, R = 2, 90 %: 2.54 -> 2.29 ms)
-__global__ void __launch_bounds__(256, ((!DENSE && R <= 2) ? 4 : R <= 4 ? 3 : 2)) scape_fused_step_kernel(const __grid_constant__ StepParams p) {
+__global__ void __launch_bounds__(256, step_ctas_per_sm(R, DENSE, CLIPT)) scape_fused_step_kernel(const __grid_constant__ StepParams p) {
   extern __shared__ __align__(16) unsigned char step_smem[];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const uint32_t wpb = blockDim.x >> 5;
