@@ -320,7 +320,7 @@ __device__ __forceinline__ void dense_compute(const StepParams& p, uint32_t i0, 
     const float gh = __fdiv_rn(__fsub_rn(bb, pq), p.c1);                                    // l.13 (Eq. 3)
     const float vmq = __fmul_rn(p.b2, __fmul_rn(mo[q], mo[q]));
     mn[q] = bb;                                                                             // l.12
-    if (CLIPT && p.clip) {
+    if (CLIPT) {                                          // the CLIPT instantiations run with p.clip != 0 only (launch_fused)
       // l.14 needs the norm of g^ over the whole mask first: park what l.15-17 need; theta of
       // this entry is updated by clip_update_kernel
       if (!GUARD || i0 + q < p.N) {
@@ -408,7 +408,7 @@ __device__ __forceinline__ void sparse_compute(const StepParams& p, uint32_t c, 
                                                float (&th)[4], const float (&mo)[4],
                                                float (&gg)[R][4], float (&ee)[R][4], StageA& sa, const CandRing& cr) {
   uint32_t key0[4];             // bits(|m~^0|): the selection statistic of l.11
-  const bool deferred = CLIPT && p.clip;                  // theta on the mask is left to clip_update_kernel / dist_update_kernel
+  constexpr bool deferred = CLIPT;                        // (p.clip != 0 there) theta on the mask is left to clip_update_kernel / dist_update_kernel
   if (cnt == 0) {
     // no selected entry in this chunk (88 % of the chunks at 99.9 % sparsity): l.6-8 and l.17 only
 #pragma unroll
@@ -634,7 +634,7 @@ __host__ __device__ constexpr uint32_t step_smem_bytes(int R, bool dense) {
 // spill, i.e. a FIFTH CTA (40 of 64 warp slots): N = 2^28 kernel 1.111 -> 1.059 / 1.008 -> 0.956 / 0.908 -> 0.901 ms
 // at 90 / 99 / 99.9 %, N = 2^30 4.45 -> 4.25 / 4.04 -> 3.89 ms.  Not further: six CTAs (40 registers) spill 68 bytes
 // and lose (1.186 / 1.064 ms); R = 2 spills 44 bytes at five CTAs (1.540 -> 1.639 ms at 90 %); the deferred-update
-// (CLIPT) instantiations of R = 1 spill 24-52 bytes at five (workers mode 1.094 -> 1.125 ms); three CTAs (69 registers)
+// (CLIPT) instantiations of R = 1 gain nothing at five (8 bytes of spills; workers mode 1.094 -> 1.097 ms); three CTAs (69 registers)
 // lose at R = 1 (1.223 / 1.107 ms) and at R = 2 (1.579 / 1.450 against 1.540 / 1.392).
 __host__ __device__ constexpr int step_ctas_per_sm(int R, bool dense, bool clipt) {
   return dense ? (R <= 4 ? 3 : 2) : (R == 1 && !clipt) ? 5 : R <= 2 ? 4 : R <= 4 ? 3 : 2;
