@@ -677,6 +677,17 @@ def main():
                 del ga, th0
             also.append(measure_also(nm, wa, cache[nm][0].clone(), cache[nm][1], Ka, Wa, peak))
         cache.clear()
+        # BASELINE.json config 5 at the shape of the paper's deployment (one gradient per worker):
+        # N = 2^28, R = 1, i.i.d. Gaussian gradients that never repeat inside the run
+        for sp in (0.9, 0.99):
+            torch.cuda.empty_cache()
+            wa = synth.sweep_point(28, sp, 1)
+            ga = synth.GradStream(wa, device=dev, seed=args.seed)
+            th0 = ga.theta0()
+            sets = [ga.next() for _ in range(1 + Wa + Ka)]
+            del ga
+            also.append(measure_also(f"sweep:28:{sp}:1", wa, th0, sets, Ka, Wa, peak))
+            del th0, sets
     else:
         del ring, theta
     torch.cuda.empty_cache()
